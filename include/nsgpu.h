@@ -1,0 +1,196 @@
+/* nsgpu.h -- C ABI of the B200-native batched-likelihood + nested-slice-sampling library.
+ *
+ * Hot path of arXiv 2509.13307 (Lovick, Yallup, Piras, Spurio Mancini, Handley), cited as
+ * P:L<line> of /root/reference/PAPER.md, with BASELINE.json north_star (BJ) for the kernel-level
+ * definition.  Steps a1..a14 refer to SURVEY.md section 8(a) / DESIGN.md section 2.
+ *
+ * Conventions (all entry points)
+ *  - Every call returns an nsgpu_status; nothing throws or aborts across this boundary.
+ *    nsgpu_last_error(ctx) returns a ctx-owned, NUL-terminated description of the last failure.
+ *  - "HOST" / "DEVICE" beside a pointer says where the memory lives.  DEVICE pointers are owned by
+ *    the caller (e.g. torch tensors) and must be on the ctx's device; `stream` is a cudaStream_t
+ *    passed as void* (NULL = the legacy default stream).  Calls taking a stream are asynchronous on
+ *    it unless stated otherwise.
+ *  - nsgpu_create copies every HOST input (the caller may free them on return) and owns all device
+ *    workspaces until nsgpu_destroy.  Batch calls never allocate.  A ctx is not thread-safe.
+ *  - Layouts are row-major and densely packed.  theta, u: float32; log L and all evidence
+ *    quantities: float64 (reading P1: fp32 operands in the heavy stages, fp64 for the chi^2
+ *    reduction, log L and every nested-sampling accumulator).
+ *  - There is no CPU fallback anywhere: without a CUDA device nsgpu_create fails with NSGPU_ECUDA.
+ */
+#ifndef NSGPU_H
+#define NSGPU_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define NSGPU_API __attribute__((visibility("default")))
+#else
+#define NSGPU_API
+#endif
+
+typedef struct nsgpu_ctx nsgpu_ctx; /* opaque; one per (model, GPU) */
+
+typedef enum {
+  NSGPU_OK = 0,
+  NSGPU_EINVAL = -1,  /* NULL pointer, bad enum, inconsistent sizes */
+  NSGPU_ENOMEM = -2,  /* host or device allocation failed */
+  NSGPU_ECUDA = -3,   /* a CUDA runtime/driver call failed (text in nsgpu_last_error) */
+  NSGPU_ESHAPE = -4,  /* B > max_batch, n_live > max_batch, unsupported dimension */
+  NSGPU_ENOTSPD = -5, /* Cholesky factor has a non-positive or non-finite diagonal */
+  NSGPU_ENOCONV = -6  /* nsgpu_run hit max_iter before the termination criterion (result still filled) */
+} nsgpu_status;
+
+/* ---- prior (step a1; Table 1; reading N1) ------------------------------------------
+ * The sampler works in the unit hypercube u in [0,1]^D; this table is the per-dimension transform
+ *   kind 0 uniform : theta = p0 + (p1 - p0) u        (p0 = a, p1 = b)
+ *   kind 1 gaussian: theta = p0 + p1 Phi^-1(u)       (p0 = mu, p1 = sigma)                      */
+typedef struct {
+  int32_t kind;
+  double p0, p1;
+} nsgpu_prior1d;
+
+/* ---- one emulator (steps a2-a4; BJ: "dense layers with the gated activation
+ * (beta + sigma(alpha x)(1 - beta)) x, then de-standardisation of log-spectra") ----------------
+ * n_in -> n_hidden x width -> n_out.  All arrays HOST float32, copied at create.
+ * W[l]: [fan_in][fan_out] row-major (y = x.W + b), l = 0..n_hidden; b[l]: [fan_out];
+ * alpha[l], beta[l]: [width] per hidden layer (reading E1); inputs standardised (x - in_mean)/in_std;
+ * output y = (h.W + b) * out_std + out_mean; out_kind 0: spectrum = y, 1: spectrum = 10^y (E2).   */
+typedef struct {
+  int32_t n_in, n_hidden, width, n_out, out_kind;
+  const float* const* W;
+  const float* const* b;
+  const float* const* alpha;
+  const float* const* beta;
+  const float* in_mean;
+  const float* in_std;
+  const float* out_mean;
+  const float* out_std;
+} nsgpu_emulator;
+
+/* ---- theory stage after the emulator(s) (steps a5-a9) ------------------------------------------
+ * kind 0 identity     : model = theta                       (n_data = D; sampler validation, BJ cfg 0)
+ * kind 1 emulator     : model = emulator 0 spectrum         (BJ cfg 0)
+ * kind 2 cmb_binned   : s = [spectrum_0 | spectrum_1 | ...] / theta[cal_index]^2, model = Bin . s with
+ *                       Bin a CSR matrix n_data x (n_emu * n_out)            (BJ cfg 1; readings C1-C3)
+ * kind 3 shear_limber : eqs. A1-A4 on n_chi quadrature nodes evenly spaced in the scale
+ *                       factor, the emulated log10 P(k, z) interpolated linearly in z and
+ *                       log10 k, optional cubic z-spline n_z_emu -> n_z first (BJ cfg 3b)
+ * Emulator-input assembly (step a2): emulator input j < n_theta_in is theta[emu_in_idx[j]], or the
+ * constant emu_in_const[j] where emu_in_idx[j] < 0; a shear emulator has n_in = n_theta_in + 1, its
+ * last input being the redshift of the node.  Other kinds: n_in = n_theta_in.
+ * All pointers HOST, copied at create.                                                            */
+typedef struct {
+  int32_t kind;
+  int32_t n_theta_in;
+  const int32_t* emu_in_idx;  /* [n_theta_in] */
+  const double* emu_in_const; /* [n_theta_in] */
+  /* kind 2 */
+  const int32_t* bin_ptr; /* [n_data + 1] */
+  const int32_t* bin_col; /* [nnz] */
+  const float* bin_val;   /* [nnz] */
+  int32_t cal_index;
+  /* kind 3 */
+  int32_t n_z_emu, n_z, n_chi, n_k, n_ell, n_tomo;
+  int32_t z_interp; /* 0: n_z == n_z_emu, no spline; 2: cubic not-a-knot spline n_z_emu -> n_z */
+  double z_max, k_min, k_max;
+  const double* ell;     /* [n_ell] multipoles the spectra are evaluated at (reading S7) */
+  const double* nz_mean; /* [n_tomo] Gaussian n_i(z) means */
+  double nz_sigma;
+  /* where each physical parameter sits in theta (reading S2); < 0: w0 = -1, wa = 0, eta0 = 0.7 */
+  int32_t idx_omega_b, idx_omega_cdm, idx_h, idx_w0, idx_wa, idx_eta0;
+  int32_t idx_dz; /* first of n_tomo photo-z shifts */
+  int32_t idx_ia; /* first of 3 n_tomo IA coefficients, bin-major (reading S2) */
+  int32_t idx_m;  /* first of 2 n_tomo shear-calibration coefficients, bin-major (S2) */
+} nsgpu_theory;
+
+/* flags for nsgpu_create */
+#define NSGPU_MLP_AUTO 0u   /* tcgen05 tensor-core MLP where the shape allows it, SIMT otherwise */
+#define NSGPU_MLP_SIMT 1u   /* fp32 CUDA-core MLP (on-device correctness reference) */
+#define NSGPU_MLP_TC 2u     /* require the tcgen05 path (NSGPU_ESHAPE if width % 64 != 0) */
+
+/* Create a context on CUDA device `device`.
+ * data [n_data] and chol [n_data][n_data] (lower Cholesky factor of the data covariance, row-major,
+ * upper triangle ignored; reading L2) are HOST float64.  max_batch bounds B of every batch call and
+ * n_live/n_delete of the sampler calls.  Errors: EINVAL, ESHAPE, ENOTSPD, ENOMEM, ECUDA.           */
+NSGPU_API nsgpu_status nsgpu_create(nsgpu_ctx** out, int32_t D, const nsgpu_prior1d* prior, int32_t n_emu,
+                          const nsgpu_emulator* emu, const nsgpu_theory* theory, int32_t n_data,
+                          const double* data, const double* chol, int32_t max_batch, int32_t device,
+                          uint32_t flags);
+NSGPU_API nsgpu_status nsgpu_destroy(nsgpu_ctx* ctx);
+NSGPU_API const char* nsgpu_last_error(const nsgpu_ctx* ctx); /* ctx == NULL: error text of the last failed create */
+
+/* a1: theta[B][D] = T(u[B][D]); DEVICE float32 both. */
+NSGPU_API nsgpu_status nsgpu_prior_transform(nsgpu_ctx* ctx, const float* u, int32_t B, float* theta, void* stream);
+
+/* a2-a10, the bulk likelihood evaluation: logL[B] (DEVICE float64) for theta[B][D] (DEVICE
+ * float32, physical units).  theta outside the support of a uniform prior, or a non-finite model,
+ * gives -inf, never NaN.  log L includes the Gaussian normalisation -1/2 ln det(2 pi C) (reading L1). */
+NSGPU_API nsgpu_status nsgpu_loglike_batch(nsgpu_ctx* ctx, const float* theta, int32_t B, double* logL, void* stream);
+
+/* Same computation with HOST buffers: copies theta to the device, evaluates, copies logL back and
+ * returns when logL is valid (synchronous).  This is the end-to-end entry bench.py times.           */
+NSGPU_API nsgpu_status nsgpu_loglike_batch_host(nsgpu_ctx* ctx, const float* theta_host, int32_t B, double* logL_host);
+
+/* Stage taps for parity tests (DEVICE buffers).
+ * emulate: spectrum of emulator `emu` for every theta: out [B][rows][n_out] float32, rows = n_z_emu
+ *          for kind 3 and 1 otherwise; 10^y applied where out_kind = 1.
+ * theory : model vectors [B][n_data] float64 (the input of the chi^2 stage).                        */
+NSGPU_API nsgpu_status nsgpu_emulate_batch(nsgpu_ctx* ctx, int32_t emu, const float* theta, int32_t B, float* out, void* stream);
+NSGPU_API nsgpu_status nsgpu_theory_batch(nsgpu_ctx* ctx, const float* theta, int32_t B, double* model, void* stream);
+
+/* a11-a12 (+a14): evolve n_chains constrained slice-sampling chains (Neal 2003) for n_steps
+ * moves each under log L > logL_star, started from rows start_idx[c] of the live set, directions drawn
+ * from the live-set covariance (reading N3).  u_live [n_live][D] float32, logL_live [n_live] float64,
+ * start_idx [n_chains] int32, u_out [n_chains][D] float32, logL_out [n_chains] float64: all DEVICE.
+ * n_evals (HOST, optional): number of likelihood evaluations spent.  `iteration` and `seed` select the
+ * Philox streams (reading N10).  Synchronises `stream` before returning.                             */
+NSGPU_API nsgpu_status nsgpu_slice_step(nsgpu_ctx* ctx, const float* u_live, const double* logL_live, int32_t n_live,
+                              const int32_t* start_idx, int32_t n_chains, double logL_star, int32_t n_steps,
+                              uint64_t seed, int32_t iteration, float* u_out, double* logL_out,
+                              int64_t* n_evals, void* stream);
+
+typedef struct {
+  int32_t n_live, n_delete, n_steps; /* BJ cfg 4: 1000, 500, 5 D */
+  double stop_frac;                  /* stop when Z_live / (Z + Z_live) < stop_frac (reading N7) */
+  int64_t max_iter;
+  uint64_t seed;
+} nsgpu_run_opts;
+
+typedef struct {
+  double logZ, logZ_err, logZ_err_analytic, H; /* eq. 1; error bar per reading N9 */
+  int64_t n_iter, n_dead, n_like_evals, n_rounds, n_failed_moves;
+  double seconds; /* wall time of the run, host clock */
+} nsgpu_result;
+
+/* a1-a14: the whole nested-sampling run.  Samples go to caller-allocated HOST buffers of
+ * capacity `cap` rows (may be NULL with cap = 0): theta [cap][D] float32, logL [cap], logw [cap]
+ * float64 with logw = log(L_i w_i / Z); *n_samples returns n_dead + n_live (the number
+ * needed); min(cap, needed) rows are written.  Returns NSGPU_ENOCONV if max_iter was reached.       */
+NSGPU_API nsgpu_status nsgpu_run(nsgpu_ctx* ctx, const nsgpu_run_opts* opts, nsgpu_result* res, float* theta_samples,
+                       double* logL_samples, double* logw_samples, int64_t cap, int64_t* n_samples);
+
+/* a13 tap: delete the k lowest of logL_live [n_live] (DEVICE), accumulate the evidence starting from
+ * (*logX, *logZ) (HOST in/out).  dead_idx [k] int32, logw [k] float64 (DEVICE out); *logL_star HOST. */
+NSGPU_API nsgpu_status nsgpu_delete_lowest(nsgpu_ctx* ctx, const double* logL_live, int32_t n_live, int32_t k,
+                                 double* logX, double* logZ, int32_t* dead_idx, double* logw,
+                                 double* logL_star, void* stream);
+
+/* a14 tap: lower Cholesky factor [D][D] (DEVICE float64) of the sample covariance of u_live + 1e-12 I. */
+NSGPU_API nsgpu_status nsgpu_live_cholesky(nsgpu_ctx* ctx, const float* u_live, int32_t n_live, double* L_out, void* stream);
+
+/* RNG tap: out[n][4] = Philox4x32-10(ctr[n][4], key[2]) (DEVICE uint32 in/out; key HOST). */
+NSGPU_API nsgpu_status nsgpu_debug_philox(nsgpu_ctx* ctx, const uint32_t* ctr, int32_t n, const uint32_t* key, uint32_t* out, void* stream);
+
+/* Introspection: 0 = SIMT, 1 = tcgen05 for emulator `emu`; kernels launched since create. */
+NSGPU_API int32_t nsgpu_mlp_path(const nsgpu_ctx* ctx, int32_t emu);
+NSGPU_API int64_t nsgpu_launch_count(const nsgpu_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NSGPU_H */

@@ -1,0 +1,122 @@
+// internal.cuh -- context layout and launch helpers shared by the nsgpu translation units.
+// Not part of the public boundary (include/nsgpu.h is).
+#pragma once
+
+#include <cuda_runtime.h>
+#include <cuda_fp16.h>
+#include <stdint.h>
+
+#include <algorithm>
+#include <string>
+#include <vector>
+
+#include "../../include/nsgpu.h"
+
+#define NSGPU_MAX_LAYERS 8   // n_hidden + 1 <= 8
+#define NSGPU_MAX_IN 16      // emulator inputs
+#define NSGPU_MAX_TOMO 10
+#define NSGPU_MAX_D 64       // sampler dimension (one warp per chain, two dims per lane)
+
+struct EmuDev {
+  int n_in = 0, n_hidden = 0, width = 0, n_out = 0, out_kind = 0;
+  float* W[NSGPU_MAX_LAYERS] = {};      // fp32 [fan_in][fan_out]
+  float* b[NSGPU_MAX_LAYERS] = {};
+  float* alpha[NSGPU_MAX_LAYERS] = {};
+  float* beta[NSGPU_MAX_LAYERS] = {};
+  float *in_mean = nullptr, *in_std = nullptr, *out_mean = nullptr, *out_std = nullptr;
+  int path = 0;                         // 0 SIMT, 1 tcgen05
+  // tcgen05 path: weights of layers 1..n_hidden as fp16 hi/lo, [fan_out_padded][fan_in] (K-major),
+  // scaled by 2^wexp[l] (see mlp_tc.cu)
+  __half* Whi[NSGPU_MAX_LAYERS] = {};
+  __half* Wlo[NSGPU_MAX_LAYERS] = {};
+  float wscale_inv[NSGPU_MAX_LAYERS] = {};
+  int n_out_pad = 0;
+  void* tmaps = nullptr;                // host array of CUtensorMap (opaque here)
+};
+
+struct ShearDev {
+  int n_z_emu = 0, n_z = 0, n_chi = 0, n_k = 0, n_ell = 0, n_tomo = 0, n_tap = 0;
+  double z_max = 0, k_min = 0, k_max = 0, lk0 = 0, dlk = 0, da = 0, nz_sigma = 0;
+  double *a_q = nullptr, *z_q = nullptr;   // [n_chi]
+  int* tap_start = nullptr;                // [n_chi] first emulator z node used by node q
+  double* tap_w = nullptr;                 // [n_chi][n_tap] z-interpolation weights (spline folded in)
+  double *ell = nullptr, *nz_mean = nullptr;
+  int idx_omega_b = -1, idx_omega_cdm = -1, idx_h = -1, idx_w0 = -1, idx_wa = -1, idx_eta0 = -1;
+  int idx_dz = -1, idx_ia = -1, idx_m = -1;
+};
+
+struct SamplerDev;  // sampler.cu
+
+struct nsgpu_ctx {
+  int device = 0, D = 0, n_emu = 0, n_data = 0, max_batch = 0, kind = 0;
+  uint32_t flags = 0;
+  int rows_per_theta = 1;       // n_z_emu for shear, 1 otherwise
+  int n_theta_in = 0;
+  int sm_count = 148;
+  // prior
+  int* prior_kind = nullptr;
+  double *prior_p0 = nullptr, *prior_p1 = nullptr;
+  // emulator input assembly
+  int* emu_in_idx = nullptr;
+  double* emu_in_const = nullptr;
+  float* z_emu = nullptr;       // [n_z_emu] emulator redshift nodes (fp32 inputs of the net)
+  std::vector<EmuDev> emu;
+  // cmb
+  int *bin_ptr = nullptr, *bin_col = nullptr;
+  float* bin_val = nullptr;
+  int cal_index = -1, n_spec_cols = 0;
+  ShearDev sh;
+  // gaussian
+  double* data = nullptr;       // [n_data]
+  double* Linv = nullptr;       // [n_data][n_data] inverse of the Cholesky factor, lower, fp64
+  double log_norm = 0.0;
+  // workspaces
+  void* act[2] = {nullptr, nullptr};   // [M_max][width] fp32 (SIMT) or 2 x fp16 (tcgen05)
+  float* spec = nullptr;               // [n_emu][M_max][n_out] de-standardised y (log10 where exp10)
+  double* model = nullptr;             // [max_batch][n_data]
+  float* theta_stage = nullptr;        // [max_batch][D] device staging for the host entry
+  double* logL_stage = nullptr;
+  float* theta_pinned = nullptr;       // pinned host staging
+  double* logL_pinned = nullptr;
+  SamplerDev* sampler = nullptr;
+  std::string err;
+  int64_t launches = 0;
+};
+
+#define NSGPU_CUDA(call)                                                                  \
+  do {                                                                                    \
+    cudaError_t e_ = (call);                                                              \
+    if (e_ != cudaSuccess) {                                                              \
+      ctx->err = std::string(#call) + ": " + cudaGetErrorString(e_);                      \
+      return NSGPU_ECUDA;                                                                 \
+    }                                                                                     \
+  } while (0)
+
+#define NSGPU_LAUNCH_CHECK()                                                              \
+  do {                                                                                    \
+    ctx->launches++;                                                                      \
+    cudaError_t e_ = cudaGetLastError();                                                  \
+    if (e_ != cudaSuccess) {                                                              \
+      ctx->err = std::string("kernel launch: ") + cudaGetErrorString(e_) + " at " +       \
+                 __FILE__ + ":" + std::to_string(__LINE__);                               \
+      return NSGPU_ECUDA;                                                                 \
+    }                                                                                     \
+  } while (0)
+
+// stage entry points (one per translation unit); n_rows_dev != nullptr: only the first *n_rows_dev
+// rows (theta) are live, B is then the launch bound
+nsgpu_status mlp_forward_simt(nsgpu_ctx* ctx, int e, const float* theta, int B, const int* n_rows_dev,
+                              float* spec_out, bool apply_exp10, cudaStream_t st);
+nsgpu_status mlp_forward_tc(nsgpu_ctx* ctx, int e, const float* theta, int B, const int* n_rows_dev,
+                            float* spec_out, bool apply_exp10, cudaStream_t st);
+nsgpu_status mlp_tc_prepare(nsgpu_ctx* ctx, int e, const nsgpu_emulator* h);
+void mlp_tc_release(nsgpu_ctx* ctx, int e);
+nsgpu_status shear_project(nsgpu_ctx* ctx, const float* theta, int B, const int* n_rows_dev, cudaStream_t st);
+nsgpu_status cmb_bin(nsgpu_ctx* ctx, const float* theta, int B, const int* n_rows_dev, cudaStream_t st);
+nsgpu_status copy_model(nsgpu_ctx* ctx, const float* theta, int B, const int* n_rows_dev, cudaStream_t st);
+nsgpu_status chi2_loglike(nsgpu_ctx* ctx, const float* theta, int B, const int* n_rows_dev, double* logL,
+                          cudaStream_t st);
+nsgpu_status loglike_device(nsgpu_ctx* ctx, const float* theta, int B, const int* n_rows_dev, double* logL,
+                            cudaStream_t st);
+nsgpu_status sampler_create(nsgpu_ctx* ctx);
+void sampler_destroy(nsgpu_ctx* ctx);

@@ -1,0 +1,819 @@
+// sampler.cu -- nested sampling with batch deletion and constrained slice sampling (steps a11-a14).
+//
+// P:L50  "iteratively replaces the point with the lowest likelihood ... evidence accumulated as a sum of
+//         likelihood values weighted by successively smaller prior volumes"
+// P:L52  slice sampling (Neal 2003) under a hard likelihood constraint, as in Nested Slice Sampling
+// P:L62  "selecting k live points with the lowest likelihoods ... evolving them ... in parallel"
+// The paper gives prose only; the choices it leaves open are DESIGN.md readings N1-N10.
+//
+// Design (differs from the paper's vmapped lock-step while-loops, "perfect scaling is hard to
+// achieve"): every chain is a resumable state machine owned by one warp (lanes hold the dimensions,
+// so the per-chain state lives in registers while the warp runs).  One ROUND = every unfinished chain
+// advances until it has exactly one in-box proposal that needs a likelihood (out-of-box proposals
+// are rejected on the spot and cost nothing), the proposals are compacted into a dense batch, the
+// bulk likelihood runs once on that batch, and the next round consumes the results.  Chains never
+// wait for each other inside a slice move.
+#include <math.h>
+#include <string.h>
+
+#include <algorithm>
+#include <chrono>
+#include <random>
+
+#include "internal.cuh"
+
+#define MAX_STEP_OUT 32
+#define MAX_SHRINK 64
+#define BRACKET_W 2.0
+#define MAX_LIVE 16384
+
+struct SamplerDev {
+  int cap = 0;   // max chains / live points
+  // chain state (SoA)
+  float *x0 = nullptr, *dir = nullptr, *xprop = nullptr, *theta_chain = nullptr;   // [cap][D]
+  double *l = nullptr, *r = nullptr, *t = nullptr, *logL0 = nullptr;
+  int *phase = nullptr, *cnt = nullptr, *step = nullptr, *pending = nullptr, *finished = nullptr, *need = nullptr;
+  unsigned* rng_j = nullptr;
+  int *row_of_chain = nullptr, *start_idx = nullptr;
+  // batch
+  float* theta_prop = nullptr;   // [cap][D]
+  double* logL_prop = nullptr;   // [cap]
+  // scalars: [0] n_active, [1] n_finished, [2] n_fails
+  int* counters = nullptr;
+  unsigned long long* n_evals = nullptr;
+  double* scal = nullptr;        // [0] logL_star, [1] logX, [2] logZ, [3] logZ_live, [4] stop flag
+  double* Lsig = nullptr;        // [D][D] lower Cholesky of the live covariance
+  // live set and per-iteration outputs (nsgpu_run)
+  float* u_live = nullptr;       // [cap][D]
+  double* logL_live = nullptr;
+  int *dead_idx = nullptr, *surv_idx = nullptr;
+  double* logw = nullptr;
+  float* u_out = nullptr;
+  double* logL_out = nullptr;
+  // host mirrors
+  int* h_counters = nullptr;           // pinned [4]
+  unsigned long long* h_evals = nullptr;
+  double* h_scal = nullptr;            // pinned [8]
+};
+
+namespace {
+
+// ---------------- Philox4x32-10 (Salmon et al. 2011), device side ---------------------------------
+__device__ __forceinline__ uint4 philox4x32_10(uint4 c, uint2 k) {
+#pragma unroll
+  for (int r = 0; r < 10; ++r) {
+    const unsigned hi0 = __umulhi(0xD2511F53u, c.x), lo0 = 0xD2511F53u * c.x;
+    const unsigned hi1 = __umulhi(0xCD9E8D57u, c.z), lo1 = 0xCD9E8D57u * c.z;
+    c = make_uint4(hi1 ^ c.y ^ k.x, lo1, hi0 ^ c.w ^ k.y, lo0);
+    k.x += 0x9E3779B9u;
+    k.y += 0xBB67AE85u;
+  }
+  return c;
+}
+__device__ __forceinline__ double u01(unsigned x) { return ((double)x + 0.5) * (1.0 / 4294967296.0); }
+
+struct Stream {   // reading N10: block j of (seed, chain, iteration, tag) = philox(ctr=(j,chain,iteration,tag), key=seed)
+  uint2 key;
+  unsigned chain, iteration, tag;
+  __device__ uint4 block(unsigned j) const { return philox4x32_10(make_uint4(j, chain, iteration, tag), key); }
+  __device__ double uniform(unsigned j) const { return u01(block(j).x); }
+  __device__ double normal(unsigned j0, int i) const {   // i-th normal of a run starting at block j0
+    const uint4 w = block(j0 + (unsigned)(i >> 2));
+    const int e = i & 3;
+    const unsigned a = (e < 2) ? w.x : w.z, b = (e < 2) ? w.y : w.w;
+    const double rr = sqrt(-2.0 * log(u01(a))), ang = 6.283185307179586 * u01(b);
+    return (e & 1) ? rr * sin(ang) : rr * cos(ang);
+  }
+};
+
+__global__ void philox_kernel(const uint4* ctr, int n, uint2 key, uint4* out) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) out[i] = philox4x32_10(ctr[i], key);
+}
+
+__device__ __forceinline__ double transform1(int kind, double p0, double p1, double u) {
+  return kind == 0 ? p0 + (p1 - p0) * u : p0 + p1 * normcdfinv(u);
+}
+
+enum { P_NEW = 0, P_OUT_L = 1, P_OUT_R = 2, P_SHRINK = 3 };
+
+struct RoundArgs {
+  int n_chains, D, n_steps;
+  uint2 key;
+  unsigned iteration;
+  const double* scal;      // [0] = logL_star
+  const double* Lsig;
+  const int* prior_kind;
+  const double *p0, *p1;
+  float *x0, *dir, *xprop, *theta_chain;
+  double *l, *r, *t, *logL0;
+  int *phase, *cnt, *step, *pending, *finished, *need;
+  unsigned* rng_j;
+  const int* row_of_chain;
+  const double* logL_prop;
+  int* counters;
+  float* u_out;
+  double* logL_out;
+};
+
+// a11 + a12: one warp per chain; consume last round's likelihood, advance the slice state machine to the
+// next proposal that needs a likelihood.  Phase transitions are taken from the state as it was when the
+// result was requested: a chain consumes exactly one likelihood result per round.
+__global__ void __launch_bounds__(128) slice_round_kernel(RoundArgs a) {
+  const int c = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  const int lane = threadIdx.x & 31;
+  if (c >= a.n_chains) return;
+  if (a.finished[c]) { if (lane == 0) a.need[c] = 0; return; }
+  const int D = a.D;
+  const int d0 = lane, d1 = lane + 32;
+  const bool v0 = d0 < D, v1 = d1 < D;
+  const size_t base = (size_t)c * D;
+  float xa = v0 ? a.x0[base + d0] : 0.f, xb = v1 ? a.x0[base + d1] : 0.f;
+  float da = v0 ? a.dir[base + d0] : 0.f, db = v1 ? a.dir[base + d1] : 0.f;
+  float pa = v0 ? a.xprop[base + d0] : 0.f, pb = v1 ? a.xprop[base + d1] : 0.f;
+  double l = a.l[c], r = a.r[c], t = a.t[c], logL0 = a.logL0[c];
+  int phase = a.phase[c], cnt = a.cnt[c], step = a.step[c];
+  unsigned j = a.rng_j[c];
+  const double Lstar = a.scal[0];
+  Stream S{a.key, (unsigned)c, a.iteration, 0u};
+  bool inside = false;
+  double val = 0.0;
+  if (a.pending[c]) {
+    val = a.logL_prop[a.row_of_chain[c]];
+    inside = val > Lstar;                       // strict (reading N5); -inf and NaN compare false
+  }
+  int fails = 0;
+  bool emit = false, done = false;
+  while (true) {
+    double tp = 0.0;
+    bool propose = false;
+    if (phase == P_OUT_L) {
+      if (inside) { l -= BRACKET_W; ++cnt; if (cnt < MAX_STEP_OUT) { tp = l; propose = true; } }
+      if (!propose) { cnt = 0; phase = P_OUT_R; tp = r; propose = true; }
+    } else if (phase == P_OUT_R) {
+      if (inside) { r += BRACKET_W; ++cnt; if (cnt < MAX_STEP_OUT) { tp = r; propose = true; } }
+      if (!propose) { cnt = 0; phase = P_SHRINK; t = l + (r - l) * S.uniform(j++); tp = t; propose = true; }
+    } else if (phase == P_SHRINK) {
+      if (inside) {
+        xa = pa; xb = pb; logL0 = val; ++step; phase = P_NEW;
+      } else {
+        if (t < 0.0) l = t; else r = t;
+        ++cnt;
+        if (cnt < MAX_SHRINK) { t = l + (r - l) * S.uniform(j++); tp = t; propose = true; }
+        else { ++fails; ++step; phase = P_NEW; }
+      }
+    }
+    if (phase == P_NEW && !propose) {
+      if (step >= a.n_steps) { done = true; break; }
+      // direction d = L_sigma z / ||z|| (reading N3)
+      const double za = v0 ? S.normal(j, d0) : 0.0, zb = v1 ? S.normal(j, d1) : 0.0;
+      j += (unsigned)((D + 3) >> 2);
+      double nn = za * za + zb * zb;
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) nn += __shfl_xor_sync(0xffffffffu, nn, o);
+      double acca = 0.0, accb = 0.0;
+      for (int jj = 0; jj < D; ++jj) {
+        const double zj = __shfl_sync(0xffffffffu, jj < 32 ? za : zb, jj & 31);
+        if (v0 && jj <= d0) acca += a.Lsig[(size_t)d0 * D + jj] * zj;
+        if (v1 && jj <= d1) accb += a.Lsig[(size_t)d1 * D + jj] * zj;
+      }
+      const double inv = 1.0 / sqrt(nn);
+      da = (float)(acca * inv); db = (float)(accb * inv);
+      l = -BRACKET_W * S.uniform(j++);
+      r = l + BRACKET_W;
+      cnt = 0; phase = P_OUT_L; tp = l; propose = true;
+    }
+    // propose x0 + tp d; out-of-box is rejected here without a likelihood call
+    pa = (float)((double)xa + tp * (double)da);
+    pb = (float)((double)xb + tp * (double)db);
+    const bool ok = (!v0 || (pa >= 0.f && pa <= 1.f)) && (!v1 || (pb >= 0.f && pb <= 1.f));
+    if (__all_sync(0xffffffffu, ok)) { emit = true; break; }
+    inside = false;
+  }
+  if (v0) { a.x0[base + d0] = xa; a.dir[base + d0] = da; a.xprop[base + d0] = pa; }
+  if (v1) { a.x0[base + d1] = xb; a.dir[base + d1] = db; a.xprop[base + d1] = pb; }
+  if (emit) {
+    if (v0) a.theta_chain[base + d0] = (float)transform1(a.prior_kind[d0], a.p0[d0], a.p1[d0], (double)pa);
+    if (v1) a.theta_chain[base + d1] = (float)transform1(a.prior_kind[d1], a.p0[d1], a.p1[d1], (double)pb);
+  }
+  if (done) {
+    if (v0) a.u_out[base + d0] = xa;
+    if (v1) a.u_out[base + d1] = xb;
+  }
+  if (lane == 0) {
+    a.l[c] = l; a.r[c] = r; a.t[c] = t; a.logL0[c] = logL0;
+    a.phase[c] = phase; a.cnt[c] = cnt; a.step[c] = step; a.rng_j[c] = j;
+    a.pending[c] = emit ? 1 : 0;
+    a.need[c] = emit ? 1 : 0;
+    if (fails) atomicAdd(&a.counters[2], fails);
+    if (done) { a.finished[c] = 1; a.logL_out[c] = logL0; atomicAdd(&a.counters[1], 1); }
+  }
+}
+
+// block-wide exclusive scan of one int per thread (1024 threads)
+__device__ int block_excl_scan_int(int v, int* wsum, int* total) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  int inc = v;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) { int t = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += t; }
+  if (lane == 31) wsum[warp] = inc;
+  __syncthreads();
+  if (warp == 0) {
+    int w = wsum[lane], winc = w;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { int t = __shfl_up_sync(0xffffffffu, winc, o); if (lane >= o) winc += t; }
+    wsum[lane] = winc - w;
+    if (lane == 31) *total = winc;
+  }
+  __syncthreads();
+  const int out = wsum[warp] + inc - v;
+  __syncthreads();
+  return out;
+}
+
+// compaction of the proposals that need a likelihood into a dense batch (deterministic: chain order)
+__global__ void __launch_bounds__(1024) compact_kernel(int n_chains, int D, const int* __restrict__ need,
+                                                        int* __restrict__ row_of_chain,
+                                                        const float* __restrict__ theta_chain,
+                                                        float* __restrict__ theta_prop, int* counters,
+                                                        unsigned long long* n_evals) {
+  __shared__ int wsum[32];
+  __shared__ int total;
+  int carry = 0;
+  for (int base = 0; base < n_chains; base += blockDim.x) {
+    const int c = base + threadIdx.x;
+    const int f = (c < n_chains) ? need[c] : 0;
+    const int ex = block_excl_scan_int(f, wsum, &total);
+    if (c < n_chains) row_of_chain[c] = f ? carry + ex : -1;
+    carry += total;
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) { counters[0] = carry; *n_evals += (unsigned long long)carry; }
+  for (int i = threadIdx.x; i < n_chains * D; i += blockDim.x) {
+    const int c = i / D, row = row_of_chain[c];
+    if (row >= 0) theta_prop[(size_t)row * D + (i - c * D)] = theta_chain[i];
+  }
+}
+
+__global__ void chain_init_kernel(int n_chains, int D, uint2 key, unsigned iteration, const int* __restrict__ surv_idx,
+                                  int n_surv, const int* __restrict__ start_in, int* __restrict__ start_idx,
+                                  const float* __restrict__ u_live, const double* __restrict__ logL_live,
+                                  float* x0, double* logL0, int* phase, int* cnt, int* step, int* pending,
+                                  int* finished, int* need, unsigned* rng_j) {
+  const int c = blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= n_chains) return;
+  int s;
+  if (start_in) {
+    s = start_in[c];
+  } else {   // reading N4: uniform with replacement from the survivors; Stream(seed, c, iteration, tag 1)
+    Stream S{key, (unsigned)c, iteration, 1u};
+    int pick = (int)(S.uniform(0) * n_surv);
+    s = surv_idx[min(pick, n_surv - 1)];
+  }
+  start_idx[c] = s;
+  for (int d = 0; d < D; ++d) x0[(size_t)c * D + d] = u_live[(size_t)s * D + d];
+  logL0[c] = logL_live[s];
+  phase[c] = P_NEW; cnt[c] = 0; step[c] = 0; pending[c] = 0; finished[c] = 0; need[c] = 0; rng_j[c] = 0;
+}
+
+// a14: sample covariance of the live set in u-space + 1e-12 I, lower Cholesky factor; one CTA
+__global__ void __launch_bounds__(256) live_cholesky_kernel(const float* __restrict__ u, int n, int D, double* __restrict__ L) {
+  __shared__ double mean[NSGPU_MAX_D];
+  __shared__ double cov[NSGPU_MAX_D * NSGPU_MAX_D];
+  for (int d = threadIdx.x; d < D; d += blockDim.x) {
+    double s = 0.0;
+    for (int i = 0; i < n; ++i) s += (double)u[(size_t)i * D + d];
+    mean[d] = s / n;
+  }
+  __syncthreads();
+  for (int e = threadIdx.x; e < D * D; e += blockDim.x) {
+    const int r = e / D, cidx = e - r * D;
+    if (cidx > r) { cov[e] = 0.0; continue; }
+    double s = 0.0;
+    for (int i = 0; i < n; ++i) s += ((double)u[(size_t)i * D + r] - mean[r]) * ((double)u[(size_t)i * D + cidx] - mean[cidx]);
+    cov[e] = s / (n - 1) + (r == cidx ? 1e-12 : 0.0);
+  }
+  __syncthreads();
+  // column Cholesky; D <= 64, one warp-synchronous pass per column by the whole block
+  for (int k = 0; k < D; ++k) {
+    if (threadIdx.x == 0) cov[k * D + k] = sqrt(cov[k * D + k]);
+    __syncthreads();
+    for (int i = k + 1 + threadIdx.x; i < D; i += blockDim.x) cov[i * D + k] /= cov[k * D + k];
+    __syncthreads();
+    for (int e = threadIdx.x; e < D * D; e += blockDim.x) {
+      const int i = e / D, jj = e - i * D;
+      if (jj > k && jj <= i) cov[i * D + jj] -= cov[i * D + k] * cov[jj * D + k];
+    }
+    __syncthreads();
+  }
+  for (int e = threadIdx.x; e < D * D; e += blockDim.x) L[e] = cov[e];
+}
+
+// a13: delete the k lowest live points, accumulate the evidence.  One CTA of 1024 threads.
+// Total order by (logL, index) via a bitonic sort in shared memory (reading N5); volumes by a prefix
+// sum of -1/n_j and the weights folded into log Z by a block log-sum-exp (reading N6).
+__global__ void __launch_bounds__(1024) delete_lowest_kernel(const double* __restrict__ logL, int n, int k,
+                                                              double* __restrict__ scal, int* __restrict__ dead_idx,
+                                                              int* __restrict__ surv_idx, double* __restrict__ logw) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  int np2 = 1;
+  while (np2 < n) np2 <<= 1;
+  double* key = reinterpret_cast<double*>(smem_raw);   // [np2]
+  int* idx = reinterpret_cast<int*>(key + np2);        // [np2]
+  __shared__ double red[32];
+  __shared__ double wsum[33];
+  __shared__ int isum[32];
+  __shared__ int itot;
+  for (int i = threadIdx.x; i < np2; i += blockDim.x) {
+    key[i] = i < n ? logL[i] : INFINITY;
+    idx[i] = i < n ? i : 0x7fffffff;
+  }
+  __syncthreads();
+  for (int size = 2; size <= np2; size <<= 1)
+    for (int stride = size >> 1; stride > 0; stride >>= 1) {
+      for (int i = threadIdx.x; i < np2; i += blockDim.x) {
+        const int p = i ^ stride;
+        if (p > i) {
+          const bool up = (i & size) == 0;
+          const double a = key[i], b = key[p];
+          const int ia = idx[i], ib = idx[p];
+          const bool gt = (a > b) || (a == b && ia > ib) || (a != a && b == b);
+          if (gt == up) { key[i] = b; key[p] = a; idx[i] = ib; idx[p] = ia; }
+        }
+      }
+      __syncthreads();
+    }
+  const double logX0 = scal[1], logZ0 = scal[2];
+  // prefix sum of 1/n_j (exclusive) -> log X_{j-1}; terms l_j + log w_j
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  double carry = 0.0, mx = -INFINITY;
+  for (int base = 0; base < k; base += blockDim.x) {
+    const int jj = base + threadIdx.x;
+    const double nj = (double)(n - jj);
+    const double v = jj < k ? 1.0 / nj : 0.0;
+    double inc = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { double tt = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += tt; }
+    if (lane == 31) wsum[warp] = inc;
+    __syncthreads();
+    if (warp == 0) {
+      double w = wsum[lane], winc = w;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) { double tt = __shfl_up_sync(0xffffffffu, winc, o); if (lane >= o) winc += tt; }
+      wsum[lane] = winc - w;
+      if (lane == 31) wsum[32] = winc;
+    }
+    __syncthreads();
+    if (jj < k) {
+      const double logX_prev = logX0 - (carry + wsum[warp] + inc - v);
+      const double lw = logX_prev + log(-expm1(-1.0 / nj));
+      logw[jj] = lw;
+      dead_idx[jj] = idx[jj];
+      mx = fmax(mx, key[jj] + lw);
+    }
+    carry += wsum[32];
+    __syncthreads();
+  }
+  // block log-sum-exp of the k terms together with the running log Z
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+  if (lane == 0) red[warp] = mx;
+  __syncthreads();
+  if (warp == 0) {
+    double m = red[lane];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
+    if (lane == 0) red[0] = fmax(m, logZ0);
+  }
+  __syncthreads();
+  const double M = red[0];
+  __syncthreads();
+  double se = 0.0;
+  for (int jj = threadIdx.x; jj < k; jj += blockDim.x) se += exp(key[jj] + logw[jj] - M);
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) se += __shfl_xor_sync(0xffffffffu, se, o);
+  if (lane == 0) red[warp] = se;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double tot = 0.0;
+    for (int w = 0; w < 32; ++w) tot += red[w];
+    if (logZ0 > -INFINITY) tot += exp(logZ0 - M);
+    scal[2] = (M > -INFINITY) ? M + log(tot) : -INFINITY;
+    scal[1] = logX0 - carry;
+    scal[0] = key[k - 1];                                   // L* = largest deleted
+  }
+  __syncthreads();
+  // survivors in index order: mark the dead, scan the flags
+  int* deadflag = idx;                                        // reuse after copying the dead indices out
+  __syncthreads();
+  for (int i = threadIdx.x; i < np2; i += blockDim.x) deadflag[i] = 0;
+  __syncthreads();
+  for (int jj = threadIdx.x; jj < k; jj += blockDim.x) deadflag[dead_idx[jj]] = 1;
+  __syncthreads();
+  int icarry = 0;
+  for (int base = 0; base < n; base += blockDim.x) {
+    const int i = base + threadIdx.x;
+    const int f = (i < n && !deadflag[i]) ? 1 : 0;
+    const int ex = block_excl_scan_int(f, isum, &itot);
+    if (f) surv_idx[icarry + ex] = i;
+    icarry += itot;
+    __syncthreads();
+  }
+}
+
+__global__ void replace_kernel(int k, int D, const int* __restrict__ dead_idx, const float* __restrict__ u_out,
+                               const double* __restrict__ logL_out, float* u_live, double* logL_live) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= k * D) return;
+  const int c = i / D, d = i - c * D;
+  u_live[(size_t)dead_idx[c] * D + d] = u_out[i];
+  if (d == 0) logL_live[dead_idx[c]] = logL_out[c];
+}
+
+__global__ void gather_rows_kernel(int k, int D, const int* __restrict__ rows, const float* __restrict__ src_u,
+                                   const double* __restrict__ src_l, float* dst_u, double* dst_l) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= k * D) return;
+  const int c = i / D, d = i - c * D;
+  dst_u[i] = src_u[(size_t)rows[c] * D + d];
+  if (d == 0) dst_l[c] = src_l[rows[c]];
+}
+
+// termination test (reading N7): logZ_live = logsumexp(l_live) - ln n + logX
+__global__ void __launch_bounds__(1024) live_evidence_kernel(const double* __restrict__ logL, int n, double log_stop,
+                                                              double* scal) {
+  __shared__ double red[32];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  double mx = -INFINITY;
+  for (int i = threadIdx.x; i < n; i += blockDim.x) mx = fmax(mx, logL[i]);
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+  if (lane == 0) red[warp] = mx;
+  __syncthreads();
+  if (warp == 0) {
+    double m = red[lane];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
+    if (lane == 0) red[0] = m;
+  }
+  __syncthreads();
+  const double M = red[0];
+  __syncthreads();
+  double se = 0.0;
+  for (int i = threadIdx.x; i < n; i += blockDim.x) se += exp(logL[i] - M);
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) se += __shfl_xor_sync(0xffffffffu, se, o);
+  if (lane == 0) red[warp] = se;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double tot = 0.0;
+    for (int w = 0; w < 32; ++w) tot += red[w];
+    const double lzl = M + log(tot) - log((double)n) + scal[1];
+    const double lz = scal[2];
+    const double hi = fmax(lz, lzl), lo = fmin(lz, lzl);
+    const double both = hi + log1p(exp(lo - hi));
+    scal[3] = lzl;
+    scal[4] = (lzl - both < log_stop) ? 1.0 : 0.0;
+  }
+}
+
+__global__ void init_live_kernel(int n, int D, uint2 key, float* u) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n * D) return;
+  const int p = i / D, d = i - p * D;
+  Stream S{key, (unsigned)p, 0u, 2u};     // point p: D uniforms from blocks 0..D-1, word 0
+  u[i] = (float)S.uniform((unsigned)d);
+}
+
+}  // namespace
+
+// ---------------------------------------------------------------------------------------------------
+nsgpu_status sampler_create(nsgpu_ctx* ctx) {
+  SamplerDev* S = new SamplerDev();
+  ctx->sampler = S;
+  const size_t cap = ctx->max_batch, D = ctx->D;
+  S->cap = (int)cap;
+#define A(p, T, n) NSGPU_CUDA(cudaMalloc((void**)&S->p, sizeof(T) * (n)))
+  A(x0, float, cap * D); A(dir, float, cap * D); A(xprop, float, cap * D); A(theta_chain, float, cap * D);
+  A(l, double, cap); A(r, double, cap); A(t, double, cap); A(logL0, double, cap);
+  A(phase, int, cap); A(cnt, int, cap); A(step, int, cap); A(pending, int, cap); A(finished, int, cap); A(need, int, cap);
+  A(rng_j, unsigned, cap); A(row_of_chain, int, cap); A(start_idx, int, cap);
+  A(theta_prop, float, cap * D); A(logL_prop, double, cap);
+  A(counters, int, 4); A(n_evals, unsigned long long, 1); A(scal, double, 8); A(Lsig, double, D * D);
+  A(u_live, float, cap * D); A(logL_live, double, cap); A(dead_idx, int, cap); A(surv_idx, int, cap);
+  A(logw, double, cap); A(u_out, float, cap * D); A(logL_out, double, cap);
+#undef A
+  NSGPU_CUDA(cudaMallocHost((void**)&S->h_counters, 4 * sizeof(int)));
+  NSGPU_CUDA(cudaMallocHost((void**)&S->h_evals, sizeof(unsigned long long)));
+  NSGPU_CUDA(cudaMallocHost((void**)&S->h_scal, 8 * sizeof(double)));
+  NSGPU_CUDA(cudaMemset(S->xprop, 0, sizeof(float) * cap * D));
+  NSGPU_CUDA(cudaMemset(S->dir, 0, sizeof(float) * cap * D));
+  return NSGPU_OK;
+}
+
+void sampler_destroy(nsgpu_ctx* ctx) {
+  SamplerDev* S = ctx->sampler;
+  if (!S) return;
+  void* ptrs[] = {S->x0, S->dir, S->xprop, S->theta_chain, S->l, S->r, S->t, S->logL0, S->phase, S->cnt, S->step,
+                  S->pending, S->finished, S->need, S->rng_j, S->row_of_chain, S->start_idx, S->theta_prop,
+                  S->logL_prop, S->counters, S->n_evals, S->scal, S->Lsig, S->u_live, S->logL_live, S->dead_idx,
+                  S->surv_idx, S->logw, S->u_out, S->logL_out};
+  for (void* p : ptrs) cudaFree(p);
+  cudaFreeHost(S->h_counters); cudaFreeHost(S->h_evals); cudaFreeHost(S->h_scal);
+  delete S;
+  ctx->sampler = nullptr;
+}
+
+static nsgpu_status launch_live_cholesky(nsgpu_ctx* ctx, const float* u_live, int n_live, double* L, cudaStream_t st) {
+  live_cholesky_kernel<<<1, 256, 0, st>>>(u_live, n_live, ctx->D, L);
+  NSGPU_LAUNCH_CHECK();
+  return NSGPU_OK;
+}
+
+static nsgpu_status launch_delete(nsgpu_ctx* ctx, const double* logL, int n, int k, cudaStream_t st) {
+  SamplerDev* S = ctx->sampler;
+  int np2 = 1;
+  while (np2 < n) np2 <<= 1;
+  const size_t smem = (size_t)np2 * (sizeof(double) + sizeof(int));
+  static size_t configured = 0;
+  if (smem > configured) {
+    NSGPU_CUDA(cudaFuncSetAttribute(delete_lowest_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    configured = smem;
+  }
+  delete_lowest_kernel<<<1, 1024, smem, st>>>(logL, n, k, S->scal, S->dead_idx, S->surv_idx, S->logw);
+  NSGPU_LAUNCH_CHECK();
+  return NSGPU_OK;
+}
+
+// Evolve n_chains chains to completion.  Chains were initialised by chain_init_kernel; Lsig and scal[0]
+// (L*) are set.  Host reads the finished-counter after batches of rounds (one small D2H per batch).
+static nsgpu_status evolve(nsgpu_ctx* ctx, int n_chains, int n_steps, uint64_t seed, int iteration, cudaStream_t st,
+                           int64_t* rounds_out) {
+  SamplerDev* S = ctx->sampler;
+  RoundArgs a;
+  a.n_chains = n_chains; a.D = ctx->D; a.n_steps = n_steps;
+  a.key = make_uint2((unsigned)(seed & 0xffffffffu), (unsigned)(seed >> 32));
+  a.iteration = (unsigned)iteration;
+  a.scal = S->scal; a.Lsig = S->Lsig; a.prior_kind = ctx->prior_kind; a.p0 = ctx->prior_p0; a.p1 = ctx->prior_p1;
+  a.x0 = S->x0; a.dir = S->dir; a.xprop = S->xprop; a.theta_chain = S->theta_chain;
+  a.l = S->l; a.r = S->r; a.t = S->t; a.logL0 = S->logL0;
+  a.phase = S->phase; a.cnt = S->cnt; a.step = S->step; a.pending = S->pending; a.finished = S->finished; a.need = S->need;
+  a.rng_j = S->rng_j; a.row_of_chain = S->row_of_chain; a.logL_prop = S->logL_prop; a.counters = S->counters;
+  a.u_out = S->u_out; a.logL_out = S->logL_out;
+  NSGPU_CUDA(cudaMemsetAsync(S->counters, 0, 4 * sizeof(int), st));
+  const int blocks = (n_chains * 32 + 127) / 128;
+  int64_t rounds = 0;
+  // a slice move costs ~5 proposals (SURVEY c.2): run most of the expected rounds before the first check
+  int burst = std::max(8, n_steps * 4);
+  while (true) {
+    for (int i = 0; i < burst; ++i) {
+      slice_round_kernel<<<blocks, 128, 0, st>>>(a);
+      NSGPU_LAUNCH_CHECK();
+      compact_kernel<<<1, 1024, 0, st>>>(n_chains, ctx->D, S->need, S->row_of_chain, S->theta_chain, S->theta_prop,
+                                         S->counters, S->n_evals);
+      NSGPU_LAUNCH_CHECK();
+      nsgpu_status s = loglike_device(ctx, S->theta_prop, n_chains, S->counters, S->logL_prop, st);
+      if (s != NSGPU_OK) return s;
+      ++rounds;
+    }
+    NSGPU_CUDA(cudaMemcpyAsync(S->h_counters, S->counters, 4 * sizeof(int), cudaMemcpyDeviceToHost, st));
+    NSGPU_CUDA(cudaStreamSynchronize(st));
+    if (S->h_counters[1] >= n_chains) break;
+    burst = std::max(4, n_steps / 4);
+    if (rounds > (int64_t)n_steps * (MAX_STEP_OUT * 2 + MAX_SHRINK + 4) + 16) {
+      ctx->err = "slice sampling: chains did not finish (internal error)";
+      return NSGPU_ECUDA;
+    }
+  }
+  if (rounds_out) *rounds_out += rounds;
+  return NSGPU_OK;
+}
+
+static nsgpu_status check_sampler_args(nsgpu_ctx* ctx, int n_live, int n_chains) {
+  if (!ctx) return NSGPU_EINVAL;
+  if (n_live < 2 || n_chains < 1) { ctx->err = "sampler: n_live >= 2 and n_chains >= 1 required"; return NSGPU_EINVAL; }
+  if (n_live > ctx->max_batch || n_chains > ctx->max_batch || n_live > MAX_LIVE) {
+    ctx->err = "sampler: n_live / n_chains exceed max_batch (or 16384)";
+    return NSGPU_ESHAPE;
+  }
+  cudaError_t e = cudaSetDevice(ctx->device);
+  if (e != cudaSuccess) { ctx->err = cudaGetErrorString(e); return NSGPU_ECUDA; }
+  return NSGPU_OK;
+}
+
+extern "C" nsgpu_status nsgpu_slice_step(nsgpu_ctx* ctx, const float* u_live, const double* logL_live, int32_t n_live,
+                                         const int32_t* start_idx, int32_t n_chains, double logL_star, int32_t n_steps,
+                                         uint64_t seed, int32_t iteration, float* u_out, double* logL_out,
+                                         int64_t* n_evals, void* stream) {
+  nsgpu_status s = check_sampler_args(ctx, n_live, n_chains);
+  if (s != NSGPU_OK) return s;
+  if (!u_live || !logL_live || !start_idx || !u_out || !logL_out || n_steps < 0) { ctx->err = "slice_step: bad arguments"; return NSGPU_EINVAL; }
+  SamplerDev* S = ctx->sampler;
+  cudaStream_t st = (cudaStream_t)stream;
+  const int D = ctx->D;
+  s = launch_live_cholesky(ctx, u_live, n_live, S->Lsig, st);
+  if (s != NSGPU_OK) return s;
+  S->h_scal[0] = logL_star;
+  NSGPU_CUDA(cudaMemcpyAsync(S->scal, S->h_scal, sizeof(double), cudaMemcpyHostToDevice, st));
+  NSGPU_CUDA(cudaMemsetAsync(S->n_evals, 0, sizeof(unsigned long long), st));
+  const uint2 key = make_uint2((unsigned)(seed & 0xffffffffu), (unsigned)(seed >> 32));
+  chain_init_kernel<<<(n_chains + 127) / 128, 128, 0, st>>>(n_chains, D, key, (unsigned)iteration, nullptr, 0, start_idx,
+                                                            S->start_idx, u_live, logL_live, S->x0, S->logL0, S->phase,
+                                                            S->cnt, S->step, S->pending, S->finished, S->need, S->rng_j);
+  NSGPU_LAUNCH_CHECK();
+  s = evolve(ctx, n_chains, n_steps, seed, iteration, st, nullptr);
+  if (s != NSGPU_OK) return s;
+  NSGPU_CUDA(cudaMemcpyAsync(u_out, S->u_out, sizeof(float) * (size_t)n_chains * D, cudaMemcpyDeviceToDevice, st));
+  NSGPU_CUDA(cudaMemcpyAsync(logL_out, S->logL_out, sizeof(double) * (size_t)n_chains, cudaMemcpyDeviceToDevice, st));
+  NSGPU_CUDA(cudaMemcpyAsync(S->h_evals, S->n_evals, sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
+  NSGPU_CUDA(cudaStreamSynchronize(st));
+  if (n_evals) *n_evals = (int64_t)*S->h_evals;
+  return NSGPU_OK;
+}
+
+extern "C" nsgpu_status nsgpu_delete_lowest(nsgpu_ctx* ctx, const double* logL_live, int32_t n_live, int32_t k,
+                                            double* logX, double* logZ, int32_t* dead_idx, double* logw,
+                                            double* logL_star, void* stream) {
+  nsgpu_status s = check_sampler_args(ctx, n_live, k);
+  if (s != NSGPU_OK) return s;
+  if (!logL_live || !logX || !logZ || !dead_idx || !logw || !logL_star || k >= n_live) { ctx->err = "delete_lowest: bad arguments"; return NSGPU_EINVAL; }
+  SamplerDev* S = ctx->sampler;
+  cudaStream_t st = (cudaStream_t)stream;
+  S->h_scal[0] = 0.0; S->h_scal[1] = *logX; S->h_scal[2] = *logZ;
+  NSGPU_CUDA(cudaMemcpyAsync(S->scal, S->h_scal, 3 * sizeof(double), cudaMemcpyHostToDevice, st));
+  s = launch_delete(ctx, logL_live, n_live, k, st);
+  if (s != NSGPU_OK) return s;
+  NSGPU_CUDA(cudaMemcpyAsync(dead_idx, S->dead_idx, sizeof(int) * (size_t)k, cudaMemcpyDeviceToDevice, st));
+  NSGPU_CUDA(cudaMemcpyAsync(logw, S->logw, sizeof(double) * (size_t)k, cudaMemcpyDeviceToDevice, st));
+  NSGPU_CUDA(cudaMemcpyAsync(S->h_scal, S->scal, 3 * sizeof(double), cudaMemcpyDeviceToHost, st));
+  NSGPU_CUDA(cudaStreamSynchronize(st));
+  *logL_star = S->h_scal[0]; *logX = S->h_scal[1]; *logZ = S->h_scal[2];
+  return NSGPU_OK;
+}
+
+extern "C" nsgpu_status nsgpu_live_cholesky(nsgpu_ctx* ctx, const float* u_live, int32_t n_live, double* L_out, void* stream) {
+  nsgpu_status s = check_sampler_args(ctx, n_live, 1);
+  if (s != NSGPU_OK) return s;
+  if (!u_live || !L_out) { ctx->err = "live_cholesky: NULL pointer"; return NSGPU_EINVAL; }
+  return launch_live_cholesky(ctx, u_live, n_live, L_out, (cudaStream_t)stream);
+}
+
+extern "C" nsgpu_status nsgpu_debug_philox(nsgpu_ctx* ctx, const uint32_t* ctr, int32_t n, const uint32_t* key,
+                                           uint32_t* out, void* stream) {
+  if (!ctx) return NSGPU_EINVAL;
+  if (n < 0 || (n > 0 && (!ctr || !key || !out))) { ctx->err = "debug_philox: bad arguments"; return NSGPU_EINVAL; }
+  if (n == 0) return NSGPU_OK;
+  NSGPU_CUDA(cudaSetDevice(ctx->device));
+  philox_kernel<<<(n + 255) / 256, 256, 0, (cudaStream_t)stream>>>((const uint4*)ctr, n, make_uint2(key[0], key[1]), (uint4*)out);
+  NSGPU_LAUNCH_CHECK();
+  return NSGPU_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// nsgpu_run: the outer loop.  Host code only schedules kernels and reads one flag per
+// iteration; all arithmetic on the live set happens in the kernels above.  The final summary (total
+// log Z with the live points, H, error bar by simulated volumes -- reading N9) is fp64 host arithmetic
+// over the recorded (logL, n_j) sequence.
+// ---------------------------------------------------------------------------------------------------
+extern "C" nsgpu_status nsgpu_run(nsgpu_ctx* ctx, const nsgpu_run_opts* o, nsgpu_result* res, float* theta_samples,
+                                  double* logL_samples, double* logw_samples, int64_t cap, int64_t* n_samples) {
+  if (!ctx) return NSGPU_EINVAL;
+  if (!o || !res) { ctx->err = "run: NULL options or result"; return NSGPU_EINVAL; }
+  nsgpu_status s = check_sampler_args(ctx, o->n_live, o->n_delete);
+  if (s != NSGPU_OK) return s;
+  if (o->n_delete >= o->n_live || o->n_steps < 1 || !(o->stop_frac > 0) || o->max_iter < 1) { ctx->err = "run: bad options"; return NSGPU_EINVAL; }
+  const auto t_start = std::chrono::steady_clock::now();
+  SamplerDev* S = ctx->sampler;
+  cudaStream_t st = 0;
+  const int D = ctx->D, n = o->n_live, k = o->n_delete;
+  const uint2 key = make_uint2((unsigned)(o->seed & 0xffffffffu), (unsigned)(o->seed >> 32));
+  std::vector<float> dead_u;
+  std::vector<double> dead_logL, dead_logw;
+  std::vector<int> dead_nj;
+  std::vector<float> hu((size_t)k * D);
+  std::vector<double> hl(k), hw(k);
+  float* d_dead_u = S->x0;           // scratch before chains are initialised
+  double* d_dead_l = S->logL0;
+  memset(res, 0, sizeof(*res));
+
+  init_live_kernel<<<(n * D + 255) / 256, 256, 0, st>>>(n, D, key, S->u_live);
+  NSGPU_LAUNCH_CHECK();
+  s = nsgpu_prior_transform(ctx, S->u_live, n, S->theta_prop, st);
+  if (s != NSGPU_OK) return s;
+  s = loglike_device(ctx, S->theta_prop, n, nullptr, S->logL_live, st);
+  if (s != NSGPU_OK) return s;
+  S->h_scal[0] = 0.0; S->h_scal[1] = 0.0; S->h_scal[2] = -INFINITY; S->h_scal[3] = 0.0; S->h_scal[4] = 0.0;
+  NSGPU_CUDA(cudaMemcpyAsync(S->scal, S->h_scal, 5 * sizeof(double), cudaMemcpyHostToDevice, st));
+  NSGPU_CUDA(cudaMemsetAsync(S->n_evals, 0, sizeof(unsigned long long), st));
+  int64_t it = 0, rounds = 0;
+  int n_fail_total = 0;
+  bool converged = false;
+  while (it < o->max_iter) {
+    ++it;
+    s = launch_live_cholesky(ctx, S->u_live, n, S->Lsig, st);              // before deletion
+    if (s != NSGPU_OK) return s;
+    s = launch_delete(ctx, S->logL_live, n, k, st);
+    if (s != NSGPU_OK) return s;
+    // record the dead points
+    gather_rows_kernel<<<(k * D + 255) / 256, 256, 0, st>>>(k, D, S->dead_idx, S->u_live, S->logL_live, d_dead_u, d_dead_l);
+    NSGPU_LAUNCH_CHECK();
+    NSGPU_CUDA(cudaMemcpyAsync(hu.data(), d_dead_u, sizeof(float) * (size_t)k * D, cudaMemcpyDeviceToHost, st));
+    NSGPU_CUDA(cudaMemcpyAsync(hl.data(), d_dead_l, sizeof(double) * (size_t)k, cudaMemcpyDeviceToHost, st));
+    NSGPU_CUDA(cudaMemcpyAsync(hw.data(), S->logw, sizeof(double) * (size_t)k, cudaMemcpyDeviceToHost, st));
+    NSGPU_CUDA(cudaStreamSynchronize(st));
+    dead_u.insert(dead_u.end(), hu.begin(), hu.end());
+    dead_logL.insert(dead_logL.end(), hl.begin(), hl.end());
+    dead_logw.insert(dead_logw.end(), hw.begin(), hw.end());
+    for (int j = 0; j < k; ++j) dead_nj.push_back(n - j);
+    chain_init_kernel<<<(k + 127) / 128, 128, 0, st>>>(k, D, key, (unsigned)it, S->surv_idx, n - k, nullptr, S->start_idx,
+                                                       S->u_live, S->logL_live, S->x0, S->logL0, S->phase, S->cnt, S->step,
+                                                       S->pending, S->finished, S->need, S->rng_j);
+    NSGPU_LAUNCH_CHECK();
+    s = evolve(ctx, k, o->n_steps, o->seed, (int)it, st, &rounds);
+    if (s != NSGPU_OK) return s;
+    n_fail_total += S->h_counters[2];
+    replace_kernel<<<(k * D + 255) / 256, 256, 0, st>>>(k, D, S->dead_idx, S->u_out, S->logL_out, S->u_live, S->logL_live);
+    NSGPU_LAUNCH_CHECK();
+    live_evidence_kernel<<<1, 1024, 0, st>>>(S->logL_live, n, log(o->stop_frac), S->scal);
+    NSGPU_LAUNCH_CHECK();
+    NSGPU_CUDA(cudaMemcpyAsync(S->h_scal, S->scal, 5 * sizeof(double), cudaMemcpyDeviceToHost, st));
+    NSGPU_CUDA(cudaStreamSynchronize(st));
+    if (S->h_scal[4] != 0.0) { converged = true; break; }
+  }
+  // final summary
+  const double logX = S->h_scal[1];
+  std::vector<float> live_u((size_t)n * D);
+  std::vector<double> live_l(n);
+  NSGPU_CUDA(cudaMemcpy(live_u.data(), S->u_live, sizeof(float) * (size_t)n * D, cudaMemcpyDeviceToHost));
+  NSGPU_CUDA(cudaMemcpy(live_l.data(), S->logL_live, sizeof(double) * (size_t)n, cudaMemcpyDeviceToHost));
+  NSGPU_CUDA(cudaMemcpy(S->h_evals, S->n_evals, sizeof(unsigned long long), cudaMemcpyDeviceToHost));
+  const size_t nd = dead_logL.size(), ntot = nd + n;
+  std::vector<double> all_l(ntot), all_w(ntot);
+  for (size_t i = 0; i < nd; ++i) { all_l[i] = dead_logL[i]; all_w[i] = dead_logw[i]; }
+  for (int i = 0; i < n; ++i) { all_l[nd + i] = live_l[i]; all_w[nd + i] = logX - log((double)n); }   // reading N8
+  auto logsumexp = [](const std::vector<double>& v) -> double {
+    double mx = -INFINITY;
+    for (double x : v) mx = std::max(mx, x);
+    if (!(mx > -INFINITY)) return (double)-INFINITY;
+    double sacc = 0.0;
+    for (double x : v) sacc += exp(x - mx);
+    return mx + log(sacc);
+  };
+  std::vector<double> terms(ntot);
+  for (size_t i = 0; i < ntot; ++i) terms[i] = all_l[i] + all_w[i];
+  const double logZ = logsumexp(terms);
+  double H = 0.0;
+  for (size_t i = 0; i < ntot; ++i) {
+    const double p = exp(terms[i] - logZ);
+    if (p > 0.0) H += p * (all_l[i] - logZ);
+  }
+  // error bar: redraw the volume sequence M = 1000 times with t_j = U^{1/n_j} (Skilling 2006)
+  double err_sim = 0.0;
+  {
+    std::mt19937_64 gen(o->seed * 0x9E3779B97F4A7C15ull + 99);
+    std::uniform_real_distribution<double> U(0.0, 1.0);
+    const int M = 1000;
+    std::vector<double> zs(M), tt(ntot);
+    for (int m = 0; m < M; ++m) {
+      double lx = 0.0;
+      for (size_t i = 0; i < nd; ++i) {
+        double uu = U(gen);
+        if (uu <= 0.0) uu = 1e-300;
+        const double logt = log(uu) / dead_nj[i];
+        tt[i] = dead_logL[i] + lx + log(-expm1(logt));
+        lx += logt;
+      }
+      for (int i = 0; i < n; ++i) tt[nd + i] = live_l[i] + lx - log((double)n);
+      zs[m] = logsumexp(tt);
+    }
+    double mean = 0.0;
+    for (double z : zs) mean += z;
+    mean /= M;
+    for (double z : zs) err_sim += (z - mean) * (z - mean);
+    err_sim = sqrt(err_sim / (M - 1));
+  }
+  double s1 = 0.0, s2 = 0.0;
+  for (int j = 0; j < k; ++j) { s1 += 1.0 / (n - j); s2 += 1.0 / ((double)(n - j) * (n - j)); }
+  const double cfac = n * s2 / s1;
+  res->logZ = logZ; res->logZ_err = err_sim; res->logZ_err_analytic = sqrt(std::max(cfac * H, 0.0) / n); res->H = H;
+  res->n_iter = it; res->n_dead = (int64_t)nd; res->n_like_evals = (int64_t)*S->h_evals + n; res->n_rounds = rounds;
+  res->n_failed_moves = n_fail_total;
+  if (n_samples) *n_samples = (int64_t)ntot;
+  if (cap > 0 && theta_samples && logL_samples && logw_samples) {
+    const size_t nw = std::min<size_t>((size_t)cap, ntot);
+    // theta = T(u) through the a1 kernel, in chunks of max_batch rows
+    std::vector<float> all_u(ntot * D);
+    memcpy(all_u.data(), dead_u.data(), sizeof(float) * nd * D);
+    memcpy(all_u.data() + nd * D, live_u.data(), sizeof(float) * (size_t)n * D);
+    for (size_t off = 0; off < nw; off += (size_t)ctx->max_batch) {
+      const int nb = (int)std::min<size_t>((size_t)ctx->max_batch, nw - off);
+      NSGPU_CUDA(cudaMemcpy(S->xprop, all_u.data() + off * D, sizeof(float) * (size_t)nb * D, cudaMemcpyHostToDevice));
+      s = nsgpu_prior_transform(ctx, S->xprop, nb, S->theta_prop, st);
+      if (s != NSGPU_OK) return s;
+      NSGPU_CUDA(cudaMemcpy(theta_samples + off * D, S->theta_prop, sizeof(float) * (size_t)nb * D, cudaMemcpyDeviceToHost));
+    }
+    for (size_t i = 0; i < nw; ++i) { logL_samples[i] = all_l[i]; logw_samples[i] = terms[i] - logZ; }
+  }
+  res->seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t_start).count();
+  return converged ? NSGPU_OK : NSGPU_ENOCONV;
+}

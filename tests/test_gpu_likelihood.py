@@ -1,0 +1,148 @@
+"""-m gpu: parity of the CUDA likelihood path (through the C ABI) against the fp64 oracle, element by
+element on seeded inputs.  Tolerances: BASELINE.json north_star -- emulator outputs <= 1e-4 relative
+(reading E5), |dlogL| <= 1e-3 absolute where chi2 <= 2000, 1e-6 chi2 beyond (reading T2)."""
+import numpy as np
+import pytest
+
+from oracle import gaussian, likelihood as LK, philox, prior
+from paper_2509_13307_b200 import nsgpu, workloads as W
+from tests.util import loglike_tolerance, theta_of_u, workload
+
+pytestmark = pytest.mark.gpu
+torch = pytest.importorskip("torch")
+
+
+def dev(a, dtype=None):
+    t = torch.as_tensor(np.ascontiguousarray(a), device="cuda")
+    return t if dtype is None else t.to(dtype)
+
+
+def emulator_rel_err(got, ref, out_kind):
+    if out_kind == 1:
+        return np.max(np.abs(got - ref) / np.abs(ref))
+    return np.max(np.abs(got - ref) / (np.abs(ref) + np.sqrt(np.mean(ref ** 2))))
+
+
+def test_philox_bit_exact():
+    wl = workload("identity")
+    with nsgpu.Context(wl, max_batch=8) as ctx:
+        rng = np.random.default_rng(0)
+        ctr = rng.integers(0, 2 ** 32, size=(1000, 4), dtype=np.uint64).astype(np.uint32)
+        ctr[0] = 0; ctr[1] = 0xFFFFFFFF
+        key = np.array([0xa4093822, 0x299f31d0], np.uint32)
+        got = ctx.debug_philox(dev(ctr.view(np.int32)), key).cpu().numpy().view(np.uint32)
+        np.testing.assert_array_equal(got, philox.philox4x32_10(ctr, key))
+        kat = ctx.debug_philox(dev(np.array([[0x243f6a88, 0x85a308d3, 0x13198a2e, 0x03707344]], np.uint32).view(np.int32)), key)
+        assert [hex(x) for x in kat.cpu().numpy().view(np.uint32)[0]] == ['0xd16cfe09', '0x94fdcceb', '0x5001e420', '0x24126ea1']
+
+
+@pytest.mark.parametrize("name", ["tiny_cmb", "tiny_shear", "c2"])
+def test_prior_transform(name):
+    wl = workload(name)
+    u = np.concatenate([W.u_prior_set(wl, 257), np.full((1, wl.D), 0.5), np.full((1, wl.D), 1e-6), np.full((1, wl.D), 1 - 1e-6)])
+    u32 = u.astype(np.float32)
+    with nsgpu.Context(wl, max_batch=512) as ctx:
+        got = ctx.prior_transform(dev(u32)).cpu().numpy()
+    ref = prior.transform(wl.prior_kind, wl.prior_p0, wl.prior_p1, u32.astype(np.float64))
+    scale = np.where(wl.prior_kind == 0, wl.prior_p1 - wl.prior_p0, wl.prior_p1)
+    assert np.max(np.abs(got - ref) / scale) < 2e-6
+
+
+@pytest.mark.parametrize("name,B", [("toy_small", 67), ("tiny_shear", 37), ("tiny_shear_spline", 5), ("tiny_cmb", 130),
+                                    ("toy", 300), ("toy_w64", 129)])
+@pytest.mark.parametrize("mlp", [nsgpu.MLP_SIMT, nsgpu.MLP_AUTO])
+def test_emulator_and_theory_and_loglike_small(name, B, mlp):
+    wl = workload(name)
+    u = np.concatenate([W.u_post_set(wl, B // 2), W.u_prior_set(wl, B - B // 2)])
+    theta = theta_of_u(wl, u)
+    th64 = theta.astype(np.float64)
+    with nsgpu.Context(wl, max_batch=B + 3, mlp=mlp) as ctx:
+        t = dev(theta)
+        for e, em in enumerate(wl.emulators):
+            got = ctx.emulate_batch(t, e).cpu().numpy().astype(np.float64)
+            ref = LK.emulate(wl, th64, e)
+            assert got.shape == ref.shape
+            assert emulator_rel_err(got, ref, em.out_kind) <= 1e-4
+        model = ctx.theory_batch(t).cpu().numpy()
+        ref_model = LK.theory(wl, th64)
+        scale = np.abs(ref_model) + np.sqrt(np.mean(ref_model ** 2, axis=1, keepdims=True))
+        assert np.max(np.abs(model - ref_model) / scale) < 2e-4
+        got = ctx.loglike_batch(t).cpu().numpy()
+        ref = LK.loglike(wl, th64)
+        chi2 = -2.0 * (ref - gaussian.log_norm(wl.chol))
+        assert np.all(np.isfinite(got))
+        assert np.all(np.abs(got - ref) <= loglike_tolerance(chi2)), (np.abs(got - ref) / loglike_tolerance(chi2)).max()
+        # host entry point = device entry point
+        np.testing.assert_array_equal(ctx.loglike_batch_host(theta), got)
+
+
+@pytest.mark.parametrize("name", ["c1", "c2", "c3a", "c3b"])
+def test_full_size_configs_sampled_parity(name):
+    """BASELINE.json configs at B = 4096 in the launch configuration bench.py times; the oracle checks
+    a sample of rows (the whole batch is checked for finiteness and permutation invariance)."""
+    wl = workload(name)
+    B = 4096
+    u = np.concatenate([W.u_post_set(wl, B // 2), W.u_prior_set(wl, B // 2)])
+    theta = theta_of_u(wl, u)
+    rows = np.r_[0:8, B // 2 - 4:B // 2 + 12, B - 8:B]
+    with nsgpu.Context(wl, max_batch=B) as ctx:
+        t = dev(theta)
+        got = ctx.loglike_batch(t).cpu().numpy()
+        spec = ctx.emulate_batch(t[rows].contiguous(), 0).cpu().numpy().astype(np.float64)
+        perm = torch.randperm(B, device="cuda", generator=torch.Generator(device="cuda").manual_seed(1))
+        got_perm = ctx.loglike_batch(t[perm].contiguous()).cpu().numpy()
+    assert np.all(np.isfinite(got))
+    np.testing.assert_array_equal(got_perm, got[perm.cpu().numpy()])        # bit-identical under permutation
+    th64 = theta[rows].astype(np.float64)
+    ref_spec = LK.emulate(wl, th64, 0)
+    assert emulator_rel_err(spec, ref_spec, wl.emulators[0].out_kind) <= 1e-4
+    ref = LK.loglike(wl, th64)
+    chi2 = -2.0 * (ref - gaussian.log_norm(wl.chol))
+    err = np.abs(got[rows] - ref)
+    assert np.all(err <= loglike_tolerance(chi2)), (err / loglike_tolerance(chi2)).max()
+    assert np.sum(chi2 <= 2000.0) >= 8          # the absolute-tolerance regime is actually exercised
+
+
+def test_edge_cases_and_errors():
+    wl = workload("tiny_cmb")
+    with nsgpu.Context(wl, max_batch=16) as ctx:
+        empty = torch.empty((0, wl.D), dtype=torch.float32, device="cuda")
+        assert ctx.loglike_batch(empty).shape == (0,)
+        th0 = theta_of_u(wl, wl.u_fid[None])
+        one = ctx.loglike_batch(dev(th0)).cpu().numpy()
+        full = ctx.loglike_batch(dev(np.repeat(th0, 16, axis=0))).cpu().numpy()
+        np.testing.assert_array_equal(full, np.repeat(one, 16))                # batch-size invariance
+        bad = np.repeat(th0, 4, axis=0)
+        bad[1, 2] = 5.0             # h outside its uniform box
+        bad[2, 0] = np.nan
+        bad[3, 6] = 1.2             # Gaussian-prior dimension: unbounded, finite
+        out = ctx.loglike_batch(dev(bad)).cpu().numpy()
+        assert np.isfinite(out[0]) and out[1] == -np.inf and out[2] == -np.inf and np.isfinite(out[3])
+        with pytest.raises(nsgpu.NsgpuError) as e:
+            ctx.loglike_batch(dev(np.repeat(th0, 17, axis=0)))
+        assert e.value.status == nsgpu.ESHAPE
+    notspd = W.tiny_cmb(); notspd.data = wl.data.copy(); notspd.chol = wl.chol.copy(); notspd.chol[3, 3] = -1.0
+    with pytest.raises(nsgpu.NsgpuError) as e:
+        nsgpu.Context(notspd, max_batch=4)
+    assert e.value.status == nsgpu.ENOTSPD
+    with pytest.raises(nsgpu.NsgpuError) as e:
+        nsgpu.Context(workload("tiny_shear"), max_batch=4, mlp=nsgpu.MLP_TC)      # width 48: no tcgen05 path
+    assert e.value.status == nsgpu.ESHAPE
+
+
+def test_noiseless_fiducial_gives_normalisation_constant():
+    wl = workload("tiny_shear", noise=False)
+    with nsgpu.Context(wl, max_batch=4) as ctx:
+        got = ctx.loglike_batch(dev(theta_of_u(wl, wl.u_fid[None]))).cpu().numpy()[0]
+    assert got == pytest.approx(gaussian.log_norm(wl.chol), abs=1e-3)
+
+
+def test_restricted_lcdm_matches_w0wa_at_minus1_0():
+    full, rest = workload("c3a"), workload("c4_lcdm")
+    ur = W.u_post_set(rest, 16)
+    tr = theta_of_u(rest, ur)
+    tf = np.insert(tr, 6, np.array([[-1.0], [0.0]], np.float32).repeat(16, axis=1), axis=1)
+    with nsgpu.Context(full, max_batch=16) as cf, nsgpu.Context(rest, max_batch=16) as cr:
+        a = cf.theory_batch(dev(tf)).cpu().numpy()
+        b = cr.theory_batch(dev(tr)).cpu().numpy()
+    np.testing.assert_array_equal(a, b)

@@ -1,0 +1,156 @@
+"""-m gpu: sampler kernels (a11-a14) against the oracle: exact where the result is unique (deleted set,
+weights, Cholesky factor), statistical where several results are correct (slice moves, log Z)."""
+import math
+
+import numpy as np
+import pytest
+from scipy import stats
+
+from oracle import gaussian, likelihood as LK, nested
+from paper_2509_13307_b200 import nsgpu, workloads as W
+from tests.util import theta_of_u, workload
+
+pytestmark = pytest.mark.gpu
+torch = pytest.importorskip("torch")
+
+
+def dev(a):
+    return torch.as_tensor(np.ascontiguousarray(a), device="cuda")
+
+
+@pytest.mark.parametrize("n,k", [(4, 2), (200, 100), (1000, 500), (1000, 1), (777, 333), (5000, 2500)])
+def test_delete_lowest_matches_oracle(n, k):
+    wl = workload("identity")
+    rng = np.random.default_rng(n + k)
+    logL = rng.standard_normal(n) * 50.0
+    logL[rng.integers(0, n, 5)] = logL[0]              # ties -> index order
+    with nsgpu.Context(wl, max_batch=max(n, 8)) as ctx:
+        dead, logw, logX, logZ, Lstar = ctx.delete_lowest(dev(logL), k, logX=-1.25, logZ=-3.0)
+        d_o, w_o, nj, lx_o, lz_o, ls_o = nested.delete_lowest(list(logL), k, -1.25, -3.0)
+        assert dead.cpu().numpy().tolist() == d_o                        # integer work: bit exact
+        np.testing.assert_allclose(logw.cpu().numpy(), w_o, rtol=0, atol=1e-12)
+        assert logX == pytest.approx(lx_o, abs=1e-12) and logZ == pytest.approx(lz_o, abs=1e-12) and Lstar == ls_o
+        # first iteration: log Z starts at -inf
+        _, _, _, logZ0, _ = ctx.delete_lowest(dev(logL), k, logX=0.0, logZ=-np.inf)
+        assert logZ0 == pytest.approx(nested.delete_lowest(list(logL), k, 0.0, -np.inf)[4], abs=1e-12)
+
+
+@pytest.mark.parametrize("D,n", [(6, 200), (39, 1000), (64, 300)])
+def test_live_cholesky_matches_oracle(D, n):
+    wl = W.toy_identity(D=D)
+    u = np.random.default_rng(D).random((n, D)).astype(np.float32)
+    u[:, 1] = 0.7 * u[:, 0] + 0.3 * u[:, 1]
+    with nsgpu.Context(wl, max_batch=n) as ctx:
+        L = ctx.live_cholesky(dev(u)).cpu().numpy()
+    np.testing.assert_allclose(L, nested.live_cholesky(u.astype(np.float64)), rtol=1e-9, atol=1e-12)
+
+
+def _ellipsoid_start(wl, n, c, seed=0):
+    rng = np.random.default_rng(seed)
+    D = wl.D
+    z = rng.standard_normal((n, D))
+    z = z / np.linalg.norm(z, axis=1)[:, None] * rng.random((n, 1)) ** (1.0 / D) * math.sqrt(c) * 0.999
+    return (0.5 + z @ wl.chol.T).astype(np.float32)
+
+
+def test_slice_step_valid_and_uniform_in_ellipsoid():
+    wl = W.toy_identity(D=4)
+    c = 9.0
+    Lstar = -0.5 * c + gaussian.log_norm(wl.chol)
+    u0 = _ellipsoid_start(wl, 600, c)
+    with nsgpu.Context(wl, max_batch=600) as ctx:
+        l0 = ctx.loglike_batch(ctx.prior_transform(dev(u0)))
+        assert bool((l0 > Lstar).all())
+        start = torch.arange(500, dtype=torch.int32, device="cuda")
+        u1, l1, ne = ctx.slice_step(dev(u0), l0, start, Lstar, 12, seed=3, iteration=1)
+        u1n, l1n = u1.cpu().numpy(), l1.cpu().numpy()
+        assert np.all((u1n >= 0) & (u1n <= 1)) and np.all(l1n > Lstar)
+        np.testing.assert_allclose(l1n, ctx.loglike_batch(ctx.prior_transform(u1)).cpu().numpy(), rtol=0, atol=1e-9)
+        # agrees with the oracle likelihood at the returned points
+        np.testing.assert_allclose(l1n, LK.loglike_u(wl, u1n.astype(np.float64)), atol=1e-3)
+        v = (-2.0 * (l1n - gaussian.log_norm(wl.chol)) / c) ** 2.0
+        assert stats.kstest(v, "uniform").pvalue > 1e-3
+        assert 3.0 < ne / (500 * 12) < 9.0
+        # n_steps = 0 returns the start points
+        u2, l2, ne2 = ctx.slice_step(dev(u0), l0, start, Lstar, 0)
+        np.testing.assert_array_equal(u2.cpu().numpy(), u0[:500]); assert ne2 == 0
+
+
+def test_slice_step_follows_the_oracle_trajectory_at_first():
+    """Same Philox stream definition (reading N10): until an fp32-vs-fp64 accept/reject flip, chain c
+    makes the same moves as the oracle's chain c.  One move, compared loosely."""
+    wl = W.toy_identity(D=3)
+    c = 16.0
+    Lstar = -0.5 * c + gaussian.log_norm(wl.chol)
+    u0 = _ellipsoid_start(wl, 64, c, seed=5)
+    with nsgpu.Context(wl, max_batch=64) as ctx:
+        l0 = ctx.loglike_batch(ctx.prior_transform(dev(u0)))
+        start = torch.arange(64, dtype=torch.int32, device="cuda")
+        u1, l1, _ = ctx.slice_step(dev(u0), l0, start, Lstar, 1, seed=9, iteration=4)
+    f = lambda u: LK.loglike_u(wl, u)
+    u064 = u0.astype(np.float64)
+    xs, ls, _, _ = nested.evolve_chains(f, u064, f(u064), nested.live_cholesky(u064), Lstar, 1, 9, 4)
+    close = np.max(np.abs(xs - u1.cpu().numpy()), axis=1) < 1e-4
+    assert close.mean() > 0.9
+
+
+def test_1d_interval():
+    wl = W.toy_identity(D=1, sigma=0.05)
+    # L > L*  <=>  |x - 0.5| < 0.1
+    Lstar = -0.5 * (0.1 / 0.05) ** 2 + gaussian.log_norm(wl.chol)
+    u0 = np.full((256, 1), 0.41, np.float32)
+    u_live = np.linspace(0.42, 0.58, 256, dtype=np.float32)[:, None]
+    u_live[0] = 0.41
+    with nsgpu.Context(wl, max_batch=256) as ctx:
+        ll = ctx.loglike_batch(ctx.prior_transform(dev(u_live)))
+        start = torch.zeros(256, dtype=torch.int32, device="cuda")
+        u1, l1, _ = ctx.slice_step(dev(u_live), ll, start, Lstar, 3, seed=2)
+    x = u1.cpu().numpy()[:, 0]
+    assert np.all(np.abs(x - 0.5) < 0.1 + 1e-6)
+    assert stats.kstest((x - 0.4) / 0.2, "uniform").pvalue > 1e-3
+
+
+@pytest.mark.parametrize("D,n_live,k", [(6, 200, 100), (6, 200, 1)])
+def test_run_identity_gaussian_closed_form(D, n_live, k):
+    """log Z = 0 (normalised tight Gaussian in the unit cube), H = -1/2 ln((2 pi e)^D det Sigma)."""
+    wl = W.toy_identity(D=D)
+    Sigma = wl.chol @ wl.chol.T
+    H_exact = -0.5 * math.log((2 * math.pi * math.e) ** D * np.linalg.det(Sigma))
+    seeds = (1, 2, 3, 4, 5) if k > 1 else (1,)
+    zs, errs = [], []
+    with nsgpu.Context(wl, max_batch=n_live) as ctx:
+        for seed in seeds:
+            r = ctx.run(n_live, k, 5 * D if k > 1 else 2 * D, stop_frac=1e-3, seed=seed, max_iter=20000)
+            assert r["converged"]
+            assert abs(r["logZ"]) <= 3.0 * r["logZ_err"] + 0.05, r
+            assert r["logZ_err"] == pytest.approx(r["logZ_err_analytic"], rel=0.3)
+            assert r["H"] == pytest.approx(H_exact, abs=1.0)
+            w = np.exp(r["logw"])
+            assert w.sum() == pytest.approx(1.0, abs=1e-9)
+            np.testing.assert_allclose(w @ r["theta"].astype(np.float64), 0.5, atol=0.02)
+            assert r["n_failed_moves"] == 0
+            zs.append(r["logZ"]); errs.append(r["logZ_err"])
+    if len(zs) > 1:
+        assert np.std(zs, ddof=1) < 2.5 * np.mean(errs)       # scatter consistent with the reported error
+        assert abs(np.mean(zs)) < 3.0 * np.mean(errs) / math.sqrt(len(zs)) + 0.05
+
+
+def test_run_toy_emulator_agrees_with_oracle_ns():
+    """c0 (BASELINE.json configs[0]): no closed form; GPU log Z vs the oracle's own NS run."""
+    wl = workload("toy")
+    with nsgpu.Context(wl, max_batch=200) as ctx:
+        g = [ctx.run(200, 100, 30, seed=s, return_samples=False) for s in (1, 2, 3)]
+    o = nested.run(lambda u: LK.loglike_u(wl, u), wl.D, 200, 100, 30, seed=11)
+    zg = np.mean([r["logZ"] for r in g]); eg = np.mean([r["logZ_err"] for r in g]) / math.sqrt(3)
+    assert all(r["converged"] for r in g) and o["converged"]
+    assert abs(zg - o["logZ"]) <= 3.0 * math.hypot(eg, o["logZ_err"])
+    assert np.mean([r["H"] for r in g]) == pytest.approx(o["H"], rel=0.2)
+
+
+def test_run_constant_likelihood():
+    """degenerate case: identical log L everywhere -> weights telescope, log Z = log L exactly."""
+    wl = W.toy_identity(D=2, sigma=1e6)          # flat to 1e-13 over the unit square
+    with nsgpu.Context(wl, max_batch=64) as ctx:
+        r = ctx.run(64, 32, 4, seed=1, max_iter=6)
+    assert r["logZ"] == pytest.approx(gaussian.log_norm(wl.chol), abs=1e-9)
+    assert not r["converged"] or r["n_iter"] <= 6
