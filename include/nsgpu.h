@@ -174,6 +174,11 @@ typedef struct {
 NSGPU_API nsgpu_status nsgpu_run(nsgpu_ctx* ctx, const nsgpu_run_opts* opts, nsgpu_result* res, float* theta_samples,
                        double* logL_samples, double* logw_samples, int64_t cap, int64_t* n_samples);
 
+/* Samples of the last nsgpu_run on this ctx (kept until the next run or destroy): same buffers and
+ * meaning as nsgpu_run's; *n_samples returns the number available; cap = 0 only queries the count. */
+NSGPU_API nsgpu_status nsgpu_last_samples(nsgpu_ctx* ctx, float* theta_samples, double* logL_samples,
+                                          double* logw_samples, int64_t cap, int64_t* n_samples);
+
 /* a13 tap: delete the k lowest of logL_live [n_live] (DEVICE), accumulate the evidence starting from
  * (*logX, *logZ) (HOST in/out).  dead_idx [k] int32, logw [k] float64 (DEVICE out); *logL_star HOST. */
 NSGPU_API nsgpu_status nsgpu_delete_lowest(nsgpu_ctx* ctx, const double* logL_live, int32_t n_live, int32_t k,
@@ -185,6 +190,16 @@ NSGPU_API nsgpu_status nsgpu_live_cholesky(nsgpu_ctx* ctx, const float* u_live, 
 
 /* RNG tap: out[n][4] = Philox4x32-10(ctr[n][4], key[2]) (DEVICE uint32 in/out; key HOST). */
 NSGPU_API nsgpu_status nsgpu_debug_philox(nsgpu_ctx* ctx, const uint32_t* ctr, int32_t n, const uint32_t* key, uint32_t* out, void* stream);
+
+/* Per-stage device timing with CUDA events recorded on the caller's stream around the library's own
+ * launches (for roofline accounting; off by default).  Stages: 0 first emulator layer (a2+a3),
+ * 1 hidden-layer GEMMs (a3), 2 output-layer GEMM (a4), 3 shear projection (a5-a8), 4 CMB binning (a9),
+ * 5 chi^2 (a10), 6 slice round + compaction (a11-a12), 7 identity/emulator copy.
+ * nsgpu_stage_times synchronises the device, adds the elapsed times since the last call into
+ * ms[8] / count[8] (HOST, overwritten) and resets the accumulators.                                 */
+#define NSGPU_N_STAGES 8
+NSGPU_API nsgpu_status nsgpu_set_profiling(nsgpu_ctx* ctx, int32_t on);
+NSGPU_API nsgpu_status nsgpu_stage_times(nsgpu_ctx* ctx, double* ms, int64_t* count);
 
 /* Introspection: 0 = SIMT, 1 = tcgen05 for emulator `emu`; kernels launched since create. */
 NSGPU_API int32_t nsgpu_mlp_path(const nsgpu_ctx* ctx, int32_t emu);

@@ -344,6 +344,8 @@ extern "C" nsgpu_status nsgpu_destroy(nsgpu_ctx* ctx) {
   cudaSetDevice(ctx->device);
   cudaDeviceSynchronize();
   sampler_destroy(ctx);
+  for (auto& ev : ctx->stage_events) { cudaEventDestroy(ev.a); cudaEventDestroy(ev.b); }
+  for (cudaEvent_t ev : ctx->event_pool) cudaEventDestroy(ev);
   for (size_t e = 0; e < ctx->emu.size(); ++e) {
     EmuDev& E = ctx->emu[e];
     mlp_tc_release(ctx, (int)e);
@@ -369,6 +371,30 @@ extern "C" const char* nsgpu_last_error(const nsgpu_ctx* ctx) { return ctx ? ctx
 extern "C" int32_t nsgpu_mlp_path(const nsgpu_ctx* ctx, int32_t emu) {
   if (!ctx || emu < 0 || emu >= ctx->n_emu) return -1;
   return ctx->emu[emu].path;
+}
+
+extern "C" nsgpu_status nsgpu_set_profiling(nsgpu_ctx* ctx, int32_t on) {
+  if (!ctx) return NSGPU_EINVAL;
+  ctx->profiling = on != 0;
+  return NSGPU_OK;
+}
+
+extern "C" nsgpu_status nsgpu_stage_times(nsgpu_ctx* ctx, double* ms, int64_t* count) {
+  if (!ctx || !ms || !count) return NSGPU_EINVAL;
+  NSGPU_CUDA(cudaSetDevice(ctx->device));
+  NSGPU_CUDA(cudaDeviceSynchronize());
+  for (auto& ev : ctx->stage_events) {
+    float t = 0.f;
+    if (cudaEventElapsedTime(&t, ev.a, ev.b) == cudaSuccess) { ctx->stage_ms[ev.stage] += t; ctx->stage_count[ev.stage]++; }
+    ctx->event_pool.push_back(ev.a);
+    ctx->event_pool.push_back(ev.b);
+  }
+  ctx->stage_events.clear();
+  for (int i = 0; i < NSGPU_N_STAGES; ++i) {
+    ms[i] = ctx->stage_ms[i]; count[i] = ctx->stage_count[i];
+    ctx->stage_ms[i] = 0.0; ctx->stage_count[i] = 0;
+  }
+  return NSGPU_OK;
 }
 
 extern "C" int64_t nsgpu_launch_count(const nsgpu_ctx* ctx) { return ctx ? ctx->launches : -1; }

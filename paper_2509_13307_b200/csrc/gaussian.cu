@@ -88,6 +88,7 @@ nsgpu_status chi2_loglike(nsgpu_ctx* ctx, const float* theta, int B, const int* 
     NSGPU_CUDA(cudaFuncSetAttribute(chi2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     configured = smem;
   }
+  StageTimer tm(ctx, 5, st);
   chi2_kernel<<<(B + TB - 1) / TB, TB * RG, smem, st>>>(ctx->model, ctx->data, ctx->Linv, n, B, n_rows_dev, theta,
                                                          ctx->D, ctx->prior_kind, ctx->prior_p0, ctx->prior_p1,
                                                          ctx->log_norm, logL);

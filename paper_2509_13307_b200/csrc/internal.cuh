@@ -15,6 +15,7 @@
 #define NSGPU_MAX_LAYERS 8   // n_hidden + 1 <= 8
 #define NSGPU_MAX_IN 16      // emulator inputs
 #define NSGPU_MAX_TOMO 10
+#define NSGPU_N_STAGES 8
 #define NSGPU_MAX_D 64       // sampler dimension (one warp per chain, two dims per lane)
 
 struct EmuDev {
@@ -81,6 +82,30 @@ struct nsgpu_ctx {
   SamplerDev* sampler = nullptr;
   std::string err;
   int64_t launches = 0;
+  // optional per-stage CUDA-event timing (nsgpu_set_profiling / nsgpu_stage_times)
+  bool profiling = false;
+  struct StageEv { int stage; cudaEvent_t a, b; };
+  std::vector<StageEv> stage_events;
+  std::vector<cudaEvent_t> event_pool;
+  double stage_ms[NSGPU_N_STAGES] = {};
+  int64_t stage_count[NSGPU_N_STAGES] = {};
+};
+
+// RAII stage timer: records an event pair on `st` around the enclosed launches when profiling is on
+struct StageTimer {
+  nsgpu_ctx* ctx; cudaStream_t st; int idx = -1;
+  StageTimer(nsgpu_ctx* c, int stage, cudaStream_t s) : ctx(c), st(s) {
+    if (!c->profiling) return;
+    nsgpu_ctx::StageEv ev; ev.stage = stage;
+    for (cudaEvent_t* e : {&ev.a, &ev.b}) {
+      if (!c->event_pool.empty()) { *e = c->event_pool.back(); c->event_pool.pop_back(); }
+      else cudaEventCreate(e);
+    }
+    cudaEventRecord(ev.a, s);
+    c->stage_events.push_back(ev);
+    idx = (int)c->stage_events.size() - 1;
+  }
+  ~StageTimer() { if (idx >= 0) cudaEventRecord(ctx->stage_events[idx].b, st); }
 };
 
 #define NSGPU_CUDA(call)                                                                  \

@@ -119,6 +119,7 @@ nsgpu_status mlp_forward_simt(nsgpu_ctx* ctx, int e, const float* theta, int B, 
   float* cur = (float*)ctx->act[0];
   float* nxt = (float*)ctx->act[1];
   {
+    StageTimer tm(ctx, 0, st);
     dim3 grid(M, (E.width + 127) / 128);
     mlp_first_layer_simt<<<grid, 128, 0, st>>>(theta, ctx->D, rpt, M, n_rows_dev, ctx->emu_in_idx,
                                                ctx->emu_in_const, ctx->n_theta_in, ctx->z_emu, E.n_in,
@@ -127,6 +128,7 @@ nsgpu_status mlp_forward_simt(nsgpu_ctx* ctx, int e, const float* theta, int B, 
     NSGPU_LAUNCH_CHECK();
   }
   for (int l = 1; l < E.n_hidden; ++l) {
+    StageTimer tm(ctx, 1, st);
     dim3 grid((M + 63) / 64, (E.width + 63) / 64);
     gemm_simt<0><<<grid, 256, 0, st>>>(cur, E.W[l], E.b[l], E.alpha[l], E.beta[l], M, E.width, E.width,
                                        n_rows_dev, rpt, 0, nxt);
@@ -134,6 +136,7 @@ nsgpu_status mlp_forward_simt(nsgpu_ctx* ctx, int e, const float* theta, int B, 
     float* t = cur; cur = nxt; nxt = t;
   }
   {
+    StageTimer tm(ctx, 2, st);
     dim3 grid((M + 63) / 64, (E.n_out + 63) / 64);
     gemm_simt<1><<<grid, 256, 0, st>>>(cur, E.W[E.n_hidden], E.b[E.n_hidden], E.out_std, E.out_mean, M,
                                        E.n_out, E.width, n_rows_dev, rpt, apply_exp10 ? 1 : 0, spec_out);

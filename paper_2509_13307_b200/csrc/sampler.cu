@@ -54,6 +54,9 @@ struct SamplerDev {
   int* h_counters = nullptr;           // pinned [4]
   unsigned long long* h_evals = nullptr;
   double* h_scal = nullptr;            // pinned [8]
+  // samples of the last nsgpu_run (host): theta [n][D], logL [n], logw [n]
+  std::vector<float> last_theta;
+  std::vector<double> last_logL, last_logw;
 };
 
 namespace {
@@ -567,11 +570,14 @@ static nsgpu_status evolve(nsgpu_ctx* ctx, int n_chains, int n_steps, uint64_t s
   int burst = std::max(8, n_steps * 4);
   while (true) {
     for (int i = 0; i < burst; ++i) {
+      {
+      StageTimer tm(ctx, 6, st);
       slice_round_kernel<<<blocks, 128, 0, st>>>(a);
       NSGPU_LAUNCH_CHECK();
       compact_kernel<<<1, 1024, 0, st>>>(n_chains, ctx->D, S->need, S->row_of_chain, S->theta_chain, S->theta_prop,
                                          S->counters, S->n_evals);
       NSGPU_LAUNCH_CHECK();
+      }
       nsgpu_status s = loglike_device(ctx, S->theta_prop, n_chains, S->counters, S->logL_prop, st);
       if (s != NSGPU_OK) return s;
       ++rounds;
@@ -666,6 +672,21 @@ extern "C" nsgpu_status nsgpu_debug_philox(nsgpu_ctx* ctx, const uint32_t* ctr, 
   NSGPU_CUDA(cudaSetDevice(ctx->device));
   philox_kernel<<<(n + 255) / 256, 256, 0, (cudaStream_t)stream>>>((const uint4*)ctr, n, make_uint2(key[0], key[1]), (uint4*)out);
   NSGPU_LAUNCH_CHECK();
+  return NSGPU_OK;
+}
+
+extern "C" nsgpu_status nsgpu_last_samples(nsgpu_ctx* ctx, float* theta_samples, double* logL_samples,
+                                           double* logw_samples, int64_t cap, int64_t* n_samples) {
+  if (!ctx) return NSGPU_EINVAL;
+  SamplerDev* S = ctx->sampler;
+  const int64_t ntot = (int64_t)S->last_logL.size();
+  if (n_samples) *n_samples = ntot;
+  if (cap <= 0) return NSGPU_OK;
+  if (!theta_samples || !logL_samples || !logw_samples) { ctx->err = "last_samples: NULL buffer"; return NSGPU_EINVAL; }
+  const size_t nw = (size_t)std::min<int64_t>(cap, ntot);
+  memcpy(theta_samples, S->last_theta.data(), sizeof(float) * nw * ctx->D);
+  memcpy(logL_samples, S->last_logL.data(), sizeof(double) * nw);
+  memcpy(logw_samples, S->last_logw.data(), sizeof(double) * nw);
   return NSGPU_OK;
 }
 
@@ -799,20 +820,27 @@ extern "C" nsgpu_status nsgpu_run(nsgpu_ctx* ctx, const nsgpu_run_opts* o, nsgpu
   res->n_iter = it; res->n_dead = (int64_t)nd; res->n_like_evals = (int64_t)*S->h_evals + n; res->n_rounds = rounds;
   res->n_failed_moves = n_fail_total;
   if (n_samples) *n_samples = (int64_t)ntot;
-  if (cap > 0 && theta_samples && logL_samples && logw_samples) {
-    const size_t nw = std::min<size_t>((size_t)cap, ntot);
-    // theta = T(u) through the a1 kernel, in chunks of max_batch rows
+  {
+    // theta = T(u) through the a1 kernel, in chunks of max_batch rows; kept in the ctx for nsgpu_last_samples
     std::vector<float> all_u(ntot * D);
     memcpy(all_u.data(), dead_u.data(), sizeof(float) * nd * D);
     memcpy(all_u.data() + nd * D, live_u.data(), sizeof(float) * (size_t)n * D);
-    for (size_t off = 0; off < nw; off += (size_t)ctx->max_batch) {
-      const int nb = (int)std::min<size_t>((size_t)ctx->max_batch, nw - off);
+    S->last_theta.resize(ntot * D);
+    S->last_logL = all_l;
+    S->last_logw.resize(ntot);
+    for (size_t i = 0; i < ntot; ++i) S->last_logw[i] = terms[i] - logZ;
+    for (size_t off = 0; off < ntot; off += (size_t)ctx->max_batch) {
+      const int nb = (int)std::min<size_t>((size_t)ctx->max_batch, ntot - off);
       NSGPU_CUDA(cudaMemcpy(S->xprop, all_u.data() + off * D, sizeof(float) * (size_t)nb * D, cudaMemcpyHostToDevice));
       s = nsgpu_prior_transform(ctx, S->xprop, nb, S->theta_prop, st);
       if (s != NSGPU_OK) return s;
-      NSGPU_CUDA(cudaMemcpy(theta_samples + off * D, S->theta_prop, sizeof(float) * (size_t)nb * D, cudaMemcpyDeviceToHost));
+      NSGPU_CUDA(cudaMemcpy(S->last_theta.data() + off * D, S->theta_prop, sizeof(float) * (size_t)nb * D, cudaMemcpyDeviceToHost));
     }
-    for (size_t i = 0; i < nw; ++i) { logL_samples[i] = all_l[i]; logw_samples[i] = terms[i] - logZ; }
+  }
+  if (cap > 0 && theta_samples && logL_samples && logw_samples) {
+    int64_t got = 0;
+    s = nsgpu_last_samples(ctx, theta_samples, logL_samples, logw_samples, cap, &got);
+    if (s != NSGPU_OK) return s;
   }
   res->seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t_start).count();
   return converged ? NSGPU_OK : NSGPU_ENOCONV;

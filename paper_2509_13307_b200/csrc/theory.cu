@@ -272,6 +272,7 @@ nsgpu_status shear_project(nsgpu_ctx* ctx, const float* theta, int B, const int*
     NSGPU_CUDA(cudaFuncSetAttribute(shear_project_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     configured = smem;
   }
+  StageTimer tm(ctx, 3, st);
   shear_project_kernel<<<B, 256, smem, st>>>(theta, ctx->D, n_rows_dev, ctx->spec, A, ctx->model, ctx->n_data);
   NSGPU_LAUNCH_CHECK();
   return NSGPU_OK;
@@ -289,6 +290,7 @@ nsgpu_status cmb_bin(nsgpu_ctx* ctx, const float* theta, int B, const int* n_row
     configured = smem;
   }
   const size_t emu_stride = (size_t)ctx->max_batch * ctx->rows_per_theta * n_out;
+  StageTimer tm(ctx, 4, st);
   cmb_bin_kernel<<<B, 256, smem, st>>>(theta, ctx->D, n_rows_dev, ctx->spec, ctx->n_emu, n_out, emu_stride, mask,
                                        ctx->cal_index, ctx->bin_ptr, ctx->bin_col, ctx->bin_val, ctx->n_data,
                                        ctx->model);
@@ -303,6 +305,7 @@ nsgpu_status copy_model(nsgpu_ctx* ctx, const float* theta, int B, const int* n_
   const int n = ctx->n_data;
   const int ex = (!ident && ctx->emu[0].out_kind == 1) ? 1 : 0;
   int blocks = (int)std::min<size_t>(((size_t)B * n + 255) / 256, 148 * 8);
+  StageTimer tm(ctx, 7, st);
   copy_model_kernel<<<blocks, 256, 0, st>>>(src, n, B, n_rows_dev, ex, ctx->model);
   NSGPU_LAUNCH_CHECK();
   return NSGPU_OK;

@@ -21,8 +21,8 @@ MLP_AUTO, MLP_SIMT, MLP_TC = 0, 1, 2
 
 EXPORTS = ["nsgpu_create", "nsgpu_destroy", "nsgpu_last_error", "nsgpu_prior_transform",
            "nsgpu_loglike_batch", "nsgpu_loglike_batch_host", "nsgpu_emulate_batch", "nsgpu_theory_batch",
-           "nsgpu_slice_step", "nsgpu_run", "nsgpu_delete_lowest", "nsgpu_live_cholesky",
-           "nsgpu_debug_philox", "nsgpu_mlp_path", "nsgpu_launch_count"]
+           "nsgpu_slice_step", "nsgpu_run", "nsgpu_last_samples", "nsgpu_delete_lowest", "nsgpu_live_cholesky",
+           "nsgpu_debug_philox", "nsgpu_set_profiling", "nsgpu_stage_times", "nsgpu_mlp_path", "nsgpu_launch_count"]
 
 
 class NsgpuError(RuntimeError):
@@ -104,12 +104,18 @@ def lib():
                                    vp, vp, C.POINTER(C.c_int64), vp]
     L.nsgpu_run.restype = C.c_int
     L.nsgpu_run.argtypes = [vp, C.POINTER(_RunOpts), C.POINTER(_Result), vp, vp, vp, C.c_int64, C.POINTER(C.c_int64)]
+    L.nsgpu_last_samples.restype = C.c_int
+    L.nsgpu_last_samples.argtypes = [vp, vp, vp, vp, C.c_int64, C.POINTER(C.c_int64)]
     L.nsgpu_delete_lowest.restype = C.c_int
     L.nsgpu_delete_lowest.argtypes = [vp, vp, C.c_int32, C.c_int32, _pd, _pd, vp, vp, _pd, vp]
     L.nsgpu_live_cholesky.restype = C.c_int
     L.nsgpu_live_cholesky.argtypes = [vp, vp, C.c_int32, vp, vp]
     L.nsgpu_debug_philox.restype = C.c_int
     L.nsgpu_debug_philox.argtypes = [vp, vp, C.c_int32, C.POINTER(C.c_uint32), vp, vp]
+    L.nsgpu_set_profiling.restype = C.c_int
+    L.nsgpu_set_profiling.argtypes = [vp, C.c_int32]
+    L.nsgpu_stage_times.restype = C.c_int
+    L.nsgpu_stage_times.argtypes = [vp, _pd, C.POINTER(C.c_int64)]
     L.nsgpu_mlp_path.restype = C.c_int32
     L.nsgpu_mlp_path.argtypes = [vp, C.c_int32]
     L.nsgpu_launch_count.restype = C.c_int64
@@ -318,22 +324,28 @@ class Context:
         o = _RunOpts(int(n_live), int(n_delete), int(n_steps), float(stop_frac), int(max_iter), int(seed))
         r = _Result()
         ns = C.c_int64(0)
-        cap = 0
-        th = ll = lw = None
-        if return_samples:
-            cap = int(max_iter) * int(n_delete) + int(n_live) if max_iter < 4096 else 4096 * int(n_delete) + int(n_live)
-            th = np.empty((cap, self.D), np.float32); ll = np.empty(cap, np.float64); lw = np.empty(cap, np.float64)
-        st = self._check(lib().nsgpu_run(self._h, C.byref(o), C.byref(r),
-                                         th.ctypes.data_as(C.c_void_p) if cap else None,
-                                         ll.ctypes.data_as(C.c_void_p) if cap else None,
-                                         lw.ctypes.data_as(C.c_void_p) if cap else None, cap, C.byref(ns)),
+        st = self._check(lib().nsgpu_run(self._h, C.byref(o), C.byref(r), None, None, None, 0, C.byref(ns)),
                          allow=(ENOCONV,))
         out = {f: getattr(r, f) for f, _ in _Result._fields_}
         out["converged"] = st == OK
         if return_samples:
-            n = min(cap, ns.value)
-            out.update(theta=th[:n], logL=ll[:n], logw=lw[:n], n_samples=ns.value)
+            n = ns.value
+            th = np.empty((n, self.D), np.float32); ll = np.empty(n, np.float64); lw = np.empty(n, np.float64)
+            self._check(lib().nsgpu_last_samples(self._h, th.ctypes.data_as(C.c_void_p), ll.ctypes.data_as(C.c_void_p),
+                                                 lw.ctypes.data_as(C.c_void_p), n, C.byref(ns)))
+            out.update(theta=th, logL=ll, logw=lw, n_samples=n)
         return out
+
+    STAGES = ["mlp_first", "mlp_hidden", "mlp_out", "shear_project", "cmb_bin", "chi2", "slice_round", "copy_model"]
+
+    def set_profiling(self, on: bool):
+        self._check(lib().nsgpu_set_profiling(self._h, 1 if on else 0))
+
+    def stage_times(self):
+        """{stage: (total_ms, launches_timed)} since the last call (synchronises the device)."""
+        ms = (C.c_double * 8)(); cnt = (C.c_int64 * 8)()
+        self._check(lib().nsgpu_stage_times(self._h, ms, cnt))
+        return {n: (ms[i], cnt[i]) for i, n in enumerate(self.STAGES)}
 
     def mlp_path(self, emu=0):
         return lib().nsgpu_mlp_path(self._h, emu)
