@@ -1,0 +1,331 @@
+#!/usr/bin/env python
+"""bench.py -- likelihood evaluations/s of the nsgpu hot path (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl nsgpu|reference]
+                    [--workload c3a|c3b|c2|c1|c0] [--batch 4096]
+
+A "step" is one pass of the whole likelihood path (steps a2-a10 of DESIGN.md: emulator MLP -> z
+interpolation + Limber projection (or CMB binning) -> Gaussian chi^2) over one batch of `--batch`
+synthetic parameter vectors.  Default workload: c3a, the 39-D w0wa cosmic-shear likelihood at batch
+4096 that BASELINE.json's metric is quoted on.  One process per GPU; under torchrun every rank
+evaluates its own batch (independent thetas: weak scaling, no data-path collective) and rank 0
+prints ONE JSON line.
+
+  value      device-timed evaluations/s with theta resident in HBM (CUDA events, max over ranks)
+  e2e        the same through nsgpu_loglike_batch_host: pinned-host theta in, host logL out, every step
+  roofline   dominant kernel (hidden-layer GEMMs) from the library's per-stage CUDA events recorded on
+             the launching stream during the timed region
+  cpu_baseline  the fp64 oracle (oracle/, as it stands) timed on the host cores on a bounded sample
+
+`--impl reference` times the oracle itself (there is no reference implementation: DESIGN.md).
+"""
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2509_13307_b200 import workloads as W  # noqa: E402
+
+METRIC = "likelihood evals/sec at batch 4096 (39-D shear); % tensor/HBM roofline"
+UNIT = "evals/s"
+MAKERS = {"c0": W.toy, "c1": W.cmb, "c2": W.c2, "c3a": W.c3a, "c3b": W.c3b}
+
+
+def flops_per_row(em):
+    """algorithmic (useful) flops of one emulator row, hidden-hidden GEMMs and all layers."""
+    hidden = 2.0 * em.width * em.width * (em.n_hidden - 1)
+    total = 2.0 * em.n_in * em.width + hidden + 2.0 * em.width * em.n_out
+    return hidden, total
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return {"hbm_gbs": d["hbm_gbs"], "bf16_burst": d["bf16_tflops"],
+                "bf16_sustained": d.get("bf16_tflops_sustained", d["bf16_tflops"]), "src": "measured"}
+    return {"hbm_gbs": 6650.0, "bf16_burst": 1590.0, "bf16_sustained": 1400.0, "src": "fallback"}
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), line.strip()))
+
+    def stop(self, t0, t1):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, mx, reasons = [], None, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        rows = [r for t, r in self.rows if t0 <= t <= t1 + 0.2] or [r for _, r in self.rows]
+        for r in rows:
+            f = [x.strip() for x in r.split(",")]
+            try:
+                sm.append(float(f[0])); mx = float(f[1])
+            except (ValueError, IndexError):
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": mx, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def make_context(nsgpu, torch, wl, batch, device):
+    """Attach a synthetic data vector made by the CUDA path itself at the fiducial point (the product
+    never touches oracle/): first a context with a placeholder Gaussian, then the real one."""
+    n = wl.n_data
+    wl.data, wl.chol = np.zeros(n), np.eye(n)
+    with nsgpu.Context(wl, max_batch=8, device=device) as c0:
+        u0 = torch.as_tensor(wl.u_fid[None].astype(np.float32), device=f"cuda:{device}")
+        m0 = c0.theory_batch(c0.prior_transform(u0)).cpu().numpy()[0]
+    if wl.theory.kind == W.THEORY_EMULATOR:
+        W.attach_toy_data(wl, m0)
+    else:
+        W.attach_data(wl, m0, noise=True)
+    return nsgpu.Context(wl, max_batch=batch, device=device)
+
+
+def theta_batches(nsgpu, torch, ctx, wl, batch, rank, n_sets, device):
+    """n_sets distinct batches: half S_post (around the fiducial), half S_prior (DESIGN.md input recipe)."""
+    out_dev, out_host = [], []
+    for s in range(n_sets):
+        u = np.concatenate([W.u_post_set(wl, batch // 2, seed=1000 * rank + s),
+                            W.u_prior_set(wl, batch - batch // 2, seed=1000 * rank + s)]).astype(np.float32)
+        th = ctx.prior_transform(torch.as_tensor(u, device=f"cuda:{device}"))
+        out_dev.append(th)
+        out_host.append(th.cpu().numpy())
+    return out_dev, out_host
+
+
+def oracle_rate(wl, n_theta, repeats=1):
+    """fp64 oracle evaluations/s on the host cores (bench cpu_baseline / reference arm only)."""
+    from oracle import likelihood as LK, prior
+    u = np.concatenate([W.u_post_set(wl, n_theta // 2, seed=77), W.u_prior_set(wl, n_theta - n_theta // 2, seed=77)])
+    th = prior.transform(wl.prior_kind, wl.prior_p0, wl.prior_p1, u).astype(np.float32).astype(np.float64)
+    LK.loglike(wl, th[:4])
+    t0 = time.perf_counter()
+    for _ in range(repeats):
+        LK.loglike(wl, th)
+    dt = (time.perf_counter() - t0) / repeats
+    return n_theta / dt, dt
+
+
+def oracle_threads():
+    try:
+        from threadpoolctl import threadpool_info
+        n = [p.get("num_threads", 1) for p in threadpool_info() if p.get("user_api") == "blas"]
+        return max(n) if n else 1
+    except Exception:
+        return 1
+
+
+def attach_oracle_data(wl):
+    from oracle import likelihood as LK, prior
+    th0 = prior.transform(wl.prior_kind, wl.prior_p0, wl.prior_p1, wl.u_fid[None]).astype(np.float32).astype(np.float64)
+    m0 = LK.theory(wl, th0)[0]
+    (W.attach_toy_data if wl.theory.kind == W.THEORY_EMULATOR else W.attach_data)(wl, m0)
+    return wl
+
+
+def run_reference(args, rank):
+    """--impl reference: there is no reference code (paper text only); the arm times the oracle."""
+    if rank != 0:
+        return
+    wl = attach_oracle_data(MAKERS[args.workload]())
+    n = args.ref_sample
+    for _ in range(args.warmup):
+        oracle_rate(wl, min(n, 16))
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle_rate(wl, n)
+    dt = time.perf_counter() - t0
+    value = n * args.steps / dt
+    cores = oracle_threads()
+    sample = f"{n} of {args.batch} thetas per step (half S_post, half S_prior), fp64 numpy oracle as it stands"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"{wl.name} B={args.batch}", "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+def run_nsgpu(args, rank, world, local_rank):
+    import torch
+    from paper_2509_13307_b200 import nsgpu
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (nsgpu has no CPU fallback)")
+    nsgpu.lib()                                   # fails loudly if libnsgpu.so is missing
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        torch.cuda.set_device(local_rank)
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    dev = local_rank
+    torch.cuda.set_device(dev)
+    wl = MAKERS[args.workload]()
+    B = args.batch
+    ctx = make_context(nsgpu, torch, wl, B, dev)
+    n_sets = 4
+    th_dev, th_host = theta_batches(nsgpu, torch, ctx, wl, B, rank, n_sets, dev)
+    out = torch.empty(B, dtype=torch.float64, device=f"cuda:{dev}")
+    host_out = np.empty(B, np.float64)
+    stream = torch.cuda.current_stream()
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def reduce_max(x):
+        if dist is None:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device=f"cuda:{dev}")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    # ---- device-resident timing: value ------------------------------------------------------------
+    for i in range(args.warmup):
+        ctx.loglike_batch(th_dev[i % n_sets], out=out)
+    torch.cuda.synchronize()
+    ctx.set_profiling(True)
+    ctx.stage_times()                              # reset accumulators
+    sampler = ClockSampler(dev)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.25)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    l0 = ctx.launch_count()
+    t_wall0 = time.time()
+    e0.record(stream)
+    for i in range(args.steps):
+        ctx.loglike_batch(th_dev[i % n_sets], out=out)
+    e1.record(stream)
+    barrier()
+    t_wall1 = time.time()
+    launches = ctx.launch_count() - l0
+    ms = reduce_max(e0.elapsed_time(e1))
+    clocks = sampler.stop(t_wall0, t_wall1) if rank == 0 else None
+    stages = ctx.stage_times()
+    ctx.set_profiling(False)
+    finite = bool(torch.isfinite(out).all().item())
+
+    # ---- end to end through the host entry point: e2e ------------------------------------------------
+    for i in range(min(args.warmup, 3)):
+        ctx.loglike_batch_host(th_host[i % n_sets], out=host_out)
+    barrier()
+    t0 = time.perf_counter()
+    for i in range(args.steps):
+        ctx.loglike_batch_host(th_host[i % n_sets], out=host_out)
+    torch.cuda.synchronize()
+    ms_e2e = reduce_max((time.perf_counter() - t0) * 1e3)
+    barrier()
+
+    if rank == 0:
+        pk = peaks()
+        em = wl.emulators[0]
+        rows = B * ctx.rows
+        n_emu = len(wl.emulators)
+        hid_flops, tot_flops = flops_per_row(em)
+        h_ms, h_cnt = stages["mlp_hidden"]
+        launch_flops = 2.0 * rows * em.width * em.width           # one hidden GEMM launch
+        ach = launch_flops * h_cnt / (h_ms * 1e-3) / 1e12 if h_ms > 0 else 0.0
+        mlp_path = ctx.mlp_path(0)
+        if mlp_path == 1:      # tcgen05 fp16 hi/lo split: kind::f16 peak, 3 MMA passes per useful flop
+            peak, peak_note = pk["bf16_sustained"], f"{pk['src']} bf16/fp16 sustained (kind::f16, 3-pass hi/lo split)"
+        else:                  # fp32 CUDA-core GEMM: tensor peak is still the yardstick the north star names
+            peak, peak_note = pk["bf16_sustained"] * 0.5, f"{pk['src']} bf16 sustained x 0.5 (nominal TF32 ratio); SIMT fp32 path"
+        total_stage_ms = sum(v[0] for v in stages.values())
+        roofline = {"bound": "tensor", "kernel": "mlp_hidden", "achieved": ach, "peak": peak, "unit": "TFLOP/s",
+                    "frac": ach / peak if peak else None, "traffic": None, "peak_note": peak_note,
+                    "algorithmic_flops_per_launch": launch_flops, "launches_timed": h_cnt,
+                    "avg_launch_ms": h_ms / h_cnt if h_cnt else None,
+                    "share_of_step": h_ms / total_stage_ms if total_stage_ms else None,
+                    "stage_ms_per_step": {k: v[0] / args.steps for k, v in stages.items() if v[1]}}
+        # HBM-bound projection / binning stage beside it
+        proj = "shear_project" if wl.theory.kind == W.THEORY_SHEAR_LIMBER else ("cmb_bin" if wl.theory.kind == W.THEORY_CMB_BINNED else None)
+        if proj and stages[proj][1]:
+            p_ms, p_cnt = stages[proj]
+            bytes_launch = B * (n_emu * ctx.rows * em.n_out * 4 + wl.n_data * 8 + wl.D * 4)
+            gbs = bytes_launch * p_cnt / (p_ms * 1e-3) / 1e9
+            roofline["projection"] = {"bound": "hbm", "kernel": proj, "achieved": gbs, "peak": pk["hbm_gbs"], "unit": "GB/s",
+                                      "frac": gbs / pk["hbm_gbs"], "algorithmic_bytes_per_launch": bytes_launch}
+        cpu_n = args.cpu_sample
+        wl_o = attach_oracle_data(MAKERS[args.workload]())
+        cpu_v, cpu_dt = oracle_rate(wl_o, cpu_n)
+        total = B * world * args.steps
+        print(json.dumps({
+            "metric": METRIC, "value": total / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": f"{wl.name} B={B} per GPU", "D": wl.D, "rows_per_theta": ctx.rows, "n_data": wl.n_data,
+                       "mlp_path": "tcgen05-f16x3" if mlp_path == 1 else "simt-f32",
+                       "l2": "per-step intermediates (activations, spectra) exceed the 126 MB L2; theta batches rotate over 4 sets",
+                       "outputs_finite": finite},
+            "clocks": clocks,
+            "e2e": {"value": total / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": B * wl.D * 4, "d2h_bytes_per_step": B * 8,
+                    "ms_per_step": ms_e2e / args.steps},
+            "gpu_launches": int(launches),
+            "roofline": roofline,
+            "cpu_baseline": {"value": cpu_v, "unit": UNIT, "cores": oracle_threads(), "kind": "oracle",
+                             "sample": f"{cpu_n} of {B} thetas, {cpu_dt:.1f} s, fp64 numpy oracle as it stands"}}))
+    ctx.close()
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="nsgpu", choices=["nsgpu", "reference"])
+    ap.add_argument("--workload", default="c3a", choices=sorted(MAKERS))
+    ap.add_argument("--batch", type=int, default=4096)
+    ap.add_argument("--cpu-sample", type=int, default=768)
+    ap.add_argument("--ref-sample", type=int, default=128)
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank)
+    else:
+        run_nsgpu(args, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()

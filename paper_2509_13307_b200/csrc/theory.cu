@@ -84,7 +84,8 @@ __global__ void __launch_bounds__(256) shear_project_kernel(const float* __restr
   double* Wt = s1 + nq;                                // [nt][nq] total window
   double* Pg = Wt + (size_t)nt * nq;                   // [n_ell][nq]
   double* wsum = Pg + (size_t)A.n_ell * nq;            // [33]
-  float* table = reinterpret_cast<float*>(wsum + 34);  // [n_z_emu][n_k]
+  const size_t n_dbl = ((size_t)nq * (6 + nt + A.n_ell) + 34 + 1) & ~(size_t)1;   // keep the table 16-byte aligned
+  float* table = reinterpret_cast<float*>(chi + n_dbl);  // [n_z_emu][n_k]
 
   const float* th = theta + (size_t)b * D;
   // stage this theta's log10 P table (the kernel's only large HBM read)
@@ -253,7 +254,7 @@ __global__ void copy_model_kernel(const float* __restrict__ src, int n, int B, c
 }  // namespace
 
 static size_t shear_smem_bytes(const ShearDev& S) {
-  size_t d = (size_t)S.n_chi * (6 + S.n_tomo + S.n_ell) + 34;
+  size_t d = ((size_t)S.n_chi * (6 + S.n_tomo + S.n_ell) + 34 + 1) & ~(size_t)1;
   return d * sizeof(double) + (size_t)S.n_z_emu * S.n_k * sizeof(float) + 16;
 }
 
