@@ -1,13 +1,526 @@
-// mlp_tc.cu -- tcgen05/TMEM emulator GEMMs (placeholder: not built yet, SIMT path is used).
-#include "internal.cuh"
+// mlp_tc.cu -- emulator MLP on the 5th-generation tensor cores (steps a2-a4).
+//
+// One emulator evaluation (BJ north_star): x = (theta_emu[, z] - mu_in)/sigma_in; hidden
+// layers h <- (beta + sigma(alpha t)(1 - beta)) t with t = h.W + b; y = (h.W + b) sigma_out + mu_out.
+//
+// Precision (reading P1): the 1e-4 relative tolerance on 10^y rules out single-pass
+// TF32 (rms 7e-4).  Every GEMM operand is split into two fp16 numbers, x = hi + lo (22 significant
+// bits), and the product is three kind::f16 MMA passes  hi.hi + lo.hi + hi.lo  accumulated in fp32 in
+// TMEM -- the accuracy of 3xTF32 at twice its tensor rate.  Weights are split once at create (scaled by
+// a power of two so that hi and lo are normal fp16 numbers); activations are split in the epilogue of
+// the layer that produces them (scaled by 16) and travel to the next layer as fp16 hi/lo planes.
+//
+// Kernel: persistent, one CTA per SM, 192 threads = 4 epilogue warps + 1 TMA producer warp + 1 MMA
+// warp.  Tile 128 rows x BLOCK_N columns; K in blocks of 64 (one 128-byte swizzle atom); per k-block
+// TMA brings four tiles (A_hi, A_lo, W_hi, W_lo) and the MMA thread issues 3 x 4 tcgen05.mma; two
+// TMEM accumulators (2 x 256 columns) so that the epilogue of tile i (tcgen05.ld, bias, activation,
+// hi/lo split, global stores) overlaps the MMAs of tile i+1.
+#include <cuda.h>
 
-nsgpu_status mlp_tc_prepare(nsgpu_ctx* ctx, int e, const nsgpu_emulator*) {
-  if ((ctx->flags & 3u) == NSGPU_MLP_TC) { ctx->err = "tcgen05 MLP path not built"; return NSGPU_ESHAPE; }
-  ctx->emu[e].path = 0;
+#include <cmath>
+#include <cstring>
+
+#include "internal.cuh"
+#include "tc_ptx.cuh"
+
+namespace {
+
+constexpr int BLOCK_M = 128;
+constexpr int BLOCK_K = 64;                    // fp16 elements: one 128-byte swizzle row
+constexpr int A_TILE_BYTES = BLOCK_M * 128;    // 16 KB
+constexpr float ACT_SCALE = 16.0f;             // activations are stored as fp16 hi/lo of 16 h
+constexpr int SMEM_BUDGET = 225 * 1024;
+// The 4 truncating hi.hi accumulation steps of one k-block shrink a partial by 1.05e-7 on average
+// (measured: output-vs-oracle regression slope -4.19e-7 over 4 layers, identical for K = 128 and 512);
+// the nearest fp32 factor undoes the mean of that bias.
+constexpr float TRUNC_COMP = 1.0f + 1.1920929e-7f;
+
+__host__ __device__ constexpr int stage_bytes(int block_n) { return 2 * A_TILE_BYTES + 2 * block_n * 128; }
+__host__ __device__ constexpr int num_stages(int block_n) {
+  int s = (SMEM_BUDGET - 1024 - 10 * 1024) / stage_bytes(block_n);   // 1 KB alignment slack, 10 KB params + barriers
+  return s > 6 ? 6 : s;
+}
+
+struct GemmArgs {
+  int M_host;                 // rows to process (upper bound when n_rows_dev != nullptr)
+  const int* n_rows_dev;      // live thetas (device) or nullptr
+  int rows_per_theta;
+  int K;                      // fan-in (multiple of 64)
+  int N_pad;                  // padded fan-out (multiple of BLOCK_N)
+  int n_valid;                // true fan-out
+  const float4* p_hidden;     // [N_pad] {bias, -alpha log2 e, 16 beta, 16 (1 - beta)}
+  const float2* p_out;        // [N_pad] {cscale sigma_out, b sigma_out + mu_out}
+  float cscale;               // 2^-(wexp + 4): undoes the operand scalings
+  __half *out_hi, *out_lo;    // next layer's A planes [M][ld_out]
+  int ld_out;
+  float* out_f32;             // output layer: [M][ld_f32]
+  int ld_f32;
+  int apply_exp10;
+};
+
+__device__ __forceinline__ float ex2_approx(float x) { float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float rcp_approx(float x) { float y; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+
+// 16 (beta + sigma(alpha t)(1 - beta)) t with p = {., -alpha log2 e, 16 beta, 16 (1 - beta)};
+// sigma(s) = 1/(1 + 2^(-s log2 e)): 2^x -> inf gives 0, -> 0 gives 1 (no NaN path)
+__device__ __forceinline__ float gated_act16(float t, const float4& p) {
+  const float sg = rcp_approx(1.0f + ex2_approx(p.y * t));
+  return fmaf(sg, p.w, p.z) * t;
+}
+
+// x -> (hi, lo) fp16 pair planes, two elements at a time
+__device__ __forceinline__ void split2(float a, float b, uint32_t& hi, uint32_t& lo) {
+  const __half2 h = __floats2half2_rn(a, b);
+  const float2 hf = __half22float2(h);
+  const __half2 l = __floats2half2_rn(a - hf.x, b - hf.y);
+  hi = *reinterpret_cast<const uint32_t*>(&h);
+  lo = *reinterpret_cast<const uint32_t*>(&l);
+}
+
+// a2 + first hidden layer (K = n_in <= 16: CUDA cores), output as the fp16 hi/lo planes of 16 h.
+// 256 threads, 16 rows per block, each thread owns neuron pairs (2j, 2j+1).
+constexpr int FL_ROWS = 16;
+__global__ void __launch_bounds__(256) mlp_first_layer_tc(const float* __restrict__ theta, int D, int rows_per_theta,
+                                                          int M, const int* __restrict__ n_rows_dev,
+                                                          const int* __restrict__ emu_in_idx,
+                                                          const double* __restrict__ emu_in_const, int n_theta_in,
+                                                          const float* __restrict__ z_emu, int n_in,
+                                                          const float* __restrict__ in_mean,
+                                                          const float* __restrict__ in_std, const float* __restrict__ W,
+                                                          const float4* __restrict__ params, int width,
+                                                          __half* __restrict__ out_hi, __half* __restrict__ out_lo) {
+  if (n_rows_dev) M = min(M, (*n_rows_dev) * rows_per_theta);
+  const int m0 = blockIdx.x * FL_ROWS;
+  if (m0 >= M) return;
+  __shared__ float x[FL_ROWS][NSGPU_MAX_IN];
+  for (int i = threadIdx.x; i < FL_ROWS * NSGPU_MAX_IN; i += blockDim.x) {
+    const int r = i / NSGPU_MAX_IN, c = i - r * NSGPU_MAX_IN;
+    if (c >= n_in) { x[r][c] = 0.0f; continue; }
+    const int m = min(m0 + r, M - 1);
+    const int th = m / rows_per_theta, zi = m - th * rows_per_theta;
+    float v;
+    if (c < n_theta_in) {
+      const int src = emu_in_idx[c];
+      v = src >= 0 ? theta[(size_t)th * D + src] : (float)emu_in_const[c];
+    } else {
+      v = z_emu[zi];
+    }
+    x[r][c] = (v - in_mean[c]) / in_std[c];
+  }
+  __syncthreads();
+  for (int j = threadIdx.x * 2; j < width; j += blockDim.x * 2) {
+    const float4 p0 = params[j], p1 = params[j + 1];
+    float w0[NSGPU_MAX_IN], w1[NSGPU_MAX_IN];
+#pragma unroll
+    for (int i = 0; i < NSGPU_MAX_IN; ++i) {
+      w0[i] = i < n_in ? W[(size_t)i * width + j] : 0.0f;
+      w1[i] = i < n_in ? W[(size_t)i * width + j + 1] : 0.0f;
+    }
+#pragma unroll 2
+    for (int r = 0; r < FL_ROWS; ++r) {
+      if (m0 + r >= M) break;
+      float t0 = p0.x, t1 = p1.x;
+#pragma unroll
+      for (int i = 0; i < NSGPU_MAX_IN; ++i) { t0 = fmaf(x[r][i], w0[i], t0); t1 = fmaf(x[r][i], w1[i], t1); }
+      uint32_t hi, lo;
+      split2(gated_act16(t0, p0), gated_act16(t1, p1), hi, lo);
+      const size_t o = (size_t)(m0 + r) * width + j;
+      *reinterpret_cast<uint32_t*>(out_hi + o) = hi;
+      *reinterpret_cast<uint32_t*>(out_lo + o) = lo;
+    }
+  }
+}
+
+// C[M][N] = epi(A[M][K] . W[N][K]^T) with A, W as fp16 hi/lo planes (three MMA passes).
+// EPI 0: hidden layer -> next layer's hi/lo planes; EPI 1: output layer -> fp32 y (optionally 10^y).
+//
+// Accumulation ("tensor-core accumulator truncation"): tcgen05.mma adds into its
+// fp32 TMEM accumulator with truncation, which over a K = 512 chain of 96 instructions shrinks every
+// output by ~2e-6 -- a coherent error the 1e-3 log L tolerance cannot absorb.  So the tensor core
+// only ever accumulates ONE k-block (64 inputs: 8 small correction MMAs first, then the 4 hi.hi MMAs)
+// into a fresh TMEM partial; the 8 epilogue warps pull each partial into registers (tcgen05.ld) and do
+// the cross-k-block summation in round-to-nearest fp32 there, while the MMA thread fills the other
+// partial buffer.  Bias, activation, hi/lo split and the global stores then run from registers.
+constexpr int GEMM_THREADS = 320;              // warps 0-7 epilogue, warp 8 TMA producer, warp 9 MMA issuer
+template <int BLOCK_N, int EPI>
+__global__ void __launch_bounds__(GEMM_THREADS, 1) mlp_gemm_tc(const __grid_constant__ CUtensorMap tm_ahi,
+                                                               const __grid_constant__ CUtensorMap tm_alo,
+                                                               const __grid_constant__ CUtensorMap tm_whi,
+                                                               const __grid_constant__ CUtensorMap tm_wlo, GemmArgs g) {
+  constexpr int STAGES = num_stages(BLOCK_N);
+  constexpr int STAGE = stage_bytes(BLOCK_N);
+  constexpr int B_TILE_BYTES = BLOCK_N * 128;
+  constexpr int CPT = BLOCK_N / 2;                               // columns per epilogue thread
+  constexpr uint32_t IDESC = tc::idesc_f16_f32(BLOCK_M, BLOCK_N);
+  static_assert(STAGES >= 2, "need at least two smem stages");
+  static_assert(BLOCK_N % 32 == 0 && BLOCK_N >= 32 && BLOCK_N <= 256, "UMMA N for M = 128; CPT multiple of 16");
+
+  extern __shared__ unsigned char smem_dyn[];
+  const uint32_t base = (tc::smem_u32(smem_dyn) + 1023u) & ~1023u;       // SWIZZLE_128B tiles: 1024-byte aligned
+  unsigned char* base_ptr = smem_dyn + (base - tc::smem_u32(smem_dyn));
+  const uint32_t bars = base + STAGES * STAGE;                            // full[S], empty[S], pfull[2], pempty[2]
+  const uint32_t full0 = bars, empty0 = bars + 8 * STAGES, pfull0 = bars + 16 * STAGES, pempty0 = pfull0 + 16;
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(base_ptr + STAGES * STAGE + 16 * STAGES + 32);
+  float* params = reinterpret_cast<float*>(base_ptr + STAGES * STAGE + 16 * STAGES + 64);   // 16-byte aligned
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  int M = g.M_host;
+  if (g.n_rows_dev) M = min(M, (*g.n_rows_dev) * g.rows_per_theta);
+  const int n_blocks = g.N_pad / BLOCK_N;
+  const int num_tiles = ((M + BLOCK_M - 1) / BLOCK_M) * n_blocks;
+  const int k_blocks = g.K / BLOCK_K;
+
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < STAGES; ++s) { tc::mbar_init(full0 + 8 * s, 1); tc::mbar_init(empty0 + 8 * s, 1); }
+    for (int b = 0; b < 2; ++b) { tc::mbar_init(pfull0 + 8 * b, 1); tc::mbar_init(pempty0 + 8 * b, 8); }
+    tc::fence_barrier_init();
+  }
+  if (warp == 9) tc::tmem_alloc(tc::smem_u32(tmem_slot), 512);
+  if (warp == 8 && lane == 0) {
+    tc::prefetch_tmap(&tm_ahi); tc::prefetch_tmap(&tm_alo); tc::prefetch_tmap(&tm_whi); tc::prefetch_tmap(&tm_wlo);
+  }
+  if (EPI == 0) {   // hidden layers: N_pad <= 512 -> 8 KB of per-column parameters staged once
+    for (int i = threadIdx.x; i < g.N_pad; i += blockDim.x) reinterpret_cast<float4*>(params)[i] = g.p_hidden[i];
+  }
+  tc::fence_before_sync();
+  __syncthreads();
+  tc::fence_after_sync();
+  const uint32_t tmem_base = *tmem_slot;
+
+  if (warp == 8) {
+    // ===== TMA producer =====
+    if (lane == 0) {
+      uint32_t stage = 0, phase = 0;
+      for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
+        const int m_blk = tile / n_blocks, n_blk = tile - m_blk * n_blocks;
+        for (int kb = 0; kb < k_blocks; ++kb) {
+          tc::mbar_wait(empty0 + 8 * stage, phase ^ 1);
+          const uint32_t s0 = base + stage * STAGE, fb = full0 + 8 * stage;
+          tc::mbar_arrive_expect_tx(fb, STAGE);
+          tc::tma_load_2d(s0, &tm_ahi, kb * BLOCK_K, m_blk * BLOCK_M, fb);
+          tc::tma_load_2d(s0 + A_TILE_BYTES, &tm_alo, kb * BLOCK_K, m_blk * BLOCK_M, fb);
+          tc::tma_load_2d(s0 + 2 * A_TILE_BYTES, &tm_whi, kb * BLOCK_K, n_blk * BLOCK_N, fb);
+          tc::tma_load_2d(s0 + 2 * A_TILE_BYTES + B_TILE_BYTES, &tm_wlo, kb * BLOCK_K, n_blk * BLOCK_N, fb);
+          if (++stage == STAGES) { stage = 0; phase ^= 1; }
+        }
+      }
+    }
+  } else if (warp == 9) {
+    // ===== MMA issuer (one thread): one fresh TMEM partial per k-block =====
+    if (lane == 0) {
+      uint32_t stage = 0, phase = 0, pcount = 0;
+      for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
+        for (int kb = 0; kb < k_blocks; ++kb, ++pcount) {
+          const uint32_t pb = pcount & 1, pphase = (pcount >> 1) & 1;
+          tc::mbar_wait(pempty0 + 8 * pb, pphase ^ 1);          // the epilogue has pulled this partial
+          tc::mbar_wait(full0 + 8 * stage, phase);
+          tc::fence_after_sync();
+          const uint32_t d_tmem = tmem_base + pb * 256;
+          const uint32_t s0 = base + stage * STAGE;
+          const uint64_t a_hi = tc::smem_desc_sw128(s0), a_lo = tc::smem_desc_sw128(s0 + A_TILE_BYTES);
+          const uint64_t b_hi = tc::smem_desc_sw128(s0 + 2 * A_TILE_BYTES);
+          const uint64_t b_lo = tc::smem_desc_sw128(s0 + 2 * A_TILE_BYTES + B_TILE_BYTES);
+          // UMMA_K = 16 fp16 = 32 bytes: +2 in the descriptor's address field per k step.
+          // Corrections first (the accumulator is still ~2^-11 of its final size), hi.hi last.
+#pragma unroll
+          for (int k = 0; k < BLOCK_K / 16; ++k) {
+            const uint64_t adv = (uint64_t)(2 * k);
+            tc::mma_f16_ss(d_tmem, a_lo + adv, b_hi + adv, IDESC, k != 0);
+            tc::mma_f16_ss(d_tmem, a_hi + adv, b_lo + adv, IDESC, 1);
+          }
+#pragma unroll
+          for (int k = 0; k < BLOCK_K / 16; ++k) {
+            const uint64_t adv = (uint64_t)(2 * k);
+            tc::mma_f16_ss(d_tmem, a_hi + adv, b_hi + adv, IDESC, 1);
+          }
+          tc::mma_commit(empty0 + 8 * stage);                   // smem slot free when these MMAs retire
+          tc::mma_commit(pfull0 + 8 * pb);                      // partial complete
+          if (++stage == STAGES) { stage = 0; phase ^= 1; }
+        }
+      }
+    }
+  } else {
+    // ===== epilogue warps 0..7: TMEM lanes 32 (warp % 4) .., columns CPT (warp / 4) .. =====
+    const int q = warp & 3, hcol = warp >> 2;
+    uint32_t pcount = 0;
+    for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
+      const int m_blk = tile / n_blocks, n_blk = tile - m_blk * n_blocks;
+      float acc[CPT];
+      for (int kb = 0; kb < k_blocks; ++kb, ++pcount) {
+        const uint32_t pb = pcount & 1, pphase = (pcount >> 1) & 1;
+        tc::mbar_wait(pfull0 + 8 * pb, pphase);
+        tc::fence_after_sync();
+        const uint32_t t_src = tmem_base + pb * 256 + ((uint32_t)(q * 32) << 16) + hcol * CPT;
+#pragma unroll
+        for (int c = 0; c < CPT / 16; ++c) {
+          uint32_t r[16];
+          tc::tmem_ld_32x16(t_src + 16 * c, r);
+          tc::tmem_ld_wait();
+          if (kb == 0) {
+#pragma unroll
+            for (int j = 0; j < 16; ++j) acc[16 * c + j] = __uint_as_float(r[j]);
+          } else {
+#pragma unroll
+            for (int j = 0; j < 16; ++j) acc[16 * c + j] += __uint_as_float(r[j]);
+          }
+        }
+        tc::fence_before_sync();
+        __syncwarp();
+        if (lane == 0) tc::mbar_arrive(pempty0 + 8 * pb);
+      }
+      const int row = m_blk * BLOCK_M + q * 32 + lane;
+      const bool row_ok = row < M;
+      const int n0 = n_blk * BLOCK_N + hcol * CPT;
+      if (EPI == 0) {
+        const float4* p = reinterpret_cast<const float4*>(params) + n0;
+        __half* dh = g.out_hi + (size_t)row * g.ld_out + n0;
+        __half* dl = g.out_lo + (size_t)row * g.ld_out + n0;
+#pragma unroll
+        for (int c = 0; c < CPT / 8; ++c) {
+          uint32_t hi[4], lo[4];
+#pragma unroll
+          for (int j = 0; j < 4; ++j) {
+            const float4 pa = p[8 * c + 2 * j], pb2 = p[8 * c + 2 * j + 1];
+            const float ta = fmaf(acc[8 * c + 2 * j], g.cscale, pa.x);
+            const float tb = fmaf(acc[8 * c + 2 * j + 1], g.cscale, pb2.x);
+            split2(gated_act16(ta, pa), gated_act16(tb, pb2), hi[j], lo[j]);
+          }
+          if (row_ok) {
+            reinterpret_cast<uint4*>(dh)[c] = make_uint4(hi[0], hi[1], hi[2], hi[3]);
+            reinterpret_cast<uint4*>(dl)[c] = make_uint4(lo[0], lo[1], lo[2], lo[3]);
+          }
+        }
+      } else {
+        const float2* p = g.p_out + n0;            // warp-uniform addresses: L1 broadcast
+        float* dst = g.out_f32 + (size_t)row * g.ld_f32 + n0;
+        const bool vec = (g.ld_f32 & 3) == 0;
+#pragma unroll
+        for (int c = 0; c < CPT / 4; ++c) {
+          float y[4];
+#pragma unroll
+          for (int j = 0; j < 4; ++j) {
+            const float2 pj = __ldg(p + 4 * c + j);
+            y[j] = fmaf(acc[4 * c + j], pj.x, pj.y);
+            if (g.apply_exp10) y[j] = exp10f(y[j]);
+          }
+          if (row_ok) {
+            if (vec && n0 + 4 * c + 4 <= g.n_valid) {
+              reinterpret_cast<float4*>(dst)[c] = make_float4(y[0], y[1], y[2], y[3]);
+            } else {
+#pragma unroll
+              for (int j = 0; j < 4; ++j)
+                if (n0 + 4 * c + j < g.n_valid) dst[4 * c + j] = y[j];
+            }
+          }
+        }
+      }
+    }
+  }
+  tc::fence_before_sync();
+  __syncthreads();
+  if (warp == 9) tc::tmem_dealloc(tmem_base, 512);
+}
+
+}  // namespace
+
+// ---------------------------------------------------------------------------------------------------
+// host side
+// ---------------------------------------------------------------------------------------------------
+namespace {
+
+struct TcLayer {
+  int K = 0, N_pad = 0, n_valid = 0, block_n = 0, wexp = 0;
+  __half *Whi = nullptr, *Wlo = nullptr;     // [N_pad][K] K-major, scaled by 2^wexp
+  float4* p_hidden = nullptr;                // layers 0 .. n_hidden-1
+  float2* p_out = nullptr;                   // output layer
+  CUtensorMap tm_whi, tm_wlo;
+};
+
+struct TcState {
+  std::vector<TcLayer> layers;               // index = layer 0 .. n_hidden (layer 0 uses p_hidden only)
+  CUtensorMap tm_act[2][2];                  // [buffer][hi, lo]
+  __half* act[2][2] = {};
+  size_t M_max = 0;
+};
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn encode_fn() {
+  static EncodeTiledFn fn = nullptr;
+  if (!fn) {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+        q == cudaDriverEntryPointSuccess)
+      fn = (EncodeTiledFn)p;
+  }
+  return fn;
+}
+
+// fp16 [rows][cols] row-major, box = box_rows x 64 columns (128 bytes), 128-byte swizzle, OOB -> 0
+bool make_tmap(CUtensorMap* tm, const void* ptr, size_t rows, size_t cols, int box_rows) {
+  EncodeTiledFn fn = encode_fn();
+  if (!fn) return false;
+  const cuuint64_t dims[2] = {(cuuint64_t)cols, (cuuint64_t)rows};
+  const cuuint64_t strides[1] = {(cuuint64_t)cols * sizeof(__half)};
+  const cuuint32_t box[2] = {(cuuint32_t)BLOCK_K, (cuuint32_t)box_rows};
+  const cuuint32_t estr[2] = {1, 1};
+  return fn(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 2, const_cast<void*>(ptr), dims, strides, box, estr,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+int pick_block_n(int n, bool hidden) {
+  if (hidden) return n % 256 == 0 ? 256 : (n % 128 == 0 ? 128 : 64);
+  const int cand[4] = {256, 224, 128, 64};
+  int best = 64, best_pad = 1 << 30;
+  for (int c : cand) {
+    const int pad = (n + c - 1) / c * c;
+    if (pad < best_pad) { best_pad = pad; best = c; }
+  }
+  return best;
+}
+
+template <int BN, int EPI>
+nsgpu_status launch_gemm(nsgpu_ctx* ctx, const CUtensorMap& ahi, const CUtensorMap& alo, const TcLayer& L,
+                         const GemmArgs& g, cudaStream_t st) {
+  const int smem = num_stages(BN) * stage_bytes(BN) + 16 * num_stages(BN) + 64 + (EPI == 0 ? 16 * g.N_pad : 0) + 1024;
+  static bool configured = false;
+  if (!configured) {
+    NSGPU_CUDA(cudaFuncSetAttribute(mlp_gemm_tc<BN, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BUDGET));
+    configured = true;
+  }
+  const int tiles = ((g.M_host + BLOCK_M - 1) / BLOCK_M) * (g.N_pad / BN);
+  const int grid = std::min(tiles, ctx->sm_count);
+  mlp_gemm_tc<BN, EPI><<<grid, GEMM_THREADS, smem, st>>>(ahi, alo, L.tm_whi, L.tm_wlo, g);
+  NSGPU_LAUNCH_CHECK();
   return NSGPU_OK;
 }
-void mlp_tc_release(nsgpu_ctx*, int) {}
-nsgpu_status mlp_forward_tc(nsgpu_ctx* ctx, int, const float*, int, const int*, float*, bool, cudaStream_t) {
-  ctx->err = "tcgen05 MLP path not built";
-  return NSGPU_ESHAPE;
+
+template <int EPI>
+nsgpu_status dispatch_gemm(nsgpu_ctx* ctx, const CUtensorMap& ahi, const CUtensorMap& alo, const TcLayer& L,
+                           const GemmArgs& g, cudaStream_t st) {
+  switch (L.block_n) {
+    case 256: return launch_gemm<256, EPI>(ctx, ahi, alo, L, g, st);
+    case 224: return launch_gemm<224, EPI>(ctx, ahi, alo, L, g, st);
+    case 128: return launch_gemm<128, EPI>(ctx, ahi, alo, L, g, st);
+    default: return launch_gemm<64, EPI>(ctx, ahi, alo, L, g, st);
+  }
+}
+
+}  // namespace
+
+nsgpu_status mlp_tc_prepare(nsgpu_ctx* ctx, int e, const nsgpu_emulator* h) {
+  EmuDev& E = ctx->emu[e];
+  if (!encode_fn()) { ctx->err = "cuTensorMapEncodeTiled not available from the driver"; return NSGPU_ECUDA; }
+  TcState* T = new TcState();
+  E.tmaps = T;
+  const int width = h->width, nh = h->n_hidden;
+  const size_t M_max = (size_t)ctx->max_batch * ctx->rows_per_theta;
+  T->M_max = M_max;
+  T->layers.resize(nh + 1);
+  const float log2e = 1.4426950408889634f;
+  for (int l = 0; l <= nh; ++l) {
+    TcLayer& L = T->layers[l];
+    const bool hidden = l < nh;
+    L.K = l == 0 ? h->n_in : width;
+    L.n_valid = hidden ? width : h->n_out;
+    L.block_n = pick_block_n(L.n_valid, hidden);
+    L.N_pad = (L.n_valid + L.block_n - 1) / L.block_n * L.block_n;
+    if (l >= 1) {
+      // W[l] is [K][n_valid] row-major at the ABI; the tensor core wants K-major [N_pad][K].
+      const float* W = h->W[l];
+      float wmax = 0.f;
+      for (size_t i = 0; i < (size_t)L.K * L.n_valid; ++i) wmax = std::max(wmax, fabsf(W[i]));
+      L.wexp = wmax > 0.f ? (int)floorf(log2f(4096.0f / wmax)) : 0;
+      L.wexp = std::min(std::max(L.wexp, -8), 24);
+      const float sc = ldexpf(1.0f, L.wexp);
+      std::vector<__half> hi((size_t)L.N_pad * L.K, __float2half_rn(0.f)), lo(hi);
+      for (int k = 0; k < L.K; ++k)
+        for (int n = 0; n < L.n_valid; ++n) {
+          const float w = W[(size_t)k * L.n_valid + n] * sc;
+          const __half wh = __float2half_rn(w);
+          hi[(size_t)n * L.K + k] = wh;
+          lo[(size_t)n * L.K + k] = __float2half_rn(w - __half2float(wh));
+        }
+      NSGPU_CUDA(cudaMalloc((void**)&L.Whi, hi.size() * sizeof(__half)));
+      NSGPU_CUDA(cudaMalloc((void**)&L.Wlo, lo.size() * sizeof(__half)));
+      NSGPU_CUDA(cudaMemcpy(L.Whi, hi.data(), hi.size() * sizeof(__half), cudaMemcpyHostToDevice));
+      NSGPU_CUDA(cudaMemcpy(L.Wlo, lo.data(), lo.size() * sizeof(__half), cudaMemcpyHostToDevice));
+      if (!make_tmap(&L.tm_whi, L.Whi, L.N_pad, L.K, L.block_n) || !make_tmap(&L.tm_wlo, L.Wlo, L.N_pad, L.K, L.block_n)) {
+        ctx->err = "cuTensorMapEncodeTiled failed for a weight plane";
+        return NSGPU_ECUDA;
+      }
+    }
+    if (hidden) {
+      std::vector<float4> p(L.N_pad, make_float4(0.f, 0.f, 0.f, 0.f));
+      for (int n = 0; n < width; ++n) {
+        const float be = h->beta[l][n];
+        p[n] = make_float4(h->b[l][n], -h->alpha[l][n] * log2e, ACT_SCALE * be, ACT_SCALE * (1.0f - be));
+      }
+      NSGPU_CUDA(cudaMalloc((void**)&L.p_hidden, p.size() * sizeof(float4)));
+      NSGPU_CUDA(cudaMemcpy(L.p_hidden, p.data(), p.size() * sizeof(float4), cudaMemcpyHostToDevice));
+    } else {
+      const float cs = ldexpf(1.0f, -(L.wexp + 4)) * TRUNC_COMP;
+      std::vector<float2> p(L.N_pad, make_float2(0.f, 0.f));
+      for (int n = 0; n < h->n_out; ++n)
+        p[n] = make_float2(cs * h->out_std[n], h->b[l][n] * h->out_std[n] + h->out_mean[n]);
+      NSGPU_CUDA(cudaMalloc((void**)&L.p_out, p.size() * sizeof(float2)));
+      NSGPU_CUDA(cudaMemcpy(L.p_out, p.data(), p.size() * sizeof(float2), cudaMemcpyHostToDevice));
+    }
+  }
+  for (int i = 0; i < 2; ++i) {
+    T->act[i][0] = reinterpret_cast<__half*>(ctx->act[i]);
+    T->act[i][1] = T->act[i][0] + M_max * width;
+    for (int pl = 0; pl < 2; ++pl)
+      if (!make_tmap(&T->tm_act[i][pl], T->act[i][pl], M_max, width, BLOCK_M)) {
+        ctx->err = "cuTensorMapEncodeTiled failed for an activation plane";
+        return NSGPU_ECUDA;
+      }
+  }
+  return NSGPU_OK;
+}
+
+void mlp_tc_release(nsgpu_ctx* ctx, int e) {
+  TcState* T = reinterpret_cast<TcState*>(ctx->emu[e].tmaps);
+  if (!T) return;
+  for (TcLayer& L : T->layers) { cudaFree(L.Whi); cudaFree(L.Wlo); cudaFree(L.p_hidden); cudaFree(L.p_out); }
+  delete T;
+  ctx->emu[e].tmaps = nullptr;
+}
+
+nsgpu_status mlp_forward_tc(nsgpu_ctx* ctx, int e, const float* theta, int B, const int* n_rows_dev, float* spec_out,
+                            bool apply_exp10, cudaStream_t st) {
+  const EmuDev& E = ctx->emu[e];
+  TcState* T = reinterpret_cast<TcState*>(E.tmaps);
+  const int rpt = ctx->rows_per_theta;
+  const int M = B * rpt;
+  if (M == 0) return NSGPU_OK;
+  int cur = 0;
+  {
+    StageTimer tm(ctx, 0, st);
+    mlp_first_layer_tc<<<(M + FL_ROWS - 1) / FL_ROWS, 256, 0, st>>>(theta, ctx->D, rpt, M, n_rows_dev, ctx->emu_in_idx,
+                                                                   ctx->emu_in_const, ctx->n_theta_in, ctx->z_emu, E.n_in,
+                                                                   E.in_mean, E.in_std, E.W[0], T->layers[0].p_hidden,
+                                                                   E.width, T->act[0][0], T->act[0][1]);
+    NSGPU_LAUNCH_CHECK();
+  }
+  for (int l = 1; l <= E.n_hidden; ++l) {
+    const TcLayer& L = T->layers[l];
+    const bool hidden = l < E.n_hidden;
+    GemmArgs g;
+    memset(&g, 0, sizeof(g));
+    g.M_host = M; g.n_rows_dev = n_rows_dev; g.rows_per_theta = rpt; g.K = L.K; g.N_pad = L.N_pad; g.n_valid = L.n_valid;
+    g.p_hidden = L.p_hidden; g.p_out = L.p_out; g.cscale = ldexpf(1.0f, -(L.wexp + 4)) * TRUNC_COMP;
+    g.out_hi = T->act[cur ^ 1][0]; g.out_lo = T->act[cur ^ 1][1]; g.ld_out = E.width;
+    g.out_f32 = spec_out; g.ld_f32 = E.n_out; g.apply_exp10 = apply_exp10 ? 1 : 0;
+    StageTimer tm(ctx, hidden ? 1 : 2, st);
+    nsgpu_status s = hidden ? dispatch_gemm<0>(ctx, T->tm_act[cur][0], T->tm_act[cur][1], L, g, st)
+                            : dispatch_gemm<1>(ctx, T->tm_act[cur][0], T->tm_act[cur][1], L, g, st);
+    if (s != NSGPU_OK) return s;
+    cur ^= 1;
+  }
+  return NSGPU_OK;
 }
