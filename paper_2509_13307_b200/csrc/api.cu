@@ -145,6 +145,14 @@ nsgpu_status build_shear(nsgpu_ctx* ctx, const nsgpu_theory* t) {
   for (int m = 0; m < t->n_z_emu; ++m) zef[m] = (float)ze[m];
   NSGPU_CUDA(upload(&S.a_q, a_q.data(), a_q.size()));
   NSGPU_CUDA(upload(&S.z_q, z_q.data(), z_q.size()));
+  {
+    std::vector<double> ln1pz(t->n_chi), lellh(t->n_ell), lf(t->n_ell);
+    for (int q = 0; q < t->n_chi; ++q) ln1pz[q] = log1p(z_q[q]);
+    for (int b = 0; b < t->n_ell; ++b) { lellh[b] = log10(t->ell[b] + 0.5); lf[b] = log(t->ell[b] / 550.0) / log(30.0); }
+    NSGPU_CUDA(upload(&S.ln1pz, ln1pz.data(), ln1pz.size()));
+    NSGPU_CUDA(upload(&S.lellh, lellh.data(), lellh.size()));
+    NSGPU_CUDA(upload(&S.lf, lf.data(), lf.size()));
+  }
   NSGPU_CUDA(upload(&S.tap_start, tap_start.data(), tap_start.size()));
   NSGPU_CUDA(upload(&S.tap_w, tap_w.data(), tap_w.size()));
   NSGPU_CUDA(upload(&S.ell, t->ell, (size_t)t->n_ell));
@@ -277,14 +285,20 @@ nsgpu_status create_impl(nsgpu_ctx* ctx, int32_t D, const nsgpu_prior1d* prior, 
         Linv[i * n + c] = -s / chol[i * n + i];
       }
     }
-    NSGPU_CUDA(upload(&ctx->Linv, Linv.data(), n * n));
+    // stored transposed: LinvT[j][i] = Linv[i][j] (non-zero for i >= j), so that for a fixed column j the
+    // rows i are contiguous -- coalesced for the row-per-thread chi^2 kernel
+    std::vector<double> LinvT(n * n, 0.0);
+    for (size_t i = 0; i < n; ++i)
+      for (size_t j = 0; j <= i; ++j) LinvT[j * n + i] = Linv[i * n + j];
+    NSGPU_CUDA(upload(&ctx->Linv, LinvT.data(), n * n));
     NSGPU_CUDA(upload(&ctx->data, data, n));
   }
 
   // workspaces
   const size_t M_max = (size_t)max_batch * ctx->rows_per_theta;
   if (n_emu > 0) {
-    const size_t act_bytes = M_max * (size_t)width_max * sizeof(float);
+    // fp32 [M][width] (SIMT) or two fp16 planes in 128-row tiles (tcgen05): pad M to a multiple of 128
+    const size_t act_bytes = ((M_max + 127) / 128 * 128) * (size_t)width_max * sizeof(float);
     NSGPU_CUDA(cudaMalloc(&ctx->act[0], act_bytes));
     NSGPU_CUDA(cudaMalloc(&ctx->act[1], act_bytes));
     NSGPU_CUDA(cudaMalloc((void**)&ctx->spec, (size_t)n_emu * M_max * emu[0].n_out * sizeof(float)));
@@ -309,6 +323,8 @@ nsgpu_status create_impl(nsgpu_ctx* ctx, int32_t D, const nsgpu_prior1d* prior, 
       if (s != NSGPU_OK) return s;
     }
   }
+  // the tcgen05 output layer writes the shear table as [theta][k][z] (coalesced for a row-per-thread epilogue)
+  ctx->spec_kz = th->kind == 3 && n_emu == 1 && ctx->emu[0].path == 1;
   return sampler_create(ctx);
 }
 
@@ -356,7 +372,7 @@ extern "C" nsgpu_status nsgpu_destroy(nsgpu_ctx* ctx) {
   cudaFree(ctx->emu_in_idx); cudaFree(ctx->emu_in_const); cudaFree(ctx->z_emu);
   cudaFree(ctx->bin_ptr); cudaFree(ctx->bin_col); cudaFree(ctx->bin_val);
   ShearDev& S = ctx->sh;
-  cudaFree(S.a_q); cudaFree(S.z_q); cudaFree(S.tap_start); cudaFree(S.tap_w); cudaFree(S.ell); cudaFree(S.nz_mean);
+  cudaFree(S.a_q); cudaFree(S.z_q); cudaFree(S.ln1pz); cudaFree(S.lellh); cudaFree(S.lf); cudaFree(S.tap_start); cudaFree(S.tap_w); cudaFree(S.ell); cudaFree(S.nz_mean);
   cudaFree(ctx->data); cudaFree(ctx->Linv);
   cudaFree(ctx->act[0]); cudaFree(ctx->act[1]); cudaFree(ctx->spec); cudaFree(ctx->model);
   cudaFree(ctx->theta_stage); cudaFree(ctx->logL_stage);
@@ -403,8 +419,9 @@ static nsgpu_status run_emulators(nsgpu_ctx* ctx, const float* theta, int B, con
   const size_t stride = (size_t)ctx->max_batch * ctx->rows_per_theta * (ctx->n_emu ? ctx->emu[0].n_out : 0);
   for (int e = 0; e < ctx->n_emu; ++e) {
     float* out = ctx->spec + e * stride;
-    nsgpu_status s = ctx->emu[e].path == 1 ? mlp_forward_tc(ctx, e, theta, B, n_rows_dev, out, false, st)
-                                           : mlp_forward_simt(ctx, e, theta, B, n_rows_dev, out, false, st);
+    nsgpu_status s = ctx->emu[e].path == 1
+                         ? mlp_forward_tc(ctx, e, theta, B, n_rows_dev, out, ctx->spec_kz ? NSGPU_SPEC_KZ : 0, st)
+                         : mlp_forward_simt(ctx, e, theta, B, n_rows_dev, out, 0, st);
     if (s != NSGPU_OK) return s;
   }
   return NSGPU_OK;
@@ -463,8 +480,9 @@ extern "C" nsgpu_status nsgpu_emulate_batch(nsgpu_ctx* ctx, int32_t e, const flo
   if (s != NSGPU_OK || B == 0) return s;
   if (e < 0 || e >= ctx->n_emu) { ctx->err = "emulate: emulator index out of range"; return NSGPU_EINVAL; }
   const bool ex = ctx->emu[e].out_kind == 1;
-  return ctx->emu[e].path == 1 ? mlp_forward_tc(ctx, e, theta, B, nullptr, out, ex, (cudaStream_t)stream)
-                               : mlp_forward_simt(ctx, e, theta, B, nullptr, out, ex, (cudaStream_t)stream);
+  const int mode = ex ? NSGPU_SPEC_EXP10 : 0;
+  return ctx->emu[e].path == 1 ? mlp_forward_tc(ctx, e, theta, B, nullptr, out, mode, (cudaStream_t)stream)
+                               : mlp_forward_simt(ctx, e, theta, B, nullptr, out, mode, (cudaStream_t)stream);
 }
 
 extern "C" nsgpu_status nsgpu_theory_batch(nsgpu_ctx* ctx, const float* theta, int32_t B, double* model, void* stream) {

@@ -11,46 +11,73 @@
 
 namespace {
 
-constexpr int TB = 16;   // thetas per CTA
-constexpr int RG = 16;   // row groups per CTA (TB * RG = 256 threads)
+constexpr int TB = 8;    // thetas per CTA: every inverse-factor element loaded from L2 is used TB times
 
-__global__ void __launch_bounds__(TB* RG) chi2_kernel(const double* __restrict__ model,
-                                                      const double* __restrict__ data,
-                                                      const double* __restrict__ Linv, int n, int B,
-                                                      const int* __restrict__ n_rows_dev,
-                                                      const float* __restrict__ theta, int D,
-                                                      const int* __restrict__ prior_kind,
-                                                      const double* __restrict__ p0, const double* __restrict__ p1,
-                                                      double log_norm, double* __restrict__ logL) {
+// w = Linv r for TB thetas at once, one thread per PAIR of rows (t, n-1-t): the pair has n+1 non-zero
+// columns whatever t is, so the triangular work is balanced across threads.  For a fixed column j the
+// threads read LinvT[j][t] and LinvT[j][n-1-t] (coalesced) and the TB residuals r[j][.] (one broadcast
+// shared-memory line).  fp64 throughout; chi^2 = sum over rows of w^2 by a block reduction.
+__global__ void __launch_bounds__(512) chi2_kernel(const double* __restrict__ model, const double* __restrict__ data,
+                                                    const double* __restrict__ LinvT, int n, int B,
+                                                    const int* __restrict__ n_rows_dev, const float* __restrict__ theta,
+                                                    int D, const int* __restrict__ prior_kind,
+                                                    const double* __restrict__ p0, const double* __restrict__ p1,
+                                                    double log_norm, double* __restrict__ logL) {
   if (n_rows_dev) B = min(B, *n_rows_dev);
   const int b0 = blockIdx.x * TB;
   if (b0 >= B) return;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   double* r = reinterpret_cast<double*>(smem_raw);       // [n][TB]
-  double* part = r + (size_t)n * TB;                     // [RG][TB]
-  const int lane = threadIdx.x % TB, grp = threadIdx.x / TB;
+  double* part = r + (size_t)n * TB;                     // [32][TB] per-warp partial chi^2
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarp = blockDim.x >> 5;
   // residuals, transposed into [j][theta] (coalesced global reads along j)
-  for (int i = threadIdx.x; i < n * TB; i += blockDim.x) {
+  for (int i = tid; i < n * TB; i += blockDim.x) {
     const int t = i / n, j = i - t * n;
     const int b = b0 + t;
     r[(size_t)j * TB + t] = (b < B) ? model[(size_t)b * n + j] - data[j] : 0.0;
   }
   __syncthreads();
-  double ss = 0.0;
-  // rows are dealt round-robin to the row groups so the triangular work is balanced
-  for (int i = grp; i < n; i += RG) {
-    const double* Li = Linv + (size_t)i * n;
-    double acc = 0.0;
-    for (int j = 0; j <= i; ++j) acc = fma(__ldg(Li + j), r[(size_t)j * TB + lane], acc);
-    ss = fma(acc, acc, ss);
+  const int half = (n + 1) >> 1;
+  const int ra = tid, rb = n - 1 - tid;                  // rows of this thread (ra <= rb); ra == rb for the middle row
+  double wa[TB], wb[TB];
+#pragma unroll
+  for (int t = 0; t < TB; ++t) { wa[t] = 0.0; wb[t] = 0.0; }
+  if (tid < half) {
+    // columns j <= ra feed both rows; ra < j <= rb only the long row
+    for (int j = 0; j <= ra; ++j) {
+      const double la = LinvT[(size_t)j * n + ra], lb = LinvT[(size_t)j * n + rb];
+      const double2* rj = reinterpret_cast<const double2*>(r + (size_t)j * TB);
+#pragma unroll
+      for (int t = 0; t < TB / 2; ++t) {
+        const double2 v = rj[t];
+        wa[2 * t] = fma(la, v.x, wa[2 * t]); wa[2 * t + 1] = fma(la, v.y, wa[2 * t + 1]);
+        wb[2 * t] = fma(lb, v.x, wb[2 * t]); wb[2 * t + 1] = fma(lb, v.y, wb[2 * t + 1]);
+      }
+    }
+    for (int j = ra + 1; j <= rb; ++j) {
+      const double lb = LinvT[(size_t)j * n + rb];
+      const double2* rj = reinterpret_cast<const double2*>(r + (size_t)j * TB);
+#pragma unroll
+      for (int t = 0; t < TB / 2; ++t) {
+        const double2 v = rj[t];
+        wb[2 * t] = fma(lb, v.x, wb[2 * t]); wb[2 * t + 1] = fma(lb, v.y, wb[2 * t + 1]);
+      }
+    }
   }
-  part[grp * TB + lane] = ss;
+  const bool two = tid < half && ra != rb;
+#pragma unroll
+  for (int t = 0; t < TB; ++t) {
+    double ss = (tid < half ? wb[t] * wb[t] : 0.0) + (two ? wa[t] * wa[t] : 0.0);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) ss += __shfl_xor_sync(0xffffffffu, ss, o);
+    if (lane == 0) part[warp * TB + t] = ss;
+  }
   __syncthreads();
-  if (grp == 0) {
-    const int b = b0 + lane;
+  if (tid < TB) {
+    const int b = b0 + tid;
     if (b < B) {
       double chi2 = 0.0;
-      for (int g = 0; g < RG; ++g) chi2 += part[g * TB + lane];
+      for (int w = 0; w < nwarp; ++w) chi2 += part[w * TB + tid];
       double out = -0.5 * chi2 + log_norm;
       // support of the uniform priors (compared in the float32 theta arrives in) and finiteness
       bool ok = isfinite(out);
@@ -82,14 +109,16 @@ nsgpu_status chi2_loglike(nsgpu_ctx* ctx, const float* theta, int B, const int* 
                           cudaStream_t st) {
   if (B == 0) return NSGPU_OK;
   const int n = ctx->n_data;
-  const size_t smem = ((size_t)n * TB + RG * TB) * sizeof(double);
+  const int threads = std::min(512, (((n + 1) / 2 + 31) / 32) * 32);
+  if ((n + 1) / 2 > 512) { ctx->err = "chi2: n_data > 1024 not supported"; return NSGPU_ESHAPE; }
+  const size_t smem = ((size_t)n * TB + 32 * TB) * sizeof(double);
   static size_t configured = 0;
   if (smem > configured) {
     NSGPU_CUDA(cudaFuncSetAttribute(chi2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     configured = smem;
   }
   StageTimer tm(ctx, 5, st);
-  chi2_kernel<<<(B + TB - 1) / TB, TB * RG, smem, st>>>(ctx->model, ctx->data, ctx->Linv, n, B, n_rows_dev, theta,
+  chi2_kernel<<<(B + TB - 1) / TB, threads, smem, st>>>(ctx->model, ctx->data, ctx->Linv, n, B, n_rows_dev, theta,
                                                          ctx->D, ctx->prior_kind, ctx->prior_p0, ctx->prior_p1,
                                                          ctx->log_norm, logL);
   NSGPU_LAUNCH_CHECK();

@@ -38,7 +38,8 @@ struct EmuDev {
 struct ShearDev {
   int n_z_emu = 0, n_z = 0, n_chi = 0, n_k = 0, n_ell = 0, n_tomo = 0, n_tap = 0;
   double z_max = 0, k_min = 0, k_max = 0, lk0 = 0, dlk = 0, da = 0, nz_sigma = 0;
-  double *a_q = nullptr, *z_q = nullptr;   // [n_chi]
+  double *a_q = nullptr, *z_q = nullptr, *ln1pz = nullptr;   // [n_chi]
+  double *lellh = nullptr, *lf = nullptr;                    // [n_ell] log10(ell + 1/2), ln(ell/550)/ln 30
   int* tap_start = nullptr;                // [n_chi] first emulator z node used by node q
   double* tap_w = nullptr;                 // [n_chi][n_tap] z-interpolation weights (spline folded in)
   double *ell = nullptr, *nz_mean = nullptr;
@@ -69,11 +70,12 @@ struct nsgpu_ctx {
   ShearDev sh;
   // gaussian
   double* data = nullptr;       // [n_data]
-  double* Linv = nullptr;       // [n_data][n_data] inverse of the Cholesky factor, lower, fp64
+  double* Linv = nullptr;       // [n_data][n_data] TRANSPOSE of the inverse Cholesky factor: LinvT[j][i], fp64
   double log_norm = 0.0;
   // workspaces
   void* act[2] = {nullptr, nullptr};   // [M_max][width] fp32 (SIMT) or 2 x fp16 (tcgen05)
   float* spec = nullptr;               // [n_emu][M_max][n_out] de-standardised y (log10 where exp10)
+  bool spec_kz = false;                // shear + tcgen05: per theta [n_k][n_z_emu] instead of [n_z_emu][n_k]
   double* model = nullptr;             // [max_batch][n_data]
   float* theta_stage = nullptr;        // [max_batch][D] device staging for the host entry
   double* logL_stage = nullptr;
@@ -130,10 +132,13 @@ struct StageTimer {
 
 // stage entry points (one per translation unit); n_rows_dev != nullptr: only the first *n_rows_dev
 // rows (theta) are live, B is then the launch bound
+// spectrum output modes of the emulator forward pass
+#define NSGPU_SPEC_EXP10 1   // write 10^y (emulate tap) instead of y
+#define NSGPU_SPEC_KZ 2      // shear only: table layout [theta][k][z] (z fastest) instead of [theta][z][k]
 nsgpu_status mlp_forward_simt(nsgpu_ctx* ctx, int e, const float* theta, int B, const int* n_rows_dev,
-                              float* spec_out, bool apply_exp10, cudaStream_t st);
+                              float* spec_out, int mode, cudaStream_t st);
 nsgpu_status mlp_forward_tc(nsgpu_ctx* ctx, int e, const float* theta, int B, const int* n_rows_dev,
-                            float* spec_out, bool apply_exp10, cudaStream_t st);
+                            float* spec_out, int mode, cudaStream_t st);
 nsgpu_status mlp_tc_prepare(nsgpu_ctx* ctx, int e, const nsgpu_emulator* h);
 void mlp_tc_release(nsgpu_ctx* ctx, int e);
 nsgpu_status shear_project(nsgpu_ctx* ctx, const float* theta, int B, const int* n_rows_dev, cudaStream_t st);

@@ -111,7 +111,8 @@ __global__ void __launch_bounds__(256) gemm_simt(const float* __restrict__ A, co
 }  // namespace
 
 nsgpu_status mlp_forward_simt(nsgpu_ctx* ctx, int e, const float* theta, int B, const int* n_rows_dev,
-                              float* spec_out, bool apply_exp10, cudaStream_t st) {
+                              float* spec_out, int mode, cudaStream_t st) {
+  const bool apply_exp10 = (mode & NSGPU_SPEC_EXP10) != 0;
   const EmuDev& E = ctx->emu[e];
   const int rpt = ctx->rows_per_theta;
   const int M = B * rpt;

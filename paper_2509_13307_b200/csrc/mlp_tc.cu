@@ -10,14 +10,19 @@
 // a power of two so that hi and lo are normal fp16 numbers); activations are split in the epilogue of
 // the layer that produces them (scaled by 16) and travel to the next layer as fp16 hi/lo planes.
 //
-// Kernel: persistent, one CTA per SM, 192 threads = 4 epilogue warps + 1 TMA producer warp + 1 MMA
-// warp.  Tile 128 rows x BLOCK_N columns; K in blocks of 64 (one 128-byte swizzle atom); per k-block
-// TMA brings four tiles (A_hi, A_lo, W_hi, W_lo) and the MMA thread issues 3 x 4 tcgen05.mma; two
-// TMEM accumulators (2 x 256 columns) so that the epilogue of tile i (tcgen05.ld, bias, activation,
-// hi/lo split, global stores) overlaps the MMAs of tile i+1.
+// Activation planes live in HBM in the tensor core's own canonical (no-swizzle, K-major) operand
+// layout, [M/128 tiles][K/8 pieces][128 rows][8 halves]: a 128-row x 64-column k-block of A is 16 KB
+// contiguous (one cp.async.bulk per plane, no tensor map), and the epilogue -- where a thread owns a
+// ROW of the accumulator -- writes 16-byte pieces that are contiguous across the lanes of a warp.
+//
+// Kernel: persistent, one CTA per SM: epilogue warps + 1 TMA producer warp + 1 MMA warp.  Tile 128 rows
+// x BLOCK_N columns; K in blocks of 64; per k-block the producer brings four tiles (A_hi, A_lo by bulk
+// copy; W_hi, W_lo by tiled TMA with 128-byte swizzle) and the MMA thread issues 12 tcgen05.mma into a
+// fresh TMEM partial (two partial buffers); the epilogue warps sum the partials in registers.
 #include <cuda.h>
 
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 
 #include "internal.cuh"
@@ -26,8 +31,9 @@
 namespace {
 
 constexpr int BLOCK_M = 128;
-constexpr int BLOCK_K = 64;                    // fp16 elements: one 128-byte swizzle row
-constexpr int A_TILE_BYTES = BLOCK_M * 128;    // 16 KB
+constexpr int BLOCK_K = 64;                    // fp16 elements per k-block
+constexpr int A_TILE_BYTES = BLOCK_M * 128;    // 16 KB: 8 pieces x (128 rows x 16 bytes)
+constexpr int PIECE_HALVES = BLOCK_M * 8;      // one 16-byte piece of every row of a tile: 2 KB
 constexpr float ACT_SCALE = 16.0f;             // activations are stored as fp16 hi/lo of 16 h
 constexpr int SMEM_BUDGET = 225 * 1024;
 // The 4 truncating hi.hi accumulation steps of one k-block shrink a partial by 1.05e-7 on average
@@ -48,14 +54,17 @@ struct GemmArgs {
   int K;                      // fan-in (multiple of 64)
   int N_pad;                  // padded fan-out (multiple of BLOCK_N)
   int n_valid;                // true fan-out
+  const __half *a_hi, *a_lo;  // input planes, canonical layout, K columns
   const float4* p_hidden;     // [N_pad] {bias, -alpha log2 e, 16 beta, 16 (1 - beta)}
   const float2* p_out;        // [N_pad] {cscale sigma_out, b sigma_out + mu_out}
   float cscale;               // 2^-(wexp + 4): undoes the operand scalings
-  __half *out_hi, *out_lo;    // next layer's A planes [M][ld_out]
+  __half *out_hi, *out_lo;    // next layer's planes (canonical layout, ld_out columns)
   int ld_out;
-  float* out_f32;             // output layer: [M][ld_f32]
-  int ld_f32;
+  float* out_f32;             // output layer
+  int ld_f32;                 // out_mode 0: y[m][n] at m ld_f32 + n
+  int out_mode;               // out_mode 1: y at theta(m) (n_valid rpt) + n rpt + z(m)  ([theta][n][z], z fastest)
   int apply_exp10;
+  int dbg;                    // timing experiments only (NSGPU_TC_DBG)
 };
 
 __device__ __forceinline__ float ex2_approx(float x) { float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
@@ -77,9 +86,9 @@ __device__ __forceinline__ void split2(float a, float b, uint32_t& hi, uint32_t&
   lo = *reinterpret_cast<const uint32_t*>(&l);
 }
 
-// a2 + first hidden layer (K = n_in <= 16: CUDA cores), output as the fp16 hi/lo planes of 16 h.
-// 256 threads, 16 rows per block, each thread owns neuron pairs (2j, 2j+1).
-constexpr int FL_ROWS = 16;
+// a2 + first hidden layer (K = n_in <= 16: CUDA cores), output as the canonical fp16 hi/lo planes of
+// 16 h.  One CTA per 128-row tile; lane = row, each warp walks 16-byte pieces (8 neurons) so that a
+// warp's stores are 512 contiguous bytes.  W0 and the activation parameters are staged in shared memory.
 __global__ void __launch_bounds__(256) mlp_first_layer_tc(const float* __restrict__ theta, int D, int rows_per_theta,
                                                           int M, const int* __restrict__ n_rows_dev,
                                                           const int* __restrict__ emu_in_idx,
@@ -90,43 +99,52 @@ __global__ void __launch_bounds__(256) mlp_first_layer_tc(const float* __restric
                                                           const float4* __restrict__ params, int width,
                                                           __half* __restrict__ out_hi, __half* __restrict__ out_lo) {
   if (n_rows_dev) M = min(M, (*n_rows_dev) * rows_per_theta);
-  const int m0 = blockIdx.x * FL_ROWS;
+  const int m0 = blockIdx.x * BLOCK_M;
   if (m0 >= M) return;
-  __shared__ float x[FL_ROWS][NSGPU_MAX_IN];
-  for (int i = threadIdx.x; i < FL_ROWS * NSGPU_MAX_IN; i += blockDim.x) {
-    const int r = i / NSGPU_MAX_IN, c = i - r * NSGPU_MAX_IN;
-    if (c >= n_in) { x[r][c] = 0.0f; continue; }
-    const int m = min(m0 + r, M - 1);
-    const int th = m / rows_per_theta, zi = m - th * rows_per_theta;
-    float v;
-    if (c < n_theta_in) {
-      const int src = emu_in_idx[c];
-      v = src >= 0 ? theta[(size_t)th * D + src] : (float)emu_in_const[c];
-    } else {
-      v = z_emu[zi];
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  float4* sp = reinterpret_cast<float4*>(smem_raw);          // [width]
+  float* sW = reinterpret_cast<float*>(sp + width);          // [n_in][width]
+  for (int i = threadIdx.x; i < width; i += blockDim.x) sp[i] = params[i];
+  for (int i = threadIdx.x; i < n_in * width; i += blockDim.x) sW[i] = W[i];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int r = (warp & 3) * 32 + lane;                      // row within the tile
+  const int m = min(m0 + r, M - 1);
+  const int th = m / rows_per_theta, zi = m - th * rows_per_theta;
+  float x[NSGPU_MAX_IN];
+#pragma unroll
+  for (int c = 0; c < NSGPU_MAX_IN; ++c) {
+    float v = 0.0f;
+    if (c < n_in) {
+      if (c < n_theta_in) {
+        const int src = emu_in_idx[c];
+        v = src >= 0 ? theta[(size_t)th * D + src] : (float)emu_in_const[c];
+      } else {
+        v = z_emu[zi];
+      }
+      v = (v - in_mean[c]) / in_std[c];
     }
-    x[r][c] = (v - in_mean[c]) / in_std[c];
+    x[c] = v;
   }
   __syncthreads();
-  for (int j = threadIdx.x * 2; j < width; j += blockDim.x * 2) {
-    const float4 p0 = params[j], p1 = params[j + 1];
-    float w0[NSGPU_MAX_IN], w1[NSGPU_MAX_IN];
+  const int n_pieces = width >> 3, half_pieces = (n_pieces + 1) >> 1;
+  const int p_begin = (warp >> 2) * half_pieces, p_end = min(p_begin + half_pieces, n_pieces);
+  const size_t tile_base = (size_t)blockIdx.x * ((size_t)BLOCK_M * width) + (size_t)r * 8;
+  for (int p = p_begin; p < p_end; ++p) {
+    uint32_t hi[4], lo[4];
 #pragma unroll
-    for (int i = 0; i < NSGPU_MAX_IN; ++i) {
-      w0[i] = i < n_in ? W[(size_t)i * width + j] : 0.0f;
-      w1[i] = i < n_in ? W[(size_t)i * width + j + 1] : 0.0f;
+    for (int jj = 0; jj < 4; ++jj) {
+      const int j = 8 * p + 2 * jj;
+      const float4 pa = sp[j], pb = sp[j + 1];
+      float t0 = pa.x, t1 = pb.x;
+#pragma unroll
+      for (int c = 0; c < NSGPU_MAX_IN; ++c)
+        if (c < n_in) { t0 = fmaf(x[c], sW[c * width + j], t0); t1 = fmaf(x[c], sW[c * width + j + 1], t1); }
+      split2(gated_act16(t0, pa), gated_act16(t1, pb), hi[jj], lo[jj]);
     }
-#pragma unroll 2
-    for (int r = 0; r < FL_ROWS; ++r) {
-      if (m0 + r >= M) break;
-      float t0 = p0.x, t1 = p1.x;
-#pragma unroll
-      for (int i = 0; i < NSGPU_MAX_IN; ++i) { t0 = fmaf(x[r][i], w0[i], t0); t1 = fmaf(x[r][i], w1[i], t1); }
-      uint32_t hi, lo;
-      split2(gated_act16(t0, p0), gated_act16(t1, p1), hi, lo);
-      const size_t o = (size_t)(m0 + r) * width + j;
-      *reinterpret_cast<uint32_t*>(out_hi + o) = hi;
-      *reinterpret_cast<uint32_t*>(out_lo + o) = lo;
+    if (m0 + r < M) {
+      const size_t o = tile_base + (size_t)p * PIECE_HALVES;
+      *reinterpret_cast<uint4*>(out_hi + o) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
+      *reinterpret_cast<uint4*>(out_lo + o) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
     }
   }
 }
@@ -138,22 +156,22 @@ __global__ void __launch_bounds__(256) mlp_first_layer_tc(const float* __restric
 // fp32 TMEM accumulator with truncation, which over a K = 512 chain of 96 instructions shrinks every
 // output by ~2e-6 -- a coherent error the 1e-3 log L tolerance cannot absorb.  So the tensor core
 // only ever accumulates ONE k-block (64 inputs: 8 small correction MMAs first, then the 4 hi.hi MMAs)
-// into a fresh TMEM partial; the 8 epilogue warps pull each partial into registers (tcgen05.ld) and do
+// into a fresh TMEM partial; the epilogue warps pull each partial into registers (tcgen05.ld) and do
 // the cross-k-block summation in round-to-nearest fp32 there, while the MMA thread fills the other
 // partial buffer.  Bias, activation, hi/lo split and the global stores then run from registers.
-constexpr int GEMM_THREADS = 320;              // warps 0-7 epilogue, warp 8 TMA producer, warp 9 MMA issuer
+constexpr int EPI_WARPS = 8;                         // 2 per TMEM lane quarter, each half of the tile's columns
+constexpr int GEMM_THREADS = 32 * (EPI_WARPS + 2);   // + TMA producer warp, + MMA issuer warp
 template <int BLOCK_N, int EPI>
-__global__ void __launch_bounds__(GEMM_THREADS, 1) mlp_gemm_tc(const __grid_constant__ CUtensorMap tm_ahi,
-                                                               const __grid_constant__ CUtensorMap tm_alo,
-                                                               const __grid_constant__ CUtensorMap tm_whi,
+__global__ void __launch_bounds__(GEMM_THREADS, 1) mlp_gemm_tc(const __grid_constant__ CUtensorMap tm_whi,
                                                                const __grid_constant__ CUtensorMap tm_wlo, GemmArgs g) {
   constexpr int STAGES = num_stages(BLOCK_N);
   constexpr int STAGE = stage_bytes(BLOCK_N);
   constexpr int B_TILE_BYTES = BLOCK_N * 128;
-  constexpr int CPT = BLOCK_N / 2;                               // columns per epilogue thread
+  constexpr int CPT = BLOCK_N / (EPI_WARPS / 4);                 // columns per epilogue thread
+  constexpr int LDC = (CPT % 16 == 0) ? 16 : 8;                  // columns per tcgen05.ld
   constexpr uint32_t IDESC = tc::idesc_f16_f32(BLOCK_M, BLOCK_N);
   static_assert(STAGES >= 2, "need at least two smem stages");
-  static_assert(BLOCK_N % 32 == 0 && BLOCK_N >= 32 && BLOCK_N <= 256, "UMMA N for M = 128; CPT multiple of 16");
+  static_assert(BLOCK_N % 32 == 0 && BLOCK_N >= 32 && BLOCK_N <= 256 && CPT % 8 == 0, "UMMA N for M = 128; CPT multiple of 8");
 
   extern __shared__ unsigned char smem_dyn[];
   const uint32_t base = (tc::smem_u32(smem_dyn) + 1023u) & ~1023u;       // SWIZZLE_128B tiles: 1024-byte aligned
@@ -172,13 +190,11 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) mlp_gemm_tc(const __grid_cons
 
   if (threadIdx.x == 0) {
     for (int s = 0; s < STAGES; ++s) { tc::mbar_init(full0 + 8 * s, 1); tc::mbar_init(empty0 + 8 * s, 1); }
-    for (int b = 0; b < 2; ++b) { tc::mbar_init(pfull0 + 8 * b, 1); tc::mbar_init(pempty0 + 8 * b, 8); }
+    for (int b = 0; b < 2; ++b) { tc::mbar_init(pfull0 + 8 * b, 1); tc::mbar_init(pempty0 + 8 * b, EPI_WARPS); }
     tc::fence_barrier_init();
   }
-  if (warp == 9) tc::tmem_alloc(tc::smem_u32(tmem_slot), 512);
-  if (warp == 8 && lane == 0) {
-    tc::prefetch_tmap(&tm_ahi); tc::prefetch_tmap(&tm_alo); tc::prefetch_tmap(&tm_whi); tc::prefetch_tmap(&tm_wlo);
-  }
+  if (warp == EPI_WARPS + 1) tc::tmem_alloc(tc::smem_u32(tmem_slot), 512);
+  if (warp == EPI_WARPS && lane == 0) { tc::prefetch_tmap(&tm_whi); tc::prefetch_tmap(&tm_wlo); }
   if (EPI == 0) {   // hidden layers: N_pad <= 512 -> 8 KB of per-column parameters staged once
     for (int i = threadIdx.x; i < g.N_pad; i += blockDim.x) reinterpret_cast<float4*>(params)[i] = g.p_hidden[i];
   }
@@ -187,25 +203,28 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) mlp_gemm_tc(const __grid_cons
   tc::fence_after_sync();
   const uint32_t tmem_base = *tmem_slot;
 
-  if (warp == 8) {
+  if (warp == EPI_WARPS) {
     // ===== TMA producer =====
     if (lane == 0) {
       uint32_t stage = 0, phase = 0;
       for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
         const int m_blk = tile / n_blocks, n_blk = tile - m_blk * n_blocks;
+        // this tile's A rows: k-block kb is the 16 KB starting at piece 8 kb
+        const size_t a_tile = (size_t)m_blk * ((size_t)BLOCK_M * g.K);
         for (int kb = 0; kb < k_blocks; ++kb) {
           tc::mbar_wait(empty0 + 8 * stage, phase ^ 1);
           const uint32_t s0 = base + stage * STAGE, fb = full0 + 8 * stage;
           tc::mbar_arrive_expect_tx(fb, STAGE);
-          tc::tma_load_2d(s0, &tm_ahi, kb * BLOCK_K, m_blk * BLOCK_M, fb);
-          tc::tma_load_2d(s0 + A_TILE_BYTES, &tm_alo, kb * BLOCK_K, m_blk * BLOCK_M, fb);
+          const size_t a_off = a_tile + (size_t)kb * 8 * PIECE_HALVES;
+          tc::bulk_load(s0, g.a_hi + a_off, A_TILE_BYTES, fb);
+          tc::bulk_load(s0 + A_TILE_BYTES, g.a_lo + a_off, A_TILE_BYTES, fb);
           tc::tma_load_2d(s0 + 2 * A_TILE_BYTES, &tm_whi, kb * BLOCK_K, n_blk * BLOCK_N, fb);
           tc::tma_load_2d(s0 + 2 * A_TILE_BYTES + B_TILE_BYTES, &tm_wlo, kb * BLOCK_K, n_blk * BLOCK_N, fb);
           if (++stage == STAGES) { stage = 0; phase ^= 1; }
         }
       }
     }
-  } else if (warp == 9) {
+  } else if (warp == EPI_WARPS + 1) {
     // ===== MMA issuer (one thread): one fresh TMEM partial per k-block =====
     if (lane == 0) {
       uint32_t stage = 0, phase = 0, pcount = 0;
@@ -217,21 +236,23 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) mlp_gemm_tc(const __grid_cons
           tc::fence_after_sync();
           const uint32_t d_tmem = tmem_base + pb * 256;
           const uint32_t s0 = base + stage * STAGE;
-          const uint64_t a_hi = tc::smem_desc_sw128(s0), a_lo = tc::smem_desc_sw128(s0 + A_TILE_BYTES);
+          // A: canonical no-swizzle K-major tile -- 16-byte pieces 2048 bytes apart along K (leading
+          // byte offset), 8-row groups 128 bytes apart along M (stride byte offset); one MMA consumes
+          // two pieces (K = 16).  W: 128-byte-swizzled rows, 32 bytes per MMA.
+          const uint64_t a_hi = tc::smem_desc_nosw(s0, 2048, 128), a_lo = tc::smem_desc_nosw(s0 + A_TILE_BYTES, 2048, 128);
           const uint64_t b_hi = tc::smem_desc_sw128(s0 + 2 * A_TILE_BYTES);
           const uint64_t b_lo = tc::smem_desc_sw128(s0 + 2 * A_TILE_BYTES + B_TILE_BYTES);
-          // UMMA_K = 16 fp16 = 32 bytes: +2 in the descriptor's address field per k step.
           // Corrections first (the accumulator is still ~2^-11 of its final size), hi.hi last.
 #pragma unroll
           for (int k = 0; k < BLOCK_K / 16; ++k) {
-            const uint64_t adv = (uint64_t)(2 * k);
-            tc::mma_f16_ss(d_tmem, a_lo + adv, b_hi + adv, IDESC, k != 0);
-            tc::mma_f16_ss(d_tmem, a_hi + adv, b_lo + adv, IDESC, 1);
+            const uint64_t adv_a = (uint64_t)(256 * k), adv_b = (uint64_t)(2 * k);
+            tc::mma_f16_ss(d_tmem, a_lo + adv_a, b_hi + adv_b, IDESC, k != 0);
+            tc::mma_f16_ss(d_tmem, a_hi + adv_a, b_lo + adv_b, IDESC, 1);
           }
 #pragma unroll
           for (int k = 0; k < BLOCK_K / 16; ++k) {
-            const uint64_t adv = (uint64_t)(2 * k);
-            tc::mma_f16_ss(d_tmem, a_hi + adv, b_hi + adv, IDESC, 1);
+            const uint64_t adv_a = (uint64_t)(256 * k), adv_b = (uint64_t)(2 * k);
+            tc::mma_f16_ss(d_tmem, a_hi + adv_a, b_hi + adv_b, IDESC, 1);
           }
           tc::mma_commit(empty0 + 8 * stage);                   // smem slot free when these MMAs retire
           tc::mma_commit(pfull0 + 8 * pb);                      // partial complete
@@ -240,7 +261,7 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) mlp_gemm_tc(const __grid_cons
       }
     }
   } else {
-    // ===== epilogue warps 0..7: TMEM lanes 32 (warp % 4) .., columns CPT (warp / 4) .. =====
+    // ===== epilogue warps: TMEM lanes 32 (warp % 4) .., columns CPT (warp / 4) .. =====
     const int q = warp & 3, hcol = warp >> 2;
     uint32_t pcount = 0;
     for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
@@ -252,29 +273,33 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) mlp_gemm_tc(const __grid_cons
         tc::fence_after_sync();
         const uint32_t t_src = tmem_base + pb * 256 + ((uint32_t)(q * 32) << 16) + hcol * CPT;
 #pragma unroll
-        for (int c = 0; c < CPT / 16; ++c) {
-          uint32_t r[16];
-          tc::tmem_ld_32x16(t_src + 16 * c, r);
+        for (int c = 0; c < CPT / LDC; ++c) {
+          uint32_t r[LDC];
+          tc::tmem_ld_cols(t_src + LDC * c, r);
           tc::tmem_ld_wait();
           if (kb == 0) {
 #pragma unroll
-            for (int j = 0; j < 16; ++j) acc[16 * c + j] = __uint_as_float(r[j]);
+            for (int j = 0; j < LDC; ++j) acc[LDC * c + j] = __uint_as_float(r[j]);
           } else {
 #pragma unroll
-            for (int j = 0; j < 16; ++j) acc[16 * c + j] += __uint_as_float(r[j]);
+            for (int j = 0; j < LDC; ++j) acc[LDC * c + j] += __uint_as_float(r[j]);
           }
         }
         tc::fence_before_sync();
         __syncwarp();
         if (lane == 0) tc::mbar_arrive(pempty0 + 8 * pb);
       }
-      const int row = m_blk * BLOCK_M + q * 32 + lane;
+      const int r_in = q * 32 + lane;
+      const int row = m_blk * BLOCK_M + r_in;
       const bool row_ok = row < M;
       const int n0 = n_blk * BLOCK_N + hcol * CPT;
+      if (g.dbg & 16) continue;   // timing experiment: no epilogue math / stores
       if (EPI == 0) {
         const float4* p = reinterpret_cast<const float4*>(params) + n0;
-        __half* dh = g.out_hi + (size_t)row * g.ld_out + n0;
-        __half* dl = g.out_lo + (size_t)row * g.ld_out + n0;
+        // canonical layout: piece (n0/8 + c) of this tile, 16 bytes per row: lanes are contiguous
+        const size_t o = (size_t)m_blk * ((size_t)BLOCK_M * g.ld_out) + (size_t)(n0 >> 3) * PIECE_HALVES + (size_t)r_in * 8;
+        __half* dh = g.out_hi + o;
+        __half* dl = g.out_lo + o;
 #pragma unroll
         for (int c = 0; c < CPT / 8; ++c) {
           uint32_t hi[4], lo[4];
@@ -286,30 +311,44 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) mlp_gemm_tc(const __grid_cons
             split2(gated_act16(ta, pa), gated_act16(tb, pb2), hi[j], lo[j]);
           }
           if (row_ok) {
-            reinterpret_cast<uint4*>(dh)[c] = make_uint4(hi[0], hi[1], hi[2], hi[3]);
-            reinterpret_cast<uint4*>(dl)[c] = make_uint4(lo[0], lo[1], lo[2], lo[3]);
+            *reinterpret_cast<uint4*>(dh + (size_t)c * PIECE_HALVES) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
+            *reinterpret_cast<uint4*>(dl + (size_t)c * PIECE_HALVES) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
           }
         }
       } else {
         const float2* p = g.p_out + n0;            // warp-uniform addresses: L1 broadcast
-        float* dst = g.out_f32 + (size_t)row * g.ld_f32 + n0;
-        const bool vec = (g.ld_f32 & 3) == 0;
+        if (g.out_mode == 1) {
+          // [theta][n][z] with z fastest: consecutive rows (lanes) of one theta are contiguous
+          const int rr = row_ok ? row : 0;
+          const int th = rr / g.rows_per_theta, zi = rr - th * g.rows_per_theta;
+          float* dst = g.out_f32 + (size_t)th * ((size_t)g.n_valid * g.rows_per_theta) + zi;
 #pragma unroll
-        for (int c = 0; c < CPT / 4; ++c) {
-          float y[4];
-#pragma unroll
-          for (int j = 0; j < 4; ++j) {
-            const float2 pj = __ldg(p + 4 * c + j);
-            y[j] = fmaf(acc[4 * c + j], pj.x, pj.y);
-            if (g.apply_exp10) y[j] = exp10f(y[j]);
+          for (int j = 0; j < CPT; ++j) {
+            const float2 pj = __ldg(p + j);
+            float y = fmaf(acc[j], pj.x, pj.y);
+            if (g.apply_exp10) y = exp10f(y);
+            if (row_ok && n0 + j < g.n_valid) dst[(size_t)(n0 + j) * g.rows_per_theta] = y;
           }
-          if (row_ok) {
-            if (vec && n0 + 4 * c + 4 <= g.n_valid) {
-              reinterpret_cast<float4*>(dst)[c] = make_float4(y[0], y[1], y[2], y[3]);
-            } else {
+        } else {
+          float* dst = g.out_f32 + (size_t)row * g.ld_f32 + n0;
+          const bool vec = (g.ld_f32 & 3) == 0;
 #pragma unroll
-              for (int j = 0; j < 4; ++j)
-                if (n0 + 4 * c + j < g.n_valid) dst[4 * c + j] = y[j];
+          for (int c = 0; c < CPT / 4; ++c) {
+            float y[4];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+              const float2 pj = __ldg(p + 4 * c + j);
+              y[j] = fmaf(acc[4 * c + j], pj.x, pj.y);
+              if (g.apply_exp10) y[j] = exp10f(y[j]);
+            }
+            if (row_ok) {
+              if (vec && n0 + 4 * c + 4 <= g.n_valid) {
+                reinterpret_cast<float4*>(dst)[c] = make_float4(y[0], y[1], y[2], y[3]);
+              } else {
+#pragma unroll
+                for (int j = 0; j < 4; ++j)
+                  if (n0 + 4 * c + j < g.n_valid) dst[4 * c + j] = y[j];
+              }
             }
           }
         }
@@ -318,7 +357,7 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) mlp_gemm_tc(const __grid_cons
   }
   tc::fence_before_sync();
   __syncthreads();
-  if (warp == 9) tc::tmem_dealloc(tmem_base, 512);
+  if (warp == EPI_WARPS + 1) tc::tmem_dealloc(tmem_base, 512);
 }
 
 }  // namespace
@@ -338,9 +377,8 @@ struct TcLayer {
 
 struct TcState {
   std::vector<TcLayer> layers;               // index = layer 0 .. n_hidden (layer 0 uses p_hidden only)
-  CUtensorMap tm_act[2][2];                  // [buffer][hi, lo]
-  __half* act[2][2] = {};
-  size_t M_max = 0;
+  __half* act[2][2] = {};                    // [buffer][hi, lo] canonical-layout planes
+  size_t M_pad = 0;
 };
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
@@ -384,8 +422,7 @@ int pick_block_n(int n, bool hidden) {
 }
 
 template <int BN, int EPI>
-nsgpu_status launch_gemm(nsgpu_ctx* ctx, const CUtensorMap& ahi, const CUtensorMap& alo, const TcLayer& L,
-                         const GemmArgs& g, cudaStream_t st) {
+nsgpu_status launch_gemm(nsgpu_ctx* ctx, const TcLayer& L, const GemmArgs& g, cudaStream_t st) {
   const int smem = num_stages(BN) * stage_bytes(BN) + 16 * num_stages(BN) + 64 + (EPI == 0 ? 16 * g.N_pad : 0) + 1024;
   static bool configured = false;
   if (!configured) {
@@ -394,19 +431,18 @@ nsgpu_status launch_gemm(nsgpu_ctx* ctx, const CUtensorMap& ahi, const CUtensorM
   }
   const int tiles = ((g.M_host + BLOCK_M - 1) / BLOCK_M) * (g.N_pad / BN);
   const int grid = std::min(tiles, ctx->sm_count);
-  mlp_gemm_tc<BN, EPI><<<grid, GEMM_THREADS, smem, st>>>(ahi, alo, L.tm_whi, L.tm_wlo, g);
+  mlp_gemm_tc<BN, EPI><<<grid, GEMM_THREADS, smem, st>>>(L.tm_whi, L.tm_wlo, g);
   NSGPU_LAUNCH_CHECK();
   return NSGPU_OK;
 }
 
 template <int EPI>
-nsgpu_status dispatch_gemm(nsgpu_ctx* ctx, const CUtensorMap& ahi, const CUtensorMap& alo, const TcLayer& L,
-                           const GemmArgs& g, cudaStream_t st) {
+nsgpu_status dispatch_gemm(nsgpu_ctx* ctx, const TcLayer& L, const GemmArgs& g, cudaStream_t st) {
   switch (L.block_n) {
-    case 256: return launch_gemm<256, EPI>(ctx, ahi, alo, L, g, st);
-    case 224: return launch_gemm<224, EPI>(ctx, ahi, alo, L, g, st);
-    case 128: return launch_gemm<128, EPI>(ctx, ahi, alo, L, g, st);
-    default: return launch_gemm<64, EPI>(ctx, ahi, alo, L, g, st);
+    case 256: return launch_gemm<256, EPI>(ctx, L, g, st);
+    case 224: return launch_gemm<224, EPI>(ctx, L, g, st);
+    case 128: return launch_gemm<128, EPI>(ctx, L, g, st);
+    default: return launch_gemm<64, EPI>(ctx, L, g, st);
   }
 }
 
@@ -419,7 +455,8 @@ nsgpu_status mlp_tc_prepare(nsgpu_ctx* ctx, int e, const nsgpu_emulator* h) {
   E.tmaps = T;
   const int width = h->width, nh = h->n_hidden;
   const size_t M_max = (size_t)ctx->max_batch * ctx->rows_per_theta;
-  T->M_max = M_max;
+  const size_t M_pad = (M_max + BLOCK_M - 1) / BLOCK_M * BLOCK_M;       // api.cu sizes ctx->act for this
+  T->M_pad = M_pad;
   T->layers.resize(nh + 1);
   const float log2e = 1.4426950408889634f;
   for (int l = 0; l <= nh; ++l) {
@@ -473,12 +510,9 @@ nsgpu_status mlp_tc_prepare(nsgpu_ctx* ctx, int e, const nsgpu_emulator* h) {
   }
   for (int i = 0; i < 2; ++i) {
     T->act[i][0] = reinterpret_cast<__half*>(ctx->act[i]);
-    T->act[i][1] = T->act[i][0] + M_max * width;
-    for (int pl = 0; pl < 2; ++pl)
-      if (!make_tmap(&T->tm_act[i][pl], T->act[i][pl], M_max, width, BLOCK_M)) {
-        ctx->err = "cuTensorMapEncodeTiled failed for an activation plane";
-        return NSGPU_ECUDA;
-      }
+    T->act[i][1] = T->act[i][0] + M_pad * width;
+    // rows past the live ones are read by the last tile of a batch (results discarded): keep them finite
+    NSGPU_CUDA(cudaMemset(ctx->act[i], 0, M_pad * width * 2 * sizeof(__half)));
   }
   return NSGPU_OK;
 }
@@ -492,7 +526,7 @@ void mlp_tc_release(nsgpu_ctx* ctx, int e) {
 }
 
 nsgpu_status mlp_forward_tc(nsgpu_ctx* ctx, int e, const float* theta, int B, const int* n_rows_dev, float* spec_out,
-                            bool apply_exp10, cudaStream_t st) {
+                            int mode, cudaStream_t st) {
   const EmuDev& E = ctx->emu[e];
   TcState* T = reinterpret_cast<TcState*>(E.tmaps);
   const int rpt = ctx->rows_per_theta;
@@ -501,10 +535,12 @@ nsgpu_status mlp_forward_tc(nsgpu_ctx* ctx, int e, const float* theta, int B, co
   int cur = 0;
   {
     StageTimer tm(ctx, 0, st);
-    mlp_first_layer_tc<<<(M + FL_ROWS - 1) / FL_ROWS, 256, 0, st>>>(theta, ctx->D, rpt, M, n_rows_dev, ctx->emu_in_idx,
-                                                                   ctx->emu_in_const, ctx->n_theta_in, ctx->z_emu, E.n_in,
-                                                                   E.in_mean, E.in_std, E.W[0], T->layers[0].p_hidden,
-                                                                   E.width, T->act[0][0], T->act[0][1]);
+    const size_t smem = (size_t)E.width * sizeof(float4) + (size_t)E.n_in * E.width * sizeof(float);
+    mlp_first_layer_tc<<<(M + BLOCK_M - 1) / BLOCK_M, 256, smem, st>>>(theta, ctx->D, rpt, M, n_rows_dev, ctx->emu_in_idx,
+                                                                      ctx->emu_in_const, ctx->n_theta_in, ctx->z_emu,
+                                                                      E.n_in, E.in_mean, E.in_std, E.W[0],
+                                                                      T->layers[0].p_hidden, E.width, T->act[0][0],
+                                                                      T->act[0][1]);
     NSGPU_LAUNCH_CHECK();
   }
   for (int l = 1; l <= E.n_hidden; ++l) {
@@ -514,11 +550,13 @@ nsgpu_status mlp_forward_tc(nsgpu_ctx* ctx, int e, const float* theta, int B, co
     memset(&g, 0, sizeof(g));
     g.M_host = M; g.n_rows_dev = n_rows_dev; g.rows_per_theta = rpt; g.K = L.K; g.N_pad = L.N_pad; g.n_valid = L.n_valid;
     g.p_hidden = L.p_hidden; g.p_out = L.p_out; g.cscale = ldexpf(1.0f, -(L.wexp + 4)) * TRUNC_COMP;
+    g.a_hi = T->act[cur][0]; g.a_lo = T->act[cur][1];
     g.out_hi = T->act[cur ^ 1][0]; g.out_lo = T->act[cur ^ 1][1]; g.ld_out = E.width;
-    g.out_f32 = spec_out; g.ld_f32 = E.n_out; g.apply_exp10 = apply_exp10 ? 1 : 0;
+    g.out_f32 = spec_out; g.ld_f32 = E.n_out; g.apply_exp10 = (mode & NSGPU_SPEC_EXP10) ? 1 : 0;
+    g.out_mode = (mode & NSGPU_SPEC_KZ) ? 1 : 0;
+    { const char* dbg = getenv("NSGPU_TC_DBG"); g.dbg = dbg ? atoi(dbg) : 0; }
     StageTimer tm(ctx, hidden ? 1 : 2, st);
-    nsgpu_status s = hidden ? dispatch_gemm<0>(ctx, T->tm_act[cur][0], T->tm_act[cur][1], L, g, st)
-                            : dispatch_gemm<1>(ctx, T->tm_act[cur][0], T->tm_act[cur][1], L, g, st);
+    nsgpu_status s = hidden ? dispatch_gemm<0>(ctx, L, g, st) : dispatch_gemm<1>(ctx, L, g, st);
     if (s != NSGPU_OK) return s;
     cur ^= 1;
   }

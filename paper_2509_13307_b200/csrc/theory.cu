@@ -24,81 +24,103 @@ __device__ __forceinline__ double warp_sum(double v) {
   return v;
 }
 
-// In-place exclusive prefix sum of arr[0..n) (or suffix sum when `reverse`) by the whole block.
-// wsum: shared scratch of 33 doubles.
-__device__ void block_scan_exclusive(double* arr, int n, bool reverse, double* wsum) {
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
-  double carry = 0.0;
-  for (int base = 0; base < n; base += blockDim.x) {
-    int i = base + threadIdx.x;
-    int idx = reverse ? n - 1 - i : i;
-    double v = (i < n) ? arr[idx] : 0.0;
-    double inc = v;
+// exp(x) in fp64 for |x| < 700: n = rint(x log2 e), r = x - n ln 2 (two-constant reduction), degree-11
+// Taylor polynomial on |r| <= 0.347 (truncation 0.347^12/12! = 6e-15), scaled by 2^n through the exponent
+// field.  A third of the instructions of the library routine; the projection spends most of its
+// arithmetic in 2^y and Gaussian evaluations.
+__device__ __forceinline__ double exp_fast(double x) {
+  if (x < -700.0) return 0.0;
+  const double n = rint(x * 1.4426950408889634);
+  double r = fma(n, -6.93147180369123816490e-01, x);
+  r = fma(n, -1.90821492927058770002e-10, r);
+  double p = 2.505210838544172e-08;           // 1/11!
+  p = fma(p, r, 2.755731922398589e-07);       // 1/10!
+  p = fma(p, r, 2.7557319223985893e-06);      // 1/9!
+  p = fma(p, r, 2.48015873015873e-05);        // 1/8!
+  p = fma(p, r, 1.984126984126984e-04);       // 1/7!
+  p = fma(p, r, 1.3888888888888889e-03);      // 1/6!
+  p = fma(p, r, 8.333333333333333e-03);       // 1/5!
+  p = fma(p, r, 4.1666666666666664e-02);      // 1/4!
+  p = fma(p, r, 1.6666666666666666e-01);      // 1/3!
+  p = fma(p, r, 0.5);
+  p = fma(p, r, 1.0);
+  p = fma(p, r, 1.0);
+  const int e = (int)n;
+  return __hiloint2double(__double2hiint(p) + (e << 20), __double2loint(p));
+}
+
+// Exclusive prefix (or suffix, when `reverse`) sum of arr[0..n) in place by ONE warp: each lane sums a
+// contiguous chunk, a shuffle scan carries across lanes.  No block-level synchronisation inside.
+__device__ void warp_scan_exclusive(double* arr, int n, bool reverse, int lane) {
+  const int per = (n + 31) >> 5;
+  const int b0 = lane * per, b1 = min(b0 + per, n);
+  double local = 0.0;
+  for (int i = b0; i < b1; ++i) local += arr[reverse ? n - 1 - i : i];
+  double inc = local;
 #pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-      double t = __shfl_up_sync(0xffffffffu, inc, o);
-      if (lane >= o) inc += t;
-    }
-    if (lane == 31) wsum[warp] = inc;
-    __syncthreads();
-    if (warp == 0) {
-      double w = (lane < nwarp) ? wsum[lane] : 0.0;
-      double winc = w;
-#pragma unroll
-      for (int o = 1; o < 32; o <<= 1) {
-        double t = __shfl_up_sync(0xffffffffu, winc, o);
-        if (lane >= o) winc += t;
-      }
-      if (lane < nwarp) wsum[lane] = winc - w;      // exclusive warp offsets
-      if (lane == nwarp - 1) wsum[32] = winc;       // chunk total
-    }
-    __syncthreads();
-    if (i < n) arr[idx] = carry + wsum[warp] + inc - v;
-    carry += wsum[32];
-    __syncthreads();
+  for (int o = 1; o < 32; o <<= 1) {
+    const double t = __shfl_up_sync(0xffffffffu, inc, o);
+    if (lane >= o) inc += t;
+  }
+  double run = inc - local;
+  for (int i = b0; i < b1; ++i) {
+    const int idx = reverse ? n - 1 - i : i;
+    const double v = arr[idx];
+    arr[idx] = run;
+    run += v;
   }
 }
 
 struct ShearArgs {
   int n_z_emu, n_chi, n_k, n_ell, n_tomo, n_tap;
+  int sz, sk;   // table strides: element (z node m, k node j) at m sz + j sk
   double k_min, k_max, lk0, dlk, da, nz_sigma;
-  const double *a_q, *z_q, *tap_w, *ell, *nz_mean;
+  const double *a_q, *z_q, *ln1pz, *tap_w, *ell, *lellh, *lf, *nz_mean;
   const int* tap_start;
   int idx_omega_b, idx_omega_cdm, idx_h, idx_w0, idx_wa, idx_eta0, idx_dz, idx_ia, idx_m;
 };
 
-__global__ void __launch_bounds__(256) shear_project_kernel(const float* __restrict__ theta, int D,
-                                                            const int* __restrict__ n_rows_dev,
-                                                            const float* __restrict__ spec, ShearArgs A,
-                                                            double* __restrict__ model, int n_data) {
+// One CTA per theta.  Thread 0 starts a bulk asynchronous copy (TMA, cp.async.bulk) of this theta's
+// log10 P table into shared memory -- the kernel's only large HBM read -- and the CTA computes the
+// background and the windows (which do not need the table) while it lands.
+constexpr int SHEAR_THREADS = 256;
+__global__ void __launch_bounds__(SHEAR_THREADS, 2) shear_project_kernel(const float* __restrict__ theta, int D,
+                                                                         const int* __restrict__ n_rows_dev,
+                                                                         const float* __restrict__ spec, ShearArgs A,
+                                                                         double* __restrict__ model, int n_data) {
   const int b = blockIdx.x;
   if (n_rows_dev && b >= *n_rows_dev) return;
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  const int nq = A.n_chi, nt = A.n_tomo;
+  const int nq = A.n_chi, nt = A.n_tomo, nqp = nq | 1;
+  const int n_scr = max(2 * nt, A.n_ell);
   double* chi = reinterpret_cast<double*>(smem_raw);   // [nq]
   double* Eq = chi + nq;                               // [nq]
   double* Dq = Eq + nq;                                // [nq]
   double* gq = Dq + nq;                                // [nq]   dchi / chi^2
-  double* s0 = gq + nq;                                // [nq]   scratch (suffix sum A)
-  double* s1 = s0 + nq;                                // [nq]   scratch (suffix sum B)
-  double* Wt = s1 + nq;                                // [nt][nq] total window
-  double* Pg = Wt + (size_t)nt * nq;                   // [n_ell][nq]
-  double* wsum = Pg + (size_t)A.n_ell * nq;            // [33]
-  const size_t n_dbl = ((size_t)nq * (6 + nt + A.n_ell) + 34 + 1) & ~(size_t)1;   // keep the table 16-byte aligned
-  float* table = reinterpret_cast<float*>(chi + n_dbl);  // [n_z_emu][n_k]
+  double* hs = gq + nq;                                // [nq]   half-cell terms, then log10 chi
+  double* Wt = hs + nq;                                // [nt][nq] total window
+  double* scr = Wt + (size_t)nt * nq;                  // [n_scr][nqp]: scan arrays, then Pg[n_ell][nqp]
+  size_t n_dbl = (size_t)nq * (5 + nt) + (size_t)n_scr * nqp + 2;
+  n_dbl = (n_dbl + 1) & ~(size_t)1;
+  unsigned long long* bar = reinterpret_cast<unsigned long long*>(chi + n_dbl - 2);   // 8-byte mbarrier
+  float* table = reinterpret_cast<float*>(chi + n_dbl);   // [n_z_emu][n_k], 16-byte aligned
 
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarp = blockDim.x >> 5;
   const float* th = theta + (size_t)b * D;
-  // stage this theta's log10 P table (the kernel's only large HBM read)
-  {
-    const float* src = spec + (size_t)b * A.n_z_emu * A.n_k;
-    const int n = A.n_z_emu * A.n_k;
-    if ((n & 3) == 0 && ((reinterpret_cast<uintptr_t>(src) & 15) == 0)) {
-      const float4* s4 = reinterpret_cast<const float4*>(src);
-      float4* d4 = reinterpret_cast<float4*>(table);
-      for (int i = threadIdx.x; i < n / 4; i += blockDim.x) d4[i] = __ldg(s4 + i);
-    } else {
-      for (int i = threadIdx.x; i < n; i += blockDim.x) table[i] = __ldg(src + i);
+  const float* src = spec + (size_t)b * A.n_z_emu * A.n_k;
+  const unsigned table_bytes = (unsigned)(A.n_z_emu * A.n_k) * 4u;
+  const bool bulk = (table_bytes & 15u) == 0 && ((reinterpret_cast<uintptr_t>(src) & 15) == 0);
+  const unsigned bar_s = (unsigned)__cvta_generic_to_shared(bar);
+  if (bulk) {
+    if (tid == 0) {
+      asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar_s) : "memory");
+      asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+      asm volatile("{\n.reg .b64 st;\nmbarrier.arrive.expect_tx.shared::cta.b64 st, [%0], %1;\n}" ::"r"(bar_s), "r"(table_bytes) : "memory");
+      asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                   ::"r"((unsigned)__cvta_generic_to_shared(table)), "l"(src), "r"(table_bytes), "r"(bar_s) : "memory");
     }
+  } else {
+    for (int i = tid; i < A.n_z_emu * A.n_k; i += blockDim.x) table[i] = __ldg(src + i);
   }
   const double ob = th[A.idx_omega_b], oc = th[A.idx_omega_cdm], h = th[A.idx_h];
   const double Om = (ob + oc) / (h * h);
@@ -106,105 +128,122 @@ __global__ void __launch_bounds__(256) shear_project_kernel(const float* __restr
   const double wa = A.idx_wa >= 0 ? (double)th[A.idx_wa] : 0.0;
   const double eta0 = A.idx_eta0 >= 0 ? (double)th[A.idx_eta0] : 0.7;
   const double gam = 0.55 + 0.05 * (1.0 + w0 + 0.5 * wa);
+  const double de_exp = 3.0 * (1.0 + w0 + wa);
 
-  // a6: E_q, f_q da -> chi (exclusive scan + half cell), growth exponent -> ln D
-  for (int q = threadIdx.x; q < nq; q += blockDim.x) {
-    const double a = A.a_q[q], z = A.z_q[q];
-    const double E2 = Om * (1.0 + z) * (1.0 + z) * (1.0 + z) +
-                      (1.0 - Om) * pow(1.0 + z, 3.0 * (1.0 + w0 + wa)) * exp(-3.0 * wa * z / (1.0 + z));
+  // a6: E_q; f_q da and the growth integrand go to the scan arrays
+  double* sc_f = scr;
+  double* sc_g = scr + nqp;
+  for (int q = tid; q < nq; q += blockDim.x) {
+    const double a = A.a_q[q], z = A.z_q[q], opz = 1.0 + z;
+    const double E2 = Om * opz * opz * opz + (1.0 - Om) * exp_fast(de_exp * A.ln1pz[q] - 3.0 * wa * z / opz);
     const double E = sqrt(E2);
     Eq[q] = E;
-    const double f = 1.0 / (a * a * E);
-    gq[q] = f * A.da;                                         // f_q da
+    const double fda = A.da / (a * a * E);
     const double Om_a = Om / (a * a * a) / E2;
-    s1[q] = pow(Om_a, gam) * A.da / a;                        // growth integrand
-    chi[q] = gq[q];
-    Dq[q] = s1[q];
+    const double gi = exp_fast(gam * log(Om_a)) * A.da / a;
+    gq[q] = fda;
+    hs[q] = gi;
+    sc_f[q] = fda;
+    sc_g[q] = gi;
   }
   __syncthreads();
-  block_scan_exclusive(chi, nq, false, wsum);
-  block_scan_exclusive(Dq, nq, false, wsum);
-  for (int q = threadIdx.x; q < nq; q += blockDim.x) {
-    const double c = C_OVER_H0 * (chi[q] + 0.5 * gq[q]);
+  if (warp == 0) warp_scan_exclusive(sc_f, nq, false, lane);
+  else if (warp == 1) warp_scan_exclusive(sc_g, nq, false, lane);
+  __syncthreads();
+  for (int q = tid; q < nq; q += blockDim.x) {
+    const double c = C_OVER_H0 * (sc_f[q] + 0.5 * gq[q]);
     chi[q] = c;
-    Dq[q] = exp(-(Dq[q] + 0.5 * s1[q]));
+    Dq[q] = exp_fast(-(sc_g[q] + 0.5 * hs[q]));
     gq[q] = C_OVER_H0 * gq[q] / (c * c);                      // dchi_q / chi_q^2
   }
   __syncthreads();
 
-  // a7: per tomographic bin, n_i(z - dz_i), W^gamma by two suffix sums (A - chi B), W^I, total
+  // a7: n_i(z - dz_i); W^I; the two suffix sums of W^gamma = A - chi B for all bins at once
   const double norm = 1.0 / (A.nz_sigma * 2.5066282746310002);   // 1/(sigma sqrt(2 pi))
-  for (int i = 0; i < nt; ++i) {
+  for (int it = tid; it < nt * nq; it += blockDim.x) {
+    const int i = it / nq, q = it - i * nq;
     const double mu = A.nz_mean[i] + (double)th[A.idx_dz + i];
     const double A0 = th[A.idx_ia + 3 * i], A1 = th[A.idx_ia + 3 * i + 1], A2 = th[A.idx_ia + 3 * i + 2];
-    for (int q = threadIdx.x; q < nq; q += blockDim.x) {
-      const double z = A.z_q[q], a = A.a_q[q];
-      const double u = (z - mu) / A.nz_sigma;
-      const double nz = exp(-0.5 * u * u) * norm;
-      const double w = nz * A.da / (a * a);                   // n_i(z_q) dz_q
-      s0[q] = w;
-      s1[q] = w / chi[q];
-      const double x = (1.0 + z) / 1.62 - 1.0;
-      const double Aia = A0 + A1 * x + A2 * x * x;
-      Wt[(size_t)i * nq + q] = -Aia * C1_RHOCR * Om / Dq[q] * nz * Eq[q] / C_OVER_H0;   // W^I (eq. A4)
-    }
-    __syncthreads();
-    block_scan_exclusive(s0, nq, true, wsum);
-    block_scan_exclusive(s1, nq, true, wsum);
-    for (int q = threadIdx.x; q < nq; q += blockDim.x) {
-      const double wg = 1.5 * Om / (C_OVER_H0 * C_OVER_H0) * (1.0 + A.z_q[q]) * chi[q] * (s0[q] - chi[q] * s1[q]);
-      Wt[(size_t)i * nq + q] += wg;                           // + W^gamma (eq. A3)
-    }
-    __syncthreads();
+    const double z = A.z_q[q], a = A.a_q[q];
+    const double u = (z - mu) / A.nz_sigma;
+    const double nz = exp_fast(-0.5 * u * u) * norm;
+    const double w = nz * A.da / (a * a);                     // n_i(z_q) dz_q
+    scr[(size_t)(2 * i) * nqp + q] = w;
+    scr[(size_t)(2 * i + 1) * nqp + q] = w / chi[q];
+    const double x = (1.0 + z) / 1.62 - 1.0;
+    const double Aia = A0 + A1 * x + A2 * x * x;
+    Wt[(size_t)i * nq + q] = -Aia * C1_RHOCR * Om / Dq[q] * nz * Eq[q] / C_OVER_H0;   // W^I (eq. A4)
+  }
+  __syncthreads();
+  for (int c = warp; c < 2 * nt; c += nwarp) warp_scan_exclusive(scr + (size_t)c * nqp, nq, true, lane);
+  __syncthreads();
+  for (int it = tid; it < nt * nq; it += blockDim.x) {
+    const int i = it / nq, q = it - i * nq;
+    const double s0 = scr[(size_t)(2 * i) * nqp + q], s1 = scr[(size_t)(2 * i + 1) * nqp + q];
+    const double wg = 1.5 * Om / (C_OVER_H0 * C_OVER_H0) * (1.0 + A.z_q[q]) * chi[q] * (s0 - chi[q] * s1);
+    Wt[(size_t)i * nq + q] += wg;                             // + W^gamma (eq. A3)
+    if (i == 0) hs[q] = log10(chi[q]);
+  }
+  __syncthreads();
+  if (bulk) {   // the table has landed?
+    unsigned ok = 0;
+    while (!ok)
+      asm volatile("{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], 0;\nselp.u32 %0, 1, 0, p;\n}"
+                   : "=r"(ok) : "r"(bar_s) : "memory");
   }
 
-  // a5 + a8 (lookup): P(k = (ell+1/2)/chi_q, z_q) g_q for every (ell, q)
+  // a5 + a8 (lookup): P(k = (ell+1/2)/chi_q, z_q) g_q for every (ell, q); log10 k = log10(ell+1/2) - log10 chi
+  double* Pg = scr;                                           // [n_ell][nqp]
   const int n_lookup = A.n_ell * nq;
-  for (int it = threadIdx.x; it < n_lookup; it += blockDim.x) {
+  const double inv_dlk = 1.0 / A.dlk, bar_amp = (eta0 - 0.7) * 0.1;
+  for (int it = tid; it < n_lookup; it += blockDim.x) {
     const int bl = it / nq, q = it - bl * nq;
     const double k = (A.ell[bl] + 0.5) / chi[q];
     double P = 0.0;
     if (k >= A.k_min && k <= A.k_max) {
-      const double x = log10(k);
-      int j = (int)floor((x - A.lk0) / A.dlk);
+      const double x = A.lellh[bl] - hs[q];
+      int j = (int)floor((x - A.lk0) * inv_dlk);
       j = min(max(j, 0), A.n_k - 2);
-      const double s = (x - (A.lk0 + j * A.dlk)) / A.dlk;
+      const double s = (x - (A.lk0 + j * A.dlk)) * inv_dlk;
       const int m0 = A.tap_start[q];
       const double* tw = A.tap_w + (size_t)q * A.n_tap;
       double lo = 0.0, hi = 0.0;
       for (int t = 0; t < A.n_tap; ++t) {
-        const float* row = table + (size_t)(m0 + t) * A.n_k + j;
-        lo += tw[t] * (double)row[0];
-        hi += tw[t] * (double)row[1];
+        const float* row = table + (size_t)(m0 + t) * A.sz + (size_t)j * A.sk;
+        const double w = tw[t];
+        lo = fma(w, (double)row[0], lo);
+        hi = fma(w, (double)row[A.sk], hi);
       }
       double y = (1.0 - s) * lo + s * hi;
-      y -= (eta0 - 0.7) * 0.1 * k * k / (k * k + 1.0);
-      P = exp10(y);
+      y -= bar_amp * k * k / (k * k + 1.0);
+      P = exp_fast(y * 2.302585092994046);
     }
-    Pg[it] = P * gq[q];
+    Pg[(size_t)bl * nqp + q] = P * gq[q];
   }
   __syncthreads();
 
-  // a8 (sum): C_ij(ell) = sum_q Wt_i Wt_j Pg; one warp per output, lanes stride q, shuffle reduce
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
+  // a8 (sum): C_ij(ell) = sum_q Wt_i Wt_j Pg; one thread per output, q serial (operands broadcast or
+  // conflict-free from shared memory: consecutive threads differ in ell, Pg rows have odd stride)
   const int n_pairs = nt * (nt + 1) / 2;
-  for (int o = warp; o < n_pairs * A.n_ell; o += nwarp) {
+  for (int o = tid; o < n_pairs * A.n_ell; o += blockDim.x) {
     const int p = o / A.n_ell, bl = o - p * A.n_ell;
     int i = 0, rem = p;                                        // pair p -> (i <= j), row-major upper
     while (rem >= nt - i) { rem -= nt - i; ++i; }
     const int j = i + rem;
     const double* wi = Wt + (size_t)i * nq;
     const double* wj = Wt + (size_t)j * nq;
-    const double* pg = Pg + (size_t)bl * nq;
-    double acc = 0.0;
-    for (int q = lane; q < nq; q += 32) acc += wi[q] * wj[q] * pg[q];
-    acc = warp_sum(acc);
-    if (lane == 0) {
-      const double lf = log(A.ell[bl] / 550.0) / 3.4011973816621555;   // ln(ell/550)/ln 30
-      const double mi = (double)th[A.idx_m + 2 * i] + (double)th[A.idx_m + 2 * i + 1] * lf;
-      const double mj = (double)th[A.idx_m + 2 * j] + (double)th[A.idx_m + 2 * j + 1] * lf;
-      model[(size_t)b * n_data + o] = (1.0 + mi) * (1.0 + mj) * acc;
+    const double* pg = Pg + (size_t)bl * nqp;
+    double acc0 = 0.0, acc1 = 0.0;
+    int q = 0;
+    for (; q + 1 < nq; q += 2) {
+      acc0 = fma(wi[q] * wj[q], pg[q], acc0);
+      acc1 = fma(wi[q + 1] * wj[q + 1], pg[q + 1], acc1);
     }
+    if (q < nq) acc0 = fma(wi[q] * wj[q], pg[q], acc0);
+    const double lf = A.lf[bl];                                // ln(ell/550)/ln 30
+    const double mi = (double)th[A.idx_m + 2 * i] + (double)th[A.idx_m + 2 * i + 1] * lf;
+    const double mj = (double)th[A.idx_m + 2 * j] + (double)th[A.idx_m + 2 * j + 1] * lf;
+    model[(size_t)b * n_data + o] = (1.0 + mi) * (1.0 + mj) * (acc0 + acc1);
   }
 }
 
@@ -254,7 +293,9 @@ __global__ void copy_model_kernel(const float* __restrict__ src, int n, int B, c
 }  // namespace
 
 static size_t shear_smem_bytes(const ShearDev& S) {
-  size_t d = ((size_t)S.n_chi * (6 + S.n_tomo + S.n_ell) + 34 + 1) & ~(size_t)1;
+  const size_t nqp = (size_t)S.n_chi | 1, n_scr = (size_t)std::max(2 * S.n_tomo, S.n_ell);
+  size_t d = (size_t)S.n_chi * (5 + S.n_tomo) + n_scr * nqp + 2;
+  d = (d + 1) & ~(size_t)1;
   return d * sizeof(double) + (size_t)S.n_z_emu * S.n_k * sizeof(float) + 16;
 }
 
@@ -263,8 +304,10 @@ nsgpu_status shear_project(nsgpu_ctx* ctx, const float* theta, int B, const int*
   const ShearDev& S = ctx->sh;
   ShearArgs A;
   A.n_z_emu = S.n_z_emu; A.n_chi = S.n_chi; A.n_k = S.n_k; A.n_ell = S.n_ell; A.n_tomo = S.n_tomo; A.n_tap = S.n_tap;
+  A.sz = ctx->spec_kz ? 1 : S.n_k; A.sk = ctx->spec_kz ? S.n_z_emu : 1;
   A.k_min = S.k_min; A.k_max = S.k_max; A.lk0 = S.lk0; A.dlk = S.dlk; A.da = S.da; A.nz_sigma = S.nz_sigma;
-  A.a_q = S.a_q; A.z_q = S.z_q; A.tap_w = S.tap_w; A.ell = S.ell; A.nz_mean = S.nz_mean; A.tap_start = S.tap_start;
+  A.a_q = S.a_q; A.z_q = S.z_q; A.ln1pz = S.ln1pz; A.tap_w = S.tap_w; A.ell = S.ell; A.lellh = S.lellh; A.lf = S.lf;
+  A.nz_mean = S.nz_mean; A.tap_start = S.tap_start;
   A.idx_omega_b = S.idx_omega_b; A.idx_omega_cdm = S.idx_omega_cdm; A.idx_h = S.idx_h; A.idx_w0 = S.idx_w0;
   A.idx_wa = S.idx_wa; A.idx_eta0 = S.idx_eta0; A.idx_dz = S.idx_dz; A.idx_ia = S.idx_ia; A.idx_m = S.idx_m;
   const size_t smem = shear_smem_bytes(S);
@@ -274,7 +317,7 @@ nsgpu_status shear_project(nsgpu_ctx* ctx, const float* theta, int B, const int*
     configured = smem;
   }
   StageTimer tm(ctx, 3, st);
-  shear_project_kernel<<<B, 256, smem, st>>>(theta, ctx->D, n_rows_dev, ctx->spec, A, ctx->model, ctx->n_data);
+  shear_project_kernel<<<B, SHEAR_THREADS, smem, st>>>(theta, ctx->D, n_rows_dev, ctx->spec, A, ctx->model, ctx->n_data);
   NSGPU_LAUNCH_CHECK();
   return NSGPU_OK;
 }
