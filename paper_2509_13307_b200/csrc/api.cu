@@ -287,10 +287,10 @@ nsgpu_status create_impl(nsgpu_ctx* ctx, int32_t D, const nsgpu_prior1d* prior, 
     }
     // stored transposed: LinvT[j][i] = Linv[i][j] (non-zero for i >= j), so that for a fixed column j the
     // rows i are contiguous -- coalesced for the row-per-thread chi^2 kernel
-    std::vector<double> LinvT(n * n, 0.0);
+    std::vector<double> LinvT(n * n + 2, 0.0);   // + padding: the chi^2 kernel copies whole 16-byte units
     for (size_t i = 0; i < n; ++i)
       for (size_t j = 0; j <= i; ++j) LinvT[j * n + i] = Linv[i * n + j];
-    NSGPU_CUDA(upload(&ctx->Linv, LinvT.data(), n * n));
+    NSGPU_CUDA(upload(&ctx->Linv, LinvT.data(), n * n + 2));
     NSGPU_CUDA(upload(&ctx->data, data, n));
   }
 

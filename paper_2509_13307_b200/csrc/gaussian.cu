@@ -8,28 +8,45 @@
 // Residuals, products and the sum of squares are fp64 (reading P1): n(n+1)/2 MAC per theta is three
 // orders of magnitude below the emulator's work, and an fp32 whitening would eat the 1e-3 budget.
 #include "internal.cuh"
+#include "tc_ptx.cuh"
 
 namespace {
 
-constexpr int TB = 8;    // thetas per CTA: every inverse-factor element loaded from L2 is used TB times
 
-// w = Linv r for TB thetas at once, one thread per PAIR of rows (t, n-1-t): the pair has n+1 non-zero
-// columns whatever t is, so the triangular work is balanced across threads.  For a fixed column j the
-// threads read LinvT[j][t] and LinvT[j][n-1-t] (coalesced) and the TB residuals r[j][.] (one broadcast
-// shared-memory line).  fp64 throughout; chi^2 = sum over rows of w^2 by a block reduction.
-__global__ void __launch_bounds__(512) chi2_kernel(const double* __restrict__ model, const double* __restrict__ data,
-                                                    const double* __restrict__ LinvT, int n, int B,
-                                                    const int* __restrict__ n_rows_dev, const float* __restrict__ theta,
-                                                    int D, const int* __restrict__ prior_kind,
-                                                    const double* __restrict__ p0, const double* __restrict__ p1,
-                                                    double log_norm, double* __restrict__ logL) {
+// w = Linv r for TB thetas at once.  A thread owns a PAIR of rows (t, n-1-t) -- n+1 non-zero columns
+// whatever t is, so the triangular work is balanced -- and TG of the CTA's TB thetas.  The factor is
+// streamed through shared memory in chunks of CH columns (LinvT rows, contiguous in memory) by bulk
+// asynchronous copies, double buffered: thread 0 starts chunk c+1 while the CTA multiplies chunk c.
+// The column index is uniform across a warp, so the residuals r[j][.] are one broadcast line of
+// shared memory (a per-lane column made every load a 26-way bank conflict) and the factor elements
+// S[j][row] are conflict-free; LinvT is stored as a full matrix whose upper part is zero, so lanes for
+// which column j lies above their row just add 0.  fp64 throughout; chi^2 = sum over rows of w^2.
+template <int TB, int TG, int MAXT>
+__global__ void __launch_bounds__(MAXT) chi2_kernel(const double* __restrict__ model, const double* __restrict__ data,
+                                                     const double* __restrict__ LinvT, int n, int B, int RT, int CH,
+                                                     const int* __restrict__ n_rows_dev, const float* __restrict__ theta,
+                                                     int D, const int* __restrict__ prior_kind,
+                                                     const double* __restrict__ p0, const double* __restrict__ p1,
+                                                     double log_norm, double* __restrict__ logL) {
   if (n_rows_dev) B = min(B, *n_rows_dev);
   const int b0 = blockIdx.x * TB;
   if (b0 >= B) return;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   double* r = reinterpret_cast<double*>(smem_raw);       // [n][TB]
   double* part = r + (size_t)n * TB;                     // [32][TB] per-warp partial chi^2
+  unsigned long long* bars = reinterpret_cast<unsigned long long*>(part + 32 * TB);   // full[2], empty[2]
+  double* S = reinterpret_cast<double*>(bars + 4);       // [2][CH][n], 16-byte aligned (n TB even)
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarp = blockDim.x >> 5;
+  const uint32_t full0 = tc::smem_u32(bars), empty0 = full0 + 16;
+  const int n_chunks = (n + CH - 1) / CH;
+  if (tid == 0) {
+    tc::mbar_init(full0, 1); tc::mbar_init(full0 + 8, 1);
+    tc::mbar_init(empty0, nwarp); tc::mbar_init(empty0 + 8, nwarp);
+    tc::fence_barrier_init();
+    const uint32_t bytes = ((uint32_t)min(CH, n) * n * 8u + 15u) & ~15u;   // LinvT has 2 doubles of padding
+    tc::mbar_arrive_expect_tx(full0, bytes);
+    tc::bulk_load(tc::smem_u32(S), LinvT, bytes, full0);
+  }
   // residuals, transposed into [j][theta] (coalesced global reads along j)
   for (int i = tid; i < n * TB; i += blockDim.x) {
     const int t = i / n, j = i - t * n;
@@ -38,46 +55,62 @@ __global__ void __launch_bounds__(512) chi2_kernel(const double* __restrict__ mo
   }
   __syncthreads();
   const int half = (n + 1) >> 1;
-  const int ra = tid, rb = n - 1 - tid;                  // rows of this thread (ra <= rb); ra == rb for the middle row
-  double wa[TB], wb[TB];
+  const int rt = tid % RT, grp = tid / RT;               // RT is a multiple of 32: a warp has one group
+  const int ra = rt, rb = n - 1 - rt;                    // rows of this thread (ra <= rb); equal for the middle row
+  const double* rg = r + grp * TG;                       // this group's thetas
+  const int rt0 = rt & ~31;                              // first row-pair of this warp
+  const int ja_end = min(rt0 + 31, half - 1);            // last column any lane's short row needs
+  const int jb_end = n - 1 - rt0;                        // last column any lane's long row needs
+  const int ia = min(ra, n - 1), ib = max(rb, 0);        // clamp the idle lanes of the last warp
+  double wa[TG], wb[TG];
 #pragma unroll
-  for (int t = 0; t < TB; ++t) { wa[t] = 0.0; wb[t] = 0.0; }
-  if (tid < half) {
-    // columns j <= ra feed both rows; ra < j <= rb only the long row
-    for (int j = 0; j <= ra; ++j) {
-      const double la = LinvT[(size_t)j * n + ra], lb = LinvT[(size_t)j * n + rb];
-      const double2* rj = reinterpret_cast<const double2*>(r + (size_t)j * TB);
+  for (int t = 0; t < TG; ++t) { wa[t] = 0.0; wb[t] = 0.0; }
+  for (int c = 0; c < n_chunks; ++c) {
+    const int buf = c & 1;
+    if (tid == 0 && c + 1 < n_chunks) {                    // prefetch the next chunk into the other buffer
+      const int nb = buf ^ 1, j1 = (c + 1) * CH;
+      if (c >= 1) tc::mbar_wait(empty0 + 8 * nb, ((c - 1) >> 1) & 1);
+      const uint32_t bytes = ((uint32_t)min(CH, n - j1) * n * 8u + 15u) & ~15u;
+      tc::mbar_arrive_expect_tx(full0 + 8 * nb, bytes);
+      tc::bulk_load(tc::smem_u32(S + (size_t)nb * CH * n), LinvT + (size_t)j1 * n, bytes, full0 + 8 * nb);
+    }
+    tc::mbar_wait(full0 + 8 * buf, (c >> 1) & 1);
+    const double* Sb = S + (size_t)buf * CH * n;
+    const int j0 = c * CH, jn = min(CH, n - j0);
+    if (j0 <= jb_end) {
+#pragma unroll 4
+      for (int jj = 0; jj < jn; ++jj) {
+        const int j = j0 + jj;
+        const double lb = Sb[(size_t)jj * n + ib];
+        double v[TG];
 #pragma unroll
-      for (int t = 0; t < TB / 2; ++t) {
-        const double2 v = rj[t];
-        wa[2 * t] = fma(la, v.x, wa[2 * t]); wa[2 * t + 1] = fma(la, v.y, wa[2 * t + 1]);
-        wb[2 * t] = fma(lb, v.x, wb[2 * t]); wb[2 * t + 1] = fma(lb, v.y, wb[2 * t + 1]);
+        for (int t = 0; t < TG; ++t) v[t] = rg[(size_t)j * TB + t];
+#pragma unroll
+        for (int t = 0; t < TG; ++t) wb[t] = fma(lb, v[t], wb[t]);
+        if (j <= ja_end) {                                   // warp-uniform: the short rows end early
+          const double la = Sb[(size_t)jj * n + ia];
+#pragma unroll
+          for (int t = 0; t < TG; ++t) wa[t] = fma(la, v[t], wa[t]);
+        }
       }
     }
-    for (int j = ra + 1; j <= rb; ++j) {
-      const double lb = LinvT[(size_t)j * n + rb];
-      const double2* rj = reinterpret_cast<const double2*>(r + (size_t)j * TB);
-#pragma unroll
-      for (int t = 0; t < TB / 2; ++t) {
-        const double2 v = rj[t];
-        wb[2 * t] = fma(lb, v.x, wb[2 * t]); wb[2 * t + 1] = fma(lb, v.y, wb[2 * t + 1]);
-      }
-    }
+    __syncwarp();
+    if (lane == 0) tc::mbar_arrive(empty0 + 8 * buf);
   }
-  const bool two = tid < half && ra != rb;
+  const bool one = rt < half, two = one && ra != rb;
 #pragma unroll
-  for (int t = 0; t < TB; ++t) {
-    double ss = (tid < half ? wb[t] * wb[t] : 0.0) + (two ? wa[t] * wa[t] : 0.0);
+  for (int t = 0; t < TG; ++t) {
+    double ss = (one ? wb[t] * wb[t] : 0.0) + (two ? wa[t] * wa[t] : 0.0);
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) ss += __shfl_xor_sync(0xffffffffu, ss, o);
-    if (lane == 0) part[warp * TB + t] = ss;
+    if (lane == 0) part[(warp % (RT >> 5)) * TB + grp * TG + t] = ss;   // one slot per (row-warp, theta)
   }
   __syncthreads();
   if (tid < TB) {
     const int b = b0 + tid;
     if (b < B) {
       double chi2 = 0.0;
-      for (int w = 0; w < nwarp; ++w) chi2 += part[w * TB + tid];
+      for (int w = 0; w < (RT >> 5); ++w) chi2 += part[w * TB + tid];
       double out = -0.5 * chi2 + log_norm;
       // support of the uniform priors (compared in the float32 theta arrives in) and finiteness
       bool ok = isfinite(out);
@@ -109,18 +142,31 @@ nsgpu_status chi2_loglike(nsgpu_ctx* ctx, const float* theta, int B, const int* 
                           cudaStream_t st) {
   if (B == 0) return NSGPU_OK;
   const int n = ctx->n_data;
-  const int threads = std::min(512, (((n + 1) / 2 + 31) / 32) * 32);
-  if ((n + 1) / 2 > 512) { ctx->err = "chi2: n_data > 1024 not supported"; return NSGPU_ESHAPE; }
-  const size_t smem = ((size_t)n * TB + 32 * TB) * sizeof(double);
+  const int RT = (((n + 1) / 2 + 31) / 32) * 32;        // row-pair threads, whole warps
+  if (RT > 1024) { ctx->err = "chi2: n_data > 2048 not supported"; return NSGPU_ESHAPE; }
+  // thetas per thread TG = 8 (each factor element read from shared memory feeds 8 FMAs), G thread
+  // groups per CTA, TB = 8 G thetas per CTA
+  const int groups = RT <= 160 ? 4 : (RT <= 320 ? 2 : 1);
+  const int TBv = groups * 8;
+  // chunk of CH factor columns per buffer: two buffers within ~110 KB, CH even
+  int CH = (int)((110 * 1024 / 2) / ((size_t)n * 8));
+  CH = std::max(2, std::min(16, CH & ~1));
+  const size_t smem = ((size_t)n * TBv + 32 * TBv + 4) * sizeof(double) + 2 * (size_t)CH * n * sizeof(double);
   static size_t configured = 0;
   if (smem > configured) {
-    NSGPU_CUDA(cudaFuncSetAttribute(chi2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    if (smem > 220 * 1024) { ctx->err = "chi2: tiles exceed shared memory"; return NSGPU_ESHAPE; }
+    NSGPU_CUDA(cudaFuncSetAttribute(chi2_kernel<32, 8, 640>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    NSGPU_CUDA(cudaFuncSetAttribute(chi2_kernel<16, 8, 640>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    NSGPU_CUDA(cudaFuncSetAttribute(chi2_kernel<8, 8, 1024>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     configured = smem;
   }
   StageTimer tm(ctx, 5, st);
-  chi2_kernel<<<(B + TB - 1) / TB, threads, smem, st>>>(ctx->model, ctx->data, ctx->Linv, n, B, n_rows_dev, theta,
-                                                         ctx->D, ctx->prior_kind, ctx->prior_p0, ctx->prior_p1,
-                                                         ctx->log_norm, logL);
+  const int grid = (B + TBv - 1) / TBv, threads = groups * RT;
+#define NSGPU_CHI2_ARGS ctx->model, ctx->data, ctx->Linv, n, B, RT, CH, n_rows_dev, theta, ctx->D, ctx->prior_kind, ctx->prior_p0, ctx->prior_p1, ctx->log_norm, logL
+  if (groups == 4) chi2_kernel<32, 8, 640><<<grid, threads, smem, st>>>(NSGPU_CHI2_ARGS);
+  else if (groups == 2) chi2_kernel<16, 8, 640><<<grid, threads, smem, st>>>(NSGPU_CHI2_ARGS);
+  else chi2_kernel<8, 8, 1024><<<grid, threads, smem, st>>>(NSGPU_CHI2_ARGS);
+#undef NSGPU_CHI2_ARGS
   NSGPU_LAUNCH_CHECK();
   return NSGPU_OK;
 }

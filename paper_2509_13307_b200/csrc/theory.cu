@@ -49,6 +49,14 @@ __device__ __forceinline__ double exp_fast(double x) {
   return __hiloint2double(__double2hiint(p) + (e << 20), __double2loint(p));
 }
 
+// 1/x in fp64 for normal positive x: fp32 reciprocal seed, two Newton steps (relative error < 1e-15)
+__device__ __forceinline__ double rcp_fast(double x) {
+  double r = (double)__frcp_rn((float)x);
+  r = fma(r, fma(-x, r, 1.0), r);
+  r = fma(r, fma(-x, r, 1.0), r);
+  return r;
+}
+
 // Exclusive prefix (or suffix, when `reverse`) sum of arr[0..n) in place by ONE warp: each lane sums a
 // contiguous chunk, a shuffle scan carries across lanes.  No block-level synchronisation inside.
 __device__ void warp_scan_exclusive(double* arr, int n, bool reverse, int lane) {
@@ -98,9 +106,10 @@ __global__ void __launch_bounds__(SHEAR_THREADS, 2) shear_project_kernel(const f
   double* Dq = Eq + nq;                                // [nq]
   double* gq = Dq + nq;                                // [nq]   dchi / chi^2
   double* hs = gq + nq;                                // [nq]   half-cell terms, then log10 chi
-  double* Wt = hs + nq;                                // [nt][nq] total window
+  double* ichi = hs + nq;                              // [nq]   1 / chi
+  double* Wt = ichi + nq;                              // [nt][nq] total window
   double* scr = Wt + (size_t)nt * nq;                  // [n_scr][nqp]: scan arrays, then Pg[n_ell][nqp]
-  size_t n_dbl = (size_t)nq * (5 + nt) + (size_t)n_scr * nqp + 2;
+  size_t n_dbl = (size_t)nq * (6 + nt) + (size_t)n_scr * nqp + 2;
   n_dbl = (n_dbl + 1) & ~(size_t)1;
   unsigned long long* bar = reinterpret_cast<unsigned long long*>(chi + n_dbl - 2);   // 8-byte mbarrier
   float* table = reinterpret_cast<float*>(chi + n_dbl);   // [n_z_emu][n_k], 16-byte aligned
@@ -152,27 +161,30 @@ __global__ void __launch_bounds__(SHEAR_THREADS, 2) shear_project_kernel(const f
   __syncthreads();
   for (int q = tid; q < nq; q += blockDim.x) {
     const double c = C_OVER_H0 * (sc_f[q] + 0.5 * gq[q]);
+    const double ic = rcp_fast(c);
     chi[q] = c;
-    Dq[q] = exp_fast(-(sc_g[q] + 0.5 * hs[q]));
-    gq[q] = C_OVER_H0 * gq[q] / (c * c);                      // dchi_q / chi_q^2
+    ichi[q] = ic;
+    Dq[q] = exp_fast(sc_g[q] + 0.5 * hs[q]);                  // 1 / D_q
+    gq[q] = C_OVER_H0 * gq[q] * ic * ic;                      // dchi_q / chi_q^2
   }
   __syncthreads();
 
   // a7: n_i(z - dz_i); W^I; the two suffix sums of W^gamma = A - chi B for all bins at once
-  const double norm = 1.0 / (A.nz_sigma * 2.5066282746310002);   // 1/(sigma sqrt(2 pi))
+  const double inv_sig = 1.0 / A.nz_sigma;
+  const double norm = inv_sig / 2.5066282746310002;              // 1/(sigma sqrt(2 pi))
   for (int it = tid; it < nt * nq; it += blockDim.x) {
     const int i = it / nq, q = it - i * nq;
     const double mu = A.nz_mean[i] + (double)th[A.idx_dz + i];
     const double A0 = th[A.idx_ia + 3 * i], A1 = th[A.idx_ia + 3 * i + 1], A2 = th[A.idx_ia + 3 * i + 2];
     const double z = A.z_q[q], a = A.a_q[q];
-    const double u = (z - mu) / A.nz_sigma;
+    const double u = (z - mu) * inv_sig;
     const double nz = exp_fast(-0.5 * u * u) * norm;
-    const double w = nz * A.da / (a * a);                     // n_i(z_q) dz_q
+    const double w = nz * A.da * (1.0 + z) * (1.0 + z);       // n_i(z_q) dz_q, dz = da / a^2
     scr[(size_t)(2 * i) * nqp + q] = w;
-    scr[(size_t)(2 * i + 1) * nqp + q] = w / chi[q];
+    scr[(size_t)(2 * i + 1) * nqp + q] = w * ichi[q];
     const double x = (1.0 + z) / 1.62 - 1.0;
     const double Aia = A0 + A1 * x + A2 * x * x;
-    Wt[(size_t)i * nq + q] = -Aia * C1_RHOCR * Om / Dq[q] * nz * Eq[q] / C_OVER_H0;   // W^I (eq. A4)
+    Wt[(size_t)i * nq + q] = -Aia * (C1_RHOCR / C_OVER_H0) * Om * Dq[q] * nz * Eq[q];   // W^I (eq. A4); Dq holds 1/D
   }
   __syncthreads();
   for (int c = warp; c < 2 * nt; c += nwarp) warp_scan_exclusive(scr + (size_t)c * nqp, nq, true, lane);
@@ -198,7 +210,7 @@ __global__ void __launch_bounds__(SHEAR_THREADS, 2) shear_project_kernel(const f
   const double inv_dlk = 1.0 / A.dlk, bar_amp = (eta0 - 0.7) * 0.1;
   for (int it = tid; it < n_lookup; it += blockDim.x) {
     const int bl = it / nq, q = it - bl * nq;
-    const double k = (A.ell[bl] + 0.5) / chi[q];
+    const double k = (A.ell[bl] + 0.5) * ichi[q];
     double P = 0.0;
     if (k >= A.k_min && k <= A.k_max) {
       const double x = A.lellh[bl] - hs[q];
@@ -215,35 +227,53 @@ __global__ void __launch_bounds__(SHEAR_THREADS, 2) shear_project_kernel(const f
         hi = fma(w, (double)row[A.sk], hi);
       }
       double y = (1.0 - s) * lo + s * hi;
-      y -= bar_amp * k * k / (k * k + 1.0);
+      const double k2 = k * k;
+      y -= bar_amp * k2 * rcp_fast(k2 + 1.0);
       P = exp_fast(y * 2.302585092994046);
     }
     Pg[(size_t)bl * nqp + q] = P * gq[q];
   }
   __syncthreads();
 
-  // a8 (sum): C_ij(ell) = sum_q Wt_i Wt_j Pg; one thread per output, q serial (operands broadcast or
-  // conflict-free from shared memory: consecutive threads differ in ell, Pg rows have odd stride)
+  // a8 (sum): C_ij(ell) = sum_q Wt_i Wt_j Pg.  Work item = (pair, group of 4 ell); 4 adjacent lanes share
+  // an item and split the q range, so the window product is formed once per 4 outputs; a 2-step shuffle
+  // reduction joins the four partial sums.
   const int n_pairs = nt * (nt + 1) / 2;
-  for (int o = tid; o < n_pairs * A.n_ell; o += blockDim.x) {
-    const int p = o / A.n_ell, bl = o - p * A.n_ell;
+  const int n_lg = (A.n_ell + 3) >> 2, n_items = n_pairs * n_lg;
+  const int part = tid & 3;
+  for (int item0 = 0; item0 < n_items; item0 += blockDim.x >> 2) {
+    const int item = item0 + (tid >> 2);
+    const bool live = item < n_items;
+    const int p = live ? item / n_lg : 0, lg = live ? item - p * n_lg : 0;
     int i = 0, rem = p;                                        // pair p -> (i <= j), row-major upper
     while (rem >= nt - i) { rem -= nt - i; ++i; }
     const int j = i + rem;
     const double* wi = Wt + (size_t)i * nq;
     const double* wj = Wt + (size_t)j * nq;
-    const double* pg = Pg + (size_t)bl * nqp;
-    double acc0 = 0.0, acc1 = 0.0;
-    int q = 0;
-    for (; q + 1 < nq; q += 2) {
-      acc0 = fma(wi[q] * wj[q], pg[q], acc0);
-      acc1 = fma(wi[q + 1] * wj[q + 1], pg[q + 1], acc1);
+    const int l0 = 4 * lg;
+    const double* pg0 = Pg + (size_t)min(l0, A.n_ell - 1) * nqp;
+    const double* pg1 = Pg + (size_t)min(l0 + 1, A.n_ell - 1) * nqp;
+    const double* pg2 = Pg + (size_t)min(l0 + 2, A.n_ell - 1) * nqp;
+    const double* pg3 = Pg + (size_t)min(l0 + 3, A.n_ell - 1) * nqp;
+    double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+    if (live)
+      for (int q = part; q < nq; q += 4) {
+        const double ww = wi[q] * wj[q];
+        a0 = fma(ww, pg0[q], a0); a1 = fma(ww, pg1[q], a1); a2 = fma(ww, pg2[q], a2); a3 = fma(ww, pg3[q], a3);
+      }
+#pragma unroll
+    for (int o = 1; o < 4; o <<= 1) {
+      a0 += __shfl_xor_sync(0xffffffffu, a0, o); a1 += __shfl_xor_sync(0xffffffffu, a1, o);
+      a2 += __shfl_xor_sync(0xffffffffu, a2, o); a3 += __shfl_xor_sync(0xffffffffu, a3, o);
     }
-    if (q < nq) acc0 = fma(wi[q] * wj[q], pg[q], acc0);
-    const double lf = A.lf[bl];                                // ln(ell/550)/ln 30
-    const double mi = (double)th[A.idx_m + 2 * i] + (double)th[A.idx_m + 2 * i + 1] * lf;
-    const double mj = (double)th[A.idx_m + 2 * j] + (double)th[A.idx_m + 2 * j + 1] * lf;
-    model[(size_t)b * n_data + o] = (1.0 + mi) * (1.0 + mj) * (acc0 + acc1);
+    const int bl = l0 + part;                                  // lane `part` writes ell l0 + part
+    if (live && bl < A.n_ell) {
+      const double acc = part == 0 ? a0 : (part == 1 ? a1 : (part == 2 ? a2 : a3));
+      const double lf = A.lf[bl];                              // ln(ell/550)/ln 30
+      const double mi = (double)th[A.idx_m + 2 * i] + (double)th[A.idx_m + 2 * i + 1] * lf;
+      const double mj = (double)th[A.idx_m + 2 * j] + (double)th[A.idx_m + 2 * j + 1] * lf;
+      model[(size_t)b * n_data + (size_t)p * A.n_ell + bl] = (1.0 + mi) * (1.0 + mj) * acc;
+    }
   }
 }
 
@@ -294,7 +324,7 @@ __global__ void copy_model_kernel(const float* __restrict__ src, int n, int B, c
 
 static size_t shear_smem_bytes(const ShearDev& S) {
   const size_t nqp = (size_t)S.n_chi | 1, n_scr = (size_t)std::max(2 * S.n_tomo, S.n_ell);
-  size_t d = (size_t)S.n_chi * (5 + S.n_tomo) + n_scr * nqp + 2;
+  size_t d = (size_t)S.n_chi * (6 + S.n_tomo) + n_scr * nqp + 2;
   d = (d + 1) & ~(size_t)1;
   return d * sizeof(double) + (size_t)S.n_z_emu * S.n_k * sizeof(float) + 16;
 }
