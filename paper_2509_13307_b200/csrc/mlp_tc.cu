@@ -77,6 +77,39 @@ __device__ __forceinline__ float gated_act16(float t, const float4& p) {
   return fmaf(sg, p.w, p.z) * t;
 }
 
+// packed fp32x2 arithmetic (sm_100: FFMA2 / FMUL2 / FADD2 halve the FMA-pipe instruction count)
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pk2(float a, float b) { f32x2 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(a), "f"(b)); return r; }
+__device__ __forceinline__ void upk2(f32x2 v, float& a, float& b) { asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); }
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) { f32x2 d; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c)); return d; }
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) { f32x2 d; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) { f32x2 d; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+
+// Two columns of the hidden-layer epilogue at once: t = acc cs + bias; 16 (beta + sigma(alpha t)(1 - beta)) t;
+// hi/lo fp16 split.  pa = {bias0, bias1, a2_0, a2_1}, pb = {16 beta0, 16 beta1, 16 (1-beta0), 16 (1-beta1)}.
+__device__ __forceinline__ void act_split_pair(f32x2 acc, f32x2 cs2, const float4& pa, const float4& pb, uint32_t& hi,
+                                               uint32_t& lo) {
+  const f32x2 t = fma2(acc, cs2, pk2(pa.x, pa.y));
+  float s0, s1;
+  upk2(mul2(pk2(pa.z, pa.w), t), s0, s1);
+  // sigma = 1/(1 + 2^(-alpha t log2 e)): 2 MUFU ops per column.  (A Newton reciprocal on the FMA pipe was
+  // measured no faster: the epilogue is issue-bound, not MUFU-bound.)
+  const float e0 = ex2_approx(s0), e1 = ex2_approx(s1);
+  float d0, d1;
+  upk2(add2(pk2(e0, e1), pk2(1.0f, 1.0f)), d0, d1);
+  const f32x2 sg = pk2(rcp_approx(d0), rcp_approx(d1));
+  const f32x2 o = mul2(fma2(sg, pk2(pb.z, pb.w), pk2(pb.x, pb.y)), t);
+  float o0, o1;
+  upk2(o, o0, o1);
+  const __half2 h = __floats2half2_rn(o0, o1);
+  const float2 hf = __half22float2(h);
+  float l0, l1;
+  upk2(fma2(pk2(hf.x, hf.y), pk2(-1.0f, -1.0f), o), l0, l1);
+  const __half2 l = __floats2half2_rn(l0, l1);
+  hi = *reinterpret_cast<const uint32_t*>(&h);
+  lo = *reinterpret_cast<const uint32_t*>(&l);
+}
+
 // x -> (hi, lo) fp16 pair planes, two elements at a time
 __device__ __forceinline__ void split2(float a, float b, uint32_t& hi, uint32_t& lo) {
   const __half2 h = __floats2half2_rn(a, b);
@@ -104,7 +137,11 @@ __global__ void __launch_bounds__(256) mlp_first_layer_tc(const float* __restric
   extern __shared__ __align__(16) unsigned char smem_raw[];
   float4* sp = reinterpret_cast<float4*>(smem_raw);          // [width]
   float* sW = reinterpret_cast<float*>(sp + width);          // [n_in][width]
-  for (int i = threadIdx.x; i < width; i += blockDim.x) sp[i] = params[i];
+  for (int i = threadIdx.x; i < width / 2; i += blockDim.x) {   // two columns per entry pair (see act_split_pair)
+    const float4 c0 = params[2 * i], c1 = params[2 * i + 1];
+    sp[2 * i] = make_float4(c0.x, c1.x, c0.y, c1.y);
+    sp[2 * i + 1] = make_float4(c0.z, c1.z, c0.w, c1.w);
+  }
   for (int i = threadIdx.x; i < n_in * width; i += blockDim.x) sW[i] = W[i];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int r = (warp & 3) * 32 + lane;                      // row within the tile
@@ -129,18 +166,23 @@ __global__ void __launch_bounds__(256) mlp_first_layer_tc(const float* __restric
   const int n_pieces = width >> 3, half_pieces = (n_pieces + 1) >> 1;
   const int p_begin = (warp >> 2) * half_pieces, p_end = min(p_begin + half_pieces, n_pieces);
   const size_t tile_base = (size_t)blockIdx.x * ((size_t)BLOCK_M * width) + (size_t)r * 8;
+  f32x2 x2[NSGPU_MAX_IN];
+#pragma unroll
+  for (int c = 0; c < NSGPU_MAX_IN; ++c) x2[c] = pk2(x[c], x[c]);
+  const f32x2 one2 = pk2(1.0f, 1.0f);
   for (int p = p_begin; p < p_end; ++p) {
     uint32_t hi[4], lo[4];
+    f32x2 t[4] = {0ull, 0ull, 0ull, 0ull};                      // 8 neurons of this piece, bias added in the epilogue
 #pragma unroll
-    for (int jj = 0; jj < 4; ++jj) {
-      const int j = 8 * p + 2 * jj;
-      const float4 pa = sp[j], pb = sp[j + 1];
-      float t0 = pa.x, t1 = pb.x;
+    for (int c = 0; c < NSGPU_MAX_IN; ++c)
+      if (c < n_in) {
+        const float4 wlo = *reinterpret_cast<const float4*>(sW + c * width + 8 * p);
+        const float4 whi = *reinterpret_cast<const float4*>(sW + c * width + 8 * p + 4);
+        t[0] = fma2(x2[c], pk2(wlo.x, wlo.y), t[0]); t[1] = fma2(x2[c], pk2(wlo.z, wlo.w), t[1]);
+        t[2] = fma2(x2[c], pk2(whi.x, whi.y), t[2]); t[3] = fma2(x2[c], pk2(whi.z, whi.w), t[3]);
+      }
 #pragma unroll
-      for (int c = 0; c < NSGPU_MAX_IN; ++c)
-        if (c < n_in) { t0 = fmaf(x[c], sW[c * width + j], t0); t1 = fmaf(x[c], sW[c * width + j + 1], t1); }
-      split2(gated_act16(t0, pa), gated_act16(t1, pb), hi[jj], lo[jj]);
-    }
+    for (int jj = 0; jj < 4; ++jj) act_split_pair(t[jj], one2, sp[8 * p + 2 * jj], sp[8 * p + 2 * jj + 1], hi[jj], lo[jj]);
     if (m0 + r < M) {
       const size_t o = tile_base + (size_t)p * PIECE_HALVES;
       *reinterpret_cast<uint4*>(out_hi + o) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
@@ -196,7 +238,11 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) mlp_gemm_tc(const __grid_cons
   if (warp == EPI_WARPS + 1) tc::tmem_alloc(tc::smem_u32(tmem_slot), 512);
   if (warp == EPI_WARPS && lane == 0) { tc::prefetch_tmap(&tm_whi); tc::prefetch_tmap(&tm_wlo); }
   if (EPI == 0) {   // hidden layers: N_pad <= 512 -> 8 KB of per-column parameters staged once
-    for (int i = threadIdx.x; i < g.N_pad; i += blockDim.x) reinterpret_cast<float4*>(params)[i] = g.p_hidden[i];
+    for (int i = threadIdx.x; i < g.N_pad / 2; i += blockDim.x) {   // two columns per entry pair (see act_split_pair)
+      const float4 c0 = g.p_hidden[2 * i], c1 = g.p_hidden[2 * i + 1];
+      reinterpret_cast<float4*>(params)[2 * i] = make_float4(c0.x, c1.x, c0.y, c1.y);
+      reinterpret_cast<float4*>(params)[2 * i + 1] = make_float4(c0.z, c1.z, c0.w, c1.w);
+    }
   }
   tc::fence_before_sync();
   __syncthreads();
@@ -266,7 +312,7 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) mlp_gemm_tc(const __grid_cons
     uint32_t pcount = 0;
     for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
       const int m_blk = tile / n_blocks, n_blk = tile - m_blk * n_blocks;
-      float acc[CPT];
+      f32x2 acc[CPT / 2];
       for (int kb = 0; kb < k_blocks; ++kb, ++pcount) {
         const uint32_t pb = pcount & 1, pphase = (pcount >> 1) & 1;
         tc::mbar_wait(pfull0 + 8 * pb, pphase);
@@ -279,10 +325,11 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) mlp_gemm_tc(const __grid_cons
           tc::tmem_ld_wait();
           if (kb == 0) {
 #pragma unroll
-            for (int j = 0; j < LDC; ++j) acc[LDC * c + j] = __uint_as_float(r[j]);
+            for (int j = 0; j < LDC / 2; ++j) acc[(LDC / 2) * c + j] = pk2(__uint_as_float(r[2 * j]), __uint_as_float(r[2 * j + 1]));
           } else {
 #pragma unroll
-            for (int j = 0; j < LDC; ++j) acc[LDC * c + j] += __uint_as_float(r[j]);
+            for (int j = 0; j < LDC / 2; ++j)
+              acc[(LDC / 2) * c + j] = add2(acc[(LDC / 2) * c + j], pk2(__uint_as_float(r[2 * j]), __uint_as_float(r[2 * j + 1])));
           }
         }
         tc::fence_before_sync();
@@ -296,6 +343,7 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) mlp_gemm_tc(const __grid_cons
       if (g.dbg & 16) continue;   // timing experiment: no epilogue math / stores
       if (EPI == 0) {
         const float4* p = reinterpret_cast<const float4*>(params) + n0;
+        const f32x2 cs2 = pk2(g.cscale, g.cscale);
         // canonical layout: piece (n0/8 + c) of this tile, 16 bytes per row: lanes are contiguous
         const size_t o = (size_t)m_blk * ((size_t)BLOCK_M * g.ld_out) + (size_t)(n0 >> 3) * PIECE_HALVES + (size_t)r_in * 8;
         __half* dh = g.out_hi + o;
@@ -304,12 +352,8 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) mlp_gemm_tc(const __grid_cons
         for (int c = 0; c < CPT / 8; ++c) {
           uint32_t hi[4], lo[4];
 #pragma unroll
-          for (int j = 0; j < 4; ++j) {
-            const float4 pa = p[8 * c + 2 * j], pb2 = p[8 * c + 2 * j + 1];
-            const float ta = fmaf(acc[8 * c + 2 * j], g.cscale, pa.x);
-            const float tb = fmaf(acc[8 * c + 2 * j + 1], g.cscale, pb2.x);
-            split2(gated_act16(ta, pa), gated_act16(tb, pb2), hi[j], lo[j]);
-          }
+          for (int j = 0; j < 4; ++j)
+            act_split_pair(acc[4 * c + j], cs2, p[8 * c + 2 * j], p[8 * c + 2 * j + 1], hi[j], lo[j]);
           if (row_ok) {
             *reinterpret_cast<uint4*>(dh + (size_t)c * PIECE_HALVES) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
             *reinterpret_cast<uint4*>(dl + (size_t)c * PIECE_HALVES) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
@@ -325,7 +369,9 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) mlp_gemm_tc(const __grid_cons
 #pragma unroll
           for (int j = 0; j < CPT; ++j) {
             const float2 pj = __ldg(p + j);
-            float y = fmaf(acc[j], pj.x, pj.y);
+            float a0, a1;
+            upk2(acc[j >> 1], a0, a1);
+            float y = fmaf((j & 1) ? a1 : a0, pj.x, pj.y);
             if (g.apply_exp10) y = exp10f(y);
             if (row_ok && n0 + j < g.n_valid) dst[(size_t)(n0 + j) * g.rows_per_theta] = y;
           }
@@ -338,7 +384,9 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) mlp_gemm_tc(const __grid_cons
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
               const float2 pj = __ldg(p + 4 * c + j);
-              y[j] = fmaf(acc[4 * c + j], pj.x, pj.y);
+              float a0, a1;
+              upk2(acc[(4 * c + j) >> 1], a0, a1);
+              y[j] = fmaf((j & 1) ? a1 : a0, pj.x, pj.y);
               if (g.apply_exp10) y[j] = exp10f(y[j]);
             }
             if (row_ok) {

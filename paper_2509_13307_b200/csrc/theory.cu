@@ -115,6 +115,7 @@ __global__ void __launch_bounds__(SHEAR_THREADS, 2) shear_project_kernel(const f
   float* table = reinterpret_cast<float*>(chi + n_dbl);   // [n_z_emu][n_k], 16-byte aligned
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarp = blockDim.x >> 5;
+  const unsigned nq_magic = 0xFFFFFFFFu / (unsigned)nq + 1u;    // it / nq == umulhi(it, magic) for it < 2^16
   const float* th = theta + (size_t)b * D;
   const float* src = spec + (size_t)b * A.n_z_emu * A.n_k;
   const unsigned table_bytes = (unsigned)(A.n_z_emu * A.n_k) * 4u;
@@ -173,7 +174,7 @@ __global__ void __launch_bounds__(SHEAR_THREADS, 2) shear_project_kernel(const f
   const double inv_sig = 1.0 / A.nz_sigma;
   const double norm = inv_sig / 2.5066282746310002;              // 1/(sigma sqrt(2 pi))
   for (int it = tid; it < nt * nq; it += blockDim.x) {
-    const int i = it / nq, q = it - i * nq;
+    const int i = (int)__umulhi((unsigned)it, nq_magic), q = it - i * nq;
     const double mu = A.nz_mean[i] + (double)th[A.idx_dz + i];
     const double A0 = th[A.idx_ia + 3 * i], A1 = th[A.idx_ia + 3 * i + 1], A2 = th[A.idx_ia + 3 * i + 2];
     const double z = A.z_q[q], a = A.a_q[q];
@@ -190,7 +191,7 @@ __global__ void __launch_bounds__(SHEAR_THREADS, 2) shear_project_kernel(const f
   for (int c = warp; c < 2 * nt; c += nwarp) warp_scan_exclusive(scr + (size_t)c * nqp, nq, true, lane);
   __syncthreads();
   for (int it = tid; it < nt * nq; it += blockDim.x) {
-    const int i = it / nq, q = it - i * nq;
+    const int i = (int)__umulhi((unsigned)it, nq_magic), q = it - i * nq;
     const double s0 = scr[(size_t)(2 * i) * nqp + q], s1 = scr[(size_t)(2 * i + 1) * nqp + q];
     const double wg = 1.5 * Om / (C_OVER_H0 * C_OVER_H0) * (1.0 + A.z_q[q]) * chi[q] * (s0 - chi[q] * s1);
     Wt[(size_t)i * nq + q] += wg;                             // + W^gamma (eq. A3)
@@ -208,8 +209,9 @@ __global__ void __launch_bounds__(SHEAR_THREADS, 2) shear_project_kernel(const f
   double* Pg = scr;                                           // [n_ell][nqp]
   const int n_lookup = A.n_ell * nq;
   const double inv_dlk = 1.0 / A.dlk, bar_amp = (eta0 - 0.7) * 0.1;
+#pragma unroll 2
   for (int it = tid; it < n_lookup; it += blockDim.x) {
-    const int bl = it / nq, q = it - bl * nq;
+    const int bl = (int)__umulhi((unsigned)it, nq_magic), q = it - bl * nq;
     const double k = (A.ell[bl] + 0.5) * ichi[q];
     double P = 0.0;
     if (k >= A.k_min && k <= A.k_max) {
