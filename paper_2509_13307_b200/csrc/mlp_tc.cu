@@ -57,6 +57,7 @@ struct GemmArgs {
   const __half *a_hi, *a_lo;  // input planes, canonical layout, K columns
   const float4* p_hidden;     // [N_pad] {bias, -alpha log2 e, 16 beta, 16 (1 - beta)}
   const float2* p_out;        // [N_pad] {cscale sigma_out, b sigma_out + mu_out}
+  const float4* p_out4;       // [N_pad/2] the same for column pairs: {s1_0, s1_1, s0_0, s0_1}
   float cscale;               // 2^-(wexp + 4): undoes the operand scalings
   __half *out_hi, *out_lo;    // next layer's planes (canonical layout, ld_out columns)
   int ld_out;
@@ -211,6 +212,8 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) mlp_gemm_tc(const __grid_cons
   constexpr int B_TILE_BYTES = BLOCK_N * 128;
   constexpr int CPT = BLOCK_N / (EPI_WARPS / 4);                 // columns per epilogue thread
   constexpr int LDC = (CPT % 16 == 0) ? 16 : 8;                  // columns per tcgen05.ld
+  constexpr int NPB = BLOCK_N <= 128 ? 4 : 2;                    // TMEM partial buffers (ring)
+  constexpr int PB_COLS = 512 / NPB;
   constexpr uint32_t IDESC = tc::idesc_f16_f32(BLOCK_M, BLOCK_N);
   static_assert(STAGES >= 2, "need at least two smem stages");
   static_assert(BLOCK_N % 32 == 0 && BLOCK_N >= 32 && BLOCK_N <= 256 && CPT % 8 == 0, "UMMA N for M = 128; CPT multiple of 8");
@@ -219,9 +222,9 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) mlp_gemm_tc(const __grid_cons
   const uint32_t base = (tc::smem_u32(smem_dyn) + 1023u) & ~1023u;       // SWIZZLE_128B tiles: 1024-byte aligned
   unsigned char* base_ptr = smem_dyn + (base - tc::smem_u32(smem_dyn));
   const uint32_t bars = base + STAGES * STAGE;                            // full[S], empty[S], pfull[2], pempty[2]
-  const uint32_t full0 = bars, empty0 = bars + 8 * STAGES, pfull0 = bars + 16 * STAGES, pempty0 = pfull0 + 16;
-  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(base_ptr + STAGES * STAGE + 16 * STAGES + 32);
-  float* params = reinterpret_cast<float*>(base_ptr + STAGES * STAGE + 16 * STAGES + 64);   // 16-byte aligned
+  const uint32_t full0 = bars, empty0 = bars + 8 * STAGES, pfull0 = bars + 16 * STAGES, pempty0 = pfull0 + 32;
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(base_ptr + STAGES * STAGE + 16 * STAGES + 64);
+  float* params = reinterpret_cast<float*>(base_ptr + STAGES * STAGE + 16 * STAGES + 80);   // 16-byte aligned
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   int M = g.M_host;
@@ -232,7 +235,7 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) mlp_gemm_tc(const __grid_cons
 
   if (threadIdx.x == 0) {
     for (int s = 0; s < STAGES; ++s) { tc::mbar_init(full0 + 8 * s, 1); tc::mbar_init(empty0 + 8 * s, 1); }
-    for (int b = 0; b < 2; ++b) { tc::mbar_init(pfull0 + 8 * b, 1); tc::mbar_init(pempty0 + 8 * b, EPI_WARPS); }
+    for (int b = 0; b < NPB; ++b) { tc::mbar_init(pfull0 + 8 * b, 1); tc::mbar_init(pempty0 + 8 * b, EPI_WARPS); }
     tc::fence_barrier_init();
   }
   if (warp == EPI_WARPS + 1) tc::tmem_alloc(tc::smem_u32(tmem_slot), 512);
@@ -276,11 +279,11 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) mlp_gemm_tc(const __grid_cons
       uint32_t stage = 0, phase = 0, pcount = 0;
       for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
         for (int kb = 0; kb < k_blocks; ++kb, ++pcount) {
-          const uint32_t pb = pcount & 1, pphase = (pcount >> 1) & 1;
+          const uint32_t pb = pcount % NPB, pphase = (pcount / NPB) & 1;
           tc::mbar_wait(pempty0 + 8 * pb, pphase ^ 1);          // the epilogue has pulled this partial
           tc::mbar_wait(full0 + 8 * stage, phase);
           tc::fence_after_sync();
-          const uint32_t d_tmem = tmem_base + pb * 256;
+          const uint32_t d_tmem = tmem_base + pb * PB_COLS;
           const uint32_t s0 = base + stage * STAGE;
           // A: canonical no-swizzle K-major tile -- 16-byte pieces 2048 bytes apart along K (leading
           // byte offset), 8-row groups 128 bytes apart along M (stride byte offset); one MMA consumes
@@ -314,10 +317,10 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) mlp_gemm_tc(const __grid_cons
       const int m_blk = tile / n_blocks, n_blk = tile - m_blk * n_blocks;
       f32x2 acc[CPT / 2];
       for (int kb = 0; kb < k_blocks; ++kb, ++pcount) {
-        const uint32_t pb = pcount & 1, pphase = (pcount >> 1) & 1;
+        const uint32_t pb = pcount % NPB, pphase = (pcount / NPB) & 1;
         tc::mbar_wait(pfull0 + 8 * pb, pphase);
         tc::fence_after_sync();
-        const uint32_t t_src = tmem_base + pb * 256 + ((uint32_t)(q * 32) << 16) + hcol * CPT;
+        const uint32_t t_src = tmem_base + pb * PB_COLS + ((uint32_t)(q * 32) << 16) + hcol * CPT;
 #pragma unroll
         for (int c = 0; c < CPT / LDC; ++c) {
           uint32_t r[LDC];
@@ -361,19 +364,21 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) mlp_gemm_tc(const __grid_cons
         }
       } else {
         const float2* p = g.p_out + n0;            // warp-uniform addresses: L1 broadcast
+        const float4* p4 = g.p_out4 + (n0 >> 1);
         if (g.out_mode == 1) {
           // [theta][n][z] with z fastest: consecutive rows (lanes) of one theta are contiguous
           const int rr = row_ok ? row : 0;
           const int th = rr / g.rows_per_theta, zi = rr - th * g.rows_per_theta;
           float* dst = g.out_f32 + (size_t)th * ((size_t)g.n_valid * g.rows_per_theta) + zi;
 #pragma unroll
-          for (int j = 0; j < CPT; ++j) {
-            const float2 pj = __ldg(p + j);
-            float a0, a1;
-            upk2(acc[j >> 1], a0, a1);
-            float y = fmaf((j & 1) ? a1 : a0, pj.x, pj.y);
-            if (g.apply_exp10) y = exp10f(y);
-            if (row_ok && n0 + j < g.n_valid) dst[(size_t)(n0 + j) * g.rows_per_theta] = y;
+          for (int j = 0; j < CPT / 2; ++j) {                 // two columns per step: one 16-byte parameter load, one FFMA2
+            const float4 pj = __ldg(p4 + j);                 // {s1_0, s1_1, s0_0, s0_1}
+            float y0, y1;
+            upk2(fma2(acc[j], pk2(pj.x, pj.y), pk2(pj.z, pj.w)), y0, y1);
+            if (g.apply_exp10) { y0 = exp10f(y0); y1 = exp10f(y1); }
+            const int n = n0 + 2 * j;
+            if (row_ok && n < g.n_valid) dst[(size_t)n * g.rows_per_theta] = y0;
+            if (row_ok && n + 1 < g.n_valid) dst[(size_t)(n + 1) * g.rows_per_theta] = y1;
           }
         } else {
           float* dst = g.out_f32 + (size_t)row * g.ld_f32 + n0;
@@ -420,6 +425,7 @@ struct TcLayer {
   __half *Whi = nullptr, *Wlo = nullptr;     // [N_pad][K] K-major, scaled by 2^wexp
   float4* p_hidden = nullptr;                // layers 0 .. n_hidden-1
   float2* p_out = nullptr;                   // output layer
+  float4* p_out4 = nullptr;
   CUtensorMap tm_whi, tm_wlo;
 };
 
@@ -459,7 +465,7 @@ bool make_tmap(CUtensorMap* tm, const void* ptr, size_t rows, size_t cols, int b
 }
 
 int pick_block_n(int n, bool hidden) {
-  if (hidden) return n % 256 == 0 ? 256 : (n % 128 == 0 ? 128 : 64);
+  if (hidden) return n % 256 == 0 ? 256 : (n % 128 == 0 ? 128 : 64);   // 128 (4 TMEM partials) measured no faster than 256
   const int cand[4] = {256, 224, 128, 64};
   int best = 64, best_pad = 1 << 30;
   for (int c : cand) {
@@ -471,7 +477,7 @@ int pick_block_n(int n, bool hidden) {
 
 template <int BN, int EPI>
 nsgpu_status launch_gemm(nsgpu_ctx* ctx, const TcLayer& L, const GemmArgs& g, cudaStream_t st) {
-  const int smem = num_stages(BN) * stage_bytes(BN) + 16 * num_stages(BN) + 64 + (EPI == 0 ? 16 * g.N_pad : 0) + 1024;
+  const int smem = num_stages(BN) * stage_bytes(BN) + 16 * num_stages(BN) + 128 + (EPI == 0 ? 16 * g.N_pad : 0) + 1024;
   static bool configured = false;
   if (!configured) {
     NSGPU_CUDA(cudaFuncSetAttribute(mlp_gemm_tc<BN, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BUDGET));
@@ -554,6 +560,10 @@ nsgpu_status mlp_tc_prepare(nsgpu_ctx* ctx, int e, const nsgpu_emulator* h) {
         p[n] = make_float2(cs * h->out_std[n], h->b[l][n] * h->out_std[n] + h->out_mean[n]);
       NSGPU_CUDA(cudaMalloc((void**)&L.p_out, p.size() * sizeof(float2)));
       NSGPU_CUDA(cudaMemcpy(L.p_out, p.data(), p.size() * sizeof(float2), cudaMemcpyHostToDevice));
+      std::vector<float4> p4(L.N_pad / 2);
+      for (int n = 0; n < L.N_pad / 2; ++n) p4[n] = make_float4(p[2 * n].x, p[2 * n + 1].x, p[2 * n].y, p[2 * n + 1].y);
+      NSGPU_CUDA(cudaMalloc((void**)&L.p_out4, p4.size() * sizeof(float4)));
+      NSGPU_CUDA(cudaMemcpy(L.p_out4, p4.data(), p4.size() * sizeof(float4), cudaMemcpyHostToDevice));
     }
   }
   for (int i = 0; i < 2; ++i) {
@@ -568,7 +578,7 @@ nsgpu_status mlp_tc_prepare(nsgpu_ctx* ctx, int e, const nsgpu_emulator* h) {
 void mlp_tc_release(nsgpu_ctx* ctx, int e) {
   TcState* T = reinterpret_cast<TcState*>(ctx->emu[e].tmaps);
   if (!T) return;
-  for (TcLayer& L : T->layers) { cudaFree(L.Whi); cudaFree(L.Wlo); cudaFree(L.p_hidden); cudaFree(L.p_out); }
+  for (TcLayer& L : T->layers) { cudaFree(L.Whi); cudaFree(L.Wlo); cudaFree(L.p_hidden); cudaFree(L.p_out); cudaFree(L.p_out4); }
   delete T;
   ctx->emu[e].tmaps = nullptr;
 }
@@ -597,7 +607,7 @@ nsgpu_status mlp_forward_tc(nsgpu_ctx* ctx, int e, const float* theta, int B, co
     GemmArgs g;
     memset(&g, 0, sizeof(g));
     g.M_host = M; g.n_rows_dev = n_rows_dev; g.rows_per_theta = rpt; g.K = L.K; g.N_pad = L.N_pad; g.n_valid = L.n_valid;
-    g.p_hidden = L.p_hidden; g.p_out = L.p_out; g.cscale = ldexpf(1.0f, -(L.wexp + 4)) * TRUNC_COMP;
+    g.p_hidden = L.p_hidden; g.p_out = L.p_out; g.p_out4 = L.p_out4; g.cscale = ldexpf(1.0f, -(L.wexp + 4)) * TRUNC_COMP;
     g.a_hi = T->act[cur][0]; g.a_lo = T->act[cur][1];
     g.out_hi = T->act[cur ^ 1][0]; g.out_lo = T->act[cur ^ 1][1]; g.ld_out = E.width;
     g.out_f32 = spec_out; g.ld_f32 = E.n_out; g.apply_exp10 = (mode & NSGPU_SPEC_EXP10) ? 1 : 0;
