@@ -47,6 +47,20 @@ def flops_per_row(em):
     return hidden, total
 
 
+def ncu_traffic(workload, batch):
+    """dram bytes per launch of the dominant kernel from the committed ncu summary (profiles/r1_traffic.md);
+    None for workloads that were not captured."""
+    if workload != "c3a" or batch != 4096:
+        return None
+    try:
+        for line in open(os.path.join(ROOT, "profiles", "r1_traffic.md")):
+            if line.strip().startswith("traffic_bytes_per_launch"):
+                return int(line.split("=")[1])
+    except OSError:
+        pass
+    return None
+
+
 def peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -270,7 +284,8 @@ def run_nsgpu(args, rank, world, local_rank):
             peak, peak_note = pk["bf16_sustained"] * 0.5, f"{pk['src']} bf16 sustained x 0.5 (nominal TF32 ratio); SIMT fp32 path"
         total_stage_ms = sum(v[0] for v in stages.values())
         roofline = {"bound": "tensor", "kernel": "mlp_hidden", "achieved": ach, "peak": peak, "unit": "TFLOP/s",
-                    "frac": ach / peak if peak else None, "traffic": None, "peak_note": peak_note,
+                    "frac": ach / peak if peak else None, "traffic": ncu_traffic(args.workload, B), "peak_note": peak_note,
+                    "issued_frac": (3.0 if mlp_path == 1 else 1.0) * ach / peak if peak else None,
                     "algorithmic_flops_per_launch": launch_flops, "launches_timed": h_cnt,
                     "avg_launch_ms": h_ms / h_cnt if h_cnt else None,
                     "share_of_step": h_ms / total_stage_ms if total_stage_ms else None,
