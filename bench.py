@@ -196,19 +196,68 @@ def run_reference(args, rank):
         "gpu_launches": 0}))
 
 
+class Ranks:
+    """One process per GPU.  The theta batches are independent, so the ranks share no data: the process
+    group only provides the barrier around the timed region and the max-over-ranks of the elapsed time
+    (weak scaling: value = thetas of ALL ranks / slowest rank's time)."""
+
+    def __init__(self, world, backend, device=None):
+        self.world, self.dist, self.device = world, None, device
+        if world > 1:
+            import torch.distributed as dist
+            kw = {"device_id": device} if (backend == "nccl" and device is not None) else {}
+            dist.init_process_group(backend, **kw)
+            self.dist = dist
+
+    def barrier(self):
+        if self.dist is not None:
+            self.dist.barrier()
+
+    def reduce_max(self, x):
+        if self.dist is None:
+            return float(x)
+        import torch
+        t = torch.tensor([x], dtype=torch.float64, device=self.device if self.device is not None else "cpu")
+        self.dist.all_reduce(t, op=self.dist.ReduceOp.MAX)
+        return float(t.item())
+
+    def close(self):
+        if self.dist is not None:
+            self.dist.destroy_process_group()
+
+
+def aggregate(batch, world, steps, ms_max):
+    """whole-job throughput from the slowest rank's time"""
+    return batch * world * steps / (ms_max * 1e-3)
+
+
+def run_dry_cpu(args, rank, world):
+    """--dry-run-cpu: the multi-rank plumbing of this file without a GPU (gloo), for the CPU test suite:
+    every rank 'runs' steps that take (rank + 1) x 10 ms; rank 0 prints the JSON line."""
+    ranks = Ranks(world, "gloo")
+    ranks.barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        time.sleep(0.01 * (rank + 1))
+    ms = ranks.reduce_max((time.perf_counter() - t0) * 1e3)
+    ranks.barrier()
+    if rank == 0:
+        print(json.dumps({"metric": METRIC, "value": aggregate(args.batch, world, args.steps, ms), "unit": UNIT,
+                          "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps,
+                          "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+                          "data": "synthetic", "config": {"workload": "dry-run-cpu"}, "gpu_launches": 0}))
+    ranks.close()
+
+
 def run_nsgpu(args, rank, world, local_rank):
     import torch
     from paper_2509_13307_b200 import nsgpu
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (nsgpu has no CPU fallback)")
     nsgpu.lib()                                   # fails loudly if libnsgpu.so is missing
-    dist = None
-    if world > 1:
-        import torch.distributed as dist
-        torch.cuda.set_device(local_rank)
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     dev = local_rank
     torch.cuda.set_device(dev)
+    ranks = Ranks(world, "nccl", torch.device("cuda", dev))
     wl = MAKERS[args.workload]()
     B = args.batch
     ctx = make_context(nsgpu, torch, wl, B, dev)
@@ -219,16 +268,10 @@ def run_nsgpu(args, rank, world, local_rank):
     stream = torch.cuda.current_stream()
 
     def barrier():
-        if dist is not None:
-            dist.barrier()
+        ranks.barrier()
         torch.cuda.synchronize()
 
-    def reduce_max(x):
-        if dist is None:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device=f"cuda:{dev}")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+    reduce_max = ranks.reduce_max
 
     # ---- device-resident timing: value ------------------------------------------------------------
     for i in range(args.warmup):
@@ -303,7 +346,7 @@ def run_nsgpu(args, rank, world, local_rank):
         cpu_v, cpu_dt = oracle_rate(wl_o, cpu_n)
         total = B * world * args.steps
         print(json.dumps({
-            "metric": METRIC, "value": total / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "metric": METRIC, "value": aggregate(B, world, args.steps, ms), "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": f"{wl.name} B={B} per GPU", "D": wl.D, "rows_per_theta": ctx.rows, "n_data": wl.n_data,
@@ -318,8 +361,7 @@ def run_nsgpu(args, rank, world, local_rank):
             "cpu_baseline": {"value": cpu_v, "unit": UNIT, "cores": oracle_threads(), "kind": "oracle",
                              "sample": f"{cpu_n} of {B} thetas, {cpu_dt:.1f} s, fp64 numpy oracle as it stands"}}))
     ctx.close()
-    if dist is not None:
-        dist.destroy_process_group()
+    ranks.close()
 
 
 def main():
@@ -332,11 +374,14 @@ def main():
     ap.add_argument("--batch", type=int, default=4096)
     ap.add_argument("--cpu-sample", type=int, default=768)
     ap.add_argument("--ref-sample", type=int, default=128)
+    ap.add_argument("--dry-run-cpu", action="store_true", help=argparse.SUPPRESS)
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-    if args.impl == "reference":
+    if args.dry_run_cpu:
+        run_dry_cpu(args, rank, world)
+    elif args.impl == "reference":
         run_reference(args, rank)
     else:
         run_nsgpu(args, rank, world, local_rank)

@@ -1,0 +1,32 @@
+"""-m "not gpu": the multi-rank plumbing of bench.py (one process per GPU, barrier, max over ranks, rank 0
+prints one JSON line) under torchrun with the gloo backend, world_size 2."""
+import json
+import os
+import subprocess
+import sys
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _torchrun(extra, port):
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2", "--master-addr",
+           "127.0.0.1", "--master-port", str(port), os.path.join(ROOT, "bench.py"), "--gpus", "2", "--steps", "3",
+           "--warmup", "1"] + extra
+    out = subprocess.run(cmd, cwd=ROOT, capture_output=True, text=True, timeout=300)
+    assert out.returncode == 0, out.stderr[-2000:]
+    return [json.loads(l) for l in out.stdout.splitlines() if l.startswith("{")]
+
+
+def test_two_ranks_weak_scaling_max_over_ranks():
+    lines = _torchrun(["--dry-run-cpu", "--batch", "4096"], 29611)
+    assert len(lines) == 1                              # rank 0 alone prints
+    j = lines[0]
+    assert j["n_gpus"] == 2 and j["scaling"] == "weak" and j["steps"] == 3
+    # rank 1 sleeps 20 ms per step: the slowest rank sets the time, both ranks' thetas count
+    assert 19.0 <= j["ms_per_step"] <= 60.0
+    assert abs(j["value"] - 2 * 4096 * 3 / (j["ms_per_step"] * 3 * 1e-3)) < 1e-6 * j["value"]
+
+
+def test_reference_arm_prints_from_rank0_only():
+    lines = _torchrun(["--impl", "reference", "--workload", "c0", "--ref-sample", "8"], 29612)
+    assert len(lines) == 1 and lines[0]["impl"] == "reference" and lines[0]["cpu_baseline"]["kind"] == "oracle"
