@@ -34,18 +34,21 @@ __global__ void __launch_bounds__(MAXT) chi2_kernel(const double* __restrict__ m
   extern __shared__ __align__(16) unsigned char smem_raw[];
   double* r = reinterpret_cast<double*>(smem_raw);       // [n][TB]
   double* part = r + (size_t)n * TB;                     // [32][TB] per-warp partial chi^2
-  unsigned long long* bars = reinterpret_cast<unsigned long long*>(part + 32 * TB);   // full[2], empty[2]
-  double* S = reinterpret_cast<double*>(bars + 4);       // [2][CH][n], 16-byte aligned (n TB even)
+  constexpr int NBUF = 4;                                // factor chunks in flight: copy latency, not bandwidth, bounds a CTA
+  unsigned long long* bars = reinterpret_cast<unsigned long long*>(part + 32 * TB);   // full[NBUF], empty[NBUF]
+  double* S = reinterpret_cast<double*>(bars + 2 * NBUF);  // [NBUF][CH][n], 16-byte aligned (n TB even)
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarp = blockDim.x >> 5;
-  const uint32_t full0 = tc::smem_u32(bars), empty0 = full0 + 16;
+  const uint32_t full0 = tc::smem_u32(bars), empty0 = full0 + 8 * NBUF;
   const int n_chunks = (n + CH - 1) / CH;
   if (tid == 0) {
-    tc::mbar_init(full0, 1); tc::mbar_init(full0 + 8, 1);
-    tc::mbar_init(empty0, nwarp); tc::mbar_init(empty0 + 8, nwarp);
+    for (int b = 0; b < NBUF; ++b) { tc::mbar_init(full0 + 8 * b, 1); tc::mbar_init(empty0 + 8 * b, nwarp); }
     tc::fence_barrier_init();
-    const uint32_t bytes = ((uint32_t)min(CH, n) * n * 8u + 15u) & ~15u;   // LinvT has 2 doubles of padding
-    tc::mbar_arrive_expect_tx(full0, bytes);
-    tc::bulk_load(tc::smem_u32(S), LinvT, bytes, full0);
+    for (int c = 0; c < NBUF - 1 && c < n_chunks; ++c) {     // prologue: NBUF-1 chunks in flight
+      const int j1 = c * CH;
+      const uint32_t bytes = ((uint32_t)min(CH, n - j1) * n * 8u + 15u) & ~15u;   // LinvT has 2 doubles of padding
+      tc::mbar_arrive_expect_tx(full0 + 8 * c, bytes);
+      tc::bulk_load(tc::smem_u32(S + (size_t)c * CH * n), LinvT + (size_t)j1 * n, bytes, full0 + 8 * c);
+    }
   }
   // residuals, transposed into [j][theta] (coalesced global reads along j)
   for (int i = tid; i < n * TB; i += blockDim.x) {
@@ -66,15 +69,15 @@ __global__ void __launch_bounds__(MAXT) chi2_kernel(const double* __restrict__ m
 #pragma unroll
   for (int t = 0; t < TG; ++t) { wa[t] = 0.0; wb[t] = 0.0; }
   for (int c = 0; c < n_chunks; ++c) {
-    const int buf = c & 1;
-    if (tid == 0 && c + 1 < n_chunks) {                    // prefetch the next chunk into the other buffer
-      const int nb = buf ^ 1, j1 = (c + 1) * CH;
-      if (c >= 1) tc::mbar_wait(empty0 + 8 * nb, ((c - 1) >> 1) & 1);
+    const int buf = c % NBUF;
+    if (tid == 0 && c + NBUF - 1 < n_chunks) {             // refill the buffer chunk c-1 used
+      const int cn = c + NBUF - 1, nb = cn % NBUF, j1 = cn * CH;
+      if (c >= 1) tc::mbar_wait(empty0 + 8 * nb, ((c - 1) / NBUF) & 1);
       const uint32_t bytes = ((uint32_t)min(CH, n - j1) * n * 8u + 15u) & ~15u;
       tc::mbar_arrive_expect_tx(full0 + 8 * nb, bytes);
       tc::bulk_load(tc::smem_u32(S + (size_t)nb * CH * n), LinvT + (size_t)j1 * n, bytes, full0 + 8 * nb);
     }
-    tc::mbar_wait(full0 + 8 * buf, (c >> 1) & 1);
+    tc::mbar_wait(full0 + 8 * buf, (c / NBUF) & 1);
     const double* Sb = S + (size_t)buf * CH * n;
     const int j0 = c * CH, jn = min(CH, n - j0);
     if (j0 <= jb_end) {
@@ -144,28 +147,38 @@ nsgpu_status chi2_loglike(nsgpu_ctx* ctx, const float* theta, int B, const int* 
   const int n = ctx->n_data;
   const int RT = (((n + 1) / 2 + 31) / 32) * 32;        // row-pair threads, whole warps
   if (RT > 1024) { ctx->err = "chi2: n_data > 2048 not supported"; return NSGPU_ESHAPE; }
-  // thetas per thread TG = 8 (each factor element read from shared memory feeds 8 FMAs), G thread
-  // groups per CTA, TB = 8 G thetas per CTA
+  // G thread groups per CTA, TG thetas per thread, TB = G TG thetas per CTA.  Large batches: TG = 8 (each
+  // factor element read from shared memory feeds 8 FMAs).  Small batches (the nested-sampling rounds):
+  // fewer thetas per CTA so that the grid still covers the SMs.
   const int groups = RT <= 160 ? 4 : (RT <= 320 ? 2 : 1);
-  const int TBv = groups * 8;
-  // chunk of CH factor columns per buffer: two buffers within ~110 KB, CH even
-  int CH = (int)((110 * 1024 / 2) / ((size_t)n * 8));
+  int tg = 8;
+  while (tg > 2 && groups > 1 && (B + groups * tg - 1) / (groups * tg) < ctx->sm_count / 2) tg >>= 1;
+  const int TBv = groups * tg;
+  // chunk of CH factor columns per buffer: four buffers within ~100 KB, CH even
+  int CH = (int)((100 * 1024 / 4) / ((size_t)n * 8));
   CH = std::max(2, std::min(16, CH & ~1));
-  const size_t smem = ((size_t)n * TBv + 32 * TBv + 4) * sizeof(double) + 2 * (size_t)CH * n * sizeof(double);
-  static size_t configured = 0;
-  if (smem > configured) {
-    if (smem > 220 * 1024) { ctx->err = "chi2: tiles exceed shared memory"; return NSGPU_ESHAPE; }
-    NSGPU_CUDA(cudaFuncSetAttribute(chi2_kernel<32, 8, 640>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    NSGPU_CUDA(cudaFuncSetAttribute(chi2_kernel<16, 8, 640>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    NSGPU_CUDA(cudaFuncSetAttribute(chi2_kernel<8, 8, 1024>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    configured = smem;
-  }
+  const size_t smem = ((size_t)n * TBv + 32 * TBv + 8) * sizeof(double) + 4 * (size_t)CH * n * sizeof(double);
+  if (smem > 220 * 1024) { ctx->err = "chi2: tiles exceed shared memory"; return NSGPU_ESHAPE; }
   StageTimer tm(ctx, 5, st);
   const int grid = (B + TBv - 1) / TBv, threads = groups * RT;
 #define NSGPU_CHI2_ARGS ctx->model, ctx->data, ctx->Linv, n, B, RT, CH, n_rows_dev, theta, ctx->D, ctx->prior_kind, ctx->prior_p0, ctx->prior_p1, ctx->log_norm, logL
-  if (groups == 4) chi2_kernel<32, 8, 640><<<grid, threads, smem, st>>>(NSGPU_CHI2_ARGS);
-  else if (groups == 2) chi2_kernel<16, 8, 640><<<grid, threads, smem, st>>>(NSGPU_CHI2_ARGS);
-  else chi2_kernel<8, 8, 1024><<<grid, threads, smem, st>>>(NSGPU_CHI2_ARGS);
+#define NSGPU_CHI2_LAUNCH(TB_, TG_, MAXT_)                                                                        \
+  do {                                                                                                            \
+    static size_t configured = 0;                                                                                 \
+    if (smem > configured) {                                                                                      \
+      NSGPU_CUDA(cudaFuncSetAttribute(chi2_kernel<TB_, TG_, MAXT_>, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024)); \
+      configured = 220 * 1024;                                                                                    \
+    }                                                                                                             \
+    chi2_kernel<TB_, TG_, MAXT_><<<grid, threads, smem, st>>>(NSGPU_CHI2_ARGS);                                   \
+  } while (0)
+  if (groups == 4 && tg == 8) NSGPU_CHI2_LAUNCH(32, 8, 640);
+  else if (groups == 4 && tg == 4) NSGPU_CHI2_LAUNCH(16, 4, 640);
+  else if (groups == 4) NSGPU_CHI2_LAUNCH(8, 2, 640);
+  else if (groups == 2 && tg == 8) NSGPU_CHI2_LAUNCH(16, 8, 640);
+  else if (groups == 2 && tg == 4) NSGPU_CHI2_LAUNCH(8, 4, 640);
+  else if (groups == 2) NSGPU_CHI2_LAUNCH(4, 2, 640);
+  else NSGPU_CHI2_LAUNCH(8, 8, 1024);
+#undef NSGPU_CHI2_LAUNCH
 #undef NSGPU_CHI2_ARGS
   NSGPU_LAUNCH_CHECK();
   return NSGPU_OK;

@@ -209,6 +209,7 @@ __global__ void __launch_bounds__(SHEAR_THREADS, 2) shear_project_kernel(const f
   double* Pg = scr;                                           // [n_ell][nqp]
   const int n_lookup = A.n_ell * nq;
   const double inv_dlk = 1.0 / A.dlk, bar_amp = (eta0 - 0.7) * 0.1;
+  const bool vec_taps = A.sz == 1 && A.n_tap == A.n_z_emu && (A.n_tap & 3) == 0 && bulk;   // tap_start == 0 for all q
 #pragma unroll 2
   for (int it = tid; it < n_lookup; it += blockDim.x) {
     const int bl = (int)__umulhi((unsigned)it, nq_magic), q = it - bl * nq;
@@ -222,11 +223,26 @@ __global__ void __launch_bounds__(SHEAR_THREADS, 2) shear_project_kernel(const f
       const int m0 = A.tap_start[q];
       const double* tw = A.tap_w + (size_t)q * A.n_tap;
       double lo = 0.0, hi = 0.0;
-      for (int t = 0; t < A.n_tap; ++t) {
-        const float* row = table + (size_t)(m0 + t) * A.sz + (size_t)j * A.sk;
-        const double w = tw[t];
-        lo = fma(w, (double)row[0], lo);
-        hi = fma(w, (double)row[A.sk], hi);
+      if (vec_taps) {
+        // [k][z] table, taps = all emulator nodes (spline folded in): the taps of one k are contiguous
+        const float4* r0 = reinterpret_cast<const float4*>(table + (size_t)j * A.sk);
+        const float4* r1 = reinterpret_cast<const float4*>(table + (size_t)(j + 1) * A.sk);
+        const double2* tw2 = reinterpret_cast<const double2*>(tw);
+        for (int t4 = 0; t4 < A.n_tap / 4; ++t4) {
+          const float4 a = r0[t4], c = r1[t4];
+          const double2 w01 = __ldg(tw2 + 2 * t4), w23 = __ldg(tw2 + 2 * t4 + 1);
+          lo = fma(w01.x, (double)a.x, lo); lo = fma(w01.y, (double)a.y, lo);
+          lo = fma(w23.x, (double)a.z, lo); lo = fma(w23.y, (double)a.w, lo);
+          hi = fma(w01.x, (double)c.x, hi); hi = fma(w01.y, (double)c.y, hi);
+          hi = fma(w23.x, (double)c.z, hi); hi = fma(w23.y, (double)c.w, hi);
+        }
+      } else {
+        for (int t = 0; t < A.n_tap; ++t) {
+          const float* row = table + (size_t)(m0 + t) * A.sz + (size_t)j * A.sk;
+          const double w = tw[t];
+          lo = fma(w, (double)row[0], lo);
+          hi = fma(w, (double)row[A.sk], hi);
+        }
       }
       double y = (1.0 - s) * lo + s * hi;
       const double k2 = k * k;
