@@ -158,6 +158,7 @@ nsgpu_status build_shear(nsgpu_ctx* ctx, const nsgpu_theory* t) {
   NSGPU_CUDA(upload(&S.ell, t->ell, (size_t)t->n_ell));
   NSGPU_CUDA(upload(&S.nz_mean, t->nz_mean, (size_t)t->n_tomo));
   NSGPU_CUDA(upload(&ctx->z_emu, zef.data(), zef.size()));
+  NSGPU_CUDA(cudaMalloc((void**)&S.aux, (size_t)ctx->max_batch * (3 + t->n_tomo) * t->n_chi * sizeof(double)));
   return NSGPU_OK;
 }
 
@@ -372,7 +373,7 @@ extern "C" nsgpu_status nsgpu_destroy(nsgpu_ctx* ctx) {
   cudaFree(ctx->emu_in_idx); cudaFree(ctx->emu_in_const); cudaFree(ctx->z_emu);
   cudaFree(ctx->bin_ptr); cudaFree(ctx->bin_col); cudaFree(ctx->bin_val);
   ShearDev& S = ctx->sh;
-  cudaFree(S.a_q); cudaFree(S.z_q); cudaFree(S.ln1pz); cudaFree(S.lellh); cudaFree(S.lf); cudaFree(S.tap_start); cudaFree(S.tap_w); cudaFree(S.ell); cudaFree(S.nz_mean);
+  cudaFree(S.aux); cudaFree(S.a_q); cudaFree(S.z_q); cudaFree(S.ln1pz); cudaFree(S.lellh); cudaFree(S.lf); cudaFree(S.tap_start); cudaFree(S.tap_w); cudaFree(S.ell); cudaFree(S.nz_mean);
   cudaFree(ctx->data); cudaFree(ctx->Linv);
   cudaFree(ctx->act[0]); cudaFree(ctx->act[1]); cudaFree(ctx->spec); cudaFree(ctx->model);
   cudaFree(ctx->theta_stage); cudaFree(ctx->logL_stage);

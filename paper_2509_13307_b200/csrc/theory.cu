@@ -91,10 +91,18 @@ struct ShearArgs {
 // One CTA per theta.  Thread 0 starts a bulk asynchronous copy (TMA, cp.async.bulk) of this theta's
 // log10 P table into shared memory -- the kernel's only large HBM read -- and the CTA computes the
 // background and the windows (which do not need the table) while it lands.
+//
+// PHASE 0: everything in one launch (fallback for grids whose scratch arrays are not 16-byte sized).
+// PHASE 1: background + windows only (a6, a7), no table: many CTAs per SM; writes gq, log10 chi, 1/chi and the
+//          total windows to `aux` [(3 + n_tomo) n_chi doubles per theta].
+// PHASE 2: table + aux by bulk copy, then lookups and Limber sums (a5, a8).  Splitting takes the serial,
+//          table-free prologue out of the kernel whose occupancy the 84 KB table pins at two CTAs per SM.
 constexpr int SHEAR_THREADS = 256;
+template <int PHASE>
 __global__ void __launch_bounds__(SHEAR_THREADS, 2) shear_project_kernel(const float* __restrict__ theta, int D,
                                                                          const int* __restrict__ n_rows_dev,
                                                                          const float* __restrict__ spec, ShearArgs A,
+                                                                         double* __restrict__ aux,
                                                                          double* __restrict__ model, int n_data) {
   const int b = blockIdx.x;
   if (n_rows_dev && b >= *n_rows_dev) return;
@@ -121,16 +129,25 @@ __global__ void __launch_bounds__(SHEAR_THREADS, 2) shear_project_kernel(const f
   const unsigned table_bytes = (unsigned)(A.n_z_emu * A.n_k) * 4u;
   const bool bulk = (table_bytes & 15u) == 0 && ((reinterpret_cast<uintptr_t>(src) & 15) == 0);
   const unsigned bar_s = (unsigned)__cvta_generic_to_shared(bar);
-  if (bulk) {
-    if (tid == 0) {
-      asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar_s) : "memory");
-      asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-      asm volatile("{\n.reg .b64 st;\nmbarrier.arrive.expect_tx.shared::cta.b64 st, [%0], %1;\n}" ::"r"(bar_s), "r"(table_bytes) : "memory");
-      asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                   ::"r"((unsigned)__cvta_generic_to_shared(table)), "l"(src), "r"(table_bytes), "r"(bar_s) : "memory");
+  const unsigned aux_bytes = (unsigned)((3 + nt) * nq) * 8u;   // gq, hs, ichi, Wt are contiguous in shared memory
+  const double* aux_b = aux + (size_t)b * (3 + nt) * nq;
+  if (PHASE != 1) {
+    if (bulk) {
+      if (tid == 0) {
+        const unsigned total = table_bytes + (PHASE == 2 ? aux_bytes : 0u);
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar_s) : "memory");
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("{\n.reg .b64 st;\nmbarrier.arrive.expect_tx.shared::cta.b64 st, [%0], %1;\n}" ::"r"(bar_s), "r"(total) : "memory");
+        asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                     ::"r"((unsigned)__cvta_generic_to_shared(table)), "l"(src), "r"(table_bytes), "r"(bar_s) : "memory");
+        if (PHASE == 2)
+          asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                       ::"r"((unsigned)__cvta_generic_to_shared(gq)), "l"(aux_b), "r"(aux_bytes), "r"(bar_s) : "memory");
+      }
+    } else {
+      for (int i = tid; i < A.n_z_emu * A.n_k; i += blockDim.x) table[i] = __ldg(src + i);
     }
-  } else {
-    for (int i = tid; i < A.n_z_emu * A.n_k; i += blockDim.x) table[i] = __ldg(src + i);
+    if (PHASE == 2) __syncthreads();   // the mbarrier is initialised before anyone polls it
   }
   const double ob = th[A.idx_omega_b], oc = th[A.idx_omega_cdm], h = th[A.idx_h];
   const double Om = (ob + oc) / (h * h);
@@ -140,6 +157,7 @@ __global__ void __launch_bounds__(SHEAR_THREADS, 2) shear_project_kernel(const f
   const double gam = 0.55 + 0.05 * (1.0 + w0 + 0.5 * wa);
   const double de_exp = 3.0 * (1.0 + w0 + wa);
 
+  if (PHASE != 2) {
   // a6: E_q; f_q da and the growth integrand go to the scan arrays
   double* sc_f = scr;
   double* sc_g = scr + nqp;
@@ -198,7 +216,12 @@ __global__ void __launch_bounds__(SHEAR_THREADS, 2) shear_project_kernel(const f
     if (i == 0) hs[q] = log10(chi[q]);
   }
   __syncthreads();
-  if (bulk) {   // the table has landed?
+  if (PHASE == 1) {   // hand gq, log10 chi, 1/chi and the windows to the table kernel
+    for (int i = tid; i < (3 + nt) * nq; i += blockDim.x) aux[(size_t)b * (3 + nt) * nq + i] = gq[i];
+    return;
+  }
+  }   // PHASE != 2
+  if (bulk) {   // the table (and aux) have landed?
     unsigned ok = 0;
     while (!ok)
       asm volatile("{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], 0;\nselp.u32 %0, 1, 0, p;\n}"
@@ -359,13 +382,25 @@ nsgpu_status shear_project(nsgpu_ctx* ctx, const float* theta, int B, const int*
   A.idx_omega_b = S.idx_omega_b; A.idx_omega_cdm = S.idx_omega_cdm; A.idx_h = S.idx_h; A.idx_w0 = S.idx_w0;
   A.idx_wa = S.idx_wa; A.idx_eta0 = S.idx_eta0; A.idx_dz = S.idx_dz; A.idx_ia = S.idx_ia; A.idx_m = S.idx_m;
   const size_t smem = shear_smem_bytes(S);
+  const size_t smem1 = smem - (size_t)S.n_z_emu * S.n_k * sizeof(float);       // phase 1 stages no table
   static size_t configured = 0;
   if (smem > configured) {
-    NSGPU_CUDA(cudaFuncSetAttribute(shear_project_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    NSGPU_CUDA(cudaFuncSetAttribute(shear_project_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    NSGPU_CUDA(cudaFuncSetAttribute(shear_project_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    NSGPU_CUDA(cudaFuncSetAttribute(shear_project_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     configured = smem;
   }
+  // the two-kernel split needs 16-byte sized / aligned pieces for the bulk copies
+  const bool split = ((size_t)S.n_z_emu * S.n_k * 4) % 16 == 0 && ((size_t)(3 + S.n_tomo) * S.n_chi * 8) % 16 == 0 &&
+                     ((size_t)3 * S.n_chi * 8) % 16 == 0 && S.aux != nullptr;
   StageTimer tm(ctx, 3, st);
-  shear_project_kernel<<<B, SHEAR_THREADS, smem, st>>>(theta, ctx->D, n_rows_dev, ctx->spec, A, ctx->model, ctx->n_data);
+  if (split) {
+    shear_project_kernel<1><<<B, 128, smem1, st>>>(theta, ctx->D, n_rows_dev, ctx->spec, A, S.aux, ctx->model, ctx->n_data);
+    NSGPU_LAUNCH_CHECK();
+    shear_project_kernel<2><<<B, SHEAR_THREADS, smem, st>>>(theta, ctx->D, n_rows_dev, ctx->spec, A, S.aux, ctx->model, ctx->n_data);
+  } else {
+    shear_project_kernel<0><<<B, SHEAR_THREADS, smem, st>>>(theta, ctx->D, n_rows_dev, ctx->spec, A, S.aux, ctx->model, ctx->n_data);
+  }
   NSGPU_LAUNCH_CHECK();
   return NSGPU_OK;
 }
