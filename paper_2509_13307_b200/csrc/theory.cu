@@ -33,18 +33,17 @@ __device__ __forceinline__ double exp_fast(double x) {
   const double n = rint(x * 1.4426950408889634);
   double r = fma(n, -6.93147180369123816490e-01, x);
   r = fma(n, -1.90821492927058770002e-10, r);
-  double p = 2.505210838544172e-08;           // 1/11!
-  p = fma(p, r, 2.755731922398589e-07);       // 1/10!
-  p = fma(p, r, 2.7557319223985893e-06);      // 1/9!
-  p = fma(p, r, 2.48015873015873e-05);        // 1/8!
-  p = fma(p, r, 1.984126984126984e-04);       // 1/7!
-  p = fma(p, r, 1.3888888888888889e-03);      // 1/6!
-  p = fma(p, r, 8.333333333333333e-03);       // 1/5!
-  p = fma(p, r, 4.1666666666666664e-02);      // 1/4!
-  p = fma(p, r, 1.6666666666666666e-01);      // 1/3!
-  p = fma(p, r, 0.5);
-  p = fma(p, r, 1.0);
-  p = fma(p, r, 1.0);
+  // Estrin evaluation of sum_{i<=11} r^i / i!: dependency depth 4 instead of the 11 of Horner's rule (the
+  // lookups are latency-bound: 16 warps per SM)
+  const double r2 = r * r, r4 = r2 * r2, r8 = r4 * r4;
+  const double a0 = fma(r, 1.0, 1.0);
+  const double a1 = fma(r, 1.6666666666666666e-01, 0.5);
+  const double a2 = fma(r, 8.333333333333333e-03, 4.1666666666666664e-02);
+  const double a3 = fma(r, 1.984126984126984e-04, 1.3888888888888889e-03);
+  const double a4 = fma(r, 2.7557319223985893e-06, 2.48015873015873e-05);
+  const double a5 = fma(r, 2.505210838544172e-08, 2.755731922398589e-07);
+  const double b0 = fma(a1, r2, a0), b1 = fma(a3, r2, a2), b2 = fma(a5, r2, a4);
+  const double p = fma(b2, r8, fma(b1, r4, b0));
   const int e = (int)n;
   return __hiloint2double(__double2hiint(p) + (e << 20), __double2loint(p));
 }
@@ -230,49 +229,62 @@ __global__ void __launch_bounds__(SHEAR_THREADS, 2) shear_project_kernel(const f
 
   // a5 + a8 (lookup): P(k = (ell+1/2)/chi_q, z_q) g_q for every (ell, q); log10 k = log10(ell+1/2) - log10 chi
   double* Pg = scr;                                           // [n_ell][nqp]
-  const int n_lookup = A.n_ell * nq;
   const double inv_dlk = 1.0 / A.dlk, bar_amp = (eta0 - 0.7) * 0.1;
   const bool vec_taps = A.sz == 1 && A.n_tap == A.n_z_emu && (A.n_tap & 3) == 0 && bulk;   // tap_start == 0 for all q
+  // Work item = (quadrature node q, group of 4 ell): the per-node quantities (1/chi, log10 chi, g_q, the z taps)
+  // are loaded once and serve four lookups; consecutive lanes have consecutive q.
+  const int n_lg4 = (A.n_ell + 3) >> 2;
+  for (int item = tid; item < n_lg4 * nq; item += blockDim.x) {
+    const int lg = (int)__umulhi((unsigned)item, nq_magic), q = item - lg * nq;
+    const double ic = ichi[q], lc = hs[q], g_q = gq[q];
+    const int m0 = A.tap_start[q];
+    const double* tw = A.tap_w + (size_t)q * A.n_tap;
+    const double tw0 = tw[0], tw1 = A.n_tap > 1 ? tw[1] : 0.0;
+    const float* col0 = table + (size_t)m0 * A.sz;             // two-tap fast path: rows m0, m0 + 1
 #pragma unroll 2
-  for (int it = tid; it < n_lookup; it += blockDim.x) {
-    const int bl = (int)__umulhi((unsigned)it, nq_magic), q = it - bl * nq;
-    const double k = (A.ell[bl] + 0.5) * ichi[q];
-    double P = 0.0;
-    if (k >= A.k_min && k <= A.k_max) {
-      const double x = A.lellh[bl] - hs[q];
-      int j = (int)floor((x - A.lk0) * inv_dlk);
-      j = min(max(j, 0), A.n_k - 2);
-      const double s = (x - (A.lk0 + j * A.dlk)) * inv_dlk;
-      const int m0 = A.tap_start[q];
-      const double* tw = A.tap_w + (size_t)q * A.n_tap;
-      double lo = 0.0, hi = 0.0;
-      if (vec_taps) {
-        // [k][z] table, taps = all emulator nodes (spline folded in): the taps of one k are contiguous
-        const float4* r0 = reinterpret_cast<const float4*>(table + (size_t)j * A.sk);
-        const float4* r1 = reinterpret_cast<const float4*>(table + (size_t)(j + 1) * A.sk);
-        const double2* tw2 = reinterpret_cast<const double2*>(tw);
-        for (int t4 = 0; t4 < A.n_tap / 4; ++t4) {
-          const float4 a = r0[t4], c = r1[t4];
-          const double2 w01 = __ldg(tw2 + 2 * t4), w23 = __ldg(tw2 + 2 * t4 + 1);
-          lo = fma(w01.x, (double)a.x, lo); lo = fma(w01.y, (double)a.y, lo);
-          lo = fma(w23.x, (double)a.z, lo); lo = fma(w23.y, (double)a.w, lo);
-          hi = fma(w01.x, (double)c.x, hi); hi = fma(w01.y, (double)c.y, hi);
-          hi = fma(w23.x, (double)c.z, hi); hi = fma(w23.y, (double)c.w, hi);
+    for (int u = 0; u < 4; ++u) {
+      const int bl = 4 * lg + u;
+      if (bl >= A.n_ell) break;
+      const double k = (A.ell[bl] + 0.5) * ic;
+      double P = 0.0;
+      if (k >= A.k_min && k <= A.k_max) {
+        const double x = A.lellh[bl] - lc;
+        int j = (int)floor((x - A.lk0) * inv_dlk);
+        j = min(max(j, 0), A.n_k - 2);
+        const double s = (x - (A.lk0 + j * A.dlk)) * inv_dlk;
+        double lo = 0.0, hi = 0.0;
+        if (vec_taps) {
+          // [k][z] table, taps = all emulator nodes (spline folded in): the taps of one k are contiguous
+          const float4* r0 = reinterpret_cast<const float4*>(table + (size_t)j * A.sk);
+          const float4* r1 = reinterpret_cast<const float4*>(table + (size_t)(j + 1) * A.sk);
+          const double2* tw2 = reinterpret_cast<const double2*>(tw);
+          for (int t4 = 0; t4 < A.n_tap / 4; ++t4) {
+            const float4 a = r0[t4], c = r1[t4];
+            const double2 w01 = __ldg(tw2 + 2 * t4), w23 = __ldg(tw2 + 2 * t4 + 1);
+            lo = fma(w01.x, (double)a.x, lo); lo = fma(w01.y, (double)a.y, lo);
+            lo = fma(w23.x, (double)a.z, lo); lo = fma(w23.y, (double)a.w, lo);
+            hi = fma(w01.x, (double)c.x, hi); hi = fma(w01.y, (double)c.y, hi);
+            hi = fma(w23.x, (double)c.z, hi); hi = fma(w23.y, (double)c.w, hi);
+          }
+        } else if (A.n_tap == 2) {
+          const float* r0 = col0 + (size_t)j * A.sk;
+          lo = fma(tw1, (double)r0[A.sz], tw0 * (double)r0[0]);
+          hi = fma(tw1, (double)r0[A.sk + A.sz], tw0 * (double)r0[A.sk]);
+        } else {
+          for (int t = 0; t < A.n_tap; ++t) {
+            const float* row = table + (size_t)(m0 + t) * A.sz + (size_t)j * A.sk;
+            const double w = tw[t];
+            lo = fma(w, (double)row[0], lo);
+            hi = fma(w, (double)row[A.sk], hi);
+          }
         }
-      } else {
-        for (int t = 0; t < A.n_tap; ++t) {
-          const float* row = table + (size_t)(m0 + t) * A.sz + (size_t)j * A.sk;
-          const double w = tw[t];
-          lo = fma(w, (double)row[0], lo);
-          hi = fma(w, (double)row[A.sk], hi);
-        }
+        double y = fma(s, hi - lo, lo);
+        const double k2 = k * k;
+        y -= bar_amp * k2 * rcp_fast(k2 + 1.0);
+        P = exp_fast(y * 2.302585092994046);
       }
-      double y = (1.0 - s) * lo + s * hi;
-      const double k2 = k * k;
-      y -= bar_amp * k2 * rcp_fast(k2 + 1.0);
-      P = exp_fast(y * 2.302585092994046);
+      Pg[(size_t)bl * nqp + q] = P * g_q;
     }
-    Pg[(size_t)bl * nqp + q] = P * gq[q];
   }
   __syncthreads();
 
