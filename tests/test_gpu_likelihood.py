@@ -146,3 +146,40 @@ def test_restricted_lcdm_matches_w0wa_at_minus1_0():
         a = cf.theory_batch(dev(tf)).cpu().numpy()
         b = cr.theory_batch(dev(tr)).cpu().numpy()
     np.testing.assert_array_equal(a, b)
+
+
+@pytest.mark.parametrize("width,n_hidden,n_out,B", [(64, 1, 7, 1), (192, 2, 33, 127), (256, 3, 100, 129), (320, 2, 9, 260),
+                                                    (512, 1, 420, 131)])
+def test_tensor_core_path_odd_shapes(width, n_hidden, n_out, B):
+    """tcgen05 path on shapes off the benchmark grid: K = 64..512 (1..8 k-blocks), fan-out not a multiple of the
+    tile or of 8, one hidden layer (no hidden GEMM at all), row counts with ragged 128-row tails, B = 1."""
+    wl = W.toy(seed=4000 + width, width=width, n_out=n_out, n_hidden=n_hidden)
+    th0 = theta_of_u(wl, wl.u_fid[None]).astype(np.float64)
+    W.attach_toy_data(wl, LK.theory(wl, th0)[0])
+    theta = theta_of_u(wl, W.u_prior_set(wl, B))
+    with nsgpu.Context(wl, max_batch=B, mlp=nsgpu.MLP_TC) as ctx:
+        assert ctx.mlp_path(0) == 1
+        t = dev(theta)
+        got = ctx.emulate_batch(t, 0).cpu().numpy().astype(np.float64)
+        ll = ctx.loglike_batch(t).cpu().numpy()
+    ref = LK.emulate(wl, theta.astype(np.float64), 0)
+    assert emulator_rel_err(got, ref, 0) <= 1e-4
+    ref_ll = LK.loglike(wl, theta.astype(np.float64))
+    chi2 = -2.0 * (ref_ll - gaussian.log_norm(wl.chol))
+    assert np.all(np.abs(ll - ref_ll) <= loglike_tolerance(chi2))
+
+
+def test_tensor_core_and_simt_paths_agree_on_shear():
+    """the two on-device MLP paths (different table layouts into the projection) give the same log L"""
+    wl = W.shear(seed=21, w0wa=True, n_z_emu=9, n_z=9, width=64, n_hidden=2, n_k=40, n_chi=24, n_ell=6, n_tomo=3, name="s64")
+    th0 = theta_of_u(wl, wl.u_fid[None]).astype(np.float64)
+    W.attach_data(wl, LK.theory(wl, th0)[0])
+    theta = theta_of_u(wl, np.concatenate([W.u_post_set(wl, 70), W.u_prior_set(wl, 70)]))
+    out = []
+    for mlp in (nsgpu.MLP_SIMT, nsgpu.MLP_TC):
+        with nsgpu.Context(wl, max_batch=140, mlp=mlp) as ctx:
+            out.append(ctx.loglike_batch(dev(theta)).cpu().numpy())
+    ref = LK.loglike(wl, theta.astype(np.float64))
+    chi2 = -2.0 * (ref - gaussian.log_norm(wl.chol))
+    for o in out:
+        assert np.all(np.abs(o - ref) <= loglike_tolerance(chi2))
