@@ -2,9 +2,9 @@
 evaluation the paper calls the primary bottleneck; steps a2-a10)."""
 import numpy as np
 
-from . import cmb, emulator, gaussian, prior, shear
+from . import cmb, cmb_tt, emulator, gaussian, prior, shear
 
-IDENTITY, EMULATOR, CMB_BINNED, SHEAR_LIMBER = 0, 1, 2, 3
+IDENTITY, EMULATOR, CMB_BINNED, SHEAR_LIMBER, CMB_TT_CV = 0, 1, 2, 3, 4
 
 
 def _emu_theta_inputs(th, theta):
@@ -31,7 +31,7 @@ def theory(wl, theta):
     B = len(theta)
     if th.kind == IDENTITY:
         return theta.copy()
-    if th.kind == EMULATOR:
+    if th.kind in (EMULATOR, CMB_TT_CV):
         return emulator.mlp_forward(wl.emulators[0], _emu_theta_inputs(th, theta))
     if th.kind == CMB_BINNED:
         X = _emu_theta_inputs(th, theta)
@@ -52,7 +52,10 @@ def loglike(wl, theta):
     out = np.full(len(theta), -np.inf)
     if np.any(ok):
         model = theory(wl, theta[ok])
-        ll = gaussian.loglike(wl.chol, model, wl.data)
+        if wl.theory.kind == CMB_TT_CV:      # per-multipole chi^2_{2l+1} likelihood, no covariance
+            ll = cmb_tt.loglike_spectrum(cmb_tt.ells(wl.theory, wl.n_data), wl.data, model)
+        else:
+            ll = gaussian.loglike(wl.chol, model, wl.data)
         ll[~np.isfinite(ll)] = -np.inf
         out[ok] = ll
     return out

@@ -25,6 +25,7 @@ THEORY_IDENTITY = 0
 THEORY_EMULATOR = 1
 THEORY_CMB_BINNED = 2
 THEORY_SHEAR_LIMBER = 3
+THEORY_CMB_TT_CV = 4     # the paper's cosmic-variance TT likelihood: chi^2_{2l+1} per multipole
 
 PRIOR_UNIFORM = 0
 PRIOR_GAUSSIAN = 1
@@ -67,6 +68,8 @@ class Theory:
     bin_col: Optional[np.ndarray] = None    # int32 [nnz], columns in [0, n_spec*n_out)
     bin_val: Optional[np.ndarray] = None    # float32 [nnz]
     cal_index: int = -1
+    # --- cmb_tt_cv ---
+    ell_min: int = 2
     # --- shear_limber ---
     n_z_emu: int = 0
     n_z: int = 0
@@ -284,6 +287,38 @@ def cmb(seed: int = 1001, width: int = 512, n_hidden: int = 4, ell_max: int = 25
     theta_fid = [0.02242, 0.11933, 0.6766, 0.0544, 0.9665, 3.047, 1.0]
     return Workload("c1_cmb", seed, D, kind, p0, p1, emus, th, n_data,
                     _u_of_theta(rows, theta_fid), names)
+
+
+def cmb_tt(seed: int = 1005, width: int = 512, n_hidden: int = 4, ell_max: int = 2508) -> Workload:
+    """The paper's CMB run: 6 cosmological parameters on the Table-1 box (tau per reading
+    C4), one TT emulator 6 -> 4 x 512 -> 2507 (l = 2..2508), cosmic-variance likelihood, no covariance.
+    `chol` stays None; `data` = observed C_l (attach_cmb_tt_data)."""
+    rng = np.random.default_rng(seed)
+    rows = [(PRIOR_UNIFORM, 0.01875, 0.02625), (PRIOR_UNIFORM, 0.05, 0.255), (PRIOR_UNIFORM, 0.64, 0.982),
+            (PRIOR_UNIFORM, 0.01, 0.15), (PRIOR_UNIFORM, 0.84, 1.1), (PRIOR_UNIFORM, 1.61, 3.91)]
+    names = ["omega_b", "omega_cdm", "h", "tau", "n_s", "lnAs"]
+    D = len(rows)
+    kind, p0, p1 = _prior_arrays(rows)
+    mu_in, sd_in = _in_standardisation(rows)
+    n_out = ell_max - 1
+    ell = np.arange(2, ell_max + 1, dtype=np.float64)
+    mu_out = -9.0 - 2.0 * np.log10(np.maximum(ell, 100.0) / 100.0)
+    # a cosmic-variance likelihood over 2507 multipoles is razor sharp: sigma_out = 0.01 keeps the synthetic
+    # posterior a finite fraction of the prior box (random weights have no physical smoothness in l)
+    emu = make_emulator(rng, D, n_hidden, width, n_out, OUT_EXP10, mu_in, sd_in, mu_out, np.full(n_out, 0.01))
+    th = Theory(kind=THEORY_CMB_TT_CV, emu_in_idx=np.arange(D, dtype=np.int32), emu_in_const=np.zeros(D), ell_min=2)
+    theta_fid = [0.02242, 0.11933, 0.6766, 0.0544, 0.9665, 3.047]
+    return Workload("cmb_tt_cv", seed, D, kind, p0, p1, [emu], th, n_out, _u_of_theta(rows, theta_fid), names)
+
+
+def attach_cmb_tt_data(wl: Workload, model_fid: np.ndarray, noise: bool = True) -> Workload:
+    """observed spectrum: C_l(theta_0) x chi^2_{2l+1} / (2l+1) (a cosmic-variance draw), or noise-free."""
+    rng = np.random.default_rng(wl.seed + 77)
+    nu = 2.0 * (wl.theory.ell_min + np.arange(wl.n_data)) + 1.0
+    c0 = np.asarray(model_fid, np.float64)
+    wl.data = c0 * (rng.chisquare(nu) / nu if noise else 1.0)
+    wl.chol = None
+    return wl
 
 
 # ----------------------------------------------------------------------------------------
