@@ -37,7 +37,7 @@ from paper_2509_13307_b200 import workloads as W  # noqa: E402
 
 METRIC = "likelihood evals/sec at batch 4096 (39-D shear); % tensor/HBM roofline"
 UNIT = "evals/s"
-MAKERS = {"c0": W.toy, "c1": W.cmb, "c2": W.c2, "c3a": W.c3a, "c3b": W.c3b}
+MAKERS = {"c0": W.toy, "c1": W.cmb, "c2": W.c2, "c3a": W.c3a, "c3b": W.c3b, "cmb_tt": W.cmb_tt}
 
 
 def flops_per_row(em):
@@ -118,11 +118,13 @@ def make_context(nsgpu, torch, wl, batch, device):
     """Attach a synthetic data vector made by the CUDA path itself at the fiducial point (the product
     never touches oracle/): first a context with a placeholder Gaussian, then the real one."""
     n = wl.n_data
-    wl.data, wl.chol = np.zeros(n), np.eye(n)
+    wl.data, wl.chol = (np.ones(n), None) if wl.theory.kind == W.THEORY_CMB_TT_CV else (np.zeros(n), np.eye(n))
     with nsgpu.Context(wl, max_batch=8, device=device) as c0:
         u0 = torch.as_tensor(wl.u_fid[None].astype(np.float32), device=f"cuda:{device}")
         m0 = c0.theory_batch(c0.prior_transform(u0)).cpu().numpy()[0]
-    if wl.theory.kind == W.THEORY_EMULATOR:
+    if wl.theory.kind == W.THEORY_CMB_TT_CV:
+        W.attach_cmb_tt_data(wl, m0, noise=True)
+    elif wl.theory.kind == W.THEORY_EMULATOR:
         W.attach_toy_data(wl, m0)
     else:
         W.attach_data(wl, m0, noise=True)
@@ -167,6 +169,8 @@ def attach_oracle_data(wl):
     from oracle import likelihood as LK, prior
     th0 = prior.transform(wl.prior_kind, wl.prior_p0, wl.prior_p1, wl.u_fid[None]).astype(np.float32).astype(np.float64)
     m0 = LK.theory(wl, th0)[0]
+    if wl.theory.kind == W.THEORY_CMB_TT_CV:
+        return W.attach_cmb_tt_data(wl, m0)
     (W.attach_toy_data if wl.theory.kind == W.THEORY_EMULATOR else W.attach_data)(wl, m0)
     return wl
 
@@ -334,7 +338,7 @@ def run_nsgpu(args, rank, world, local_rank):
                     "share_of_step": h_ms / total_stage_ms if total_stage_ms else None,
                     "stage_ms_per_step": {k: v[0] / args.steps for k, v in stages.items() if v[1]}}
         # HBM-bound projection / binning stage beside it
-        proj = "shear_project" if wl.theory.kind == W.THEORY_SHEAR_LIMBER else ("cmb_bin" if wl.theory.kind == W.THEORY_CMB_BINNED else None)
+        proj = "shear_project" if wl.theory.kind == W.THEORY_SHEAR_LIMBER else ("cmb_bin" if wl.theory.kind in (W.THEORY_CMB_BINNED, W.THEORY_CMB_TT_CV) else None)
         if proj and stages[proj][1]:
             p_ms, p_cnt = stages[proj]
             bytes_launch = B * (n_emu * ctx.rows * em.n_out * 4 + wl.n_data * 8 + wl.D * 4)

@@ -80,6 +80,10 @@ typedef struct {
  * kind 3 shear_limber : eqs. A1-A4 on n_chi quadrature nodes evenly spaced in the scale
  *                       factor, the emulated log10 P(k, z) interpolated linearly in z and
  *                       log10 k, optional cubic z-spline n_z_emu -> n_z first (BJ cfg 3b)
+ * kind 4 cmb_tt_cv   : the paper's own CMB likelihood: nu_l Chat_l / C_l ~ chi^2_{nu_l}, nu_l = 2 l + 1,
+ *                       independently per multipole l = ell_min + i; emulator 0 gives C_l = 10^y (out_kind 1),
+ *                       `data` holds the observed Chat_l > 0, n_data = n_out, `chol` is not used (may be NULL);
+ *                       log L = sum_l log[(nu_l / C_l) f_chi2(nu_l Chat_l / C_l; nu_l)]
  * Emulator-input assembly (step a2): emulator input j < n_theta_in is theta[emu_in_idx[j]], or the
  * constant emu_in_const[j] where emu_in_idx[j] < 0; a shear emulator has n_in = n_theta_in + 1, its
  * last input being the redshift of the node.  Other kinds: n_in = n_theta_in.
@@ -94,6 +98,8 @@ typedef struct {
   const int32_t* bin_col; /* [nnz] */
   const float* bin_val;   /* [nnz] */
   int32_t cal_index;
+  /* kind 4 */
+  int32_t ell_min;
   /* kind 3 */
   int32_t n_z_emu, n_z, n_chi, n_k, n_ell, n_tomo;
   int32_t z_interp; /* 0: n_z == n_z_emu, no spline; 2: cubic not-a-knot spline n_z_emu -> n_z */

@@ -166,11 +166,11 @@ nsgpu_status create_impl(nsgpu_ctx* ctx, int32_t D, const nsgpu_prior1d* prior, 
                          const nsgpu_emulator* emu, const nsgpu_theory* th, int32_t n_data, const double* data,
                          const double* chol, int32_t max_batch, int32_t device, uint32_t flags) {
   if (D < 1 || D > NSGPU_MAX_D) { ctx->err = "D must be in [1, 64]"; return NSGPU_ESHAPE; }
-  if (!prior || !th || !data || !chol || n_data < 1 || max_batch < 1 || n_emu < 0 || (n_emu > 0 && !emu)) {
+  if (!prior || !th || !data || (!chol && th->kind != 4) || n_data < 1 || max_batch < 1 || n_emu < 0 || (n_emu > 0 && !emu)) {
     ctx->err = "create: NULL pointer or non-positive size";
     return NSGPU_EINVAL;
   }
-  if (th->kind < 0 || th->kind > 3) { ctx->err = "unknown theory kind"; return NSGPU_EINVAL; }
+  if (th->kind < 0 || th->kind > 4) { ctx->err = "unknown theory kind"; return NSGPU_EINVAL; }
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
     ctx->err = "no CUDA device: nsgpu has no CPU fallback";
@@ -197,7 +197,7 @@ nsgpu_status create_impl(nsgpu_ctx* ctx, int32_t D, const nsgpu_prior1d* prior, 
   NSGPU_CUDA(upload(&ctx->prior_p1, p1.data(), (size_t)D));
 
   // theory-dependent shape checks
-  const int need_emu = th->kind == 0 ? 0 : (th->kind == 2 ? -1 : 1);
+  const int need_emu = th->kind == 0 ? 0 : (th->kind == 2 ? -1 : 1);   // kinds 1, 3, 4: exactly one emulator
   if (need_emu == 0 && n_data != D) { ctx->err = "identity theory needs n_data == D"; return NSGPU_ESHAPE; }
   if (need_emu == 1 && n_emu != 1) { ctx->err = "this theory kind takes exactly one emulator"; return NSGPU_EINVAL; }
   if (need_emu == -1 && (n_emu < 1 || n_emu > 8)) { ctx->err = "cmb_binned takes 1..8 emulators"; return NSGPU_EINVAL; }
@@ -248,9 +248,11 @@ nsgpu_status create_impl(nsgpu_ctx* ctx, int32_t D, const nsgpu_prior1d* prior, 
     NSGPU_CUDA(upload(&E.in_mean, h.in_mean, (size_t)h.n_in));
     NSGPU_CUDA(upload(&E.in_std, h.in_std, (size_t)h.n_in));
     NSGPU_CUDA(upload(&E.out_mean, h.out_mean, (size_t)h.n_out));
+    { std::vector<float> z((size_t)h.n_out, 0.0f); NSGPU_CUDA(upload(&E.out_zero, z.data(), z.size())); }
     NSGPU_CUDA(upload(&E.out_std, h.out_std, (size_t)h.n_out));
   }
-  if (th->kind == 1 && emu[0].n_out != n_data) { ctx->err = "emulator theory needs n_out == n_data"; return NSGPU_ESHAPE; }
+  if ((th->kind == 1 || th->kind == 4) && emu[0].n_out != n_data) { ctx->err = "emulator theory needs n_out == n_data"; return NSGPU_ESHAPE; }
+  if (th->kind == 4 && (emu[0].out_kind != 1 || th->ell_min < 0)) { ctx->err = "cmb_tt_cv needs an exp10 emulator and ell_min >= 0"; return NSGPU_EINVAL; }
   if (th->kind == 3 && emu[0].n_out != th->n_k) { ctx->err = "shear: emulator n_out != n_k"; return NSGPU_ESHAPE; }
   if (th->kind == 2) {
     if (!th->bin_ptr || !th->bin_col || !th->bin_val || th->cal_index < 0 || th->cal_index >= D) {
@@ -267,6 +269,25 @@ nsgpu_status create_impl(nsgpu_ctx* ctx, int32_t D, const nsgpu_prior1d* prior, 
     ctx->cal_index = th->cal_index;
   }
 
+  if (th->kind == 4) {
+    // cosmic-variance TT likelihood: log p_l = const_l - (nu/2) ln C_l - nu Chat_l / (2 C_l) with ln C = y ln 10.
+    // Per multipole the kernel needs a_l = (nu/2) ln 10 and b_l = nu Chat_l / 2; the constants are summed here in fp64.
+    const size_t n = n_data;
+    std::vector<double> ta(n), tb(n);
+    double cst = 0.0;
+    for (size_t i = 0; i < n; ++i) {
+      const double nu = 2.0 * (th->ell_min + (double)i) + 1.0, ch = data[i];
+      if (!(ch > 0.0) || !std::isfinite(ch)) { ctx->err = "cmb_tt_cv: observed spectrum must be positive"; return NSGPU_EINVAL; }
+      ta[i] = 0.5 * nu * log(10.0);
+      tb[i] = 0.5 * nu * ch;
+      cst += log(nu) + (0.5 * nu - 1.0) * (log(nu) + log(ch)) - 0.5 * nu * log(2.0) - lgamma(0.5 * nu);
+    }
+    ctx->log_norm = cst;
+    NSGPU_CUDA(upload(&ctx->tt_a, ta.data(), n));
+    NSGPU_CUDA(upload(&ctx->tt_b, tb.data(), n));
+    { std::vector<double> mu(n); for (size_t i = 0; i < n; ++i) mu[i] = (double)emu[0].out_mean[i]; NSGPU_CUDA(upload(&ctx->tt_mu, mu.data(), n)); }
+    NSGPU_CUDA(upload(&ctx->data, data, n));
+  } else {
   // Gaussian: invert the Cholesky factor once (forward substitution on the identity, fp64)
   {
     const size_t n = n_data;
@@ -293,6 +314,7 @@ nsgpu_status create_impl(nsgpu_ctx* ctx, int32_t D, const nsgpu_prior1d* prior, 
       for (size_t j = 0; j <= i; ++j) LinvT[j * n + i] = Linv[i * n + j];
     NSGPU_CUDA(upload(&ctx->Linv, LinvT.data(), n * n + 2));
     NSGPU_CUDA(upload(&ctx->data, data, n));
+  }
   }
 
   // workspaces
@@ -367,14 +389,14 @@ extern "C" nsgpu_status nsgpu_destroy(nsgpu_ctx* ctx) {
     EmuDev& E = ctx->emu[e];
     mlp_tc_release(ctx, (int)e);
     for (int l = 0; l < NSGPU_MAX_LAYERS; ++l) { cudaFree(E.W[l]); cudaFree(E.b[l]); cudaFree(E.alpha[l]); cudaFree(E.beta[l]); }
-    cudaFree(E.in_mean); cudaFree(E.in_std); cudaFree(E.out_mean); cudaFree(E.out_std);
+    cudaFree(E.in_mean); cudaFree(E.in_std); cudaFree(E.out_mean); cudaFree(E.out_std); cudaFree(E.out_zero);
   }
   cudaFree(ctx->prior_kind); cudaFree(ctx->prior_p0); cudaFree(ctx->prior_p1);
   cudaFree(ctx->emu_in_idx); cudaFree(ctx->emu_in_const); cudaFree(ctx->z_emu);
   cudaFree(ctx->bin_ptr); cudaFree(ctx->bin_col); cudaFree(ctx->bin_val);
   ShearDev& S = ctx->sh;
   cudaFree(S.aux); cudaFree(S.a_q); cudaFree(S.z_q); cudaFree(S.ln1pz); cudaFree(S.lellh); cudaFree(S.lf); cudaFree(S.tap_start); cudaFree(S.tap_w); cudaFree(S.ell); cudaFree(S.nz_mean);
-  cudaFree(ctx->data); cudaFree(ctx->Linv);
+  cudaFree(ctx->data); cudaFree(ctx->Linv); cudaFree(ctx->tt_a); cudaFree(ctx->tt_b); cudaFree(ctx->tt_mu);
   cudaFree(ctx->act[0]); cudaFree(ctx->act[1]); cudaFree(ctx->spec); cudaFree(ctx->model);
   cudaFree(ctx->theta_stage); cudaFree(ctx->logL_stage);
   cudaFreeHost(ctx->theta_pinned); cudaFreeHost(ctx->logL_pinned);
@@ -420,9 +442,9 @@ static nsgpu_status run_emulators(nsgpu_ctx* ctx, const float* theta, int B, con
   const size_t stride = (size_t)ctx->max_batch * ctx->rows_per_theta * (ctx->n_emu ? ctx->emu[0].n_out : 0);
   for (int e = 0; e < ctx->n_emu; ++e) {
     float* out = ctx->spec + e * stride;
-    nsgpu_status s = ctx->emu[e].path == 1
-                         ? mlp_forward_tc(ctx, e, theta, B, n_rows_dev, out, ctx->spec_kz ? NSGPU_SPEC_KZ : 0, st)
-                         : mlp_forward_simt(ctx, e, theta, B, n_rows_dev, out, 0, st);
+    const int mode = (ctx->spec_kz ? NSGPU_SPEC_KZ : 0) | (ctx->kind == 4 ? NSGPU_SPEC_NOMEAN : 0);
+    nsgpu_status s = ctx->emu[e].path == 1 ? mlp_forward_tc(ctx, e, theta, B, n_rows_dev, out, mode, st)
+                                           : mlp_forward_simt(ctx, e, theta, B, n_rows_dev, out, mode & NSGPU_SPEC_NOMEAN, st);
     if (s != NSGPU_OK) return s;
   }
   return NSGPU_OK;
@@ -433,7 +455,8 @@ static nsgpu_status theory_device(nsgpu_ctx* ctx, const float* theta, int B, con
   if (s != NSGPU_OK) return s;
   switch (ctx->kind) {
     case 0:
-    case 1: return copy_model(ctx, theta, B, n_rows_dev, st);
+    case 1:
+    case 4: return copy_model(ctx, theta, B, n_rows_dev, st);
     case 2: return cmb_bin(ctx, theta, B, n_rows_dev, st);
     default: return shear_project(ctx, theta, B, n_rows_dev, st);
   }
@@ -441,6 +464,11 @@ static nsgpu_status theory_device(nsgpu_ctx* ctx, const float* theta, int B, con
 
 nsgpu_status loglike_device(nsgpu_ctx* ctx, const float* theta, int B, const int* n_rows_dev, double* logL,
                             cudaStream_t st) {
+  if (ctx->kind == 4) {   // the per-multipole likelihood reads the emulated log-spectrum directly
+    nsgpu_status s4 = run_emulators(ctx, theta, B, n_rows_dev, st);
+    if (s4 != NSGPU_OK) return s4;
+    return cmb_tt_loglike(ctx, theta, B, n_rows_dev, logL, st);
+  }
   nsgpu_status s = theory_device(ctx, theta, B, n_rows_dev, st);
   if (s != NSGPU_OK) return s;
   return chi2_loglike(ctx, theta, B, n_rows_dev, logL, st);

@@ -24,7 +24,7 @@ struct EmuDev {
   float* b[NSGPU_MAX_LAYERS] = {};
   float* alpha[NSGPU_MAX_LAYERS] = {};
   float* beta[NSGPU_MAX_LAYERS] = {};
-  float *in_mean = nullptr, *in_std = nullptr, *out_mean = nullptr, *out_std = nullptr;
+  float *in_mean = nullptr, *in_std = nullptr, *out_mean = nullptr, *out_std = nullptr, *out_zero = nullptr;
   int path = 0;                         // 0 SIMT, 1 tcgen05
   // tcgen05 path: weights of layers 1..n_hidden as fp16 hi/lo, [fan_out_padded][fan_in] (K-major),
   // scaled by 2^wexp[l] (see mlp_tc.cu)
@@ -73,6 +73,7 @@ struct nsgpu_ctx {
   double* data = nullptr;       // [n_data]
   double* Linv = nullptr;       // [n_data][n_data] TRANSPOSE of the inverse Cholesky factor: LinvT[j][i], fp64
   double log_norm = 0.0;
+  double *tt_a = nullptr, *tt_b = nullptr, *tt_mu = nullptr;   // kind 4: (nu/2) ln 10 and nu Chat / 2 per multipole
   // workspaces
   void* act[2] = {nullptr, nullptr};   // [M_max][width] fp32 (SIMT) or 2 x fp16 (tcgen05)
   float* spec = nullptr;               // [n_emu][M_max][n_out] de-standardised y (log10 where exp10)
@@ -135,6 +136,7 @@ struct StageTimer {
 // rows (theta) are live, B is then the launch bound
 // spectrum output modes of the emulator forward pass
 #define NSGPU_SPEC_EXP10 1   // write 10^y (emulate tap) instead of y
+#define NSGPU_SPEC_NOMEAN 4  // write y - mu_out (the consumer adds mu_out in fp64)
 #define NSGPU_SPEC_KZ 2      // shear only: table layout [theta][k][z] (z fastest) instead of [theta][z][k]
 nsgpu_status mlp_forward_simt(nsgpu_ctx* ctx, int e, const float* theta, int B, const int* n_rows_dev,
                               float* spec_out, int mode, cudaStream_t st);
@@ -144,6 +146,7 @@ nsgpu_status mlp_tc_prepare(nsgpu_ctx* ctx, int e, const nsgpu_emulator* h);
 void mlp_tc_release(nsgpu_ctx* ctx, int e);
 nsgpu_status shear_project(nsgpu_ctx* ctx, const float* theta, int B, const int* n_rows_dev, cudaStream_t st);
 nsgpu_status cmb_bin(nsgpu_ctx* ctx, const float* theta, int B, const int* n_rows_dev, cudaStream_t st);
+nsgpu_status cmb_tt_loglike(nsgpu_ctx* ctx, const float* theta, int B, const int* n_rows_dev, double* logL, cudaStream_t st);
 nsgpu_status copy_model(nsgpu_ctx* ctx, const float* theta, int B, const int* n_rows_dev, cudaStream_t st);
 nsgpu_status chi2_loglike(nsgpu_ctx* ctx, const float* theta, int B, const int* n_rows_dev, double* logL,
                           cudaStream_t st);

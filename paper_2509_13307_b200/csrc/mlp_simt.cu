@@ -139,7 +139,8 @@ nsgpu_status mlp_forward_simt(nsgpu_ctx* ctx, int e, const float* theta, int B, 
   {
     StageTimer tm(ctx, 2, st);
     dim3 grid((M + 63) / 64, (E.n_out + 63) / 64);
-    gemm_simt<1><<<grid, 256, 0, st>>>(cur, E.W[E.n_hidden], E.b[E.n_hidden], E.out_std, E.out_mean, M,
+    gemm_simt<1><<<grid, 256, 0, st>>>(cur, E.W[E.n_hidden], E.b[E.n_hidden], E.out_std,
+                                       (mode & NSGPU_SPEC_NOMEAN) ? E.out_zero : E.out_mean, M,
                                        E.n_out, E.width, n_rows_dev, rpt, apply_exp10 ? 1 : 0, spec_out);
     NSGPU_LAUNCH_CHECK();
   }

@@ -424,8 +424,8 @@ struct TcLayer {
   int K = 0, N_pad = 0, n_valid = 0, block_n = 0, wexp = 0;
   __half *Whi = nullptr, *Wlo = nullptr;     // [N_pad][K] K-major, scaled by 2^wexp
   float4* p_hidden = nullptr;                // layers 0 .. n_hidden-1
-  float2* p_out = nullptr;                   // output layer
-  float4* p_out4 = nullptr;
+  float2 *p_out = nullptr, *p_out_nm = nullptr;     // output layer (with / without mu_out)
+  float4 *p_out4 = nullptr, *p_out4_nm = nullptr;
   CUtensorMap tm_whi, tm_wlo;
 };
 
@@ -555,15 +555,21 @@ nsgpu_status mlp_tc_prepare(nsgpu_ctx* ctx, int e, const nsgpu_emulator* h) {
       NSGPU_CUDA(cudaMemcpy(L.p_hidden, p.data(), p.size() * sizeof(float4), cudaMemcpyHostToDevice));
     } else {
       const float cs = ldexpf(1.0f, -(L.wexp + 4)) * TRUNC_COMP;
-      std::vector<float2> p(L.N_pad, make_float2(0.f, 0.f));
-      for (int n = 0; n < h->n_out; ++n)
-        p[n] = make_float2(cs * h->out_std[n], h->b[l][n] * h->out_std[n] + h->out_mean[n]);
-      NSGPU_CUDA(cudaMalloc((void**)&L.p_out, p.size() * sizeof(float2)));
-      NSGPU_CUDA(cudaMemcpy(L.p_out, p.data(), p.size() * sizeof(float2), cudaMemcpyHostToDevice));
-      std::vector<float4> p4(L.N_pad / 2);
-      for (int n = 0; n < L.N_pad / 2; ++n) p4[n] = make_float4(p[2 * n].x, p[2 * n + 1].x, p[2 * n].y, p[2 * n + 1].y);
-      NSGPU_CUDA(cudaMalloc((void**)&L.p_out4, p4.size() * sizeof(float4)));
-      NSGPU_CUDA(cudaMemcpy(L.p_out4, p4.data(), p4.size() * sizeof(float4), cudaMemcpyHostToDevice));
+      // two parameter sets: with mu_out folded in, and without (NSGPU_SPEC_NOMEAN: the consumer adds mu_out
+      // in fp64, so that the fp32 table carries only the O(sigma_out) deviation)
+      for (int nomean = 0; nomean < 2; ++nomean) {
+        std::vector<float2> p(L.N_pad, make_float2(0.f, 0.f));
+        for (int n = 0; n < h->n_out; ++n)
+          p[n] = make_float2(cs * h->out_std[n], h->b[l][n] * h->out_std[n] + (nomean ? 0.0f : h->out_mean[n]));
+        std::vector<float4> p4(L.N_pad / 2);
+        for (int n = 0; n < L.N_pad / 2; ++n) p4[n] = make_float4(p[2 * n].x, p[2 * n + 1].x, p[2 * n].y, p[2 * n + 1].y);
+        float2** d2 = nomean ? &L.p_out_nm : &L.p_out;
+        float4** d4 = nomean ? &L.p_out4_nm : &L.p_out4;
+        NSGPU_CUDA(cudaMalloc((void**)d2, p.size() * sizeof(float2)));
+        NSGPU_CUDA(cudaMemcpy(*d2, p.data(), p.size() * sizeof(float2), cudaMemcpyHostToDevice));
+        NSGPU_CUDA(cudaMalloc((void**)d4, p4.size() * sizeof(float4)));
+        NSGPU_CUDA(cudaMemcpy(*d4, p4.data(), p4.size() * sizeof(float4), cudaMemcpyHostToDevice));
+      }
     }
   }
   for (int i = 0; i < 2; ++i) {
@@ -578,7 +584,7 @@ nsgpu_status mlp_tc_prepare(nsgpu_ctx* ctx, int e, const nsgpu_emulator* h) {
 void mlp_tc_release(nsgpu_ctx* ctx, int e) {
   TcState* T = reinterpret_cast<TcState*>(ctx->emu[e].tmaps);
   if (!T) return;
-  for (TcLayer& L : T->layers) { cudaFree(L.Whi); cudaFree(L.Wlo); cudaFree(L.p_hidden); cudaFree(L.p_out); cudaFree(L.p_out4); }
+  for (TcLayer& L : T->layers) { cudaFree(L.Whi); cudaFree(L.Wlo); cudaFree(L.p_hidden); cudaFree(L.p_out); cudaFree(L.p_out4); cudaFree(L.p_out_nm); cudaFree(L.p_out4_nm); }
   delete T;
   ctx->emu[e].tmaps = nullptr;
 }
@@ -607,7 +613,7 @@ nsgpu_status mlp_forward_tc(nsgpu_ctx* ctx, int e, const float* theta, int B, co
     GemmArgs g;
     memset(&g, 0, sizeof(g));
     g.M_host = M; g.n_rows_dev = n_rows_dev; g.rows_per_theta = rpt; g.K = L.K; g.N_pad = L.N_pad; g.n_valid = L.n_valid;
-    g.p_hidden = L.p_hidden; g.p_out = L.p_out; g.p_out4 = L.p_out4; g.cscale = ldexpf(1.0f, -(L.wexp + 4)) * TRUNC_COMP;
+    g.p_hidden = L.p_hidden; g.p_out = (mode & NSGPU_SPEC_NOMEAN) ? L.p_out_nm : L.p_out; g.p_out4 = (mode & NSGPU_SPEC_NOMEAN) ? L.p_out4_nm : L.p_out4; g.cscale = ldexpf(1.0f, -(L.wexp + 4)) * TRUNC_COMP;
     g.a_hi = T->act[cur][0]; g.a_lo = T->act[cur][1];
     g.out_hi = T->act[cur ^ 1][0]; g.out_lo = T->act[cur ^ 1][1]; g.ld_out = E.width;
     g.out_f32 = spec_out; g.ld_f32 = E.n_out; g.apply_exp10 = (mode & NSGPU_SPEC_EXP10) ? 1 : 0;

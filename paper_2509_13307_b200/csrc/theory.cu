@@ -362,13 +362,46 @@ __global__ void __launch_bounds__(256) cmb_bin_kernel(const float* __restrict__ 
   }
 }
 
+// kind 4: log L = const - sum_l [ a_l y_l + b_l 10^(-y_l) ], y = emulated log10 C_l.  One CTA per theta,
+// fp64 terms and reduction; reads 4 n_out bytes per theta (HBM-bound), writes log L directly.
+__global__ void __launch_bounds__(128) cmb_tt_kernel(const float* __restrict__ theta, int D, int B,
+                                                     const int* __restrict__ n_rows_dev, const float* __restrict__ spec,
+                                                     int n, const double* __restrict__ ta, const double* __restrict__ tb,
+                                                     const double* __restrict__ mu, double cst, const int* __restrict__ prior_kind,
+                                                     const double* __restrict__ p0, const double* __restrict__ p1,
+                                                     double* __restrict__ logL) {
+  const int b = blockIdx.x;
+  if (n_rows_dev) B = min(B, *n_rows_dev);
+  if (b >= B) return;
+  __shared__ double red[4];
+  const float* y = spec + (size_t)b * n;
+  double acc = 0.0;
+  for (int i = threadIdx.x; i < n; i += blockDim.x) {
+    const double yi = (double)__ldg(y + i) + mu[i];            // the table holds y - mu_out (fp32), mu_out added in fp64
+    acc += fma(ta[i], yi, tb[i] * exp_fast(-2.302585092994046 * yi));
+  }
+  acc = warp_sum(acc);
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = acc;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double out = cst - (red[0] + red[1] + red[2] + red[3]);
+    bool ok = isfinite(out);
+    for (int d = 0; d < D; ++d) {
+      const float v = theta[(size_t)b * D + d];
+      if (!isfinite(v)) ok = false;
+      if (prior_kind[d] == 0 && (v < (float)p0[d] || v > (float)p1[d])) ok = false;
+    }
+    logL[b] = ok ? out : -INFINITY;
+  }
+}
+
 // kind 0: model = theta; kind 1: model = spectrum of emulator 0 (10^y where out_kind = 1)
 __global__ void copy_model_kernel(const float* __restrict__ src, int n, int B, const int* __restrict__ n_rows_dev,
-                                  int apply_exp10, double* __restrict__ model) {
+                                  int apply_exp10, const double* __restrict__ mu, double* __restrict__ model) {
   if (n_rows_dev) B = min(B, *n_rows_dev);
   const size_t total = (size_t)B * n;
   for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
-    const double y = (double)src[i];
+    const double y = (double)src[i] + (mu ? mu[i % n] : 0.0);
     model[i] = apply_exp10 ? exp10(y) : y;
   }
 }
@@ -437,6 +470,15 @@ nsgpu_status cmb_bin(nsgpu_ctx* ctx, const float* theta, int B, const int* n_row
   return NSGPU_OK;
 }
 
+nsgpu_status cmb_tt_loglike(nsgpu_ctx* ctx, const float* theta, int B, const int* n_rows_dev, double* logL, cudaStream_t st) {
+  if (B == 0) return NSGPU_OK;
+  StageTimer tm(ctx, 4, st);
+  cmb_tt_kernel<<<B, 128, 0, st>>>(theta, ctx->D, B, n_rows_dev, ctx->spec, ctx->n_data, ctx->tt_a, ctx->tt_b, ctx->tt_mu, ctx->log_norm,
+                                   ctx->prior_kind, ctx->prior_p0, ctx->prior_p1, logL);
+  NSGPU_LAUNCH_CHECK();
+  return NSGPU_OK;
+}
+
 nsgpu_status copy_model(nsgpu_ctx* ctx, const float* theta, int B, const int* n_rows_dev, cudaStream_t st) {
   if (B == 0) return NSGPU_OK;
   const bool ident = ctx->kind == 0;
@@ -445,7 +487,7 @@ nsgpu_status copy_model(nsgpu_ctx* ctx, const float* theta, int B, const int* n_
   const int ex = (!ident && ctx->emu[0].out_kind == 1) ? 1 : 0;
   int blocks = (int)std::min<size_t>(((size_t)B * n + 255) / 256, 148 * 8);
   StageTimer tm(ctx, 7, st);
-  copy_model_kernel<<<blocks, 256, 0, st>>>(src, n, B, n_rows_dev, ex, ctx->model);
+  copy_model_kernel<<<blocks, 256, 0, st>>>(src, n, B, n_rows_dev, ex, ctx->kind == 4 ? ctx->tt_mu : nullptr, ctx->model);
   NSGPU_LAUNCH_CHECK();
   return NSGPU_OK;
 }

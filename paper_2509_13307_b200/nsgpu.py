@@ -48,7 +48,7 @@ class _Emulator(C.Structure):
 
 class _Theory(C.Structure):
     _fields_ = [("kind", C.c_int32), ("n_theta_in", C.c_int32), ("emu_in_idx", _pi), ("emu_in_const", _pd),
-                ("bin_ptr", _pi), ("bin_col", _pi), ("bin_val", _pf), ("cal_index", C.c_int32),
+                ("bin_ptr", _pi), ("bin_col", _pi), ("bin_val", _pf), ("cal_index", C.c_int32), ("ell_min", C.c_int32),
                 ("n_z_emu", C.c_int32), ("n_z", C.c_int32), ("n_chi", C.c_int32), ("n_k", C.c_int32),
                 ("n_ell", C.c_int32), ("n_tomo", C.c_int32), ("z_interp", C.c_int32),
                 ("z_max", C.c_double), ("k_min", C.c_double), ("k_max", C.c_double),
@@ -143,7 +143,7 @@ class Context:
 
     def __init__(self, wl, max_batch: int, device: int = 0, mlp: int = MLP_AUTO):
         L = lib()
-        if wl.data is None or wl.chol is None:
+        if wl.data is None or (wl.chol is None and wl.theory.kind != 4):
             raise ValueError("workload has no data vector / Cholesky factor attached")
         self._keep = []           # host arrays must outlive nsgpu_create only, kept anyway for clarity
         keep = self._keep.append
@@ -174,6 +174,7 @@ class Context:
         t.n_theta_in = len(idx)
         t.emu_in_idx, t.emu_in_const = _ptr(idx, _pi), _ptr(cst, _pd)
         t.cal_index = th.cal_index
+        t.ell_min = int(getattr(th, "ell_min", 2))
         if th.kind == 2:
             bp, bc, bv = (np.ascontiguousarray(th.bin_ptr, np.int32), np.ascontiguousarray(th.bin_col, np.int32),
                           _f32(th.bin_val))
@@ -188,13 +189,13 @@ class Context:
             keep(ell); keep(nzm)
             t.ell, t.nz_mean = _ptr(ell, _pd), _ptr(nzm, _pd)
         data = np.ascontiguousarray(wl.data, np.float64)
-        chol = np.ascontiguousarray(wl.chol, np.float64)
+        chol = np.ascontiguousarray(wl.chol, np.float64) if wl.chol is not None else None
         self._h = C.c_void_p()
         self.D, self.n_data, self.max_batch, self.device = D, wl.n_data, int(max_batch), int(device)
         self.rows = th.n_z_emu if th.kind == 3 else 1
         self.n_out = wl.emulators[0].n_out if n_emu else 0
         st = L.nsgpu_create(C.byref(self._h), D, prior, n_emu, emus, C.byref(t), wl.n_data, _ptr(data, _pd),
-                            _ptr(chol, _pd), int(max_batch), int(device), int(mlp))
+                            _ptr(chol, _pd) if chol is not None else None, int(max_batch), int(device), int(mlp))
         if st != OK:
             msg = L.nsgpu_last_error(None)
             self._h = C.c_void_p()

@@ -183,3 +183,30 @@ def test_tensor_core_and_simt_paths_agree_on_shear():
     chi2 = -2.0 * (ref - gaussian.log_norm(wl.chol))
     for o in out:
         assert np.all(np.abs(o - ref) <= loglike_tolerance(chi2))
+
+
+@pytest.mark.parametrize("name,B", [("tiny_cmb_tt", 130), ("cmb_tt", 4096)])
+def test_cmb_tt_cosmic_variance_likelihood(name, B):
+    """SURVEY 8(f) NEXT #2, the paper's own CMB likelihood: chi^2_{2l+1} per multipole, no covariance.
+    Tolerance as reading T2 with the effective chi^2 = 2 (log L_saturated - log L)."""
+    from oracle import cmb_tt
+    wl = workload(name)
+    u = np.concatenate([W.u_post_set(wl, B // 2, scale=2e-4), W.u_prior_set(wl, B - B // 2)])
+    theta = theta_of_u(wl, u)
+    rows = np.arange(B) if B <= 256 else np.r_[0:12, B // 2 - 6:B // 2 + 6, B - 12:B]
+    with nsgpu.Context(wl, max_batch=B) as ctx:
+        t = dev(theta)
+        got = ctx.loglike_batch(t).cpu().numpy()
+        model = ctx.theory_batch(t[rows].contiguous()).cpu().numpy()
+        np.testing.assert_array_equal(ctx.loglike_batch_host(theta), got)
+    th64 = theta[rows].astype(np.float64)
+    ref_model = LK.theory(wl, th64)
+    assert np.max(np.abs(model - ref_model) / ref_model) <= 1e-4
+    ref = LK.loglike(wl, th64)
+    ell = cmb_tt.ells(wl.theory, wl.n_data)
+    sat = cmb_tt.loglike_spectrum(ell, wl.data, wl.data[None])[0]
+    chi2_eff = 2.0 * (sat - ref)
+    assert np.all(np.isfinite(got)) and np.all(chi2_eff > -1e-6)
+    err = np.abs(got[rows] - ref)
+    assert np.all(err <= loglike_tolerance(chi2_eff)), (err / loglike_tolerance(chi2_eff)).max()
+    assert np.sum(chi2_eff <= 2000.0 + wl.n_data) >= 4 or B <= 256

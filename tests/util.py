@@ -16,6 +16,7 @@ MAKERS = {
     "tiny_shear_lcdm": lambda: W.tiny_shear(w0wa=False), "tiny_cmb": W.tiny_cmb,
     "c1": W.cmb, "c2": W.c2, "c3a": W.c3a, "c3b": W.c3b, "c4_lcdm": W.c4_lcdm,
     "toy_w64": lambda: W.toy(width=64, n_out=100, n_hidden=3),
+    "cmb_tt": W.cmb_tt, "tiny_cmb_tt": lambda: W.cmb_tt(seed=9, width=64, n_hidden=2, ell_max=131),
 }
 
 
@@ -32,7 +33,9 @@ def workload(name, noise=True):
         return wl
     th0 = theta_of_u(wl, wl.u_fid[None]).astype(np.float64)
     m0 = LK.theory(wl, th0)[0]
-    if wl.theory.kind == 1:
+    if wl.theory.kind == 4:
+        W.attach_cmb_tt_data(wl, m0, noise=noise)
+    elif wl.theory.kind == 1:
         W.attach_toy_data(wl, m0)
     else:
         W.attach_data(wl, m0, noise=noise)
