@@ -192,6 +192,75 @@ __global__ void __launch_bounds__(256) mlp_first_layer_tc(const float* __restric
   }
 }
 
+// Epilogue of NP column pairs (pairs P0 .. P0+NP-1 of the thread's CPT/2; a[i] is pair P0 + i) of one accumulator
+// row: EPI 0 bias + gated activation + hi/lo split into the next layer's canonical planes; EPI 1 de-standardised
+// fp32 output (row-major, or [theta][n][z] for the shear table).
+struct TileRef { int m_blk, n0, r_in, row; bool row_ok; };
+template <int EPI, int P0, int NP>
+__device__ __forceinline__ void epi_pairs(const f32x2* a, const TileRef& t, const GemmArgs& g, const float* params) {
+  static_assert(P0 % 4 == 0 && NP % 4 == 0, "whole 16-byte pieces");
+  const int n0 = t.n0 + 2 * P0;                                  // first column of this slice
+  if (EPI == 0) {
+    const float4* p = reinterpret_cast<const float4*>(params) + n0;
+    const f32x2 cs2 = pk2(g.cscale, g.cscale);
+    // canonical layout: piece n0/8 + c of this tile, 16 bytes per row: lanes are contiguous
+    const size_t o = (size_t)t.m_blk * ((size_t)BLOCK_M * g.ld_out) + (size_t)(n0 >> 3) * PIECE_HALVES + (size_t)t.r_in * 8;
+    __half* dh = g.out_hi + o;
+    __half* dl = g.out_lo + o;
+#pragma unroll
+    for (int c = 0; c < NP / 4; ++c) {
+      uint32_t hi[4], lo[4];
+#pragma unroll
+      for (int j = 0; j < 4; ++j) act_split_pair(a[4 * c + j], cs2, p[8 * c + 2 * j], p[8 * c + 2 * j + 1], hi[j], lo[j]);
+      if (t.row_ok) {
+        *reinterpret_cast<uint4*>(dh + (size_t)c * PIECE_HALVES) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
+        *reinterpret_cast<uint4*>(dl + (size_t)c * PIECE_HALVES) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
+      }
+    }
+  } else {
+    const float4* p4 = g.p_out4 + (n0 >> 1);                       // warp-uniform addresses: L1 broadcast
+    const int rr = t.row_ok ? t.row : 0;
+    if (g.out_mode == 1) {
+      // [theta][n][z] with z fastest: consecutive rows (lanes) of one theta are contiguous
+      const int th = rr / g.rows_per_theta, zi = rr - th * g.rows_per_theta;
+      float* dst = g.out_f32 + (size_t)th * ((size_t)g.n_valid * g.rows_per_theta) + zi;
+#pragma unroll
+      for (int j = 0; j < NP; ++j) {                               // two columns per step: one 16-byte parameter load, one FFMA2
+        const float4 pj = __ldg(p4 + j);                           // {s1_0, s1_1, s0_0, s0_1}
+        float y0, y1;
+        upk2(fma2(a[j], pk2(pj.x, pj.y), pk2(pj.z, pj.w)), y0, y1);
+        if (g.apply_exp10) { y0 = exp10f(y0); y1 = exp10f(y1); }
+        const int n = n0 + 2 * j;
+        if (t.row_ok && n < g.n_valid) dst[(size_t)n * g.rows_per_theta] = y0;
+        if (t.row_ok && n + 1 < g.n_valid) dst[(size_t)(n + 1) * g.rows_per_theta] = y1;
+      }
+    } else {
+      float* dst = g.out_f32 + (size_t)rr * g.ld_f32 + n0;
+      const bool vec = (g.ld_f32 & 3) == 0;
+#pragma unroll
+      for (int c = 0; c < NP / 2; ++c) {
+        float y[4];
+        const float4 pa = __ldg(p4 + 2 * c), pb = __ldg(p4 + 2 * c + 1);
+        upk2(fma2(a[2 * c], pk2(pa.x, pa.y), pk2(pa.z, pa.w)), y[0], y[1]);
+        upk2(fma2(a[2 * c + 1], pk2(pb.x, pb.y), pk2(pb.z, pb.w)), y[2], y[3]);
+        if (g.apply_exp10) {
+#pragma unroll
+          for (int j = 0; j < 4; ++j) y[j] = exp10f(y[j]);
+        }
+        if (t.row_ok) {
+          if (vec && n0 + 4 * c + 4 <= g.n_valid) {
+            reinterpret_cast<float4*>(dst)[c] = make_float4(y[0], y[1], y[2], y[3]);
+          } else {
+#pragma unroll
+            for (int j = 0; j < 4; ++j)
+              if (n0 + 4 * c + j < g.n_valid) dst[4 * c + j] = y[j];
+          }
+        }
+      }
+    }
+  }
+}
+
 // C[M][N] = epi(A[M][K] . W[N][K]^T) with A, W as fp16 hi/lo planes (three MMA passes).
 // EPI 0: hidden layer -> next layer's hi/lo planes; EPI 1: output layer -> fp32 y (optionally 10^y).
 //
@@ -203,7 +272,8 @@ __global__ void __launch_bounds__(256) mlp_first_layer_tc(const float* __restric
 // the cross-k-block summation in round-to-nearest fp32 there, while the MMA thread fills the other
 // partial buffer.  Bias, activation, hi/lo split and the global stores then run from registers.
 constexpr int EPI_WARPS = 8;                         // 2 per TMEM lane quarter, each half of the tile's columns
-constexpr int GEMM_THREADS = 32 * (EPI_WARPS + 2);   // + TMA producer warp, + MMA issuer warp
+constexpr int GEMM_THREADS = 384;                    // warpgroups 0-1 epilogue; warpgroup 2: TMA producer, MMA issuer, 2 idle
+constexpr int DEFER_PAIRS = 24;                      // 48 columns of a finished tile wait in registers (see below)
 template <int BLOCK_N, int EPI>
 __global__ void __launch_bounds__(GEMM_THREADS, 1) mlp_gemm_tc(const __grid_constant__ CUtensorMap tm_whi,
                                                                const __grid_constant__ CUtensorMap tm_wlo, GemmArgs g) {
@@ -251,7 +321,9 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) mlp_gemm_tc(const __grid_cons
   __syncthreads();
   tc::fence_after_sync();
   const uint32_t tmem_base = *tmem_slot;
-
+  // registers: 384 x 168 at launch -> 232 for the epilogue warpgroups (accumulators + deferred columns), 40 for the rest
+  if (warp >= EPI_WARPS) {
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
   if (warp == EPI_WARPS) {
     // ===== TMA producer =====
     if (lane == 0) {
@@ -309,13 +381,33 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) mlp_gemm_tc(const __grid_cons
         }
       }
     }
+  }
   } else {
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 232;");
     // ===== epilogue warps: TMEM lanes 32 (warp % 4) .., columns CPT (warp / 4) .. =====
+    // The accumulators of a tile live in registers, so its epilogue can overlap only the two k-blocks of the next
+    // tile that the partial ring holds.  To shorten that critical section the last DEFP column pairs of a finished
+    // tile are parked in spare registers and processed, 16 columns at a time, in the idle slots after the next
+    // tile's first drains.
+    constexpr int NPAIR = CPT / 2;
+    constexpr int DEFP = (NPAIR >= 48) ? DEFER_PAIRS : 0;
+    constexpr int IMM = NPAIR - DEFP, NCH = DEFP / 8;
     const int q = warp & 3, hcol = warp >> 2;
     uint32_t pcount = 0;
+    f32x2 prev[DEFP > 0 ? DEFP : 1];
+    TileRef pt = {0, 0, 0, 0, false};
+    int pdone = NCH;                                            // deferred chunks already processed (NCH: none pending)
+#define NSGPU_RUN_CHUNK(c)                                                          \
+  do {                                                                              \
+    if (DEFP > 0) {                                                                 \
+      if ((c) == 0) epi_pairs<EPI, IMM, 8>(prev, pt, g, params);                    \
+      else if ((c) == 1) epi_pairs<EPI, IMM + 8, 8>(prev + (DEFP > 8 ? 8 : 0), pt, g, params);   \
+      else epi_pairs<EPI, IMM + 16, 8>(prev + (DEFP > 16 ? 16 : 0), pt, g, params); \
+    }                                                                               \
+  } while (0)
     for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
       const int m_blk = tile / n_blocks, n_blk = tile - m_blk * n_blocks;
-      f32x2 acc[CPT / 2];
+      f32x2 acc[NPAIR];
       for (int kb = 0; kb < k_blocks; ++kb, ++pcount) {
         const uint32_t pb = pcount % NPB, pphase = (pcount / NPB) & 1;
         tc::mbar_wait(pfull0 + 8 * pb, pphase);
@@ -338,75 +430,21 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) mlp_gemm_tc(const __grid_cons
         tc::fence_before_sync();
         __syncwarp();
         if (lane == 0) tc::mbar_arrive(pempty0 + 8 * pb);
+        if (DEFP > 0 && pdone < NCH && kb >= 1) { NSGPU_RUN_CHUNK(pdone); ++pdone; }
       }
+      while (DEFP > 0 && pdone < NCH) { NSGPU_RUN_CHUNK(pdone); ++pdone; }   // short K: not enough idle slots
       const int r_in = q * 32 + lane;
-      const int row = m_blk * BLOCK_M + r_in;
-      const bool row_ok = row < M;
-      const int n0 = n_blk * BLOCK_N + hcol * CPT;
-      if (g.dbg & 16) continue;   // timing experiment: no epilogue math / stores
-      if (EPI == 0) {
-        const float4* p = reinterpret_cast<const float4*>(params) + n0;
-        const f32x2 cs2 = pk2(g.cscale, g.cscale);
-        // canonical layout: piece (n0/8 + c) of this tile, 16 bytes per row: lanes are contiguous
-        const size_t o = (size_t)m_blk * ((size_t)BLOCK_M * g.ld_out) + (size_t)(n0 >> 3) * PIECE_HALVES + (size_t)r_in * 8;
-        __half* dh = g.out_hi + o;
-        __half* dl = g.out_lo + o;
+      const TileRef ct = {m_blk, n_blk * BLOCK_N + hcol * CPT, r_in, m_blk * BLOCK_M + r_in, m_blk * BLOCK_M + r_in < M};
+      epi_pairs<EPI, 0, IMM>(acc, ct, g, params);
+      if (DEFP > 0) {
 #pragma unroll
-        for (int c = 0; c < CPT / 8; ++c) {
-          uint32_t hi[4], lo[4];
-#pragma unroll
-          for (int j = 0; j < 4; ++j)
-            act_split_pair(acc[4 * c + j], cs2, p[8 * c + 2 * j], p[8 * c + 2 * j + 1], hi[j], lo[j]);
-          if (row_ok) {
-            *reinterpret_cast<uint4*>(dh + (size_t)c * PIECE_HALVES) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
-            *reinterpret_cast<uint4*>(dl + (size_t)c * PIECE_HALVES) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
-          }
-        }
-      } else {
-        const float2* p = g.p_out + n0;            // warp-uniform addresses: L1 broadcast
-        const float4* p4 = g.p_out4 + (n0 >> 1);
-        if (g.out_mode == 1) {
-          // [theta][n][z] with z fastest: consecutive rows (lanes) of one theta are contiguous
-          const int rr = row_ok ? row : 0;
-          const int th = rr / g.rows_per_theta, zi = rr - th * g.rows_per_theta;
-          float* dst = g.out_f32 + (size_t)th * ((size_t)g.n_valid * g.rows_per_theta) + zi;
-#pragma unroll
-          for (int j = 0; j < CPT / 2; ++j) {                 // two columns per step: one 16-byte parameter load, one FFMA2
-            const float4 pj = __ldg(p4 + j);                 // {s1_0, s1_1, s0_0, s0_1}
-            float y0, y1;
-            upk2(fma2(acc[j], pk2(pj.x, pj.y), pk2(pj.z, pj.w)), y0, y1);
-            if (g.apply_exp10) { y0 = exp10f(y0); y1 = exp10f(y1); }
-            const int n = n0 + 2 * j;
-            if (row_ok && n < g.n_valid) dst[(size_t)n * g.rows_per_theta] = y0;
-            if (row_ok && n + 1 < g.n_valid) dst[(size_t)(n + 1) * g.rows_per_theta] = y1;
-          }
-        } else {
-          float* dst = g.out_f32 + (size_t)row * g.ld_f32 + n0;
-          const bool vec = (g.ld_f32 & 3) == 0;
-#pragma unroll
-          for (int c = 0; c < CPT / 4; ++c) {
-            float y[4];
-#pragma unroll
-            for (int j = 0; j < 4; ++j) {
-              const float2 pj = __ldg(p + 4 * c + j);
-              float a0, a1;
-              upk2(acc[(4 * c + j) >> 1], a0, a1);
-              y[j] = fmaf((j & 1) ? a1 : a0, pj.x, pj.y);
-              if (g.apply_exp10) y[j] = exp10f(y[j]);
-            }
-            if (row_ok) {
-              if (vec && n0 + 4 * c + 4 <= g.n_valid) {
-                reinterpret_cast<float4*>(dst)[c] = make_float4(y[0], y[1], y[2], y[3]);
-              } else {
-#pragma unroll
-                for (int j = 0; j < 4; ++j)
-                  if (n0 + 4 * c + j < g.n_valid) dst[4 * c + j] = y[j];
-              }
-            }
-          }
-        }
+        for (int i = 0; i < DEFP; ++i) prev[i] = acc[IMM + i];
+        pt = ct;
+        pdone = 0;
       }
     }
+    while (DEFP > 0 && pdone < NCH) { NSGPU_RUN_CHUNK(pdone); ++pdone; }
+#undef NSGPU_RUN_CHUNK
   }
   tc::fence_before_sync();
   __syncthreads();
