@@ -273,7 +273,7 @@ __device__ __forceinline__ void epi_pairs(const f32x2* a, const TileRef& t, cons
 // partial buffer.  Bias, activation, hi/lo split and the global stores then run from registers.
 constexpr int EPI_WARPS = 8;                         // 2 per TMEM lane quarter, each half of the tile's columns
 constexpr int GEMM_THREADS = 384;                    // warpgroups 0-1 epilogue; warpgroup 2: TMA producer, MMA issuer, 2 idle
-constexpr int DEFER_PAIRS = 24;                      // 48 columns of a finished tile wait in registers (see below)
+constexpr int DEFER_PAIRS = 32;                      // 64 columns of a finished tile wait in registers (see below)
 template <int BLOCK_N, int EPI>
 __global__ void __launch_bounds__(GEMM_THREADS, 1) mlp_gemm_tc(const __grid_constant__ CUtensorMap tm_whi,
                                                                const __grid_constant__ CUtensorMap tm_wlo, GemmArgs g) {
@@ -390,20 +390,19 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) mlp_gemm_tc(const __grid_cons
     // tile are parked in spare registers and processed, 16 columns at a time, in the idle slots after the next
     // tile's first drains.
     constexpr int NPAIR = CPT / 2;
-    constexpr int DEFP = (NPAIR >= 48) ? DEFER_PAIRS : 0;
+    constexpr int DEFP = (NPAIR >= 48) ? (EPI == 0 ? DEFER_PAIRS : DEFER_PAIRS - 8) : 0;   // the output epilogue needs more temporaries
     constexpr int IMM = NPAIR - DEFP, NCH = DEFP / 8;
     const int q = warp & 3, hcol = warp >> 2;
     uint32_t pcount = 0;
     f32x2 prev[DEFP > 0 ? DEFP : 1];
     TileRef pt = {0, 0, 0, 0, false};
     int pdone = NCH;                                            // deferred chunks already processed (NCH: none pending)
+#define NSGPU_CHUNK_CASE(i) \
+  if ((c_) == (i) && DEFP > 8 * (i)) epi_pairs<EPI, IMM + (DEFP > 8 * (i) ? 8 * (i) : 0), 8>(prev + (DEFP > 8 * (i) ? 8 * (i) : 0), pt, g, params)
 #define NSGPU_RUN_CHUNK(c)                                                          \
   do {                                                                              \
-    if (DEFP > 0) {                                                                 \
-      if ((c) == 0) epi_pairs<EPI, IMM, 8>(prev, pt, g, params);                    \
-      else if ((c) == 1) epi_pairs<EPI, IMM + 8, 8>(prev + (DEFP > 8 ? 8 : 0), pt, g, params);   \
-      else epi_pairs<EPI, IMM + 16, 8>(prev + (DEFP > 16 ? 16 : 0), pt, g, params); \
-    }                                                                               \
+    const int c_ = (c);                                                             \
+    NSGPU_CHUNK_CASE(0); NSGPU_CHUNK_CASE(1); NSGPU_CHUNK_CASE(2); NSGPU_CHUNK_CASE(3); NSGPU_CHUNK_CASE(4); NSGPU_CHUNK_CASE(5); \
   } while (0)
     for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
       const int m_blk = tile / n_blocks, n_blk = tile - m_blk * n_blocks;
@@ -445,6 +444,7 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) mlp_gemm_tc(const __grid_cons
     }
     while (DEFP > 0 && pdone < NCH) { NSGPU_RUN_CHUNK(pdone); ++pdone; }
 #undef NSGPU_RUN_CHUNK
+#undef NSGPU_CHUNK_CASE
   }
   tc::fence_before_sync();
   __syncthreads();
