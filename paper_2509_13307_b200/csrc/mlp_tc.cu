@@ -123,6 +123,7 @@ __device__ __forceinline__ void split2(float a, float b, uint32_t& hi, uint32_t&
 // a2 + first hidden layer (K = n_in <= 16: CUDA cores), output as the canonical fp16 hi/lo planes of
 // 16 h.  One CTA per 128-row tile; lane = row, each warp walks 16-byte pieces (8 neurons) so that a
 // warp's stores are 512 contiguous bytes.  W0 and the activation parameters are staged in shared memory.
+template <int NIN>
 __global__ void __launch_bounds__(256) mlp_first_layer_tc(const float* __restrict__ theta, int D, int rows_per_theta,
                                                           int M, const int* __restrict__ n_rows_dev,
                                                           const int* __restrict__ emu_in_idx,
@@ -148,11 +149,11 @@ __global__ void __launch_bounds__(256) mlp_first_layer_tc(const float* __restric
   const int r = (warp & 3) * 32 + lane;                      // row within the tile
   const int m = min(m0 + r, M - 1);
   const int th = m / rows_per_theta, zi = m - th * rows_per_theta;
-  float x[NSGPU_MAX_IN];
+  float x[NIN];                                             // NIN = n_in at compile time: no predicated-off work
 #pragma unroll
-  for (int c = 0; c < NSGPU_MAX_IN; ++c) {
+  for (int c = 0; c < NIN; ++c) {
     float v = 0.0f;
-    if (c < n_in) {
+    {
       if (c < n_theta_in) {
         const int src = emu_in_idx[c];
         v = src >= 0 ? theta[(size_t)th * D + src] : (float)emu_in_const[c];
@@ -167,16 +168,15 @@ __global__ void __launch_bounds__(256) mlp_first_layer_tc(const float* __restric
   const int n_pieces = width >> 3, half_pieces = (n_pieces + 1) >> 1;
   const int p_begin = (warp >> 2) * half_pieces, p_end = min(p_begin + half_pieces, n_pieces);
   const size_t tile_base = (size_t)blockIdx.x * ((size_t)BLOCK_M * width) + (size_t)r * 8;
-  f32x2 x2[NSGPU_MAX_IN];
+  f32x2 x2[NIN];
 #pragma unroll
-  for (int c = 0; c < NSGPU_MAX_IN; ++c) x2[c] = pk2(x[c], x[c]);
+  for (int c = 0; c < NIN; ++c) x2[c] = pk2(x[c], x[c]);
   const f32x2 one2 = pk2(1.0f, 1.0f);
   for (int p = p_begin; p < p_end; ++p) {
     uint32_t hi[4], lo[4];
     f32x2 t[4] = {0ull, 0ull, 0ull, 0ull};                      // 8 neurons of this piece, bias added in the epilogue
 #pragma unroll
-    for (int c = 0; c < NSGPU_MAX_IN; ++c)
-      if (c < n_in) {
+    for (int c = 0; c < NIN; ++c) {
         const float4 wlo = *reinterpret_cast<const float4*>(sW + c * width + 8 * p);
         const float4 whi = *reinterpret_cast<const float4*>(sW + c * width + 8 * p + 4);
         t[0] = fma2(x2[c], pk2(wlo.x, wlo.y), t[0]); t[1] = fma2(x2[c], pk2(wlo.z, wlo.w), t[1]);
@@ -638,11 +638,15 @@ nsgpu_status mlp_forward_tc(nsgpu_ctx* ctx, int e, const float* theta, int B, co
   {
     StageTimer tm(ctx, 0, st);
     const size_t smem = (size_t)E.width * sizeof(float4) + (size_t)E.n_in * E.width * sizeof(float);
-    mlp_first_layer_tc<<<(M + BLOCK_M - 1) / BLOCK_M, 256, smem, st>>>(theta, ctx->D, rpt, M, n_rows_dev, ctx->emu_in_idx,
-                                                                      ctx->emu_in_const, ctx->n_theta_in, ctx->z_emu,
-                                                                      E.n_in, E.in_mean, E.in_std, E.W[0],
-                                                                      T->layers[0].p_hidden, E.width, T->act[0][0],
-                                                                      T->act[0][1]);
+#define NSGPU_FL(N_) case N_: mlp_first_layer_tc<N_><<<(M + BLOCK_M - 1) / BLOCK_M, 256, smem, st>>>ARGS_; break;
+#define ARGS_ (theta, ctx->D, rpt, M, n_rows_dev, ctx->emu_in_idx,                                                                       ctx->emu_in_const, ctx->n_theta_in, ctx->z_emu,                                                                       E.n_in, E.in_mean, E.in_std, E.W[0],                                                                       T->layers[0].p_hidden, E.width, T->act[0][0],                                                                       T->act[0][1])
+    switch (E.n_in) {
+      NSGPU_FL(1) NSGPU_FL(2) NSGPU_FL(3) NSGPU_FL(4) NSGPU_FL(5) NSGPU_FL(6) NSGPU_FL(7) NSGPU_FL(8)
+      NSGPU_FL(9) NSGPU_FL(10) NSGPU_FL(11) NSGPU_FL(12) NSGPU_FL(13) NSGPU_FL(14) NSGPU_FL(15) NSGPU_FL(16)
+      default: ctx->err = "emulator n_in > 16"; return NSGPU_ESHAPE;
+    }
+#undef ARGS_
+#undef NSGPU_FL
     NSGPU_LAUNCH_CHECK();
   }
   for (int l = 1; l <= E.n_hidden; ++l) {
