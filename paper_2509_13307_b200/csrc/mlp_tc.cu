@@ -65,7 +65,6 @@ struct GemmArgs {
   int ld_f32;                 // out_mode 0: y[m][n] at m ld_f32 + n
   int out_mode;               // out_mode 1: y at theta(m) (n_valid rpt) + n rpt + z(m)  ([theta][n][z], z fastest)
   int apply_exp10;
-  int dbg;                    // timing experiments only (NSGPU_TC_DBG)
 };
 
 __device__ __forceinline__ float ex2_approx(float x) { float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
@@ -660,7 +659,6 @@ nsgpu_status mlp_forward_tc(nsgpu_ctx* ctx, int e, const float* theta, int B, co
     g.out_hi = T->act[cur ^ 1][0]; g.out_lo = T->act[cur ^ 1][1]; g.ld_out = E.width;
     g.out_f32 = spec_out; g.ld_f32 = E.n_out; g.apply_exp10 = (mode & NSGPU_SPEC_EXP10) ? 1 : 0;
     g.out_mode = (mode & NSGPU_SPEC_KZ) ? 1 : 0;
-    { const char* dbg = getenv("NSGPU_TC_DBG"); g.dbg = dbg ? atoi(dbg) : 0; }
     StageTimer tm(ctx, hidden ? 1 : 2, st);
     nsgpu_status s = hidden ? dispatch_gemm<0>(ctx, L, g, st) : dispatch_gemm<1>(ctx, L, g, st);
     if (s != NSGPU_OK) return s;
