@@ -116,7 +116,12 @@ __global__ void __launch_bounds__(SHEAR_THREADS, 2) shear_project_kernel(const f
   double* ichi = hs + nq;                              // [nq]   1 / chi
   double* Wt = ichi + nq;                              // [nt][nq] total window
   double* scr = Wt + (size_t)nt * nq;                  // [n_scr][nqp]: scan arrays, then Pg[n_ell][nqp]
-  size_t n_dbl = (size_t)nq * (6 + nt) + (size_t)n_scr * nqp + 2;
+  const int n_tap_s = A.n_tap <= 4 ? A.n_tap : 0;      // few taps: the z-interpolation weights are staged too
+  double* c_ell = scr + (size_t)n_scr * nqp;           // [n_ell] ell + 1/2
+  double* c_lell = c_ell + A.n_ell;                    // [n_ell] log10(ell + 1/2)
+  double* c_tw = c_lell + A.n_ell;                     // [nq][n_tap_s]
+  int* c_ts = reinterpret_cast<int*>(c_tw + (size_t)nq * n_tap_s);   // [nq] first tap row
+  size_t n_dbl = (size_t)nq * (6 + nt) + (size_t)n_scr * nqp + 2 * A.n_ell + (size_t)nq * n_tap_s + (nq + 1) / 2 + 2;
   n_dbl = (n_dbl + 1) & ~(size_t)1;
   unsigned long long* bar = reinterpret_cast<unsigned long long*>(chi + n_dbl - 2);   // 8-byte mbarrier
   float* table = reinterpret_cast<float*>(chi + n_dbl);   // [n_z_emu][n_k], 16-byte aligned
@@ -147,6 +152,11 @@ __global__ void __launch_bounds__(SHEAR_THREADS, 2) shear_project_kernel(const f
       for (int i = tid; i < A.n_z_emu * A.n_k; i += blockDim.x) table[i] = __ldg(src + i);
     }
     if (PHASE == 2) __syncthreads();   // the mbarrier is initialised before anyone polls it
+  }
+  if (PHASE != 1) {   // small constant tables of the lookups (published by the __syncthreads below / in the phases)
+    for (int i = tid; i < A.n_ell; i += blockDim.x) { c_ell[i] = A.ell[i] + 0.5; c_lell[i] = A.lellh[i]; }
+    for (int i = tid; i < nq; i += blockDim.x) c_ts[i] = A.tap_start[i];
+    for (int i = tid; i < nq * n_tap_s; i += blockDim.x) c_tw[i] = A.tap_w[i];
   }
   const double ob = th[A.idx_omega_b], oc = th[A.idx_omega_cdm], h = th[A.idx_h];
   const double Om = (ob + oc) / (h * h);
@@ -220,6 +230,7 @@ __global__ void __launch_bounds__(SHEAR_THREADS, 2) shear_project_kernel(const f
     return;
   }
   }   // PHASE != 2
+  if (PHASE == 2) __syncthreads();   // constant tables staged
   if (bulk) {   // the table (and aux) have landed?
     unsigned ok = 0;
     while (!ok)
@@ -237,18 +248,18 @@ __global__ void __launch_bounds__(SHEAR_THREADS, 2) shear_project_kernel(const f
   for (int item = tid; item < n_lg4 * nq; item += blockDim.x) {
     const int lg = (int)__umulhi((unsigned)item, nq_magic), q = item - lg * nq;
     const double ic = ichi[q], lc = hs[q], g_q = gq[q];
-    const int m0 = A.tap_start[q];
-    const double* tw = A.tap_w + (size_t)q * A.n_tap;
+    const int m0 = c_ts[q];
+    const double* tw = n_tap_s ? c_tw + (size_t)q * A.n_tap : A.tap_w + (size_t)q * A.n_tap;
     const double tw0 = tw[0], tw1 = A.n_tap > 1 ? tw[1] : 0.0;
     const float* col0 = table + (size_t)m0 * A.sz;             // two-tap fast path: rows m0, m0 + 1
 #pragma unroll 2
     for (int u = 0; u < 4; ++u) {
       const int bl = 4 * lg + u;
       if (bl >= A.n_ell) break;
-      const double k = (A.ell[bl] + 0.5) * ic;
+      const double k = c_ell[bl] * ic;
       double P = 0.0;
       if (k >= A.k_min && k <= A.k_max) {
-        const double x = A.lellh[bl] - lc;
+        const double x = c_lell[bl] - lc;
         int j = (int)floor((x - A.lk0) * inv_dlk);
         j = min(max(j, 0), A.n_k - 2);
         const double s = (x - (A.lk0 + j * A.dlk)) * inv_dlk;
@@ -410,7 +421,8 @@ __global__ void copy_model_kernel(const float* __restrict__ src, int n, int B, c
 
 static size_t shear_smem_bytes(const ShearDev& S) {
   const size_t nqp = (size_t)S.n_chi | 1, n_scr = (size_t)std::max(2 * S.n_tomo, S.n_ell);
-  size_t d = (size_t)S.n_chi * (6 + S.n_tomo) + n_scr * nqp + 2;
+  const size_t n_tap_s = S.n_tap <= 4 ? S.n_tap : 0;
+  size_t d = (size_t)S.n_chi * (6 + S.n_tomo) + n_scr * nqp + 2 * S.n_ell + (size_t)S.n_chi * n_tap_s + (S.n_chi + 1) / 2 + 2;
   d = (d + 1) & ~(size_t)1;
   return d * sizeof(double) + (size_t)S.n_z_emu * S.n_k * sizeof(float) + 16;
 }
