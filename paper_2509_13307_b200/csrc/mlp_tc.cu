@@ -463,7 +463,9 @@ struct TcLayer {
   float4* p_hidden = nullptr;                // layers 0 .. n_hidden-1
   float2 *p_out = nullptr, *p_out_nm = nullptr;     // output layer (with / without mu_out)
   float4 *p_out4 = nullptr, *p_out4_nm = nullptr;
-  CUtensorMap tm_whi, tm_wlo;
+  CUtensorMap tm_whi, tm_wlo;                // box = block_n rows
+  CUtensorMap tm_whi_s[2], tm_wlo_s[2];      // hidden layers: boxes of 128 and 64 rows for small batches
+  bool has_s[2] = {false, false};
 };
 
 struct TcState {
@@ -513,7 +515,7 @@ int pick_block_n(int n, bool hidden) {
 }
 
 template <int BN, int EPI>
-nsgpu_status launch_gemm(nsgpu_ctx* ctx, const TcLayer& L, const GemmArgs& g, cudaStream_t st) {
+nsgpu_status launch_gemm(nsgpu_ctx* ctx, const CUtensorMap& whi, const CUtensorMap& wlo, const GemmArgs& g, cudaStream_t st) {
   const int smem = num_stages(BN) * stage_bytes(BN) + 16 * num_stages(BN) + 128 + (EPI == 0 ? 16 * g.N_pad : 0) + 1024;
   static bool configured = false;
   if (!configured) {
@@ -522,18 +524,29 @@ nsgpu_status launch_gemm(nsgpu_ctx* ctx, const TcLayer& L, const GemmArgs& g, cu
   }
   const int tiles = ((g.M_host + BLOCK_M - 1) / BLOCK_M) * (g.N_pad / BN);
   const int grid = std::min(tiles, ctx->sm_count);
-  mlp_gemm_tc<BN, EPI><<<grid, GEMM_THREADS, smem, st>>>(L.tm_whi, L.tm_wlo, g);
+  mlp_gemm_tc<BN, EPI><<<grid, GEMM_THREADS, smem, st>>>(whi, wlo, g);
   NSGPU_LAUNCH_CHECK();
   return NSGPU_OK;
 }
 
 template <int EPI>
 nsgpu_status dispatch_gemm(nsgpu_ctx* ctx, const TcLayer& L, const GemmArgs& g, cudaStream_t st) {
+  // Small batches (few 128-row blocks): narrower tiles so that the grid still covers the SMs.
+  if (EPI == 0) {
+    const int m_blocks = (g.M_host + BLOCK_M - 1) / BLOCK_M;
+    int bn = L.block_n;
+    while (bn > 64 && m_blocks * (g.N_pad / bn) < ctx->sm_count && L.has_s[bn == 256 ? 0 : 1]) bn >>= 1;
+    if (bn != L.block_n) {
+      const int i = bn == 128 ? 0 : 1;
+      return bn == 128 ? launch_gemm<128, EPI>(ctx, L.tm_whi_s[i], L.tm_wlo_s[i], g, st)
+                       : launch_gemm<64, EPI>(ctx, L.tm_whi_s[i], L.tm_wlo_s[i], g, st);
+    }
+  }
   switch (L.block_n) {
-    case 256: return launch_gemm<256, EPI>(ctx, L, g, st);
-    case 224: return launch_gemm<224, EPI>(ctx, L, g, st);
-    case 128: return launch_gemm<128, EPI>(ctx, L, g, st);
-    default: return launch_gemm<64, EPI>(ctx, L, g, st);
+    case 256: return launch_gemm<256, EPI>(ctx, L.tm_whi, L.tm_wlo, g, st);
+    case 224: return launch_gemm<224, EPI>(ctx, L.tm_whi, L.tm_wlo, g, st);
+    case 128: return launch_gemm<128, EPI>(ctx, L.tm_whi, L.tm_wlo, g, st);
+    default: return launch_gemm<64, EPI>(ctx, L.tm_whi, L.tm_wlo, g, st);
   }
 }
 
@@ -580,6 +593,12 @@ nsgpu_status mlp_tc_prepare(nsgpu_ctx* ctx, int e, const nsgpu_emulator* h) {
       if (!make_tmap(&L.tm_whi, L.Whi, L.N_pad, L.K, L.block_n) || !make_tmap(&L.tm_wlo, L.Wlo, L.N_pad, L.K, L.block_n)) {
         ctx->err = "cuTensorMapEncodeTiled failed for a weight plane";
         return NSGPU_ECUDA;
+      }
+      if (hidden) {   // narrower boxes over the same planes (N_pad = width is a multiple of 64)
+        const int bs[2] = {128, 64};
+        for (int i = 0; i < 2; ++i)
+          L.has_s[i] = bs[i] < L.block_n && L.N_pad % bs[i] == 0 && make_tmap(&L.tm_whi_s[i], L.Whi, L.N_pad, L.K, bs[i]) &&
+                       make_tmap(&L.tm_wlo_s[i], L.Wlo, L.N_pad, L.K, bs[i]);
       }
     }
     if (hidden) {
