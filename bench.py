@@ -2,7 +2,7 @@
 """bench.py -- likelihood evaluations/s of the nsgpu hot path (BASELINE.json metric).
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl nsgpu|reference]
-                    [--workload c3a|c3b|c2|c1|c0] [--batch 4096]
+                    [--workload c3a|c3b|c2|c1|c0|cmb_tt|c5i|c5] [--batch 4096]
 
 A "step" is one pass of the whole likelihood path (steps a2-a10 of DESIGN.md: emulator MLP -> z
 interpolation + Limber projection (or CMB binning) -> Gaussian chi^2) over one batch of `--batch`
@@ -37,7 +37,8 @@ from paper_2509_13307_b200 import workloads as W  # noqa: E402
 
 METRIC = "likelihood evals/sec at batch 4096 (39-D shear); % tensor/HBM roofline"
 UNIT = "evals/s"
-MAKERS = {"c0": W.toy, "c1": W.cmb, "c2": W.c2, "c3a": W.c3a, "c3b": W.c3b, "cmb_tt": W.cmb_tt}
+MAKERS = {"c0": W.toy, "c1": W.cmb, "c2": W.c2, "c3a": W.c3a, "c3b": W.c3b, "cmb_tt": W.cmb_tt,
+          "c5i": lambda: W.c5(True), "c5": lambda: W.c5(False)}
 
 
 def flops_per_row(em):
@@ -114,12 +115,12 @@ class ClockSampler:
                 "samples": len(sm)}
 
 
-def make_context(nsgpu, torch, wl, batch, device):
+def make_context(nsgpu, torch, wl, batch, device, flags=0):
     """Attach a synthetic data vector made by the CUDA path itself at the fiducial point (the product
     never touches oracle/): first a context with a placeholder Gaussian, then the real one."""
     n = wl.n_data
     wl.data, wl.chol = (np.ones(n), None) if wl.theory.kind == W.THEORY_CMB_TT_CV else (np.zeros(n), np.eye(n))
-    with nsgpu.Context(wl, max_batch=8, device=device) as c0:
+    with nsgpu.Context(wl, max_batch=8, device=device, mlp=flags) as c0:
         u0 = torch.as_tensor(wl.u_fid[None].astype(np.float32), device=f"cuda:{device}")
         m0 = c0.theory_batch(c0.prior_transform(u0)).cpu().numpy()[0]
     if wl.theory.kind == W.THEORY_CMB_TT_CV:
@@ -128,7 +129,7 @@ def make_context(nsgpu, torch, wl, batch, device):
         W.attach_toy_data(wl, m0)
     else:
         W.attach_data(wl, m0, noise=True)
-    return nsgpu.Context(wl, max_batch=batch, device=device)
+    return nsgpu.Context(wl, max_batch=batch, device=device, mlp=flags)
 
 
 def theta_batches(nsgpu, torch, ctx, wl, batch, rank, n_sets, device):
@@ -264,7 +265,7 @@ def run_nsgpu(args, rank, world, local_rank):
     ranks = Ranks(world, "nccl", torch.device("cuda", dev))
     wl = MAKERS[args.workload]()
     B = args.batch
-    ctx = make_context(nsgpu, torch, wl, B, dev)
+    ctx = make_context(nsgpu, torch, wl, B, dev, nsgpu.SHEAR_STREAM if args.shear_stream else 0)
     n_sets = 4
     th_dev, th_host = theta_batches(nsgpu, torch, ctx, wl, B, rank, n_sets, dev)
     out = torch.empty(B, dtype=torch.float64, device=f"cuda:{dev}")
@@ -378,6 +379,8 @@ def main():
     ap.add_argument("--batch", type=int, default=4096)
     ap.add_argument("--cpu-sample", type=int, default=768)
     ap.add_argument("--ref-sample", type=int, default=16)
+    ap.add_argument("--shear-stream", action="store_true",
+                    help="shear workloads: use the streaming projection kernels even where the resident one fits")
     ap.add_argument("--dry-run-cpu", action="store_true", help=argparse.SUPPRESS)
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))

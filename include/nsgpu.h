@@ -110,14 +110,19 @@ typedef struct {
   /* where each physical parameter sits in theta (reading S2); < 0: w0 = -1, wa = 0, eta0 = 0.7 */
   int32_t idx_omega_b, idx_omega_cdm, idx_h, idx_w0, idx_wa, idx_eta0;
   int32_t idx_dz; /* first of n_tomo photo-z shifts */
-  int32_t idx_ia; /* first of 3 n_tomo IA coefficients, bin-major (reading S2) */
-  int32_t idx_m;  /* first of 2 n_tomo shear-calibration coefficients, bin-major (S2) */
+  int32_t idx_ia; /* first of n_ia_terms n_tomo IA coefficients, bin-major (reading S2) */
+  int32_t idx_m;  /* first of n_m_terms n_tomo shear-calibration coefficients, bin-major (S2) */
+  /* coefficients per bin: A_i(z) = A_i0 + A_i1 x + A_i2 x^2 truncated after n_ia_terms in 1..3, m_i(l) = m_i0 +
+   * m_i1 ln(l/550)/ln 30 after n_m_terms in 1..2.  (1, 1) is the paper's one amplitude and one bias per bin
+   * (P:L344, L350); (3, 2) the BASELINE.json configs[2..4] layout.                                        */
+  int32_t n_ia_terms, n_m_terms;
 } nsgpu_theory;
 
 /* flags for nsgpu_create */
 #define NSGPU_MLP_AUTO 0u   /* tcgen05 tensor-core MLP where the shape allows it, SIMT otherwise */
 #define NSGPU_MLP_SIMT 1u   /* fp32 CUDA-core MLP (on-device correctness reference) */
 #define NSGPU_MLP_TC 2u     /* require the tcgen05 path (NSGPU_ESHAPE if width % 64 != 0) */
+#define NSGPU_SHEAR_STREAM 4u /* kind 3: use the streaming projection kernels even where the grids fit shared memory */
 
 /* Create a context on CUDA device `device`.
  * data [n_data] and chol [n_data][n_data] (lower Cholesky factor of the data covariance, row-major,

@@ -173,6 +173,16 @@ def limber_cl(th, chi, dchi, z_q, Wg, Wi, table, z_lim, lk, eta0):
     return C
 
 
+def _bin_terms(theta, first, n_tomo, n_terms, n_max):
+    """[n_tomo, n_max] coefficients, bin-major in theta with n_terms per bin, higher ones zero
+    (n_terms = 1: the paper's single amplitude / bias per bin)."""
+    out = np.zeros((n_tomo, n_max))
+    for i in range(n_tomo):
+        for t in range(n_terms):
+            out[i, t] = theta[first + n_terms * i + t]
+    return out
+
+
 def physical_parameters(th, theta):
     """unpack one theta row by the parameter map (reading S2)."""
     g = lambda i, default: (float(theta[i]) if i >= 0 else default)
@@ -181,8 +191,8 @@ def physical_parameters(th, theta):
     return dict(Om=(ob + oc) / (h * h), w0=g(th.idx_w0, -1.0), wa=g(th.idx_wa, 0.0),
                 eta0=g(th.idx_eta0, 0.7),
                 dz=np.array([theta[th.idx_dz + i] for i in range(nt)], np.float64),
-                A=np.array([[theta[th.idx_ia + 3 * i + t] for t in range(3)] for i in range(nt)], np.float64),
-                m=np.array([[theta[th.idx_m + 2 * i + t] for t in range(2)] for i in range(nt)], np.float64))
+                A=_bin_terms(theta, th.idx_ia, nt, th.n_ia_terms, 3),
+                m=_bin_terms(theta, th.idx_m, nt, th.n_m_terms, 2))
 
 
 def emulator_inputs(th, theta, z_nodes):

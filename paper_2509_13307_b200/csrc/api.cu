@@ -92,7 +92,12 @@ nsgpu_status build_shear(nsgpu_ctx* ctx, const nsgpu_theory* t) {
   const int idx[] = {t->idx_omega_b, t->idx_omega_cdm, t->idx_h, t->idx_dz, t->idx_ia, t->idx_m};
   for (int v : idx)
     if (v < 0 || v >= ctx->D) { ctx->err = "shear theory: parameter index out of range"; return NSGPU_EINVAL; }
-  if (t->idx_dz + t->n_tomo > ctx->D || t->idx_ia + 3 * t->n_tomo > ctx->D || t->idx_m + 2 * t->n_tomo > ctx->D ||
+  if (t->n_ia_terms < 1 || t->n_ia_terms > 3 || t->n_m_terms < 1 || t->n_m_terms > 2) {
+    ctx->err = "shear theory: n_ia_terms must be 1..3 and n_m_terms 1..2";
+    return NSGPU_EINVAL;
+  }
+  if (t->idx_dz + t->n_tomo > ctx->D || t->idx_ia + t->n_ia_terms * t->n_tomo > ctx->D ||
+      t->idx_m + t->n_m_terms * t->n_tomo > ctx->D ||
       t->idx_w0 >= ctx->D || t->idx_wa >= ctx->D || t->idx_eta0 >= ctx->D) {
     ctx->err = "shear theory: parameter block exceeds D";
     return NSGPU_EINVAL;
@@ -103,6 +108,7 @@ nsgpu_status build_shear(nsgpu_ctx* ctx, const nsgpu_theory* t) {
   S.dlk = (log10(t->k_max) - log10(t->k_min)) / (t->n_k - 1);
   S.idx_omega_b = t->idx_omega_b; S.idx_omega_cdm = t->idx_omega_cdm; S.idx_h = t->idx_h; S.idx_w0 = t->idx_w0;
   S.idx_wa = t->idx_wa; S.idx_eta0 = t->idx_eta0; S.idx_dz = t->idx_dz; S.idx_ia = t->idx_ia; S.idx_m = t->idx_m;
+  S.n_ia_terms = t->n_ia_terms; S.n_m_terms = t->n_m_terms;
   // quadrature nodes: midpoints of n_chi equal cells in the scale factor, a = 1 .. 1/(1+z_max) (S3)
   const double a_min = 1.0 / (1.0 + t->z_max);
   S.da = (1.0 - a_min) / t->n_chi;
@@ -159,6 +165,11 @@ nsgpu_status build_shear(nsgpu_ctx* ctx, const nsgpu_theory* t) {
   NSGPU_CUDA(upload(&S.nz_mean, t->nz_mean, (size_t)t->n_tomo));
   NSGPU_CUDA(upload(&ctx->z_emu, zef.data(), zef.size()));
   NSGPU_CUDA(cudaMalloc((void**)&S.aux, (size_t)ctx->max_batch * (3 + t->n_tomo) * t->n_chi * sizeof(double)));
+  // the resident projection keeps a theta's table and scratch in shared memory (two CTAs per SM); larger
+  // grids -- the paper's 1025 nodes and 10 bins -- take the streaming kernels
+  S.streaming = (ctx->flags & NSGPU_SHEAR_STREAM) != 0 || shear_resident_smem(S) > 113 * 1024;
+  if (S.streaming)
+    NSGPU_CUDA(cudaMalloc((void**)&S.pg, (size_t)ctx->max_batch * t->n_ell * ((t->n_chi + 1) & ~1) * sizeof(double)));
   return NSGPU_OK;
 }
 
@@ -309,10 +320,11 @@ nsgpu_status create_impl(nsgpu_ctx* ctx, int32_t D, const nsgpu_prior1d* prior, 
     }
     // stored transposed: LinvT[j][i] = Linv[i][j] (non-zero for i >= j), so that for a fixed column j the
     // rows i are contiguous -- coalesced for the row-per-thread chi^2 kernel
-    std::vector<double> LinvT(n * n + 2, 0.0);   // + padding: the chi^2 kernel copies whole 16-byte units
+    const size_t ns = n + (n & 1);               // even row stride: every 16-byte unit of a row starts at an even column
+    std::vector<double> LinvT(n * ns, 0.0);
     for (size_t i = 0; i < n; ++i)
-      for (size_t j = 0; j <= i; ++j) LinvT[j * n + i] = Linv[i * n + j];
-    NSGPU_CUDA(upload(&ctx->Linv, LinvT.data(), n * n + 2));
+      for (size_t j = 0; j <= i; ++j) LinvT[j * ns + i] = Linv[i * n + j];
+    NSGPU_CUDA(upload(&ctx->Linv, LinvT.data(), n * ns));
     NSGPU_CUDA(upload(&ctx->data, data, n));
   }
   }
@@ -395,7 +407,7 @@ extern "C" nsgpu_status nsgpu_destroy(nsgpu_ctx* ctx) {
   cudaFree(ctx->emu_in_idx); cudaFree(ctx->emu_in_const); cudaFree(ctx->z_emu);
   cudaFree(ctx->bin_ptr); cudaFree(ctx->bin_col); cudaFree(ctx->bin_val);
   ShearDev& S = ctx->sh;
-  cudaFree(S.aux); cudaFree(S.a_q); cudaFree(S.z_q); cudaFree(S.ln1pz); cudaFree(S.lellh); cudaFree(S.lf); cudaFree(S.tap_start); cudaFree(S.tap_w); cudaFree(S.ell); cudaFree(S.nz_mean);
+  cudaFree(S.aux); cudaFree(S.pg); cudaFree(S.a_q); cudaFree(S.z_q); cudaFree(S.ln1pz); cudaFree(S.lellh); cudaFree(S.lf); cudaFree(S.tap_start); cudaFree(S.tap_w); cudaFree(S.ell); cudaFree(S.nz_mean);
   cudaFree(ctx->data); cudaFree(ctx->Linv); cudaFree(ctx->tt_a); cudaFree(ctx->tt_b); cudaFree(ctx->tt_mu);
   cudaFree(ctx->act[0]); cudaFree(ctx->act[1]); cudaFree(ctx->spec); cudaFree(ctx->model);
   cudaFree(ctx->theta_stage); cudaFree(ctx->logL_stage);

@@ -20,7 +20,10 @@ namespace {
 // The column index is uniform across a warp, so the residuals r[j][.] are one broadcast line of
 // shared memory (a per-lane column made every load a 26-way bank conflict) and the factor elements
 // S[j][row] are conflict-free; LinvT is stored as a full matrix whose upper part is zero, so lanes for
-// which column j lies above their row just add 0.  fp64 throughout; chi^2 = sum over rows of w^2.
+// which column j lies above their row just add 0.  Only the part of a chunk that can be non-zero is
+// copied (rows i >= first column of the chunk: half the factor on average; LinvT rows have an even stride
+// so that every such piece is 16-byte aligned); rows above it are masked, never read.
+// fp64 throughout; chi^2 = sum over rows of w^2.
 template <int TB, int TG, int MAXT>
 __global__ void __launch_bounds__(MAXT) chi2_kernel(const double* __restrict__ model, const double* __restrict__ data,
                                                      const double* __restrict__ LinvT, int n, int B, int RT, int CH,
@@ -36,19 +39,31 @@ __global__ void __launch_bounds__(MAXT) chi2_kernel(const double* __restrict__ m
   double* part = r + (size_t)n * TB;                     // [32][TB] per-warp partial chi^2
   constexpr int NBUF = 4;                                // factor chunks in flight: copy latency, not bandwidth, bounds a CTA
   unsigned long long* bars = reinterpret_cast<unsigned long long*>(part + 32 * TB);   // full[NBUF], empty[NBUF]
-  double* S = reinterpret_cast<double*>(bars + 2 * NBUF);  // [NBUF][CH][n], 16-byte aligned (n TB even)
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarp = blockDim.x >> 5;
   const uint32_t full0 = tc::smem_u32(bars), empty0 = full0 + 8 * NBUF;
+  double* S = reinterpret_cast<double*>(bars + 2 * NBUF);  // [NBUF][CH][ns], 16-byte aligned (n TB even)
+  const int ns = n + (n & 1);
+  // chunk c -> buffer: columns j0 .. j0 + jn, rows j0 .. ns of each (one bulk copy per column)
+  const bool tri = (size_t)CH * ns * 8 >= 16 * 1024;       // small chunks: one copy of whole rows is cheaper to issue
+  auto load_chunk = [&](int c, int buf) {
+    const int j0 = c * CH, jn = min(CH, n - j0);
+    if (!tri) {
+      const uint32_t bytes = (uint32_t)jn * ns * 8u;
+      tc::mbar_arrive_expect_tx(full0 + 8 * buf, bytes);
+      tc::bulk_load(tc::smem_u32(S + (size_t)buf * CH * ns), LinvT + (size_t)j0 * ns, bytes, full0 + 8 * buf);
+      return;
+    }
+    const uint32_t bytes = (uint32_t)(ns - j0) * 8u;
+    tc::mbar_arrive_expect_tx(full0 + 8 * buf, bytes * jn);
+    for (int jj = 0; jj < jn; ++jj)
+      tc::bulk_load(tc::smem_u32(S + ((size_t)buf * CH + jj) * ns + j0), LinvT + (size_t)(j0 + jj) * ns + j0, bytes,
+                    full0 + 8 * buf);
+  };
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarp = blockDim.x >> 5;
   const int n_chunks = (n + CH - 1) / CH;
   if (tid == 0) {
     for (int b = 0; b < NBUF; ++b) { tc::mbar_init(full0 + 8 * b, 1); tc::mbar_init(empty0 + 8 * b, nwarp); }
     tc::fence_barrier_init();
-    for (int c = 0; c < NBUF - 1 && c < n_chunks; ++c) {     // prologue: NBUF-1 chunks in flight
-      const int j1 = c * CH;
-      const uint32_t bytes = ((uint32_t)min(CH, n - j1) * n * 8u + 15u) & ~15u;   // LinvT has 2 doubles of padding
-      tc::mbar_arrive_expect_tx(full0 + 8 * c, bytes);
-      tc::bulk_load(tc::smem_u32(S + (size_t)c * CH * n), LinvT + (size_t)j1 * n, bytes, full0 + 8 * c);
-    }
+    for (int c = 0; c < NBUF - 1 && c < n_chunks; ++c) load_chunk(c, c);   // prologue: NBUF-1 chunks in flight
   }
   // residuals, transposed into [j][theta] (coalesced global reads along j)
   for (int i = tid; i < n * TB; i += blockDim.x) {
@@ -71,27 +86,26 @@ __global__ void __launch_bounds__(MAXT) chi2_kernel(const double* __restrict__ m
   for (int c = 0; c < n_chunks; ++c) {
     const int buf = c % NBUF;
     if (tid == 0 && c + NBUF - 1 < n_chunks) {             // refill the buffer chunk c-1 used
-      const int cn = c + NBUF - 1, nb = cn % NBUF, j1 = cn * CH;
+      const int cn = c + NBUF - 1, nb = cn % NBUF;
       if (c >= 1) tc::mbar_wait(empty0 + 8 * nb, ((c - 1) / NBUF) & 1);
-      const uint32_t bytes = ((uint32_t)min(CH, n - j1) * n * 8u + 15u) & ~15u;
-      tc::mbar_arrive_expect_tx(full0 + 8 * nb, bytes);
-      tc::bulk_load(tc::smem_u32(S + (size_t)nb * CH * n), LinvT + (size_t)j1 * n, bytes, full0 + 8 * nb);
+      load_chunk(cn, nb);
     }
     tc::mbar_wait(full0 + 8 * buf, (c / NBUF) & 1);
-    const double* Sb = S + (size_t)buf * CH * n;
+    const double* Sb = S + (size_t)buf * CH * ns;
     const int j0 = c * CH, jn = min(CH, n - j0);
+    const bool has_a = ia >= j0, has_b = ib >= j0;           // rows above the chunk were not copied
     if (j0 <= jb_end) {
 #pragma unroll 4
       for (int jj = 0; jj < jn; ++jj) {
         const int j = j0 + jj;
-        const double lb = Sb[(size_t)jj * n + ib];
+        const double lb = has_b ? Sb[(size_t)jj * ns + ib] : 0.0;
         double v[TG];
 #pragma unroll
         for (int t = 0; t < TG; ++t) v[t] = rg[(size_t)j * TB + t];
 #pragma unroll
         for (int t = 0; t < TG; ++t) wb[t] = fma(lb, v[t], wb[t]);
         if (j <= ja_end) {                                   // warp-uniform: the short rows end early
-          const double la = Sb[(size_t)jj * n + ia];
+          const double la = has_a ? Sb[(size_t)jj * ns + ia] : 0.0;
 #pragma unroll
           for (int t = 0; t < TG; ++t) wa[t] = fma(la, v[t], wa[t]);
         }
@@ -155,9 +169,12 @@ nsgpu_status chi2_loglike(nsgpu_ctx* ctx, const float* theta, int B, const int* 
   while (tg > 2 && groups > 1 && (B + groups * tg - 1) / (groups * tg) < ctx->sm_count / 2) tg >>= 1;
   const int TBv = groups * tg;
   // chunk of CH factor columns per buffer: four buffers within ~100 KB, CH even
-  int CH = (int)((100 * 1024 / 4) / ((size_t)n * 8));
+  const size_t ns = (size_t)n + (n & 1);
+  const size_t smem_fixed = ((size_t)n * TBv + 32 * TBv + 8) * sizeof(double);
+  int CH = (int)((100 * 1024 / 4) / (ns * 8));
   CH = std::max(2, std::min(16, CH & ~1));
-  const size_t smem = ((size_t)n * TBv + 32 * TBv + 8) * sizeof(double) + 4 * (size_t)CH * n * sizeof(double);
+  if (CH < 4 && smem_fixed + 4 * 4 * ns * sizeof(double) <= 216 * 1024) CH = 4;   // large n: use what is left
+  const size_t smem = smem_fixed + 4 * (size_t)CH * ns * sizeof(double);
   if (smem > 220 * 1024) { ctx->err = "chi2: tiles exceed shared memory"; return NSGPU_ESHAPE; }
   StageTimer tm(ctx, 5, st);
   const int grid = (B + TBv - 1) / TBv, threads = groups * RT;
@@ -177,6 +194,7 @@ nsgpu_status chi2_loglike(nsgpu_ctx* ctx, const float* theta, int B, const int* 
   else if (groups == 2 && tg == 8) NSGPU_CHI2_LAUNCH(16, 8, 640);
   else if (groups == 2 && tg == 4) NSGPU_CHI2_LAUNCH(8, 4, 640);
   else if (groups == 2) NSGPU_CHI2_LAUNCH(4, 2, 640);
+  else if (threads <= 640) NSGPU_CHI2_LAUNCH(8, 8, 640);
   else NSGPU_CHI2_LAUNCH(8, 8, 1024);
 #undef NSGPU_CHI2_LAUNCH
 #undef NSGPU_CHI2_ARGS

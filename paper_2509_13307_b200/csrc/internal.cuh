@@ -44,8 +44,10 @@ struct ShearDev {
   double* tap_w = nullptr;                 // [n_chi][n_tap] z-interpolation weights (spline folded in)
   double *ell = nullptr, *nz_mean = nullptr;
   double* aux = nullptr;                   // [max_batch][(3 + n_tomo) n_chi] hand-off between the two projection kernels
+  double* pg = nullptr;                    // streaming path: [max_batch][n_ell][n_chi rounded up to even] P g_q
   int idx_omega_b = -1, idx_omega_cdm = -1, idx_h = -1, idx_w0 = -1, idx_wa = -1, idx_eta0 = -1;
-  int idx_dz = -1, idx_ia = -1, idx_m = -1;
+  int idx_dz = -1, idx_ia = -1, idx_m = -1, n_ia_terms = 3, n_m_terms = 2;
+  bool streaming = false;                  // chunked projection kernels (grids too large for the resident one, or forced)
 };
 
 struct SamplerDev;  // sampler.cu
@@ -145,6 +147,7 @@ nsgpu_status mlp_forward_tc(nsgpu_ctx* ctx, int e, const float* theta, int B, co
 nsgpu_status mlp_tc_prepare(nsgpu_ctx* ctx, int e, const nsgpu_emulator* h);
 void mlp_tc_release(nsgpu_ctx* ctx, int e);
 nsgpu_status shear_project(nsgpu_ctx* ctx, const float* theta, int B, const int* n_rows_dev, cudaStream_t st);
+size_t shear_resident_smem(const ShearDev& S);
 nsgpu_status cmb_bin(nsgpu_ctx* ctx, const float* theta, int B, const int* n_rows_dev, cudaStream_t st);
 nsgpu_status cmb_tt_loglike(nsgpu_ctx* ctx, const float* theta, int B, const int* n_rows_dev, double* logL, cudaStream_t st);
 nsgpu_status copy_model(nsgpu_ctx* ctx, const float* theta, int B, const int* n_rows_dev, cudaStream_t st);

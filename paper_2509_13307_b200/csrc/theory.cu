@@ -84,7 +84,7 @@ struct ShearArgs {
   double k_min, k_max, lk0, dlk, da, nz_sigma;
   const double *a_q, *z_q, *ln1pz, *tap_w, *ell, *lellh, *lf, *nz_mean;
   const int* tap_start;
-  int idx_omega_b, idx_omega_cdm, idx_h, idx_w0, idx_wa, idx_eta0, idx_dz, idx_ia, idx_m;
+  int idx_omega_b, idx_omega_cdm, idx_h, idx_w0, idx_wa, idx_eta0, idx_dz, idx_ia, idx_m, n_ia_terms, n_m_terms;
 };
 
 // One CTA per theta.  Thread 0 starts a bulk asynchronous copy (TMA, cp.async.bulk) of this theta's
@@ -203,8 +203,9 @@ __global__ void __launch_bounds__(SHEAR_THREADS, 2) shear_project_kernel(const f
   for (int it = tid; it < nt * nq; it += blockDim.x) {
     const int i = (int)__umulhi((unsigned)it, nq_magic), q = it - i * nq;
     const double mu = A.nz_mean[i] + (double)th[A.idx_dz + i];
-    const double A0 = th[A.idx_ia + 3 * i], A1 = th[A.idx_ia + 3 * i + 1], A2 = th[A.idx_ia + 3 * i + 2];
-    const double z = A.z_q[q], a = A.a_q[q];
+    const float* ia = th + A.idx_ia + A.n_ia_terms * i;
+    const double A0 = ia[0], A1 = A.n_ia_terms > 1 ? (double)ia[1] : 0.0, A2 = A.n_ia_terms > 2 ? (double)ia[2] : 0.0;
+    const double z = A.z_q[q];
     const double u = (z - mu) * inv_sig;
     const double nz = exp_fast(-0.5 * u * u) * norm;
     const double w = nz * A.da * (1.0 + z) * (1.0 + z);       // n_i(z_q) dz_q, dz = da / a^2
@@ -334,11 +335,310 @@ __global__ void __launch_bounds__(SHEAR_THREADS, 2) shear_project_kernel(const f
     if (live && bl < A.n_ell) {
       const double acc = part == 0 ? a0 : (part == 1 ? a1 : (part == 2 ? a2 : a3));
       const double lf = A.lf[bl];                              // ln(ell/550)/ln 30
-      const double mi = (double)th[A.idx_m + 2 * i] + (double)th[A.idx_m + 2 * i + 1] * lf;
-      const double mj = (double)th[A.idx_m + 2 * j] + (double)th[A.idx_m + 2 * j + 1] * lf;
+      const float* mpi = th + A.idx_m + A.n_m_terms * i;
+      const float* mpj = th + A.idx_m + A.n_m_terms * j;
+      const double mi = (double)mpi[0] + (A.n_m_terms > 1 ? (double)mpi[1] * lf : 0.0);
+      const double mj = (double)mpj[0] + (A.n_m_terms > 1 ? (double)mpj[1] * lf : 0.0);
       model[(size_t)b * n_data + (size_t)p * A.n_ell + bl] = (1.0 + mi) * (1.0 + mj) * acc;
     }
   }
+}
+
+// ---- streaming projection (any grid size) --------------------------------------------------------------
+// The resident kernel above keeps the whole log10 P table and all scratch arrays of a theta in shared
+// memory: that caps it at ~50 z nodes x 420 k and ~100 quadrature nodes.  The paper's own grid is 1025
+// nodes and 10 bins: the two kernels below do the same arithmetic with shared memory that
+// does not grow with the table -- the table is read in place (each lookup touches two 32-byte sectors; the
+// lanes of a warp hold consecutive quadrature nodes, whose taps are neighbours in the [k][z] layout), and
+// the quadrature axis is walked in chunks.
+
+// a6 + a7 for any n_chi: background and total windows to `aux` ([theta][(3 + n_tomo) n_chi]: g_q, log10 chi,
+// 1/chi, W_i).  The suffix scans of the shear windows run G bins at a time so that shared memory is
+// (4 + 2 G) n_chi doubles.
+__global__ void __launch_bounds__(256) shear_windows_kernel(const float* __restrict__ theta, int D,
+                                                            const int* __restrict__ n_rows_dev, ShearArgs A, int G,
+                                                            double* __restrict__ aux) {
+  const int b = blockIdx.x;
+  if (n_rows_dev && b >= *n_rows_dev) return;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int nq = A.n_chi, nt = A.n_tomo, nqp = nq | 1;
+  double* chi = reinterpret_cast<double*>(smem_raw);   // [nqp] f_q da first, then chi_q
+  double* Eq = chi + nqp;
+  double* iD = Eq + nqp;                               // growth integrand first, then 1 / D_q
+  double* ichi = iD + nqp;
+  double* scr = ichi + nqp;                            // [2 G][nqp] scan arrays
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarp = blockDim.x >> 5;
+  const float* th = theta + (size_t)b * D;
+  double* aux_b = aux + (size_t)b * (3 + nt) * nq;
+  const double ob = th[A.idx_omega_b], oc = th[A.idx_omega_cdm], h = th[A.idx_h];
+  const double Om = (ob + oc) / (h * h);
+  const double w0 = A.idx_w0 >= 0 ? (double)th[A.idx_w0] : -1.0;
+  const double wa = A.idx_wa >= 0 ? (double)th[A.idx_wa] : 0.0;
+  const double gam = 0.55 + 0.05 * (1.0 + w0 + 0.5 * wa);
+  const double de_exp = 3.0 * (1.0 + w0 + wa);
+  for (int q = tid; q < nq; q += blockDim.x) {
+    const double a = A.a_q[q], z = A.z_q[q], opz = 1.0 + z;
+    const double E2 = Om * opz * opz * opz + (1.0 - Om) * exp_fast(de_exp * A.ln1pz[q] - 3.0 * wa * z / opz);
+    const double E = sqrt(E2);
+    const double fda = A.da / (a * a * E);
+    const double gi = exp_fast(gam * log(Om / (a * a * a) / E2)) * A.da / a;
+    Eq[q] = E; chi[q] = fda; iD[q] = gi;
+    scr[q] = fda; scr[nqp + q] = gi;
+  }
+  __syncthreads();
+  if (warp == 0) warp_scan_exclusive(scr, nq, false, lane);
+  else if (warp == 1) warp_scan_exclusive(scr + nqp, nq, false, lane);
+  __syncthreads();
+  for (int q = tid; q < nq; q += blockDim.x) {
+    const double fda = chi[q];
+    const double c = C_OVER_H0 * (scr[q] + 0.5 * fda);
+    const double ic = rcp_fast(c);
+    chi[q] = c;
+    ichi[q] = ic;
+    iD[q] = exp_fast(scr[nqp + q] + 0.5 * iD[q]);
+    aux_b[q] = C_OVER_H0 * fda * ic * ic;               // g_q = dchi_q / chi_q^2
+    aux_b[nq + q] = log10(c);
+    aux_b[2 * nq + q] = ic;
+  }
+  __syncthreads();
+  const double inv_sig = 1.0 / A.nz_sigma;
+  const double norm = inv_sig / 2.5066282746310002;
+  double* Wt = aux_b + 3 * (size_t)nq;
+  for (int i0 = 0; i0 < nt; i0 += G) {
+    const int g = min(G, nt - i0);
+    for (int it = tid; it < g * nq; it += blockDim.x) {
+      const int ii = it / nq, q = it - ii * nq, i = i0 + ii;
+      const double mu = A.nz_mean[i] + (double)th[A.idx_dz + i];
+      const float* ia = th + A.idx_ia + A.n_ia_terms * i;
+      const double A0 = ia[0], A1 = A.n_ia_terms > 1 ? (double)ia[1] : 0.0, A2 = A.n_ia_terms > 2 ? (double)ia[2] : 0.0;
+      const double z = A.z_q[q];
+      const double u = (z - mu) * inv_sig;
+      const double nz = exp_fast(-0.5 * u * u) * norm;
+      const double w = nz * A.da * (1.0 + z) * (1.0 + z);
+      scr[(size_t)(2 * ii) * nqp + q] = w;
+      scr[(size_t)(2 * ii + 1) * nqp + q] = w * ichi[q];
+      const double x = (1.0 + z) / 1.62 - 1.0;
+      const double Aia = A0 + A1 * x + A2 * x * x;
+      Wt[(size_t)i * nq + q] = -Aia * (C1_RHOCR / C_OVER_H0) * Om * iD[q] * nz * Eq[q];   // W^I (eq. A4)
+    }
+    __syncthreads();
+    for (int c = warp; c < 2 * g; c += nwarp) warp_scan_exclusive(scr + (size_t)c * nqp, nq, true, lane);
+    __syncthreads();
+    for (int it = tid; it < g * nq; it += blockDim.x) {   // same thread wrote W^I at this address above
+      const int ii = it / nq, q = it - ii * nq, i = i0 + ii;
+      const double s0 = scr[(size_t)(2 * ii) * nqp + q], s1 = scr[(size_t)(2 * ii + 1) * nqp + q];
+      Wt[(size_t)i * nq + q] += 1.5 * Om / (C_OVER_H0 * C_OVER_H0) * (1.0 + A.z_q[q]) * chi[q] * (s0 - chi[q] * s1);
+    }
+    __syncthreads();
+  }
+}
+
+// a5 + a8 (lookup) for any grid: P(k = (ell + 1/2)/chi_q, z_q) g_q for every (ell, q) to `pg` ([theta][ell][nq2],
+// nq2 = n_chi rounded up to even).  One thread per (q, group of 4 ell), consecutive lanes = consecutive q; the
+// table is read in place: no shared memory, so the SM holds 2048 threads and the L2 latency of the 16 loads
+// each thread has in flight is covered.
+__global__ void __launch_bounds__(256) shear_power_kernel(const float* __restrict__ theta, int D,
+                                                          const int* __restrict__ n_rows_dev,
+                                                          const float* __restrict__ spec, ShearArgs A,
+                                                          const double* __restrict__ aux, int blocks_per_theta,
+                                                          double* __restrict__ pg) {
+  const int b = blockIdx.x / blocks_per_theta, blk = blockIdx.x - b * blocks_per_theta;
+  if (n_rows_dev && b >= *n_rows_dev) return;
+  const int nq = A.n_chi, nq2 = (nq + 1) & ~1, n_lg4 = (A.n_ell + 3) >> 2;
+  const int it = blk * blockDim.x + threadIdx.x;
+  if (it >= n_lg4 * nq) return;
+  const int lg = it / nq, q = it - lg * nq;
+  const float* th = theta + (size_t)b * D;
+  const float* table = spec + (size_t)b * A.n_z_emu * A.n_k;
+  const double* aux_b = aux + (size_t)b * (3 + A.n_tomo) * nq;
+  double* out = pg + (size_t)b * A.n_ell * nq2 + q;
+  const double eta0 = A.idx_eta0 >= 0 ? (double)th[A.idx_eta0] : 0.7;
+  const double inv_dlk = 1.0 / A.dlk, bar_amp = (eta0 - 0.7) * 0.1;
+  const double g_q = aux_b[q], lc = aux_b[nq + q], ic = aux_b[2 * nq + q];
+  const double* tw = A.tap_w + (size_t)q * A.n_tap;
+  const float* col0 = table + (size_t)A.tap_start[q] * A.sz;
+  const int l0 = 4 * lg, nl = min(4, A.n_ell - l0);
+  double kk[4], ss[4];
+  const float* r0[4];
+  bool ok[4];
+#pragma unroll
+  for (int u = 0; u < 4; ++u) {
+    const int bl = min(l0 + u, A.n_ell - 1);
+    kk[u] = (A.ell[bl] + 0.5) * ic;
+    ok[u] = u < nl && kk[u] >= A.k_min && kk[u] <= A.k_max;
+    const double x = A.lellh[bl] - lc;
+    int j = (int)floor((x - A.lk0) * inv_dlk);
+    j = min(max(j, 0), A.n_k - 2);
+    ss[u] = (x - (A.lk0 + j * A.dlk)) * inv_dlk;
+    r0[u] = col0 + (size_t)j * A.sk;
+  }
+  double lo[4], hi[4];
+  if (A.n_tap == 2) {
+    float f[4][4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {   // all 16 loads are issued before the first use
+      f[u][0] = __ldg(r0[u]); f[u][1] = __ldg(r0[u] + A.sz); f[u][2] = __ldg(r0[u] + A.sk); f[u][3] = __ldg(r0[u] + A.sk + A.sz);
+    }
+    const double tw0 = tw[0], tw1 = tw[1];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      lo[u] = fma(tw1, (double)f[u][1], tw0 * (double)f[u][0]);
+      hi[u] = fma(tw1, (double)f[u][3], tw0 * (double)f[u][2]);
+    }
+  } else {
+#pragma unroll
+    for (int u = 0; u < 4; ++u) { lo[u] = 0.0; hi[u] = 0.0; }
+    for (int t = 0; t < A.n_tap; ++t) {
+      const double w = tw[t];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        lo[u] = fma(w, (double)__ldg(r0[u] + (size_t)t * A.sz), lo[u]);
+        hi[u] = fma(w, (double)__ldg(r0[u] + (size_t)t * A.sz + A.sk), hi[u]);
+      }
+    }
+  }
+#pragma unroll
+  for (int u = 0; u < 4; ++u) {
+    if (u >= nl) break;
+    double P = 0.0;
+    if (ok[u]) {
+      double y = fma(ss[u], hi[u] - lo[u], lo[u]);
+      const double k2 = kk[u] * kk[u];
+      const float k2f = (float)k2;                     // |bar_amp| <= 0.03: fp32 is 3e-9 of log10 P here
+      y -= bar_amp * (double)__fdividef(k2f, k2f + 1.0f);
+      P = exp_fast(y * 2.302585092994046);
+    }
+    out[(size_t)(l0 + u) * nq2] = P * g_q;
+  }
+}
+
+// a8 (sum) for any grid: C_ij(ell) = sum_q W_i W_j (P g)_q as a register-tiled product over chunks of QC
+// quadrature nodes.  A thread owns 2 x 2 bin pairs x LB multipoles (20 accumulators) and every NS-th node of
+// the chunk.  The lanes of a warp are different tiles at the SAME node: a shared-memory load touches at most
+// 5 distinct rows, which the odd row stride puts in different banks -- one wavefront per load, so the 9 loads
+// per node stay under the 24 fp64 operations they feed.
+constexpr int LIMBER_THREADS = 256;
+constexpr int LIMBER_LB = 5;      // multipoles per thread tile
+constexpr int LIMBER_QC = 128;    // quadrature nodes per chunk
+constexpr int LIMBER_QCP = LIMBER_QC + 1;
+__global__ void __launch_bounds__(LIMBER_THREADS, 2) shear_limber_kernel(const float* __restrict__ theta, int D,
+                                                                         const int* __restrict__ n_rows_dev, ShearArgs A,
+                                                                         const double* __restrict__ aux,
+                                                                         const double* __restrict__ pg_all, int IW,
+                                                                         double* __restrict__ model, int n_data) {
+  const int b = blockIdx.x;
+  if (n_rows_dev && b >= *n_rows_dev) return;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int nq = A.n_chi, nq2 = (nq + 1) & ~1, nt = A.n_tomo;
+  const int ntp = (nt + 1) & ~1, n_lb = (A.n_ell + LIMBER_LB - 1) / LIMBER_LB, nlp = n_lb * LIMBER_LB;
+  double* Wc = reinterpret_cast<double*>(smem_raw);     // two buffers of [ntp][QCP] windows + [nlp][QCP] P g
+  double* Pg = Wc + (size_t)ntp * LIMBER_QCP;
+  const int tid = threadIdx.x;
+  const float* th = theta + (size_t)b * D;
+  const double* w_b = aux + ((size_t)b * (3 + nt) + 3) * nq;
+  const double* pg_b = pg_all + (size_t)b * A.n_ell * nq2;
+  for (int i = tid; i < 2 * (ntp + nlp) * LIMBER_QCP; i += blockDim.x) Wc[i] = 0.0;   // padding rows stay zero
+
+  // this thread's tile: IW = tiles rounded up to whole warps, NS = slices of the quadrature axis
+  const int n_ib = ntp >> 1, n_items = n_ib * (n_ib + 1) / 2 * n_lb;
+  const int slice = tid / IW, item = tid - slice * IW, NS = blockDim.x / IW;
+  const bool live = item < n_items && slice < NS;
+  int ib = 0, jb = 0, lb = 0;
+  if (live) {
+    const int bp = item / n_lb;
+    lb = item - bp * n_lb;
+    int rem = bp;
+    while (rem >= n_ib - ib) { rem -= n_ib - ib; ++ib; }
+    jb = ib + rem;
+  }
+  const double* wi = Wc + (size_t)(2 * ib) * LIMBER_QCP;
+  const double* wj = Wc + (size_t)(2 * jb) * LIMBER_QCP;
+  const double* pg = Pg + (size_t)(lb * LIMBER_LB) * LIMBER_QCP;
+  double acc[4][LIMBER_LB];
+#pragma unroll
+  for (int c = 0; c < 4; ++c)
+#pragma unroll
+    for (int u = 0; u < LIMBER_LB; ++u) acc[c][u] = 0.0;
+
+  // chunk c of the windows and of P g goes to buffer c & 1 by 8-byte asynchronous copies (the rows of `aux`
+  // start at odd element offsets), issued one chunk ahead of the arithmetic
+  const int n_chunks = (nq + LIMBER_QC - 1) / LIMBER_QC;
+  const size_t buf_doubles = (size_t)(ntp + nlp) * LIMBER_QCP;
+  auto stage = [&](int c) {
+    const int q0 = c * LIMBER_QC, qn = min(LIMBER_QC, nq - q0);
+    double* Wb = Wc + (size_t)(c & 1) * buf_doubles;
+    double* Pb = Wb + (size_t)ntp * LIMBER_QCP;
+    for (int i = tid; i < (nt + A.n_ell) * LIMBER_QC; i += blockDim.x) {
+      const int r = i / LIMBER_QC, qq = i - r * LIMBER_QC;
+      double* dst = (r < nt ? Wb + (size_t)r * LIMBER_QCP : Pb + (size_t)(r - nt) * LIMBER_QCP) + qq;
+      if (qq < qn) {
+        const double* src = r < nt ? w_b + (size_t)r * nq + q0 + qq : pg_b + (size_t)(r - nt) * nq2 + q0 + qq;
+        asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((unsigned)__cvta_generic_to_shared(dst)), "l"(src) : "memory");
+      } else {
+        *dst = 0.0;                                      // ragged tail of the last chunk
+      }
+    }
+    asm volatile("cp.async.commit_group;" ::: "memory");
+  };
+  __syncthreads();                                       // zero fill done
+  stage(0);
+  for (int c = 0; c < n_chunks; ++c) {
+    if (c + 1 < n_chunks) {
+      stage(c + 1);                                      // buffer (c + 1) & 1 was consumed before the barrier that ended chunk c - 1
+      asm volatile("cp.async.wait_group 1;" ::: "memory");
+    } else {
+      asm volatile("cp.async.wait_group 0;" ::: "memory");
+    }
+    __syncthreads();
+    if (live) {
+      const size_t o = (size_t)(c & 1) * buf_doubles;
+      const double *wi_c = wi + o, *wj_c = wj + o, *pg_c = pg + o;
+#pragma unroll 2
+      for (int qq = slice; qq < LIMBER_QC; qq += NS) {
+        const double a0 = wi_c[qq], a1 = wi_c[LIMBER_QCP + qq], b0 = wj_c[qq], b1 = wj_c[LIMBER_QCP + qq];
+        const double w00 = a0 * b0, w01 = a0 * b1, w10 = a1 * b0, w11 = a1 * b1;
+#pragma unroll
+        for (int u = 0; u < LIMBER_LB; ++u) {
+          const double p = pg_c[(size_t)u * LIMBER_QCP + qq];
+          acc[0][u] = fma(w00, p, acc[0][u]); acc[1][u] = fma(w01, p, acc[1][u]);
+          acc[2][u] = fma(w10, p, acc[2][u]); acc[3][u] = fma(w11, p, acc[3][u]);
+        }
+      }
+    }
+    __syncthreads();                                     // chunk c consumed: its buffer may be refilled
+  }
+  // join the slices in a fixed order through shared memory (the chunk buffers are free now): slice s parks
+  // its sums, slice 0 adds them
+  double* red = Wc;                                      // [IW][20] <= (ntp + nlp) QCP doubles (host-checked)
+  for (int s = 1; s < NS; ++s) {
+    __syncthreads();
+    if (live && slice == s)
+#pragma unroll
+      for (int c = 0; c < 4; ++c)
+#pragma unroll
+        for (int u = 0; u < LIMBER_LB; ++u) red[(size_t)(c * LIMBER_LB + u) * IW + item] = acc[c][u];
+    __syncthreads();
+    if (live && slice == 0)
+#pragma unroll
+      for (int c = 0; c < 4; ++c)
+#pragma unroll
+        for (int u = 0; u < LIMBER_LB; ++u) acc[c][u] += red[(size_t)(c * LIMBER_LB + u) * IW + item];
+  }
+  if (!live || slice != 0) return;
+#pragma unroll
+  for (int c = 0; c < 4; ++c)
+#pragma unroll
+    for (int u = 0; u < LIMBER_LB; ++u) {
+      const int i = 2 * ib + (c >> 1), j = 2 * jb + (c & 1), bl = lb * LIMBER_LB + u;
+      if (i > j || j >= nt || bl >= A.n_ell) continue;
+      const int p = i * nt - i * (i - 1) / 2 + (j - i);
+      const double lf = A.lf[bl];
+      const float* mpi = th + A.idx_m + A.n_m_terms * i;
+      const float* mpj = th + A.idx_m + A.n_m_terms * j;
+      const double mi = (double)mpi[0] + (A.n_m_terms > 1 ? (double)mpi[1] * lf : 0.0);
+      const double mj = (double)mpj[0] + (A.n_m_terms > 1 ? (double)mpj[1] * lf : 0.0);
+      model[(size_t)b * n_data + (size_t)p * A.n_ell + bl] = (1.0 + mi) * (1.0 + mj) * acc[c][u];
+    }
 }
 
 // a9: one CTA per theta.  Stage the n_emu spectra in shared memory (coalesced, 10^y applied once per
@@ -438,6 +738,40 @@ nsgpu_status shear_project(nsgpu_ctx* ctx, const float* theta, int B, const int*
   A.nz_mean = S.nz_mean; A.tap_start = S.tap_start;
   A.idx_omega_b = S.idx_omega_b; A.idx_omega_cdm = S.idx_omega_cdm; A.idx_h = S.idx_h; A.idx_w0 = S.idx_w0;
   A.idx_wa = S.idx_wa; A.idx_eta0 = S.idx_eta0; A.idx_dz = S.idx_dz; A.idx_ia = S.idx_ia; A.idx_m = S.idx_m;
+  A.n_ia_terms = S.n_ia_terms; A.n_m_terms = S.n_m_terms;
+  StageTimer tm(ctx, 3, st);
+  if (S.streaming) {
+    const size_t nqp = (size_t)S.n_chi | 1;
+    // bins per scan pass: as many as keep the windows kernel at three CTAs per SM
+    int G = S.n_tomo;
+    while (G > 1 && (4 + 2 * (size_t)G) * nqp * sizeof(double) > 72 * 1024) --G;
+    const size_t smem_w = (4 + 2 * (size_t)G) * nqp * sizeof(double);
+    const int ntp = (S.n_tomo + 1) & ~1, n_lb = (S.n_ell + LIMBER_LB - 1) / LIMBER_LB;
+    const int n_items = (ntp / 2) * (ntp / 2 + 1) / 2 * n_lb;
+    if (n_items > LIMBER_THREADS || smem_w > 220 * 1024) {
+      ctx->err = "shear: n_tomo x n_ell or n_chi too large for the streaming projection";
+      return NSGPU_ESHAPE;
+    }
+    const int IW = (n_items + 31) & ~31;                  // tiles per slice of the quadrature axis, whole warps
+    const size_t smem_l = std::max((size_t)2 * (ntp + n_lb * LIMBER_LB) * LIMBER_QCP, (size_t)IW * 4 * LIMBER_LB) * sizeof(double);
+    static size_t conf_w = 0, conf_l = 0;
+    if (smem_w > conf_w) {
+      NSGPU_CUDA(cudaFuncSetAttribute(shear_windows_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_w));
+      conf_w = smem_w;
+    }
+    if (smem_l > conf_l) {
+      NSGPU_CUDA(cudaFuncSetAttribute(shear_limber_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_l));
+      conf_l = smem_l;
+    }
+    shear_windows_kernel<<<B, S.n_chi > 256 ? 256 : 128, smem_w, st>>>(theta, ctx->D, n_rows_dev, A, G, S.aux);
+    NSGPU_LAUNCH_CHECK();
+    const int bpt = (((S.n_ell + 3) / 4) * S.n_chi + 255) / 256;
+    shear_power_kernel<<<(unsigned)((size_t)B * bpt), 256, 0, st>>>(theta, ctx->D, n_rows_dev, ctx->spec, A, S.aux, bpt, S.pg);
+    NSGPU_LAUNCH_CHECK();
+    shear_limber_kernel<<<B, LIMBER_THREADS, smem_l, st>>>(theta, ctx->D, n_rows_dev, A, S.aux, S.pg, IW, ctx->model, ctx->n_data);
+    NSGPU_LAUNCH_CHECK();
+    return NSGPU_OK;
+  }
   const size_t smem = shear_smem_bytes(S);
   const size_t smem1 = smem - (size_t)S.n_z_emu * S.n_k * sizeof(float);       // phase 1 stages no table
   static size_t configured = 0;
@@ -450,7 +784,6 @@ nsgpu_status shear_project(nsgpu_ctx* ctx, const float* theta, int B, const int*
   // the two-kernel split needs 16-byte sized / aligned pieces for the bulk copies
   const bool split = ((size_t)S.n_z_emu * S.n_k * 4) % 16 == 0 && ((size_t)(3 + S.n_tomo) * S.n_chi * 8) % 16 == 0 &&
                      ((size_t)3 * S.n_chi * 8) % 16 == 0 && S.aux != nullptr;
-  StageTimer tm(ctx, 3, st);
   if (split) {
     shear_project_kernel<1><<<B, 128, smem1, st>>>(theta, ctx->D, n_rows_dev, ctx->spec, A, S.aux, ctx->model, ctx->n_data);
     NSGPU_LAUNCH_CHECK();
@@ -461,6 +794,9 @@ nsgpu_status shear_project(nsgpu_ctx* ctx, const float* theta, int B, const int*
   NSGPU_LAUNCH_CHECK();
   return NSGPU_OK;
 }
+
+// shared memory of the resident projection; the caller switches to the streaming kernels when it does not fit
+size_t shear_resident_smem(const ShearDev& S) { return shear_smem_bytes(S); }
 
 nsgpu_status cmb_bin(nsgpu_ctx* ctx, const float* theta, int B, const int* n_rows_dev, cudaStream_t st) {
   if (B == 0) return NSGPU_OK;

@@ -18,6 +18,7 @@ OK, EINVAL, ENOMEM, ECUDA, ESHAPE, ENOTSPD, ENOCONV = 0, -1, -2, -3, -4, -5, -6
 STATUS_NAMES = {0: "NSGPU_OK", -1: "NSGPU_EINVAL", -2: "NSGPU_ENOMEM", -3: "NSGPU_ECUDA",
                 -4: "NSGPU_ESHAPE", -5: "NSGPU_ENOTSPD", -6: "NSGPU_ENOCONV"}
 MLP_AUTO, MLP_SIMT, MLP_TC = 0, 1, 2
+SHEAR_STREAM = 4          # OR into `mlp`: streaming projection kernels even for grids that fit shared memory
 
 EXPORTS = ["nsgpu_create", "nsgpu_destroy", "nsgpu_last_error", "nsgpu_prior_transform",
            "nsgpu_loglike_batch", "nsgpu_loglike_batch_host", "nsgpu_emulate_batch", "nsgpu_theory_batch",
@@ -55,7 +56,8 @@ class _Theory(C.Structure):
                 ("ell", _pd), ("nz_mean", _pd), ("nz_sigma", C.c_double),
                 ("idx_omega_b", C.c_int32), ("idx_omega_cdm", C.c_int32), ("idx_h", C.c_int32),
                 ("idx_w0", C.c_int32), ("idx_wa", C.c_int32), ("idx_eta0", C.c_int32),
-                ("idx_dz", C.c_int32), ("idx_ia", C.c_int32), ("idx_m", C.c_int32)]
+                ("idx_dz", C.c_int32), ("idx_ia", C.c_int32), ("idx_m", C.c_int32),
+                ("n_ia_terms", C.c_int32), ("n_m_terms", C.c_int32)]
 
 
 class _RunOpts(C.Structure):
@@ -182,7 +184,7 @@ class Context:
             t.bin_ptr, t.bin_col, t.bin_val = _ptr(bp, _pi), _ptr(bc, _pi), _ptr(bv, _pf)
         if th.kind == 3:
             for name in ("n_z_emu", "n_z", "n_chi", "n_k", "n_ell", "n_tomo", "z_interp", "idx_omega_b", "idx_omega_cdm",
-                         "idx_h", "idx_w0", "idx_wa", "idx_eta0", "idx_dz", "idx_ia", "idx_m"):
+                         "idx_h", "idx_w0", "idx_wa", "idx_eta0", "idx_dz", "idx_ia", "idx_m", "n_ia_terms", "n_m_terms"):
                 setattr(t, name, int(getattr(th, name)))
             t.z_max, t.k_min, t.k_max, t.nz_sigma = float(th.z_max), float(th.k_min), float(th.k_max), float(th.nz_sigma)
             ell = np.ascontiguousarray(th.ell, np.float64); nzm = np.ascontiguousarray(th.nz_mean, np.float64)

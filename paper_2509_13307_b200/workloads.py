@@ -92,8 +92,10 @@ class Theory:
     idx_wa: int = -1      # <0 => wa = 0
     idx_eta0: int = -1
     idx_dz: int = -1      # first of n_tomo photo-z shifts
-    idx_ia: int = -1      # first of 3*n_tomo IA coefficients (A_{i,0..2} bin-major)
-    idx_m: int = -1       # first of 2*n_tomo shear-calibration coefficients (m_{i,0..1} bin-major)
+    idx_ia: int = -1      # first of n_ia_terms*n_tomo IA coefficients (A_{i,0..} bin-major)
+    idx_m: int = -1       # first of n_m_terms*n_tomo shear-calibration coefficients (m_{i,0..} bin-major)
+    n_ia_terms: int = 3   # 3, 2: BASELINE.json configs[2..4]; 1, 1: the paper's single amplitude and bias per bin
+    n_m_terms: int = 2
 
 
 @dataclass
@@ -326,7 +328,8 @@ def attach_cmb_tt_data(wl: Workload, model_fid: np.ndarray, noise: bool = True) 
 # ----------------------------------------------------------------------------------------
 def shear(seed: int = 1002, w0wa: bool = False, fix_w0wa: bool = False, n_z_emu: int = 50,
           n_z: int = 50, width: int = 512, n_hidden: int = 4, n_k: int = 420, n_chi: int = 100,
-          n_ell: int = 20, n_tomo: int = 5, name: Optional[str] = None) -> Workload:
+          n_ell: int = 20, n_tomo: int = 5, name: Optional[str] = None, z_max: float = 2.0,
+          n_ia_terms: int = 3, n_m_terms: int = 2) -> Workload:
     """theta layout (reading S2):
     [omega_b, omega_cdm, h, n_s, lnAs, c_min, (w0, wa,) eta_0, dz_0.., A_{i,0..2} (bin-major), m_{i,0..1}].
     `w0wa` adds w0, wa as sampled parameters; `fix_w0wa` builds the 9-input emulator of the
@@ -338,7 +341,6 @@ def shear(seed: int = 1002, w0wa: bool = False, fix_w0wa: bool = False, n_z_emu:
     cosmo_names = ["omega_b", "omega_cdm", "h", "n_s", "lnAs", "c_min"]
     cosmo_fid = [0.02242, 0.11933, 0.6766, 0.9665, 3.047, 2.6]
     de_rows = [(PRIOR_UNIFORM, -3.0, 1.0), (PRIOR_UNIFORM, -3.0, 2.0)]   # reading S14 (BJ cfg 3)
-    z_max = 2.0
     emu_rows = list(cosmo_rows) + (de_rows if (w0wa or fix_w0wa) else [])
     rows, names, fid = list(cosmo_rows), list(cosmo_names), list(cosmo_fid)
     if w0wa:
@@ -350,13 +352,14 @@ def shear(seed: int = 1002, w0wa: bool = False, fix_w0wa: bool = False, n_z_emu:
         rows.append((PRIOR_GAUSSIAN, 0.0, 0.01)); names.append(f"dz_{i}"); fid.append(0.0)
     idx_ia = len(rows)
     for i in range(n_tomo):
-        for t in range(3):
+        for t in range(n_ia_terms):
             rows.append((PRIOR_UNIFORM, -6.0, 6.0)); names.append(f"A_{i}_{t}")
             fid.append(1.0 - 0.1 * (i + 1) if t == 0 else 0.0)
     idx_m = len(rows)
     for i in range(n_tomo):
         rows.append((PRIOR_GAUSSIAN, 0.01, 0.02)); names.append(f"m_{i}_0"); fid.append(0.01)
-        rows.append((PRIOR_GAUSSIAN, 0.0, 0.02)); names.append(f"m_{i}_1"); fid.append(0.0)
+        if n_m_terms > 1:
+            rows.append((PRIOR_GAUSSIAN, 0.0, 0.02)); names.append(f"m_{i}_1"); fid.append(0.0)
     D = len(rows)
     kind, p0, p1 = _prior_arrays(rows)
     mu_in, sd_in = _in_standardisation(emu_rows + [(PRIOR_UNIFORM, 0.0, z_max)])
@@ -379,7 +382,8 @@ def shear(seed: int = 1002, w0wa: bool = False, fix_w0wa: bool = False, n_z_emu:
                 z_max=z_max, k_min=k_min, k_max=k_max, ell=ell, nz_mean=nz_mean, nz_sigma=0.1,
                 idx_omega_b=0, idx_omega_cdm=1, idx_h=2,
                 idx_w0=(6 if w0wa else -1), idx_wa=(7 if w0wa else -1),
-                idx_eta0=idx_eta0, idx_dz=idx_dz, idx_ia=idx_ia, idx_m=idx_m)
+                idx_eta0=idx_eta0, idx_dz=idx_dz, idx_ia=idx_ia, idx_m=idx_m,
+                n_ia_terms=n_ia_terms, n_m_terms=n_m_terms)
     n_pairs = n_tomo * (n_tomo + 1) // 2
     if name is None:
         name = "shear_w0wa" if w0wa else ("shear_lcdm_restricted" if fix_w0wa else "shear_lcdm")
@@ -402,6 +406,24 @@ def c3b() -> Workload:
 def c4_lcdm() -> Workload:
     """LambdaCDM restriction of c3a: same 9-input emulator weights, w0 = -1, wa = 0 pinned."""
     return shear(seed=1003, fix_w0wa=True, name="c4_shear_lcdm_37d_restricted")
+
+
+def c5(interpolated: bool = True, w0wa: bool = True) -> Workload:
+    """Paper-shape shear: 10 tomographic bins (55 spectra), one
+    A_IA, m and D_z per bin (37/39-D, Table 1, no invented terms), 1025 quadrature nodes evenly spaced in the
+    scale factor down to z = 5.02; emulator at 1025 z nodes, or (`interpolated`, the paper's Shear (I)) on a 10x
+    coarser grid of 103 nodes followed by linear interpolation in z."""
+    nz = 103 if interpolated else 1025
+    return shear(seed=1006, w0wa=w0wa, fix_w0wa=not w0wa, n_z_emu=nz, n_z=nz, n_chi=1025, n_tomo=10, z_max=5.02,
+                 n_ia_terms=1, n_m_terms=1,
+                 name=("c5i" if interpolated else "c5") + "_shear_paper_shape_" + ("39d" if w0wa else "37d"))
+
+
+def tiny_shear_paper(seed: int = 9) -> Workload:
+    """Small workload with the paper-shape parameter layout (one A_IA and m per bin) and a quadrature grid
+    longer than one chunk of the projection kernel."""
+    return shear(seed=seed, w0wa=True, n_z_emu=17, n_z=17, width=48, n_hidden=2, n_k=37, n_chi=301, n_ell=7,
+                 n_tomo=4, z_max=5.02, n_ia_terms=1, n_m_terms=1, name="tiny_shear_paper")
 
 
 def tiny_shear(seed: int = 7, w0wa: bool = True, spline: bool = False) -> Workload:

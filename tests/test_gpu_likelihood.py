@@ -210,3 +210,71 @@ def test_cmb_tt_cosmic_variance_likelihood(name, B):
     err = np.abs(got[rows] - ref)
     assert np.all(err <= loglike_tolerance(chi2_eff)), (err / loglike_tolerance(chi2_eff)).max()
     assert np.sum(chi2_eff <= 2000.0 + wl.n_data) >= 4 or B <= 256
+
+
+def _theory_and_loglike_match(wl, theta, ctx):
+    th64 = theta.astype(np.float64)
+    t = dev(theta)
+    model = ctx.theory_batch(t).cpu().numpy()
+    ref_model = LK.theory(wl, th64)
+    scale = np.abs(ref_model) + np.sqrt(np.mean(ref_model ** 2, axis=1, keepdims=True))
+    assert np.max(np.abs(model - ref_model) / scale) < 2e-4
+    got = ctx.loglike_batch(t).cpu().numpy()
+    ref = LK.loglike(wl, th64)
+    chi2 = -2.0 * (ref - gaussian.log_norm(wl.chol))
+    assert np.all(np.isfinite(got))
+    assert np.all(np.abs(got - ref) <= loglike_tolerance(chi2)), (np.abs(got - ref) / loglike_tolerance(chi2)).max()
+
+
+@pytest.mark.parametrize("name,B", [("tiny_shear", 37), ("tiny_shear_spline", 5), ("tiny_shear_lcdm", 9),
+                                    ("tiny_shear_paper", 21)])
+def test_streaming_projection_small(name, B):
+    """the chunked projection kernels (windows + direct-lookup Limber product) on grids of
+    one chunk and of several chunks with a ragged tail (301 quadrature nodes), odd and even bin counts, two-tap
+    and spline-folded z interpolation, both per-bin coefficient layouts."""
+    wl = workload(name)
+    theta = theta_of_u(wl, np.concatenate([W.u_post_set(wl, B // 2), W.u_prior_set(wl, B - B // 2)]))
+    with nsgpu.Context(wl, max_batch=B, mlp=nsgpu.MLP_SIMT | nsgpu.SHEAR_STREAM) as ctx:
+        _theory_and_loglike_match(wl, theta, ctx)
+
+
+def test_streaming_projection_tensor_core_layout():
+    """streaming kernels against the [k][z] table the tcgen05 output layer writes, and agreement with the
+    resident kernel on the same context inputs"""
+    wl = W.shear(seed=22, w0wa=True, n_z_emu=11, n_z=11, width=64, n_hidden=2, n_k=40, n_chi=150, n_ell=11, n_tomo=5,
+                 z_max=3.0, n_ia_terms=1, n_m_terms=2, name="s64p")
+    th0 = theta_of_u(wl, wl.u_fid[None]).astype(np.float64)
+    W.attach_data(wl, LK.theory(wl, th0)[0])
+    theta = theta_of_u(wl, np.concatenate([W.u_post_set(wl, 40), W.u_prior_set(wl, 30)]))
+    out = []
+    for flags in (nsgpu.MLP_TC | nsgpu.SHEAR_STREAM, nsgpu.MLP_TC):
+        with nsgpu.Context(wl, max_batch=70, mlp=flags) as ctx:
+            _theory_and_loglike_match(wl, theta, ctx)
+            out.append(ctx.theory_batch(dev(theta)).cpu().numpy())
+    # same table; fp64 both ways except the baryon term of the streaming lookups (fp32: <= 3e-9 of log10 P)
+    assert np.max(np.abs(out[0] - out[1]) / (np.abs(out[1]) + 1e-300)) < 1e-7
+
+
+@pytest.mark.parametrize("name,B", [("c5i", 512), ("c5", 96)])
+def test_paper_shape_shear_sampled_parity(name, B):
+    """Paper-shape shear: 10 bins / 55 spectra, 1025 quadrature nodes to z = 5.02, one
+    A_IA, m, D_z per bin (39-D); emulator on 103 nodes + linear z interpolation (Shear (I)) or on 1025 nodes."""
+    wl = workload(name)
+    # 1100 data points: chi^2 ~ 1100 at the truth, so the posterior-like set sits closer to it than for c1-c3
+    u = np.concatenate([W.u_post_set(wl, B // 2, scale=0.002), W.u_prior_set(wl, B // 2)])
+    theta = theta_of_u(wl, u)
+    rows = np.r_[0:4, B // 2 - 2:B // 2 + 4, B - 2:B]
+    with nsgpu.Context(wl, max_batch=B) as ctx:
+        t = dev(theta)
+        got = ctx.loglike_batch(t).cpu().numpy()
+        model = ctx.theory_batch(t[rows].contiguous()).cpu().numpy()
+    assert np.all(np.isfinite(got))
+    th64 = theta[rows].astype(np.float64)
+    ref_model = LK.theory(wl, th64)
+    scale = np.abs(ref_model) + np.sqrt(np.mean(ref_model ** 2, axis=1, keepdims=True))
+    assert np.max(np.abs(model - ref_model) / scale) < 2e-4
+    ref = LK.loglike(wl, th64)
+    chi2 = -2.0 * (ref - gaussian.log_norm(wl.chol))
+    err = np.abs(got[rows] - ref)
+    assert np.all(err <= loglike_tolerance(chi2)), (err / loglike_tolerance(chi2)).max()
+    assert np.sum(chi2 <= 2000.0) >= 4

@@ -225,3 +225,32 @@ def test_spline_variant_close_to_full_on_smooth_table():
     a = S.model_vector(full.theory, theta, f(S.z_nodes_emulator(full.theory)))
     b = S.model_vector(spl.theory, theta, f(S.z_nodes_emulator(spl.theory)))
     np.testing.assert_allclose(b, a, rtol=5e-3)
+
+
+def test_single_coefficient_layout_is_the_truncated_expansion():
+    """one A_IA and one m per bin.  The (1, 1) parameter layout must give exactly the model of
+    the (3, 2) layout with the higher coefficients set to zero, and moving A_i / m_i of ONE bin must change
+    exactly the spectra that bin takes part in."""
+    import dataclasses
+    wl = W.tiny_shear_paper()
+    th = wl.theory
+    assert (th.n_ia_terms, th.n_m_terms) == (1, 1) and wl.D == 9 + 3 * th.n_tomo
+    from oracle import prior
+    theta = prior.transform(wl.prior_kind, wl.prior_p0, wl.prior_p1, wl.u_fid)
+    rng = np.random.default_rng(3)
+    theta[th.idx_ia:th.idx_ia + th.n_tomo] = rng.uniform(-2, 2, th.n_tomo)
+    theta[th.idx_m:th.idx_m + th.n_tomo] = rng.uniform(-0.05, 0.05, th.n_tomo)
+    table = 2.0 + 0.1 * rng.standard_normal((th.n_z_emu, th.n_k))
+    m11 = S.model_vector(th, theta, table)
+    # the same physical point in the (3, 2) layout
+    nt = th.n_tomo
+    wide = np.concatenate([theta[:th.idx_ia],
+                           np.stack([theta[th.idx_ia:th.idx_ia + nt], np.zeros(nt), np.zeros(nt)], 1).ravel(),
+                           np.stack([theta[th.idx_m:th.idx_m + nt], np.zeros(nt)], 1).ravel()])
+    th32 = dataclasses.replace(th, n_ia_terms=3, n_m_terms=2, idx_m=th.idx_ia + 3 * nt)
+    np.testing.assert_array_equal(S.model_vector(th32, wide, table), m11)
+    # locality: bin 2's amplitude and bias touch only pairs containing bin 2
+    for idx in (th.idx_ia + 2, th.idx_m + 2):
+        mod = theta.copy(); mod[idx] += 0.3
+        changed = (S.model_vector(th, mod, table) != m11).reshape(-1, th.n_ell).any(axis=1)
+        assert [bool(c) for c in changed] == [2 in ij for ij in S.pair_index(nt)]

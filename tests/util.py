@@ -16,6 +16,7 @@ MAKERS = {
     "tiny_shear_lcdm": lambda: W.tiny_shear(w0wa=False), "tiny_cmb": W.tiny_cmb,
     "c1": W.cmb, "c2": W.c2, "c3a": W.c3a, "c3b": W.c3b, "c4_lcdm": W.c4_lcdm,
     "toy_w64": lambda: W.toy(width=64, n_out=100, n_hidden=3),
+    "tiny_shear_paper": W.tiny_shear_paper, "c5i": lambda: W.c5(True), "c5": lambda: W.c5(False),
     "cmb_tt": W.cmb_tt, "tiny_cmb_tt": lambda: W.cmb_tt(seed=9, width=64, n_hidden=2, ell_max=131),
 }
 
