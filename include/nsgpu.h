@@ -122,6 +122,8 @@ typedef struct {
 #define NSGPU_MLP_AUTO 0u   /* tcgen05 tensor-core MLP where the shape allows it, SIMT otherwise */
 #define NSGPU_MLP_SIMT 1u   /* fp32 CUDA-core MLP (on-device correctness reference) */
 #define NSGPU_MLP_TC 2u     /* require the tcgen05 path (NSGPU_ESHAPE if width % 64 != 0) */
+#define NSGPU_CHI2_STREAMED 8u /* chi^2 by the factor-streaming kernel (one CTA = all rows of 8..32 thetas) whatever n_data */
+#define NSGPU_CHI2_TILED 16u   /* chi^2 by the tiled kernels (128-row blocks x 32..64 thetas) whatever n_data; default: n_data >= 512 */
 #define NSGPU_SHEAR_STREAM 4u /* kind 3: use the streaming projection kernels even where the grids fit shared memory */
 
 /* Create a context on CUDA device `device`.

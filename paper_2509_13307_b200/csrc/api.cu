@@ -339,6 +339,11 @@ nsgpu_status create_impl(nsgpu_ctx* ctx, int32_t D, const nsgpu_prior1d* prior, 
     NSGPU_CUDA(cudaMalloc((void**)&ctx->spec, (size_t)n_emu * M_max * emu[0].n_out * sizeof(float)));
   }
   NSGPU_CUDA(cudaMalloc((void**)&ctx->model, (size_t)max_batch * n_data * sizeof(double)));
+  if (th->kind != 4) {   // chi^2 workspaces: transposed residuals [n_data][batch rounded up to 64], partial sums per row block
+    const size_t bp = ((size_t)max_batch + 63) & ~(size_t)63;
+    NSGPU_CUDA(cudaMalloc((void**)&ctx->resid_t, (size_t)n_data * bp * sizeof(double)));
+    NSGPU_CUDA(cudaMalloc((void**)&ctx->chi2_part, (size_t)((n_data + 127) / 128) * bp * sizeof(double)));
+  }
   NSGPU_CUDA(cudaMalloc((void**)&ctx->theta_stage, (size_t)max_batch * D * sizeof(float)));
   NSGPU_CUDA(cudaMalloc((void**)&ctx->logL_stage, (size_t)max_batch * sizeof(double)));
   NSGPU_CUDA(cudaMallocHost((void**)&ctx->theta_pinned, (size_t)max_batch * D * sizeof(float)));
@@ -409,7 +414,7 @@ extern "C" nsgpu_status nsgpu_destroy(nsgpu_ctx* ctx) {
   ShearDev& S = ctx->sh;
   cudaFree(S.aux); cudaFree(S.pg); cudaFree(S.a_q); cudaFree(S.z_q); cudaFree(S.ln1pz); cudaFree(S.lellh); cudaFree(S.lf); cudaFree(S.tap_start); cudaFree(S.tap_w); cudaFree(S.ell); cudaFree(S.nz_mean);
   cudaFree(ctx->data); cudaFree(ctx->Linv); cudaFree(ctx->tt_a); cudaFree(ctx->tt_b); cudaFree(ctx->tt_mu);
-  cudaFree(ctx->act[0]); cudaFree(ctx->act[1]); cudaFree(ctx->spec); cudaFree(ctx->model);
+  cudaFree(ctx->act[0]); cudaFree(ctx->act[1]); cudaFree(ctx->spec); cudaFree(ctx->model); cudaFree(ctx->resid_t); cudaFree(ctx->chi2_part);
   cudaFree(ctx->theta_stage); cudaFree(ctx->logL_stage);
   cudaFreeHost(ctx->theta_pinned); cudaFreeHost(ctx->logL_pinned);
   cudaGetLastError();

@@ -81,6 +81,8 @@ struct nsgpu_ctx {
   float* spec = nullptr;               // [n_emu][M_max][n_out] de-standardised y (log10 where exp10)
   bool spec_kz = false;                // shear + tcgen05: per theta [n_k][n_z_emu] instead of [n_z_emu][n_k]
   double* model = nullptr;             // [max_batch][n_data]
+  double* resid_t = nullptr;           // [n_data][max_batch rounded up to 64] model - data, transposed (chi^2 operand)
+  double* chi2_part = nullptr;         // [row blocks of 128][max_batch rounded up to 64] partial sums of w^2
   float* theta_stage = nullptr;        // [max_batch][D] device staging for the host entry
   double* logL_stage = nullptr;
   float* theta_pinned = nullptr;       // pinned host staging

@@ -2,6 +2,10 @@
 (37-D), on the synthetic cosmic-shear likelihood (c3a weights; mock data from the LambdaCDM truth).
 
     python -m paper_2509_13307_b200.examples.model_comparison [--n-live 1000] [--n-delete 500] [--seeds 1]
+                                                              [--shape c4|paper-interp|paper]
+
+`--shape paper-interp` / `paper` run the same comparison on the paper-shape likelihood (10 bins, 55 spectra,
+1025 quadrature nodes; emulator on 103 z nodes + linear interpolation, or on all 1025: PAPER.md L353, L359).
 
 Prints one JSON line per run and a summary with log Z +- error per model, the log Bayes factor, total
 likelihood evaluations and wall time.  The mock data vector is produced by the CUDA path itself at the
@@ -36,9 +40,13 @@ def main():
     ap.add_argument("--seeds", type=int, default=1)
     ap.add_argument("--stop-frac", type=float, default=1e-3)
     ap.add_argument("--max-iter", type=int, default=100000)
+    ap.add_argument("--shape", default="c4", choices=["c4", "paper-interp", "paper"])
     args = ap.parse_args()
-    full = _mock_data(W.c3a())
-    rest = W.c4_lcdm()
+    if args.shape == "c4":
+        full, rest = _mock_data(W.c3a()), W.c4_lcdm()
+    else:
+        interp = args.shape == "paper-interp"
+        full, rest = _mock_data(W.c5(interp, w0wa=True)), W.c5(interp, w0wa=False)
     rest.data, rest.chol = full.data, full.chol
     out = {}
     for name, wl in (("w0waCDM", full), ("LCDM", rest)):
@@ -53,7 +61,7 @@ def main():
         out[name] = runs
     z = {k: np.mean([r["logZ"] for r in v]) for k, v in out.items()}
     e = {k: math.sqrt(np.mean([r["logZ_err"] ** 2 for r in v]) / len(v)) for k, v in out.items()}
-    print(json.dumps({"summary": {k: {"logZ": z[k], "err": e[k], "evals": int(np.mean([r["n_like_evals"] for r in v])),
+    print(json.dumps({"shape": args.shape, "summary": {k: {"logZ": z[k], "err": e[k], "evals": int(np.mean([r["n_like_evals"] for r in v])),
                                        "seconds": float(np.mean([r["seconds"] for r in v])),
                                        "iterations": int(np.mean([r["n_iter"] for r in v]))} for k, v in out.items()},
                       "logB_LCDM_over_w0wa": z["LCDM"] - z["w0waCDM"],

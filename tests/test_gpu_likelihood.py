@@ -278,3 +278,20 @@ def test_paper_shape_shear_sampled_parity(name, B):
     err = np.abs(got[rows] - ref)
     assert np.all(err <= loglike_tolerance(chi2)), (err / loglike_tolerance(chi2)).max()
     assert np.sum(chi2 <= 2000.0) >= 4
+
+
+@pytest.mark.parametrize("name,B", [("toy", 300), ("tiny_cmb", 130), ("tiny_shear_paper", 70), ("c1", 200)])
+def test_both_chi2_kernels(name, B):
+    """the factor-streaming and the tiled whitening kernels (row-block tails: n = 100, 23, 70, 613; theta-block
+    tails; one-block and several-block factors) against the oracle, and bit-identical under permutation"""
+    wl = workload(name)
+    theta = theta_of_u(wl, np.concatenate([W.u_post_set(wl, B // 2), W.u_prior_set(wl, B - B // 2)]))
+    ref = LK.loglike(wl, theta.astype(np.float64))
+    chi2 = -2.0 * (ref - gaussian.log_norm(wl.chol))
+    perm = np.random.default_rng(5).permutation(B)
+    for flag in (nsgpu.CHI2_STREAMED, nsgpu.CHI2_TILED):
+        with nsgpu.Context(wl, max_batch=B + 5, mlp=flag) as ctx:
+            got = ctx.loglike_batch(dev(theta)).cpu().numpy()
+            got_p = ctx.loglike_batch(dev(theta[perm])).cpu().numpy()
+        assert np.all(np.abs(got - ref) <= loglike_tolerance(chi2)), flag
+        np.testing.assert_array_equal(got_p, got[perm])
