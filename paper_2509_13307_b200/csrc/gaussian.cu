@@ -43,7 +43,7 @@ __global__ void __launch_bounds__(MAXT) chi2_kernel(const double* __restrict__ m
   double* S = reinterpret_cast<double*>(bars + 2 * NBUF);  // [NBUF][CH][ns], 16-byte aligned (n TB even)
   const int ns = n + (n & 1);
   // chunk c -> buffer: columns j0 .. j0 + jn, rows j0 .. ns of each (one bulk copy per column)
-  const bool tri = (size_t)CH * ns * 8 >= 16 * 1024;       // small chunks: one copy of whole rows is cheaper to issue
+  const bool tri = ns >= 512;                               // short rows: one copy of whole rows is cheaper to issue
   auto load_chunk = [&](int c, int buf) {
     const int j0 = c * CH, jn = min(CH, n - j0);
     if (!tri) {

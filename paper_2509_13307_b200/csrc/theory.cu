@@ -355,6 +355,7 @@ __global__ void __launch_bounds__(SHEAR_THREADS, 2) shear_project_kernel(const f
 // a6 + a7 for any n_chi: background and total windows to `aux` ([theta][(3 + n_tomo) n_chi]: g_q, log10 chi,
 // 1/chi, W_i).  The suffix scans of the shear windows run G bins at a time so that shared memory is
 // (4 + 2 G) n_chi doubles.
+constexpr int WIN_ITEMS = 16;   // (bin, node) items per thread and scan pass
 __global__ void __launch_bounds__(256) shear_windows_kernel(const float* __restrict__ theta, int D,
                                                             const int* __restrict__ n_rows_dev, ShearArgs A, int G,
                                                             double* __restrict__ aux) {
@@ -406,28 +407,39 @@ __global__ void __launch_bounds__(256) shear_windows_kernel(const float* __restr
   double* Wt = aux_b + 3 * (size_t)nq;
   for (int i0 = 0; i0 < nt; i0 += G) {
     const int g = min(G, nt - i0);
-    for (int it = tid; it < g * nq; it += blockDim.x) {
-      const int ii = it / nq, q = it - ii * nq, i = i0 + ii;
-      const double mu = A.nz_mean[i] + (double)th[A.idx_dz + i];
-      const float* ia = th + A.idx_ia + A.n_ia_terms * i;
-      const double A0 = ia[0], A1 = A.n_ia_terms > 1 ? (double)ia[1] : 0.0, A2 = A.n_ia_terms > 2 ? (double)ia[2] : 0.0;
-      const double z = A.z_q[q];
-      const double u = (z - mu) * inv_sig;
-      const double nz = exp_fast(-0.5 * u * u) * norm;
-      const double w = nz * A.da * (1.0 + z) * (1.0 + z);
-      scr[(size_t)(2 * ii) * nqp + q] = w;
-      scr[(size_t)(2 * ii + 1) * nqp + q] = w * ichi[q];
-      const double x = (1.0 + z) / 1.62 - 1.0;
-      const double Aia = A0 + A1 * x + A2 * x * x;
-      Wt[(size_t)i * nq + q] = -Aia * (C1_RHOCR / C_OVER_H0) * Om * iD[q] * nz * Eq[q];   // W^I (eq. A4)
+    double wI[WIN_ITEMS];                                  // W^I of this thread's (bin, node) items, kept across the scans
+#pragma unroll
+    for (int s = 0; s < WIN_ITEMS; ++s) {
+      const int it = tid + s * blockDim.x;
+      wI[s] = 0.0;
+      if (it < g * nq) {
+        const int ii = it / nq, q = it - ii * nq, i = i0 + ii;
+        const double mu = A.nz_mean[i] + (double)th[A.idx_dz + i];
+        const float* ia = th + A.idx_ia + A.n_ia_terms * i;
+        const double A0 = ia[0], A1 = A.n_ia_terms > 1 ? (double)ia[1] : 0.0, A2 = A.n_ia_terms > 2 ? (double)ia[2] : 0.0;
+        const double z = A.z_q[q];
+        const double u = (z - mu) * inv_sig;
+        const double nz = exp_fast(-0.5 * u * u) * norm;
+        const double w = nz * A.da * (1.0 + z) * (1.0 + z);
+        scr[(size_t)(2 * ii) * nqp + q] = w;
+        scr[(size_t)(2 * ii + 1) * nqp + q] = w * ichi[q];
+        const double x = (1.0 + z) / 1.62 - 1.0;
+        const double Aia = A0 + A1 * x + A2 * x * x;
+        wI[s] = -Aia * (C1_RHOCR / C_OVER_H0) * Om * iD[q] * nz * Eq[q];   // W^I (eq. A4)
+      }
     }
     __syncthreads();
     for (int c = warp; c < 2 * g; c += nwarp) warp_scan_exclusive(scr + (size_t)c * nqp, nq, true, lane);
     __syncthreads();
-    for (int it = tid; it < g * nq; it += blockDim.x) {   // same thread wrote W^I at this address above
-      const int ii = it / nq, q = it - ii * nq, i = i0 + ii;
-      const double s0 = scr[(size_t)(2 * ii) * nqp + q], s1 = scr[(size_t)(2 * ii + 1) * nqp + q];
-      Wt[(size_t)i * nq + q] += 1.5 * Om / (C_OVER_H0 * C_OVER_H0) * (1.0 + A.z_q[q]) * chi[q] * (s0 - chi[q] * s1);
+#pragma unroll
+    for (int s = 0; s < WIN_ITEMS; ++s) {
+      const int it = tid + s * blockDim.x;
+      if (it < g * nq) {
+        const int ii = it / nq, q = it - ii * nq, i = i0 + ii;
+        const double s0 = scr[(size_t)(2 * ii) * nqp + q], s1 = scr[(size_t)(2 * ii + 1) * nqp + q];
+        Wt[(size_t)i * nq + q] =
+            wI[s] + 1.5 * Om / (C_OVER_H0 * C_OVER_H0) * (1.0 + A.z_q[q]) * chi[q] * (s0 - chi[q] * s1);   // + W^gamma (eq. A3)
+      }
     }
     __syncthreads();
   }
@@ -744,11 +756,12 @@ nsgpu_status shear_project(nsgpu_ctx* ctx, const float* theta, int B, const int*
     const size_t nqp = (size_t)S.n_chi | 1;
     // bins per scan pass: as many as keep the windows kernel at three CTAs per SM
     int G = S.n_tomo;
-    while (G > 1 && (4 + 2 * (size_t)G) * nqp * sizeof(double) > 72 * 1024) --G;
+    const int win_threads = S.n_chi > 256 ? 256 : 128;
+    while (G > 1 && ((4 + 2 * (size_t)G) * nqp * sizeof(double) > 72 * 1024 || G * S.n_chi > win_threads * WIN_ITEMS)) --G;
     const size_t smem_w = (4 + 2 * (size_t)G) * nqp * sizeof(double);
     const int ntp = (S.n_tomo + 1) & ~1, n_lb = (S.n_ell + LIMBER_LB - 1) / LIMBER_LB;
     const int n_items = (ntp / 2) * (ntp / 2 + 1) / 2 * n_lb;
-    if (n_items > LIMBER_THREADS || smem_w > 220 * 1024) {
+    if (n_items > LIMBER_THREADS || smem_w > 220 * 1024 || G * S.n_chi > win_threads * WIN_ITEMS) {
       ctx->err = "shear: n_tomo x n_ell or n_chi too large for the streaming projection";
       return NSGPU_ESHAPE;
     }
@@ -763,7 +776,7 @@ nsgpu_status shear_project(nsgpu_ctx* ctx, const float* theta, int B, const int*
       NSGPU_CUDA(cudaFuncSetAttribute(shear_limber_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_l));
       conf_l = smem_l;
     }
-    shear_windows_kernel<<<B, S.n_chi > 256 ? 256 : 128, smem_w, st>>>(theta, ctx->D, n_rows_dev, A, G, S.aux);
+    shear_windows_kernel<<<B, win_threads, smem_w, st>>>(theta, ctx->D, n_rows_dev, A, G, S.aux);
     NSGPU_LAUNCH_CHECK();
     const int bpt = (((S.n_ell + 3) / 4) * S.n_chi + 255) / 256;
     shear_power_kernel<<<(unsigned)((size_t)B * bpt), 256, 0, st>>>(theta, ctx->D, n_rows_dev, ctx->spec, A, S.aux, bpt, S.pg);
