@@ -187,6 +187,20 @@ typedef struct {
 NSGPU_API nsgpu_status nsgpu_run(nsgpu_ctx* ctx, const nsgpu_run_opts* opts, nsgpu_result* res, float* theta_samples,
                        double* logL_samples, double* logw_samples, int64_t cap, int64_t* n_samples);
 
+/* Multi-GPU nested sampling: one process per GPU, every rank holds the whole
+ * live set and calls this with the same options.  Rank r evolves the chains nsgpu_shard_range gives it; the only
+ * exchange of an iteration is an all-gather of the k new points, done through `allgather`: send and recv are DEVICE
+ * pointers, every rank contributes bytes_per_rank bytes and receives world * bytes_per_rank bytes ordered by rank
+ * (the layout of ncclAllGather); it must have completed, or be ordered on `stream`, when it returns; non-zero =
+ * failure.  The Philox streams are keyed by the GLOBAL chain index, so the result does not depend on `world`:
+ * every rank returns the same nsgpu_result, equal to nsgpu_run's.  n_like_evals is the total over ranks.         */
+typedef int32_t (*nsgpu_allgather_fn)(void* user, const void* send, void* recv, int64_t bytes_per_rank, void* stream);
+NSGPU_API nsgpu_status nsgpu_run_sharded(nsgpu_ctx* ctx, const nsgpu_run_opts* opts, int32_t rank, int32_t world,
+                               nsgpu_allgather_fn allgather, void* user, nsgpu_result* res, float* theta_samples,
+                               double* logL_samples, double* logw_samples, int64_t cap, int64_t* n_samples);
+/* chains [*first, *first + *count) of n_chains belong to `rank`: contiguous blocks of ceil(n_chains / world). Host only. */
+NSGPU_API void nsgpu_shard_range(int32_t n_chains, int32_t rank, int32_t world, int32_t* first, int32_t* count);
+
 /* Samples of the last nsgpu_run on this ctx (kept until the next run or destroy): same buffers and
  * meaning as nsgpu_run's; *n_samples returns the number available; cap = 0 only queries the count. */
 NSGPU_API nsgpu_status nsgpu_last_samples(nsgpu_ctx* ctx, float* theta_samples, double* logL_samples,

@@ -102,6 +102,7 @@ enum { P_NEW = 0, P_OUT_L = 1, P_OUT_R = 2, P_SHRINK = 3 };
 
 struct RoundArgs {
   int n_chains, D, n_steps;
+  int chain0;              // global id of this launch's chain 0 (sharded runs: the Philox streams are per GLOBAL chain)
   uint2 key;
   unsigned iteration;
   const double* scal;      // [0] = logL_star
@@ -138,7 +139,7 @@ __global__ void __launch_bounds__(128) slice_round_kernel(RoundArgs a) {
   int phase = a.phase[c], cnt = a.cnt[c], step = a.step[c];
   unsigned j = a.rng_j[c];
   const double Lstar = a.scal[0];
-  Stream S{a.key, (unsigned)c, a.iteration, 0u};
+  Stream S{a.key, (unsigned)(a.chain0 + c), a.iteration, 0u};
   bool inside = false;
   double val = 0.0;
   if (a.pending[c]) {
@@ -258,7 +259,7 @@ __global__ void __launch_bounds__(1024) compact_kernel(int n_chains, int D, cons
   }
 }
 
-__global__ void chain_init_kernel(int n_chains, int D, uint2 key, unsigned iteration, const int* __restrict__ surv_idx,
+__global__ void chain_init_kernel(int n_chains, int chain0, int D, uint2 key, unsigned iteration, const int* __restrict__ surv_idx,
                                   int n_surv, const int* __restrict__ start_in, int* __restrict__ start_idx,
                                   const float* __restrict__ u_live, const double* __restrict__ logL_live,
                                   float* x0, double* logL0, int* phase, int* cnt, int* step, int* pending,
@@ -269,7 +270,7 @@ __global__ void chain_init_kernel(int n_chains, int D, uint2 key, unsigned itera
   if (start_in) {
     s = start_in[c];
   } else {   // reading N4: uniform with replacement from the survivors; Stream(seed, c, iteration, tag 1)
-    Stream S{key, (unsigned)c, iteration, 1u};
+    Stream S{key, (unsigned)(chain0 + c), iteration, 1u};
     int pick = (int)(S.uniform(0) * n_surv);
     s = surv_idx[min(pick, n_surv - 1)];
   }
@@ -550,11 +551,11 @@ static nsgpu_status launch_delete(nsgpu_ctx* ctx, const double* logL, int n, int
 
 // Evolve n_chains chains to completion.  Chains were initialised by chain_init_kernel; Lsig and scal[0]
 // (L*) are set.  Host reads the finished-counter after batches of rounds (one small D2H per batch).
-static nsgpu_status evolve(nsgpu_ctx* ctx, int n_chains, int n_steps, uint64_t seed, int iteration, cudaStream_t st,
+static nsgpu_status evolve(nsgpu_ctx* ctx, int n_chains, int chain0, int n_steps, uint64_t seed, int iteration, cudaStream_t st,
                            int64_t* rounds_out) {
   SamplerDev* S = ctx->sampler;
   RoundArgs a;
-  a.n_chains = n_chains; a.D = ctx->D; a.n_steps = n_steps;
+  a.n_chains = n_chains; a.D = ctx->D; a.n_steps = n_steps; a.chain0 = chain0;
   a.key = make_uint2((unsigned)(seed & 0xffffffffu), (unsigned)(seed >> 32));
   a.iteration = (unsigned)iteration;
   a.scal = S->scal; a.Lsig = S->Lsig; a.prior_kind = ctx->prior_kind; a.p0 = ctx->prior_p0; a.p1 = ctx->prior_p1;
@@ -623,11 +624,11 @@ extern "C" nsgpu_status nsgpu_slice_step(nsgpu_ctx* ctx, const float* u_live, co
   NSGPU_CUDA(cudaMemcpyAsync(S->scal, S->h_scal, sizeof(double), cudaMemcpyHostToDevice, st));
   NSGPU_CUDA(cudaMemsetAsync(S->n_evals, 0, sizeof(unsigned long long), st));
   const uint2 key = make_uint2((unsigned)(seed & 0xffffffffu), (unsigned)(seed >> 32));
-  chain_init_kernel<<<(n_chains + 127) / 128, 128, 0, st>>>(n_chains, D, key, (unsigned)iteration, nullptr, 0, start_idx,
+  chain_init_kernel<<<(n_chains + 127) / 128, 128, 0, st>>>(n_chains, 0, D, key, (unsigned)iteration, nullptr, 0, start_idx,
                                                             S->start_idx, u_live, logL_live, S->x0, S->logL0, S->phase,
                                                             S->cnt, S->step, S->pending, S->finished, S->need, S->rng_j);
   NSGPU_LAUNCH_CHECK();
-  s = evolve(ctx, n_chains, n_steps, seed, iteration, st, nullptr);
+  s = evolve(ctx, n_chains, 0, n_steps, seed, iteration, st, nullptr);
   if (s != NSGPU_OK) return s;
   NSGPU_CUDA(cudaMemcpyAsync(u_out, S->u_out, sizeof(float) * (size_t)n_chains * D, cudaMemcpyDeviceToDevice, st));
   NSGPU_CUDA(cudaMemcpyAsync(logL_out, S->logL_out, sizeof(double) * (size_t)n_chains, cudaMemcpyDeviceToDevice, st));
@@ -696,10 +697,19 @@ extern "C" nsgpu_status nsgpu_last_samples(nsgpu_ctx* ctx, float* theta_samples,
 // log Z with the live points, H, error bar by simulated volumes -- reading N9) is fp64 host arithmetic
 // over the recorded (logL, n_j) sequence.
 // ---------------------------------------------------------------------------------------------------
-extern "C" nsgpu_status nsgpu_run(nsgpu_ctx* ctx, const nsgpu_run_opts* o, nsgpu_result* res, float* theta_samples,
-                                  double* logL_samples, double* logw_samples, int64_t cap, int64_t* n_samples) {
+extern "C" void nsgpu_shard_range(int32_t n_chains, int32_t rank, int32_t world, int32_t* first, int32_t* count) {
+  const int per = world > 0 ? (n_chains + world - 1) / world : n_chains;
+  const int c0 = std::min(n_chains, rank * per);
+  if (first) *first = c0;
+  if (count) *count = std::max(0, std::min(n_chains, c0 + per) - c0);
+}
+
+static nsgpu_status run_impl(nsgpu_ctx* ctx, const nsgpu_run_opts* o, int rank, int world, nsgpu_allgather_fn exch,
+                             void* user, nsgpu_result* res, float* theta_samples, double* logL_samples,
+                             double* logw_samples, int64_t cap, int64_t* n_samples) {
   if (!ctx) return NSGPU_EINVAL;
   if (!o || !res) { ctx->err = "run: NULL options or result"; return NSGPU_EINVAL; }
+  if (world < 1 || rank < 0 || rank >= world || (world > 1 && !exch)) { ctx->err = "run: bad rank / world / exchange function"; return NSGPU_EINVAL; }
   nsgpu_status s = check_sampler_args(ctx, o->n_live, o->n_delete);
   if (s != NSGPU_OK) return s;
   if (o->n_delete >= o->n_live || o->n_steps < 1 || !(o->stop_frac > 0) || o->max_iter < 1) { ctx->err = "run: bad options"; return NSGPU_EINVAL; }
@@ -716,6 +726,20 @@ extern "C" nsgpu_status nsgpu_run(nsgpu_ctx* ctx, const nsgpu_run_opts* o, nsgpu
   float* d_dead_u = S->x0;           // scratch before chains are initialised
   double* d_dead_l = S->logL0;
   memset(res, 0, sizeof(*res));
+  // sharded runs (S 8(e)): rank r evolves the global chains [c0, c0 + n_loc); everything else is done by every
+  // rank on identical data, so that after the exchange all ranks hold the same live set, bit for bit
+  int32_t c0 = 0, n_loc = k;
+  nsgpu_shard_range(k, rank, world, &c0, &n_loc);
+  const int per = (k + world - 1) / world;
+  struct Gather {                      // [world * per] rows: global chain g sits at row g
+    float* u = nullptr; double* l = nullptr; unsigned long long* cnt = nullptr;
+    ~Gather() { cudaFree(u); cudaFree(l); cudaFree(cnt); }
+  } G;
+  if (world > 1) {
+    NSGPU_CUDA(cudaMalloc((void**)&G.u, sizeof(float) * (size_t)world * per * D));
+    NSGPU_CUDA(cudaMalloc((void**)&G.l, sizeof(double) * (size_t)world * per));
+    NSGPU_CUDA(cudaMalloc((void**)&G.cnt, sizeof(unsigned long long) * 4 * (size_t)(world + 1)));
+  }
 
   init_live_kernel<<<(n * D + 255) / 256, 256, 0, st>>>(n, D, key, S->u_live);
   NSGPU_LAUNCH_CHECK();
@@ -746,14 +770,27 @@ extern "C" nsgpu_status nsgpu_run(nsgpu_ctx* ctx, const nsgpu_run_opts* o, nsgpu
     dead_logL.insert(dead_logL.end(), hl.begin(), hl.end());
     dead_logw.insert(dead_logw.end(), hw.begin(), hw.end());
     for (int j = 0; j < k; ++j) dead_nj.push_back(n - j);
-    chain_init_kernel<<<(k + 127) / 128, 128, 0, st>>>(k, D, key, (unsigned)it, S->surv_idx, n - k, nullptr, S->start_idx,
-                                                       S->u_live, S->logL_live, S->x0, S->logL0, S->phase, S->cnt, S->step,
-                                                       S->pending, S->finished, S->need, S->rng_j);
-    NSGPU_LAUNCH_CHECK();
-    s = evolve(ctx, k, o->n_steps, o->seed, (int)it, st, &rounds);
-    if (s != NSGPU_OK) return s;
-    n_fail_total += S->h_counters[2];
-    replace_kernel<<<(k * D + 255) / 256, 256, 0, st>>>(k, D, S->dead_idx, S->u_out, S->logL_out, S->u_live, S->logL_live);
+    if (n_loc > 0) {
+      chain_init_kernel<<<(n_loc + 127) / 128, 128, 0, st>>>(n_loc, c0, D, key, (unsigned)it, S->surv_idx, n - k, nullptr,
+                                                             S->start_idx, S->u_live, S->logL_live, S->x0, S->logL0, S->phase,
+                                                             S->cnt, S->step, S->pending, S->finished, S->need, S->rng_j);
+      NSGPU_LAUNCH_CHECK();
+      s = evolve(ctx, n_loc, c0, o->n_steps, o->seed, (int)it, st, &rounds);
+      if (s != NSGPU_OK) return s;
+      n_fail_total += S->h_counters[2];
+    }
+    const float* new_u = S->u_out;
+    const double* new_l = S->logL_out;
+    if (world > 1) {   // the one exchange of an iteration: all-gather of the new points (k (D + 2) words in all)
+      NSGPU_CUDA(cudaStreamSynchronize(st));
+      if (exch(user, S->u_out, G.u, (int64_t)sizeof(float) * per * D, st) != 0 ||
+          exch(user, S->logL_out, G.l, (int64_t)sizeof(double) * per, st) != 0) {
+        ctx->err = "run: exchange function failed";
+        return NSGPU_ECUDA;
+      }
+      new_u = G.u; new_l = G.l;
+    }
+    replace_kernel<<<(k * D + 255) / 256, 256, 0, st>>>(k, D, S->dead_idx, new_u, new_l, S->u_live, S->logL_live);
     NSGPU_LAUNCH_CHECK();
     live_evidence_kernel<<<1, 1024, 0, st>>>(S->logL_live, n, log(o->stop_frac), S->scal);
     NSGPU_LAUNCH_CHECK();
@@ -768,6 +805,20 @@ extern "C" nsgpu_status nsgpu_run(nsgpu_ctx* ctx, const nsgpu_run_opts* o, nsgpu
   NSGPU_CUDA(cudaMemcpy(live_u.data(), S->u_live, sizeof(float) * (size_t)n * D, cudaMemcpyDeviceToHost));
   NSGPU_CUDA(cudaMemcpy(live_l.data(), S->logL_live, sizeof(double) * (size_t)n, cudaMemcpyDeviceToHost));
   NSGPU_CUDA(cudaMemcpy(S->h_evals, S->n_evals, sizeof(unsigned long long), cudaMemcpyDeviceToHost));
+  unsigned long long evals_all = *S->h_evals;
+  if (world > 1) {   // totals over ranks: evaluations and failed moves add, rounds take the longest rank
+    unsigned long long mine[4] = {*S->h_evals, (unsigned long long)rounds, (unsigned long long)n_fail_total, 0ull};
+    std::vector<unsigned long long> all(4 * (size_t)world);
+    NSGPU_CUDA(cudaMemcpy(G.cnt, mine, sizeof(mine), cudaMemcpyHostToDevice));
+    if (exch(user, G.cnt, G.cnt + 4, (int64_t)sizeof(mine), st) != 0) { ctx->err = "run: exchange function failed"; return NSGPU_ECUDA; }
+    NSGPU_CUDA(cudaMemcpy(all.data(), G.cnt + 4, sizeof(mine) * world, cudaMemcpyDeviceToHost));
+    evals_all = 0; n_fail_total = 0;
+    for (int r = 0; r < world; ++r) {
+      evals_all += all[4 * r];
+      rounds = std::max<int64_t>(rounds, (int64_t)all[4 * r + 1]);
+      n_fail_total += (int)all[4 * r + 2];
+    }
+  }
   const size_t nd = dead_logL.size(), ntot = nd + n;
   std::vector<double> all_l(ntot), all_w(ntot);
   for (size_t i = 0; i < nd; ++i) { all_l[i] = dead_logL[i]; all_w[i] = dead_logw[i]; }
@@ -817,7 +868,7 @@ extern "C" nsgpu_status nsgpu_run(nsgpu_ctx* ctx, const nsgpu_run_opts* o, nsgpu
   for (int j = 0; j < k; ++j) { s1 += 1.0 / (n - j); s2 += 1.0 / ((double)(n - j) * (n - j)); }
   const double cfac = n * s2 / s1;
   res->logZ = logZ; res->logZ_err = err_sim; res->logZ_err_analytic = sqrt(std::max(cfac * H, 0.0) / n); res->H = H;
-  res->n_iter = it; res->n_dead = (int64_t)nd; res->n_like_evals = (int64_t)*S->h_evals + n; res->n_rounds = rounds;
+  res->n_iter = it; res->n_dead = (int64_t)nd; res->n_like_evals = (int64_t)evals_all + n; res->n_rounds = rounds;
   res->n_failed_moves = n_fail_total;
   if (n_samples) *n_samples = (int64_t)ntot;
   {
@@ -844,4 +895,16 @@ extern "C" nsgpu_status nsgpu_run(nsgpu_ctx* ctx, const nsgpu_run_opts* o, nsgpu
   }
   res->seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t_start).count();
   return converged ? NSGPU_OK : NSGPU_ENOCONV;
+}
+
+extern "C" nsgpu_status nsgpu_run(nsgpu_ctx* ctx, const nsgpu_run_opts* o, nsgpu_result* res, float* theta_samples,
+                                  double* logL_samples, double* logw_samples, int64_t cap, int64_t* n_samples) {
+  return run_impl(ctx, o, 0, 1, nullptr, nullptr, res, theta_samples, logL_samples, logw_samples, cap, n_samples);
+}
+
+extern "C" nsgpu_status nsgpu_run_sharded(nsgpu_ctx* ctx, const nsgpu_run_opts* o, int32_t rank, int32_t world,
+                                          nsgpu_allgather_fn allgather, void* user, nsgpu_result* res,
+                                          float* theta_samples, double* logL_samples, double* logw_samples, int64_t cap,
+                                          int64_t* n_samples) {
+  return run_impl(ctx, o, rank, world, allgather, user, res, theta_samples, logL_samples, logw_samples, cap, n_samples);
 }

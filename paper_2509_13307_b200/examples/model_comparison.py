@@ -7,6 +7,10 @@
 `--shape paper-interp` / `paper` run the same comparison on the paper-shape likelihood (10 bins, 55 spectra,
 1025 quadrature nodes; emulator on 103 z nodes + linear interpolation, or on all 1025: PAPER.md L353, L359).
 
+Multi-GPU: launch with `python -m torch.distributed.run --nnodes=1 --nproc-per-node N --master-addr
+127.0.0.1 -m paper_2509_13307_b200.examples.model_comparison ...`; every rank holds the live set, evolves its share of
+the 500 chains per iteration and all-gathers the new points over NCCL (`Context.run_sharded`); rank 0 prints.
+
 Prints one JSON line per run and a summary with log Z +- error per model, the log Bayes factor, total
 likelihood evaluations and wall time.  The mock data vector is produced by the CUDA path itself at the
 fiducial point (the product never calls the oracle).
@@ -14,11 +18,24 @@ fiducial point (the product never calls the oracle).
 import argparse
 import json
 import math
+import os
 
 import numpy as np
 import torch
 
 from paper_2509_13307_b200 import nsgpu, workloads as W
+
+
+def _ranks():
+    """(rank, world, device) from the torchrun environment; a plain `python -m ...` is one rank on cuda:0"""
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if world == 1:
+        return 0, 1, 0
+    import torch.distributed as dist
+    dev = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(dev)
+    dist.init_process_group("nccl")
+    return dist.get_rank(), world, dev
 
 
 def _mock_data(wl_w0wa, device=0):
@@ -42,23 +59,30 @@ def main():
     ap.add_argument("--max-iter", type=int, default=100000)
     ap.add_argument("--shape", default="c4", choices=["c4", "paper-interp", "paper"])
     args = ap.parse_args()
+    rank, world, dev = _ranks()
     if args.shape == "c4":
-        full, rest = _mock_data(W.c3a()), W.c4_lcdm()
+        full, rest = _mock_data(W.c3a(), dev), W.c4_lcdm()
     else:
         interp = args.shape == "paper-interp"
-        full, rest = _mock_data(W.c5(interp, w0wa=True)), W.c5(interp, w0wa=False)
+        full, rest = _mock_data(W.c5(interp, w0wa=True), dev), W.c5(interp, w0wa=False)
     rest.data, rest.chol = full.data, full.chol
     out = {}
     for name, wl in (("w0waCDM", full), ("LCDM", rest)):
         runs = []
-        with nsgpu.Context(wl, max_batch=args.n_live) as ctx:
+        with nsgpu.Context(wl, max_batch=args.n_live, device=dev) as ctx:
             for seed in range(1, args.seeds + 1):
-                r = ctx.run(args.n_live, args.n_delete, 5 * wl.D, stop_frac=args.stop_frac, max_iter=args.max_iter,
-                            seed=seed, return_samples=False)
-                r["model"], r["D"], r["seed"] = name, wl.D, seed
-                print(json.dumps(r), flush=True)
+                kw = dict(stop_frac=args.stop_frac, max_iter=args.max_iter, seed=seed, return_samples=False)
+                if world == 1:
+                    r = ctx.run(args.n_live, args.n_delete, 5 * wl.D, **kw)
+                else:
+                    r = ctx.run_sharded(args.n_live, args.n_delete, 5 * wl.D, rank=rank, world=world, **kw)
+                r["model"], r["D"], r["seed"], r["n_gpus"] = name, wl.D, seed, world
+                if rank == 0:
+                    print(json.dumps(r), flush=True)
                 runs.append(r)
         out[name] = runs
+    if rank != 0:
+        return
     z = {k: np.mean([r["logZ"] for r in v]) for k, v in out.items()}
     e = {k: math.sqrt(np.mean([r["logZ_err"] ** 2 for r in v]) / len(v)) for k, v in out.items()}
     print(json.dumps({"shape": args.shape, "summary": {k: {"logZ": z[k], "err": e[k], "evals": int(np.mean([r["n_like_evals"] for r in v])),

@@ -24,7 +24,8 @@ SHEAR_STREAM = 4          # OR into `mlp`: streaming projection kernels even for
 EXPORTS = ["nsgpu_create", "nsgpu_destroy", "nsgpu_last_error", "nsgpu_prior_transform",
            "nsgpu_loglike_batch", "nsgpu_loglike_batch_host", "nsgpu_emulate_batch", "nsgpu_theory_batch",
            "nsgpu_slice_step", "nsgpu_run", "nsgpu_last_samples", "nsgpu_delete_lowest", "nsgpu_live_cholesky",
-           "nsgpu_debug_philox", "nsgpu_set_profiling", "nsgpu_stage_times", "nsgpu_mlp_path", "nsgpu_launch_count"]
+           "nsgpu_debug_philox", "nsgpu_set_profiling", "nsgpu_stage_times", "nsgpu_mlp_path", "nsgpu_launch_count",
+           "nsgpu_run_sharded", "nsgpu_shard_range"]
 
 
 class NsgpuError(RuntimeError):
@@ -72,6 +73,9 @@ class _Result(C.Structure):
                 ("n_failed_moves", C.c_int64), ("seconds", C.c_double)]
 
 
+# int32 allgather(void* user, const void* send, void* recv, int64 bytes_per_rank, void* stream)  (include/nsgpu.h)
+ALLGATHER_FN = C.CFUNCTYPE(C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p)
+
 _lib = None
 
 
@@ -107,6 +111,11 @@ def lib():
                                    vp, vp, C.POINTER(C.c_int64), vp]
     L.nsgpu_run.restype = C.c_int
     L.nsgpu_run.argtypes = [vp, C.POINTER(_RunOpts), C.POINTER(_Result), vp, vp, vp, C.c_int64, C.POINTER(C.c_int64)]
+    L.nsgpu_run_sharded.restype = C.c_int
+    L.nsgpu_run_sharded.argtypes = [vp, C.POINTER(_RunOpts), C.c_int32, C.c_int32, ALLGATHER_FN, vp, C.POINTER(_Result),
+                                    vp, vp, vp, C.c_int64, C.POINTER(C.c_int64)]
+    L.nsgpu_shard_range.restype = None
+    L.nsgpu_shard_range.argtypes = [C.c_int32, C.c_int32, C.c_int32, C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
     L.nsgpu_last_samples.restype = C.c_int
     L.nsgpu_last_samples.argtypes = [vp, vp, vp, vp, C.c_int64, C.POINTER(C.c_int64)]
     L.nsgpu_delete_lowest.restype = C.c_int
@@ -139,6 +148,52 @@ def _stream_ptr(stream=None):
     import torch
     s = torch.cuda.current_stream() if stream is None else stream
     return C.c_void_p(s.cuda_stream)
+
+
+def shard_range(n_chains, rank, world):
+    """(first, count) of the chains rank `rank` of `world` evolves (nsgpu_shard_range; host only)."""
+    a, b = C.c_int32(0), C.c_int32(0)
+    lib().nsgpu_shard_range(int(n_chains), int(rank), int(world), C.byref(a), C.byref(b))
+    return a.value, b.value
+
+
+class _RawBuffer:
+    """a device (or host) pointer as a flat uint8 array for torch (zero copy)"""
+
+    def __init__(self, ptr, nbytes, cuda):
+        iface = {"shape": (int(nbytes),), "typestr": "|u1", "data": (int(ptr), False), "version": 2 if cuda else 3, "strides": None}
+        if cuda:
+            self.__cuda_array_interface__ = iface
+        else:
+            self.__array_interface__ = iface
+
+
+def torch_allgather(device=None, group=None):
+    """The exchange step of nsgpu_run_sharded on torch.distributed: `all_gather_into_tensor` straight on the
+    library's buffers (NCCL for device pointers; `device=None` treats them as host pointers, for gloo tests).
+    Returns a Python callable with the nsgpu_allgather_fn signature."""
+    import torch
+    import torch.distributed as dist
+
+    def cb(user, send, recv, nbytes, stream):
+        try:
+            world = dist.get_world_size(group)
+            if device is None:
+                s = torch.from_numpy(np.asarray(_RawBuffer(send, nbytes, False)))
+                r = torch.from_numpy(np.asarray(_RawBuffer(recv, nbytes * world, False)))
+            else:
+                s = torch.as_tensor(_RawBuffer(send, nbytes, True), device=f"cuda:{device}")
+                r = torch.as_tensor(_RawBuffer(recv, nbytes * world, True), device=f"cuda:{device}")
+            dist.all_gather_into_tensor(r, s, group=group)
+            if device is not None:
+                torch.cuda.synchronize(device)
+            return 0
+        except Exception as e:          # never let an exception cross the C boundary
+            import sys
+            print(f"nsgpu allgather failed: {e!r}", file=sys.stderr)
+            return 1
+
+    return cb
 
 
 class Context:
@@ -330,6 +385,31 @@ class Context:
         ns = C.c_int64(0)
         st = self._check(lib().nsgpu_run(self._h, C.byref(o), C.byref(r), None, None, None, 0, C.byref(ns)),
                          allow=(ENOCONV,))
+        out = {f: getattr(r, f) for f, _ in _Result._fields_}
+        out["converged"] = st == OK
+        if return_samples:
+            n = ns.value
+            th = np.empty((n, self.D), np.float32); ll = np.empty(n, np.float64); lw = np.empty(n, np.float64)
+            self._check(lib().nsgpu_last_samples(self._h, th.ctypes.data_as(C.c_void_p), ll.ctypes.data_as(C.c_void_p),
+                                                 lw.ctypes.data_as(C.c_void_p), n, C.byref(ns)))
+            out.update(theta=th, logL=ll, logw=lw, n_samples=n)
+        return out
+
+    def run_sharded(self, n_live, n_delete, n_steps, stop_frac=1e-3, max_iter=100000, seed=1, rank=None, world=None,
+                    allgather=None, return_samples=True):
+        """nsgpu_run_sharded: the same run with the k chains of an iteration split over `world` processes (one GPU
+        each, every rank calls this with the same arguments).  `allgather` defaults to torch.distributed
+        (`torch_allgather`, NCCL on device buffers); every rank gets the same result as `run`."""
+        import torch.distributed as dist
+        if rank is None:
+            rank, world = dist.get_rank(), dist.get_world_size()
+        cb = allgather if allgather is not None else torch_allgather(self.device)
+        fn = ALLGATHER_FN(cb)
+        o = _RunOpts(int(n_live), int(n_delete), int(n_steps), float(stop_frac), int(max_iter), int(seed))
+        r = _Result()
+        ns = C.c_int64(0)
+        st = self._check(lib().nsgpu_run_sharded(self._h, C.byref(o), int(rank), int(world), fn, None, C.byref(r),
+                                                 None, None, None, 0, C.byref(ns)), allow=(ENOCONV,))
         out = {f: getattr(r, f) for f, _ in _Result._fields_}
         out["converged"] = st == OK
         if return_samples:
