@@ -336,7 +336,8 @@ nsgpu_status create_impl(nsgpu_ctx* ctx, int32_t D, const nsgpu_prior1d* prior, 
     const size_t act_bytes = ((M_max + 127) / 128 * 128) * (size_t)width_max * sizeof(float);
     NSGPU_CUDA(cudaMalloc(&ctx->act[0], act_bytes));
     NSGPU_CUDA(cudaMalloc(&ctx->act[1], act_bytes));
-    NSGPU_CUDA(cudaMalloc((void**)&ctx->spec, (size_t)n_emu * M_max * emu[0].n_out * sizeof(float)));
+    ctx->spec_ld = th->kind == 3 ? emu[0].n_out : (emu[0].n_out + 3) & ~3;
+    NSGPU_CUDA(cudaMalloc((void**)&ctx->spec, (size_t)n_emu * M_max * ctx->spec_ld * sizeof(float)));
   }
   NSGPU_CUDA(cudaMalloc((void**)&ctx->model, (size_t)max_batch * n_data * sizeof(double)));
   if (th->kind != 4) {   // chi^2 workspaces: transposed residuals [n_data][batch rounded up to 64], partial sums per row block
@@ -456,12 +457,12 @@ extern "C" nsgpu_status nsgpu_stage_times(nsgpu_ctx* ctx, double* ms, int64_t* c
 extern "C" int64_t nsgpu_launch_count(const nsgpu_ctx* ctx) { return ctx ? ctx->launches : -1; }
 
 static nsgpu_status run_emulators(nsgpu_ctx* ctx, const float* theta, int B, const int* n_rows_dev, cudaStream_t st) {
-  const size_t stride = (size_t)ctx->max_batch * ctx->rows_per_theta * (ctx->n_emu ? ctx->emu[0].n_out : 0);
+  const size_t stride = (size_t)ctx->max_batch * ctx->rows_per_theta * ctx->spec_ld;
   for (int e = 0; e < ctx->n_emu; ++e) {
     float* out = ctx->spec + e * stride;
     const int mode = (ctx->spec_kz ? NSGPU_SPEC_KZ : 0) | (ctx->kind == 4 ? NSGPU_SPEC_NOMEAN : 0);
-    nsgpu_status s = ctx->emu[e].path == 1 ? mlp_forward_tc(ctx, e, theta, B, n_rows_dev, out, mode, st)
-                                           : mlp_forward_simt(ctx, e, theta, B, n_rows_dev, out, mode & NSGPU_SPEC_NOMEAN, st);
+    nsgpu_status s = ctx->emu[e].path == 1 ? mlp_forward_tc(ctx, e, theta, B, n_rows_dev, out, ctx->spec_ld, mode, st)
+                                           : mlp_forward_simt(ctx, e, theta, B, n_rows_dev, out, ctx->spec_ld, mode & NSGPU_SPEC_NOMEAN, st);
     if (s != NSGPU_OK) return s;
   }
   return NSGPU_OK;
@@ -527,8 +528,8 @@ extern "C" nsgpu_status nsgpu_emulate_batch(nsgpu_ctx* ctx, int32_t e, const flo
   if (e < 0 || e >= ctx->n_emu) { ctx->err = "emulate: emulator index out of range"; return NSGPU_EINVAL; }
   const bool ex = ctx->emu[e].out_kind == 1;
   const int mode = ex ? NSGPU_SPEC_EXP10 : 0;
-  return ctx->emu[e].path == 1 ? mlp_forward_tc(ctx, e, theta, B, nullptr, out, mode, (cudaStream_t)stream)
-                               : mlp_forward_simt(ctx, e, theta, B, nullptr, out, mode, (cudaStream_t)stream);
+  return ctx->emu[e].path == 1 ? mlp_forward_tc(ctx, e, theta, B, nullptr, out, ctx->emu[e].n_out, mode, (cudaStream_t)stream)
+                               : mlp_forward_simt(ctx, e, theta, B, nullptr, out, ctx->emu[e].n_out, mode, (cudaStream_t)stream);
 }
 
 extern "C" nsgpu_status nsgpu_theory_batch(nsgpu_ctx* ctx, const float* theta, int32_t B, double* model, void* stream) {

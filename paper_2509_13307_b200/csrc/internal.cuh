@@ -78,7 +78,8 @@ struct nsgpu_ctx {
   double *tt_a = nullptr, *tt_b = nullptr, *tt_mu = nullptr;   // kind 4: (nu/2) ln 10 and nu Chat / 2 per multipole
   // workspaces
   void* act[2] = {nullptr, nullptr};   // [M_max][width] fp32 (SIMT) or 2 x fp16 (tcgen05)
-  float* spec = nullptr;               // [n_emu][M_max][n_out] de-standardised y (log10 where exp10)
+  float* spec = nullptr;               // [n_emu][M_max][spec_ld] de-standardised y (log10 where exp10)
+  int spec_ld = 0;                     // row stride: n_out, rounded up to 4 floats for one-row-per-theta tables (16-byte stores)
   bool spec_kz = false;                // shear + tcgen05: per theta [n_k][n_z_emu] instead of [n_z_emu][n_k]
   double* model = nullptr;             // [max_batch][n_data]
   double* resid_t = nullptr;           // [n_data][max_batch rounded up to 64] model - data, transposed (chi^2 operand)
@@ -143,9 +144,9 @@ struct StageTimer {
 #define NSGPU_SPEC_NOMEAN 4  // write y - mu_out (the consumer adds mu_out in fp64)
 #define NSGPU_SPEC_KZ 2      // shear only: table layout [theta][k][z] (z fastest) instead of [theta][z][k]
 nsgpu_status mlp_forward_simt(nsgpu_ctx* ctx, int e, const float* theta, int B, const int* n_rows_dev,
-                              float* spec_out, int mode, cudaStream_t st);
+                              float* spec_out, int ld_spec, int mode, cudaStream_t st);
 nsgpu_status mlp_forward_tc(nsgpu_ctx* ctx, int e, const float* theta, int B, const int* n_rows_dev,
-                            float* spec_out, int mode, cudaStream_t st);
+                            float* spec_out, int ld_spec, int mode, cudaStream_t st);
 nsgpu_status mlp_tc_prepare(nsgpu_ctx* ctx, int e, const nsgpu_emulator* h);
 void mlp_tc_release(nsgpu_ctx* ctx, int e);
 nsgpu_status shear_project(nsgpu_ctx* ctx, const float* theta, int B, const int* n_rows_dev, cudaStream_t st);

@@ -55,7 +55,7 @@ __global__ void __launch_bounds__(256) gemm_simt(const float* __restrict__ A, co
                                                  const float* __restrict__ bias, const float* __restrict__ p0,
                                                  const float* __restrict__ p1, int M, int N, int K,
                                                  const int* __restrict__ n_rows_dev, int rows_per_theta,
-                                                 int apply_exp10, float* __restrict__ C) {
+                                                 int apply_exp10, float* __restrict__ C, int ldc) {
   if (n_rows_dev) M = min(M, (*n_rows_dev) * rows_per_theta);
   const int m0 = blockIdx.x * 64, n0 = blockIdx.y * 64;
   if (m0 >= M) return;
@@ -103,7 +103,7 @@ __global__ void __launch_bounds__(256) gemm_simt(const float* __restrict__ A, co
         v = fmaf(t, p0[gn], p1[gn]);           // p0 = sigma_out, p1 = mu_out
         if (apply_exp10) v = exp10f(v);
       }
-      C[(size_t)gm * N + gn] = v;
+      C[(size_t)gm * ldc + gn] = v;
     }
   }
 }
@@ -111,7 +111,7 @@ __global__ void __launch_bounds__(256) gemm_simt(const float* __restrict__ A, co
 }  // namespace
 
 nsgpu_status mlp_forward_simt(nsgpu_ctx* ctx, int e, const float* theta, int B, const int* n_rows_dev,
-                              float* spec_out, int mode, cudaStream_t st) {
+                              float* spec_out, int ld_spec, int mode, cudaStream_t st) {
   const bool apply_exp10 = (mode & NSGPU_SPEC_EXP10) != 0;
   const EmuDev& E = ctx->emu[e];
   const int rpt = ctx->rows_per_theta;
@@ -132,7 +132,7 @@ nsgpu_status mlp_forward_simt(nsgpu_ctx* ctx, int e, const float* theta, int B, 
     StageTimer tm(ctx, 1, st);
     dim3 grid((M + 63) / 64, (E.width + 63) / 64);
     gemm_simt<0><<<grid, 256, 0, st>>>(cur, E.W[l], E.b[l], E.alpha[l], E.beta[l], M, E.width, E.width,
-                                       n_rows_dev, rpt, 0, nxt);
+                                       n_rows_dev, rpt, 0, nxt, E.width);
     NSGPU_LAUNCH_CHECK();
     float* t = cur; cur = nxt; nxt = t;
   }
@@ -141,7 +141,7 @@ nsgpu_status mlp_forward_simt(nsgpu_ctx* ctx, int e, const float* theta, int B, 
     dim3 grid((M + 63) / 64, (E.n_out + 63) / 64);
     gemm_simt<1><<<grid, 256, 0, st>>>(cur, E.W[E.n_hidden], E.b[E.n_hidden], E.out_std,
                                        (mode & NSGPU_SPEC_NOMEAN) ? E.out_zero : E.out_mean, M,
-                                       E.n_out, E.width, n_rows_dev, rpt, apply_exp10 ? 1 : 0, spec_out);
+                                       E.n_out, E.width, n_rows_dev, rpt, apply_exp10 ? 1 : 0, spec_out, ld_spec);
     NSGPU_LAUNCH_CHECK();
   }
   return NSGPU_OK;

@@ -646,7 +646,7 @@ void mlp_tc_release(nsgpu_ctx* ctx, int e) {
 }
 
 nsgpu_status mlp_forward_tc(nsgpu_ctx* ctx, int e, const float* theta, int B, const int* n_rows_dev, float* spec_out,
-                            int mode, cudaStream_t st) {
+                            int ld_spec, int mode, cudaStream_t st) {
   const EmuDev& E = ctx->emu[e];
   TcState* T = reinterpret_cast<TcState*>(E.tmaps);
   const int rpt = ctx->rows_per_theta;
@@ -676,7 +676,7 @@ nsgpu_status mlp_forward_tc(nsgpu_ctx* ctx, int e, const float* theta, int B, co
     g.p_hidden = L.p_hidden; g.p_out = (mode & NSGPU_SPEC_NOMEAN) ? L.p_out_nm : L.p_out; g.p_out4 = (mode & NSGPU_SPEC_NOMEAN) ? L.p_out4_nm : L.p_out4; g.cscale = ldexpf(1.0f, -(L.wexp + 4)) * TRUNC_COMP;
     g.a_hi = T->act[cur][0]; g.a_lo = T->act[cur][1];
     g.out_hi = T->act[cur ^ 1][0]; g.out_lo = T->act[cur ^ 1][1]; g.ld_out = E.width;
-    g.out_f32 = spec_out; g.ld_f32 = E.n_out; g.apply_exp10 = (mode & NSGPU_SPEC_EXP10) ? 1 : 0;
+    g.out_f32 = spec_out; g.ld_f32 = ld_spec; g.apply_exp10 = (mode & NSGPU_SPEC_EXP10) ? 1 : 0;
     g.out_mode = (mode & NSGPU_SPEC_KZ) ? 1 : 0;
     StageTimer tm(ctx, hidden ? 1 : 2, st);
     nsgpu_status s = hidden ? dispatch_gemm<0>(ctx, L, g, st) : dispatch_gemm<1>(ctx, L, g, st);

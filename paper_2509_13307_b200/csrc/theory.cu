@@ -653,43 +653,57 @@ __global__ void __launch_bounds__(LIMBER_THREADS, 2) shear_limber_kernel(const f
     }
 }
 
-// a9: one CTA per theta.  Stage the n_emu spectra in shared memory (coalesced, 10^y applied once per
-// multipole, / A_cal^2), then one thread per bin walks its CSR row.
-__global__ void __launch_bounds__(256) cmb_bin_kernel(const float* __restrict__ theta, int D,
+// a9: model[b][r] = sum_e Bin[r][e] s_b[col_e] / A_cal^2, s = 10^y (or y) of the three emulated spectra.  One thread
+// per (bin r, block of CB_T thetas): a CSR entry is read once and serves CB_T thetas; for a fixed theta the lanes
+// of a warp (adjacent bins) read adjacent runs of the spectrum row and write adjacent model entries.  No shared
+// memory: 2048 threads per SM cover the load latency.  fp64 from the table value onward.
+constexpr int CB_T = 8;
+__global__ void __launch_bounds__(128) cmb_bin_kernel(const float* __restrict__ theta, int D, int B,
                                                       const int* __restrict__ n_rows_dev,
-                                                      const float* __restrict__ spec, int n_emu, int n_out,
+                                                      const float* __restrict__ spec, int n_emu, int n_out, int ld,
                                                       size_t emu_stride, unsigned exp10_mask, int cal_index,
                                                       const int* __restrict__ bin_ptr,
                                                       const int* __restrict__ bin_col,
                                                       const float* __restrict__ bin_val, int n_data,
                                                       double* __restrict__ model) {
-  const int b = blockIdx.x;
-  if (n_rows_dev && b >= *n_rows_dev) return;
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-  double* s = reinterpret_cast<double*>(smem_raw);   // [n_emu * n_out]
-  const double acal = theta[(size_t)b * D + cal_index];
-  const double inv = 1.0 / (acal * acal);
-  for (int e = 0; e < n_emu; ++e) {
-    const float* src = spec + e * emu_stride + (size_t)b * n_out;
-    const bool ex = (exp10_mask >> e) & 1u;
-    for (int i = threadIdx.x; i < n_out; i += blockDim.x) {
-      const double y = (double)__ldg(src + i);
-      s[e * n_out + i] = (ex ? exp10(y) : y) * inv;
+  if (n_rows_dev) B = min(B, *n_rows_dev);
+  const int b0 = blockIdx.y * CB_T;
+  if (b0 >= B) return;
+  const int r = blockIdx.x * blockDim.x + threadIdx.x;
+  if (r >= n_data) return;
+  const int nb = min(CB_T, B - b0);
+  double acc[CB_T];
+#pragma unroll
+  for (int t = 0; t < CB_T; ++t) acc[t] = 0.0;
+  const int e1 = bin_ptr[r + 1];
+  for (int e = bin_ptr[r]; e < e1; ++e) {
+    const int col = bin_col[e];
+    const double v = (double)bin_val[e];
+    const int em = col / n_out;                          // which emulator's spectrum
+    const float* src = spec + em * emu_stride + (size_t)b0 * ld + (col - em * n_out);
+    const bool ex = (exp10_mask >> em) & 1u;
+    float y[CB_T];
+#pragma unroll
+    for (int t = 0; t < CB_T; ++t) y[t] = __ldg(src + (size_t)min(t, nb - 1) * ld);
+#pragma unroll
+    for (int t = 0; t < CB_T; ++t) {
+      const double sv = ex ? exp_fast((double)y[t] * 2.302585092994046) : (double)y[t];
+      acc[t] = fma(v, sv, acc[t]);
     }
   }
-  __syncthreads();
-  for (int r = threadIdx.x; r < n_data; r += blockDim.x) {
-    double acc = 0.0;
-    for (int e = bin_ptr[r]; e < bin_ptr[r + 1]; ++e) acc += (double)bin_val[e] * s[bin_col[e]];
-    model[(size_t)b * n_data + r] = acc;
-  }
+#pragma unroll
+  for (int t = 0; t < CB_T; ++t)
+    if (t < nb) {
+      const double acal = theta[(size_t)(b0 + t) * D + cal_index];
+      model[(size_t)(b0 + t) * n_data + r] = acc[t] / (acal * acal);
+    }
 }
 
 // kind 4: log L = const - sum_l [ a_l y_l + b_l 10^(-y_l) ], y = emulated log10 C_l.  One CTA per theta,
 // fp64 terms and reduction; reads 4 n_out bytes per theta (HBM-bound), writes log L directly.
 __global__ void __launch_bounds__(128) cmb_tt_kernel(const float* __restrict__ theta, int D, int B,
                                                      const int* __restrict__ n_rows_dev, const float* __restrict__ spec,
-                                                     int n, const double* __restrict__ ta, const double* __restrict__ tb,
+                                                     int n, int ld, const double* __restrict__ ta, const double* __restrict__ tb,
                                                      const double* __restrict__ mu, double cst, const int* __restrict__ prior_kind,
                                                      const double* __restrict__ p0, const double* __restrict__ p1,
                                                      double* __restrict__ logL) {
@@ -697,7 +711,7 @@ __global__ void __launch_bounds__(128) cmb_tt_kernel(const float* __restrict__ t
   if (n_rows_dev) B = min(B, *n_rows_dev);
   if (b >= B) return;
   __shared__ double red[4];
-  const float* y = spec + (size_t)b * n;
+  const float* y = spec + (size_t)b * ld;
   double acc = 0.0;
   for (int i = threadIdx.x; i < n; i += blockDim.x) {
     const double yi = (double)__ldg(y + i) + mu[i];            // the table holds y - mu_out (fp32), mu_out added in fp64
@@ -719,12 +733,13 @@ __global__ void __launch_bounds__(128) cmb_tt_kernel(const float* __restrict__ t
 }
 
 // kind 0: model = theta; kind 1: model = spectrum of emulator 0 (10^y where out_kind = 1)
-__global__ void copy_model_kernel(const float* __restrict__ src, int n, int B, const int* __restrict__ n_rows_dev,
+__global__ void copy_model_kernel(const float* __restrict__ src, int n, int ld, int B, const int* __restrict__ n_rows_dev,
                                   int apply_exp10, const double* __restrict__ mu, double* __restrict__ model) {
   if (n_rows_dev) B = min(B, *n_rows_dev);
   const size_t total = (size_t)B * n;
   for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
-    const double y = (double)src[i] + (mu ? mu[i % n] : 0.0);
+    const size_t b = i / n, j = i - b * n;
+    const double y = (double)src[b * ld + j] + (mu ? mu[j] : 0.0);
     model[i] = apply_exp10 ? exp10(y) : y;
   }
 }
@@ -816,16 +831,11 @@ nsgpu_status cmb_bin(nsgpu_ctx* ctx, const float* theta, int B, const int* n_row
   const int n_out = ctx->emu[0].n_out;
   unsigned mask = 0;
   for (int e = 0; e < ctx->n_emu; ++e) mask |= (ctx->emu[e].out_kind == 1 ? 1u : 0u) << e;
-  const size_t smem = (size_t)ctx->n_emu * n_out * sizeof(double);
-  static size_t configured = 0;
-  if (smem > configured) {
-    NSGPU_CUDA(cudaFuncSetAttribute(cmb_bin_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    configured = smem;
-  }
-  const size_t emu_stride = (size_t)ctx->max_batch * ctx->rows_per_theta * n_out;
+  const size_t emu_stride = (size_t)ctx->max_batch * ctx->rows_per_theta * ctx->spec_ld;
   StageTimer tm(ctx, 4, st);
-  cmb_bin_kernel<<<B, 256, smem, st>>>(theta, ctx->D, n_rows_dev, ctx->spec, ctx->n_emu, n_out, emu_stride, mask,
-                                       ctx->cal_index, ctx->bin_ptr, ctx->bin_col, ctx->bin_val, ctx->n_data,
+  dim3 grid((ctx->n_data + 127) / 128, (B + CB_T - 1) / CB_T);
+  cmb_bin_kernel<<<grid, 128, 0, st>>>(theta, ctx->D, B, n_rows_dev, ctx->spec, ctx->n_emu, n_out, ctx->spec_ld, emu_stride,
+                                       mask, ctx->cal_index, ctx->bin_ptr, ctx->bin_col, ctx->bin_val, ctx->n_data,
                                        ctx->model);
   NSGPU_LAUNCH_CHECK();
   return NSGPU_OK;
@@ -834,7 +844,7 @@ nsgpu_status cmb_bin(nsgpu_ctx* ctx, const float* theta, int B, const int* n_row
 nsgpu_status cmb_tt_loglike(nsgpu_ctx* ctx, const float* theta, int B, const int* n_rows_dev, double* logL, cudaStream_t st) {
   if (B == 0) return NSGPU_OK;
   StageTimer tm(ctx, 4, st);
-  cmb_tt_kernel<<<B, 128, 0, st>>>(theta, ctx->D, B, n_rows_dev, ctx->spec, ctx->n_data, ctx->tt_a, ctx->tt_b, ctx->tt_mu, ctx->log_norm,
+  cmb_tt_kernel<<<B, 128, 0, st>>>(theta, ctx->D, B, n_rows_dev, ctx->spec, ctx->n_data, ctx->spec_ld, ctx->tt_a, ctx->tt_b, ctx->tt_mu, ctx->log_norm,
                                    ctx->prior_kind, ctx->prior_p0, ctx->prior_p1, logL);
   NSGPU_LAUNCH_CHECK();
   return NSGPU_OK;
@@ -848,7 +858,7 @@ nsgpu_status copy_model(nsgpu_ctx* ctx, const float* theta, int B, const int* n_
   const int ex = (!ident && ctx->emu[0].out_kind == 1) ? 1 : 0;
   int blocks = (int)std::min<size_t>(((size_t)B * n + 255) / 256, 148 * 8);
   StageTimer tm(ctx, 7, st);
-  copy_model_kernel<<<blocks, 256, 0, st>>>(src, n, B, n_rows_dev, ex, ctx->kind == 4 ? ctx->tt_mu : nullptr, ctx->model);
+  copy_model_kernel<<<blocks, 256, 0, st>>>(src, n, ident ? n : ctx->spec_ld, B, n_rows_dev, ex, ctx->kind == 4 ? ctx->tt_mu : nullptr, ctx->model);
   NSGPU_LAUNCH_CHECK();
   return NSGPU_OK;
 }
