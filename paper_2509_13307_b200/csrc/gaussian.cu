@@ -146,7 +146,7 @@ __global__ void __launch_bounds__(MAXT) chi2_kernel(const double* __restrict__ m
 // 8 thetas), which is what bounds it for n ~ 1000.  Here a CTA owns a 128-row block of Linv and TG*8 thetas:
 // the factor crosses L2 -> shared memory once per 64 thetas.  Operands: LinvT (column j contiguous over rows)
 // and the residuals transposed to [n][batch] so that both tiles of a k-step are contiguous pieces moved by
-// bulk asynchronous copies through a 4-stage ring.  A warp owns 8 (TG) thetas and all 128 rows: the residuals
+// bulk asynchronous copies through a ring of stages.  A warp owns 8 (TG) thetas and all 128 rows: the residuals
 // of a column are one broadcast line, the factor column is conflict-free; 4 x TG fp64 accumulators per lane.
 // Partial sums of w^2 per (row block, theta) are joined in a fixed order by chi2_finalize_kernel.
 constexpr int CT_ROWS = 128, CT_KC = 8, CT_NBUF = 4, CT_WARPS = 8;
@@ -192,20 +192,25 @@ __global__ void __launch_bounds__(CT_WARPS * 32, 2) chi2_tile_kernel(const doubl
   const int K = min(i0 + CT_ROWS, n);                     // columns 0 .. K-1 reach this row block
   const int n_steps = (K + CT_KC - 1) / CT_KC;
   const uint32_t full0 = tc::smem_u32(bars), empty0 = full0 + 8 * CT_NBUF;
-  auto load_step = [&](int s, int buf) {
+  // one k-step = 2 CT_KC small copies: issued by the lanes of warp 0 in parallel (a single thread issuing them one
+  // after the other put ~1000 clk per step on the critical path of its warp)
+  auto load_step = [&](int s, int buf) {                 // whole warp 0
     const int j0 = s * CT_KC, jn = min(CT_KC, K - j0);
-    tc::mbar_arrive_expect_tx(full0 + 8 * buf, (uint32_t)jn * (uint32_t)(rows * 8 + TBLK * 8));
-    for (int jj = 0; jj < jn; ++jj) {
-      tc::bulk_load(tc::smem_u32(&Ls[buf][jj][0]), LinvT + (size_t)(j0 + jj) * ns + i0, (uint32_t)rows * 8u, full0 + 8 * buf);
-      tc::bulk_load(tc::smem_u32(&Rs[buf][jj][0]), rt + (size_t)(j0 + jj) * ldr + b0, TBLK * 8u, full0 + 8 * buf);
-    }
+    if (lane == 0) tc::mbar_arrive_expect_tx(full0 + 8 * buf, (uint32_t)jn * (uint32_t)(rows * 8 + TBLK * 8));
+    __syncwarp();
+    if (lane < jn)
+      tc::bulk_load(tc::smem_u32(&Ls[buf][lane][0]), LinvT + (size_t)(j0 + lane) * ns + i0, (uint32_t)rows * 8u, full0 + 8 * buf);
+    else if (lane >= 16 && lane - 16 < jn)
+      tc::bulk_load(tc::smem_u32(&Rs[buf][lane - 16][0]), rt + (size_t)(j0 + lane - 16) * ldr + b0, TBLK * 8u, full0 + 8 * buf);
   };
+  static_assert(CT_KC <= 16, "one lane per copy");
   if (tid == 0) {
     for (int b = 0; b < CT_NBUF; ++b) { tc::mbar_init(full0 + 8 * b, 1); tc::mbar_init(empty0 + 8 * b, CT_WARPS); }
     tc::fence_barrier_init();
-    for (int s = 0; s < CT_NBUF - 1 && s < n_steps; ++s) load_step(s, s);
   }
   __syncthreads();
+  if (warp == 0)
+    for (int s = 0; s < CT_NBUF - 1 && s < n_steps; ++s) load_step(s, s);
   double acc[4][TG];
 #pragma unroll
   for (int r = 0; r < 4; ++r)
@@ -213,15 +218,15 @@ __global__ void __launch_bounds__(CT_WARPS * 32, 2) chi2_tile_kernel(const doubl
     for (int t = 0; t < TG; ++t) acc[r][t] = 0.0;
   for (int s = 0; s < n_steps; ++s) {
     const int buf = s % CT_NBUF;
-    if (tid == 0 && s + CT_NBUF - 1 < n_steps) {
+    if (warp == 0 && s + CT_NBUF - 1 < n_steps) {
       const int sn = s + CT_NBUF - 1, nb = sn % CT_NBUF;
-      if (s >= 1) tc::mbar_wait(empty0 + 8 * nb, ((s - 1) / CT_NBUF) & 1);
+      if (s >= 1 && lane == 0) tc::mbar_wait(empty0 + 8 * nb, ((s - 1) / CT_NBUF) & 1);
+      __syncwarp();
       load_step(sn, nb);
     }
     tc::mbar_wait(full0 + 8 * buf, (s / CT_NBUF) & 1);
     const int jn = min(CT_KC, K - s * CT_KC);
-#pragma unroll 4
-    for (int jj = 0; jj < jn; ++jj) {
+    auto column = [&](int jj) {
       double l[4], v[TG];
 #pragma unroll
       for (int r = 0; r < 4; ++r) l[r] = Ls[buf][jj][lane + 32 * r];
@@ -231,6 +236,12 @@ __global__ void __launch_bounds__(CT_WARPS * 32, 2) chi2_tile_kernel(const doubl
       for (int r = 0; r < 4; ++r)
 #pragma unroll
         for (int t = 0; t < TG; ++t) acc[r][t] = fma(l[r], v[t], acc[r][t]);
+    };
+    if (jn == CT_KC) {                                   // every step but the last: fully unrolled
+#pragma unroll
+      for (int jj = 0; jj < CT_KC; ++jj) column(jj);
+    } else {
+      for (int jj = 0; jj < jn; ++jj) column(jj);
     }
     __syncwarp();
     if (lane == 0) tc::mbar_arrive(empty0 + 8 * buf);
