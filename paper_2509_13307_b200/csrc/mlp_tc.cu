@@ -130,11 +130,9 @@ __global__ void __launch_bounds__(256) mlp_first_layer_tc(const float* __restric
                                                           const float* __restrict__ z_emu, int n_in,
                                                           const float* __restrict__ in_mean,
                                                           const float* __restrict__ in_std, const float* __restrict__ W,
-                                                          const float4* __restrict__ params, int width,
+                                                          const float4* __restrict__ params, int width, int split,
                                                           __half* __restrict__ out_hi, __half* __restrict__ out_lo) {
   if (n_rows_dev) M = min(M, (*n_rows_dev) * rows_per_theta);
-  const int m0 = blockIdx.x * BLOCK_M;
-  if (m0 >= M) return;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   float4* sp = reinterpret_cast<float4*>(smem_raw);          // [width]
   float* sW = reinterpret_cast<float*>(sp + width);          // [n_in][width]
@@ -144,15 +142,25 @@ __global__ void __launch_bounds__(256) mlp_first_layer_tc(const float* __restric
     sp[2 * i + 1] = make_float4(c0.z, c1.z, c0.w, c1.w);
   }
   for (int i = threadIdx.x; i < n_in * width; i += blockDim.x) sW[i] = W[i];
+  __syncthreads();
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int r = (warp & 3) * 32 + lane;                      // row within the tile
-  const int m = min(m0 + r, M - 1);
-  const int th = m / rows_per_theta, zi = m - th * rows_per_theta;
-  float x[NIN];                                             // NIN = n_in at compile time: no predicated-off work
+  const int n_pieces = width >> 3;
+  const int ppi = (n_pieces + split - 1) / split;      // pieces per work item
+  const int half = (ppi + 1) >> 1;                           // ... per warp group
+  const int n_items = ((M + BLOCK_M - 1) / BLOCK_M) * split;
+  const f32x2 one2 = pk2(1.0f, 1.0f);
+  // a work item is (128-row tile, 1/split of its pieces); the host launches one CTA per item.  split = 1 for large
+  // batches (measured: finer items only add input gathers there), 4 when whole tiles would leave SMs idle.
+  for (int item = blockIdx.x; item < n_items; item += gridDim.x) {
+    const int tile = item / split, part = item - tile * split;
+    const int m0 = tile * BLOCK_M;
+    const int m = min(m0 + r, M - 1);
+    const int th = m / rows_per_theta, zi = m - th * rows_per_theta;
+    f32x2 x2[NIN];                                          // NIN = n_in at compile time: no predicated-off work
 #pragma unroll
-  for (int c = 0; c < NIN; ++c) {
-    float v = 0.0f;
-    {
+    for (int c = 0; c < NIN; ++c) {
+      float v;
       if (c < n_theta_in) {
         const int src = emu_in_idx[c];
         v = src >= 0 ? theta[(size_t)th * D + src] : (float)emu_in_const[c];
@@ -160,33 +168,28 @@ __global__ void __launch_bounds__(256) mlp_first_layer_tc(const float* __restric
         v = z_emu[zi];
       }
       v = (v - in_mean[c]) / in_std[c];
+      x2[c] = pk2(v, v);
     }
-    x[c] = v;
-  }
-  __syncthreads();
-  const int n_pieces = width >> 3, half_pieces = (n_pieces + 1) >> 1;
-  const int p_begin = (warp >> 2) * half_pieces, p_end = min(p_begin + half_pieces, n_pieces);
-  const size_t tile_base = (size_t)blockIdx.x * ((size_t)BLOCK_M * width) + (size_t)r * 8;
-  f32x2 x2[NIN];
+    const int p_begin = part * ppi + (warp >> 2) * half;
+    const int p_end = min(min(p_begin + half, (part + 1) * ppi), n_pieces);
+    const size_t tile_base = (size_t)tile * ((size_t)BLOCK_M * width) + (size_t)r * 8;
+    for (int p = p_begin; p < p_end; ++p) {
+      uint32_t hi[4], lo[4];
+      f32x2 t[4] = {0ull, 0ull, 0ull, 0ull};                    // 8 neurons of this piece, bias added in the epilogue
 #pragma unroll
-  for (int c = 0; c < NIN; ++c) x2[c] = pk2(x[c], x[c]);
-  const f32x2 one2 = pk2(1.0f, 1.0f);
-  for (int p = p_begin; p < p_end; ++p) {
-    uint32_t hi[4], lo[4];
-    f32x2 t[4] = {0ull, 0ull, 0ull, 0ull};                      // 8 neurons of this piece, bias added in the epilogue
-#pragma unroll
-    for (int c = 0; c < NIN; ++c) {
+      for (int c = 0; c < NIN; ++c) {
         const float4 wlo = *reinterpret_cast<const float4*>(sW + c * width + 8 * p);
         const float4 whi = *reinterpret_cast<const float4*>(sW + c * width + 8 * p + 4);
         t[0] = fma2(x2[c], pk2(wlo.x, wlo.y), t[0]); t[1] = fma2(x2[c], pk2(wlo.z, wlo.w), t[1]);
         t[2] = fma2(x2[c], pk2(whi.x, whi.y), t[2]); t[3] = fma2(x2[c], pk2(whi.z, whi.w), t[3]);
       }
 #pragma unroll
-    for (int jj = 0; jj < 4; ++jj) act_split_pair(t[jj], one2, sp[8 * p + 2 * jj], sp[8 * p + 2 * jj + 1], hi[jj], lo[jj]);
-    if (m0 + r < M) {
-      const size_t o = tile_base + (size_t)p * PIECE_HALVES;
-      *reinterpret_cast<uint4*>(out_hi + o) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
-      *reinterpret_cast<uint4*>(out_lo + o) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
+      for (int jj = 0; jj < 4; ++jj) act_split_pair(t[jj], one2, sp[8 * p + 2 * jj], sp[8 * p + 2 * jj + 1], hi[jj], lo[jj]);
+      if (m0 + r < M) {
+        const size_t o = tile_base + (size_t)p * PIECE_HALVES;
+        *reinterpret_cast<uint4*>(out_hi + o) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
+        *reinterpret_cast<uint4*>(out_lo + o) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
+      }
     }
   }
 }
@@ -656,8 +659,11 @@ nsgpu_status mlp_forward_tc(nsgpu_ctx* ctx, int e, const float* theta, int B, co
   {
     StageTimer tm(ctx, 0, st);
     const size_t smem = (size_t)E.width * sizeof(float4) + (size_t)E.n_in * E.width * sizeof(float);
-#define NSGPU_FL(N_) case N_: mlp_first_layer_tc<N_><<<(M + BLOCK_M - 1) / BLOCK_M, 256, smem, st>>>ARGS_; break;
-#define ARGS_ (theta, ctx->D, rpt, M, n_rows_dev, ctx->emu_in_idx,                                                                       ctx->emu_in_const, ctx->n_theta_in, ctx->z_emu,                                                                       E.n_in, E.in_mean, E.in_std, E.W[0],                                                                       T->layers[0].p_hidden, E.width, T->act[0][0],                                                                       T->act[0][1])
+    const int fl_tiles = (M + BLOCK_M - 1) / BLOCK_M;
+    const int fl_split = fl_tiles >= 4 * ctx->sm_count ? 1 : 4;
+    const int fl_grid = fl_tiles * fl_split;
+#define NSGPU_FL(N_) case N_: mlp_first_layer_tc<N_><<<fl_grid, 256, smem, st>>>ARGS_; break;
+#define ARGS_ (theta, ctx->D, rpt, M, n_rows_dev, ctx->emu_in_idx,                                                                       ctx->emu_in_const, ctx->n_theta_in, ctx->z_emu,                                                                       E.n_in, E.in_mean, E.in_std, E.W[0],                                                                       T->layers[0].p_hidden, E.width, fl_split, T->act[0][0],                                                                       T->act[0][1])
     switch (E.n_in) {
       NSGPU_FL(1) NSGPU_FL(2) NSGPU_FL(3) NSGPU_FL(4) NSGPU_FL(5) NSGPU_FL(6) NSGPU_FL(7) NSGPU_FL(8)
       NSGPU_FL(9) NSGPU_FL(10) NSGPU_FL(11) NSGPU_FL(12) NSGPU_FL(13) NSGPU_FL(14) NSGPU_FL(15) NSGPU_FL(16)

@@ -595,13 +595,9 @@ __global__ void __launch_bounds__(LIMBER_THREADS, 2) shear_limber_kernel(const f
   __syncthreads();                                       // zero fill done
   stage(0);
   for (int c = 0; c < n_chunks; ++c) {
-    if (c + 1 < n_chunks) {
-      stage(c + 1);                                      // buffer (c + 1) & 1 was consumed before the barrier that ended chunk c - 1
-      asm volatile("cp.async.wait_group 1;" ::: "memory");
-    } else {
-      asm volatile("cp.async.wait_group 0;" ::: "memory");
-    }
-    __syncthreads();
+    asm volatile("cp.async.wait_group 0;" ::: "memory"); // this thread's copies of chunk c (the only group in flight)
+    __syncthreads();                                     // everyone's copies landed; everyone is done with chunk c - 1
+    if (c + 1 < n_chunks) stage(c + 1);                  // into the buffer chunk c - 1 used; overlaps the arithmetic below
     if (live) {
       const size_t o = (size_t)(c & 1) * buf_doubles;
       const double *wi_c = wi + o, *wj_c = wj + o, *pg_c = pg + o;
@@ -617,7 +613,6 @@ __global__ void __launch_bounds__(LIMBER_THREADS, 2) shear_limber_kernel(const f
         }
       }
     }
-    __syncthreads();                                     // chunk c consumed: its buffer may be refilled
   }
   // join the slices in a fixed order through shared memory (the chunk buffers are free now): slice s parks
   // its sums, slice 0 adds them
