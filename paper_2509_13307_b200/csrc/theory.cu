@@ -11,6 +11,8 @@
 // the emulator, and the absolute log L tolerance leaves no room for fp32 round-off downstream of
 // the network.  The oracle sums the four terms of eq. A1 separately; this kernel
 // projects the factored form (W^gamma + W^I)_i (W^gamma + W^I)_j once.
+#include <math_constants.h>
+
 #include "internal.cuh"
 
 namespace {
@@ -30,6 +32,7 @@ __device__ __forceinline__ double warp_sum(double v) {
 // arithmetic in 2^y and Gaussian evaluations.
 __device__ __forceinline__ double exp_fast(double x) {
   if (x < -700.0) return 0.0;
+  if (x > 709.0) return CUDART_INF;                      // past the exponent range: overflow, not garbage
   const double n = rint(x * 1.4426950408889634);
   double r = fma(n, -6.93147180369123816490e-01, x);
   r = fma(n, -1.90821492927058770002e-10, r);
