@@ -309,12 +309,8 @@ nsgpu_status chi2_loglike(nsgpu_ctx* ctx, const float* theta, int B, const int* 
     const bool small = (size_t)n_rb * ((B + 63) / 64) < (size_t)ctx->sm_count;
     const int tblk = small ? 32 : 64, n_tb = (B + tblk - 1) / tblk;
     const size_t smem_t = (size_t)CT_NBUF * CT_KC * (CT_ROWS + tblk) * sizeof(double) + 2 * CT_NBUF * 8;
-    static bool configured = false;
-    if (!configured) {
-      NSGPU_CUDA(cudaFuncSetAttribute(chi2_tile_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024));
-      NSGPU_CUDA(cudaFuncSetAttribute(chi2_tile_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024));
-      configured = true;
-    }
+    NSGPU_CUDA(nsgpu_ensure_smem(ctx, chi2_tile_kernel<8>, smem_t));
+    NSGPU_CUDA(nsgpu_ensure_smem(ctx, chi2_tile_kernel<4>, smem_t));
     if (small) chi2_tile_kernel<4><<<n_rb * n_tb, CT_WARPS * 32, smem_t, st>>>(ctx->Linv, ctx->resid_t, n, B, n_rows_dev, ldr, n_tb, ctx->chi2_part);
     else chi2_tile_kernel<8><<<n_rb * n_tb, CT_WARPS * 32, smem_t, st>>>(ctx->Linv, ctx->resid_t, n, B, n_rows_dev, ldr, n_tb, ctx->chi2_part);
     NSGPU_LAUNCH_CHECK();
@@ -345,11 +341,7 @@ nsgpu_status chi2_loglike(nsgpu_ctx* ctx, const float* theta, int B, const int* 
 #define NSGPU_CHI2_ARGS ctx->model, ctx->data, ctx->Linv, n, B, RT, CH, n_rows_dev, theta, ctx->D, ctx->prior_kind, ctx->prior_p0, ctx->prior_p1, ctx->log_norm, logL
 #define NSGPU_CHI2_LAUNCH(TB_, TG_, MAXT_)                                                                        \
   do {                                                                                                            \
-    static size_t configured = 0;                                                                                 \
-    if (smem > configured) {                                                                                      \
-      NSGPU_CUDA(cudaFuncSetAttribute(chi2_kernel<TB_, TG_, MAXT_>, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024)); \
-      configured = 220 * 1024;                                                                                    \
-    }                                                                                                             \
+    NSGPU_CUDA(nsgpu_ensure_smem(ctx, chi2_kernel<TB_, TG_, MAXT_>, 220 * 1024));                                   \
     chi2_kernel<TB_, TG_, MAXT_><<<grid, threads, smem, st>>>(NSGPU_CHI2_ARGS);                                   \
   } while (0)
   if (groups == 4 && tg == 8) NSGPU_CHI2_LAUNCH(32, 8, 640);

@@ -7,6 +7,7 @@
 #include <stdint.h>
 
 #include <algorithm>
+#include <map>
 #include <string>
 #include <vector>
 
@@ -91,6 +92,7 @@ struct nsgpu_ctx {
   SamplerDev* sampler = nullptr;
   std::string err;
   int64_t launches = 0;
+  std::map<const void*, size_t> smem_limit;   // dynamic shared memory opted in per kernel, on this context's device
   // optional per-stage CUDA-event timing (nsgpu_set_profiling / nsgpu_stage_times)
   bool profiling = false;
   struct StageEv { int stage; cudaEvent_t a, b; };
@@ -125,6 +127,17 @@ struct StageTimer {
       return NSGPU_ECUDA;                                                                 \
     }                                                                                     \
   } while (0)
+
+// Raise a kernel's dynamic shared-memory limit to `bytes` on the context's device (function attributes are per
+// device: the bookkeeping lives in the context, not in a process-wide static).
+template <class F>
+inline cudaError_t nsgpu_ensure_smem(nsgpu_ctx* ctx, F* fn, size_t bytes) {
+  size_t& cur = ctx->smem_limit[reinterpret_cast<const void*>(fn)];
+  if (bytes <= cur) return cudaSuccess;
+  const cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+  if (e == cudaSuccess) cur = bytes;
+  return e;
+}
 
 #define NSGPU_LAUNCH_CHECK()                                                              \
   do {                                                                                    \

@@ -520,11 +520,7 @@ int pick_block_n(int n, bool hidden) {
 template <int BN, int EPI>
 nsgpu_status launch_gemm(nsgpu_ctx* ctx, const CUtensorMap& whi, const CUtensorMap& wlo, const GemmArgs& g, cudaStream_t st) {
   const int smem = num_stages(BN) * stage_bytes(BN) + 16 * num_stages(BN) + 128 + (EPI == 0 ? 16 * g.N_pad : 0) + 1024;
-  static bool configured = false;
-  if (!configured) {
-    NSGPU_CUDA(cudaFuncSetAttribute(mlp_gemm_tc<BN, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BUDGET));
-    configured = true;
-  }
+  NSGPU_CUDA(nsgpu_ensure_smem(ctx, mlp_gemm_tc<BN, EPI>, SMEM_BUDGET));
   const int tiles = ((g.M_host + BLOCK_M - 1) / BLOCK_M) * (g.N_pad / BN);
   const int grid = std::min(tiles, ctx->sm_count);
   mlp_gemm_tc<BN, EPI><<<grid, GEMM_THREADS, smem, st>>>(whi, wlo, g);

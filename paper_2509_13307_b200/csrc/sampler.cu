@@ -539,11 +539,7 @@ static nsgpu_status launch_delete(nsgpu_ctx* ctx, const double* logL, int n, int
   int np2 = 1;
   while (np2 < n) np2 <<= 1;
   const size_t smem = (size_t)np2 * (sizeof(double) + sizeof(int));
-  static size_t configured = 0;
-  if (smem > configured) {
-    NSGPU_CUDA(cudaFuncSetAttribute(delete_lowest_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    configured = smem;
-  }
+  NSGPU_CUDA(nsgpu_ensure_smem(ctx, delete_lowest_kernel, smem));
   delete_lowest_kernel<<<1, 1024, smem, st>>>(logL, n, k, S->scal, S->dead_idx, S->surv_idx, S->logw);
   NSGPU_LAUNCH_CHECK();
   return NSGPU_OK;

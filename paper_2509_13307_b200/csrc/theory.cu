@@ -780,15 +780,8 @@ nsgpu_status shear_project(nsgpu_ctx* ctx, const float* theta, int B, const int*
     }
     const int IW = (n_items + 31) & ~31;                  // tiles per slice of the quadrature axis, whole warps
     const size_t smem_l = std::max((size_t)2 * (ntp + n_lb * LIMBER_LB) * LIMBER_QCP, (size_t)IW * 4 * LIMBER_LB) * sizeof(double);
-    static size_t conf_w = 0, conf_l = 0;
-    if (smem_w > conf_w) {
-      NSGPU_CUDA(cudaFuncSetAttribute(shear_windows_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_w));
-      conf_w = smem_w;
-    }
-    if (smem_l > conf_l) {
-      NSGPU_CUDA(cudaFuncSetAttribute(shear_limber_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_l));
-      conf_l = smem_l;
-    }
+    NSGPU_CUDA(nsgpu_ensure_smem(ctx, shear_windows_kernel, smem_w));
+    NSGPU_CUDA(nsgpu_ensure_smem(ctx, shear_limber_kernel, smem_l));
     shear_windows_kernel<<<B, win_threads, smem_w, st>>>(theta, ctx->D, n_rows_dev, A, G, S.aux);
     NSGPU_LAUNCH_CHECK();
     const int bpt = (((S.n_ell + 3) / 4) * S.n_chi + 255) / 256;
@@ -800,13 +793,9 @@ nsgpu_status shear_project(nsgpu_ctx* ctx, const float* theta, int B, const int*
   }
   const size_t smem = shear_smem_bytes(S);
   const size_t smem1 = smem - (size_t)S.n_z_emu * S.n_k * sizeof(float);       // phase 1 stages no table
-  static size_t configured = 0;
-  if (smem > configured) {
-    NSGPU_CUDA(cudaFuncSetAttribute(shear_project_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    NSGPU_CUDA(cudaFuncSetAttribute(shear_project_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    NSGPU_CUDA(cudaFuncSetAttribute(shear_project_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    configured = smem;
-  }
+  NSGPU_CUDA(nsgpu_ensure_smem(ctx, shear_project_kernel<0>, smem));
+  NSGPU_CUDA(nsgpu_ensure_smem(ctx, shear_project_kernel<1>, smem));
+  NSGPU_CUDA(nsgpu_ensure_smem(ctx, shear_project_kernel<2>, smem));
   // the two-kernel split needs 16-byte sized / aligned pieces for the bulk copies
   const bool split = ((size_t)S.n_z_emu * S.n_k * 4) % 16 == 0 && ((size_t)(3 + S.n_tomo) * S.n_chi * 8) % 16 == 0 &&
                      ((size_t)3 * S.n_chi * 8) % 16 == 0 && S.aux != nullptr;
