@@ -29,6 +29,7 @@
 
 struct SamplerDev {
   int cap = 0;   // max chains / live points
+  int rounds_needed = 0, rounds_n_steps = -1;   // rounds the last evolve() took (for that n_steps): sizes the next first burst
   // chain state (SoA)
   float *x0 = nullptr, *dir = nullptr, *xprop = nullptr, *theta_chain = nullptr;   // [cap][D]
   double *l = nullptr, *r = nullptr, *t = nullptr, *logL0 = nullptr;
@@ -563,8 +564,11 @@ static nsgpu_status evolve(nsgpu_ctx* ctx, int n_chains, int chain0, int n_steps
   NSGPU_CUDA(cudaMemsetAsync(S->counters, 0, 4 * sizeof(int), st));
   const int blocks = (n_chains * 32 + 127) / 128;
   int64_t rounds = 0;
-  // a slice move costs ~5 proposals (SURVEY c.2): run most of the expected rounds before the first check
-  int burst = std::max(8, n_steps * 4);
+  // Rounds are launched in bursts and the finished-counter is read after each burst (one small D2H).  A round
+  // after the last chain has finished is a dozen empty launches, a check is a pipeline drain: the first burst
+  // runs up to just short of what the previous call on this context needed (n_steps to start with: no chain
+  // can finish earlier), then short bursts until every chain is done.
+  int burst = std::max(8, (S->rounds_needed > 0 && S->rounds_n_steps == n_steps) ? S->rounds_needed - 24 : n_steps);
   while (true) {
     for (int i = 0; i < burst; ++i) {
       {
@@ -582,12 +586,14 @@ static nsgpu_status evolve(nsgpu_ctx* ctx, int n_chains, int chain0, int n_steps
     NSGPU_CUDA(cudaMemcpyAsync(S->h_counters, S->counters, 4 * sizeof(int), cudaMemcpyDeviceToHost, st));
     NSGPU_CUDA(cudaStreamSynchronize(st));
     if (S->h_counters[1] >= n_chains) break;
-    burst = std::max(4, n_steps / 4);
+    burst = 16;
     if (rounds > (int64_t)n_steps * (MAX_STEP_OUT * 2 + MAX_SHRINK + 4) + 16) {
       ctx->err = "slice sampling: chains did not finish (internal error)";
       return NSGPU_ECUDA;
     }
   }
+  S->rounds_needed = (int)std::min<int64_t>(rounds, 1 << 30);
+  S->rounds_n_steps = n_steps;
   if (rounds_out) *rounds_out += rounds;
   return NSGPU_OK;
 }
