@@ -128,6 +128,19 @@ def test_edge_cases_and_errors():
     with pytest.raises(nsgpu.NsgpuError) as e:
         nsgpu.Context(workload("tiny_shear"), max_batch=4, mlp=nsgpu.MLP_TC)      # width 48: no tcgen05 path
     assert e.value.status == nsgpu.ESHAPE
+    import copy
+    bad_terms = copy.deepcopy(workload("tiny_shear_paper")); bad_terms.theory.n_ia_terms = 4
+    with pytest.raises(nsgpu.NsgpuError) as e:
+        nsgpu.Context(bad_terms, max_batch=4)
+    assert e.value.status == nsgpu.EINVAL
+    over = copy.deepcopy(workload("tiny_shear_paper")); over.theory.n_m_terms = 2     # block of 2 n_tomo runs past D
+    with pytest.raises(nsgpu.NsgpuError) as e:
+        nsgpu.Context(over, max_batch=4)
+    assert e.value.status == nsgpu.EINVAL
+    with nsgpu.Context(workload("identity"), max_batch=64) as ctx:
+        with pytest.raises(nsgpu.NsgpuError) as e:                                 # more than one rank needs an exchange
+            ctx.run_sharded(64, 32, 5, rank=2, world=2, allgather=lambda *a: 0)
+        assert e.value.status == nsgpu.EINVAL
 
 
 def test_noiseless_fiducial_gives_normalisation_constant():
