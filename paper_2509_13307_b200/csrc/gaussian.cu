@@ -146,8 +146,7 @@ __global__ void __launch_bounds__(MAXT) chi2_kernel(const double* __restrict__ m
 // 8 thetas), which is what bounds it for n ~ 1000.  Here a CTA owns a 128-row block of Linv and TG*8 thetas:
 // the factor crosses L2 -> shared memory once per 64 thetas.  Operands: LinvT (column j contiguous over rows)
 // and the residuals transposed to [n][batch] so that both tiles of a k-step are contiguous pieces moved by
-// bulk asynchronous copies through a ring of stages.  A warp owns 8 (TG) thetas and all 128 rows: the residuals
-// of a column are one broadcast line, the factor column is conflict-free; 4 x TG fp64 accumulators per lane.
+// bulk asynchronous copies through a ring of stages.  The product itself runs on the fp64 tensor cores (DMMA).
 // Partial sums of w^2 per (row block, theta) are joined in a fixed order by chi2_finalize_kernel.
 constexpr int CT_ROWS = 128, CT_KC = 8, CT_NBUF = 4, CT_WARPS = 8;
 
@@ -168,20 +167,32 @@ __global__ void residual_transpose_kernel(const double* __restrict__ model, cons
   }
 }
 
+// D (8x8) += A (8x4, row) . B (4x8, col) on the fp64 tensor cores.  Fragments (PTX ISA, mma.m8n8k4 .f64): lane l holds
+// A[l >> 2][l & 3], B[l & 3][l >> 2] and D[l >> 2][2 (l & 3) + {0, 1}].
+__device__ __forceinline__ void dmma_8x8x4(double (&d)[2], double a, double b) {
+  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};"
+               : "+d"(d[0]), "+d"(d[1]) : "d"(a), "d"(b));
+}
+
+// TG = thetas per CTA / 8 (8: 64 thetas, 4: 32).  A warp owns 16 rows (two 8-row MMA tiles) and all the CTA's thetas:
+// per 4 columns of the factor it loads 2 A and TG B fragments and issues 2 TG DMMAs (256 FMA each) -- an eighth of
+// the instructions of the scalar formulation, which ran at half the fp64 rate for instruction overhead alone.  The
+// tile rows are padded by 8 doubles so that a fragment load (4 columns x 8 rows) covers every bank exactly twice.
 template <int TG>
 __global__ void __launch_bounds__(CT_WARPS * 32, 2) chi2_tile_kernel(const double* __restrict__ LinvT,
                                                                      const double* __restrict__ rt, int n, int B,
                                                                      const int* __restrict__ n_rows_dev, size_t ldr,
                                                                      int n_tb, double* __restrict__ part) {
-  constexpr int TBLK = CT_WARPS * TG;                     // thetas per CTA
+  constexpr int TBLK = 8 * TG;                            // thetas per CTA
+  constexpr int LDL = CT_ROWS + 8, LDR = TBLK + 8;        // padded tile rows (stride = 8 mod 16 doubles)
   const int live = n_rows_dev ? min(B, *n_rows_dev) : B;
   const int n_rb = (n + CT_ROWS - 1) / CT_ROWS;
   const int rb = n_rb - 1 - blockIdx.x / n_tb;            // longest row blocks first
   const int b0 = (blockIdx.x % n_tb) * TBLK;
   if (b0 >= live) return;
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  typedef double LTile[CT_KC][CT_ROWS];
-  typedef double RTile[CT_KC][TBLK];
+  typedef double LTile[CT_KC][LDL];
+  typedef double RTile[CT_KC][LDR];
   LTile* Ls = reinterpret_cast<LTile*>(smem_raw);                                   // [CT_NBUF]
   RTile* Rs = reinterpret_cast<RTile*>(smem_raw + sizeof(LTile) * CT_NBUF);         // [CT_NBUF]
   unsigned long long* bars = reinterpret_cast<unsigned long long*>(smem_raw + (sizeof(LTile) + sizeof(RTile)) * CT_NBUF);
@@ -203,7 +214,7 @@ __global__ void __launch_bounds__(CT_WARPS * 32, 2) chi2_tile_kernel(const doubl
     else if (lane >= 16 && lane - 16 < jn)
       tc::bulk_load(tc::smem_u32(&Rs[buf][lane - 16][0]), rt + (size_t)(j0 + lane - 16) * ldr + b0, TBLK * 8u, full0 + 8 * buf);
   };
-  static_assert(CT_KC <= 16, "one lane per copy");
+  static_assert(CT_KC <= 16 && CT_KC % 4 == 0 && CT_ROWS == 16 * CT_WARPS, "one lane per copy; whole MMA k-steps; 16 rows per warp");
   if (tid == 0) {
     for (int b = 0; b < CT_NBUF; ++b) { tc::mbar_init(full0 + 8 * b, 1); tc::mbar_init(empty0 + 8 * b, CT_WARPS); }
     tc::fence_barrier_init();
@@ -211,11 +222,12 @@ __global__ void __launch_bounds__(CT_WARPS * 32, 2) chi2_tile_kernel(const doubl
   __syncthreads();
   if (warp == 0)
     for (int s = 0; s < CT_NBUF - 1 && s < n_steps; ++s) load_step(s, s);
-  double acc[4][TG];
+  double acc[2][TG][2];
 #pragma unroll
-  for (int r = 0; r < 4; ++r)
+  for (int m = 0; m < 2; ++m)
 #pragma unroll
-    for (int t = 0; t < TG; ++t) acc[r][t] = 0.0;
+    for (int t = 0; t < TG; ++t) { acc[m][t][0] = 0.0; acc[m][t][1] = 0.0; }
+  const int fk = lane & 3, fr = lane >> 2;               // fragment coordinates of this lane
   for (int s = 0; s < n_steps; ++s) {
     const int buf = s % CT_NBUF;
     if (warp == 0 && s + CT_NBUF - 1 < n_steps) {
@@ -226,34 +238,48 @@ __global__ void __launch_bounds__(CT_WARPS * 32, 2) chi2_tile_kernel(const doubl
     }
     tc::mbar_wait(full0 + 8 * buf, (s / CT_NBUF) & 1);
     const int jn = min(CT_KC, K - s * CT_KC);
-    auto column = [&](int jj) {
-      double l[4], v[TG];
 #pragma unroll
-      for (int r = 0; r < 4; ++r) l[r] = Ls[buf][jj][lane + 32 * r];
+    for (int ks = 0; ks < CT_KC / 4; ++ks) {
+      const int jj = 4 * ks + fk;
+      const bool in = jj < jn;                            // columns past K in the last step were not copied
+      double a[2], v[TG];
 #pragma unroll
-      for (int t = 0; t < TG; ++t) v[t] = Rs[buf][jj][warp * TG + t];
+      for (int m = 0; m < 2; ++m) a[m] = in ? Ls[buf][jj][16 * warp + 8 * m + fr] : 0.0;
 #pragma unroll
-      for (int r = 0; r < 4; ++r)
+      for (int t = 0; t < TG; ++t) v[t] = in ? Rs[buf][jj][8 * t + fr] : 0.0;
 #pragma unroll
-        for (int t = 0; t < TG; ++t) acc[r][t] = fma(l[r], v[t], acc[r][t]);
-    };
-    if (jn == CT_KC) {                                   // every step but the last: fully unrolled
+      for (int m = 0; m < 2; ++m)
 #pragma unroll
-      for (int jj = 0; jj < CT_KC; ++jj) column(jj);
-    } else {
-      for (int jj = 0; jj < jn; ++jj) column(jj);
+        for (int t = 0; t < TG; ++t) dmma_8x8x4(acc[m][t], a[m], v[t]);
     }
     __syncwarp();
     if (lane == 0) tc::mbar_arrive(empty0 + 8 * buf);
   }
+  // sum of w^2 over this warp's 16 rows for each theta (lanes with equal fk hold the same two thetas of a tile),
+  // then over the 8 warps through shared memory in a fixed order
+  __syncthreads();                                       // every warp is done with the ring: reuse it
+  double* red = reinterpret_cast<double*>(smem_raw);     // [CT_WARPS][TBLK]
 #pragma unroll
-  for (int t = 0; t < TG; ++t) {
+  for (int t = 0; t < TG; ++t)
+#pragma unroll
+    for (int e = 0; e < 2; ++e) {
+      double ss = 0.0;
+#pragma unroll
+      for (int m = 0; m < 2; ++m) {
+        const bool ok = i0 + 16 * warp + 8 * m + fr < n;  // rows past n hold stale tiles
+        ss += ok ? acc[m][t][e] * acc[m][t][e] : 0.0;
+      }
+      ss += __shfl_xor_sync(0xffffffffu, ss, 4);
+      ss += __shfl_xor_sync(0xffffffffu, ss, 8);
+      ss += __shfl_xor_sync(0xffffffffu, ss, 16);
+      if (fr == 0) red[warp * TBLK + 8 * t + 2 * fk + e] = ss;
+    }
+  __syncthreads();
+  if (tid < TBLK) {
     double ss = 0.0;
 #pragma unroll
-    for (int r = 0; r < 4; ++r) ss += (i0 + lane + 32 * r < n) ? acc[r][t] * acc[r][t] : 0.0;   // rows past n hold stale tiles
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) ss += __shfl_xor_sync(0xffffffffu, ss, o);
-    if (lane == 0) part[(size_t)rb * ldr + b0 + warp * TG + t] = ss;
+    for (int w = 0; w < CT_WARPS; ++w) ss += red[w * TBLK + tid];
+    part[(size_t)rb * ldr + b0 + tid] = ss;
   }
 }
 
@@ -308,7 +334,7 @@ nsgpu_status chi2_loglike(nsgpu_ctx* ctx, const float* theta, int B, const int* 
     // 64 thetas per CTA; 32 when that would leave SMs idle (the nested-sampling rounds)
     const bool small = (size_t)n_rb * ((B + 63) / 64) < (size_t)ctx->sm_count;
     const int tblk = small ? 32 : 64, n_tb = (B + tblk - 1) / tblk;
-    const size_t smem_t = (size_t)CT_NBUF * CT_KC * (CT_ROWS + tblk) * sizeof(double) + 2 * CT_NBUF * 8;
+    const size_t smem_t = (size_t)CT_NBUF * CT_KC * (CT_ROWS + 8 + tblk + 8) * sizeof(double) + 2 * CT_NBUF * 8;
     NSGPU_CUDA(nsgpu_ensure_smem(ctx, chi2_tile_kernel<8>, smem_t));
     NSGPU_CUDA(nsgpu_ensure_smem(ctx, chi2_tile_kernel<4>, smem_t));
     if (small) chi2_tile_kernel<4><<<n_rb * n_tb, CT_WARPS * 32, smem_t, st>>>(ctx->Linv, ctx->resid_t, n, B, n_rows_dev, ldr, n_tb, ctx->chi2_part);
