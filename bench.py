@@ -265,7 +265,7 @@ def run_nsgpu(args, rank, world, local_rank):
     ranks = Ranks(world, "nccl", torch.device("cuda", dev))
     wl = MAKERS[args.workload]()
     B = args.batch
-    ctx = make_context(nsgpu, torch, wl, B, dev, nsgpu.SHEAR_STREAM if args.shear_stream else 0)
+    ctx = make_context(nsgpu, torch, wl, B, dev, (nsgpu.SHEAR_STREAM if args.shear_stream else 0) | args.ctx_flags)
     n_sets = 4
     th_dev, th_host = theta_batches(nsgpu, torch, ctx, wl, B, rank, n_sets, dev)
     out = torch.empty(B, dtype=torch.float64, device=f"cuda:{dev}")
@@ -381,6 +381,7 @@ def main():
     ap.add_argument("--ref-sample", type=int, default=16)
     ap.add_argument("--shear-stream", action="store_true",
                     help="shear workloads: use the streaming projection kernels even where the resident one fits")
+    ap.add_argument("--ctx-flags", type=int, default=0, help=argparse.SUPPRESS)      # extra nsgpu_create flags (kernel A/B runs)
     ap.add_argument("--dry-run-cpu", action="store_true", help=argparse.SUPPRESS)
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))

@@ -320,9 +320,9 @@ nsgpu_status chi2_loglike(nsgpu_ctx* ctx, const float* theta, int B, const int* 
                           cudaStream_t st) {
   if (B == 0) return NSGPU_OK;
   const int n = ctx->n_data;
-  // n >= 512: tiled path (transposed residuals, blocked triangular product, fixed-order join).  Measured at
-  // B = 4096: n = 1100 0.40 vs 1.03 ms, n = 613 0.18 vs 0.25 ms; n = 300 0.095 vs 0.065 ms (three launches and
-  // short k loops), so small problems stay on the single streaming kernel below.
+  // n >= 512: tiled path (transposed residuals, blocked triangular product on the fp64 tensor cores, fixed-order
+  // join).  Measured at B = 4096: n = 1100 0.25 vs 1.03 ms, n = 613 0.12 vs 0.25 ms; n = 300 0.073 vs 0.064 ms
+  // (three launches and short k loops), so small problems stay on the single streaming kernel below.
   const bool tiled = (ctx->flags & NSGPU_CHI2_TILED) ? true : ((ctx->flags & NSGPU_CHI2_STREAMED) ? false : n >= 512);
   if (ctx->resid_t && tiled) {
     const size_t ldr = ((size_t)ctx->max_batch + 63) & ~(size_t)63;
