@@ -164,12 +164,19 @@ nsgpu_status build_shear(nsgpu_ctx* ctx, const nsgpu_theory* t) {
   NSGPU_CUDA(upload(&S.ell, t->ell, (size_t)t->n_ell));
   NSGPU_CUDA(upload(&S.nz_mean, t->nz_mean, (size_t)t->n_tomo));
   NSGPU_CUDA(upload(&ctx->z_emu, zef.data(), zef.size()));
-  NSGPU_CUDA(cudaMalloc((void**)&S.aux, (size_t)ctx->max_batch * (3 + t->n_tomo) * t->n_chi * sizeof(double)));
+  {   // rows of n_chi rounded up to even (the streaming kernels bulk-copy row pieces); padding stays zero
+    const size_t aux_bytes = (size_t)ctx->max_batch * (3 + t->n_tomo) * ((t->n_chi + 1) & ~1) * sizeof(double);
+    NSGPU_CUDA(cudaMalloc((void**)&S.aux, aux_bytes));
+    NSGPU_CUDA(cudaMemset(S.aux, 0, aux_bytes));
+  }
   // the resident projection keeps a theta's table and scratch in shared memory (two CTAs per SM); larger
   // grids -- the paper's 1025 nodes and 10 bins -- take the streaming kernels
   S.streaming = (ctx->flags & NSGPU_SHEAR_STREAM) != 0 || shear_resident_smem(S) > 113 * 1024;
-  if (S.streaming)
-    NSGPU_CUDA(cudaMalloc((void**)&S.pg, (size_t)ctx->max_batch * t->n_ell * ((t->n_chi + 1) & ~1) * sizeof(double)));
+  if (S.streaming) {
+    const size_t pg_bytes = (size_t)ctx->max_batch * t->n_ell * ((t->n_chi + 1) & ~1) * sizeof(double);
+    NSGPU_CUDA(cudaMalloc((void**)&S.pg, pg_bytes));
+    NSGPU_CUDA(cudaMemset(S.pg, 0, pg_bytes));
+  }
   return NSGPU_OK;
 }
 

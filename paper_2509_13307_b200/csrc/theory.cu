@@ -14,6 +14,7 @@
 #include <math_constants.h>
 
 #include "internal.cuh"
+#include "tc_ptx.cuh"
 
 namespace {
 
@@ -373,7 +374,8 @@ __global__ void __launch_bounds__(256) shear_windows_kernel(const float* __restr
   double* scr = ichi + nqp;                            // [2 G][nqp] scan arrays
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarp = blockDim.x >> 5;
   const float* th = theta + (size_t)b * D;
-  double* aux_b = aux + (size_t)b * (3 + nt) * nq;
+  const int nqs = (nq + 1) & ~1;                       // row stride of `aux` here: even, rows are bulk-copied in chunks
+  double* aux_b = aux + (size_t)b * (3 + nt) * nqs;
   const double ob = th[A.idx_omega_b], oc = th[A.idx_omega_cdm], h = th[A.idx_h];
   const double Om = (ob + oc) / (h * h);
   const double w0 = A.idx_w0 >= 0 ? (double)th[A.idx_w0] : -1.0;
@@ -401,13 +403,13 @@ __global__ void __launch_bounds__(256) shear_windows_kernel(const float* __restr
     ichi[q] = ic;
     iD[q] = exp_fast(scr[nqp + q] + 0.5 * iD[q]);
     aux_b[q] = C_OVER_H0 * fda * ic * ic;               // g_q = dchi_q / chi_q^2
-    aux_b[nq + q] = log10(c);
-    aux_b[2 * nq + q] = ic;
+    aux_b[nqs + q] = log10(c);
+    aux_b[2 * nqs + q] = ic;
   }
   __syncthreads();
   const double inv_sig = 1.0 / A.nz_sigma;
   const double norm = inv_sig / 2.5066282746310002;
-  double* Wt = aux_b + 3 * (size_t)nq;
+  double* Wt = aux_b + 3 * (size_t)nqs;
   for (int i0 = 0; i0 < nt; i0 += G) {
     const int g = min(G, nt - i0);
     double wI[WIN_ITEMS];                                  // W^I of this thread's (bin, node) items, kept across the scans
@@ -440,7 +442,7 @@ __global__ void __launch_bounds__(256) shear_windows_kernel(const float* __restr
       if (it < g * nq) {
         const int ii = it / nq, q = it - ii * nq, i = i0 + ii;
         const double s0 = scr[(size_t)(2 * ii) * nqp + q], s1 = scr[(size_t)(2 * ii + 1) * nqp + q];
-        Wt[(size_t)i * nq + q] =
+        Wt[(size_t)i * nqs + q] =
             wI[s] + 1.5 * Om / (C_OVER_H0 * C_OVER_H0) * (1.0 + A.z_q[q]) * chi[q] * (s0 - chi[q] * s1);   // + W^gamma (eq. A3)
       }
     }
@@ -465,11 +467,11 @@ __global__ void __launch_bounds__(256) shear_power_kernel(const float* __restric
   const int lg = it / nq, q = it - lg * nq;
   const float* th = theta + (size_t)b * D;
   const float* table = spec + (size_t)b * A.n_z_emu * A.n_k;
-  const double* aux_b = aux + (size_t)b * (3 + A.n_tomo) * nq;
+  const double* aux_b = aux + (size_t)b * (3 + A.n_tomo) * nq2;
   double* out = pg + (size_t)b * A.n_ell * nq2 + q;
   const double eta0 = A.idx_eta0 >= 0 ? (double)th[A.idx_eta0] : 0.7;
   const double inv_dlk = 1.0 / A.dlk, bar_amp = (eta0 - 0.7) * 0.1;
-  const double g_q = aux_b[q], lc = aux_b[nq + q], ic = aux_b[2 * nq + q];
+  const double g_q = aux_b[q], lc = aux_b[nq2 + q], ic = aux_b[2 * nq2 + q];
   const double* tw = A.tap_w + (size_t)q * A.n_tap;
   const float* col0 = table + (size_t)A.tap_start[q] * A.sz;
   const int l0 = 4 * lg, nl = min(4, A.n_ell - l0);
@@ -527,128 +529,167 @@ __global__ void __launch_bounds__(256) shear_power_kernel(const float* __restric
   }
 }
 
-// a8 (sum) for any grid: C_ij(ell) = sum_q W_i W_j (P g)_q as a register-tiled product over chunks of QC
-// quadrature nodes.  A thread owns 2 x 2 bin pairs x LB multipoles (20 accumulators) and every NS-th node of
-// the chunk.  The lanes of a warp are different tiles at the SAME node: a shared-memory load touches at most
-// 5 distinct rows, which the odd row stride puts in different banks -- one wavefront per load, so the 9 loads
-// per node stay under the 24 fp64 operations they feed.
+// a8 (sum) for any grid: C_ij(ell) = sum_q W_i W_j (P g)_q is, per theta, the product of WW [pairs][q] with
+// (P g)^T [q][ell] (55 x 1025 by 1025 x 20 for the paper's grid): a dense fp64 contraction, done on the fp64 tensor
+// cores (mma.m8n8k4.f64).  Fragments: lane l holds A[l >> 2][l & 3] (pair, node), B[l & 3][l >> 2] (node, ell) and
+// D[l >> 2][2 (l & 3) + {0, 1}].  The A element W_i W_j is formed on the fly by the one lane that needs it (two
+// shared-memory loads and a DMUL), so the pair products never exist in memory.  A warp owns two 8-pair tiles x all
+// ell tiles and a slice of the 4-node k-steps of each chunk; chunks of QC nodes of W and P g are staged by 8-byte
+// cp.async into a double buffer, one chunk ahead.  Row stride = 4 mod 16 doubles: a fragment load (8 rows x 4
+// consecutive nodes) covers every bank exactly twice.
 constexpr int LIMBER_THREADS = 256;
-constexpr int LIMBER_LB = 5;      // multipoles per thread tile
-constexpr int LIMBER_QC = 128;    // quadrature nodes per chunk
-constexpr int LIMBER_QCP = LIMBER_QC + 1;
-__global__ void __launch_bounds__(LIMBER_THREADS, 2) shear_limber_kernel(const float* __restrict__ theta, int D,
+constexpr int LIMBER_QC = 64;                 // quadrature nodes per chunk
+constexpr int LIMBER_LD = LIMBER_QC + 4;      // row stride of the staged chunks
+constexpr int LIMBER_MAX_NT = 4;              // ell tiles of 8: n_ell <= 32
+__device__ __forceinline__ void dmma_8x8x4(double (&d)[2], double a, double b) {
+  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};"
+               : "+d"(d[0]), "+d"(d[1]) : "d"(a), "d"(b));
+}
+template <int NT>
+__global__ void __launch_bounds__(LIMBER_THREADS, 3) shear_limber_kernel(const float* __restrict__ theta, int D,
                                                                          const int* __restrict__ n_rows_dev, ShearArgs A,
                                                                          const double* __restrict__ aux,
-                                                                         const double* __restrict__ pg_all, int IW,
+                                                                         const double* __restrict__ pg_all,
                                                                          double* __restrict__ model, int n_data) {
   const int b = blockIdx.x;
   if (n_rows_dev && b >= *n_rows_dev) return;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int nq = A.n_chi, nq2 = (nq + 1) & ~1, nt = A.n_tomo;
-  const int ntp = (nt + 1) & ~1, n_lb = (A.n_ell + LIMBER_LB - 1) / LIMBER_LB, nlp = n_lb * LIMBER_LB;
-  double* Wc = reinterpret_cast<double*>(smem_raw);     // two buffers of [ntp][QCP] windows + [nlp][QCP] P g
-  double* Pg = Wc + (size_t)ntp * LIMBER_QCP;
-  const int tid = threadIdx.x;
+  const int n_pairs = nt * (nt + 1) / 2;
+  const int MT = (n_pairs + 7) >> 3;                                   // 8-row MMA tiles; NT 8-column tiles (template)
+  const int MP = (MT + 1) >> 1, KS = (LIMBER_THREADS / 32) / MP;       // m-tile pairs; k-slices (warps per pair)
+  const int w_rows = nt + 1, p_rows = NT * 8;                          // + one zero row for the padding pairs
+  const size_t buf_doubles = (size_t)(w_rows + p_rows) * LIMBER_LD;
+  double* sm = reinterpret_cast<double*>(smem_raw);                    // two buffers of [w_rows + p_rows][LD]
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const float* th = theta + (size_t)b * D;
-  const double* w_b = aux + ((size_t)b * (3 + nt) + 3) * nq;
+  const double* w_b = aux + ((size_t)b * (3 + nt) + 3) * nq2;
   const double* pg_b = pg_all + (size_t)b * A.n_ell * nq2;
-  for (int i = tid; i < 2 * (ntp + nlp) * LIMBER_QCP; i += blockDim.x) Wc[i] = 0.0;   // padding rows stay zero
+  for (int i = tid; i < 2 * (int)buf_doubles; i += blockDim.x) sm[i] = 0.0;   // padding rows and columns stay zero
 
-  // this thread's tile: IW = tiles rounded up to whole warps, NS = slices of the quadrature axis
-  const int n_ib = ntp >> 1, n_items = n_ib * (n_ib + 1) / 2 * n_lb;
-  const int slice = tid / IW, item = tid - slice * IW, NS = blockDim.x / IW;
-  const bool live = item < n_items && slice < NS;
-  int ib = 0, jb = 0, lb = 0;
-  if (live) {
-    const int bp = item / n_lb;
-    lb = item - bp * n_lb;
-    int rem = bp;
-    while (rem >= n_ib - ib) { rem -= n_ib - ib; ++ib; }
-    jb = ib + rem;
+  // this warp's tiles and this lane's fragment rows
+  const int mp = warp / KS, kslice = warp - mp * KS;
+  const bool active = mp < MP;
+  const int fk = lane & 3, fr = lane >> 2;
+  int wi_off[2], wj_off[2];                                            // row offsets of W_i, W_j for the lane's two pairs
+#pragma unroll
+  for (int m = 0; m < 2; ++m) {
+    const int p = (2 * mp + m) * 8 + fr;
+    int i = nt, j = nt;                                                // the zero row
+    if (active && p < n_pairs) {
+      i = 0;
+      int rem = p;
+      while (rem >= nt - i) { rem -= nt - i; ++i; }
+      j = i + rem;
+    }
+    wi_off[m] = i * LIMBER_LD + fk;
+    wj_off[m] = j * LIMBER_LD + fk;
   }
-  const double* wi = Wc + (size_t)(2 * ib) * LIMBER_QCP;
-  const double* wj = Wc + (size_t)(2 * jb) * LIMBER_QCP;
-  const double* pg = Pg + (size_t)(lb * LIMBER_LB) * LIMBER_QCP;
-  double acc[4][LIMBER_LB];
+  const bool two = active && 2 * mp + 1 < MT;                          // the last pair of tiles may be a single tile
+  double acc[2][NT][2];
 #pragma unroll
-  for (int c = 0; c < 4; ++c)
+  for (int m = 0; m < 2; ++m)
 #pragma unroll
-    for (int u = 0; u < LIMBER_LB; ++u) acc[c][u] = 0.0;
+    for (int t = 0; t < NT; ++t) { acc[m][t][0] = 0.0; acc[m][t][1] = 0.0; }
 
-  // chunk c of the windows and of P g goes to buffer c & 1 by 8-byte asynchronous copies (the rows of `aux`
-  // start at odd element offsets), issued one chunk ahead of the arithmetic
+  // chunk c of the windows and of P g goes to buffer c & 1: one bulk asynchronous copy per row (512 bytes), issued by
+  // the lanes of warp 0 in parallel, completion on the buffer's mbarrier; one chunk ahead of the arithmetic.
+  // (`aux` and `pg` rows have even strides and a zeroed padding element, so every piece is 16-byte sized and aligned.)
   const int n_chunks = (nq + LIMBER_QC - 1) / LIMBER_QC;
-  const size_t buf_doubles = (size_t)(ntp + nlp) * LIMBER_QCP;
-  auto stage = [&](int c) {
-    const int q0 = c * LIMBER_QC, qn = min(LIMBER_QC, nq - q0);
-    double* Wb = Wc + (size_t)(c & 1) * buf_doubles;
-    double* Pb = Wb + (size_t)ntp * LIMBER_QCP;
-    for (int i = tid; i < (nt + A.n_ell) * LIMBER_QC; i += blockDim.x) {
-      const int r = i / LIMBER_QC, qq = i - r * LIMBER_QC;
-      double* dst = (r < nt ? Wb + (size_t)r * LIMBER_QCP : Pb + (size_t)(r - nt) * LIMBER_QCP) + qq;
-      if (qq < qn) {
-        const double* src = r < nt ? w_b + (size_t)r * nq + q0 + qq : pg_b + (size_t)(r - nt) * nq2 + q0 + qq;
-        asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((unsigned)__cvta_generic_to_shared(dst)), "l"(src) : "memory");
-      } else {
-        *dst = 0.0;                                      // ragged tail of the last chunk
+  const int n_rows_st = nt + A.n_ell;
+  unsigned long long* bars = reinterpret_cast<unsigned long long*>(sm + 2 * buf_doubles);   // full[2]
+  const uint32_t full0 = (uint32_t)__cvta_generic_to_shared(bars);
+  auto stage = [&](int c) {                              // all threads
+    const int q0 = c * LIMBER_QC, cnt = min(LIMBER_QC, nq2 - q0);      // even
+    double* Wb = sm + (size_t)(c & 1) * buf_doubles;
+    double* Pb = Wb + (size_t)w_rows * LIMBER_LD;
+    if (cnt < LIMBER_QC)                                 // ragged last chunk: clear what the copies do not cover
+      for (int i = tid; i < n_rows_st * (LIMBER_QC - cnt); i += blockDim.x) {
+        const int r = i / (LIMBER_QC - cnt), qq = cnt + i - r * (LIMBER_QC - cnt);
+        (r < nt ? Wb + (size_t)r * LIMBER_LD : Pb + (size_t)(r - nt) * LIMBER_LD)[qq] = 0.0;
+      }
+    if (warp == 0) {
+      const uint32_t bar = full0 + 8 * (c & 1);
+      if (lane == 0)
+        asm volatile("{\n.reg .b64 st;\nmbarrier.arrive.expect_tx.shared::cta.b64 st, [%0], %1;\n}" ::"r"(bar), "r"((uint32_t)(n_rows_st * cnt * 8)) : "memory");
+      __syncwarp();
+      for (int r = lane; r < n_rows_st; r += 32) {
+        double* dst = r < nt ? Wb + (size_t)r * LIMBER_LD : Pb + (size_t)(r - nt) * LIMBER_LD;
+        const double* src = (r < nt ? w_b + (size_t)r * nq2 : pg_b + (size_t)(r - nt) * nq2) + q0;
+        asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                     ::"r"((uint32_t)__cvta_generic_to_shared(dst)), "l"(src), "r"((uint32_t)(cnt * 8)), "r"(bar) : "memory");
       }
     }
-    asm volatile("cp.async.commit_group;" ::: "memory");
   };
-  __syncthreads();                                       // zero fill done
+  if (tid == 0) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(full0) : "memory");
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(full0 + 8) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();                                       // zero fill done, barriers initialised
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy zero fill before async-proxy writes
   stage(0);
   for (int c = 0; c < n_chunks; ++c) {
-    asm volatile("cp.async.wait_group 0;" ::: "memory"); // this thread's copies of chunk c (the only group in flight)
-    __syncthreads();                                     // everyone's copies landed; everyone is done with chunk c - 1
-    if (c + 1 < n_chunks) stage(c + 1);                  // into the buffer chunk c - 1 used; overlaps the arithmetic below
-    if (live) {
-      const size_t o = (size_t)(c & 1) * buf_doubles;
-      const double *wi_c = wi + o, *wj_c = wj + o, *pg_c = pg + o;
-#pragma unroll 2
-      for (int qq = slice; qq < LIMBER_QC; qq += NS) {
-        const double a0 = wi_c[qq], a1 = wi_c[LIMBER_QCP + qq], b0 = wj_c[qq], b1 = wj_c[LIMBER_QCP + qq];
-        const double w00 = a0 * b0, w01 = a0 * b1, w10 = a1 * b0, w11 = a1 * b1;
+    tc::mbar_wait(full0 + 8 * (c & 1), (c >> 1) & 1);     // chunk c has landed (bounded wait: traps instead of hanging)
+    __syncthreads();                                     // everyone is done with chunk c - 1: its buffer may be refilled
+    if (c + 1 < n_chunks) stage(c + 1);                  // overlaps the arithmetic below
+    if (active) {
+      const double* Wb = sm + (size_t)(c & 1) * buf_doubles;
+      const double* Pb = Wb + (size_t)w_rows * LIMBER_LD + (size_t)fr * LIMBER_LD + fk;
+      const double *wi0 = Wb + wi_off[0], *wj0 = Wb + wj_off[0], *wi1 = Wb + wi_off[1], *wj1 = Wb + wj_off[1];
+      if (two) {
+#pragma unroll 4
+        for (int q = 4 * kslice; q < LIMBER_QC; q += 4 * KS) {
+          const double a0 = wi0[q] * wj0[q], a1 = wi1[q] * wj1[q];
 #pragma unroll
-        for (int u = 0; u < LIMBER_LB; ++u) {
-          const double p = pg_c[(size_t)u * LIMBER_QCP + qq];
-          acc[0][u] = fma(w00, p, acc[0][u]); acc[1][u] = fma(w01, p, acc[1][u]);
-          acc[2][u] = fma(w10, p, acc[2][u]); acc[3][u] = fma(w11, p, acc[3][u]);
+          for (int t = 0; t < NT; ++t) {
+            const double bv = Pb[8 * t * LIMBER_LD + q];
+            dmma_8x8x4(acc[0][t], a0, bv);
+            dmma_8x8x4(acc[1][t], a1, bv);
+          }
+        }
+      } else {
+#pragma unroll 4
+        for (int q = 4 * kslice; q < LIMBER_QC; q += 4 * KS) {
+          const double a0 = wi0[q] * wj0[q];
+#pragma unroll
+          for (int t = 0; t < NT; ++t) dmma_8x8x4(acc[0][t], a0, Pb[8 * t * LIMBER_LD + q]);
         }
       }
     }
   }
-  // join the slices in a fixed order through shared memory (the chunk buffers are free now): slice s parks
-  // its sums, slice 0 adds them
-  double* red = Wc;                                      // [IW][20] <= (ntp + nlp) QCP doubles (host-checked)
-  for (int s = 1; s < NS; ++s) {
-    __syncthreads();
-    if (live && slice == s)
+  // join the k-slices in a fixed order through shared memory (the chunk buffers are free after the barrier), apply
+  // the shear-calibration factors and write the model
+  __syncthreads();
+  const int ldc = NT * 8;
+  double* red = sm;                                      // [KS][MT * 8][NT * 8]
+  if (active) {
 #pragma unroll
-      for (int c = 0; c < 4; ++c)
+    for (int m = 0; m < 2; ++m) {
+      if (m == 1 && !two) break;
+      const int row = (2 * mp + m) * 8 + fr;
 #pragma unroll
-        for (int u = 0; u < LIMBER_LB; ++u) red[(size_t)(c * LIMBER_LB + u) * IW + item] = acc[c][u];
-    __syncthreads();
-    if (live && slice == 0)
-#pragma unroll
-      for (int c = 0; c < 4; ++c)
-#pragma unroll
-        for (int u = 0; u < LIMBER_LB; ++u) acc[c][u] += red[(size_t)(c * LIMBER_LB + u) * IW + item];
-  }
-  if (!live || slice != 0) return;
-#pragma unroll
-  for (int c = 0; c < 4; ++c)
-#pragma unroll
-    for (int u = 0; u < LIMBER_LB; ++u) {
-      const int i = 2 * ib + (c >> 1), j = 2 * jb + (c & 1), bl = lb * LIMBER_LB + u;
-      if (i > j || j >= nt || bl >= A.n_ell) continue;
-      const int p = i * nt - i * (i - 1) / 2 + (j - i);
-      const double lf = A.lf[bl];
-      const float* mpi = th + A.idx_m + A.n_m_terms * i;
-      const float* mpj = th + A.idx_m + A.n_m_terms * j;
-      const double mi = (double)mpi[0] + (A.n_m_terms > 1 ? (double)mpi[1] * lf : 0.0);
-      const double mj = (double)mpj[0] + (A.n_m_terms > 1 ? (double)mpj[1] * lf : 0.0);
-      model[(size_t)b * n_data + (size_t)p * A.n_ell + bl] = (1.0 + mi) * (1.0 + mj) * acc[c][u];
+      for (int t = 0; t < NT; ++t) {
+        double* dst = red + ((size_t)kslice * MT * 8 + row) * ldc + 8 * t + 2 * fk;
+        dst[0] = acc[m][t][0]; dst[1] = acc[m][t][1];
+      }
     }
+  }
+  __syncthreads();
+  for (int o = tid; o < n_pairs * A.n_ell; o += blockDim.x) {
+    const int p = o / A.n_ell, bl = o - p * A.n_ell;
+    double v = 0.0;
+    for (int k = 0; k < KS; ++k) v += red[((size_t)k * MT * 8 + p) * ldc + bl];
+    int i = 0, rem = p;
+    while (rem >= nt - i) { rem -= nt - i; ++i; }
+    const int j = i + rem;
+    const double lf = A.lf[bl];
+    const float* mpi = th + A.idx_m + A.n_m_terms * i;
+    const float* mpj = th + A.idx_m + A.n_m_terms * j;
+    const double mi = (double)mpi[0] + (A.n_m_terms > 1 ? (double)mpi[1] * lf : 0.0);
+    const double mj = (double)mpj[0] + (A.n_m_terms > 1 ? (double)mpj[1] * lf : 0.0);
+    model[(size_t)b * n_data + o] = (1.0 + mi) * (1.0 + mj) * v;
+  }
 }
 
 // a9: model[b][r] = sum_e Bin[r][e] s_b[col_e] / A_cal^2, s = 10^y (or y) of the three emulated spectra.  One thread
@@ -772,22 +813,27 @@ nsgpu_status shear_project(nsgpu_ctx* ctx, const float* theta, int B, const int*
     const int win_threads = S.n_chi > 256 ? 256 : 128;
     while (G > 1 && ((4 + 2 * (size_t)G) * nqp * sizeof(double) > 72 * 1024 || G * S.n_chi > win_threads * WIN_ITEMS)) --G;
     const size_t smem_w = (4 + 2 * (size_t)G) * nqp * sizeof(double);
-    const int ntp = (S.n_tomo + 1) & ~1, n_lb = (S.n_ell + LIMBER_LB - 1) / LIMBER_LB;
-    const int n_items = (ntp / 2) * (ntp / 2 + 1) / 2 * n_lb;
-    if (n_items > LIMBER_THREADS || smem_w > 220 * 1024 || G * S.n_chi > win_threads * WIN_ITEMS) {
-      ctx->err = "shear: n_tomo x n_ell or n_chi too large for the streaming projection";
+    const int n_pairs = S.n_tomo * (S.n_tomo + 1) / 2, MT = (n_pairs + 7) / 8, NT = (S.n_ell + 7) / 8;
+    const int MP = (MT + 1) / 2;
+    if (MP > LIMBER_THREADS / 32 || NT > LIMBER_MAX_NT || smem_w > 220 * 1024 || G * S.n_chi > win_threads * WIN_ITEMS) {
+      ctx->err = "shear: n_tomo, n_ell (> 32) or n_chi too large for the streaming projection";
       return NSGPU_ESHAPE;
     }
-    const int IW = (n_items + 31) & ~31;                  // tiles per slice of the quadrature axis, whole warps
-    const size_t smem_l = std::max((size_t)2 * (ntp + n_lb * LIMBER_LB) * LIMBER_QCP, (size_t)IW * 4 * LIMBER_LB) * sizeof(double);
+    const int KS = (LIMBER_THREADS / 32) / MP;
+    const size_t smem_l = std::max((size_t)2 * (S.n_tomo + 1 + NT * 8) * LIMBER_LD + 2, (size_t)KS * MT * 8 * NT * 8) * sizeof(double);
     NSGPU_CUDA(nsgpu_ensure_smem(ctx, shear_windows_kernel, smem_w));
-    NSGPU_CUDA(nsgpu_ensure_smem(ctx, shear_limber_kernel, smem_l));
     shear_windows_kernel<<<B, win_threads, smem_w, st>>>(theta, ctx->D, n_rows_dev, A, G, S.aux);
     NSGPU_LAUNCH_CHECK();
     const int bpt = (((S.n_ell + 3) / 4) * S.n_chi + 255) / 256;
     shear_power_kernel<<<(unsigned)((size_t)B * bpt), 256, 0, st>>>(theta, ctx->D, n_rows_dev, ctx->spec, A, S.aux, bpt, S.pg);
     NSGPU_LAUNCH_CHECK();
-    shear_limber_kernel<<<B, LIMBER_THREADS, smem_l, st>>>(theta, ctx->D, n_rows_dev, A, S.aux, S.pg, IW, ctx->model, ctx->n_data);
+#define NSGPU_LIMBER(NT_)                                                                                              \
+  case NT_:                                                                                                           \
+    NSGPU_CUDA(nsgpu_ensure_smem(ctx, shear_limber_kernel<NT_>, smem_l));                                              \
+    shear_limber_kernel<NT_><<<B, LIMBER_THREADS, smem_l, st>>>(theta, ctx->D, n_rows_dev, A, S.aux, S.pg, ctx->model, ctx->n_data); \
+    break;
+    switch (NT) { NSGPU_LIMBER(1) NSGPU_LIMBER(2) NSGPU_LIMBER(3) NSGPU_LIMBER(4) }
+#undef NSGPU_LIMBER
     NSGPU_LAUNCH_CHECK();
     return NSGPU_OK;
   }
