@@ -176,12 +176,14 @@ __global__ void __launch_bounds__(SHEAR_THREADS, 2) shear_project_kernel(const f
   double* sc_g = scr + nqp;
   for (int q = tid; q < nq; q += blockDim.x) {
     const double a = A.a_q[q], z = A.z_q[q], opz = 1.0 + z;
-    const double E2 = Om * opz * opz * opz + (1.0 - Om) * exp_fast(de_exp * A.ln1pz[q] - 3.0 * wa * z / opz);
+    // reciprocals by rcp_fast (1e-15): an fp64 division is ~30 instructions
+    const double E2 = Om * opz * opz * opz + (1.0 - Om) * exp_fast(de_exp * A.ln1pz[q] - 3.0 * wa * z * rcp_fast(opz));
     const double E = sqrt(E2);
     Eq[q] = E;
-    const double fda = A.da / (a * a * E);
-    const double Om_a = Om / (a * a * a) / E2;
-    const double gi = exp_fast(gam * log(Om_a)) * A.da / a;
+    const double ia_ = rcp_fast(a);
+    const double fda = A.da * rcp_fast(a * a * E);
+    const double Om_a = Om * rcp_fast(a * a * a * E2);
+    const double gi = exp_fast(gam * log(Om_a)) * A.da * ia_;
     gq[q] = fda;
     hs[q] = gi;
     sc_f[q] = fda;
@@ -204,6 +206,7 @@ __global__ void __launch_bounds__(SHEAR_THREADS, 2) shear_project_kernel(const f
   // a7: n_i(z - dz_i); W^I; the two suffix sums of W^gamma = A - chi B for all bins at once
   const double inv_sig = 1.0 / A.nz_sigma;
   const double norm = inv_sig / 2.5066282746310002;              // 1/(sigma sqrt(2 pi))
+  const double wg_fac = 1.5 * Om / (C_OVER_H0 * C_OVER_H0);
   for (int it = tid; it < nt * nq; it += blockDim.x) {
     const int i = (int)__umulhi((unsigned)it, nq_magic), q = it - i * nq;
     const double mu = A.nz_mean[i] + (double)th[A.idx_dz + i];
@@ -215,7 +218,7 @@ __global__ void __launch_bounds__(SHEAR_THREADS, 2) shear_project_kernel(const f
     const double w = nz * A.da * (1.0 + z) * (1.0 + z);       // n_i(z_q) dz_q, dz = da / a^2
     scr[(size_t)(2 * i) * nqp + q] = w;
     scr[(size_t)(2 * i + 1) * nqp + q] = w * ichi[q];
-    const double x = (1.0 + z) / 1.62 - 1.0;
+    const double x = fma(1.0 + z, 1.0 / 1.62, -1.0);          // a multiply: an fp64 division is ~30 instructions
     const double Aia = A0 + A1 * x + A2 * x * x;
     Wt[(size_t)i * nq + q] = -Aia * (C1_RHOCR / C_OVER_H0) * Om * Dq[q] * nz * Eq[q];   // W^I (eq. A4); Dq holds 1/D
   }
@@ -225,7 +228,7 @@ __global__ void __launch_bounds__(SHEAR_THREADS, 2) shear_project_kernel(const f
   for (int it = tid; it < nt * nq; it += blockDim.x) {
     const int i = (int)__umulhi((unsigned)it, nq_magic), q = it - i * nq;
     const double s0 = scr[(size_t)(2 * i) * nqp + q], s1 = scr[(size_t)(2 * i + 1) * nqp + q];
-    const double wg = 1.5 * Om / (C_OVER_H0 * C_OVER_H0) * (1.0 + A.z_q[q]) * chi[q] * (s0 - chi[q] * s1);
+    const double wg = wg_fac * (1.0 + A.z_q[q]) * chi[q] * (s0 - chi[q] * s1);
     Wt[(size_t)i * nq + q] += wg;                             // + W^gamma (eq. A3)
     if (i == 0) hs[q] = log10(chi[q]);
   }
@@ -359,7 +362,7 @@ __global__ void __launch_bounds__(SHEAR_THREADS, 2) shear_project_kernel(const f
 // a6 + a7 for any n_chi: background and total windows to `aux` ([theta][(3 + n_tomo) n_chi]: g_q, log10 chi,
 // 1/chi, W_i).  The suffix scans of the shear windows run G bins at a time so that shared memory is
 // (4 + 2 G) n_chi doubles.
-constexpr int WIN_ITEMS = 16;   // (bin, node) items per thread and scan pass
+constexpr int WIN_G = 4, WIN_Q = 5;   // bins per scan pass; quadrature nodes per thread
 __global__ void __launch_bounds__(256) shear_windows_kernel(const float* __restrict__ theta, int D,
                                                             const int* __restrict__ n_rows_dev, ShearArgs A, int G,
                                                             double* __restrict__ aux) {
@@ -384,10 +387,10 @@ __global__ void __launch_bounds__(256) shear_windows_kernel(const float* __restr
   const double de_exp = 3.0 * (1.0 + w0 + wa);
   for (int q = tid; q < nq; q += blockDim.x) {
     const double a = A.a_q[q], z = A.z_q[q], opz = 1.0 + z;
-    const double E2 = Om * opz * opz * opz + (1.0 - Om) * exp_fast(de_exp * A.ln1pz[q] - 3.0 * wa * z / opz);
+    const double E2 = Om * opz * opz * opz + (1.0 - Om) * exp_fast(de_exp * A.ln1pz[q] - 3.0 * wa * z * rcp_fast(opz));
     const double E = sqrt(E2);
-    const double fda = A.da / (a * a * E);
-    const double gi = exp_fast(gam * log(Om / (a * a * a) / E2)) * A.da / a;
+    const double fda = A.da * rcp_fast(a * a * E);
+    const double gi = exp_fast(gam * log(Om * rcp_fast(a * a * a * E2))) * A.da * rcp_fast(a);
     Eq[q] = E; chi[q] = fda; iD[q] = gi;
     scr[q] = fda; scr[nqp + q] = gi;
   }
@@ -409,41 +412,56 @@ __global__ void __launch_bounds__(256) shear_windows_kernel(const float* __restr
   __syncthreads();
   const double inv_sig = 1.0 / A.nz_sigma;
   const double norm = inv_sig / 2.5066282746310002;
+  const double wg_fac = 1.5 * Om / (C_OVER_H0 * C_OVER_H0);
   double* Wt = aux_b + 3 * (size_t)nqs;
+  // A thread owns up to WIN_Q quadrature nodes (tid, tid + blockDim, ...) and walks the G bins of a pass for each:
+  // no index division, one base pointer per bin; the W^I of its (bin, node) items stay in registers across the scans,
+  // so each window is written once.
   for (int i0 = 0; i0 < nt; i0 += G) {
     const int g = min(G, nt - i0);
-    double wI[WIN_ITEMS];                                  // W^I of this thread's (bin, node) items, kept across the scans
+    double wI[WIN_G][WIN_Q];
 #pragma unroll
-    for (int s = 0; s < WIN_ITEMS; ++s) {
-      const int it = tid + s * blockDim.x;
-      wI[s] = 0.0;
-      if (it < g * nq) {
-        const int ii = it / nq, q = it - ii * nq, i = i0 + ii;
+    for (int ii = 0; ii < WIN_G; ++ii) {
+      if (ii < g) {
+        const int i = i0 + ii;
         const double mu = A.nz_mean[i] + (double)th[A.idx_dz + i];
         const float* ia = th + A.idx_ia + A.n_ia_terms * i;
         const double A0 = ia[0], A1 = A.n_ia_terms > 1 ? (double)ia[1] : 0.0, A2 = A.n_ia_terms > 2 ? (double)ia[2] : 0.0;
-        const double z = A.z_q[q];
-        const double u = (z - mu) * inv_sig;
-        const double nz = exp_fast(-0.5 * u * u) * norm;
-        const double w = nz * A.da * (1.0 + z) * (1.0 + z);
-        scr[(size_t)(2 * ii) * nqp + q] = w;
-        scr[(size_t)(2 * ii + 1) * nqp + q] = w * ichi[q];
-        const double x = (1.0 + z) / 1.62 - 1.0;
-        const double Aia = A0 + A1 * x + A2 * x * x;
-        wI[s] = -Aia * (C1_RHOCR / C_OVER_H0) * Om * iD[q] * nz * Eq[q];   // W^I (eq. A4)
+        double* s0 = scr + (size_t)(2 * ii) * nqp;
+        double* s1 = s0 + nqp;
+#pragma unroll
+        for (int s = 0; s < WIN_Q; ++s) {
+          const int q = tid + s * (int)blockDim.x;
+          wI[ii][s] = 0.0;
+          if (q < nq) {
+            const double z = A.z_q[q], opz = 1.0 + z;
+            const double u = (z - mu) * inv_sig;
+            const double nz = exp_fast(-0.5 * u * u) * norm;
+            const double w = nz * A.da * opz * opz;                    // n_i(z_q) dz_q, dz = da / a^2
+            s0[q] = w;
+            s1[q] = w * ichi[q];
+            const double x = fma(opz, 1.0 / 1.62, -1.0);               // a multiply: an fp64 division is ~30 instructions
+            const double Aia = A0 + A1 * x + A2 * x * x;
+            wI[ii][s] = -Aia * (C1_RHOCR / C_OVER_H0) * Om * iD[q] * nz * Eq[q];   // W^I (eq. A4)
+          }
+        }
       }
     }
     __syncthreads();
     for (int c = warp; c < 2 * g; c += nwarp) warp_scan_exclusive(scr + (size_t)c * nqp, nq, true, lane);
     __syncthreads();
 #pragma unroll
-    for (int s = 0; s < WIN_ITEMS; ++s) {
-      const int it = tid + s * blockDim.x;
-      if (it < g * nq) {
-        const int ii = it / nq, q = it - ii * nq, i = i0 + ii;
-        const double s0 = scr[(size_t)(2 * ii) * nqp + q], s1 = scr[(size_t)(2 * ii + 1) * nqp + q];
-        Wt[(size_t)i * nqs + q] =
-            wI[s] + 1.5 * Om / (C_OVER_H0 * C_OVER_H0) * (1.0 + A.z_q[q]) * chi[q] * (s0 - chi[q] * s1);   // + W^gamma (eq. A3)
+    for (int ii = 0; ii < WIN_G; ++ii) {
+      if (ii < g) {
+        const double* s0 = scr + (size_t)(2 * ii) * nqp;
+        const double* s1 = s0 + nqp;
+        double* wt = Wt + (size_t)(i0 + ii) * nqs;
+#pragma unroll
+        for (int s = 0; s < WIN_Q; ++s) {
+          const int q = tid + s * (int)blockDim.x;
+          if (q < nq)
+            wt[q] = wI[ii][s] + wg_fac * (1.0 + A.z_q[q]) * chi[q] * (s0[q] - chi[q] * s1[q]);   // + W^gamma (eq. A3)
+        }
       }
     }
     __syncthreads();
@@ -809,13 +827,13 @@ nsgpu_status shear_project(nsgpu_ctx* ctx, const float* theta, int B, const int*
   if (S.streaming) {
     const size_t nqp = (size_t)S.n_chi | 1;
     // bins per scan pass: as many as keep the windows kernel at three CTAs per SM
-    int G = S.n_tomo;
     const int win_threads = S.n_chi > 256 ? 256 : 128;
-    while (G > 1 && ((4 + 2 * (size_t)G) * nqp * sizeof(double) > 72 * 1024 || G * S.n_chi > win_threads * WIN_ITEMS)) --G;
+    int G = std::min(S.n_tomo, WIN_G);
+    while (G > 1 && (4 + 2 * (size_t)G) * nqp * sizeof(double) > 72 * 1024) --G;
     const size_t smem_w = (4 + 2 * (size_t)G) * nqp * sizeof(double);
     const int n_pairs = S.n_tomo * (S.n_tomo + 1) / 2, MT = (n_pairs + 7) / 8, NT = (S.n_ell + 7) / 8;
     const int MP = (MT + 1) / 2;
-    if (MP > LIMBER_THREADS / 32 || NT > LIMBER_MAX_NT || smem_w > 220 * 1024 || G * S.n_chi > win_threads * WIN_ITEMS) {
+    if (MP > LIMBER_THREADS / 32 || NT > LIMBER_MAX_NT || smem_w > 220 * 1024 || S.n_chi > win_threads * WIN_Q) {
       ctx->err = "shear: n_tomo, n_ell (> 32) or n_chi too large for the streaming projection";
       return NSGPU_ESHAPE;
     }
