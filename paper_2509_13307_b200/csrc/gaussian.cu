@@ -7,6 +7,8 @@
 // triangular product w = Linv r -- the limit of a blocked TRSM with pre-inverted diagonal blocks.
 // Residuals, products and the sum of squares are fp64 (reading P1): n(n+1)/2 MAC per theta is three
 // orders of magnitude below the emulator's work, and an fp32 whitening would eat the 1e-3 budget.
+// Two kernels: chi2_kernel streams the factor through every CTA (n_data < 512); chi2_tile_kernel is a blocked
+// triangular product on the fp64 tensor cores (larger data vectors).
 #include "internal.cuh"
 #include "tc_ptx.cuh"
 
@@ -130,6 +132,129 @@ __global__ void __launch_bounds__(MAXT) chi2_kernel(const double* __restrict__ m
       for (int w = 0; w < (RT >> 5); ++w) chi2 += part[w * TB + tid];
       double out = -0.5 * chi2 + log_norm;
       // support of the uniform priors (compared in the float32 theta arrives in) and finiteness
+      bool ok = isfinite(out);
+      for (int d = 0; d < D; ++d) {
+        const float v = theta[(size_t)b * D + d];
+        if (!isfinite(v)) ok = false;
+        if (prior_kind[d] == 0 && (v < (float)p0[d] || v > (float)p1[d])) ok = false;
+      }
+      logL[b] = ok ? out : -INFINITY;
+    }
+  }
+}
+
+// ---- the same streaming scheme on the fp64 tensor cores (n_data < 512) ---------------------------------------
+// One CTA = all rows of 8 NTL thetas; the factor is streamed in chunks of CH columns as above, but the product is
+// DMMA (m8n8k4): a warp owns the pair of 8-row tiles (w, MT-1-w) -- balanced triangular work as with the row pairs
+// -- times NTL 8-theta tiles.  Per 4 columns: 2 A fragments, NTL B fragments, up to 2 NTL DMMAs of 256 FMA.
+// Shared-memory rows are padded to a stride of 8 mod 16 doubles (fragment loads cover every bank twice); only rows
+// >= the chunk's first column are copied (one bulk copy per column, issued by parallel lanes), the rest is masked.
+__device__ __forceinline__ void dmma_8x8x4_s(double (&d)[2], double a, double b) {
+  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};"
+               : "+d"(d[0]), "+d"(d[1]) : "d"(a), "d"(b));
+}
+template <int NTL, int MAXT>
+__global__ void __launch_bounds__(MAXT) chi2_mma_kernel(const double* __restrict__ model, const double* __restrict__ data,
+                                                         const double* __restrict__ LinvT, int n, int B, int CH, int nsp,
+                                                         const int* __restrict__ n_rows_dev, const float* __restrict__ theta,
+                                                         int D, const int* __restrict__ prior_kind,
+                                                         const double* __restrict__ p0, const double* __restrict__ p1,
+                                                         double log_norm, double* __restrict__ logL) {
+  constexpr int TB = 8 * NTL, TBP = TB + 8, NBUF = 4;
+  if (n_rows_dev) B = min(B, *n_rows_dev);
+  const int b0 = blockIdx.x * TB;
+  if (b0 >= B) return;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int n4 = (n + 3) & ~3, ns = n + (n & 1);
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarp = blockDim.x >> 5;
+  double* r = reinterpret_cast<double*>(smem_raw);        // [n4][TBP] residuals, rows n .. n4-1 zero
+  double* part = r + (size_t)n4 * TBP;                    // [nwarp][TB]
+  unsigned long long* bars = reinterpret_cast<unsigned long long*>(part + (size_t)nwarp * TB);   // full[NBUF], empty[NBUF]
+  double* S = reinterpret_cast<double*>(bars + 2 * NBUF); // [NBUF][CH][nsp]
+  const uint32_t full0 = tc::smem_u32(bars), empty0 = full0 + 8 * NBUF;
+  const int n_chunks = (n + CH - 1) / CH;
+  auto load_chunk = [&](int c, int buf) {                 // whole warp 0; CH <= 32
+    const int j0 = c * CH, jn = min(CH, n - j0);
+    const uint32_t bytes = (uint32_t)(ns - j0) * 8u;      // rows j0 .. ns-1 of each column (j0, ns even)
+    if (lane == 0) tc::mbar_arrive_expect_tx(full0 + 8 * buf, bytes * jn);
+    __syncwarp();
+    if (lane < jn)
+      tc::bulk_load(tc::smem_u32(S + ((size_t)buf * CH + lane) * nsp + j0), LinvT + (size_t)(j0 + lane) * ns + j0, bytes,
+                    full0 + 8 * buf);
+  };
+  if (tid == 0) {
+    for (int b = 0; b < NBUF; ++b) { tc::mbar_init(full0 + 8 * b, 1); tc::mbar_init(empty0 + 8 * b, nwarp); }
+    tc::fence_barrier_init();
+  }
+  for (int i = tid; i < n4 * TB; i += blockDim.x) {       // residuals, transposed into [j][theta]
+    const int t = i / n4, j = i - t * n4;
+    const int b = b0 + t;
+    r[(size_t)j * TBP + t] = (b < B && j < n) ? model[(size_t)b * n + j] - data[j] : 0.0;
+  }
+  __syncthreads();
+  if (warp == 0)
+    for (int c = 0; c < NBUF - 1 && c < n_chunks; ++c) load_chunk(c, c);
+  const int MT = (n + 7) >> 3;
+  const int mtA = warp, mtB = MT - 1 - warp;              // short and long 8-row tiles of this warp
+  const bool hasB = mtB >= mtA, hasA = mtA < mtB;         // the middle tile of an odd count is B alone
+  const int fk = lane & 3, fr = lane >> 2;
+  const int rowA = 8 * mtA + fr, rowB = 8 * mtB + fr;
+  double accA[NTL][2], accB[NTL][2];
+#pragma unroll
+  for (int t = 0; t < NTL; ++t) { accA[t][0] = accA[t][1] = 0.0; accB[t][0] = accB[t][1] = 0.0; }
+  for (int c = 0; c < n_chunks; ++c) {
+    const int buf = c % NBUF;
+    if (warp == 0 && c + NBUF - 1 < n_chunks) {
+      const int cn = c + NBUF - 1, nb = cn % NBUF;
+      if (c >= 1 && lane == 0) tc::mbar_wait(empty0 + 8 * nb, ((c - 1) / NBUF) & 1);
+      __syncwarp();
+      load_chunk(cn, nb);
+    }
+    tc::mbar_wait(full0 + 8 * buf, (c / NBUF) & 1);
+    const int j0 = c * CH;
+    if (hasB && j0 <= 8 * mtB + 7) {                      // warp-uniform: the chunk reaches this warp's long tile
+      const double* Sb = S + (size_t)buf * CH * nsp;
+      const bool rowA_in = rowA >= j0, rowB_in = rowB >= j0;   // rows above the chunk's first column were not copied
+      for (int k4 = 0; k4 < CH; k4 += 4) {
+        const int jb = j0 + k4;
+        if (jb >= n || jb > 8 * mtB + 7) break;
+        const int jj = k4 + fk;
+        const bool in = j0 + jj < n;                      // columns past n in the last chunk were not copied
+        const double* rj = r + (size_t)(j0 + jj) * TBP + fr;
+        double v[NTL];
+#pragma unroll
+        for (int t = 0; t < NTL; ++t) v[t] = rj[8 * t];   // rows n .. n4-1 of r are zero
+        const double b_ = (in && rowB_in) ? Sb[(size_t)jj * nsp + rowB] : 0.0;
+#pragma unroll
+        for (int t = 0; t < NTL; ++t) dmma_8x8x4_s(accB[t], b_, v[t]);
+        if (hasA && jb <= 8 * mtA + 7) {                  // warp-uniform: the short tile ends early
+          const double a_ = (in && rowA_in) ? Sb[(size_t)jj * nsp + rowA] : 0.0;
+#pragma unroll
+          for (int t = 0; t < NTL; ++t) dmma_8x8x4_s(accA[t], a_, v[t]);
+        }
+      }
+    }
+    __syncwarp();
+    if (lane == 0) tc::mbar_arrive(empty0 + 8 * buf);
+  }
+  // sum of w^2 over this warp's rows per theta (lanes with equal fk hold the same two thetas), then over warps
+#pragma unroll
+  for (int t = 0; t < NTL; ++t)
+#pragma unroll
+    for (int e = 0; e < 2; ++e) {
+      double ss = ((hasB && rowB < n) ? accB[t][e] * accB[t][e] : 0.0) + ((hasA && rowA < n) ? accA[t][e] * accA[t][e] : 0.0);
+      ss += __shfl_xor_sync(0xffffffffu, ss, 4);
+      ss += __shfl_xor_sync(0xffffffffu, ss, 8);
+      ss += __shfl_xor_sync(0xffffffffu, ss, 16);
+      if (fr == 0) part[(size_t)warp * TB + 8 * t + 2 * fk + e] = ss;
+    }
+  __syncthreads();
+  if (tid < TB) {
+    const int b = b0 + tid;
+    if (b < B) {
+      double chi2 = 0.0;
+      for (int w = 0; w < nwarp; ++w) chi2 += part[(size_t)w * TB + tid];
+      double out = -0.5 * chi2 + log_norm;
       bool ok = isfinite(out);
       for (int d = 0; d < D; ++d) {
         const float v = theta[(size_t)b * D + d];
@@ -344,6 +469,37 @@ nsgpu_status chi2_loglike(nsgpu_ctx* ctx, const float* theta, int B, const int* 
                                                           ctx->prior_p0, ctx->prior_p1, ctx->log_norm, logL);
     NSGPU_LAUNCH_CHECK();
     return NSGPU_OK;
+  }
+  if ((ctx->flags & NSGPU_CHI2_STREAMED) == 0 && n < 512 && n >= 8) {
+    // tensor-core streaming kernel: 32 thetas per CTA, fewer when the grid would not cover the SMs
+    int ntl = 4;
+    while (ntl > 1 && (B + 8 * ntl - 1) / (8 * ntl) < ctx->sm_count / 2) ntl >>= 1;
+    const int MT = (n + 7) / 8, warps = (MT + 1) / 2, threads = 32 * warps;
+    const int ns_ = n + (n & 1), nsp = ns_ + ((8 - ns_ % 16) + 16) % 16;      // smallest stride >= ns_ that is 8 mod 16
+    const int n4 = (n + 3) & ~3, TBP = 8 * ntl + 8;
+    const size_t smem_fixed = ((size_t)n4 * TBP + (size_t)warps * 8 * ntl + 8) * sizeof(double);
+    int CH = (int)((100 * 1024 / 4) / ((size_t)nsp * 8));
+    CH = std::max(4, std::min(16, CH & ~3));
+    const size_t smem = smem_fixed + 4 * (size_t)CH * nsp * sizeof(double);
+    if (smem <= 220 * 1024) {
+      StageTimer tm(ctx, 5, st);
+      const int grid = (B + 8 * ntl - 1) / (8 * ntl);
+#define NSGPU_CHI2_MMA(NTL_, MAXT_)                                                                                   \
+  do {                                                                                                                \
+    NSGPU_CUDA(nsgpu_ensure_smem(ctx, chi2_mma_kernel<NTL_, MAXT_>, 220 * 1024));                                      \
+    chi2_mma_kernel<NTL_, MAXT_><<<grid, threads, smem, st>>>(ctx->model, ctx->data, ctx->Linv, n, B, CH, nsp, n_rows_dev, theta, \
+                                                              ctx->D, ctx->prior_kind, ctx->prior_p0, ctx->prior_p1,   \
+                                                              ctx->log_norm, logL);                                    \
+  } while (0)
+      if (threads <= 640) {
+        if (ntl == 4) NSGPU_CHI2_MMA(4, 640); else if (ntl == 2) NSGPU_CHI2_MMA(2, 640); else NSGPU_CHI2_MMA(1, 640);
+      } else {
+        if (ntl == 4) NSGPU_CHI2_MMA(4, 1024); else if (ntl == 2) NSGPU_CHI2_MMA(2, 1024); else NSGPU_CHI2_MMA(1, 1024);
+      }
+#undef NSGPU_CHI2_MMA
+      NSGPU_LAUNCH_CHECK();
+      return NSGPU_OK;
+    }
   }
   const int RT = (((n + 1) / 2 + 31) / 32) * 32;        // row-pair threads, whole warps
   if (RT > 1024) { ctx->err = "chi2: n_data > 2048 not supported"; return NSGPU_ESHAPE; }

@@ -3,7 +3,11 @@
 // shear_project : per theta, background (a6), windows (a7), z/k interpolation of the emulated
 //                 log10 P(k,z) table staged in shared memory and the extended-Limber sums reduced over
 //                 the chi-quadrature nodes with warp shuffles (a5, a8)  [P:L330-353 eqs. A1-A4; P:L359]
+// shear_windows, shear_power, shear_limber : the same for grids that do not fit shared memory (the paper's
+//                 1025 nodes x 10 bins): windows with the bins scanned in groups, lookups against the table in
+//                 place, Limber product on the fp64 tensor cores over chunks of the quadrature axis
 // cmb_bin       : 10^y / linear, / A_cal^2, CSR binning (a9)            [BJ cfg 1; readings C1-C3]
+// cmb_tt        : the paper's cosmic-variance TT likelihood
 // copy_model    : identity / emulator-only theories (BJ cfg 0)
 //
 // HBM-bound stages: the only large read is the spectrum table written by the emulator (84 KB per
@@ -80,6 +84,12 @@ __device__ void warp_scan_exclusive(double* arr, int n, bool reverse, int lane) 
     arr[idx] = run;
     run += v;
   }
+}
+
+// D (8x8) += A (8x4, row-major) . B (4x8, column-major) on the fp64 tensor cores
+__device__ __forceinline__ void dmma_8x8x4(double (&d)[2], double a, double b) {
+  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};"
+               : "+d"(d[0]), "+d"(d[1]) : "d"(a), "d"(b));
 }
 
 struct ShearArgs {
@@ -307,10 +317,91 @@ __global__ void __launch_bounds__(SHEAR_THREADS, 2) shear_project_kernel(const f
   }
   __syncthreads();
 
+  // a8 (sum): C_ij(ell) = sum_q Wt_i Wt_j Pg is a [pairs][q] x [q][ell] product: fp64 tensor cores (mma.m8n8k4.f64;
+  // fragments: lane l holds A[l >> 2][l & 3], B[l & 3][l >> 2], D[l >> 2][2 (l & 3) + {0, 1}]).  A warp owns two
+  // 8-pair tiles x all 8-ell tiles and every KS-th 4-node k-step; the A element W_i W_j is formed on the fly by
+  // the lane that needs it.  The k-slices are joined through shared memory in a fixed order.  Falls back to the scalar loop below for more than 32 multipoles.
+  const int n_pairs = nt * (nt + 1) / 2;
+  const int MT = (n_pairs + 7) >> 3, NT = (A.n_ell + 7) >> 3;
+  const int MP = (MT + 1) >> 1;
+  if (NT <= 4 && MP <= nwarp && (size_t)(nwarp / MP) * MT * 8 * NT * 8 <= n_dbl + (size_t)A.n_z_emu * A.n_k / 2) {
+    const int KS = nwarp / MP, mp = warp / KS, kslice = warp - mp * KS;
+    const bool active = mp < MP;
+    const int fk = lane & 3, fr = lane >> 2;
+    const double *wi[2], *wj[2];
+    bool row_ok[2];
+#pragma unroll
+    for (int m = 0; m < 2; ++m) {
+      const int p = (2 * mp + m) * 8 + fr;
+      int i = 0, j = 0;
+      row_ok[m] = active && p < n_pairs;
+      if (row_ok[m]) {
+        int rem = p;
+        while (rem >= nt - i) { rem -= nt - i; ++i; }
+        j = i + rem;
+      }
+      wi[m] = Wt + (size_t)i * nq;
+      wj[m] = Wt + (size_t)j * nq;
+    }
+    const bool two = active && 2 * mp + 1 < MT;
+    double acc[2][4][2];
+#pragma unroll
+    for (int m = 0; m < 2; ++m)
+#pragma unroll
+      for (int t = 0; t < 4; ++t) { acc[m][t][0] = 0.0; acc[m][t][1] = 0.0; }
+    if (active) {
+      for (int q0 = 4 * kslice; q0 < nq; q0 += 4 * KS) {
+        const int q = q0 + fk;
+        const bool in = q < nq;                                // ragged last k-step
+        const double a0 = (in && row_ok[0]) ? wi[0][q] * wj[0][q] : 0.0;
+        const double a1 = (in && row_ok[1]) ? wi[1][q] * wj[1][q] : 0.0;
+#pragma unroll
+        for (int t = 0; t < 4; ++t) {
+          if (t < NT) {
+            const int bl = 8 * t + fr;
+            const double bv = (in && bl < A.n_ell) ? Pg[(size_t)bl * nqp + q] : 0.0;
+            dmma_8x8x4(acc[0][t], a0, bv);
+            if (two) dmma_8x8x4(acc[1][t], a1, bv);
+          }
+        }
+      }
+    }
+    __syncthreads();                                           // every warp is done with Wt and Pg: reuse the CTA's shared memory
+    double* red = chi;                                         // [KS][MT * 8][NT * 8]
+    const int ldc = NT * 8;
+    if (active) {
+#pragma unroll
+      for (int m = 0; m < 2; ++m) {
+        if (m == 1 && !two) break;
+        const int row = (2 * mp + m) * 8 + fr;
+#pragma unroll
+        for (int t = 0; t < 4; ++t)
+          if (t < NT) {
+            double* dst = red + ((size_t)kslice * MT * 8 + row) * ldc + 8 * t + 2 * fk;
+            dst[0] = acc[m][t][0]; dst[1] = acc[m][t][1];
+          }
+      }
+    }
+    __syncthreads();
+    for (int o = tid; o < n_pairs * A.n_ell; o += blockDim.x) {
+      const int p = o / A.n_ell, bl = o - p * A.n_ell;
+      double v = 0.0;
+      for (int k = 0; k < KS; ++k) v += red[((size_t)k * MT * 8 + p) * ldc + bl];
+      int i = 0, rem = p;
+      while (rem >= nt - i) { rem -= nt - i; ++i; }
+      const int j = i + rem;
+      const double lf = A.lf[bl];                              // ln(ell/550)/ln 30
+      const float* mpi = th + A.idx_m + A.n_m_terms * i;
+      const float* mpj = th + A.idx_m + A.n_m_terms * j;
+      const double mi = (double)mpi[0] + (A.n_m_terms > 1 ? (double)mpi[1] * lf : 0.0);
+      const double mj = (double)mpj[0] + (A.n_m_terms > 1 ? (double)mpj[1] * lf : 0.0);
+      model[(size_t)b * n_data + o] = (1.0 + mi) * (1.0 + mj) * v;
+    }
+    return;
+  }
   // a8 (sum): C_ij(ell) = sum_q Wt_i Wt_j Pg.  Work item = (pair, group of 4 ell); 4 adjacent lanes share
   // an item and split the q range, so the window product is formed once per 4 outputs; a 2-step shuffle
   // reduction joins the four partial sums.
-  const int n_pairs = nt * (nt + 1) / 2;
   const int n_lg = (A.n_ell + 3) >> 2, n_items = n_pairs * n_lg;
   const int part = tid & 3;
   for (int item0 = 0; item0 < n_items; item0 += blockDim.x >> 2) {
@@ -559,10 +650,6 @@ constexpr int LIMBER_THREADS = 256;
 constexpr int LIMBER_QC = 64;                 // quadrature nodes per chunk
 constexpr int LIMBER_LD = LIMBER_QC + 4;      // row stride of the staged chunks
 constexpr int LIMBER_MAX_NT = 4;              // ell tiles of 8: n_ell <= 32
-__device__ __forceinline__ void dmma_8x8x4(double (&d)[2], double a, double b) {
-  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};"
-               : "+d"(d[0]), "+d"(d[1]) : "d"(a), "d"(b));
-}
 template <int NT>
 __global__ void __launch_bounds__(LIMBER_THREADS, 3) shear_limber_kernel(const float* __restrict__ theta, int D,
                                                                          const int* __restrict__ n_rows_dev, ShearArgs A,
