@@ -153,14 +153,14 @@ __device__ __forceinline__ void dmma_8x8x4_s(double (&d)[2], double a, double b)
   asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};"
                : "+d"(d[0]), "+d"(d[1]) : "d"(a), "d"(b));
 }
-template <int NTL, int MAXT>
+template <int NTL, int MAXT, int NBUF>
 __global__ void __launch_bounds__(MAXT) chi2_mma_kernel(const double* __restrict__ model, const double* __restrict__ data,
                                                          const double* __restrict__ LinvT, int n, int B, int CH, int nsp,
                                                          const int* __restrict__ n_rows_dev, const float* __restrict__ theta,
                                                          int D, const int* __restrict__ prior_kind,
                                                          const double* __restrict__ p0, const double* __restrict__ p1,
                                                          double log_norm, double* __restrict__ logL) {
-  constexpr int TB = 8 * NTL, TBP = TB + 8, NBUF = 4;
+  constexpr int TB = 8 * NTL, TBP = TB + 8;               // NBUF chunks of the factor in flight
   if (n_rows_dev) B = min(B, *n_rows_dev);
   const int b0 = blockIdx.x * TB;
   if (b0 >= B) return;
@@ -480,22 +480,30 @@ nsgpu_status chi2_loglike(nsgpu_ctx* ctx, const float* theta, int B, const int* 
     const size_t smem_fixed = ((size_t)n4 * TBP + (size_t)warps * 8 * ntl + 8) * sizeof(double);
     int CH = (int)((100 * 1024 / 4) / ((size_t)nsp * 8));
     CH = std::max(4, std::min(16, CH & ~3));
-    const size_t smem = smem_fixed + 4 * (size_t)CH * nsp * sizeof(double);
+    // small batches are bound by the latency of the chunk ring, not by arithmetic: eight chunks in flight when
+    // the (then small) residual block leaves room
+    const int nbuf = (ntl <= 2 && smem_fixed + 8 * (size_t)CH * nsp * sizeof(double) <= 200 * 1024) ? 8 : 4;
+    const size_t smem = smem_fixed + (size_t)nbuf * CH * nsp * sizeof(double);
     if (smem <= 220 * 1024) {
       StageTimer tm(ctx, 5, st);
       const int grid = (B + 8 * ntl - 1) / (8 * ntl);
-#define NSGPU_CHI2_MMA(NTL_, MAXT_)                                                                                   \
+#define NSGPU_CHI2_MMA(NTL_, MAXT_, NBUF_)                                                                            \
   do {                                                                                                                \
-    NSGPU_CUDA(nsgpu_ensure_smem(ctx, chi2_mma_kernel<NTL_, MAXT_>, 220 * 1024));                                      \
-    chi2_mma_kernel<NTL_, MAXT_><<<grid, threads, smem, st>>>(ctx->model, ctx->data, ctx->Linv, n, B, CH, nsp, n_rows_dev, theta, \
-                                                              ctx->D, ctx->prior_kind, ctx->prior_p0, ctx->prior_p1,   \
-                                                              ctx->log_norm, logL);                                    \
+    NSGPU_CUDA(nsgpu_ensure_smem(ctx, chi2_mma_kernel<NTL_, MAXT_, NBUF_>, 220 * 1024));                               \
+    chi2_mma_kernel<NTL_, MAXT_, NBUF_><<<grid, threads, smem, st>>>(ctx->model, ctx->data, ctx->Linv, n, B, CH, nsp, n_rows_dev, \
+                                                                     theta, ctx->D, ctx->prior_kind, ctx->prior_p0,   \
+                                                                     ctx->prior_p1, ctx->log_norm, logL);             \
   } while (0)
-      if (threads <= 640) {
-        if (ntl == 4) NSGPU_CHI2_MMA(4, 640); else if (ntl == 2) NSGPU_CHI2_MMA(2, 640); else NSGPU_CHI2_MMA(1, 640);
-      } else {
-        if (ntl == 4) NSGPU_CHI2_MMA(4, 1024); else if (ntl == 2) NSGPU_CHI2_MMA(2, 1024); else NSGPU_CHI2_MMA(1, 1024);
-      }
+#define NSGPU_CHI2_MMA_T(MAXT_)                                                                                       \
+  do {                                                                                                                \
+    if (ntl == 4) NSGPU_CHI2_MMA(4, MAXT_, 4);                                                                         \
+    else if (ntl == 2 && nbuf == 8) NSGPU_CHI2_MMA(2, MAXT_, 8);                                                       \
+    else if (ntl == 2) NSGPU_CHI2_MMA(2, MAXT_, 4);                                                                    \
+    else if (nbuf == 8) NSGPU_CHI2_MMA(1, MAXT_, 8);                                                                   \
+    else NSGPU_CHI2_MMA(1, MAXT_, 4);                                                                                  \
+  } while (0)
+      if (threads <= 640) NSGPU_CHI2_MMA_T(640); else NSGPU_CHI2_MMA_T(1024);
+#undef NSGPU_CHI2_MMA_T
 #undef NSGPU_CHI2_MMA
       NSGPU_LAUNCH_CHECK();
       return NSGPU_OK;
