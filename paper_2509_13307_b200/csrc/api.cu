@@ -327,7 +327,10 @@ nsgpu_status create_impl(nsgpu_ctx* ctx, int32_t D, const nsgpu_prior1d* prior, 
     }
     // stored transposed: LinvT[j][i] = Linv[i][j] (non-zero for i >= j), so that for a fixed column j the
     // rows i are contiguous -- coalesced for the row-per-thread chi^2 kernel
-    const size_t ns = n + (n & 1);               // even row stride: every 16-byte unit of a row starts at an even column
+    // row stride: smallest >= n that is 8 mod 16 doubles -- 16-byte aligned pieces for the bulk copies, and a
+    // tensor-core fragment load (4 columns x 8 rows) from a tile with this stride covers every bank exactly twice
+    const size_t ns = n + ((8 + 16 - n % 16) % 16);
+    ctx->linv_ld = (int)ns;
     std::vector<double> LinvT(n * ns, 0.0);
     for (size_t i = 0; i < n; ++i)
       for (size_t j = 0; j <= i; ++j) LinvT[j * ns + i] = Linv[i * n + j];

@@ -75,6 +75,7 @@ struct nsgpu_ctx {
   // gaussian
   double* data = nullptr;       // [n_data]
   double* Linv = nullptr;       // [n_data][n_data] TRANSPOSE of the inverse Cholesky factor: LinvT[j][i], fp64
+  int linv_ld = 0;              // row stride of Linv (doubles): >= n_data, 8 mod 16
   double log_norm = 0.0;
   double *tt_a = nullptr, *tt_b = nullptr, *tt_mu = nullptr;   // kind 4: (nu/2) ln 10 and nu Chat / 2 per multipole
   // workspaces
