@@ -414,18 +414,28 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) mlp_gemm_tc(const __grid_cons
         tc::mbar_wait(pfull0 + 8 * pb, pphase);
         tc::fence_after_sync();
         const uint32_t t_src = tmem_base + pb * PB_COLS + ((uint32_t)(q * 32) << 16) + hcol * CPT;
+        // Two tcgen05.ld in flight per wait: the drain of a partial is a chain of load round trips on the tile's
+        // critical path (one load per wait: hidden GEMMs 6% slower); four would not leave registers for the deferral.
+        constexpr int NLD = CPT / LDC, DB = 2;
 #pragma unroll
-        for (int c = 0; c < CPT / LDC; ++c) {
-          uint32_t r[LDC];
-          tc::tmem_ld_cols(t_src + LDC * c, r);
+        for (int c0 = 0; c0 < NLD; c0 += DB) {
+          uint32_t r[DB][LDC];
+#pragma unroll
+          for (int b = 0; b < DB; ++b)
+            if (c0 + b < NLD) tc::tmem_ld_cols(t_src + LDC * (c0 + b), r[b]);
           tc::tmem_ld_wait();
-          if (kb == 0) {
 #pragma unroll
-            for (int j = 0; j < LDC / 2; ++j) acc[(LDC / 2) * c + j] = pk2(__uint_as_float(r[2 * j]), __uint_as_float(r[2 * j + 1]));
-          } else {
+          for (int b = 0; b < DB; ++b) {
+            if (c0 + b >= NLD) continue;
+            const int c = c0 + b;
+            if (kb == 0) {
 #pragma unroll
-            for (int j = 0; j < LDC / 2; ++j)
-              acc[(LDC / 2) * c + j] = add2(acc[(LDC / 2) * c + j], pk2(__uint_as_float(r[2 * j]), __uint_as_float(r[2 * j + 1])));
+              for (int j = 0; j < LDC / 2; ++j) acc[(LDC / 2) * c + j] = pk2(__uint_as_float(r[b][2 * j]), __uint_as_float(r[b][2 * j + 1]));
+            } else {
+#pragma unroll
+              for (int j = 0; j < LDC / 2; ++j)
+                acc[(LDC / 2) * c + j] = add2(acc[(LDC / 2) * c + j], pk2(__uint_as_float(r[b][2 * j]), __uint_as_float(r[b][2 * j + 1])));
+            }
           }
         }
         tc::fence_before_sync();
