@@ -124,6 +124,8 @@ typedef struct {
 #define NSGPU_MLP_TC 2u     /* require the tcgen05 path (NSGPU_ESHAPE if width % 64 != 0) */
 #define NSGPU_CHI2_STREAMED 8u /* chi^2 by the factor-streaming kernel (one CTA = all rows of 8..32 thetas) whatever n_data */
 #define NSGPU_CHI2_TILED 16u   /* chi^2 by the tiled kernels (128-row blocks x 32..64 thetas) whatever n_data; default: n_data >= 512 */
+#define NSGPU_MLP_CLUSTER 32u    /* tcgen05 GEMMs: CTA pairs that multicast the weight tiles, whatever the batch (default: large batches) */
+#define NSGPU_MLP_NO_CLUSTER 64u /* ... never */
 #define NSGPU_SHEAR_STREAM 4u /* kind 3: use the streaming projection kernels even where the grids fit shared memory */
 
 /* Create a context on CUDA device `device`.

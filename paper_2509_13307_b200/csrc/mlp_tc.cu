@@ -214,10 +214,11 @@ __device__ __forceinline__ void epi_pairs(const f32x2* a, const TileRef& t, cons
       uint32_t hi[4], lo[4];
 #pragma unroll
       for (int j = 0; j < 4; ++j) act_split_pair(a[4 * c + j], cs2, p[8 * c + 2 * j], p[8 * c + 2 * j + 1], hi[j], lo[j]);
-      if (t.row_ok) {
-        *reinterpret_cast<uint4*>(dh + (size_t)c * PIECE_HALVES) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
-        *reinterpret_cast<uint4*>(dl + (size_t)c * PIECE_HALVES) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
-      }
+      // No row test: the planes are allocated in whole 128-row tiles, so the rows past M of the last tile are
+      // stored too (finite values nobody reads).  A test here makes every 8-column piece a basic block of its own
+      // and the MUFU / conversion chains of different pieces can no longer be interleaved.
+      *reinterpret_cast<uint4*>(dh + (size_t)c * PIECE_HALVES) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
+      *reinterpret_cast<uint4*>(dl + (size_t)c * PIECE_HALVES) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
     }
   } else {
     const float4* p4 = g.p_out4 + (n0 >> 1);                       // warp-uniform addresses: L1 broadcast
@@ -276,7 +277,16 @@ __device__ __forceinline__ void epi_pairs(const f32x2* a, const TileRef& t, cons
 constexpr int EPI_WARPS = 8;                         // 2 per TMEM lane quarter, each half of the tile's columns
 constexpr int GEMM_THREADS = 384;                    // warpgroups 0-1 epilogue; warpgroup 2: TMA producer, MMA issuer, 2 idle
 constexpr int DEFER_PAIRS = 32;                      // 64 columns of a finished tile wait in registers (see below)
-template <int BLOCK_N, int EPI>
+//
+// Weight multicast (CS > 1): with one CTA per SM and 96 KB of operands per k-block, a hidden layer pulls
+// 768 KB per tile from L2 -- 44 B/clk/SM at the measured tile time, which IS the chip's L2 -> SM throughput
+// (~6300 B/clk over 148 SMs), and two thirds of it are weight tiles that every CTA working on the same column
+// block reads again.  So CS CTAs of a thread-block cluster take CS consecutive row blocks of the SAME column
+// block in lock step; each loads 1/CS of the W_hi / W_lo tile and multicasts it into the shared memory of all
+// of them (96 -> 64 KB of L2 reads per CTA and k-block for CS = 2).  A stage may be refilled
+// only when every CTA of the cluster has consumed it: the MMA commit that frees it is multicast as well and the
+// `empty` barriers count CS arrivals.  The MMA / TMEM / epilogue side is unchanged.
+template <int BLOCK_N, int EPI, int CS = 1>
 __global__ void __launch_bounds__(GEMM_THREADS, 1) mlp_gemm_tc(const __grid_constant__ CUtensorMap tm_whi,
                                                                const __grid_constant__ CUtensorMap tm_wlo, GemmArgs g) {
   constexpr int STAGES = num_stages(BLOCK_N);
@@ -302,11 +312,18 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) mlp_gemm_tc(const __grid_cons
   int M = g.M_host;
   if (g.n_rows_dev) M = min(M, (*g.n_rows_dev) * g.rows_per_theta);
   const int n_blocks = g.N_pad / BLOCK_N;
-  const int num_tiles = ((M + BLOCK_M - 1) / BLOCK_M) * n_blocks;
+  const int m_blocks = (M + BLOCK_M - 1) / BLOCK_M;
+  // work items: (group of CS row blocks, column block); CTA `crank` of a cluster takes row block CS grp + crank
+  // (clamped: the spare CTA of a ragged last group repeats the last row block and stores the same values)
+  const int crank = CS > 1 ? (int)tc::cluster_ctarank() : 0;
+  const int num_tiles = ((m_blocks + CS - 1) / CS) * n_blocks;
+  const int tile0 = blockIdx.x / CS, tile_step = gridDim.x / CS;
+  constexpr uint16_t CMASK = (uint16_t)((1u << CS) - 1u);
+  constexpr int W_SUB_BYTES = B_TILE_BYTES / CS;                 // this CTA's share of a weight tile
   const int k_blocks = g.K / BLOCK_K;
 
   if (threadIdx.x == 0) {
-    for (int s = 0; s < STAGES; ++s) { tc::mbar_init(full0 + 8 * s, 1); tc::mbar_init(empty0 + 8 * s, 1); }
+    for (int s = 0; s < STAGES; ++s) { tc::mbar_init(full0 + 8 * s, 1); tc::mbar_init(empty0 + 8 * s, CS); }
     for (int b = 0; b < NPB; ++b) { tc::mbar_init(pfull0 + 8 * b, 1); tc::mbar_init(pempty0 + 8 * b, EPI_WARPS); }
     tc::fence_barrier_init();
   }
@@ -321,6 +338,7 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) mlp_gemm_tc(const __grid_cons
   }
   tc::fence_before_sync();
   __syncthreads();
+  if (CS > 1) tc::cluster_sync();        // every CTA's barriers exist before a peer's multicast or commit reaches them
   tc::fence_after_sync();
   const uint32_t tmem_base = *tmem_slot;
   // registers: 384 x 168 at launch -> 232 for the epilogue warpgroups (accumulators + deferred columns), 40 for the rest
@@ -330,8 +348,9 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) mlp_gemm_tc(const __grid_cons
     // ===== TMA producer =====
     if (lane == 0) {
       uint32_t stage = 0, phase = 0;
-      for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
-        const int m_blk = tile / n_blocks, n_blk = tile - m_blk * n_blocks;
+      for (int tile = tile0; tile < num_tiles; tile += tile_step) {
+        const int m_grp = tile / n_blocks, n_blk = tile - m_grp * n_blocks;
+        const int m_blk = min(m_grp * CS + crank, m_blocks - 1);
         // this tile's A rows: k-block kb is the 16 KB starting at piece 8 kb
         const size_t a_tile = (size_t)m_blk * ((size_t)BLOCK_M * g.K);
         for (int kb = 0; kb < k_blocks; ++kb) {
@@ -341,8 +360,14 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) mlp_gemm_tc(const __grid_cons
           const size_t a_off = a_tile + (size_t)kb * 8 * PIECE_HALVES;
           tc::bulk_load(s0, g.a_hi + a_off, A_TILE_BYTES, fb);
           tc::bulk_load(s0 + A_TILE_BYTES, g.a_lo + a_off, A_TILE_BYTES, fb);
-          tc::tma_load_2d(s0 + 2 * A_TILE_BYTES, &tm_whi, kb * BLOCK_K, n_blk * BLOCK_N, fb);
-          tc::tma_load_2d(s0 + 2 * A_TILE_BYTES + B_TILE_BYTES, &tm_wlo, kb * BLOCK_K, n_blk * BLOCK_N, fb);
+          if (CS == 1) {
+            tc::tma_load_2d(s0 + 2 * A_TILE_BYTES, &tm_whi, kb * BLOCK_K, n_blk * BLOCK_N, fb);
+            tc::tma_load_2d(s0 + 2 * A_TILE_BYTES + B_TILE_BYTES, &tm_wlo, kb * BLOCK_K, n_blk * BLOCK_N, fb);
+          } else {   // tensor maps with boxes of BLOCK_N / CS rows
+            const int wrow = n_blk * BLOCK_N + crank * (BLOCK_N / CS);
+            tc::tma_load_2d_mc(s0 + 2 * A_TILE_BYTES + crank * W_SUB_BYTES, &tm_whi, kb * BLOCK_K, wrow, fb, CMASK);
+            tc::tma_load_2d_mc(s0 + 2 * A_TILE_BYTES + B_TILE_BYTES + crank * W_SUB_BYTES, &tm_wlo, kb * BLOCK_K, wrow, fb, CMASK);
+          }
           if (++stage == STAGES) { stage = 0; phase ^= 1; }
         }
       }
@@ -351,7 +376,7 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) mlp_gemm_tc(const __grid_cons
     // ===== MMA issuer (one thread): one fresh TMEM partial per k-block =====
     if (lane == 0) {
       uint32_t stage = 0, phase = 0, pcount = 0;
-      for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
+      for (int tile = tile0; tile < num_tiles; tile += tile_step) {
         for (int kb = 0; kb < k_blocks; ++kb, ++pcount) {
           const uint32_t pb = pcount % NPB, pphase = (pcount / NPB) & 1;
           tc::mbar_wait(pempty0 + 8 * pb, pphase ^ 1);          // the epilogue has pulled this partial
@@ -377,7 +402,8 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) mlp_gemm_tc(const __grid_cons
             const uint64_t adv_a = (uint64_t)(256 * k), adv_b = (uint64_t)(2 * k);
             tc::mma_f16_ss(d_tmem, a_hi + adv_a, b_hi + adv_b, IDESC, 1);
           }
-          tc::mma_commit(empty0 + 8 * stage);                   // smem slot free when these MMAs retire
+          if (CS == 1) tc::mma_commit(empty0 + 8 * stage);      // smem slot free when these MMAs retire
+          else tc::mma_commit_mc(empty0 + 8 * stage, CMASK);    // ... in every CTA that multicasts into it
           tc::mma_commit(pfull0 + 8 * pb);                      // partial complete
           if (++stage == STAGES) { stage = 0; phase ^= 1; }
         }
@@ -406,8 +432,9 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) mlp_gemm_tc(const __grid_cons
     const int c_ = (c);                                                             \
     NSGPU_CHUNK_CASE(0); NSGPU_CHUNK_CASE(1); NSGPU_CHUNK_CASE(2); NSGPU_CHUNK_CASE(3); NSGPU_CHUNK_CASE(4); NSGPU_CHUNK_CASE(5); \
   } while (0)
-    for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
-      const int m_blk = tile / n_blocks, n_blk = tile - m_blk * n_blocks;
+    for (int tile = tile0; tile < num_tiles; tile += tile_step) {
+      const int m_grp = tile / n_blocks, n_blk = tile - m_grp * n_blocks;
+      const int m_blk = min(m_grp * CS + crank, m_blocks - 1);
       f32x2 acc[NPAIR];
       for (int kb = 0; kb < k_blocks; ++kb, ++pcount) {
         const uint32_t pb = pcount % NPB, pphase = (pcount / NPB) & 1;
@@ -460,6 +487,7 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) mlp_gemm_tc(const __grid_cons
   }
   tc::fence_before_sync();
   __syncthreads();
+  if (CS > 1) tc::cluster_sync();        // no CTA leaves while a peer can still write into its shared memory
   if (warp == EPI_WARPS + 1) tc::tmem_dealloc(tmem_base, 512);
 }
 
@@ -479,6 +507,8 @@ struct TcLayer {
   CUtensorMap tm_whi, tm_wlo;                // box = block_n rows
   CUtensorMap tm_whi_s[2], tm_wlo_s[2];      // hidden layers: boxes of 128 and 64 rows for small batches
   bool has_s[2] = {false, false};
+  CUtensorMap tm_whi_c, tm_wlo_c;            // boxes of block_n / 2 rows: one CTA's multicast share of a tile
+  bool has_c = false;
 };
 
 struct TcState {
@@ -538,10 +568,35 @@ nsgpu_status launch_gemm(nsgpu_ctx* ctx, const CUtensorMap& whi, const CUtensorM
   return NSGPU_OK;
 }
 
+// Clusters of CS CTAs that share the weight tiles (whi / wlo: tensor maps with boxes of BN / CS rows).
+template <int BN, int EPI, int CS>
+nsgpu_status launch_gemm_cluster(nsgpu_ctx* ctx, const CUtensorMap& whi, const CUtensorMap& wlo, const GemmArgs& g,
+                                 cudaStream_t st) {
+  const int smem = num_stages(BN) * stage_bytes(BN) + 16 * num_stages(BN) + 128 + (EPI == 0 ? 16 * g.N_pad : 0) + 1024;
+  NSGPU_CUDA(nsgpu_ensure_smem(ctx, mlp_gemm_tc<BN, EPI, CS>, SMEM_BUDGET));
+  const int m_blocks = (g.M_host + BLOCK_M - 1) / BLOCK_M;
+  const int items = ((m_blocks + CS - 1) / CS) * (g.N_pad / BN);
+  const int clusters = std::min(items, ctx->sm_count / CS);
+  cudaLaunchConfig_t cfg;
+  memset(&cfg, 0, sizeof(cfg));
+  cfg.gridDim = dim3(clusters * CS);
+  cfg.blockDim = dim3(GEMM_THREADS);
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeClusterDimension;
+  attr[0].val.clusterDim.x = CS; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  NSGPU_CUDA(cudaLaunchKernelEx(&cfg, mlp_gemm_tc<BN, EPI, CS>, whi, wlo, g));
+  NSGPU_LAUNCH_CHECK();
+  return NSGPU_OK;
+}
+
 template <int EPI>
 nsgpu_status dispatch_gemm(nsgpu_ctx* ctx, const TcLayer& L, const GemmArgs& g, cudaStream_t st) {
   // Small batches (few 128-row blocks): narrower tiles so that the grid still covers the SMs.
-  if (EPI == 0) {
+  if (EPI == 0 && (ctx->flags & NSGPU_MLP_CLUSTER) == 0) {
     const int m_blocks = (g.M_host + BLOCK_M - 1) / BLOCK_M;
     int bn = L.block_n;
     while (bn > 64 && m_blocks * (g.N_pad / bn) < ctx->sm_count && L.has_s[bn == 256 ? 0 : 1]) bn >>= 1;
@@ -550,6 +605,16 @@ nsgpu_status dispatch_gemm(nsgpu_ctx* ctx, const TcLayer& L, const GemmArgs& g, 
       return bn == 128 ? launch_gemm<128, EPI>(ctx, L.tm_whi_s[i], L.tm_wlo_s[i], g, st)
                        : launch_gemm<64, EPI>(ctx, L.tm_whi_s[i], L.tm_wlo_s[i], g, st);
     }
+  }
+  // Large batches: CTA pairs share the weight tiles (see mlp_gemm_tc).  Clusters of 4 were measured 50% slower than
+  // pairs (the lock step of four CTAs costs more than the L2 reads it saves).
+  if (L.has_c && (L.block_n == 256 || L.block_n == 224)) {
+    const int m_blocks_all = (g.M_host + BLOCK_M - 1) / BLOCK_M;
+    bool pair = m_blocks_all * (g.N_pad / L.block_n) >= 2 * ctx->sm_count;
+    if (ctx->flags & NSGPU_MLP_NO_CLUSTER) pair = false;
+    if (ctx->flags & NSGPU_MLP_CLUSTER) pair = true;
+    if (pair) return L.block_n == 256 ? launch_gemm_cluster<256, EPI, 2>(ctx, L.tm_whi_c, L.tm_wlo_c, g, st)
+                                      : launch_gemm_cluster<224, EPI, 2>(ctx, L.tm_whi_c, L.tm_wlo_c, g, st);
   }
   switch (L.block_n) {
     case 256: return launch_gemm<256, EPI>(ctx, L.tm_whi, L.tm_wlo, g, st);
@@ -603,6 +668,8 @@ nsgpu_status mlp_tc_prepare(nsgpu_ctx* ctx, int e, const nsgpu_emulator* h) {
         ctx->err = "cuTensorMapEncodeTiled failed for a weight plane";
         return NSGPU_ECUDA;
       }
+      if (L.block_n == 256 || L.block_n == 224)     // multicast shares: boxes of block_n / 2 rows
+        L.has_c = make_tmap(&L.tm_whi_c, L.Whi, L.N_pad, L.K, L.block_n / 2) && make_tmap(&L.tm_wlo_c, L.Wlo, L.N_pad, L.K, L.block_n / 2);
       if (hidden) {   // narrower boxes over the same planes (N_pad = width is a multiple of 64)
         const int bs[2] = {128, 64};
         for (int i = 0; i < 2; ++i)

@@ -19,6 +19,7 @@ STATUS_NAMES = {0: "NSGPU_OK", -1: "NSGPU_EINVAL", -2: "NSGPU_ENOMEM", -3: "NSGP
                 -4: "NSGPU_ESHAPE", -5: "NSGPU_ENOTSPD", -6: "NSGPU_ENOCONV"}
 MLP_AUTO, MLP_SIMT, MLP_TC = 0, 1, 2
 CHI2_STREAMED, CHI2_TILED = 8, 16   # OR into `mlp`: force one of the two chi^2 kernels (default: tiled for n_data >= 512)
+MLP_CLUSTER, MLP_NO_CLUSTER = 32, 64   # OR into `mlp`: weight-multicast CTA pairs always / never (default: large batches)
 SHEAR_STREAM = 4          # OR into `mlp`: streaming projection kernels even for grids that fit shared memory
 
 EXPORTS = ["nsgpu_create", "nsgpu_destroy", "nsgpu_last_error", "nsgpu_prior_transform",

@@ -182,6 +182,24 @@ def test_tensor_core_path_odd_shapes(width, n_hidden, n_out, B):
     assert np.all(np.abs(ll - ref_ll) <= loglike_tolerance(chi2))
 
 
+@pytest.mark.parametrize("name,B", [("c3a", 23), ("c3a", 700), ("c1", 129), ("c2", 385)])
+def test_weight_multicast_pairs_are_bit_identical(name, B):
+    """the cluster kernel (CTA pairs, weight tiles multicast) does the same arithmetic as the
+    one-CTA kernel: same bits, for odd numbers of row blocks (the spare CTA repeats the last block) and for
+    the automatic choice; and both stay within the oracle tolerance (test_full_size_configs_sampled_parity)."""
+    wl = workload(name)
+    theta = theta_of_u(wl, np.concatenate([W.u_post_set(wl, B // 2), W.u_prior_set(wl, B - B // 2)]))
+    res = []
+    for flag in (nsgpu.MLP_NO_CLUSTER, nsgpu.MLP_CLUSTER, 0):
+        with nsgpu.Context(wl, max_batch=B, mlp=nsgpu.MLP_TC | flag) as ctx:
+            spec = ctx.emulate_batch(dev(theta), 0).cpu().numpy()
+            res.append((spec, ctx.loglike_batch(dev(theta)).cpu().numpy()))
+    for spec, ll in res[1:]:
+        np.testing.assert_array_equal(spec, res[0][0])
+        np.testing.assert_array_equal(ll, res[0][1])
+    assert np.isfinite(res[0][1]).all()
+
+
 def test_tensor_core_and_simt_paths_agree_on_shear():
     """the two on-device MLP paths (different table layouts into the projection) give the same log L"""
     wl = W.shear(seed=21, w0wa=True, n_z_emu=9, n_z=9, width=64, n_hidden=2, n_k=40, n_chi=24, n_ell=6, n_tomo=3, name="s64")
