@@ -127,6 +127,8 @@ typedef struct {
 #define NSGPU_MLP_CLUSTER 32u    /* tcgen05 GEMMs: CTA pairs that multicast the weight tiles, whatever the batch (default: large batches) */
 #define NSGPU_MLP_NO_CLUSTER 64u /* ... never */
 #define NSGPU_SHEAR_STREAM 4u /* kind 3: use the streaming projection kernels even where the grids fit shared memory */
+#define NSGPU_NO_PDL 128u /* launch every kernel with plain stream ordering (default: the kernels of a likelihood call and of a
+                            * slice-sampling round are chained by programmatic dependent launch) */
 
 /* Create a context on CUDA device `device`.
  * data [n_data] and chol [n_data][n_data] (lower Cholesky factor of the data covariance, row-major,

@@ -160,6 +160,8 @@ __global__ void __launch_bounds__(MAXT) chi2_mma_kernel(const double* __restrict
                                                          const double* __restrict__ p0, const double* __restrict__ p1,
                                                          double log_norm, double* __restrict__ logL) {
   constexpr int TB = 8 * NTL, TBP = TB + 8;               // NBUF chunks of the factor in flight
+  pdl_wait();      // launch_pdl contract: the row count and the model vectors come from earlier kernels
+  pdl_trigger();
   if (n_rows_dev) B = min(B, *n_rows_dev);
   const int b0 = blockIdx.x * TB;
   if (b0 >= B) return;
@@ -169,7 +171,8 @@ __global__ void __launch_bounds__(MAXT) chi2_mma_kernel(const double* __restrict
   double* r = reinterpret_cast<double*>(smem_raw);        // [n4][TBP] residuals, rows n .. n4-1 zero
   double* part = r + (size_t)n4 * TBP;                    // [nwarp][TB]
   unsigned long long* bars = reinterpret_cast<unsigned long long*>(part + (size_t)nwarp * TB);   // full[NBUF], empty[NBUF]
-  double* S = reinterpret_cast<double*>(bars + 2 * NBUF); // [NBUF][CH][nsp]
+  int* bad = reinterpret_cast<int*>(bars + 2 * NBUF);     // [TB] theta outside the prior support / not finite
+  double* S = reinterpret_cast<double*>(bad + TB);        // [NBUF][CH][nsp]
   const uint32_t full0 = tc::smem_u32(bars), empty0 = full0 + 8 * NBUF;
   const int n_chunks = (n + CH - 1) / CH;
   // LinvT rows have the same (padded) stride in global memory, so a chunk of CH columns is ONE contiguous bulk
@@ -187,14 +190,37 @@ __global__ void __launch_bounds__(MAXT) chi2_mma_kernel(const double* __restrict
     for (int b = 0; b < NBUF; ++b) { tc::mbar_init(full0 + 8 * b, 1); tc::mbar_init(empty0 + 8 * b, nwarp); }
     tc::fence_barrier_init();
   }
-  for (int i = tid; i < n4 * TB; i += blockDim.x) {       // residuals, transposed into [j][theta]
-    const int t = i / n4, j = i - t * n4;
-    const int b = b0 + t;
-    r[(size_t)j * TBP + t] = (b < B && j < n) ? model[(size_t)b * n + j] - data[j] : 0.0;
-  }
-  __syncthreads();
-  if (warp == 0)
+  __syncwarp();
+  if (warp == 0)                                          // the first chunks travel while the residuals are formed
     for (int c = 0; c < NBUF - 1 && c < n_chunks; ++c) load_chunk(c, c);
+  // residuals, transposed into [j][theta]: four independent loads in flight per thread (the loop is bound by the
+  // latency of the model reads, not by their number)
+  const int n_res = n4 * TB;
+  for (int i0 = tid; i0 < n_res; i0 += 4 * blockDim.x) {
+    double mv[4];
+    int jj[4], tt[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int i = i0 + u * blockDim.x;
+      const int t = i / n4, j = i - t * n4;
+      const int b = b0 + t;
+      tt[u] = t; jj[u] = j;
+      mv[u] = (i < n_res && b < B && j < n) ? __ldg(model + (size_t)b * n + j) - __ldg(data + j) : 0.0;
+    }
+#pragma unroll
+    for (int u = 0; u < 4; ++u)
+      if (i0 + u * blockDim.x < n_res) r[(size_t)jj[u] * TBP + tt[u]] = mv[u];
+  }
+  // prior support and finiteness of theta (compared in the float32 theta arrives in): all threads, one flag per theta
+  if (tid < TB) bad[tid] = 0;
+  __syncthreads();
+  for (int i = tid; i < TB * D; i += blockDim.x) {
+    const int t = i / D, d = i - t * D;
+    if (b0 + t < B) {
+      const float v = __ldg(theta + (size_t)(b0 + t) * D + d);
+      if (!isfinite(v) || (prior_kind[d] == 0 && (v < (float)p0[d] || v > (float)p1[d]))) bad[t] = 1;
+    }
+  }
   const int MT = (n + 7) >> 3;
   const int mtA = warp, mtB = MT - 1 - warp;              // short and long 8-row tiles of this warp
   const bool hasB = mtB >= mtA, hasA = mtA < mtB;         // the middle tile of an odd count is B alone
@@ -254,14 +280,8 @@ __global__ void __launch_bounds__(MAXT) chi2_mma_kernel(const double* __restrict
     if (b < B) {
       double chi2 = 0.0;
       for (int w = 0; w < nwarp; ++w) chi2 += part[(size_t)w * TB + tid];
-      double out = -0.5 * chi2 + log_norm;
-      bool ok = isfinite(out);
-      for (int d = 0; d < D; ++d) {
-        const float v = theta[(size_t)b * D + d];
-        if (!isfinite(v)) ok = false;
-        if (prior_kind[d] == 0 && (v < (float)p0[d] || v > (float)p1[d])) ok = false;
-      }
-      logL[b] = ok ? out : -INFINITY;
+      const double out = -0.5 * chi2 + log_norm;
+      logL[b] = (isfinite(out) && !bad[tid]) ? out : -INFINITY;
     }
   }
 }
@@ -476,7 +496,7 @@ nsgpu_status chi2_loglike(nsgpu_ctx* ctx, const float* theta, int B, const int* 
     const int MT = (n + 7) / 8, warps = (MT + 1) / 2, threads = 32 * warps;
     const int nsp = ctx->linv_ld;                                             // 8 mod 16 doubles, >= n rounded up to 8
     const int n4 = (n + 3) & ~3, TBP = 8 * ntl + 8;
-    const size_t smem_fixed = ((size_t)n4 * TBP + (size_t)warps * 8 * ntl + 16) * sizeof(double);   // + up to 2 x 8 mbarriers
+    const size_t smem_fixed = ((size_t)n4 * TBP + (size_t)warps * 8 * ntl + 16 + 16) * sizeof(double);   // + up to 2 x 8 mbarriers + 8 ntl prior flags
     int CH = (int)((100 * 1024 / 4) / ((size_t)nsp * 8));
     CH = std::max(4, std::min(16, CH & ~3));
     // small batches are bound by the latency of the chunk ring, not by arithmetic: eight chunks in flight when
@@ -489,9 +509,9 @@ nsgpu_status chi2_loglike(nsgpu_ctx* ctx, const float* theta, int B, const int* 
 #define NSGPU_CHI2_MMA(NTL_, MAXT_, NBUF_)                                                                            \
   do {                                                                                                                \
     NSGPU_CUDA(nsgpu_ensure_smem(ctx, chi2_mma_kernel<NTL_, MAXT_, NBUF_>, 220 * 1024));                               \
-    chi2_mma_kernel<NTL_, MAXT_, NBUF_><<<grid, threads, smem, st>>>(ctx->model, ctx->data, ctx->Linv, n, B, CH, nsp, n_rows_dev, \
-                                                                     theta, ctx->D, ctx->prior_kind, ctx->prior_p0,   \
-                                                                     ctx->prior_p1, ctx->log_norm, logL);             \
+    NSGPU_CUDA(launch_pdl(ctx, chi2_mma_kernel<NTL_, MAXT_, NBUF_>, dim3(grid), dim3(threads), smem, st, ctx->model, ctx->data, ctx->Linv, \
+                          n, B, CH, nsp, n_rows_dev, theta, ctx->D, ctx->prior_kind, ctx->prior_p0, ctx->prior_p1,     \
+                          ctx->log_norm, logL));                                                                        \
   } while (0)
 #define NSGPU_CHI2_MMA_T(MAXT_)                                                                                       \
   do {                                                                                                                \

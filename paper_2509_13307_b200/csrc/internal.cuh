@@ -7,6 +7,8 @@
 #include <stdint.h>
 
 #include <algorithm>
+#include <cstring>
+#include <utility>
 #include <map>
 #include <string>
 #include <vector>
@@ -150,6 +152,33 @@ inline cudaError_t nsgpu_ensure_smem(nsgpu_ctx* ctx, F* fn, size_t bytes) {
       return NSGPU_ECUDA;                                                                 \
     }                                                                                     \
   } while (0)
+
+// ---- programmatic dependent launch (PDL) ------------------------------------------------------------------
+// The kernels of one likelihood call / one slice-sampling round form a chain on one stream; a nested-sampling
+// round is ~10 launches of 10-100 us each, so the drain-and-launch gap between two kernels is a visible share of
+// it.  A kernel launched through launch_pdl may start (CTAs become resident as the predecessor's CTAs exit, and run
+// their prologue: barrier init, TMEM allocation, staging of constants) while its predecessor is still running.
+// Contract for every kernel launched this way: pdl_wait() before the FIRST access to anything an earlier kernel
+// wrote (it returns once the predecessor grid has completed and its writes are visible), pdl_trigger() AFTER it.
+// Because each kernel triggers only after its own wait, a kernel can overlap with its direct predecessor only:
+// everything older is complete, so stream order is preserved transitively.  Kernels launched with <<<>>> keep
+// plain stream ordering on both sides.
+#ifdef __CUDACC__
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+#endif
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_pdl(const nsgpu_ctx* ctx, void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem,
+                              cudaStream_t st, Args&&... args) {
+  cudaLaunchConfig_t cfg;
+  memset(&cfg, 0, sizeof(cfg));
+  cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = (ctx->flags & NSGPU_NO_PDL) ? 0 : 1;
+  cfg.attrs = attr; cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, kern, KArgs(std::forward<Args>(args))...);
+}
 
 // stage entry points (one per translation unit); n_rows_dev != nullptr: only the first *n_rows_dev
 // rows (theta) are live, B is then the launch bound

@@ -132,7 +132,6 @@ __global__ void __launch_bounds__(256) mlp_first_layer_tc(const float* __restric
                                                           const float* __restrict__ in_std, const float* __restrict__ W,
                                                           const float4* __restrict__ params, int width, int split,
                                                           __half* __restrict__ out_hi, __half* __restrict__ out_lo) {
-  if (n_rows_dev) M = min(M, (*n_rows_dev) * rows_per_theta);
   extern __shared__ __align__(16) unsigned char smem_raw[];
   float4* sp = reinterpret_cast<float4*>(smem_raw);          // [width]
   float* sW = reinterpret_cast<float*>(sp + width);          // [n_in][width]
@@ -142,6 +141,9 @@ __global__ void __launch_bounds__(256) mlp_first_layer_tc(const float* __restric
     sp[2 * i + 1] = make_float4(c0.z, c1.z, c0.w, c1.w);
   }
   for (int i = threadIdx.x; i < n_in * width; i += blockDim.x) sW[i] = W[i];
+  pdl_wait();                                                // constants staged above; theta and the row count below (launch_pdl contract)
+  pdl_trigger();
+  if (n_rows_dev) M = min(M, (*n_rows_dev) * rows_per_theta);
   __syncthreads();
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int r = (warp & 3) * 32 + lane;                      // row within the tile
@@ -309,19 +311,6 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) mlp_gemm_tc(const __grid_cons
   float* params = reinterpret_cast<float*>(base_ptr + STAGES * STAGE + 16 * STAGES + 80);   // 16-byte aligned
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  int M = g.M_host;
-  if (g.n_rows_dev) M = min(M, (*g.n_rows_dev) * g.rows_per_theta);
-  const int n_blocks = g.N_pad / BLOCK_N;
-  const int m_blocks = (M + BLOCK_M - 1) / BLOCK_M;
-  // work items: (group of CS row blocks, column block); CTA `crank` of a cluster takes row block CS grp + crank
-  // (clamped: the spare CTA of a ragged last group repeats the last row block and stores the same values)
-  const int crank = CS > 1 ? (int)tc::cluster_ctarank() : 0;
-  const int num_tiles = ((m_blocks + CS - 1) / CS) * n_blocks;
-  const int tile0 = blockIdx.x / CS, tile_step = gridDim.x / CS;
-  constexpr uint16_t CMASK = (uint16_t)((1u << CS) - 1u);
-  constexpr int W_SUB_BYTES = B_TILE_BYTES / CS;                 // this CTA's share of a weight tile
-  const int k_blocks = g.K / BLOCK_K;
-
   if (threadIdx.x == 0) {
     for (int s = 0; s < STAGES; ++s) { tc::mbar_init(full0 + 8 * s, 1); tc::mbar_init(empty0 + 8 * s, CS); }
     for (int b = 0; b < NPB; ++b) { tc::mbar_init(pfull0 + 8 * b, 1); tc::mbar_init(pempty0 + 8 * b, EPI_WARPS); }
@@ -336,11 +325,28 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) mlp_gemm_tc(const __grid_cons
       reinterpret_cast<float4*>(params)[2 * i + 1] = make_float4(c0.z, c1.z, c0.w, c1.w);
     }
   }
+  // everything above touches only constants and this CTA's own shared memory / TMEM: it may run while the previous
+  // layer is still finishing (launch_pdl contract); the activations and the row count are read below
+  pdl_wait();
+  pdl_trigger();
   tc::fence_before_sync();
   __syncthreads();
   if (CS > 1) tc::cluster_sync();        // every CTA's barriers exist before a peer's multicast or commit reaches them
   tc::fence_after_sync();
   const uint32_t tmem_base = *tmem_slot;
+  int M = g.M_host;
+  if (g.n_rows_dev) M = min(M, (*g.n_rows_dev) * g.rows_per_theta);
+  const int n_blocks = g.N_pad / BLOCK_N;
+  const int m_blocks = (M + BLOCK_M - 1) / BLOCK_M;
+  // work items: (group of CS row blocks, column block); CTA `crank` of a cluster takes row block CS grp + crank
+  // (clamped: the spare CTA of a ragged last group repeats the last row block and stores the same values)
+  const int crank = CS > 1 ? (int)tc::cluster_ctarank() : 0;
+  const int num_tiles = ((m_blocks + CS - 1) / CS) * n_blocks;
+  const int tile0 = blockIdx.x / CS, tile_step = gridDim.x / CS;
+  constexpr uint16_t CMASK = (uint16_t)((1u << CS) - 1u);
+  constexpr int W_SUB_BYTES = B_TILE_BYTES / CS;                 // this CTA's share of a weight tile
+  const int k_blocks = g.K / BLOCK_K;
+
   // registers: 384 x 168 at launch -> 232 for the epilogue warpgroups (accumulators + deferred columns), 40 for the rest
   if (warp >= EPI_WARPS) {
     asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
@@ -563,7 +569,7 @@ nsgpu_status launch_gemm(nsgpu_ctx* ctx, const CUtensorMap& whi, const CUtensorM
   NSGPU_CUDA(nsgpu_ensure_smem(ctx, mlp_gemm_tc<BN, EPI>, SMEM_BUDGET));
   const int tiles = ((g.M_host + BLOCK_M - 1) / BLOCK_M) * (g.N_pad / BN);
   const int grid = std::min(tiles, ctx->sm_count);
-  mlp_gemm_tc<BN, EPI><<<grid, GEMM_THREADS, smem, st>>>(whi, wlo, g);
+  NSGPU_CUDA(launch_pdl(ctx, mlp_gemm_tc<BN, EPI>, dim3(grid), dim3(GEMM_THREADS), smem, st, whi, wlo, g));
   NSGPU_LAUNCH_CHECK();
   return NSGPU_OK;
 }
@@ -583,11 +589,13 @@ nsgpu_status launch_gemm_cluster(nsgpu_ctx* ctx, const CUtensorMap& whi, const C
   cfg.blockDim = dim3(GEMM_THREADS);
   cfg.dynamicSmemBytes = smem;
   cfg.stream = st;
-  cudaLaunchAttribute attr[1];
+  cudaLaunchAttribute attr[2];
   attr[0].id = cudaLaunchAttributeClusterDimension;
   attr[0].val.clusterDim.x = CS; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+  attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;   // see launch_pdl
+  attr[1].val.programmaticStreamSerializationAllowed = (ctx->flags & NSGPU_NO_PDL) ? 0 : 1;
   cfg.attrs = attr;
-  cfg.numAttrs = 1;
+  cfg.numAttrs = 2;
   NSGPU_CUDA(cudaLaunchKernelEx(&cfg, mlp_gemm_tc<BN, EPI, CS>, whi, wlo, g));
   NSGPU_LAUNCH_CHECK();
   return NSGPU_OK;
@@ -735,8 +743,8 @@ nsgpu_status mlp_forward_tc(nsgpu_ctx* ctx, int e, const float* theta, int B, co
     const int fl_tiles = (M + BLOCK_M - 1) / BLOCK_M;
     const int fl_split = fl_tiles >= 4 * ctx->sm_count ? 1 : 4;
     const int fl_grid = fl_tiles * fl_split;
-#define NSGPU_FL(N_) case N_: mlp_first_layer_tc<N_><<<fl_grid, 256, smem, st>>>ARGS_; break;
-#define ARGS_ (theta, ctx->D, rpt, M, n_rows_dev, ctx->emu_in_idx,                                                                       ctx->emu_in_const, ctx->n_theta_in, ctx->z_emu,                                                                       E.n_in, E.in_mean, E.in_std, E.W[0],                                                                       T->layers[0].p_hidden, E.width, fl_split, T->act[0][0],                                                                       T->act[0][1])
+#define NSGPU_FL(N_) case N_: NSGPU_CUDA(launch_pdl(ctx, mlp_first_layer_tc<N_>, dim3(fl_grid), dim3(256), smem, st, ARGS_)); break;
+#define ARGS_ theta, ctx->D, rpt, M, n_rows_dev, ctx->emu_in_idx,                                                                       ctx->emu_in_const, ctx->n_theta_in, ctx->z_emu,                                                                       E.n_in, E.in_mean, E.in_std, E.W[0],                                                                       T->layers[0].p_hidden, E.width, fl_split, T->act[0][0],                                                                       T->act[0][1]
     switch (E.n_in) {
       NSGPU_FL(1) NSGPU_FL(2) NSGPU_FL(3) NSGPU_FL(4) NSGPU_FL(5) NSGPU_FL(6) NSGPU_FL(7) NSGPU_FL(8)
       NSGPU_FL(9) NSGPU_FL(10) NSGPU_FL(11) NSGPU_FL(12) NSGPU_FL(13) NSGPU_FL(14) NSGPU_FL(15) NSGPU_FL(16)

@@ -125,6 +125,8 @@ struct RoundArgs {
 // next proposal that needs a likelihood.  Phase transitions are taken from the state as it was when the
 // result was requested: a chain consumes exactly one likelihood result per round.
 __global__ void __launch_bounds__(128) slice_round_kernel(RoundArgs a) {
+  pdl_wait();      // logL_prop comes from the likelihood kernels of the previous round (launch_pdl contract)
+  pdl_trigger();
   const int c = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   const int lane = threadIdx.x & 31;
   if (c >= a.n_chains) return;
@@ -245,6 +247,8 @@ __global__ void __launch_bounds__(1024) compact_kernel(int n_chains, int D, cons
   __shared__ int wsum[32];
   __shared__ int total;
   int carry = 0;
+  pdl_wait();
+  pdl_trigger();
   for (int base = 0; base < n_chains; base += blockDim.x) {
     const int c = base + threadIdx.x;
     const int f = (c < n_chains) ? need[c] : 0;
@@ -573,10 +577,10 @@ static nsgpu_status evolve(nsgpu_ctx* ctx, int n_chains, int chain0, int n_steps
     for (int i = 0; i < burst; ++i) {
       {
       StageTimer tm(ctx, 6, st);
-      slice_round_kernel<<<blocks, 128, 0, st>>>(a);
+      NSGPU_CUDA(launch_pdl(ctx, slice_round_kernel, dim3(blocks), dim3(128), 0, st, a));
       NSGPU_LAUNCH_CHECK();
-      compact_kernel<<<1, 1024, 0, st>>>(n_chains, ctx->D, S->need, S->row_of_chain, S->theta_chain, S->theta_prop,
-                                         S->counters, S->n_evals);
+      NSGPU_CUDA(launch_pdl(ctx, compact_kernel, dim3(1), dim3(1024), 0, st, n_chains, ctx->D, S->need, S->row_of_chain, S->theta_chain,
+                            S->theta_prop, S->counters, S->n_evals));
       NSGPU_LAUNCH_CHECK();
       }
       nsgpu_status s = loglike_device(ctx, S->theta_prop, n_chains, S->counters, S->logL_prop, st);

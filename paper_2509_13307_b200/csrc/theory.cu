@@ -118,6 +118,8 @@ __global__ void __launch_bounds__(SHEAR_THREADS, 2) shear_project_kernel(const f
                                                                          double* __restrict__ aux,
                                                                          double* __restrict__ model, int n_data) {
   const int b = blockIdx.x;
+  pdl_wait();      // launch_pdl contract: the row count, the table and aux come from earlier kernels
+  pdl_trigger();
   if (n_rows_dev && b >= *n_rows_dev) return;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int nq = A.n_chi, nt = A.n_tomo, nqp = nq | 1;
@@ -951,11 +953,11 @@ nsgpu_status shear_project(nsgpu_ctx* ctx, const float* theta, int B, const int*
   const bool split = ((size_t)S.n_z_emu * S.n_k * 4) % 16 == 0 && ((size_t)(3 + S.n_tomo) * S.n_chi * 8) % 16 == 0 &&
                      ((size_t)3 * S.n_chi * 8) % 16 == 0 && S.aux != nullptr;
   if (split) {
-    shear_project_kernel<1><<<B, 128, smem1, st>>>(theta, ctx->D, n_rows_dev, ctx->spec, A, S.aux, ctx->model, ctx->n_data);
+    NSGPU_CUDA(launch_pdl(ctx, shear_project_kernel<1>, dim3(B), dim3(128), smem1, st, theta, ctx->D, n_rows_dev, ctx->spec, A, S.aux, ctx->model, ctx->n_data));
     NSGPU_LAUNCH_CHECK();
-    shear_project_kernel<2><<<B, SHEAR_THREADS, smem, st>>>(theta, ctx->D, n_rows_dev, ctx->spec, A, S.aux, ctx->model, ctx->n_data);
+    NSGPU_CUDA(launch_pdl(ctx, shear_project_kernel<2>, dim3(B), dim3(SHEAR_THREADS), smem, st, theta, ctx->D, n_rows_dev, ctx->spec, A, S.aux, ctx->model, ctx->n_data));
   } else {
-    shear_project_kernel<0><<<B, SHEAR_THREADS, smem, st>>>(theta, ctx->D, n_rows_dev, ctx->spec, A, S.aux, ctx->model, ctx->n_data);
+    NSGPU_CUDA(launch_pdl(ctx, shear_project_kernel<0>, dim3(B), dim3(SHEAR_THREADS), smem, st, theta, ctx->D, n_rows_dev, ctx->spec, A, S.aux, ctx->model, ctx->n_data));
   }
   NSGPU_LAUNCH_CHECK();
   return NSGPU_OK;

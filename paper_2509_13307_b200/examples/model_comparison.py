@@ -58,6 +58,7 @@ def main():
     ap.add_argument("--stop-frac", type=float, default=1e-3)
     ap.add_argument("--max-iter", type=int, default=100000)
     ap.add_argument("--shape", default="c4", choices=["c4", "paper-interp", "paper"])
+    ap.add_argument("--ctx-flags", type=int, default=0, help="extra nsgpu_create flags, e.g. 128 = NSGPU_NO_PDL (plain stream ordering)")
     args = ap.parse_args()
     rank, world, dev = _ranks()
     if args.shape == "c4":
@@ -69,7 +70,7 @@ def main():
     out = {}
     for name, wl in (("w0waCDM", full), ("LCDM", rest)):
         runs = []
-        with nsgpu.Context(wl, max_batch=args.n_live, device=dev) as ctx:
+        with nsgpu.Context(wl, max_batch=args.n_live, device=dev, mlp=nsgpu.MLP_AUTO | args.ctx_flags) as ctx:
             for seed in range(1, args.seeds + 1):
                 kw = dict(stop_frac=args.stop_frac, max_iter=args.max_iter, seed=seed, return_samples=False)
                 if world == 1:
