@@ -29,6 +29,7 @@
 
 struct SamplerDev {
   int cap = 0;   // max chains / live points
+  cudaStream_t run_stream = nullptr;   // nsgpu_run's own non-blocking stream: runs on different contexts overlap on the GPU
   int rounds_needed = 0, rounds_n_steps = -1;   // rounds the last evolve() took (for that n_steps): sizes the next first burst
   // chain state (SoA)
   float *x0 = nullptr, *dir = nullptr, *xprop = nullptr, *theta_chain = nullptr;   // [cap][D]
@@ -500,6 +501,7 @@ __global__ void init_live_kernel(int n, int D, uint2 key, float* u) {
 nsgpu_status sampler_create(nsgpu_ctx* ctx) {
   SamplerDev* S = new SamplerDev();
   ctx->sampler = S;
+  NSGPU_CUDA(cudaStreamCreateWithFlags(&S->run_stream, cudaStreamNonBlocking));
   const size_t cap = ctx->max_batch, D = ctx->D;
   S->cap = (int)cap;
 #define A(p, T, n) NSGPU_CUDA(cudaMalloc((void**)&S->p, sizeof(T) * (n)))
@@ -528,6 +530,7 @@ void sampler_destroy(nsgpu_ctx* ctx) {
                   S->logL_prop, S->counters, S->n_evals, S->scal, S->Lsig, S->u_live, S->logL_live, S->dead_idx,
                   S->surv_idx, S->logw, S->u_out, S->logL_out};
   for (void* p : ptrs) cudaFree(p);
+  if (S->run_stream) cudaStreamDestroy(S->run_stream);
   cudaFreeHost(S->h_counters); cudaFreeHost(S->h_evals); cudaFreeHost(S->h_scal);
   delete S;
   ctx->sampler = nullptr;
@@ -721,7 +724,9 @@ static nsgpu_status run_impl(nsgpu_ctx* ctx, const nsgpu_run_opts* o, int rank, 
   if (o->n_delete >= o->n_live || o->n_steps < 1 || !(o->stop_frac > 0) || o->max_iter < 1) { ctx->err = "run: bad options"; return NSGPU_EINVAL; }
   const auto t_start = std::chrono::steady_clock::now();
   SamplerDev* S = ctx->sampler;
-  cudaStream_t st = 0;
+  // one rank: the context's own stream, so that runs of several contexts (the two models of a comparison, driven from
+  // two host threads) share the GPU; sharded runs stay on the legacy default stream the exchange callback is ordered with
+  cudaStream_t st = world == 1 ? S->run_stream : (cudaStream_t)0;
   const int D = ctx->D, n = o->n_live, k = o->n_delete;
   const uint2 key = make_uint2((unsigned)(o->seed & 0xffffffffu), (unsigned)(o->seed >> 32));
   std::vector<float> dead_u;
@@ -808,6 +813,7 @@ static nsgpu_status run_impl(nsgpu_ctx* ctx, const nsgpu_run_opts* o, int rank, 
   const double logX = S->h_scal[1];
   std::vector<float> live_u((size_t)n * D);
   std::vector<double> live_l(n);
+  NSGPU_CUDA(cudaStreamSynchronize(st));
   NSGPU_CUDA(cudaMemcpy(live_u.data(), S->u_live, sizeof(float) * (size_t)n * D, cudaMemcpyDeviceToHost));
   NSGPU_CUDA(cudaMemcpy(live_l.data(), S->logL_live, sizeof(double) * (size_t)n, cudaMemcpyDeviceToHost));
   NSGPU_CUDA(cudaMemcpy(S->h_evals, S->n_evals, sizeof(unsigned long long), cudaMemcpyDeviceToHost));
@@ -888,10 +894,11 @@ static nsgpu_status run_impl(nsgpu_ctx* ctx, const nsgpu_run_opts* o, int rank, 
     for (size_t i = 0; i < ntot; ++i) S->last_logw[i] = terms[i] - logZ;
     for (size_t off = 0; off < ntot; off += (size_t)ctx->max_batch) {
       const int nb = (int)std::min<size_t>((size_t)ctx->max_batch, ntot - off);
-      NSGPU_CUDA(cudaMemcpy(S->xprop, all_u.data() + off * D, sizeof(float) * (size_t)nb * D, cudaMemcpyHostToDevice));
+      NSGPU_CUDA(cudaMemcpyAsync(S->xprop, all_u.data() + off * D, sizeof(float) * (size_t)nb * D, cudaMemcpyHostToDevice, st));
       s = nsgpu_prior_transform(ctx, S->xprop, nb, S->theta_prop, st);
       if (s != NSGPU_OK) return s;
-      NSGPU_CUDA(cudaMemcpy(S->last_theta.data() + off * D, S->theta_prop, sizeof(float) * (size_t)nb * D, cudaMemcpyDeviceToHost));
+      NSGPU_CUDA(cudaMemcpyAsync(S->last_theta.data() + off * D, S->theta_prop, sizeof(float) * (size_t)nb * D, cudaMemcpyDeviceToHost, st));
+      NSGPU_CUDA(cudaStreamSynchronize(st));   // copies and kernel ordered on the run's stream (not the legacy default one)
     }
   }
   if (cap > 0 && theta_samples && logL_samples && logw_samples) {

@@ -19,6 +19,8 @@ import argparse
 import json
 import math
 import os
+import threading
+import time
 
 import numpy as np
 import torch
@@ -58,6 +60,7 @@ def main():
     ap.add_argument("--stop-frac", type=float, default=1e-3)
     ap.add_argument("--max-iter", type=int, default=100000)
     ap.add_argument("--shape", default="c4", choices=["c4", "paper-interp", "paper"])
+    ap.add_argument("--sequential", action="store_true", help="one model after the other (default on one GPU: both at once)")
     ap.add_argument("--ctx-flags", type=int, default=0, help="extra nsgpu_create flags, e.g. 128 = NSGPU_NO_PDL (plain stream ordering)")
     args = ap.parse_args()
     rank, world, dev = _ranks()
@@ -68,8 +71,10 @@ def main():
         full, rest = _mock_data(W.c5(interp, w0wa=True), dev), W.c5(interp, w0wa=False)
     rest.data, rest.chol = full.data, full.chol
     out = {}
-    for name, wl in (("w0waCDM", full), ("LCDM", rest)):
+
+    def run_model(name, wl):
         runs = []
+        torch.cuda.set_device(dev)
         with nsgpu.Context(wl, max_batch=args.n_live, device=dev, mlp=nsgpu.MLP_AUTO | args.ctx_flags) as ctx:
             for seed in range(1, args.seeds + 1):
                 kw = dict(stop_frac=args.stop_frac, max_iter=args.max_iter, seed=seed, return_samples=False)
@@ -82,6 +87,21 @@ def main():
                     print(json.dumps(r), flush=True)
                 runs.append(r)
         out[name] = runs
+
+    models = (("w0waCDM", full), ("LCDM", rest))
+    t_all = time.perf_counter()
+    if world == 1 and not args.sequential:
+        # The two runs are independent and each keeps the GPU only partly busy (batches of <= n_delete proposals):
+        # one host thread per model, each nsgpu_run on its context's own stream, so their kernels share the SMs.
+        threads = [threading.Thread(target=run_model, args=m) for m in models]
+        for t in threads:
+            t.start()
+        for t in threads:
+            t.join()
+    else:
+        for m in models:
+            run_model(*m)
+    t_all = time.perf_counter() - t_all
     if rank != 0:
         return
     z = {k: np.mean([r["logZ"] for r in v]) for k, v in out.items()}
@@ -89,6 +109,7 @@ def main():
     print(json.dumps({"shape": args.shape, "summary": {k: {"logZ": z[k], "err": e[k], "evals": int(np.mean([r["n_like_evals"] for r in v])),
                                        "seconds": float(np.mean([r["seconds"] for r in v])),
                                        "iterations": int(np.mean([r["n_iter"] for r in v]))} for k, v in out.items()},
+                      "wall_seconds_all_runs": t_all, "concurrent_models": bool(world == 1 and not args.sequential),
                       "logB_LCDM_over_w0wa": z["LCDM"] - z["w0waCDM"],
                       "logB_err": math.hypot(e["LCDM"], e["w0waCDM"])}))
 
