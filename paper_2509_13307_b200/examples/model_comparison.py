@@ -60,7 +60,8 @@ def main():
     ap.add_argument("--stop-frac", type=float, default=1e-3)
     ap.add_argument("--max-iter", type=int, default=100000)
     ap.add_argument("--shape", default="c4", choices=["c4", "paper-interp", "paper"])
-    ap.add_argument("--sequential", action="store_true", help="one model after the other (default on one GPU: both at once)")
+    ap.add_argument("--sequential", action="store_true", help="one run after the other")
+    ap.add_argument("--concurrent", type=int, default=4, help="runs in flight on one GPU (models x seeds; default 4)")
     ap.add_argument("--ctx-flags", type=int, default=0, help="extra nsgpu_create flags, e.g. 128 = NSGPU_NO_PDL (plain stream ordering)")
     args = ap.parse_args()
     rank, world, dev = _ranks()
@@ -70,37 +71,44 @@ def main():
         interp = args.shape == "paper-interp"
         full, rest = _mock_data(W.c5(interp, w0wa=True), dev), W.c5(interp, w0wa=False)
     rest.data, rest.chol = full.data, full.chol
-    out = {}
+    out = {"w0waCDM": [], "LCDM": []}
+    lock = threading.Lock()
 
-    def run_model(name, wl):
-        runs = []
+    def run_model(name, wl, seeds):
         torch.cuda.set_device(dev)
         with nsgpu.Context(wl, max_batch=args.n_live, device=dev, mlp=nsgpu.MLP_AUTO | args.ctx_flags) as ctx:
-            for seed in range(1, args.seeds + 1):
+            for seed in seeds:
                 kw = dict(stop_frac=args.stop_frac, max_iter=args.max_iter, seed=seed, return_samples=False)
                 if world == 1:
                     r = ctx.run(args.n_live, args.n_delete, 5 * wl.D, **kw)
                 else:
                     r = ctx.run_sharded(args.n_live, args.n_delete, 5 * wl.D, rank=rank, world=world, **kw)
                 r["model"], r["D"], r["seed"], r["n_gpus"] = name, wl.D, seed, world
-                if rank == 0:
-                    print(json.dumps(r), flush=True)
-                runs.append(r)
-        out[name] = runs
+                with lock:
+                    if rank == 0:
+                        print(json.dumps(r), flush=True)
+                    out[name].append(r)
 
     models = (("w0waCDM", full), ("LCDM", rest))
+    all_seeds = list(range(1, args.seeds + 1))
     t_all = time.perf_counter()
-    if world == 1 and not args.sequential:
-        # The two runs are independent and each keeps the GPU only partly busy (batches of <= n_delete proposals):
-        # one host thread per model, each nsgpu_run on its context's own stream, so their kernels share the SMs.
-        threads = [threading.Thread(target=run_model, args=m) for m in models]
+    n_conc = 1 if (world > 1 or args.sequential) else max(1, args.concurrent)
+    if n_conc > 1:
+        # The runs are independent and each keeps the GPU only partly busy (batches of <= n_delete proposals, fewer
+        # as the chains of an iteration finish): one host thread and one context per worker, each nsgpu_run on its
+        # context's own stream, so their kernels share the SMs.  Workers = models x groups of seeds.
+        per_model = max(1, min(len(all_seeds), n_conc // 2))
+        jobs = [(name, wl, all_seeds[g::per_model]) for name, wl in models for g in range(per_model)]
+        threads = [threading.Thread(target=run_model, args=j) for j in jobs]
         for t in threads:
             t.start()
         for t in threads:
             t.join()
+        for v in out.values():
+            v.sort(key=lambda r: r["seed"])
     else:
-        for m in models:
-            run_model(*m)
+        for name, wl in models:
+            run_model(name, wl, all_seeds)
     t_all = time.perf_counter() - t_all
     if rank != 0:
         return
@@ -109,7 +117,7 @@ def main():
     print(json.dumps({"shape": args.shape, "summary": {k: {"logZ": z[k], "err": e[k], "evals": int(np.mean([r["n_like_evals"] for r in v])),
                                        "seconds": float(np.mean([r["seconds"] for r in v])),
                                        "iterations": int(np.mean([r["n_iter"] for r in v]))} for k, v in out.items()},
-                      "wall_seconds_all_runs": t_all, "concurrent_models": bool(world == 1 and not args.sequential),
+                      "wall_seconds_all_runs": t_all, "concurrent_runs": n_conc if n_conc == 1 else len(jobs),
                       "logB_LCDM_over_w0wa": z["LCDM"] - z["w0waCDM"],
                       "logB_err": math.hypot(e["LCDM"], e["w0waCDM"])}))
 

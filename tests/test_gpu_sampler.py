@@ -154,3 +154,33 @@ def test_run_constant_likelihood():
         r = ctx.run(64, 32, 4, seed=1, max_iter=6)
     assert r["logZ"] == pytest.approx(gaussian.log_norm(wl.chol), abs=1e-9)
     assert not r["converged"] or r["n_iter"] <= 6
+
+
+def test_concurrent_runs_on_two_contexts_equal_sequential_runs():
+    """nsgpu_run works on its context's own stream: two runs driven from two host threads share the GPU and
+    return exactly what each returns alone; NSGPU_NO_PDL (plain stream order between kernels) changes nothing."""
+    import threading
+    wl = workload("toy")
+    args = (200, 100, 30)
+    with nsgpu.Context(wl, max_batch=200) as ctx:
+        alone = {s: ctx.run(*args, seed=s) for s in (1, 2)}
+    with nsgpu.Context(wl, max_batch=200, mlp=nsgpu.MLP_AUTO | nsgpu.NO_PDL) as ctx:
+        plain = ctx.run(*args, seed=1)
+    got = {}
+
+    def work(seed):
+        with nsgpu.Context(wl, max_batch=200) as c:
+            got[seed] = c.run(*args, seed=seed)
+
+    threads = [threading.Thread(target=work, args=(s,)) for s in (1, 2)]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join()
+    for s in (1, 2):
+        for key in ("logZ", "logZ_err", "H", "n_iter", "n_like_evals"):
+            assert got[s][key] == alone[s][key], (s, key)
+        np.testing.assert_array_equal(got[s]["theta"], alone[s]["theta"])
+        np.testing.assert_array_equal(got[s]["logw"], alone[s]["logw"])
+    assert plain["logZ"] == alone[1]["logZ"] and plain["n_like_evals"] == alone[1]["n_like_evals"]
+    np.testing.assert_array_equal(plain["theta"], alone[1]["theta"])
