@@ -298,6 +298,8 @@ constexpr int CT_ROWS = 128, CT_KC = 8, CT_NBUF = 4, CT_WARPS = 8;
 __global__ void residual_transpose_kernel(const double* __restrict__ model, const double* __restrict__ data, int n, int B,
                                           const int* __restrict__ n_rows_dev, size_t ldr, double* __restrict__ rt) {
   __shared__ double tile[32][33];
+  pdl_wait();      // launch_pdl contract
+  pdl_trigger();
   const int live = n_rows_dev ? min(B, *n_rows_dev) : B;
   const int j0 = blockIdx.x * 32, b0 = blockIdx.y * 32;
   if (b0 >= ((live + 63) & ~63)) return;
@@ -330,6 +332,8 @@ __global__ void __launch_bounds__(CT_WARPS * 32, 2) chi2_tile_kernel(const doubl
                                                                      int n_tb, double* __restrict__ part) {
   constexpr int TBLK = 8 * TG;                            // thetas per CTA
   constexpr int LDL = CT_ROWS + 8, LDR = TBLK + 8;        // padded tile rows (stride = 8 mod 16 doubles)
+  pdl_wait();      // launch_pdl contract
+  pdl_trigger();
   const int live = n_rows_dev ? min(B, *n_rows_dev) : B;
   const int n_rb = (n + CT_ROWS - 1) / CT_ROWS;
   const int rb = n_rb - 1 - blockIdx.x / n_tb;            // longest row blocks first
@@ -431,6 +435,8 @@ __global__ void chi2_finalize_kernel(const double* __restrict__ part, int n_rb, 
                                      const int* __restrict__ n_rows_dev, const float* __restrict__ theta, int D,
                                      const int* __restrict__ prior_kind, const double* __restrict__ p0,
                                      const double* __restrict__ p1, double log_norm, double* __restrict__ logL) {
+  pdl_wait();      // launch_pdl contract
+  pdl_trigger();
   if (n_rows_dev) B = min(B, *n_rows_dev);
   const int b = blockIdx.x * blockDim.x + threadIdx.x;
   if (b >= B) return;
@@ -473,7 +479,7 @@ nsgpu_status chi2_loglike(nsgpu_ctx* ctx, const float* theta, int B, const int* 
     const int n_rb = (n + CT_ROWS - 1) / CT_ROWS;
     StageTimer tm(ctx, 5, st);
     dim3 tg((n + 31) / 32, (((B + 63) & ~63) + 31) / 32);
-    residual_transpose_kernel<<<tg, dim3(32, 8), 0, st>>>(ctx->model, ctx->data, n, B, n_rows_dev, ldr, ctx->resid_t);
+    NSGPU_CUDA(launch_pdl(ctx, residual_transpose_kernel, tg, dim3(32, 8), 0, st, ctx->model, ctx->data, n, B, n_rows_dev, ldr, ctx->resid_t));
     NSGPU_LAUNCH_CHECK();
     // 64 thetas per CTA; 32 when that would leave SMs idle (the nested-sampling rounds)
     const bool small = (size_t)n_rb * ((B + 63) / 64) < (size_t)ctx->sm_count;
@@ -481,11 +487,11 @@ nsgpu_status chi2_loglike(nsgpu_ctx* ctx, const float* theta, int B, const int* 
     const size_t smem_t = (size_t)CT_NBUF * CT_KC * (CT_ROWS + 8 + tblk + 8) * sizeof(double) + 2 * CT_NBUF * 8;
     NSGPU_CUDA(nsgpu_ensure_smem(ctx, chi2_tile_kernel<8>, smem_t));
     NSGPU_CUDA(nsgpu_ensure_smem(ctx, chi2_tile_kernel<4>, smem_t));
-    if (small) chi2_tile_kernel<4><<<n_rb * n_tb, CT_WARPS * 32, smem_t, st>>>(ctx->Linv, ctx->resid_t, n, ctx->linv_ld, B, n_rows_dev, ldr, n_tb, ctx->chi2_part);
-    else chi2_tile_kernel<8><<<n_rb * n_tb, CT_WARPS * 32, smem_t, st>>>(ctx->Linv, ctx->resid_t, n, ctx->linv_ld, B, n_rows_dev, ldr, n_tb, ctx->chi2_part);
+    if (small) NSGPU_CUDA(launch_pdl(ctx, chi2_tile_kernel<4>, dim3(n_rb * n_tb), dim3(CT_WARPS * 32), smem_t, st, ctx->Linv, ctx->resid_t, n, ctx->linv_ld, B, n_rows_dev, ldr, n_tb, ctx->chi2_part));
+    else NSGPU_CUDA(launch_pdl(ctx, chi2_tile_kernel<8>, dim3(n_rb * n_tb), dim3(CT_WARPS * 32), smem_t, st, ctx->Linv, ctx->resid_t, n, ctx->linv_ld, B, n_rows_dev, ldr, n_tb, ctx->chi2_part));
     NSGPU_LAUNCH_CHECK();
-    chi2_finalize_kernel<<<(B + 127) / 128, 128, 0, st>>>(ctx->chi2_part, n_rb, ldr, B, n_rows_dev, theta, ctx->D, ctx->prior_kind,
-                                                          ctx->prior_p0, ctx->prior_p1, ctx->log_norm, logL);
+    NSGPU_CUDA(launch_pdl(ctx, chi2_finalize_kernel, dim3((B + 127) / 128), dim3(128), 0, st, ctx->chi2_part, n_rb, ldr, B, n_rows_dev, theta, ctx->D,
+                          ctx->prior_kind, ctx->prior_p0, ctx->prior_p1, ctx->log_norm, logL));
     NSGPU_LAUNCH_CHECK();
     return NSGPU_OK;
   }

@@ -459,6 +459,8 @@ constexpr int WIN_G = 4, WIN_Q = 5;   // bins per scan pass; quadrature nodes pe
 __global__ void __launch_bounds__(256) shear_windows_kernel(const float* __restrict__ theta, int D,
                                                             const int* __restrict__ n_rows_dev, ShearArgs A, int G,
                                                             double* __restrict__ aux) {
+  pdl_wait();      // launch_pdl contract
+  pdl_trigger();
   const int b = blockIdx.x;
   if (n_rows_dev && b >= *n_rows_dev) return;
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -570,6 +572,8 @@ __global__ void __launch_bounds__(256) shear_power_kernel(const float* __restric
                                                           const float* __restrict__ spec, ShearArgs A,
                                                           const double* __restrict__ aux, int blocks_per_theta,
                                                           double* __restrict__ pg) {
+  pdl_wait();      // launch_pdl contract
+  pdl_trigger();
   const int b = blockIdx.x / blocks_per_theta, blk = blockIdx.x - b * blocks_per_theta;
   if (n_rows_dev && b >= *n_rows_dev) return;
   const int nq = A.n_chi, nq2 = (nq + 1) & ~1, n_lg4 = (A.n_ell + 3) >> 2;
@@ -658,6 +662,8 @@ __global__ void __launch_bounds__(LIMBER_THREADS, 3) shear_limber_kernel(const f
                                                                          const double* __restrict__ aux,
                                                                          const double* __restrict__ pg_all,
                                                                          double* __restrict__ model, int n_data) {
+  pdl_wait();      // launch_pdl contract
+  pdl_trigger();
   const int b = blockIdx.x;
   if (n_rows_dev && b >= *n_rows_dev) return;
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -812,6 +818,8 @@ __global__ void __launch_bounds__(128) cmb_bin_kernel(const float* __restrict__ 
                                                       const int* __restrict__ bin_col,
                                                       const float* __restrict__ bin_val, int n_data,
                                                       double* __restrict__ model) {
+  pdl_wait();      // launch_pdl contract
+  pdl_trigger();
   if (n_rows_dev) B = min(B, *n_rows_dev);
   const int b0 = blockIdx.y * CB_T;
   if (b0 >= B) return;
@@ -853,6 +861,8 @@ __global__ void __launch_bounds__(128) cmb_tt_kernel(const float* __restrict__ t
                                                      const double* __restrict__ mu, double cst, const int* __restrict__ prior_kind,
                                                      const double* __restrict__ p0, const double* __restrict__ p1,
                                                      double* __restrict__ logL) {
+  pdl_wait();      // launch_pdl contract
+  pdl_trigger();
   const int b = blockIdx.x;
   if (n_rows_dev) B = min(B, *n_rows_dev);
   if (b >= B) return;
@@ -881,6 +891,8 @@ __global__ void __launch_bounds__(128) cmb_tt_kernel(const float* __restrict__ t
 // kind 0: model = theta; kind 1: model = spectrum of emulator 0 (10^y where out_kind = 1)
 __global__ void copy_model_kernel(const float* __restrict__ src, int n, int ld, int B, const int* __restrict__ n_rows_dev,
                                   int apply_exp10, const double* __restrict__ mu, double* __restrict__ model) {
+  pdl_wait();      // launch_pdl contract
+  pdl_trigger();
   if (n_rows_dev) B = min(B, *n_rows_dev);
   const size_t total = (size_t)B * n;
   for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
@@ -929,15 +941,15 @@ nsgpu_status shear_project(nsgpu_ctx* ctx, const float* theta, int B, const int*
     const int KS = (LIMBER_THREADS / 32) / MP;
     const size_t smem_l = std::max((size_t)2 * (S.n_tomo + 1 + NT * 8) * LIMBER_LD + 2, (size_t)KS * MT * 8 * NT * 8) * sizeof(double);
     NSGPU_CUDA(nsgpu_ensure_smem(ctx, shear_windows_kernel, smem_w));
-    shear_windows_kernel<<<B, win_threads, smem_w, st>>>(theta, ctx->D, n_rows_dev, A, G, S.aux);
+    NSGPU_CUDA(launch_pdl(ctx, shear_windows_kernel, dim3(B), dim3(win_threads), smem_w, st, theta, ctx->D, n_rows_dev, A, G, S.aux));
     NSGPU_LAUNCH_CHECK();
     const int bpt = (((S.n_ell + 3) / 4) * S.n_chi + 255) / 256;
-    shear_power_kernel<<<(unsigned)((size_t)B * bpt), 256, 0, st>>>(theta, ctx->D, n_rows_dev, ctx->spec, A, S.aux, bpt, S.pg);
+    NSGPU_CUDA(launch_pdl(ctx, shear_power_kernel, dim3((unsigned)((size_t)B * bpt)), dim3(256), 0, st, theta, ctx->D, n_rows_dev, ctx->spec, A, S.aux, bpt, S.pg));
     NSGPU_LAUNCH_CHECK();
 #define NSGPU_LIMBER(NT_)                                                                                              \
   case NT_:                                                                                                           \
     NSGPU_CUDA(nsgpu_ensure_smem(ctx, shear_limber_kernel<NT_>, smem_l));                                              \
-    shear_limber_kernel<NT_><<<B, LIMBER_THREADS, smem_l, st>>>(theta, ctx->D, n_rows_dev, A, S.aux, S.pg, ctx->model, ctx->n_data); \
+    NSGPU_CUDA(launch_pdl(ctx, shear_limber_kernel<NT_>, dim3(B), dim3(LIMBER_THREADS), smem_l, st, theta, ctx->D, n_rows_dev, A, S.aux, S.pg, ctx->model, ctx->n_data)); \
     break;
     switch (NT) { NSGPU_LIMBER(1) NSGPU_LIMBER(2) NSGPU_LIMBER(3) NSGPU_LIMBER(4) }
 #undef NSGPU_LIMBER
@@ -974,9 +986,8 @@ nsgpu_status cmb_bin(nsgpu_ctx* ctx, const float* theta, int B, const int* n_row
   const size_t emu_stride = (size_t)ctx->max_batch * ctx->rows_per_theta * ctx->spec_ld;
   StageTimer tm(ctx, 4, st);
   dim3 grid((ctx->n_data + 127) / 128, (B + CB_T - 1) / CB_T);
-  cmb_bin_kernel<<<grid, 128, 0, st>>>(theta, ctx->D, B, n_rows_dev, ctx->spec, ctx->n_emu, n_out, ctx->spec_ld, emu_stride,
-                                       mask, ctx->cal_index, ctx->bin_ptr, ctx->bin_col, ctx->bin_val, ctx->n_data,
-                                       ctx->model);
+  NSGPU_CUDA(launch_pdl(ctx, cmb_bin_kernel, grid, dim3(128), 0, st, theta, ctx->D, B, n_rows_dev, ctx->spec, ctx->n_emu, n_out, ctx->spec_ld,
+                        emu_stride, mask, ctx->cal_index, ctx->bin_ptr, ctx->bin_col, ctx->bin_val, ctx->n_data, ctx->model));
   NSGPU_LAUNCH_CHECK();
   return NSGPU_OK;
 }
@@ -984,8 +995,8 @@ nsgpu_status cmb_bin(nsgpu_ctx* ctx, const float* theta, int B, const int* n_row
 nsgpu_status cmb_tt_loglike(nsgpu_ctx* ctx, const float* theta, int B, const int* n_rows_dev, double* logL, cudaStream_t st) {
   if (B == 0) return NSGPU_OK;
   StageTimer tm(ctx, 4, st);
-  cmb_tt_kernel<<<B, 128, 0, st>>>(theta, ctx->D, B, n_rows_dev, ctx->spec, ctx->n_data, ctx->spec_ld, ctx->tt_a, ctx->tt_b, ctx->tt_mu, ctx->log_norm,
-                                   ctx->prior_kind, ctx->prior_p0, ctx->prior_p1, logL);
+  NSGPU_CUDA(launch_pdl(ctx, cmb_tt_kernel, dim3(B), dim3(128), 0, st, theta, ctx->D, B, n_rows_dev, ctx->spec, ctx->n_data, ctx->spec_ld, ctx->tt_a,
+                        ctx->tt_b, ctx->tt_mu, ctx->log_norm, ctx->prior_kind, ctx->prior_p0, ctx->prior_p1, logL));
   NSGPU_LAUNCH_CHECK();
   return NSGPU_OK;
 }
@@ -998,7 +1009,8 @@ nsgpu_status copy_model(nsgpu_ctx* ctx, const float* theta, int B, const int* n_
   const int ex = (!ident && ctx->emu[0].out_kind == 1) ? 1 : 0;
   int blocks = (int)std::min<size_t>(((size_t)B * n + 255) / 256, 148 * 8);
   StageTimer tm(ctx, 7, st);
-  copy_model_kernel<<<blocks, 256, 0, st>>>(src, n, ident ? n : ctx->spec_ld, B, n_rows_dev, ex, ctx->kind == 4 ? ctx->tt_mu : nullptr, ctx->model);
+  NSGPU_CUDA(launch_pdl(ctx, copy_model_kernel, dim3(blocks), dim3(256), 0, st, src, n, ident ? n : ctx->spec_ld, B, n_rows_dev, ex,
+                        ctx->kind == 4 ? ctx->tt_mu : (const double*)nullptr, ctx->model));
   NSGPU_LAUNCH_CHECK();
   return NSGPU_OK;
 }
