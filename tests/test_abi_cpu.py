@@ -53,3 +53,28 @@ def test_product_does_not_import_the_oracle():
     code = ("import sys; import paper_2509_13307_b200.nsgpu, paper_2509_13307_b200.workloads, "
             "paper_2509_13307_b200.build; assert not any(m == 'oracle' or m.startswith('oracle.') for m in sys.modules)")
     subprocess.check_call([sys.executable, "-c", code], cwd=os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
+
+
+def test_binding_flag_constants_match_the_header():
+    """the flag bits the binding ORs into nsgpu_create are the header's #defines"""
+    import re
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    hdr = open(os.path.join(root, "include", "nsgpu.h")).read()
+    defs = {m.group(1): int(m.group(2)) for m in re.finditer(r"#define\s+NSGPU_(\w+)\s+(\d+)u\b", hdr)}
+    for name in ("MLP_AUTO", "MLP_SIMT", "MLP_TC", "CHI2_STREAMED", "CHI2_TILED", "MLP_CLUSTER", "MLP_NO_CLUSTER",
+                 "SHEAR_STREAM", "NO_PDL"):
+        assert getattr(nsgpu, name) == defs[name], name
+    bits = [defs[n] for n in defs if defs[n]]
+    assert len(set(bits)) == len(bits) and all(b & (b - 1) == 0 for b in bits)      # distinct single bits
+
+
+def test_examples_import_without_the_oracle_and_parse_their_arguments():
+    import subprocess, sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    for mod in ("model_comparison", "cmb_evidence"):
+        out = subprocess.run([sys.executable, "-m", f"paper_2509_13307_b200.examples.{mod}", "--help"], cwd=root,
+                             capture_output=True, text=True)
+        assert out.returncode == 0 and "--seeds" in out.stdout, out.stderr
+    code = ("import sys; import paper_2509_13307_b200.examples.model_comparison, paper_2509_13307_b200.examples.cmb_evidence; "
+            "assert not any(m == 'oracle' or m.startswith('oracle.') for m in sys.modules)")
+    subprocess.check_call([sys.executable, "-c", code], cwd=root)
