@@ -187,7 +187,10 @@ typedef struct {
 /* a1-a14: the whole nested-sampling run.  Samples go to caller-allocated HOST buffers of
  * capacity `cap` rows (may be NULL with cap = 0): theta [cap][D] float32, logL [cap], logw [cap]
  * float64 with logw = log(L_i w_i / Z); *n_samples returns n_dead + n_live (the number
- * needed); min(cap, needed) rows are written.  Returns NSGPU_ENOCONV if max_iter was reached.       */
+ * needed); min(cap, needed) rows are written.  Returns NSGPU_ENOCONV if max_iter was reached.
+ * Blocking.  The run works on a non-blocking stream the context owns: a context is not thread-safe, but runs on
+ * DIFFERENT contexts may be driven from different host threads at once and then share the GPU (a single run keeps
+ * it only partly busy: batches of <= n_delete proposals); each returns exactly what it returns alone.        */
 NSGPU_API nsgpu_status nsgpu_run(nsgpu_ctx* ctx, const nsgpu_run_opts* opts, nsgpu_result* res, float* theta_samples,
                        double* logL_samples, double* logw_samples, int64_t cap, int64_t* n_samples);
 
