@@ -135,12 +135,26 @@ __global__ void __launch_bounds__(256) mlp_first_layer_tc(const float* __restric
   extern __shared__ __align__(16) unsigned char smem_raw[];
   float4* sp = reinterpret_cast<float4*>(smem_raw);          // [width]
   float* sW = reinterpret_cast<float*>(sp + width);          // [n_in][width]
-  for (int i = threadIdx.x; i < width / 2; i += blockDim.x) {   // two columns per entry pair (see act_split_pair)
+  // Columns this CTA needs: all of them, or -- small batches, where the host launches one CTA per (tile, 1/split of
+  // the pieces) and staging 26 KB of constants per CTA was most of its life -- only those of its own part.
+  int col0 = 0, col1 = width;
+  if (split > 1 && (int)gridDim.x >= ((M + BLOCK_M - 1) / BLOCK_M) * split) {   // M: the launch bound, so one item per CTA
+    const int n_pieces_ = width >> 3, ppi_ = (n_pieces_ + split - 1) / split, part_ = blockIdx.x % split;
+    col0 = min(8 * part_ * ppi_, width);
+    col1 = min(8 * (part_ + 1) * ppi_, width);
+  }
+  for (int i = (col0 >> 1) + threadIdx.x; i < (col1 >> 1); i += blockDim.x) {   // two columns per entry pair (see act_split_pair)
     const float4 c0 = params[2 * i], c1 = params[2 * i + 1];
     sp[2 * i] = make_float4(c0.x, c1.x, c0.y, c1.y);
     sp[2 * i + 1] = make_float4(c0.z, c1.z, c0.w, c1.w);
   }
-  for (int i = threadIdx.x; i < n_in * width; i += blockDim.x) sW[i] = W[i];
+  {
+    const int nc = col1 - col0;
+    for (int i = threadIdx.x; i < n_in * nc; i += blockDim.x) {
+      const int c = i / nc, j = col0 + (i - c * nc);
+      sW[c * width + j] = W[c * width + j];
+    }
+  }
   pdl_wait();                                                // constants staged above; theta and the row count below (launch_pdl contract)
   pdl_trigger();
   if (n_rows_dev) M = min(M, (*n_rows_dev) * rows_per_theta);
