@@ -31,20 +31,40 @@
 namespace {
 
 constexpr int BLOCK_M = 128;
-constexpr int BLOCK_K = 64;                    // fp16 elements per k-block
-constexpr int A_TILE_BYTES = BLOCK_M * 128;    // 16 KB: 8 pieces x (128 rows x 16 bytes)
+// fp16 elements per k-block: a template parameter of the GEMM (64: two smem stages of 96 KB for 256-column tiles,
+// 128-byte-swizzled weight rows; 32: four stages of 48 KB, 64-byte swizzle).
 constexpr int PIECE_HALVES = BLOCK_M * 8;      // one 16-byte piece of every row of a tile: 2 KB
 constexpr float ACT_SCALE = 16.0f;             // activations are stored as fp16 hi/lo of 16 h
 constexpr int SMEM_BUDGET = 225 * 1024;
-// The 4 truncating hi.hi accumulation steps of one k-block shrink a partial by 1.05e-7 on average
-// (measured: output-vs-oracle regression slope -4.19e-7 over 4 layers, identical for K = 128 and 512);
-// the nearest fp32 factor undoes the mean of that bias.
-constexpr float TRUNC_COMP = 1.0f + 1.1920929e-7f;
+// tcgen05.mma adds into its fp32 TMEM accumulator with truncation toward zero (measured): every
+// accumulating MMA shrinks the accumulator by U[0,1) ulp.  Measured on one K = 512 layer with everything else exact
+// (profiles/r2_truncation_model.md): relative bias -c x (number of accumulations a contribution sits through), with
+// c = 3.2e-8 (0.54 x 2^-24) for sums of mixed sign and 4.9e-8 (0.82 x 2^-24) for sums of one sign, the same for
+// partials of 1, 2, 4 and 8 k-blocks; symmetric under a sign flip of the weights (toward zero, not toward -inf).
+// A partial of n k-blocks of s = BK/16 k-steps is 3 s n MMAs in the order (2 s corrections, s hi.hi) per k-block;
+// the hi.hi group j of k-block i is issued at step 3 s i + 2 s + j and is part of the accumulator at the
+// 3 s n - (3 s i + 2 s + j) later accumulations: 1.5 s n - s + 0.5 on average.  The mean of that bias is undone by one
+// factor folded into the epilogue scale (fp32, so a whole number of 2^-23); what is left is < 5e-8 per layer of slope
+// and the spread of the counts around their mean times the (random-signed) differences between the k-blocks'
+// contributions (rms 2.5e-7 |t| for 64 columns per partial, 4.6e-7 for 128: measured).
+constexpr double TRUNC_C = 3.2e-8;
+inline float trunc_comp(int K, int bk, int kpp) {
+  if (const char* ev = getenv("NSGPU_TRUNC_ULPS")) return 1.0f + (float)(atof(ev) / 8388608.0);   // kernel A/B runs
+  const int k_blocks = K / bk, st = bk / 16;
+  double wsum = 0.0;
+  for (int kb0 = 0; kb0 < k_blocks; kb0 += kpp) {
+    const int n = std::min(kpp, k_blocks - kb0);
+    wsum += n * (1.5 * st * n - st + 0.5);
+  }
+  const double ulps = std::nearbyint(TRUNC_C * (wsum / k_blocks) * 8388608.0);   // in units of 2^-23
+  return 1.0f + (float)(ulps / 8388608.0);
+}
 
-__host__ __device__ constexpr int stage_bytes(int block_n) { return 2 * A_TILE_BYTES + 2 * block_n * 128; }
-__host__ __device__ constexpr int num_stages(int block_n) {
-  int s = (SMEM_BUDGET - 1024 - 10 * 1024) / stage_bytes(block_n);   // 1 KB alignment slack, 10 KB params + barriers
-  return s > 6 ? 6 : s;
+__host__ __device__ constexpr int a_tile_bytes(int bk) { return BLOCK_M * bk * 2; }   // bk / 8 pieces x (128 rows x 16 bytes)
+__host__ __device__ constexpr int stage_bytes(int block_n, int bk) { return 2 * a_tile_bytes(bk) + 2 * block_n * bk * 2; }
+__host__ __device__ constexpr int num_stages(int block_n, int bk) {
+  int s = (SMEM_BUDGET - 1024 - 10 * 1024) / stage_bytes(block_n, bk);   // 1 KB alignment slack, 10 KB params + barriers
+  return s > 8 ? 8 : s;
 }
 
 struct GemmArgs {
@@ -52,6 +72,7 @@ struct GemmArgs {
   const int* n_rows_dev;      // live thetas (device) or nullptr
   int rows_per_theta;
   int K;                      // fan-in (multiple of 64)
+  int kpp;                    // k-blocks accumulated in TMEM per partial (1, 2, 4 ...; see mlp_gemm_tc)
   int N_pad;                  // padded fan-out (multiple of BLOCK_N)
   int n_valid;                // true fan-out
   const __half *a_hi, *a_lo;  // input planes, canonical layout, K columns
@@ -302,12 +323,13 @@ constexpr int DEFER_PAIRS = 32;                      // 64 columns of a finished
 // of them (96 -> 64 KB of L2 reads per CTA and k-block for CS = 2).  A stage may be refilled
 // only when every CTA of the cluster has consumed it: the MMA commit that frees it is multicast as well and the
 // `empty` barriers count CS arrivals.  The MMA / TMEM / epilogue side is unchanged.
-template <int BLOCK_N, int EPI, int CS = 1>
+template <int BLOCK_N, int EPI, int CS = 1, int BK = 64>
 __global__ void __launch_bounds__(GEMM_THREADS, 1) mlp_gemm_tc(const __grid_constant__ CUtensorMap tm_whi,
                                                                const __grid_constant__ CUtensorMap tm_wlo, GemmArgs g) {
-  constexpr int STAGES = num_stages(BLOCK_N);
-  constexpr int STAGE = stage_bytes(BLOCK_N);
-  constexpr int B_TILE_BYTES = BLOCK_N * 128;
+  constexpr int STAGES = num_stages(BLOCK_N, BK);
+  constexpr int STAGE = stage_bytes(BLOCK_N, BK);
+  constexpr int A_TILE_BYTES = a_tile_bytes(BK);
+  constexpr int B_TILE_BYTES = BLOCK_N * BK * 2;
   constexpr int CPT = BLOCK_N / (EPI_WARPS / 4);                 // columns per epilogue thread
   constexpr int LDC = (CPT % 16 == 0) ? 16 : 8;                  // columns per tcgen05.ld
   constexpr int NPB = BLOCK_N <= 128 ? 4 : 2;                    // TMEM partial buffers (ring)
@@ -359,7 +381,8 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) mlp_gemm_tc(const __grid_cons
   const int tile0 = blockIdx.x / CS, tile_step = gridDim.x / CS;
   constexpr uint16_t CMASK = (uint16_t)((1u << CS) - 1u);
   constexpr int W_SUB_BYTES = B_TILE_BYTES / CS;                 // this CTA's share of a weight tile
-  const int k_blocks = g.K / BLOCK_K;
+  const int k_blocks = g.K / BK;
+  const int kpp = g.kpp;
 
   // registers: 384 x 168 at launch -> 232 for the epilogue warpgroups (accumulators + deferred columns), 40 for the rest
   if (warp >= EPI_WARPS) {
@@ -377,16 +400,16 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) mlp_gemm_tc(const __grid_cons
           tc::mbar_wait(empty0 + 8 * stage, phase ^ 1);
           const uint32_t s0 = base + stage * STAGE, fb = full0 + 8 * stage;
           tc::mbar_arrive_expect_tx(fb, STAGE);
-          const size_t a_off = a_tile + (size_t)kb * 8 * PIECE_HALVES;
+          const size_t a_off = a_tile + (size_t)kb * (BK / 8) * PIECE_HALVES;
           tc::bulk_load(s0, g.a_hi + a_off, A_TILE_BYTES, fb);
           tc::bulk_load(s0 + A_TILE_BYTES, g.a_lo + a_off, A_TILE_BYTES, fb);
           if (CS == 1) {
-            tc::tma_load_2d(s0 + 2 * A_TILE_BYTES, &tm_whi, kb * BLOCK_K, n_blk * BLOCK_N, fb);
-            tc::tma_load_2d(s0 + 2 * A_TILE_BYTES + B_TILE_BYTES, &tm_wlo, kb * BLOCK_K, n_blk * BLOCK_N, fb);
+            tc::tma_load_2d(s0 + 2 * A_TILE_BYTES, &tm_whi, kb * BK, n_blk * BLOCK_N, fb);
+            tc::tma_load_2d(s0 + 2 * A_TILE_BYTES + B_TILE_BYTES, &tm_wlo, kb * BK, n_blk * BLOCK_N, fb);
           } else {   // tensor maps with boxes of BLOCK_N / CS rows
             const int wrow = n_blk * BLOCK_N + crank * (BLOCK_N / CS);
-            tc::tma_load_2d_mc(s0 + 2 * A_TILE_BYTES + crank * W_SUB_BYTES, &tm_whi, kb * BLOCK_K, wrow, fb, CMASK);
-            tc::tma_load_2d_mc(s0 + 2 * A_TILE_BYTES + B_TILE_BYTES + crank * W_SUB_BYTES, &tm_wlo, kb * BLOCK_K, wrow, fb, CMASK);
+            tc::tma_load_2d_mc(s0 + 2 * A_TILE_BYTES + crank * W_SUB_BYTES, &tm_whi, kb * BK, wrow, fb, CMASK);
+            tc::tma_load_2d_mc(s0 + 2 * A_TILE_BYTES + B_TILE_BYTES + crank * W_SUB_BYTES, &tm_wlo, kb * BK, wrow, fb, CMASK);
           }
           if (++stage == STAGES) { stage = 0; phase ^= 1; }
         }
@@ -397,35 +420,40 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) mlp_gemm_tc(const __grid_cons
     if (lane == 0) {
       uint32_t stage = 0, phase = 0, pcount = 0;
       for (int tile = tile0; tile < num_tiles; tile += tile_step) {
-        for (int kb = 0; kb < k_blocks; ++kb, ++pcount) {
+        for (int kb0 = 0; kb0 < k_blocks; kb0 += kpp, ++pcount) {
           const uint32_t pb = pcount % NPB, pphase = (pcount / NPB) & 1;
           tc::mbar_wait(pempty0 + 8 * pb, pphase ^ 1);          // the epilogue has pulled this partial
-          tc::mbar_wait(full0 + 8 * stage, phase);
-          tc::fence_after_sync();
           const uint32_t d_tmem = tmem_base + pb * PB_COLS;
-          const uint32_t s0 = base + stage * STAGE;
-          // A: canonical no-swizzle K-major tile -- 16-byte pieces 2048 bytes apart along K (leading
-          // byte offset), 8-row groups 128 bytes apart along M (stride byte offset); one MMA consumes
-          // two pieces (K = 16).  W: 128-byte-swizzled rows, 32 bytes per MMA.
-          const uint64_t a_hi = tc::smem_desc_nosw(s0, 2048, 128), a_lo = tc::smem_desc_nosw(s0 + A_TILE_BYTES, 2048, 128);
-          const uint64_t b_hi = tc::smem_desc_sw128(s0 + 2 * A_TILE_BYTES);
-          const uint64_t b_lo = tc::smem_desc_sw128(s0 + 2 * A_TILE_BYTES + B_TILE_BYTES);
-          // Corrections first (the accumulator is still ~2^-11 of its final size), hi.hi last.
+          const int kb1 = min(kb0 + kpp, k_blocks);
+          for (int kb = kb0; kb < kb1; ++kb) {
+            tc::mbar_wait(full0 + 8 * stage, phase);
+            tc::fence_after_sync();
+            const uint32_t s0 = base + stage * STAGE;
+            // A: canonical no-swizzle K-major tile -- 16-byte pieces 2048 bytes apart along K (leading
+            // byte offset), 8-row groups 128 bytes apart along M (stride byte offset); one MMA consumes
+            // two pieces (K = 16).  W: rows of BK halves, 128- or 64-byte swizzle, 32 bytes per MMA.
+            const uint64_t a_hi = tc::smem_desc_nosw(s0, 2048, 128), a_lo = tc::smem_desc_nosw(s0 + A_TILE_BYTES, 2048, 128);
+            const uint64_t b_hi = BK == 64 ? tc::smem_desc_sw128(s0 + 2 * A_TILE_BYTES) : tc::smem_desc_sw64(s0 + 2 * A_TILE_BYTES);
+            const uint64_t b_lo = BK == 64 ? tc::smem_desc_sw128(s0 + 2 * A_TILE_BYTES + B_TILE_BYTES)
+                                           : tc::smem_desc_sw64(s0 + 2 * A_TILE_BYTES + B_TILE_BYTES);
+            // Corrections first (in the first k-block of a partial the accumulator is still ~2^-11 of its final
+            // size), hi.hi last.
 #pragma unroll
-          for (int k = 0; k < BLOCK_K / 16; ++k) {
-            const uint64_t adv_a = (uint64_t)(256 * k), adv_b = (uint64_t)(2 * k);
-            tc::mma_f16_ss(d_tmem, a_lo + adv_a, b_hi + adv_b, IDESC, k != 0);
-            tc::mma_f16_ss(d_tmem, a_hi + adv_a, b_lo + adv_b, IDESC, 1);
-          }
+            for (int k = 0; k < BK / 16; ++k) {
+              const uint64_t adv_a = (uint64_t)(256 * k), adv_b = (uint64_t)(2 * k);
+              tc::mma_f16_ss(d_tmem, a_lo + adv_a, b_hi + adv_b, IDESC, (k != 0) | (kb != kb0));
+              tc::mma_f16_ss(d_tmem, a_hi + adv_a, b_lo + adv_b, IDESC, 1);
+            }
 #pragma unroll
-          for (int k = 0; k < BLOCK_K / 16; ++k) {
-            const uint64_t adv_a = (uint64_t)(256 * k), adv_b = (uint64_t)(2 * k);
-            tc::mma_f16_ss(d_tmem, a_hi + adv_a, b_hi + adv_b, IDESC, 1);
+            for (int k = 0; k < BK / 16; ++k) {
+              const uint64_t adv_a = (uint64_t)(256 * k), adv_b = (uint64_t)(2 * k);
+              tc::mma_f16_ss(d_tmem, a_hi + adv_a, b_hi + adv_b, IDESC, 1);
+            }
+            if (CS == 1) tc::mma_commit(empty0 + 8 * stage);      // smem slot free when these MMAs retire
+            else tc::mma_commit_mc(empty0 + 8 * stage, CMASK);    // ... in every CTA that multicasts into it
+            if (++stage == STAGES) { stage = 0; phase ^= 1; }
           }
-          if (CS == 1) tc::mma_commit(empty0 + 8 * stage);      // smem slot free when these MMAs retire
-          else tc::mma_commit_mc(empty0 + 8 * stage, CMASK);    // ... in every CTA that multicasts into it
-          tc::mma_commit(pfull0 + 8 * pb);                      // partial complete
-          if (++stage == STAGES) { stage = 0; phase ^= 1; }
+          tc::mma_commit(pfull0 + 8 * pb);                        // partial complete
         }
       }
     }
@@ -456,7 +484,7 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) mlp_gemm_tc(const __grid_cons
       const int m_grp = tile / n_blocks, n_blk = tile - m_grp * n_blocks;
       const int m_blk = min(m_grp * CS + crank, m_blocks - 1);
       f32x2 acc[NPAIR];
-      for (int kb = 0; kb < k_blocks; ++kb, ++pcount) {
+      for (int kb = 0; kb < k_blocks; kb += kpp, ++pcount) {
         const uint32_t pb = pcount % NPB, pphase = (pcount / NPB) & 1;
         tc::mbar_wait(pfull0 + 8 * pb, pphase);
         tc::fence_after_sync();
@@ -488,7 +516,7 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) mlp_gemm_tc(const __grid_cons
         tc::fence_before_sync();
         __syncwarp();
         if (lane == 0) tc::mbar_arrive(pempty0 + 8 * pb);
-        if (DEFP > 0 && pdone < NCH && kb >= 1) { NSGPU_RUN_CHUNK(pdone); ++pdone; }
+        if (DEFP > 0 && pdone < NCH && (kb >= 1 || kpp > 1)) { NSGPU_RUN_CHUNK(pdone); ++pdone; }
       }
       while (DEFP > 0 && pdone < NCH) { NSGPU_RUN_CHUNK(pdone); ++pdone; }   // short K: not enough idle slots
       const int r_in = q * 32 + lane;
@@ -535,6 +563,12 @@ struct TcState {
   std::vector<TcLayer> layers;               // index = layer 0 .. n_hidden (layer 0 uses p_hidden only)
   __half* act[2][2] = {};                    // [buffer][hi, lo] canonical-layout planes
   size_t M_pad = 0;
+  // k-block (64 or 32 columns) and k-blocks per TMEM partial.  Measured (profiles/r2_gemm_pipeline_ab.md): four stages of
+  // 32 columns are no faster than two of 64 (the kernel is bound by the chip's power cap, not by operand latency), and
+  // every further k-block in a partial costs precision (more truncating accumulations) for 3-5% of time.  NSGPU_BK /
+  // NSGPU_KPP override them for kernel A/B runs.
+  int bk = 64;
+  int kpp = 1;
 };
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
@@ -553,16 +587,16 @@ EncodeTiledFn encode_fn() {
   return fn;
 }
 
-// fp16 [rows][cols] row-major, box = box_rows x 64 columns (128 bytes), 128-byte swizzle, OOB -> 0
-bool make_tmap(CUtensorMap* tm, const void* ptr, size_t rows, size_t cols, int box_rows) {
+// fp16 [rows][cols] row-major, box = box_rows x bk columns (128 or 64 bytes) with the swizzle of that width, OOB -> 0
+bool make_tmap(CUtensorMap* tm, const void* ptr, size_t rows, size_t cols, int box_rows, int bk) {
   EncodeTiledFn fn = encode_fn();
   if (!fn) return false;
   const cuuint64_t dims[2] = {(cuuint64_t)cols, (cuuint64_t)rows};
   const cuuint64_t strides[1] = {(cuuint64_t)cols * sizeof(__half)};
-  const cuuint32_t box[2] = {(cuuint32_t)BLOCK_K, (cuuint32_t)box_rows};
+  const cuuint32_t box[2] = {(cuuint32_t)bk, (cuuint32_t)box_rows};
   const cuuint32_t estr[2] = {1, 1};
   return fn(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 2, const_cast<void*>(ptr), dims, strides, box, estr,
-            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, bk == 64 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_64B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
@@ -577,23 +611,23 @@ int pick_block_n(int n, bool hidden) {
   return best;
 }
 
-template <int BN, int EPI>
+template <int BN, int EPI, int BK>
 nsgpu_status launch_gemm(nsgpu_ctx* ctx, const CUtensorMap& whi, const CUtensorMap& wlo, const GemmArgs& g, cudaStream_t st) {
-  const int smem = num_stages(BN) * stage_bytes(BN) + 16 * num_stages(BN) + 128 + (EPI == 0 ? 16 * g.N_pad : 0) + 1024;
-  NSGPU_CUDA(nsgpu_ensure_smem(ctx, mlp_gemm_tc<BN, EPI>, SMEM_BUDGET));
+  const int smem = num_stages(BN, BK) * stage_bytes(BN, BK) + 16 * num_stages(BN, BK) + 128 + (EPI == 0 ? 16 * g.N_pad : 0) + 1024;
+  NSGPU_CUDA(nsgpu_ensure_smem(ctx, mlp_gemm_tc<BN, EPI, 1, BK>, SMEM_BUDGET));
   const int tiles = ((g.M_host + BLOCK_M - 1) / BLOCK_M) * (g.N_pad / BN);
   const int grid = std::min(tiles, ctx->sm_count);
-  NSGPU_CUDA(launch_pdl(ctx, mlp_gemm_tc<BN, EPI>, dim3(grid), dim3(GEMM_THREADS), smem, st, whi, wlo, g));
+  NSGPU_CUDA(launch_pdl(ctx, mlp_gemm_tc<BN, EPI, 1, BK>, dim3(grid), dim3(GEMM_THREADS), smem, st, whi, wlo, g));
   NSGPU_LAUNCH_CHECK();
   return NSGPU_OK;
 }
 
 // Clusters of CS CTAs that share the weight tiles (whi / wlo: tensor maps with boxes of BN / CS rows).
-template <int BN, int EPI, int CS>
+template <int BN, int EPI, int CS, int BK>
 nsgpu_status launch_gemm_cluster(nsgpu_ctx* ctx, const CUtensorMap& whi, const CUtensorMap& wlo, const GemmArgs& g,
                                  cudaStream_t st) {
-  const int smem = num_stages(BN) * stage_bytes(BN) + 16 * num_stages(BN) + 128 + (EPI == 0 ? 16 * g.N_pad : 0) + 1024;
-  NSGPU_CUDA(nsgpu_ensure_smem(ctx, mlp_gemm_tc<BN, EPI, CS>, SMEM_BUDGET));
+  const int smem = num_stages(BN, BK) * stage_bytes(BN, BK) + 16 * num_stages(BN, BK) + 128 + (EPI == 0 ? 16 * g.N_pad : 0) + 1024;
+  NSGPU_CUDA(nsgpu_ensure_smem(ctx, mlp_gemm_tc<BN, EPI, CS, BK>, SMEM_BUDGET));
   const int m_blocks = (g.M_host + BLOCK_M - 1) / BLOCK_M;
   const int items = ((m_blocks + CS - 1) / CS) * (g.N_pad / BN);
   const int clusters = std::min(items, ctx->sm_count / CS);
@@ -610,13 +644,13 @@ nsgpu_status launch_gemm_cluster(nsgpu_ctx* ctx, const CUtensorMap& whi, const C
   attr[1].val.programmaticStreamSerializationAllowed = (ctx->flags & NSGPU_NO_PDL) ? 0 : 1;
   cfg.attrs = attr;
   cfg.numAttrs = 2;
-  NSGPU_CUDA(cudaLaunchKernelEx(&cfg, mlp_gemm_tc<BN, EPI, CS>, whi, wlo, g));
+  NSGPU_CUDA(cudaLaunchKernelEx(&cfg, mlp_gemm_tc<BN, EPI, CS, BK>, whi, wlo, g));
   NSGPU_LAUNCH_CHECK();
   return NSGPU_OK;
 }
 
-template <int EPI>
-nsgpu_status dispatch_gemm(nsgpu_ctx* ctx, const TcLayer& L, const GemmArgs& g, cudaStream_t st) {
+template <int EPI, int BK>
+nsgpu_status dispatch_gemm_bk(nsgpu_ctx* ctx, const TcLayer& L, const GemmArgs& g, cudaStream_t st) {
   // Small batches (few 128-row blocks): narrower tiles so that the grid still covers the SMs.
   if (EPI == 0 && (ctx->flags & NSGPU_MLP_CLUSTER) == 0) {
     const int m_blocks = (g.M_host + BLOCK_M - 1) / BLOCK_M;
@@ -624,8 +658,8 @@ nsgpu_status dispatch_gemm(nsgpu_ctx* ctx, const TcLayer& L, const GemmArgs& g, 
     while (bn > 64 && m_blocks * (g.N_pad / bn) < ctx->sm_count && L.has_s[bn == 256 ? 0 : 1]) bn >>= 1;
     if (bn != L.block_n) {
       const int i = bn == 128 ? 0 : 1;
-      return bn == 128 ? launch_gemm<128, EPI>(ctx, L.tm_whi_s[i], L.tm_wlo_s[i], g, st)
-                       : launch_gemm<64, EPI>(ctx, L.tm_whi_s[i], L.tm_wlo_s[i], g, st);
+      return bn == 128 ? launch_gemm<128, EPI, BK>(ctx, L.tm_whi_s[i], L.tm_wlo_s[i], g, st)
+                       : launch_gemm<64, EPI, BK>(ctx, L.tm_whi_s[i], L.tm_wlo_s[i], g, st);
     }
   }
   // Large batches: CTA pairs share the weight tiles (see mlp_gemm_tc).  Clusters of 4 were measured 50% slower than
@@ -635,15 +669,20 @@ nsgpu_status dispatch_gemm(nsgpu_ctx* ctx, const TcLayer& L, const GemmArgs& g, 
     bool pair = m_blocks_all * (g.N_pad / L.block_n) >= 2 * ctx->sm_count;
     if (ctx->flags & NSGPU_MLP_NO_CLUSTER) pair = false;
     if (ctx->flags & NSGPU_MLP_CLUSTER) pair = true;
-    if (pair) return L.block_n == 256 ? launch_gemm_cluster<256, EPI, 2>(ctx, L.tm_whi_c, L.tm_wlo_c, g, st)
-                                      : launch_gemm_cluster<224, EPI, 2>(ctx, L.tm_whi_c, L.tm_wlo_c, g, st);
+    if (pair) return L.block_n == 256 ? launch_gemm_cluster<256, EPI, 2, BK>(ctx, L.tm_whi_c, L.tm_wlo_c, g, st)
+                                      : launch_gemm_cluster<224, EPI, 2, BK>(ctx, L.tm_whi_c, L.tm_wlo_c, g, st);
   }
   switch (L.block_n) {
-    case 256: return launch_gemm<256, EPI>(ctx, L.tm_whi, L.tm_wlo, g, st);
-    case 224: return launch_gemm<224, EPI>(ctx, L.tm_whi, L.tm_wlo, g, st);
-    case 128: return launch_gemm<128, EPI>(ctx, L.tm_whi, L.tm_wlo, g, st);
-    default: return launch_gemm<64, EPI>(ctx, L.tm_whi, L.tm_wlo, g, st);
+    case 256: return launch_gemm<256, EPI, BK>(ctx, L.tm_whi, L.tm_wlo, g, st);
+    case 224: return launch_gemm<224, EPI, BK>(ctx, L.tm_whi, L.tm_wlo, g, st);
+    case 128: return launch_gemm<128, EPI, BK>(ctx, L.tm_whi, L.tm_wlo, g, st);
+    default: return launch_gemm<64, EPI, BK>(ctx, L.tm_whi, L.tm_wlo, g, st);
   }
+}
+
+template <int EPI>
+nsgpu_status dispatch_gemm(nsgpu_ctx* ctx, const TcLayer& L, const GemmArgs& g, int bk, cudaStream_t st) {
+  return bk == 64 ? dispatch_gemm_bk<EPI, 64>(ctx, L, g, st) : dispatch_gemm_bk<EPI, 32>(ctx, L, g, st);
 }
 
 }  // namespace
@@ -657,6 +696,8 @@ nsgpu_status mlp_tc_prepare(nsgpu_ctx* ctx, int e, const nsgpu_emulator* h) {
   const size_t M_max = (size_t)ctx->max_batch * ctx->rows_per_theta;
   const size_t M_pad = (M_max + BLOCK_M - 1) / BLOCK_M * BLOCK_M;       // api.cu sizes ctx->act for this
   T->M_pad = M_pad;
+  if (const char* ev = getenv("NSGPU_BK")) T->bk = atoi(ev) == 64 ? 64 : 32;
+  if (const char* ev = getenv("NSGPU_KPP")) T->kpp = std::min(std::max(atoi(ev), 1), 16);
   T->layers.resize(nh + 1);
   const float log2e = 1.4426950408889634f;
   for (int l = 0; l <= nh; ++l) {
@@ -686,17 +727,17 @@ nsgpu_status mlp_tc_prepare(nsgpu_ctx* ctx, int e, const nsgpu_emulator* h) {
       NSGPU_CUDA(cudaMalloc((void**)&L.Wlo, lo.size() * sizeof(__half)));
       NSGPU_CUDA(cudaMemcpy(L.Whi, hi.data(), hi.size() * sizeof(__half), cudaMemcpyHostToDevice));
       NSGPU_CUDA(cudaMemcpy(L.Wlo, lo.data(), lo.size() * sizeof(__half), cudaMemcpyHostToDevice));
-      if (!make_tmap(&L.tm_whi, L.Whi, L.N_pad, L.K, L.block_n) || !make_tmap(&L.tm_wlo, L.Wlo, L.N_pad, L.K, L.block_n)) {
+      if (!make_tmap(&L.tm_whi, L.Whi, L.N_pad, L.K, L.block_n, T->bk) || !make_tmap(&L.tm_wlo, L.Wlo, L.N_pad, L.K, L.block_n, T->bk)) {
         ctx->err = "cuTensorMapEncodeTiled failed for a weight plane";
         return NSGPU_ECUDA;
       }
       if (L.block_n == 256 || L.block_n == 224)     // multicast shares: boxes of block_n / 2 rows
-        L.has_c = make_tmap(&L.tm_whi_c, L.Whi, L.N_pad, L.K, L.block_n / 2) && make_tmap(&L.tm_wlo_c, L.Wlo, L.N_pad, L.K, L.block_n / 2);
+        L.has_c = make_tmap(&L.tm_whi_c, L.Whi, L.N_pad, L.K, L.block_n / 2, T->bk) && make_tmap(&L.tm_wlo_c, L.Wlo, L.N_pad, L.K, L.block_n / 2, T->bk);
       if (hidden) {   // narrower boxes over the same planes (N_pad = width is a multiple of 64)
         const int bs[2] = {128, 64};
         for (int i = 0; i < 2; ++i)
-          L.has_s[i] = bs[i] < L.block_n && L.N_pad % bs[i] == 0 && make_tmap(&L.tm_whi_s[i], L.Whi, L.N_pad, L.K, bs[i]) &&
-                       make_tmap(&L.tm_wlo_s[i], L.Wlo, L.N_pad, L.K, bs[i]);
+          L.has_s[i] = bs[i] < L.block_n && L.N_pad % bs[i] == 0 && make_tmap(&L.tm_whi_s[i], L.Whi, L.N_pad, L.K, bs[i], T->bk) &&
+                       make_tmap(&L.tm_wlo_s[i], L.Wlo, L.N_pad, L.K, bs[i], T->bk);
       }
     }
     if (hidden) {
@@ -708,7 +749,7 @@ nsgpu_status mlp_tc_prepare(nsgpu_ctx* ctx, int e, const nsgpu_emulator* h) {
       NSGPU_CUDA(cudaMalloc((void**)&L.p_hidden, p.size() * sizeof(float4)));
       NSGPU_CUDA(cudaMemcpy(L.p_hidden, p.data(), p.size() * sizeof(float4), cudaMemcpyHostToDevice));
     } else {
-      const float cs = ldexpf(1.0f, -(L.wexp + 4)) * TRUNC_COMP;
+      const float cs = ldexpf(1.0f, -(L.wexp + 4)) * trunc_comp(L.K, T->bk, T->kpp);
       // two parameter sets: with mu_out folded in, and without (NSGPU_SPEC_NOMEAN: the consumer adds mu_out
       // in fp64, so that the fp32 table carries only the O(sigma_out) deviation)
       for (int nomean = 0; nomean < 2; ++nomean) {
@@ -774,13 +815,13 @@ nsgpu_status mlp_forward_tc(nsgpu_ctx* ctx, int e, const float* theta, int B, co
     GemmArgs g;
     memset(&g, 0, sizeof(g));
     g.M_host = M; g.n_rows_dev = n_rows_dev; g.rows_per_theta = rpt; g.K = L.K; g.N_pad = L.N_pad; g.n_valid = L.n_valid;
-    g.p_hidden = L.p_hidden; g.p_out = (mode & NSGPU_SPEC_NOMEAN) ? L.p_out_nm : L.p_out; g.p_out4 = (mode & NSGPU_SPEC_NOMEAN) ? L.p_out4_nm : L.p_out4; g.cscale = ldexpf(1.0f, -(L.wexp + 4)) * TRUNC_COMP;
+    g.p_hidden = L.p_hidden; g.p_out = (mode & NSGPU_SPEC_NOMEAN) ? L.p_out_nm : L.p_out; g.p_out4 = (mode & NSGPU_SPEC_NOMEAN) ? L.p_out4_nm : L.p_out4; g.cscale = ldexpf(1.0f, -(L.wexp + 4)) * trunc_comp(L.K, T->bk, T->kpp); g.kpp = T->kpp;
     g.a_hi = T->act[cur][0]; g.a_lo = T->act[cur][1];
     g.out_hi = T->act[cur ^ 1][0]; g.out_lo = T->act[cur ^ 1][1]; g.ld_out = E.width;
     g.out_f32 = spec_out; g.ld_f32 = ld_spec; g.apply_exp10 = (mode & NSGPU_SPEC_EXP10) ? 1 : 0;
     g.out_mode = (mode & NSGPU_SPEC_KZ) ? 1 : 0;
     StageTimer tm(ctx, hidden ? 1 : 2, st);
-    nsgpu_status s = hidden ? dispatch_gemm<0>(ctx, L, g, st) : dispatch_gemm<1>(ctx, L, g, st);
+    nsgpu_status s = hidden ? dispatch_gemm<0>(ctx, L, g, T->bk, st) : dispatch_gemm<1>(ctx, L, g, T->bk, st);
     if (s != NSGPU_OK) return s;
     cur ^= 1;
   }

@@ -154,6 +154,17 @@ __device__ __forceinline__ uint64_t smem_desc_sw128(uint32_t smem_addr) {
   return d;
 }
 
+// The same with 64-byte swizzle: rows of 64 bytes (32 fp16), 8-row groups 512 bytes apart, layout type 4.
+__device__ __forceinline__ uint64_t smem_desc_sw64(uint32_t smem_addr) {
+  uint64_t d = 0;
+  d |= (uint64_t)((smem_addr & 0x3FFFFu) >> 4);
+  d |= (uint64_t)1 << 16;
+  d |= (uint64_t)(512 >> 4) << 32;
+  d |= (uint64_t)1 << 46;
+  d |= (uint64_t)4 << 61;
+  return d;
+}
+
 // Shared-memory matrix descriptor, K-major operand tile WITHOUT swizzle (layout type 0): the tile is
 // made of 8-row x 16-byte core matrices (128 contiguous bytes); `lbo` is the byte distance between
 // core matrices adjacent along K, `sbo` between core matrices adjacent along M/N.
