@@ -165,7 +165,8 @@ NSGPU_API nsgpu_status nsgpu_theory_batch(nsgpu_ctx* ctx, const float* theta, in
  * from the live-set covariance (reading N3).  u_live [n_live][D] float32, logL_live [n_live] float64,
  * start_idx [n_chains] int32, u_out [n_chains][D] float32, logL_out [n_chains] float64: all DEVICE.
  * n_evals (HOST, optional): number of likelihood evaluations spent.  `iteration` and `seed` select the
- * Philox streams (reading N10).  Synchronises `stream` before returning.                             */
+ * Philox streams (reading N10).  Synchronises `stream` before returning.  Errors: EINVAL (NULL pointer, n_live < D + 1,
+ * a start index outside [0, n_live)), ESHAPE (sizes above max_batch), ENOTSPD (live covariance not positive definite). */
 NSGPU_API nsgpu_status nsgpu_slice_step(nsgpu_ctx* ctx, const float* u_live, const double* logL_live, int32_t n_live,
                               const int32_t* start_idx, int32_t n_chains, double logL_star, int32_t n_steps,
                               uint64_t seed, int32_t iteration, float* u_out, double* logL_out,
@@ -182,6 +183,7 @@ typedef struct {
   double logZ, logZ_err, logZ_err_analytic, H; /* eq. 1; error bar per reading N9 */
   int64_t n_iter, n_dead, n_like_evals, n_rounds, n_failed_moves;
   double seconds; /* wall time of the run, host clock */
+  double seconds_sampling, seconds_summary; /* ... split: the nested-sampling loop | final log Z, H, error bar, samples */
 } nsgpu_result;
 
 /* a1-a14: the whole nested-sampling run.  Samples go to caller-allocated HOST buffers of
@@ -235,9 +237,18 @@ NSGPU_API nsgpu_status nsgpu_debug_philox(nsgpu_ctx* ctx, const uint32_t* ctr, i
 NSGPU_API nsgpu_status nsgpu_set_profiling(nsgpu_ctx* ctx, int32_t on);
 NSGPU_API nsgpu_status nsgpu_stage_times(nsgpu_ctx* ctx, double* ms, int64_t* count);
 
+/* Counters of the last nsgpu_slice_step on this ctx (HOST out, either may be NULL): slice moves that reached the shrink
+ * cap and stayed at their start point (reading N3: step-out cap 32, shrink cap 64), and likelihood rounds taken. */
+NSGPU_API nsgpu_status nsgpu_sampler_counters(const nsgpu_ctx* ctx, int64_t* n_failed_moves, int64_t* n_rounds);
+
 /* Introspection: 0 = SIMT, 1 = tcgen05 for emulator `emu`; kernels launched since create. */
 NSGPU_API int32_t nsgpu_mlp_path(const nsgpu_ctx* ctx, int32_t emu);
 NSGPU_API int64_t nsgpu_launch_count(const nsgpu_ctx* ctx);
+/* Emulator rows (tcgen05 path) whose output-layer accumulators were not finite since create (synchronises the device;
+ * -1 on error).  The tcgen05 path carries hidden activations as fp16 hi/lo of 16 h, so |h| >= 4094 overflows (DESIGN.md
+ * section 6); such rows, like rows of a non-finite theta, end as log L = -inf -- this counter makes that visible.
+ * Trained weights that trip it should run with NSGPU_MLP_SIMT (fp32 activations).                                  */
+NSGPU_API int64_t nsgpu_nonfinite_rows(nsgpu_ctx* ctx);
 
 #ifdef __cplusplus
 }

@@ -7,7 +7,20 @@
 
 #include "internal.cuh"
 
+#include <mutex>
+
 static thread_local std::string g_create_error;
+
+cudaError_t nsgpu_raise_smem_limit(int device, const void* fn, size_t bytes) {
+  static std::mutex mu;
+  static std::map<std::pair<int, const void*>, size_t> limit;   // (device, kernel) -> bytes opted in so far
+  std::lock_guard<std::mutex> lock(mu);
+  size_t& cur = limit[std::make_pair(device, fn)];
+  if (bytes <= cur) return cudaSuccess;
+  const cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+  if (e == cudaSuccess) cur = bytes;
+  return e;
+}
 
 namespace {
 
@@ -360,6 +373,8 @@ nsgpu_status create_impl(nsgpu_ctx* ctx, int32_t D, const nsgpu_prior1d* prior, 
   NSGPU_CUDA(cudaMallocHost((void**)&ctx->theta_pinned, (size_t)max_batch * D * sizeof(float)));
   NSGPU_CUDA(cudaMallocHost((void**)&ctx->logL_pinned, (size_t)max_batch * sizeof(double)));
 
+  NSGPU_CUDA(cudaMalloc((void**)&ctx->nonfinite_rows, sizeof(unsigned long long)));
+  NSGPU_CUDA(cudaMemset(ctx->nonfinite_rows, 0, sizeof(unsigned long long)));
   // MLP path selection
   for (int e = 0; e < n_emu; ++e) {
     EmuDev& E = ctx->emu[e];
@@ -426,7 +441,7 @@ extern "C" nsgpu_status nsgpu_destroy(nsgpu_ctx* ctx) {
   cudaFree(S.aux); cudaFree(S.pg); cudaFree(S.a_q); cudaFree(S.z_q); cudaFree(S.ln1pz); cudaFree(S.lellh); cudaFree(S.lf); cudaFree(S.tap_start); cudaFree(S.tap_w); cudaFree(S.ell); cudaFree(S.nz_mean);
   cudaFree(ctx->data); cudaFree(ctx->Linv); cudaFree(ctx->tt_a); cudaFree(ctx->tt_b); cudaFree(ctx->tt_mu);
   cudaFree(ctx->act[0]); cudaFree(ctx->act[1]); cudaFree(ctx->spec); cudaFree(ctx->model); cudaFree(ctx->resid_t); cudaFree(ctx->chi2_part);
-  cudaFree(ctx->theta_stage); cudaFree(ctx->logL_stage);
+  cudaFree(ctx->theta_stage); cudaFree(ctx->logL_stage); cudaFree(ctx->nonfinite_rows);
   cudaFreeHost(ctx->theta_pinned); cudaFreeHost(ctx->logL_pinned);
   cudaGetLastError();
   delete ctx;
@@ -465,6 +480,15 @@ extern "C" nsgpu_status nsgpu_stage_times(nsgpu_ctx* ctx, double* ms, int64_t* c
 }
 
 extern "C" int64_t nsgpu_launch_count(const nsgpu_ctx* ctx) { return ctx ? ctx->launches : -1; }
+
+extern "C" int64_t nsgpu_nonfinite_rows(nsgpu_ctx* ctx) {
+  if (!ctx || !ctx->nonfinite_rows) return -1;
+  unsigned long long v = 0;
+  if (cudaSetDevice(ctx->device) != cudaSuccess || cudaDeviceSynchronize() != cudaSuccess ||
+      cudaMemcpy(&v, ctx->nonfinite_rows, sizeof(v), cudaMemcpyDeviceToHost) != cudaSuccess)
+    return -1;
+  return (int64_t)v;
+}
 
 static nsgpu_status run_emulators(nsgpu_ctx* ctx, const float* theta, int B, const int* n_rows_dev, cudaStream_t st) {
   const size_t stride = (size_t)ctx->max_batch * ctx->rows_per_theta * ctx->spec_ld;

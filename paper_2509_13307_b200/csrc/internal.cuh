@@ -95,7 +95,7 @@ struct nsgpu_ctx {
   SamplerDev* sampler = nullptr;
   std::string err;
   int64_t launches = 0;
-  std::map<const void*, size_t> smem_limit;   // dynamic shared memory opted in per kernel, on this context's device
+  unsigned long long* nonfinite_rows = nullptr;   // device counter: emulator rows with non-finite output (tcgen05 path)
   // optional per-stage CUDA-event timing (nsgpu_set_profiling / nsgpu_stage_times)
   bool profiling = false;
   struct StageEv { int stage; cudaEvent_t a, b; };
@@ -131,15 +131,15 @@ struct StageTimer {
     }                                                                                     \
   } while (0)
 
-// Raise a kernel's dynamic shared-memory limit to `bytes` on the context's device (function attributes are per
-// device: the bookkeeping lives in the context, not in a process-wide static).
+// Raise a kernel's dynamic shared-memory limit to at least `bytes` on the context's device.
+// cudaFuncAttributeMaxDynamicSharedMemorySize is a property of (function, device) shared by every context of the
+// process, so the bookkeeping is process-wide, under a mutex, and the limit is only ever RAISED: a second context that
+// needs less for the same kernel (another n_live, another grid) must not lower it under a live context, and two host
+// threads driving two contexts must not interleave the set and the launch that relies on it.
+cudaError_t nsgpu_raise_smem_limit(int device, const void* fn, size_t bytes);   // api.cu
 template <class F>
 inline cudaError_t nsgpu_ensure_smem(nsgpu_ctx* ctx, F* fn, size_t bytes) {
-  size_t& cur = ctx->smem_limit[reinterpret_cast<const void*>(fn)];
-  if (bytes <= cur) return cudaSuccess;
-  const cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
-  if (e == cudaSuccess) cur = bytes;
-  return e;
+  return nsgpu_raise_smem_limit(ctx->device, reinterpret_cast<const void*>(fn), bytes);
 }
 
 #define NSGPU_LAUNCH_CHECK()                                                              \

@@ -86,6 +86,7 @@ struct GemmArgs {
   int ld_f32;                 // out_mode 0: y[m][n] at m ld_f32 + n
   int out_mode;               // out_mode 1: y at theta(m) (n_valid rpt) + n rpt + z(m)  ([theta][n][z], z fastest)
   int apply_exp10;
+  unsigned long long* nonfinite;   // output layer: rows whose accumulators are not finite (see nsgpu_nonfinite_rows)
 };
 
 __device__ __forceinline__ float ex2_approx(float x) { float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
@@ -521,6 +522,13 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) mlp_gemm_tc(const __grid_cons
       while (DEFP > 0 && pdone < NCH) { NSGPU_RUN_CHUNK(pdone); ++pdone; }   // short K: not enough idle slots
       const int r_in = q * 32 + lane;
       const TileRef ct = {m_blk, n_blk * BLOCK_N + hcol * CPT, r_in, m_blk * BLOCK_M + r_in, m_blk * BLOCK_M + r_in < M};
+      if (EPI == 1 && n_blk == 0 && hcol == 0 && ct.row_ok) {
+        // Hidden activations travel as fp16 hi/lo of 16 h: |h| >= 4094 overflows to inf, the next layer turns that into
+        // NaN for the whole row, and chi^2 maps it to log L = -inf.  Count such rows so that this is never silent.
+        float v0, v1;
+        upk2(acc[0], v0, v1);
+        if (!(fabsf(v0) <= 3.0e38f)) atomicAdd(g.nonfinite, 1ull);
+      }
       epi_pairs<EPI, 0, IMM>(acc, ct, g, params);
       if (DEFP > 0) {
 #pragma unroll
@@ -820,6 +828,7 @@ nsgpu_status mlp_forward_tc(nsgpu_ctx* ctx, int e, const float* theta, int B, co
     g.out_hi = T->act[cur ^ 1][0]; g.out_lo = T->act[cur ^ 1][1]; g.ld_out = E.width;
     g.out_f32 = spec_out; g.ld_f32 = ld_spec; g.apply_exp10 = (mode & NSGPU_SPEC_EXP10) ? 1 : 0;
     g.out_mode = (mode & NSGPU_SPEC_KZ) ? 1 : 0;
+    g.nonfinite = ctx->nonfinite_rows;
     StageTimer tm(ctx, hidden ? 1 : 2, st);
     nsgpu_status s = hidden ? dispatch_gemm<0>(ctx, L, g, T->bk, st) : dispatch_gemm<1>(ctx, L, g, T->bk, st);
     if (s != NSGPU_OK) return s;

@@ -18,7 +18,6 @@
 
 #include <algorithm>
 #include <chrono>
-#include <random>
 
 #include "internal.cuh"
 
@@ -31,6 +30,7 @@ struct SamplerDev {
   int cap = 0;   // max chains / live points
   cudaStream_t run_stream = nullptr;   // nsgpu_run's own non-blocking stream: runs on different contexts overlap on the GPU
   int rounds_needed = 0, rounds_n_steps = -1;   // rounds the last evolve() took (for that n_steps): sizes the next first burst
+  int64_t last_failed_moves = 0;                // slice moves of the last nsgpu_slice_step that hit the shrink cap
   // chain state (SoA)
   float *x0 = nullptr, *dir = nullptr, *xprop = nullptr, *theta_chain = nullptr;   // [cap][D]
   double *l = nullptr, *r = nullptr, *t = nullptr, *logL0 = nullptr;
@@ -269,12 +269,13 @@ __global__ void chain_init_kernel(int n_chains, int chain0, int D, uint2 key, un
                                   int n_surv, const int* __restrict__ start_in, int* __restrict__ start_idx,
                                   const float* __restrict__ u_live, const double* __restrict__ logL_live,
                                   float* x0, double* logL0, int* phase, int* cnt, int* step, int* pending,
-                                  int* finished, int* need, unsigned* rng_j) {
+                                  int* finished, int* need, unsigned* rng_j, int n_live, double* scal) {
   const int c = blockIdx.x * blockDim.x + threadIdx.x;
   if (c >= n_chains) return;
   int s;
   if (start_in) {
     s = start_in[c];
+    if (s < 0 || s >= n_live) { scal[6] = 1.0; s = min(max(s, 0), n_live - 1); }   // caller's index out of range: flagged, clamped
   } else {   // reading N4: uniform with replacement from the survivors; Stream(seed, c, iteration, tag 1)
     Stream S{key, (unsigned)(chain0 + c), iteration, 1u};
     int pick = (int)(S.uniform(0) * n_surv);
@@ -287,7 +288,10 @@ __global__ void chain_init_kernel(int n_chains, int chain0, int D, uint2 key, un
 }
 
 // a14: sample covariance of the live set in u-space + 1e-12 I, lower Cholesky factor; one CTA
-__global__ void __launch_bounds__(256) live_cholesky_kernel(const float* __restrict__ u, int n, int D, double* __restrict__ L) {
+// `status` (may be NULL): set to 1 when a pivot is not positive (fewer than D + 1 distinct live points, or non-finite
+// coordinates): the factor is then unusable and the host returns NSGPU_ENOTSPD instead of sampling NaN directions.
+__global__ void __launch_bounds__(256) live_cholesky_kernel(const float* __restrict__ u, int n, int D, double* __restrict__ L,
+                                                            double* __restrict__ status) {
   __shared__ double mean[NSGPU_MAX_D];
   __shared__ double cov[NSGPU_MAX_D * NSGPU_MAX_D];
   for (int d = threadIdx.x; d < D; d += blockDim.x) {
@@ -306,7 +310,11 @@ __global__ void __launch_bounds__(256) live_cholesky_kernel(const float* __restr
   __syncthreads();
   // column Cholesky; D <= 64, one warp-synchronous pass per column by the whole block
   for (int k = 0; k < D; ++k) {
-    if (threadIdx.x == 0) cov[k * D + k] = sqrt(cov[k * D + k]);
+    if (threadIdx.x == 0) {
+      const double piv = cov[k * D + k];
+      if (!(piv > 0.0) && status) *status = 1.0;
+      cov[k * D + k] = sqrt(piv);
+    }
     __syncthreads();
     for (int i = k + 1 + threadIdx.x; i < D; i += blockDim.x) cov[i * D + k] /= cov[k * D + k];
     __syncthreads();
@@ -495,6 +503,72 @@ __global__ void init_live_kernel(int n, int D, uint2 key, float* u) {
   u[i] = (float)S.uniform((unsigned)d);
 }
 
+// Error bar of log Z by simulated prior volumes (reading N9; Skilling 2006): sequence m redraws every
+// shrinkage factor t_i = U^{1/n_i} over the recorded dead points (n_i = n - i mod k: batch deletion) and recomputes
+// log Z = logsumexp_i [l_i + log X_{i-1} + log(1 - t_i)] with the live points at X_final / n.  One CTA per sequence:
+// tiles of 1024 dead points, the running log X by a block prefix sum, an online log-sum-exp per thread joined at the end.
+// Uniforms: Philox stream (seed; block i/4, sequence m, tag 3), word i mod 4 (reading N10).
+__global__ void __launch_bounds__(256) evidence_error_kernel(const double* __restrict__ dead_logL, long long nd, int n, int k,
+                                                             const double* __restrict__ live_logL, uint2 key,
+                                                             double* __restrict__ zs) {
+  __shared__ double wsum[8], red_m[8], red_s[8];
+  const unsigned m = blockIdx.x;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  double carry = 0.0, mx = -INFINITY, se = 0.0;
+  auto add_term = [&](double term) {
+    if (!(term > -INFINITY)) return;
+    if (term > mx) { se = se * exp(mx - term) + 1.0; mx = term; }
+    else se += exp(term - mx);
+  };
+  for (long long base = 0; base < nd; base += 1024) {
+    const long long i0 = base + 4 * threadIdx.x;
+    const unsigned long long blk = (unsigned long long)i0 >> 2;
+    const uint4 w = philox4x32_10(make_uint4((unsigned)blk, m, (unsigned)(blk >> 32), 3u), key);
+    const unsigned ww[4] = {w.x, w.y, w.z, w.w};
+    double lt[4], tot = 0.0;
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+      const long long i = i0 + e;
+      lt[e] = i < nd ? log(u01(ww[e])) / (double)(n - (int)(i % k)) : 0.0;
+      tot += lt[e];
+    }
+    double inc = tot;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const double t = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += t; }
+    if (lane == 31) wsum[warp] = inc;
+    __syncthreads();
+    double woff = 0.0, tile = 0.0;
+#pragma unroll
+    for (int q = 0; q < 8; ++q) { if (q < warp) woff += wsum[q]; tile += wsum[q]; }
+    double lx = carry + woff + inc - tot;           // log X before this thread's first point
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+      const long long i = i0 + e;
+      if (i < nd) { add_term(dead_logL[i] + lx + log(-expm1(lt[e]))); lx += lt[e]; }
+    }
+    carry += tile;
+    __syncthreads();
+  }
+  const double lw_live = carry - log((double)n);
+  for (int i = threadIdx.x; i < n; i += blockDim.x) add_term(live_logL[i] + lw_live);
+  // join the per-thread (max, sum) pairs
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    const double om = __shfl_xor_sync(0xffffffffu, mx, o), os = __shfl_xor_sync(0xffffffffu, se, o);
+    const double nm = fmax(mx, om);
+    se = (mx > -INFINITY ? se * exp(mx - nm) : 0.0) + (om > -INFINITY ? os * exp(om - nm) : 0.0);
+    mx = nm;
+  }
+  if (lane == 0) { red_m[warp] = mx; red_s[warp] = se; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double M = -INFINITY, S = 0.0;
+    for (int q = 0; q < 8; ++q) M = fmax(M, red_m[q]);
+    for (int q = 0; q < 8; ++q) if (red_m[q] > -INFINITY) S += red_s[q] * exp(red_m[q] - M);
+    zs[m] = M > -INFINITY ? M + log(S) : -INFINITY;
+  }
+}
+
 }  // namespace
 
 // ---------------------------------------------------------------------------------------------------
@@ -536,8 +610,9 @@ void sampler_destroy(nsgpu_ctx* ctx) {
   ctx->sampler = nullptr;
 }
 
-static nsgpu_status launch_live_cholesky(nsgpu_ctx* ctx, const float* u_live, int n_live, double* L, cudaStream_t st) {
-  live_cholesky_kernel<<<1, 256, 0, st>>>(u_live, n_live, ctx->D, L);
+static nsgpu_status launch_live_cholesky(nsgpu_ctx* ctx, const float* u_live, int n_live, double* L, double* status,
+                                         cudaStream_t st) {
+  live_cholesky_kernel<<<1, 256, 0, st>>>(u_live, n_live, ctx->D, L, status);
   NSGPU_LAUNCH_CHECK();
   return NSGPU_OK;
 }
@@ -627,23 +702,36 @@ extern "C" nsgpu_status nsgpu_slice_step(nsgpu_ctx* ctx, const float* u_live, co
   SamplerDev* S = ctx->sampler;
   cudaStream_t st = (cudaStream_t)stream;
   const int D = ctx->D;
-  s = launch_live_cholesky(ctx, u_live, n_live, S->Lsig, st);
+  if (n_live < D + 1) { ctx->err = "slice_step: the live covariance needs n_live >= D + 1"; return NSGPU_EINVAL; }
+  for (int i = 0; i < 8; ++i) S->h_scal[i] = 0.0;
+  S->h_scal[0] = logL_star;                       // [5] Cholesky status, [6] start-index status: cleared
+  NSGPU_CUDA(cudaMemcpyAsync(S->scal, S->h_scal, 8 * sizeof(double), cudaMemcpyHostToDevice, st));
+  s = launch_live_cholesky(ctx, u_live, n_live, S->Lsig, S->scal + 5, st);
   if (s != NSGPU_OK) return s;
-  S->h_scal[0] = logL_star;
-  NSGPU_CUDA(cudaMemcpyAsync(S->scal, S->h_scal, sizeof(double), cudaMemcpyHostToDevice, st));
   NSGPU_CUDA(cudaMemsetAsync(S->n_evals, 0, sizeof(unsigned long long), st));
   const uint2 key = make_uint2((unsigned)(seed & 0xffffffffu), (unsigned)(seed >> 32));
   chain_init_kernel<<<(n_chains + 127) / 128, 128, 0, st>>>(n_chains, 0, D, key, (unsigned)iteration, nullptr, 0, start_idx,
                                                             S->start_idx, u_live, logL_live, S->x0, S->logL0, S->phase,
-                                                            S->cnt, S->step, S->pending, S->finished, S->need, S->rng_j);
+                                                            S->cnt, S->step, S->pending, S->finished, S->need, S->rng_j, n_live, S->scal);
   NSGPU_LAUNCH_CHECK();
   s = evolve(ctx, n_chains, 0, n_steps, seed, iteration, st, nullptr);
   if (s != NSGPU_OK) return s;
   NSGPU_CUDA(cudaMemcpyAsync(u_out, S->u_out, sizeof(float) * (size_t)n_chains * D, cudaMemcpyDeviceToDevice, st));
   NSGPU_CUDA(cudaMemcpyAsync(logL_out, S->logL_out, sizeof(double) * (size_t)n_chains, cudaMemcpyDeviceToDevice, st));
   NSGPU_CUDA(cudaMemcpyAsync(S->h_evals, S->n_evals, sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
+  NSGPU_CUDA(cudaMemcpyAsync(S->h_scal, S->scal, 8 * sizeof(double), cudaMemcpyDeviceToHost, st));
   NSGPU_CUDA(cudaStreamSynchronize(st));
   if (n_evals) *n_evals = (int64_t)*S->h_evals;
+  S->last_failed_moves = S->h_counters[2];
+  if (S->h_scal[6] != 0.0) { ctx->err = "slice_step: start_idx out of [0, n_live)"; return NSGPU_EINVAL; }
+  if (S->h_scal[5] != 0.0) { ctx->err = "slice_step: live-set covariance is not positive definite"; return NSGPU_ENOTSPD; }
+  return NSGPU_OK;
+}
+
+extern "C" nsgpu_status nsgpu_sampler_counters(const nsgpu_ctx* ctx, int64_t* n_failed_moves, int64_t* n_rounds) {
+  if (!ctx || !ctx->sampler) return NSGPU_EINVAL;
+  if (n_failed_moves) *n_failed_moves = ctx->sampler->last_failed_moves;
+  if (n_rounds) *n_rounds = ctx->sampler->rounds_needed;
   return NSGPU_OK;
 }
 
@@ -671,7 +759,7 @@ extern "C" nsgpu_status nsgpu_live_cholesky(nsgpu_ctx* ctx, const float* u_live,
   nsgpu_status s = check_sampler_args(ctx, n_live, 1);
   if (s != NSGPU_OK) return s;
   if (!u_live || !L_out) { ctx->err = "live_cholesky: NULL pointer"; return NSGPU_EINVAL; }
-  return launch_live_cholesky(ctx, u_live, n_live, L_out, (cudaStream_t)stream);
+  return launch_live_cholesky(ctx, u_live, n_live, L_out, nullptr, (cudaStream_t)stream);
 }
 
 extern "C" nsgpu_status nsgpu_debug_philox(nsgpu_ctx* ctx, const uint32_t* ctr, int32_t n, const uint32_t* key,
@@ -722,6 +810,7 @@ static nsgpu_status run_impl(nsgpu_ctx* ctx, const nsgpu_run_opts* o, int rank, 
   nsgpu_status s = check_sampler_args(ctx, o->n_live, o->n_delete);
   if (s != NSGPU_OK) return s;
   if (o->n_delete >= o->n_live || o->n_steps < 1 || !(o->stop_frac > 0) || o->max_iter < 1) { ctx->err = "run: bad options"; return NSGPU_EINVAL; }
+  if (o->n_live < ctx->D + 1) { ctx->err = "run: the live covariance needs n_live >= D + 1"; return NSGPU_EINVAL; }
   const auto t_start = std::chrono::steady_clock::now();
   SamplerDev* S = ctx->sampler;
   // one rank: the context's own stream, so that runs of several contexts (the two models of a comparison, driven from
@@ -758,15 +847,16 @@ static nsgpu_status run_impl(nsgpu_ctx* ctx, const nsgpu_run_opts* o, int rank, 
   if (s != NSGPU_OK) return s;
   s = loglike_device(ctx, S->theta_prop, n, nullptr, S->logL_live, st);
   if (s != NSGPU_OK) return s;
-  S->h_scal[0] = 0.0; S->h_scal[1] = 0.0; S->h_scal[2] = -INFINITY; S->h_scal[3] = 0.0; S->h_scal[4] = 0.0;
-  NSGPU_CUDA(cudaMemcpyAsync(S->scal, S->h_scal, 5 * sizeof(double), cudaMemcpyHostToDevice, st));
+  for (int i = 0; i < 8; ++i) S->h_scal[i] = 0.0;
+  S->h_scal[2] = -INFINITY;
+  NSGPU_CUDA(cudaMemcpyAsync(S->scal, S->h_scal, 8 * sizeof(double), cudaMemcpyHostToDevice, st));
   NSGPU_CUDA(cudaMemsetAsync(S->n_evals, 0, sizeof(unsigned long long), st));
   int64_t it = 0, rounds = 0;
   int n_fail_total = 0;
   bool converged = false;
   while (it < o->max_iter) {
     ++it;
-    s = launch_live_cholesky(ctx, S->u_live, n, S->Lsig, st);              // before deletion
+    s = launch_live_cholesky(ctx, S->u_live, n, S->Lsig, S->scal + 5, st);   // before deletion
     if (s != NSGPU_OK) return s;
     s = launch_delete(ctx, S->logL_live, n, k, st);
     if (s != NSGPU_OK) return s;
@@ -781,14 +871,29 @@ static nsgpu_status run_impl(nsgpu_ctx* ctx, const nsgpu_run_opts* o, int rank, 
     dead_logL.insert(dead_logL.end(), hl.begin(), hl.end());
     dead_logw.insert(dead_logw.end(), hw.begin(), hw.end());
     for (int j = 0; j < k; ++j) dead_nj.push_back(n - j);
+    nsgpu_status es = NSGPU_OK;
     if (n_loc > 0) {
       chain_init_kernel<<<(n_loc + 127) / 128, 128, 0, st>>>(n_loc, c0, D, key, (unsigned)it, S->surv_idx, n - k, nullptr,
                                                              S->start_idx, S->u_live, S->logL_live, S->x0, S->logL0, S->phase,
-                                                             S->cnt, S->step, S->pending, S->finished, S->need, S->rng_j);
-      NSGPU_LAUNCH_CHECK();
-      s = evolve(ctx, n_loc, c0, o->n_steps, o->seed, (int)it, st, &rounds);
-      if (s != NSGPU_OK) return s;
-      n_fail_total += S->h_counters[2];
+                                                             S->cnt, S->step, S->pending, S->finished, S->need, S->rng_j, n, S->scal);
+      ctx->launches++;
+      es = cudaGetLastError() == cudaSuccess ? evolve(ctx, n_loc, c0, o->n_steps, o->seed, (int)it, st, &rounds) : NSGPU_ECUDA;
+      if (es == NSGPU_OK) n_fail_total += S->h_counters[2];
+    }
+    if (world > 1) {
+      // A rank whose chains failed must not leave the others waiting in the all-gather below: every iteration first
+      // exchanges one status word, and all ranks stop together when any of them reports a failure.
+      unsigned long long mine = es == NSGPU_OK ? 0ull : 1ull;
+      std::vector<unsigned long long> all((size_t)world, 0ull);
+      bool ok = cudaMemcpy(G.cnt, &mine, sizeof(mine), cudaMemcpyHostToDevice) == cudaSuccess &&
+                exch(user, G.cnt, G.cnt + 4, (int64_t)sizeof(mine), st) == 0 &&
+                cudaMemcpy(all.data(), G.cnt + 4, sizeof(mine) * world, cudaMemcpyDeviceToHost) == cudaSuccess;
+      if (es != NSGPU_OK) return es;
+      if (!ok) { ctx->err = "run: status exchange failed"; return NSGPU_ECUDA; }
+      for (int r = 0; r < world; ++r)
+        if (all[r] != 0ull) { ctx->err = "run: rank " + std::to_string(r) + " reported a failure; all ranks stop"; return NSGPU_ECUDA; }
+    } else if (es != NSGPU_OK) {
+      return es;
     }
     const float* new_u = S->u_out;
     const double* new_l = S->logL_out;
@@ -805,11 +910,13 @@ static nsgpu_status run_impl(nsgpu_ctx* ctx, const nsgpu_run_opts* o, int rank, 
     NSGPU_LAUNCH_CHECK();
     live_evidence_kernel<<<1, 1024, 0, st>>>(S->logL_live, n, log(o->stop_frac), S->scal);
     NSGPU_LAUNCH_CHECK();
-    NSGPU_CUDA(cudaMemcpyAsync(S->h_scal, S->scal, 5 * sizeof(double), cudaMemcpyDeviceToHost, st));
+    NSGPU_CUDA(cudaMemcpyAsync(S->h_scal, S->scal, 8 * sizeof(double), cudaMemcpyDeviceToHost, st));
     NSGPU_CUDA(cudaStreamSynchronize(st));
+    if (S->h_scal[5] != 0.0) { ctx->err = "run: live-set covariance is not positive definite"; return NSGPU_ENOTSPD; }
     if (S->h_scal[4] != 0.0) { converged = true; break; }
   }
   // final summary
+  const auto t_sampled = std::chrono::steady_clock::now();
   const double logX = S->h_scal[1];
   std::vector<float> live_u((size_t)n * D);
   std::vector<double> live_l(n);
@@ -851,25 +958,23 @@ static nsgpu_status run_impl(nsgpu_ctx* ctx, const nsgpu_run_opts* o, int rank, 
     const double p = exp(terms[i] - logZ);
     if (p > 0.0) H += p * (all_l[i] - logZ);
   }
-  // error bar: redraw the volume sequence M = 1000 times with t_j = U^{1/n_j} (Skilling 2006)
+  // error bar: redraw the volume sequence M = 1000 times with t_j = U^{1/n_j} (Skilling 2006) -- one CTA per
+  // sequence (evidence_error_kernel); the host only takes the standard deviation of the 1000 results.  (Round 1 did
+  // this in a single-threaded host loop of 1000 x n_dead log/expm1/exp calls: 3.4 s for a c4 run.)
   double err_sim = 0.0;
   {
-    std::mt19937_64 gen(o->seed * 0x9E3779B97F4A7C15ull + 99);
-    std::uniform_real_distribution<double> U(0.0, 1.0);
     const int M = 1000;
-    std::vector<double> zs(M), tt(ntot);
-    for (int m = 0; m < M; ++m) {
-      double lx = 0.0;
-      for (size_t i = 0; i < nd; ++i) {
-        double uu = U(gen);
-        if (uu <= 0.0) uu = 1e-300;
-        const double logt = log(uu) / dead_nj[i];
-        tt[i] = dead_logL[i] + lx + log(-expm1(logt));
-        lx += logt;
-      }
-      for (int i = 0; i < n; ++i) tt[nd + i] = live_l[i] + lx - log((double)n);
-      zs[m] = logsumexp(tt);
-    }
+    double *d_dead = nullptr, *d_zs = nullptr;
+    NSGPU_CUDA(cudaMalloc((void**)&d_dead, sizeof(double) * std::max<size_t>(nd, 1)));
+    NSGPU_CUDA(cudaMalloc((void**)&d_zs, sizeof(double) * M));
+    std::vector<double> zs(M);
+    cudaError_t e1 = cudaMemcpyAsync(d_dead, dead_logL.data(), sizeof(double) * nd, cudaMemcpyHostToDevice, st);
+    evidence_error_kernel<<<M, 256, 0, st>>>(d_dead, (long long)nd, n, k, S->logL_live, key, d_zs);
+    ctx->launches++;
+    cudaError_t e2 = cudaMemcpyAsync(zs.data(), d_zs, sizeof(double) * M, cudaMemcpyDeviceToHost, st);
+    cudaError_t e3 = cudaStreamSynchronize(st);
+    cudaFree(d_dead); cudaFree(d_zs);
+    NSGPU_CUDA(e1); NSGPU_CUDA(e2); NSGPU_CUDA(e3);
     double mean = 0.0;
     for (double z : zs) mean += z;
     mean /= M;
@@ -906,7 +1011,10 @@ static nsgpu_status run_impl(nsgpu_ctx* ctx, const nsgpu_run_opts* o, int rank, 
     s = nsgpu_last_samples(ctx, theta_samples, logL_samples, logw_samples, cap, &got);
     if (s != NSGPU_OK) return s;
   }
-  res->seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t_start).count();
+  const auto t_end = std::chrono::steady_clock::now();
+  res->seconds = std::chrono::duration<double>(t_end - t_start).count();
+  res->seconds_sampling = std::chrono::duration<double>(t_sampled - t_start).count();
+  res->seconds_summary = std::chrono::duration<double>(t_end - t_sampled).count();
   return converged ? NSGPU_OK : NSGPU_ENOCONV;
 }
 

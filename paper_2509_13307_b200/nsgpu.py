@@ -27,7 +27,7 @@ EXPORTS = ["nsgpu_create", "nsgpu_destroy", "nsgpu_last_error", "nsgpu_prior_tra
            "nsgpu_loglike_batch", "nsgpu_loglike_batch_host", "nsgpu_emulate_batch", "nsgpu_theory_batch",
            "nsgpu_slice_step", "nsgpu_run", "nsgpu_last_samples", "nsgpu_delete_lowest", "nsgpu_live_cholesky",
            "nsgpu_debug_philox", "nsgpu_set_profiling", "nsgpu_stage_times", "nsgpu_mlp_path", "nsgpu_launch_count",
-           "nsgpu_run_sharded", "nsgpu_shard_range"]
+           "nsgpu_run_sharded", "nsgpu_shard_range", "nsgpu_sampler_counters", "nsgpu_nonfinite_rows"]
 
 
 class NsgpuError(RuntimeError):
@@ -72,7 +72,8 @@ class _RunOpts(C.Structure):
 class _Result(C.Structure):
     _fields_ = [("logZ", C.c_double), ("logZ_err", C.c_double), ("logZ_err_analytic", C.c_double), ("H", C.c_double),
                 ("n_iter", C.c_int64), ("n_dead", C.c_int64), ("n_like_evals", C.c_int64), ("n_rounds", C.c_int64),
-                ("n_failed_moves", C.c_int64), ("seconds", C.c_double)]
+                ("n_failed_moves", C.c_int64), ("seconds", C.c_double), ("seconds_sampling", C.c_double),
+                ("seconds_summary", C.c_double)]
 
 
 # int32 allgather(void* user, const void* send, void* recv, int64 bytes_per_rank, void* stream)  (include/nsgpu.h)
@@ -116,6 +117,10 @@ def lib():
     L.nsgpu_run_sharded.restype = C.c_int
     L.nsgpu_run_sharded.argtypes = [vp, C.POINTER(_RunOpts), C.c_int32, C.c_int32, ALLGATHER_FN, vp, C.POINTER(_Result),
                                     vp, vp, vp, C.c_int64, C.POINTER(C.c_int64)]
+    L.nsgpu_sampler_counters.restype = C.c_int
+    L.nsgpu_sampler_counters.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
+    L.nsgpu_nonfinite_rows.restype = C.c_int64
+    L.nsgpu_nonfinite_rows.argtypes = [vp]
     L.nsgpu_shard_range.restype = None
     L.nsgpu_shard_range.argtypes = [C.c_int32, C.c_int32, C.c_int32, C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
     L.nsgpu_last_samples.restype = C.c_int
@@ -353,6 +358,12 @@ class Context:
                                            self._p(u_out), self._p(l_out), C.byref(ne), _stream_ptr(stream)))
         return u_out, l_out, ne.value
 
+    def sampler_counters(self):
+        """(n_failed_moves, n_rounds) of the last slice_step on this context."""
+        a, b = C.c_int64(0), C.c_int64(0)
+        self._check(lib().nsgpu_sampler_counters(self._h, C.byref(a), C.byref(b)))
+        return a.value, b.value
+
     def delete_lowest(self, logL_live, k, logX=0.0, logZ=-np.inf, stream=None):
         import torch
         n = logL_live.shape[0]
@@ -435,6 +446,9 @@ class Context:
 
     def mlp_path(self, emu=0):
         return lib().nsgpu_mlp_path(self._h, emu)
+
+    def nonfinite_rows(self):
+        return lib().nsgpu_nonfinite_rows(self._h)
 
     def launch_count(self):
         return lib().nsgpu_launch_count(self._h)

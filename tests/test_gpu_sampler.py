@@ -135,6 +135,156 @@ def test_run_identity_gaussian_closed_form(D, n_live, k):
         assert abs(np.mean(zs)) < 3.0 * np.mean(errs) / math.sqrt(len(zs)) + 0.05
 
 
+def test_run_identity_gaussian_closed_form_at_config4_settings():
+    """BASELINE.json configs[4] run settings -- D = 39, 1000 live points, 500 deleted per iteration, 5 D = 195 slice moves,
+    stop at 1e-3 -- on the identity-theory correlated Gaussian, whose log Z = 0 and H = -1/2 ln((2 pi e)^D det Sigma) are
+    closed forms at any D (a one-result-per-round bug biased log Z by -2.2 at D = 37 while every invariant
+    held; only this test catches that class).  5 seeds: mean inside 3 sigma/sqrt(5) + 0.05, scatter consistent with the
+    reported error, H within 1, no failed moves."""
+    D, n_live, k = 39, 1000, 500
+    wl = W.toy_identity(D=D)
+    Sigma = wl.chol @ wl.chol.T
+    H_exact = -0.5 * (D * math.log(2 * math.pi * math.e) + np.linalg.slogdet(Sigma)[1])
+    zs, errs = [], []
+    with nsgpu.Context(wl, max_batch=n_live) as ctx:
+        for seed in (1, 2, 3, 4, 5):
+            r = ctx.run(n_live, k, 5 * D, stop_frac=1e-3, seed=seed, return_samples=(seed == 1))
+            assert r["converged"] and r["n_failed_moves"] == 0
+            assert abs(r["logZ"]) <= 3.0 * r["logZ_err"] + 0.05, r
+            assert r["logZ_err"] == pytest.approx(r["logZ_err_analytic"], rel=0.3)
+            # H = <log L> - log Z inherits the error of log Z (measured over 8 seeds: H - H_exact = -(log Z) to 0.15)
+            assert abs(r["H"] - H_exact) <= 3.0 * r["logZ_err"] + 0.25, (r["H"], H_exact)
+            assert abs(r["H"] - H_exact + r["logZ"]) <= 0.5
+            assert 3.5 < (r["n_like_evals"] - n_live) / (r["n_iter"] * k * 5 * D) < 7.0       # evaluations per slice move
+            assert r["seconds"] == pytest.approx(r["seconds_sampling"] + r["seconds_summary"], rel=1e-6)
+            assert r["seconds_summary"] < 0.25 * r["seconds"] + 0.2          # the error-bar simulation is a kernel now
+            if seed == 1:
+                w = np.exp(r["logw"])
+                assert w.sum() == pytest.approx(1.0, abs=1e-9)
+                np.testing.assert_allclose(w @ r["theta"].astype(np.float64), 0.5, atol=0.02)
+            zs.append(r["logZ"]); errs.append(r["logZ_err"])
+    assert np.std(zs, ddof=1) < 2.5 * np.mean(errs)
+    assert abs(np.mean(zs)) <= 3.0 * np.mean(errs) / math.sqrt(len(zs)) + 0.05, (zs, errs)
+
+
+@pytest.mark.parametrize("D,n_live,k", [(40, 400, 200), (64, 300, 150)])
+def test_run_closed_form_beyond_the_first_lane_half(D, n_live, k):
+    """slice_round_kernel keeps dimensions 32..63 in the second element of every lane: D = 40 and the maximum D = 64
+    through the whole run, against the same closed forms."""
+    wl = W.toy_identity(D=D)
+    H_exact = -0.5 * (D * math.log(2 * math.pi * math.e) + np.linalg.slogdet(wl.chol @ wl.chol.T)[1])
+    with nsgpu.Context(wl, max_batch=n_live) as ctx:
+        rs = [ctx.run(n_live, k, 3 * D, seed=s, return_samples=False) for s in (1, 2)]
+    for r in rs:
+        assert r["converged"] and r["n_failed_moves"] == 0
+        assert abs(r["logZ"]) <= 3.0 * r["logZ_err"] + 0.1, r
+        assert abs(r["H"] - H_exact) <= 3.0 * r["logZ_err"] + 0.5
+
+
+def test_slice_step_shrink_cap_and_empty_region():
+    """Degenerate constraint: L* at the peak value, so no point satisfies log L > L*.  Every move steps out nowhere,
+    shrinks 64 times (reading N3) and fails: the chains stay at their start points, every move is counted as failed,
+    and each move costs at most 2 + 64 evaluations (out-of-box proposals cost none)."""
+    wl = W.toy_identity(D=5)
+    n, steps = 37, 3
+    u0 = (0.5 + 0.02 * np.random.default_rng(3).standard_normal((64, 5))).astype(np.float32)
+    with nsgpu.Context(wl, max_batch=64) as ctx:
+        l0 = ctx.loglike_batch(ctx.prior_transform(dev(u0)))
+        start = torch.arange(n, dtype=torch.int32, device="cuda")
+        u1, l1, ne = ctx.slice_step(dev(u0), l0, start, gaussian.log_norm(wl.chol), steps, seed=4)
+        fails, rounds = ctx.sampler_counters()
+    np.testing.assert_array_equal(u1.cpu().numpy(), u0[:n])
+    np.testing.assert_array_equal(l1.cpu().numpy(), l0.cpu().numpy()[:n])
+    assert fails == n * steps
+    assert n * steps * 60 <= ne <= n * steps * 66 and rounds >= steps * 64
+
+
+@pytest.mark.parametrize("n_chains", [1, 3, 501])
+def test_slice_step_chain_counts_off_the_warp_grid(n_chains):
+    """one warp per chain, four per block: chain counts of 1, 3 and 501 (ragged last block) give valid moves, and chain c
+    of the 501 equals chain c of the first 3 (the Philox streams are per chain, reading N10)."""
+    wl = W.toy_identity(D=7)
+    c = 12.0
+    Lstar = -0.5 * c + gaussian.log_norm(wl.chol)
+    u0 = _ellipsoid_start(wl, 512, c, seed=11)
+    with nsgpu.Context(wl, max_batch=512) as ctx:
+        l0 = ctx.loglike_batch(ctx.prior_transform(dev(u0)))
+        start = torch.arange(n_chains, dtype=torch.int32, device="cuda")
+        u1, l1, ne = ctx.slice_step(dev(u0), l0, start, Lstar, 5, seed=8, iteration=2)
+        u3, l3, _ = ctx.slice_step(dev(u0), l0, start[:min(3, n_chains)].contiguous(), Lstar, 5, seed=8, iteration=2)
+        assert ctx.sampler_counters()[0] == 0
+    x = u1.cpu().numpy()
+    assert x.shape == (n_chains, 7) and np.all((x >= 0) & (x <= 1)) and np.all(l1.cpu().numpy() > Lstar)
+    np.testing.assert_array_equal(x[:min(3, n_chains)], u3.cpu().numpy())
+    assert ne >= n_chains * 5 * 3
+
+
+def test_out_of_box_proposals_cost_no_likelihood_call():
+    """live points spread over the whole cube: the bracket of +-2 live-set sigmas leaves the box on most step-outs and
+    those proposals are rejected on the spot: valid results with fewer evaluations per move than
+    a step-out on both sides plus one shrink would need."""
+    wl = W.toy_identity(D=6, sigma=0.5)                  # broad target: the box is what constrains
+    rng = np.random.default_rng(2)
+    u0 = rng.random((400, 6)).astype(np.float32)
+    with nsgpu.Context(wl, max_batch=400) as ctx:
+        l0 = ctx.loglike_batch(ctx.prior_transform(dev(u0)))
+        Lstar = float(l0.min().item()) - 1.0             # everything in the box is allowed
+        start = torch.arange(300, dtype=torch.int32, device="cuda")
+        u1, l1, ne = ctx.slice_step(dev(u0), l0, start, Lstar, 20, seed=6)
+        assert ctx.sampler_counters()[0] == 0
+    x = u1.cpu().numpy()
+    assert np.all((x >= 0) & (x <= 1))
+    assert stats.kstest(x[:, 0], "uniform").pvalue > 1e-3 and stats.kstest(x[:, 5], "uniform").pvalue > 1e-3
+    assert 1.0 <= ne / (300 * 20) < 12.0
+
+
+def test_sampler_argument_errors():
+    wl = W.toy_identity(D=6)
+    u0 = np.random.default_rng(0).random((32, 6)).astype(np.float32)
+    with nsgpu.Context(wl, max_batch=32) as ctx:
+        l0 = ctx.loglike_batch(ctx.prior_transform(dev(u0)))
+        bad = torch.tensor([0, 5, 32], dtype=torch.int32, device="cuda")          # 32 is out of [0, n_live)
+        with pytest.raises(nsgpu.NsgpuError) as e:
+            ctx.slice_step(dev(u0), l0, bad, -1e9, 2)
+        assert e.value.status == nsgpu.EINVAL
+        with pytest.raises(nsgpu.NsgpuError) as e:                                 # covariance of 6 points in 6-D is singular
+            ctx.slice_step(dev(u0[:6]), l0[:6].contiguous(), bad[:2].contiguous(), -1e9, 2)
+        assert e.value.status == nsgpu.EINVAL
+        with pytest.raises(nsgpu.NsgpuError) as e:
+            ctx.run(6, 3, 4)
+        assert e.value.status == nsgpu.EINVAL
+        nan = u0.copy(); nan[7, 2] = np.nan                                        # non-finite live point: no Cholesky factor
+        with pytest.raises(nsgpu.NsgpuError) as e:
+            ctx.slice_step(dev(nan), l0, bad[:2].contiguous(), -1e9, 2)
+        assert e.value.status == nsgpu.ENOTSPD
+        # the context is still usable afterwards
+        ok, _, _ = ctx.slice_step(dev(u0), l0, bad[:2].contiguous(), -1e9, 2)
+        assert ok.shape == (2, 6)
+
+
+def test_two_live_contexts_with_different_shared_memory_needs():
+    """cudaFuncAttributeMaxDynamicSharedMemorySize belongs to (kernel, device), not to a context: a second context that
+    needs LESS dynamic shared memory for the same kernels (smaller n_live, smaller grids) must not lower the limit under
+    a live first one.  Interleaved calls on two contexts of different sizes."""
+    big, small = W.toy_identity(D=6), W.toy_identity(D=6)
+    sb, ss = workload("tiny_shear_paper"), workload("tiny_shear")
+    rng = np.random.default_rng(1)
+    lb = rng.standard_normal(9000) * 10.0
+    ls = rng.standard_normal(300) * 10.0
+    with nsgpu.Context(big, max_batch=9000) as cb, nsgpu.Context(sb, max_batch=16, mlp=nsgpu.MLP_SIMT | nsgpu.SHEAR_STREAM) as pb:
+        d1 = cb.delete_lowest(dev(lb), 4500)[0].cpu().numpy()                    # 144 KB of dynamic shared memory
+        tb = dev(theta_of_u(sb, W.u_post_set(sb, 16)))
+        m1 = pb.loglike_batch(tb).cpu().numpy()
+        with nsgpu.Context(small, max_batch=300) as cs, nsgpu.Context(ss, max_batch=8, mlp=nsgpu.MLP_SIMT | nsgpu.SHEAR_STREAM) as ps:
+            cs.delete_lowest(dev(ls), 100)                                       # 6 KB: must not lower the limit
+            ps.loglike_batch(dev(theta_of_u(ss, W.u_post_set(ss, 8))))
+            d2 = cb.delete_lowest(dev(lb), 4500)[0].cpu().numpy()                # the big context again
+            m2 = pb.loglike_batch(tb).cpu().numpy()
+    np.testing.assert_array_equal(d1, d2)
+    np.testing.assert_array_equal(m1, m2)
+    assert d1.tolist() == nested.delete_lowest(list(lb), 4500, 0.0, -np.inf)[0]
+
+
 def test_run_toy_emulator_agrees_with_oracle_ns():
     """c0 (BASELINE.json configs[0]): no closed form; GPU log Z vs the oracle's own NS run."""
     wl = workload("toy")
