@@ -241,6 +241,14 @@ NSGPU_API nsgpu_status nsgpu_stage_times(nsgpu_ctx* ctx, double* ms, int64_t* co
  * cap and stayed at their start point (reading N3: step-out cap 32, shrink cap 64), and likelihood rounds taken. */
 NSGPU_API nsgpu_status nsgpu_sampler_counters(const nsgpu_ctx* ctx, int64_t* n_failed_moves, int64_t* n_rounds);
 
+/* SM clock measured on the device between the steps of a timed region (bench.py's `clocks` record).  `mark` enqueues
+ * on `stream` a tiny kernel whose blocks record the cycle counter and the global nanosecond timer of their SM (one
+ * launch, ~3 us, nothing stays resident; at most 512 marks between reads).  `read` synchronises the device and returns,
+ * for each pair of consecutive marks, the mean SM clock in MHz (cycles over time per SM, averaged over the SMs seen in
+ * both) and the end time of the interval in ms since the first mark; HOST [cap], either may be NULL; it clears the marks. */
+NSGPU_API nsgpu_status nsgpu_clock_mark(nsgpu_ctx* ctx, void* stream);
+NSGPU_API nsgpu_status nsgpu_clock_marks_read(nsgpu_ctx* ctx, double* sm_mhz, double* t_ms, int32_t cap, int32_t* n_intervals);
+
 /* Introspection: 0 = SIMT, 1 = tcgen05 for emulator `emu`; kernels launched since create. */
 NSGPU_API int32_t nsgpu_mlp_path(const nsgpu_ctx* ctx, int32_t emu);
 NSGPU_API int64_t nsgpu_launch_count(const nsgpu_ctx* ctx);

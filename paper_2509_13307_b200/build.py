@@ -13,7 +13,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB_DIR = os.path.join(HERE, "lib")
 LIB = os.path.join(LIB_DIR, "libnsgpu.so")
-SOURCES = ["api.cu", "mlp_simt.cu", "mlp_tc.cu", "theory.cu", "gaussian.cu", "sampler.cu"]
+SOURCES = ["api.cu", "mlp_simt.cu", "mlp_tc.cu", "theory.cu", "gaussian.cu", "sampler.cu", "probe.cu"]
 HEADERS = [os.path.join(CSRC, "internal.cuh"), os.path.join(os.path.dirname(HERE), "include", "nsgpu.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "--expt-relaxed-constexpr"]

@@ -424,6 +424,7 @@ extern "C" nsgpu_status nsgpu_create(nsgpu_ctx** out, int32_t D, const nsgpu_pri
 extern "C" nsgpu_status nsgpu_destroy(nsgpu_ctx* ctx) {
   if (!ctx) return NSGPU_EINVAL;
   cudaSetDevice(ctx->device);
+  nsgpu_probe_release(ctx);
   cudaDeviceSynchronize();
   sampler_destroy(ctx);
   for (auto& ev : ctx->stage_events) { cudaEventDestroy(ev.a); cudaEventDestroy(ev.b); }

@@ -93,6 +93,7 @@ struct nsgpu_ctx {
   float* theta_pinned = nullptr;       // pinned host staging
   double* logL_pinned = nullptr;
   SamplerDev* sampler = nullptr;
+  void* probe = nullptr;               // clock probe state (probe.cu)
   std::string err;
   int64_t launches = 0;
   unsigned long long* nonfinite_rows = nullptr;   // device counter: emulator rows with non-finite output (tcgen05 path)
@@ -201,5 +202,6 @@ nsgpu_status chi2_loglike(nsgpu_ctx* ctx, const float* theta, int B, const int* 
                           cudaStream_t st);
 nsgpu_status loglike_device(nsgpu_ctx* ctx, const float* theta, int B, const int* n_rows_dev, double* logL,
                             cudaStream_t st);
+void nsgpu_probe_release(nsgpu_ctx* ctx);
 nsgpu_status sampler_create(nsgpu_ctx* ctx);
 void sampler_destroy(nsgpu_ctx* ctx);

@@ -27,7 +27,8 @@ EXPORTS = ["nsgpu_create", "nsgpu_destroy", "nsgpu_last_error", "nsgpu_prior_tra
            "nsgpu_loglike_batch", "nsgpu_loglike_batch_host", "nsgpu_emulate_batch", "nsgpu_theory_batch",
            "nsgpu_slice_step", "nsgpu_run", "nsgpu_last_samples", "nsgpu_delete_lowest", "nsgpu_live_cholesky",
            "nsgpu_debug_philox", "nsgpu_set_profiling", "nsgpu_stage_times", "nsgpu_mlp_path", "nsgpu_launch_count",
-           "nsgpu_run_sharded", "nsgpu_shard_range", "nsgpu_sampler_counters", "nsgpu_nonfinite_rows"]
+           "nsgpu_run_sharded", "nsgpu_shard_range", "nsgpu_sampler_counters", "nsgpu_nonfinite_rows",
+           "nsgpu_clock_mark", "nsgpu_clock_marks_read"]
 
 
 class NsgpuError(RuntimeError):
@@ -119,6 +120,10 @@ def lib():
                                     vp, vp, vp, C.c_int64, C.POINTER(C.c_int64)]
     L.nsgpu_sampler_counters.restype = C.c_int
     L.nsgpu_sampler_counters.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
+    L.nsgpu_clock_mark.restype = C.c_int
+    L.nsgpu_clock_mark.argtypes = [vp, vp]
+    L.nsgpu_clock_marks_read.restype = C.c_int
+    L.nsgpu_clock_marks_read.argtypes = [vp, _pd, _pd, C.c_int32, C.POINTER(C.c_int32)]
     L.nsgpu_nonfinite_rows.restype = C.c_int64
     L.nsgpu_nonfinite_rows.argtypes = [vp]
     L.nsgpu_shard_range.restype = None
@@ -446,6 +451,16 @@ class Context:
 
     def mlp_path(self, emu=0):
         return lib().nsgpu_mlp_path(self._h, emu)
+
+    def clock_mark(self, stream=None):
+        """enqueue a clock mark on the stream (see nsgpu_clock_mark)"""
+        self._check(lib().nsgpu_clock_mark(self._h, _stream_ptr(stream)))
+
+    def clock_marks_read(self):
+        """(sm_mhz, t_ms) for each interval between consecutive marks; clears the marks."""
+        mhz = np.zeros(512, np.float64); t = np.zeros(512, np.float64); n = C.c_int32(0)
+        self._check(lib().nsgpu_clock_marks_read(self._h, _ptr(mhz, _pd), _ptr(t, _pd), 512, C.byref(n)))
+        return mhz[:n.value], t[:n.value]
 
     def nonfinite_rows(self):
         return lib().nsgpu_nonfinite_rows(self._h)

@@ -30,3 +30,15 @@ def test_two_ranks_weak_scaling_max_over_ranks():
 def test_reference_arm_prints_from_rank0_only():
     lines = _torchrun(["--impl", "reference", "--workload", "c0", "--ref-sample", "8"], 29612)
     assert len(lines) == 1 and lines[0]["impl"] == "reference" and lines[0]["cpu_baseline"]["kind"] == "oracle"
+
+
+def test_gpus_flag_alone_spawns_the_ranks():
+    """`python bench.py --gpus 2` with no torchrun environment must itself start two ranks (round 1 parsed --gpus and
+    ignored it: a driver calling it that way got one rank printing n_gpus 1)."""
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--steps", "3", "--warmup", "1",
+                          "--dry-run-cpu", "--batch", "512"], cwd=ROOT, capture_output=True, text=True, timeout=300, env=env)
+    assert out.returncode == 0, out.stderr[-2000:]
+    lines = [json.loads(l) for l in out.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1 and lines[0]["n_gpus"] == 2 and 19.0 <= lines[0]["ms_per_step"] <= 60.0
+    assert abs(lines[0]["value"] - 2 * 512 * 3 / (lines[0]["ms_per_step"] * 3 * 1e-3)) < 1e-6 * lines[0]["value"]
