@@ -127,6 +127,10 @@ typedef struct {
 #define NSGPU_MLP_CLUSTER 32u    /* tcgen05 GEMMs: CTA pairs that multicast the weight tiles, whatever the batch (default: large batches) */
 #define NSGPU_MLP_NO_CLUSTER 64u /* ... never */
 #define NSGPU_SHEAR_STREAM 4u /* kind 3: use the streaming projection kernels even where the grids fit shared memory */
+#define NSGPU_MLP_FUSED 256u   /* tcgen05 path: one persistent kernel for all layers (CTA pairs own row blocks, activations in an
+                                * L2-resident scratch) wherever the shape allows it (width 512, even n_hidden, n_in 6/7/9);
+                                * bit-identical to the layered path; opt-in (measured no faster: profiles/r2_fused_mlp.md) */
+#define NSGPU_MLP_LAYERED 512u /* one kernel per layer, activations through HBM (the default) */
 #define NSGPU_NO_PDL 128u /* launch every kernel with plain stream ordering (default: the kernels of a likelihood call and of a
                             * slice-sampling round are chained by programmatic dependent launch) */
 

@@ -441,7 +441,7 @@ extern "C" nsgpu_status nsgpu_destroy(nsgpu_ctx* ctx) {
   ShearDev& S = ctx->sh;
   cudaFree(S.aux); cudaFree(S.pg); cudaFree(S.a_q); cudaFree(S.z_q); cudaFree(S.ln1pz); cudaFree(S.lellh); cudaFree(S.lf); cudaFree(S.tap_start); cudaFree(S.tap_w); cudaFree(S.ell); cudaFree(S.nz_mean);
   cudaFree(ctx->data); cudaFree(ctx->Linv); cudaFree(ctx->tt_a); cudaFree(ctx->tt_b); cudaFree(ctx->tt_mu);
-  cudaFree(ctx->act[0]); cudaFree(ctx->act[1]); cudaFree(ctx->spec); cudaFree(ctx->model); cudaFree(ctx->resid_t); cudaFree(ctx->chi2_part);
+  cudaFree(ctx->act[0]); cudaFree(ctx->act[1]); cudaFree(ctx->fused_scratch); cudaFree(ctx->spec); cudaFree(ctx->model); cudaFree(ctx->resid_t); cudaFree(ctx->chi2_part);
   cudaFree(ctx->theta_stage); cudaFree(ctx->logL_stage); cudaFree(ctx->nonfinite_rows);
   cudaFreeHost(ctx->theta_pinned); cudaFreeHost(ctx->logL_pinned);
   cudaGetLastError();

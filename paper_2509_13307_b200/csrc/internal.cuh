@@ -82,6 +82,7 @@ struct nsgpu_ctx {
   double *tt_a = nullptr, *tt_b = nullptr, *tt_mu = nullptr;   // kind 4: (nu/2) ln 10 and nu Chat / 2 per multipole
   // workspaces
   void* act[2] = {nullptr, nullptr};   // [M_max][width] fp32 (SIMT) or 2 x fp16 (tcgen05)
+  void* fused_scratch = nullptr;       // fused MLP kernel: per-cluster activation scratch (L2-resident), shared by the emulators
   float* spec = nullptr;               // [n_emu][M_max][spec_ld] de-standardised y (log10 where exp10)
   int spec_ld = 0;                     // row stride: n_out, rounded up to 4 floats for one-row-per-theta tables (16-byte stores)
   bool spec_kz = false;                // shear + tcgen05: per theta [n_k][n_z_emu] instead of [n_z_emu][n_k]

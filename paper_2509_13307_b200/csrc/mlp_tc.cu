@@ -236,7 +236,9 @@ __global__ void __launch_bounds__(256) mlp_first_layer_tc(const float* __restric
 // row: EPI 0 bias + gated activation + hi/lo split into the next layer's canonical planes; EPI 1 de-standardised
 // fp32 output (row-major, or [theta][n][z] for the shear table).
 struct TileRef { int m_blk, n0, r_in, row; bool row_ok; };
-template <int EPI, int P0, int NP>
+// OUT_MODE >= 0 fixes g.out_mode at compile time and drops the 10^y code (the fused kernel: half the epilogue code, and
+// no exp10f inlined 200 times -- its emulate tap applies 10^y in a pass of its own)
+template <int EPI, int P0, int NP, int OUT_MODE = -1>
 __device__ __forceinline__ void epi_pairs(const f32x2* a, const TileRef& t, const GemmArgs& g, const float* params) {
   static_assert(P0 % 4 == 0 && NP % 4 == 0, "whole 16-byte pieces");
   const int n0 = t.n0 + 2 * P0;                                  // first column of this slice
@@ -261,7 +263,8 @@ __device__ __forceinline__ void epi_pairs(const f32x2* a, const TileRef& t, cons
   } else {
     const float4* p4 = g.p_out4 + (n0 >> 1);                       // warp-uniform addresses: L1 broadcast
     const int rr = t.row_ok ? t.row : 0;
-    if (g.out_mode == 1) {
+    const bool exp10_on = OUT_MODE < 0 && g.apply_exp10;
+    if (OUT_MODE < 0 ? g.out_mode == 1 : OUT_MODE == 1) {
       // [theta][n][z] with z fastest: consecutive rows (lanes) of one theta are contiguous
       const int th = rr / g.rows_per_theta, zi = rr - th * g.rows_per_theta;
       float* dst = g.out_f32 + (size_t)th * ((size_t)g.n_valid * g.rows_per_theta) + zi;
@@ -270,7 +273,7 @@ __device__ __forceinline__ void epi_pairs(const f32x2* a, const TileRef& t, cons
         const float4 pj = __ldg(p4 + j);                           // {s1_0, s1_1, s0_0, s0_1}
         float y0, y1;
         upk2(fma2(a[j], pk2(pj.x, pj.y), pk2(pj.z, pj.w)), y0, y1);
-        if (g.apply_exp10) { y0 = exp10f(y0); y1 = exp10f(y1); }
+        if (exp10_on) { y0 = exp10f(y0); y1 = exp10f(y1); }
         const int n = n0 + 2 * j;
         if (t.row_ok && n < g.n_valid) dst[(size_t)n * g.rows_per_theta] = y0;
         if (t.row_ok && n + 1 < g.n_valid) dst[(size_t)(n + 1) * g.rows_per_theta] = y1;
@@ -284,7 +287,7 @@ __device__ __forceinline__ void epi_pairs(const f32x2* a, const TileRef& t, cons
         const float4 pa = __ldg(p4 + 2 * c), pb = __ldg(p4 + 2 * c + 1);
         upk2(fma2(a[2 * c], pk2(pa.x, pa.y), pk2(pa.z, pa.w)), y[0], y[1]);
         upk2(fma2(a[2 * c + 1], pk2(pb.x, pb.y), pk2(pb.z, pb.w)), y[2], y[3]);
-        if (g.apply_exp10) {
+        if (exp10_on) {
 #pragma unroll
           for (int j = 0; j < 4; ++j) y[j] = exp10f(y[j]);
         }
@@ -547,6 +550,362 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) mlp_gemm_tc(const __grid_cons
   if (warp == EPI_WARPS + 1) tc::tmem_dealloc(tmem_base, 512);
 }
 
+// =====================================================================================================
+// Fused multi-layer kernel: a CTA pair owns 128-row blocks through ALL layers ("fused MLP").
+//
+// The layered path launches one kernel per layer and round-trips every activation plane through HBM (2 KB per row and
+// layer each way: 2.5 GB of the 3.85 GB a c3a step moved in round 1) and pays a launch boundary per layer (40% of a
+// nested-sampling round at B ~ 300-500).  Here a cluster of two CTAs takes row blocks cl, cl + NC, ... and carries
+// each of them from theta to the spectrum table: CTA `crank` computes column half `crank` of every hidden layer (the
+// first one on the CUDA cores, the others on the tensor cores exactly as mlp_gemm_tc does: same k-block order, same
+// partials, same epilogue arithmetic, so the results are bit-identical to the layered path) and every second column
+// block of the output layer.  Activations live in a per-cluster scratch in global memory -- two slots (row blocks in
+// flight) x two buffers (layer in / layer out) x 256 KB, 74 MB for 74 clusters -- that is rewritten for every row block
+// and therefore stays in the 126 MB L2.  Layers are separated by an mbarrier both CTAs arrive on (`ready[slot]`), not
+// by a grid-wide barrier.  Two row blocks are interleaved (A1 B1 A2 B2 ...): the epilogue of (A, l) runs while the
+// tensor core works on (B, l), and (A, l + 1) starts as soon as both halves of (A, l) are stored.
+//
+// ready[slot] completes once per (group, layer 0 .. n_layers-1) after 2 x 8 warp arrivals (both CTAs' epilogue warps,
+// each after its last store of that layer's output, fence.proxy.async, release at cluster scope); the TMA producer
+// waits for it (acquire at cluster scope) before the first bulk copy of the next layer's A operand.  The first layer
+// of the NEXT group is computed by the epilogue warps in the gaps between TMEM drains, after ready[slot] has
+// completed for layer n_layers-1 of the current group (the last reader of that buffer, in both CTAs).
+// =====================================================================================================
+constexpr int FUSED_BN_H = 256;
+constexpr int FUSED_STAGES = 2;
+constexpr int FUSED_STAGE = stage_bytes(256, 64);       // 96 KB: room for the widest tile (output tiles use less)
+constexpr int FUSED_MAX_GEMM = 6;                       // GEMM layers (n_hidden) the argument block holds
+constexpr int FL_UNIT_PIECES = 4;                       // first layer: 16-byte pieces per work unit and warp
+constexpr int FL_UNITS = 16 / FL_UNIT_PIECES;           // a warp owns 16 of the CTA's 32 pieces
+
+struct FusedArgs {
+  int M_host;
+  const int* n_rows_dev;
+  int rows_per_theta;
+  int n_layers;               // GEMM layers = n_hidden: layers 1 .. n_layers-1 hidden, layer n_layers the output
+  // first layer (a2 + layer 0)
+  const float* theta; int D; const int* emu_in_idx; const double* emu_in_const; int n_theta_in; const float* z_emu;
+  const float* in_mean; const float* in_std; const float* W0;
+  const float4* p_hidden[FUSED_MAX_GEMM];   // per-column parameters of layers 0 .. n_layers-1 (global, [512])
+  float cscale[FUSED_MAX_GEMM + 1];         // GEMM layer l = 1 .. n_layers
+  // output layer
+  const float4* p_out4; int n_blocks_out; int n_valid;
+  float* out_f32; int ld_f32; int out_mode; int apply_exp10;
+  unsigned long long* nonfinite;
+  __half* scratch;            // [clusters][2 slots][2 buffers][hi, lo][128 x 512]
+};
+struct FusedMaps { CUtensorMap hi[FUSED_MAX_GEMM], lo[FUSED_MAX_GEMM]; };   // index l - 1 for GEMM layer l
+
+// One unit of the first layer for row block `rb`: FL_UNIT_PIECES 16-byte pieces (8 neurons each) of this warp's share of
+// the CTA's column half, for the 32 rows of the warp's quarter.  Same arithmetic, in the same order, as
+// mlp_first_layer_tc.
+template <int NIN>
+__device__ __forceinline__ void fused_first_layer_unit(const FusedArgs& f, int rb, int unit, int M, int crank, int warp, int lane,
+                                                       const float* sW0, const float4* sp0, __half* out_hi, __half* out_lo) {
+  const int r = (warp & 3) * 32 + lane;
+  const int m = min(rb * BLOCK_M + r, M - 1);
+  const int th = m / f.rows_per_theta, zi = m - th * f.rows_per_theta;
+  f32x2 x2[NIN];
+#pragma unroll
+  for (int c = 0; c < NIN; ++c) {
+    float v;
+    if (c < f.n_theta_in) {
+      const int src = f.emu_in_idx[c];
+      v = src >= 0 ? f.theta[(size_t)th * f.D + src] : (float)f.emu_in_const[c];
+    } else {
+      v = f.z_emu[zi];
+    }
+    v = (v - f.in_mean[c]) / f.in_std[c];
+    x2[c] = pk2(v, v);
+  }
+  const f32x2 one2 = pk2(1.0f, 1.0f);
+  const int p_first = (warp >> 2) * 16 + unit * FL_UNIT_PIECES;            // piece within the CTA's half (0 .. 31)
+#pragma unroll 1
+  for (int pp = 0; pp < FL_UNIT_PIECES; ++pp) {
+    const int p = p_first + pp;
+    uint32_t hi[4], lo[4];
+    f32x2 t[4] = {0ull, 0ull, 0ull, 0ull};
+#pragma unroll
+    for (int c = 0; c < NIN; ++c) {
+      const float4 wlo = *reinterpret_cast<const float4*>(sW0 + c * FUSED_BN_H + 8 * p);
+      const float4 whi = *reinterpret_cast<const float4*>(sW0 + c * FUSED_BN_H + 8 * p + 4);
+      t[0] = fma2(x2[c], pk2(wlo.x, wlo.y), t[0]); t[1] = fma2(x2[c], pk2(wlo.z, wlo.w), t[1]);
+      t[2] = fma2(x2[c], pk2(whi.x, whi.y), t[2]); t[3] = fma2(x2[c], pk2(whi.z, whi.w), t[3]);
+    }
+#pragma unroll
+    for (int jj = 0; jj < 4; ++jj) act_split_pair(t[jj], one2, sp0[8 * p + 2 * jj], sp0[8 * p + 2 * jj + 1], hi[jj], lo[jj]);
+    const size_t o = (size_t)(32 * crank + p) * PIECE_HALVES + (size_t)r * 8;
+    *reinterpret_cast<uint4*>(out_hi + o) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
+    *reinterpret_cast<uint4*>(out_lo + o) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
+  }
+}
+
+
+struct FusedCtx {             // what the epilogue helpers of mlp_fused_tc need besides the tile state
+  uint32_t ready0;
+  int lane, warp, crank, cl, NC, nl, M;
+  __half* scr;
+  const float* sW0;
+  const float4* sparams;
+};
+
+// this warp's stores of one layer of one row block are done: arrive on ready[slot] of both CTAs
+__device__ __forceinline__ void fused_signal_ready(const FusedCtx& fc, int slot) {
+  tc::fence_proxy_async_all();
+  __syncwarp();
+  if (fc.lane == 0) { tc::mbar_arrive_cluster(fc.ready0 + 8 * slot, 0); tc::mbar_arrive_cluster(fc.ready0 + 8 * slot, 1); }
+}
+
+// First layer of the row block of group g that goes into slot s (this CTA's column half, this warp's share).  Called only
+// where no accumulators are live: before the first tile, and at the end of a tile.
+template <int NIN>
+__device__ __forceinline__ void fused_run_first_layer(const FusedArgs& f, const FusedCtx& fc, int s, int g) {
+  constexpr size_t PLANE = (size_t)BLOCK_M * 2 * FUSED_BN_H;
+  if (g > 0)      // buffer 0 of the slot was last read by layer nl - 1 of group g - 1, in both CTAs
+    tc::mbar_wait_cluster(fc.ready0 + 8 * s, (uint32_t)(((g - 1) * fc.nl + fc.nl - 1) & 1));
+  __half* o_hi = fc.scr + (size_t)(s * 2) * (2 * PLANE);
+#pragma unroll 1
+  for (int u = 0; u < FL_UNITS; ++u)
+    fused_first_layer_unit<NIN>(f, fc.cl + (2 * g + s) * fc.NC, u, fc.M, fc.crank, fc.warp, fc.lane, fc.sW0, fc.sparams, o_hi, o_hi + PLANE);
+  fused_signal_ready(fc, s);
+}
+
+__global__ void exp10_inplace_kernel(float* y, size_t n) {
+  for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) y[i] = exp10f(y[i]);
+}
+
+template <int BN_O, int NIN, int OUT_MODE>
+__global__ void __launch_bounds__(GEMM_THREADS, 1) mlp_fused_tc(const __grid_constant__ FusedMaps tm, const FusedArgs f) {
+  constexpr int BK = 64, A_TILE_BYTES = a_tile_bytes(BK);
+  constexpr int STAGES = FUSED_STAGES, STAGE = FUSED_STAGE;
+  constexpr int WIDTH = 2 * FUSED_BN_H;
+  constexpr int NPB = 2, PB_COLS = 256;
+  constexpr uint32_t IDESC_H = tc::idesc_f16_f32(BLOCK_M, FUSED_BN_H), IDESC_O = tc::idesc_f16_f32(BLOCK_M, BN_O);
+  constexpr size_t PLANE = (size_t)BLOCK_M * WIDTH;            // halves per plane of a row block
+  static_assert(BN_O % 32 == 0 && BN_O <= 256, "output tile width");
+
+  extern __shared__ unsigned char smem_dyn[];
+  const uint32_t base = (tc::smem_u32(smem_dyn) + 1023u) & ~1023u;
+  unsigned char* base_ptr = smem_dyn + (base - tc::smem_u32(smem_dyn));
+  const uint32_t bars = base + STAGES * STAGE;
+  const uint32_t full0 = bars, empty0 = bars + 16, pfull0 = bars + 32, pempty0 = bars + 48, ready0 = bars + 64;
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(base_ptr + STAGES * STAGE + 96);
+  float4* sparams = reinterpret_cast<float4*>(base_ptr + STAGES * STAGE + 128);      // [n_layers][256] (layer 0 first)
+  float* sW0 = reinterpret_cast<float*>(sparams + f.n_layers * FUSED_BN_H);          // [NIN][256]
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int crank = (int)tc::cluster_ctarank();
+  const int c0 = crank * FUSED_BN_H;                               // first column of this CTA's half of a hidden layer
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < STAGES; ++s) { tc::mbar_init(full0 + 8 * s, 1); tc::mbar_init(empty0 + 8 * s, 1); }
+    for (int b = 0; b < NPB; ++b) { tc::mbar_init(pfull0 + 8 * b, 1); tc::mbar_init(pempty0 + 8 * b, EPI_WARPS); }
+    for (int s = 0; s < 2; ++s) tc::mbar_init(ready0 + 8 * s, 2 * EPI_WARPS);
+    tc::fence_barrier_init();
+  }
+  if (warp == EPI_WARPS + 1) tc::tmem_alloc(tc::smem_u32(tmem_slot), 512);
+  if (warp == EPI_WARPS && lane == 0)
+    for (int l = 0; l < f.n_layers; ++l) { tc::prefetch_tmap(&tm.hi[l]); tc::prefetch_tmap(&tm.lo[l]); }
+  // constants: the per-column parameters of this CTA's half of every hidden layer, and its half of W0
+  for (int l = 0; l < f.n_layers; ++l)
+    for (int i = threadIdx.x; i < FUSED_BN_H / 2; i += blockDim.x) {
+      const float4 a = f.p_hidden[l][c0 + 2 * i], b = f.p_hidden[l][c0 + 2 * i + 1];
+      sparams[l * FUSED_BN_H + 2 * i] = make_float4(a.x, b.x, a.y, b.y);
+      sparams[l * FUSED_BN_H + 2 * i + 1] = make_float4(a.z, b.z, a.w, b.w);
+    }
+  for (int i = threadIdx.x; i < NIN * FUSED_BN_H; i += blockDim.x) {
+    const int c = i / FUSED_BN_H, j = i - c * FUSED_BN_H;
+    sW0[i] = f.W0[c * WIDTH + c0 + j];
+  }
+  pdl_wait();
+  pdl_trigger();
+  tc::fence_before_sync();
+  __syncthreads();
+  tc::cluster_sync();          // both CTAs' barriers exist before the peer's first arrive reaches them
+  tc::fence_after_sync();
+  const uint32_t tmem_base = *tmem_slot;
+  int M = f.M_host;
+  if (f.n_rows_dev) M = min(M, (*f.n_rows_dev) * f.rows_per_theta);
+  const int m_blocks = (M + BLOCK_M - 1) / BLOCK_M;
+  const int cl = blockIdx.x >> 1, NC = gridDim.x >> 1;
+  const int n_rb = cl < m_blocks ? (m_blocks - cl + NC - 1) / NC : 0;   // row blocks cl, cl + NC, ... of this cluster
+  const int n_groups = (n_rb + 1) >> 1;
+  const int nl = f.n_layers;
+  __half* const scr = f.scratch + (size_t)cl * (8 * PLANE);            // [slot][buffer][hi, lo][PLANE]
+  auto buf_hi = [&](int slot, int b) -> __half* { return scr + (size_t)(slot * 2 + b) * (2 * PLANE); };
+
+  if (warp >= EPI_WARPS) {
+    // registers: the producer and MMA threads walk a five-deep loop nest with 64-bit descriptors and pointers: with the 40
+    // registers mlp_gemm_tc leaves them they spilled into local memory on the MMA issue path (ncu: 1.2 M local loads per
+    // launch from single lanes).  56 here, 224 for the epilogue warps: what the third warpgroup gives up ((168 - 56) x 128
+    // registers) is exactly what the two epilogue warpgroups take ((224 - 168) x 256); asking for more never returns.
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");
+    if (warp == EPI_WARPS) {
+      // ===== TMA producer =====
+      if (lane == 0) {
+        uint32_t stage = 0, phase = 0;
+        for (int g = 0; g < n_groups; ++g) {
+          const int ns = min(2, n_rb - 2 * g);
+          for (int l = 1; l <= nl; ++l)
+            for (int s = 0; s < ns; ++s) {
+              const bool is_out = l == nl;
+              const int n_nb = is_out ? f.n_blocks_out : 2, bn = is_out ? BN_O : FUSED_BN_H;
+              // layer l - 1 of this row block is complete in both CTAs (completion g nl + l - 1 of ready[s])
+              tc::mbar_wait_cluster(ready0 + 8 * s, (uint32_t)((g * nl + l - 1) & 1));
+              tc::fence_proxy_async_all();
+              const __half* a_hi = buf_hi(s, (l - 1) & 1);
+              const __half* a_lo = a_hi + PLANE;
+              const uint32_t bytes = 2 * A_TILE_BYTES + 2 * bn * 128;
+              for (int nb = crank; nb < n_nb; nb += 2)
+#pragma unroll 1
+                for (int kb = 0; kb < WIDTH / BK; ++kb) {
+                  tc::mbar_wait(empty0 + 8 * stage, phase ^ 1);
+                  const uint32_t s0 = base + stage * STAGE, fb = full0 + 8 * stage;
+                  tc::mbar_arrive_expect_tx(fb, bytes);
+                  const size_t a_off = (size_t)kb * 8 * PIECE_HALVES;
+                  tc::bulk_load(s0, a_hi + a_off, A_TILE_BYTES, fb);
+                  tc::bulk_load(s0 + A_TILE_BYTES, a_lo + a_off, A_TILE_BYTES, fb);
+                  tc::tma_load_2d(s0 + 2 * A_TILE_BYTES, &tm.hi[l - 1], kb * BK, nb * bn, fb);
+                  tc::tma_load_2d(s0 + 2 * A_TILE_BYTES + bn * 128, &tm.lo[l - 1], kb * BK, nb * bn, fb);
+                  if (++stage == STAGES) { stage = 0; phase ^= 1; }
+                }
+            }
+        }
+      }
+    } else if (warp == EPI_WARPS + 1) {
+      // ===== MMA issuer: one fresh TMEM partial per k-block, as in mlp_gemm_tc =====
+      if (lane == 0) {
+        uint32_t stage = 0, phase = 0, pcount = 0;
+        for (int g = 0; g < n_groups; ++g) {
+          const int ns = min(2, n_rb - 2 * g);
+          for (int l = 1; l <= nl; ++l)
+            for (int s = 0; s < ns; ++s) {
+              const bool is_out = l == nl;
+              const int n_nb = is_out ? f.n_blocks_out : 2, bn = is_out ? BN_O : FUSED_BN_H;
+              const uint32_t idesc = is_out ? IDESC_O : IDESC_H;
+              for (int nb = crank; nb < n_nb; nb += 2)
+#pragma unroll 1
+                for (int kb = 0; kb < WIDTH / BK; ++kb, ++pcount) {
+                  const uint32_t pb = pcount % NPB, pphase = (pcount / NPB) & 1;
+                  tc::mbar_wait(pempty0 + 8 * pb, pphase ^ 1);
+                  tc::mbar_wait(full0 + 8 * stage, phase);
+                  tc::fence_after_sync();
+                  const uint32_t d_tmem = tmem_base + pb * PB_COLS;
+                  const uint32_t s0 = base + stage * STAGE;
+                  const uint64_t a_hi = tc::smem_desc_nosw(s0, 2048, 128), a_lo = tc::smem_desc_nosw(s0 + A_TILE_BYTES, 2048, 128);
+                  const uint64_t b_hi = tc::smem_desc_sw128(s0 + 2 * A_TILE_BYTES);
+                  const uint64_t b_lo = tc::smem_desc_sw128(s0 + 2 * A_TILE_BYTES + bn * 128);
+#pragma unroll
+                  for (int k = 0; k < BK / 16; ++k) {
+                    const uint64_t adv_a = (uint64_t)(256 * k), adv_b = (uint64_t)(2 * k);
+                    tc::mma_f16_ss(d_tmem, a_lo + adv_a, b_hi + adv_b, idesc, k != 0);
+                    tc::mma_f16_ss(d_tmem, a_hi + adv_a, b_lo + adv_b, idesc, 1);
+                  }
+#pragma unroll
+                  for (int k = 0; k < BK / 16; ++k) {
+                    const uint64_t adv_a = (uint64_t)(256 * k), adv_b = (uint64_t)(2 * k);
+                    tc::mma_f16_ss(d_tmem, a_hi + adv_a, b_hi + adv_b, idesc, 1);
+                  }
+                  tc::mma_commit(empty0 + 8 * stage);
+                  tc::mma_commit(pfull0 + 8 * pb);
+                  if (++stage == STAGES) { stage = 0; phase ^= 1; }
+                }
+            }
+        }
+      }
+    }
+  } else {
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 224;");
+    // ===== epilogue warps: drains + epilogues of the GEMM tiles, and the first layer of the row blocks to come =====
+    const int q = warp & 3, hcol = warp >> 2;
+    const int r_in = q * 32 + lane;
+    uint32_t pcount = 0;
+    int armed[2] = {-1, -1};                       // group whose first layer may be computed into slot s (-1: none)
+    FusedCtx fc;
+    fc.ready0 = ready0; fc.lane = lane; fc.warp = warp; fc.crank = crank; fc.cl = cl; fc.NC = NC; fc.nl = nl; fc.M = M;
+    fc.scr = scr; fc.sW0 = sW0; fc.sparams = sparams;
+    if (n_rb > 0) fused_run_first_layer<NIN>(f, fc, 0, 0);
+    if (n_rb > 1) fused_run_first_layer<NIN>(f, fc, 1, 0);
+
+// One GEMM tile on the epilogue side: pull the eight k-block partials out of TMEM into registers (round-to-nearest
+// sums), then bias + activation + split (hidden) or de-standardisation (output) and the stores.  No deferred columns
+// here (mlp_gemm_tc parks the last 64 of a tile): the next layer of this row block waits for exactly these stores.
+#define NSGPU_FUSED_TILE(EPI_, BN_, PARAMS_, CS_, OHI_, OLO_, TREF_, SLOT_)                                          \
+  do {                                                                                                              \
+    constexpr int CPT = BN_ / (EPI_WARPS / 4), NPAIR = CPT / 2, LDC = (CPT % 16 == 0) ? 16 : 8;                     \
+    _Pragma("unroll 1") for (int kb = 0; kb < WIDTH / BK; ++kb, ++pcount) {                                         \
+      const uint32_t pb = pcount % NPB, pphase = (pcount / NPB) & 1;                                                \
+      tc::mbar_wait(pfull0 + 8 * pb, pphase);                                                                       \
+      tc::fence_after_sync();                                                                                       \
+      const uint32_t t_src = tmem_base + pb * PB_COLS + ((uint32_t)(q * 32) << 16) + hcol * CPT;                    \
+      constexpr int NLD = CPT / LDC, DB = 2;                                                                        \
+      _Pragma("unroll") for (int c0_ = 0; c0_ < NLD; c0_ += DB) {                                                   \
+        uint32_t r[DB][LDC];                                                                                        \
+        _Pragma("unroll") for (int b = 0; b < DB; ++b)                                                              \
+          if (c0_ + b < NLD) tc::tmem_ld_cols(t_src + LDC * (c0_ + b), r[b]);                                       \
+        tc::tmem_ld_wait();                                                                                         \
+        _Pragma("unroll") for (int b = 0; b < DB; ++b) {                                                            \
+          if (c0_ + b >= NLD) continue;                                                                             \
+          const int c = c0_ + b;                                                                                    \
+          if (kb == 0) {                                                                                            \
+            _Pragma("unroll") for (int j = 0; j < LDC / 2; ++j)                                                     \
+              acc[(LDC / 2) * c + j] = pk2(__uint_as_float(r[b][2 * j]), __uint_as_float(r[b][2 * j + 1]));         \
+          } else {                                                                                                  \
+            _Pragma("unroll") for (int j = 0; j < LDC / 2; ++j)                                                     \
+              acc[(LDC / 2) * c + j] = add2(acc[(LDC / 2) * c + j], pk2(__uint_as_float(r[b][2 * j]), __uint_as_float(r[b][2 * j + 1]))); \
+          }                                                                                                         \
+        }                                                                                                           \
+      }                                                                                                             \
+      tc::fence_before_sync();                                                                                      \
+      __syncwarp();                                                                                                 \
+      if (lane == 0) tc::mbar_arrive(pempty0 + 8 * pb);                                                             \
+    }                                                                                                               \
+    const TileRef ct = TREF_;                                                                                       \
+    GemmArgs g_;                                                                                                    \
+    g_.rows_per_theta = f.rows_per_theta; g_.n_valid = f.n_valid; g_.p_out4 = f.p_out4; g_.ld_out = WIDTH;          \
+    g_.out_f32 = f.out_f32; g_.ld_f32 = f.ld_f32; g_.out_mode = OUT_MODE; g_.apply_exp10 = 0;                       \
+    g_.cscale = CS_; g_.out_hi = OHI_; g_.out_lo = OLO_;                                                            \
+    if (EPI_ == 1 && ct.n0 == 0 && ct.row_ok) {                                                                     \
+      float v0, v1;                                                                                                 \
+      upk2(acc[0], v0, v1);                                                                                         \
+      if (!(fabsf(v0) <= 3.0e38f)) atomicAdd(f.nonfinite, 1ull);                                                    \
+    }                                                                                                               \
+    epi_pairs<EPI_, 0, NPAIR, OUT_MODE>(acc, ct, g_, PARAMS_);                                                      \
+    if (EPI_ == 0) fused_signal_ready(fc, SLOT_);                                                                   \
+    /* first layer of the row block that takes a slot next, armed by an EARLIER tile */                            \
+    _Pragma("unroll") for (int s_ = 0; s_ < 2; ++s_)                                                                \
+      if (armed[s_] >= 0) { fused_run_first_layer<NIN>(f, fc, s_, armed[s_]); armed[s_] = -1; }                     \
+  } while (0)
+
+    f32x2 acc[FUSED_BN_H / 4];                     // one accumulator row segment: 128 columns (hidden), BN_O / 2 (output)
+    for (int g = 0; g < n_groups; ++g) {
+      const int ns = min(2, n_rb - 2 * g);
+      for (int l = 1; l <= nl; ++l)
+        for (int s = 0; s < ns; ++s) {
+          const int rb = cl + (2 * g + s) * NC;
+          if (l < nl) {
+            __half* o_hi = buf_hi(s, l & 1);
+            __half* o_lo = o_hi + PLANE;
+            const float* prm = reinterpret_cast<const float*>(sparams + l * FUSED_BN_H) - 4 * c0;
+            // hidden tile: m_blk 0 (the scratch holds one row block), columns c0 + hcol CPT ..
+            NSGPU_FUSED_TILE(0, FUSED_BN_H, prm, f.cscale[l], o_hi, o_lo,
+                             (TileRef{0, c0 + hcol * CPT, r_in, rb * BLOCK_M + r_in, rb * BLOCK_M + r_in < M}), s);
+            // the first layer of the row block that takes this slot next may start once layer nl - 1 here is done
+            if (l == nl - 1 && 2 * (g + 1) + s < n_rb) armed[s] = g + 1;
+          } else {
+            for (int nb = crank; nb < f.n_blocks_out; nb += 2)
+              NSGPU_FUSED_TILE(1, BN_O, nullptr, f.cscale[l], nullptr, nullptr,
+                               (TileRef{rb, nb * BN_O + hcol * CPT, r_in, rb * BLOCK_M + r_in, rb * BLOCK_M + r_in < M}), s);
+          }
+        }
+    }
+#undef NSGPU_FUSED_TILE
+  }
+  tc::fence_before_sync();
+  __syncthreads();
+  tc::cluster_sync();
+  if (warp == EPI_WARPS + 1) tc::tmem_dealloc(tmem_base, 512);
+}
+
 }  // namespace
 
 // ---------------------------------------------------------------------------------------------------
@@ -571,6 +930,8 @@ struct TcState {
   std::vector<TcLayer> layers;               // index = layer 0 .. n_hidden (layer 0 uses p_hidden only)
   __half* act[2][2] = {};                    // [buffer][hi, lo] canonical-layout planes
   size_t M_pad = 0;
+  bool fused_ok = false;                     // shapes the fused multi-layer kernel takes (mlp_fused_tc)
+  FusedMaps fmaps;
   // k-block (64 or 32 columns) and k-blocks per TMEM partial.  Measured (profiles/r2_gemm_pipeline_ab.md): four stages of
   // 32 columns are no faster than two of 64 (the kernel is bound by the chip's power cap, not by operand latency), and
   // every further k-block in a partial costs precision (more truncating accumulations) for 3-5% of time.  NSGPU_BK /
@@ -775,6 +1136,21 @@ nsgpu_status mlp_tc_prepare(nsgpu_ctx* ctx, int e, const nsgpu_emulator* h) {
       }
     }
   }
+  // fused multi-layer kernel: width 512 (one 256-column tile per CTA of a pair), an even number of GEMM layers, the
+  // input counts the BASELINE configurations use, output tiles of 224 or 256 columns, default k-block / partial sizes
+  {
+    const TcLayer& Lo = T->layers[nh];
+    T->fused_ok = width == 2 * FUSED_BN_H && nh % 2 == 0 && nh >= 2 && nh <= FUSED_MAX_GEMM && T->bk == 64 && T->kpp == 1 &&
+                  (h->n_in == 6 || h->n_in == 7 || h->n_in == 9) && (Lo.block_n == 224 || Lo.block_n == 256);
+    if (T->fused_ok) {
+      for (int l = 1; l <= nh; ++l) { T->fmaps.hi[l - 1] = T->layers[l].tm_whi; T->fmaps.lo[l - 1] = T->layers[l].tm_wlo; }
+      if (!ctx->fused_scratch) {
+        const size_t bytes = (size_t)(ctx->sm_count / 2) * 8 * BLOCK_M * width * sizeof(__half);   // 1 MB per cluster
+        NSGPU_CUDA(cudaMalloc(&ctx->fused_scratch, bytes));
+        NSGPU_CUDA(cudaMemset(ctx->fused_scratch, 0, bytes));
+      }
+    }
+  }
   for (int i = 0; i < 2; ++i) {
     T->act[i][0] = reinterpret_cast<__half*>(ctx->act[i]);
     T->act[i][1] = T->act[i][0] + M_pad * width;
@@ -792,6 +1168,79 @@ void mlp_tc_release(nsgpu_ctx* ctx, int e) {
   ctx->emu[e].tmaps = nullptr;
 }
 
+
+namespace {
+
+// The fused kernel is OPT-IN (NSGPU_MLP_FUSED).  Measured on B200, c3a (profiles/r2_fused_mlp.md): bit-identical to the
+// layered path and half its DRAM traffic, but not faster -- MLP 1.48 vs 1.29 ms at B = 4096 (96 KB of L2 reads per
+// k-block and CTA without weight multicast, against 64 KB: the L2 -> SM limit; no deferred epilogue), equal at B = 512,
+// 9% better at B = 256, and 2% slower inside a nested-sampling run (rounds of ~300 proposals).
+bool use_fused(const nsgpu_ctx* ctx, const TcState* T, int M) {
+  (void)M;
+  return T->fused_ok && (ctx->flags & NSGPU_MLP_FUSED) != 0 && (ctx->flags & NSGPU_MLP_LAYERED) == 0;
+}
+
+template <int BN_O, int NIN, int OUT_MODE>
+nsgpu_status launch_fused(nsgpu_ctx* ctx, const TcState* T, const FusedArgs& f, int smem, cudaStream_t st) {
+  NSGPU_CUDA(nsgpu_ensure_smem(ctx, mlp_fused_tc<BN_O, NIN, OUT_MODE>, (size_t)smem));
+  const int m_blocks = (f.M_host + BLOCK_M - 1) / BLOCK_M;
+  const int clusters = std::min(m_blocks, ctx->sm_count / 2);
+  cudaLaunchConfig_t cfg;
+  memset(&cfg, 0, sizeof(cfg));
+  cfg.gridDim = dim3(clusters * 2);
+  cfg.blockDim = dim3(GEMM_THREADS);
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = st;
+  cudaLaunchAttribute attr[2];
+  attr[0].id = cudaLaunchAttributeClusterDimension;
+  attr[0].val.clusterDim.x = 2; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+  attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[1].val.programmaticStreamSerializationAllowed = (ctx->flags & NSGPU_NO_PDL) ? 0 : 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 2;
+  NSGPU_CUDA(cudaLaunchKernelEx(&cfg, mlp_fused_tc<BN_O, NIN, OUT_MODE>, T->fmaps, f));
+  NSGPU_LAUNCH_CHECK();
+  return NSGPU_OK;
+}
+
+nsgpu_status mlp_forward_fused(nsgpu_ctx* ctx, const EmuDev& E, TcState* T, const float* theta, int M, const int* n_rows_dev,
+                               float* spec_out, int ld_spec, int mode, cudaStream_t st) {
+  const int nh = E.n_hidden;
+  FusedArgs f;
+  memset(&f, 0, sizeof(f));
+  f.M_host = M; f.n_rows_dev = n_rows_dev; f.rows_per_theta = ctx->rows_per_theta; f.n_layers = nh;
+  f.theta = theta; f.D = ctx->D; f.emu_in_idx = ctx->emu_in_idx; f.emu_in_const = ctx->emu_in_const;
+  f.n_theta_in = ctx->n_theta_in; f.z_emu = ctx->z_emu; f.in_mean = E.in_mean; f.in_std = E.in_std; f.W0 = E.W[0];
+  for (int l = 0; l < nh; ++l) f.p_hidden[l] = T->layers[l].p_hidden;
+  for (int l = 1; l <= nh; ++l) f.cscale[l] = ldexpf(1.0f, -(T->layers[l].wexp + 4)) * trunc_comp(T->layers[l].K, T->bk, T->kpp);
+  const TcLayer& Lo = T->layers[nh];
+  f.p_out4 = (mode & NSGPU_SPEC_NOMEAN) ? Lo.p_out4_nm : Lo.p_out4;
+  f.n_blocks_out = Lo.N_pad / Lo.block_n; f.n_valid = Lo.n_valid;
+  f.out_f32 = spec_out; f.ld_f32 = ld_spec; f.out_mode = (mode & NSGPU_SPEC_KZ) ? 1 : 0; f.apply_exp10 = (mode & NSGPU_SPEC_EXP10) ? 1 : 0;
+  f.nonfinite = ctx->nonfinite_rows;
+  f.scratch = reinterpret_cast<__half*>(ctx->fused_scratch);
+  const int smem = FUSED_STAGES * FUSED_STAGE + 128 + nh * FUSED_BN_H * (int)sizeof(float4) + E.n_in * FUSED_BN_H * (int)sizeof(float) + 1024;
+  nsgpu_status rs = NSGPU_ESHAPE;
+  {
+    StageTimer tm(ctx, 1, st);                     // the whole MLP is one launch: booked under the hidden-layer stage
+#define NSGPU_FUSED_CASE(BN_, NIN_)                                                                       \
+  if (Lo.block_n == BN_ && E.n_in == NIN_)                                                                \
+    rs = f.out_mode ? launch_fused<BN_, NIN_, 1>(ctx, T, f, smem, st) : launch_fused<BN_, NIN_, 0>(ctx, T, f, smem, st)
+    NSGPU_FUSED_CASE(224, 6); NSGPU_FUSED_CASE(224, 7); NSGPU_FUSED_CASE(224, 9);
+    NSGPU_FUSED_CASE(256, 6); NSGPU_FUSED_CASE(256, 7); NSGPU_FUSED_CASE(256, 9);
+#undef NSGPU_FUSED_CASE
+  }
+  if (rs != NSGPU_OK) return rs;
+  if (mode & NSGPU_SPEC_EXP10) {                   // emulate tap: 10^y as a pass of its own (same exp10f, same bits)
+    const size_t n = (size_t)M * ld_spec;
+    exp10_inplace_kernel<<<(unsigned)std::min<size_t>((n + 255) / 256, 65535), 256, 0, st>>>(spec_out, n);
+    NSGPU_LAUNCH_CHECK();
+  }
+  return NSGPU_OK;
+}
+
+}  // namespace
+
 nsgpu_status mlp_forward_tc(nsgpu_ctx* ctx, int e, const float* theta, int B, const int* n_rows_dev, float* spec_out,
                             int ld_spec, int mode, cudaStream_t st) {
   const EmuDev& E = ctx->emu[e];
@@ -799,6 +1248,7 @@ nsgpu_status mlp_forward_tc(nsgpu_ctx* ctx, int e, const float* theta, int B, co
   const int rpt = ctx->rows_per_theta;
   const int M = B * rpt;
   if (M == 0) return NSGPU_OK;
+  if (use_fused(ctx, T, M)) return mlp_forward_fused(ctx, E, T, theta, M, n_rows_dev, spec_out, ld_spec, mode, st);
   int cur = 0;
   {
     StageTimer tm(ctx, 0, st);

@@ -3,8 +3,9 @@ synccheck; one tool per GPU call, B200_PROFILING.md) and for quick checks after 
 
     compute-sanitizer --tool memcheck python -m paper_2509_13307_b200.examples.sanitizer_case
 
-  1. c3a (39-D shear, 512-wide emulator, 50 z nodes) at B = 64: first layer, tcgen05 GEMMs as single CTAs and -- forced
-     with NSGPU_MLP_CLUSTER -- as CTA pairs that multicast the weight tiles, resident projection, DMMA chi^2;
+  1. c3a (39-D shear, 512-wide emulator, 50 z nodes) at B = 64: first layer, tcgen05 GEMMs as single CTAs, -- forced
+     with NSGPU_MLP_CLUSTER -- as CTA pairs that multicast the weight tiles, and as the fused multi-layer kernel (all
+     three must agree bit for bit), resident projection, DMMA chi^2;
   2. a width-64 shear model with the streaming projection kernels and the tiled chi^2;
   3. the CMB binning path (three emulators) and the cosmic-variance TT likelihood at small sizes;
   4. a short nested-sampling run (slice rounds, compaction, deletion + evidence scan, live covariance, error-bar kernel).
@@ -32,11 +33,12 @@ def main():
     wl = _attach(W.c3a())
     u = torch.as_tensor(np.concatenate([W.u_post_set(wl, 32), W.u_prior_set(wl, 32)]).astype(np.float32), device="cuda")
     res = []
-    for flags in (nsgpu.MLP_TC | nsgpu.MLP_NO_CLUSTER, nsgpu.MLP_TC | nsgpu.MLP_CLUSTER):
+    for flags in (nsgpu.MLP_TC | nsgpu.MLP_LAYERED | nsgpu.MLP_NO_CLUSTER, nsgpu.MLP_TC | nsgpu.MLP_LAYERED | nsgpu.MLP_CLUSTER,
+                  nsgpu.MLP_TC | nsgpu.MLP_FUSED):
         with nsgpu.Context(wl, max_batch=64, mlp=flags) as ctx:
             res.append(ctx.loglike_batch(ctx.prior_transform(u)).cpu().numpy())
-    assert np.all(np.isfinite(res[0])) and np.array_equal(res[0], res[1])
-    out["c3a_B64_pairs_equal_single"] = True
+    assert np.all(np.isfinite(res[0])) and np.array_equal(res[0], res[1]) and np.array_equal(res[0], res[2])
+    out["c3a_B64_pairs_and_fused_equal_single"] = True
     ws = _attach(W.shear(seed=22, w0wa=True, n_z_emu=11, n_z=11, width=64, n_hidden=2, n_k=40, n_chi=150, n_ell=11, n_tomo=5,
                          z_max=3.0, n_ia_terms=1, n_m_terms=2, name="s64p"), nsgpu.SHEAR_STREAM)
     us = torch.as_tensor(W.u_post_set(ws, 40).astype(np.float32), device="cuda")

@@ -302,6 +302,30 @@ def test_weight_multicast_pairs_are_bit_identical(name, B):
     assert np.isfinite(res[0][1]).all()
 
 
+@pytest.mark.parametrize("name,B", [("c3a", 1), ("c3a", 23), ("c3a", 700), ("c3a", 1111), ("c1", 129), ("c1", 3000), ("c2", 385),
+                                    ("c3b", 64), ("cmb_tt", 200)])
+def test_fused_mlp_is_bit_identical_to_the_layered_path(name, B):
+    """The fused multi-layer kernel (a CTA pair carries a 128-row block through all layers, activations in an
+    L2-resident scratch) does the arithmetic of the layered kernels in the same order: same bits, for one
+    row block, for fewer row blocks than clusters, for ragged tails, for clusters with one and with several groups of row
+    blocks, for output layers of one column block per CTA (c2/c3: 2 x 224) and of five (c1: 10 x 256)."""
+    wl = workload(name)
+    theta = theta_of_u(wl, np.concatenate([W.u_post_set(wl, B // 2), W.u_prior_set(wl, B - B // 2)]))
+    res = []
+    for flag in (nsgpu.MLP_LAYERED, nsgpu.MLP_FUSED):
+        with nsgpu.Context(wl, max_batch=B, mlp=nsgpu.MLP_TC | flag) as ctx:
+            spec = ctx.emulate_batch(dev(theta), 0).cpu().numpy()
+            ll = ctx.loglike_batch(dev(theta)).cpu().numpy()
+            ll2 = ctx.loglike_batch(dev(theta)).cpu().numpy()             # the scratch is reused: same result again
+            n_launch = ctx.launch_count()
+            res.append((spec, ll, ll2, n_launch))
+    np.testing.assert_array_equal(res[1][0], res[0][0])
+    np.testing.assert_array_equal(res[1][1], res[0][1])
+    np.testing.assert_array_equal(res[1][2], res[1][1])
+    assert np.isfinite(res[0][1]).all()
+    assert res[1][3] < res[0][3]                                          # one launch instead of one per layer
+
+
 def test_tensor_core_and_simt_paths_agree_on_shear():
     """the two on-device MLP paths (different table layouts into the projection) give the same log L"""
     wl = W.shear(seed=21, w0wa=True, n_z_emu=9, n_z=9, width=64, n_hidden=2, n_k=40, n_chi=24, n_ell=6, n_tomo=3, name="s64")
