@@ -200,6 +200,17 @@ typedef struct {
 NSGPU_API nsgpu_status nsgpu_run(nsgpu_ctx* ctx, const nsgpu_run_opts* opts, nsgpu_result* res, float* theta_samples,
                        double* logL_samples, double* logw_samples, int64_t cap, int64_t* n_samples);
 
+/* n_runs independent runs (seeds[r] replaces opts->seed) of the SAME model that share every likelihood batch: a single run
+ * carries <= n_delete proposals per round and leaves the GPU half idle ("perfect scaling is hard to achieve"); here
+ * the chains of all runs advance in the same rounds, each with its own L*, direction factor, Philox key and stopping test,
+ * so res[r] (HOST [n_runs]) is exactly what nsgpu_run returns for seeds[r] (bit for bit; n_rounds and the wall times are
+ * those of the shared loop).  Needs n_runs * n_delete <= max_batch.  Samples of run r: nsgpu_multi_samples (same buffers
+ * and meaning as nsgpu_last_samples).  Returns NSGPU_ENOCONV if any run hit max_iter.  Blocking.                     */
+NSGPU_API nsgpu_status nsgpu_run_multi(nsgpu_ctx* ctx, const nsgpu_run_opts* opts, int32_t n_runs, const uint64_t* seeds,
+                                       nsgpu_result* res);
+NSGPU_API nsgpu_status nsgpu_multi_samples(nsgpu_ctx* ctx, int32_t run, float* theta_samples, double* logL_samples,
+                                           double* logw_samples, int64_t cap, int64_t* n_samples);
+
 /* Multi-GPU nested sampling: one process per GPU, every rank holds the whole
  * live set and calls this with the same options.  Rank r evolves the chains nsgpu_shard_range gives it; the only
  * exchange of an iteration is an all-gather of the k new points, done through `allgather`: send and recv are DEVICE

@@ -59,6 +59,8 @@ struct SamplerDev {
   // samples of the last nsgpu_run (host): theta [n][D], logL [n], logw [n]
   std::vector<float> last_theta;
   std::vector<double> last_logL, last_logw;
+  struct SampleSet { std::vector<float> theta; std::vector<double> logL, logw; };
+  std::vector<SampleSet> multi;        // samples of the runs of the last nsgpu_run_multi
 };
 
 namespace {
@@ -120,6 +122,14 @@ struct RoundArgs {
   int* counters;
   float* u_out;
   double* logL_out;
+  // several runs of one model sharing every round (nsgpu_run_multi): chain c belongs to run c / n_per_run and is its chain
+  // c % n_per_run; per run: scal + 8 run (L*), Lsig + D D run, keys[run], iters[run], counters evals[run] / fails[run].
+  // n_per_run = 0: one run, the scalar fields above.
+  int n_per_run;
+  const uint2* keys;
+  const unsigned* iters;
+  unsigned long long* run_evals;
+  int* run_fails;
 };
 
 // a11 + a12: one warp per chain; consume last round's likelihood, advance the slice state machine to the
@@ -142,8 +152,11 @@ __global__ void __launch_bounds__(128) slice_round_kernel(RoundArgs a) {
   double l = a.l[c], r = a.r[c], t = a.t[c], logL0 = a.logL0[c];
   int phase = a.phase[c], cnt = a.cnt[c], step = a.step[c];
   unsigned j = a.rng_j[c];
-  const double Lstar = a.scal[0];
-  Stream S{a.key, (unsigned)(a.chain0 + c), a.iteration, 0u};
+  const int run = a.n_per_run ? c / a.n_per_run : 0;
+  const int lc = c - run * a.n_per_run;                          // chain index within its run (= c for one run)
+  const double Lstar = a.scal[8 * run];
+  const double* Lsig = a.Lsig + (size_t)run * D * D;
+  Stream S{a.n_per_run ? a.keys[run] : a.key, (unsigned)(a.chain0 + lc), a.n_per_run ? a.iters[run] : a.iteration, 0u};
   bool inside = false;
   double val = 0.0;
   if (a.pending[c]) {
@@ -182,8 +195,8 @@ __global__ void __launch_bounds__(128) slice_round_kernel(RoundArgs a) {
       double acca = 0.0, accb = 0.0;
       for (int jj = 0; jj < D; ++jj) {
         const double zj = __shfl_sync(0xffffffffu, jj < 32 ? za : zb, jj & 31);
-        if (v0 && jj <= d0) acca += a.Lsig[(size_t)d0 * D + jj] * zj;
-        if (v1 && jj <= d1) accb += a.Lsig[(size_t)d1 * D + jj] * zj;
+        if (v0 && jj <= d0) acca += Lsig[(size_t)d0 * D + jj] * zj;
+        if (v1 && jj <= d1) accb += Lsig[(size_t)d1 * D + jj] * zj;
       }
       const double inv = 1.0 / sqrt(nn);
       da = (float)(acca * inv); db = (float)(accb * inv);
@@ -213,6 +226,10 @@ __global__ void __launch_bounds__(128) slice_round_kernel(RoundArgs a) {
     a.phase[c] = phase; a.cnt[c] = cnt; a.step[c] = step; a.rng_j[c] = j;
     a.pending[c] = emit ? 1 : 0;
     a.need[c] = emit ? 1 : 0;
+    if (a.n_per_run) {
+      if (emit) atomicAdd(&a.run_evals[run], 1ull);
+      if (fails) atomicAdd(&a.run_fails[run], fails);
+    }
     if (fails) atomicAdd(&a.counters[2], fails);
     if (done) { a.finished[c] = 1; a.logL_out[c] = logL0; atomicAdd(&a.counters[1], 1); }
   }
@@ -617,21 +634,28 @@ static nsgpu_status launch_live_cholesky(nsgpu_ctx* ctx, const float* u_live, in
   return NSGPU_OK;
 }
 
-static nsgpu_status launch_delete(nsgpu_ctx* ctx, const double* logL, int n, int k, cudaStream_t st) {
+static nsgpu_status launch_delete(nsgpu_ctx* ctx, const double* logL, int n, int k, cudaStream_t st, double* scal = nullptr,
+                                  int* dead_idx = nullptr, int* surv_idx = nullptr, double* logw = nullptr) {
   SamplerDev* S = ctx->sampler;
+  if (!scal) { scal = S->scal; dead_idx = S->dead_idx; surv_idx = S->surv_idx; logw = S->logw; }
   int np2 = 1;
   while (np2 < n) np2 <<= 1;
   const size_t smem = (size_t)np2 * (sizeof(double) + sizeof(int));
   NSGPU_CUDA(nsgpu_ensure_smem(ctx, delete_lowest_kernel, smem));
-  delete_lowest_kernel<<<1, 1024, smem, st>>>(logL, n, k, S->scal, S->dead_idx, S->surv_idx, S->logw);
+  delete_lowest_kernel<<<1, 1024, smem, st>>>(logL, n, k, scal, dead_idx, surv_idx, logw);
   NSGPU_LAUNCH_CHECK();
   return NSGPU_OK;
 }
 
 // Evolve n_chains chains to completion.  Chains were initialised by chain_init_kernel; Lsig and scal[0]
 // (L*) are set.  Host reads the finished-counter after batches of rounds (one small D2H per batch).
+struct MultiArgs {           // device arrays of nsgpu_run_multi (see RoundArgs)
+  int n_per_run, n_target;   // chains per run; chains that will finish (active runs x n_per_run)
+  const uint2* keys; const unsigned* iters; unsigned long long* run_evals; int* run_fails; const double* scal; const double* Lsig;
+};
+
 static nsgpu_status evolve(nsgpu_ctx* ctx, int n_chains, int chain0, int n_steps, uint64_t seed, int iteration, cudaStream_t st,
-                           int64_t* rounds_out) {
+                           int64_t* rounds_out, const MultiArgs* multi = nullptr) {
   SamplerDev* S = ctx->sampler;
   RoundArgs a;
   a.n_chains = n_chains; a.D = ctx->D; a.n_steps = n_steps; a.chain0 = chain0;
@@ -643,6 +667,10 @@ static nsgpu_status evolve(nsgpu_ctx* ctx, int n_chains, int chain0, int n_steps
   a.phase = S->phase; a.cnt = S->cnt; a.step = S->step; a.pending = S->pending; a.finished = S->finished; a.need = S->need;
   a.rng_j = S->rng_j; a.row_of_chain = S->row_of_chain; a.logL_prop = S->logL_prop; a.counters = S->counters;
   a.u_out = S->u_out; a.logL_out = S->logL_out;
+  a.n_per_run = 0; a.keys = nullptr; a.iters = nullptr; a.run_evals = nullptr; a.run_fails = nullptr;
+  if (multi) { a.n_per_run = multi->n_per_run; a.keys = multi->keys; a.iters = multi->iters; a.run_evals = multi->run_evals;
+               a.run_fails = multi->run_fails; a.scal = multi->scal; a.Lsig = multi->Lsig; }
+  const int n_target = multi ? multi->n_target : n_chains;
   NSGPU_CUDA(cudaMemsetAsync(S->counters, 0, 4 * sizeof(int), st));
   const int blocks = (n_chains * 32 + 127) / 128;
   int64_t rounds = 0;
@@ -667,7 +695,7 @@ static nsgpu_status evolve(nsgpu_ctx* ctx, int n_chains, int chain0, int n_steps
     }
     NSGPU_CUDA(cudaMemcpyAsync(S->h_counters, S->counters, 4 * sizeof(int), cudaMemcpyDeviceToHost, st));
     NSGPU_CUDA(cudaStreamSynchronize(st));
-    if (S->h_counters[1] >= n_chains) break;
+    if (S->h_counters[1] >= n_target) break;
     burst = 16;
     if (rounds > (int64_t)n_steps * (MAX_STEP_OUT * 2 + MAX_SHRINK + 4) + 16) {
       ctx->err = "slice sampling: chains did not finish (internal error)";
@@ -799,6 +827,85 @@ extern "C" void nsgpu_shard_range(int32_t n_chains, int32_t rank, int32_t world,
   const int c0 = std::min(n_chains, rank * per);
   if (first) *first = c0;
   if (count) *count = std::max(0, std::min(n_chains, c0 + per) - c0);
+}
+
+// Final summary of one run (host arithmetic over the recorded sequence, reading N8/N9): total log Z with the live points,
+// H, error bar by simulated volumes (evidence_error_kernel) and by the analytic formula, weighted samples theta = T(u).
+static nsgpu_status summarize_run(nsgpu_ctx* ctx, int n, int k, uint2 key, double logX, const std::vector<float>& dead_u,
+                                  const std::vector<double>& dead_logL, const std::vector<double>& dead_logw,
+                                  const std::vector<float>& live_u, const std::vector<double>& live_l,
+                                  const double* d_live_logL, cudaStream_t st, nsgpu_result* res, std::vector<float>& out_theta,
+                                  std::vector<double>& out_logL, std::vector<double>& out_logw) {
+  SamplerDev* S = ctx->sampler;
+  const int D = ctx->D;
+  nsgpu_status s = NSGPU_OK;
+  const size_t nd = dead_logL.size(), ntot = nd + n;
+  std::vector<double> all_l(ntot), all_w(ntot);
+  for (size_t i = 0; i < nd; ++i) { all_l[i] = dead_logL[i]; all_w[i] = dead_logw[i]; }
+  for (int i = 0; i < n; ++i) { all_l[nd + i] = live_l[i]; all_w[nd + i] = logX - log((double)n); }   // reading N8
+  auto logsumexp = [](const std::vector<double>& v) -> double {
+    double mx = -INFINITY;
+    for (double x : v) mx = std::max(mx, x);
+    if (!(mx > -INFINITY)) return (double)-INFINITY;
+    double sacc = 0.0;
+    for (double x : v) sacc += exp(x - mx);
+    return mx + log(sacc);
+  };
+  std::vector<double> terms(ntot);
+  for (size_t i = 0; i < ntot; ++i) terms[i] = all_l[i] + all_w[i];
+  const double logZ = logsumexp(terms);
+  double H = 0.0;
+  for (size_t i = 0; i < ntot; ++i) {
+    const double p = exp(terms[i] - logZ);
+    if (p > 0.0) H += p * (all_l[i] - logZ);
+  }
+  // error bar: redraw the volume sequence M = 1000 times with t_j = U^{1/n_j} (Skilling 2006; P:L182-184) -- one CTA per
+  // sequence (evidence_error_kernel); the host only takes the standard deviation of the 1000 results.  (Round 1 did
+  // this in a single-threaded host loop of 1000 x n_dead log/expm1/exp calls: 3.4 s for a c4 run.)
+  double err_sim = 0.0;
+  {
+    const int M = 1000;
+    double *d_dead = nullptr, *d_zs = nullptr;
+    NSGPU_CUDA(cudaMalloc((void**)&d_dead, sizeof(double) * std::max<size_t>(nd, 1)));
+    NSGPU_CUDA(cudaMalloc((void**)&d_zs, sizeof(double) * M));
+    std::vector<double> zs(M);
+    cudaError_t e1 = cudaMemcpyAsync(d_dead, dead_logL.data(), sizeof(double) * nd, cudaMemcpyHostToDevice, st);
+    evidence_error_kernel<<<M, 256, 0, st>>>(d_dead, (long long)nd, n, k, d_live_logL, key, d_zs);
+    ctx->launches++;
+    cudaError_t e2 = cudaMemcpyAsync(zs.data(), d_zs, sizeof(double) * M, cudaMemcpyDeviceToHost, st);
+    cudaError_t e3 = cudaStreamSynchronize(st);
+    cudaFree(d_dead); cudaFree(d_zs);
+    NSGPU_CUDA(e1); NSGPU_CUDA(e2); NSGPU_CUDA(e3);
+    double mean = 0.0;
+    for (double z : zs) mean += z;
+    mean /= M;
+    for (double z : zs) err_sim += (z - mean) * (z - mean);
+    err_sim = sqrt(err_sim / (M - 1));
+  }
+  double s1 = 0.0, s2 = 0.0;
+  for (int j = 0; j < k; ++j) { s1 += 1.0 / (n - j); s2 += 1.0 / ((double)(n - j) * (n - j)); }
+  const double cfac = n * s2 / s1;
+  res->logZ = logZ; res->logZ_err = err_sim; res->logZ_err_analytic = sqrt(std::max(cfac * H, 0.0) / n); res->H = H;
+  res->n_dead = (int64_t)nd;
+  {
+    // theta = T(u) through the a1 kernel, in chunks of max_batch rows; kept in the ctx for nsgpu_last_samples
+    std::vector<float> all_u(ntot * D);
+    memcpy(all_u.data(), dead_u.data(), sizeof(float) * nd * D);
+    memcpy(all_u.data() + nd * D, live_u.data(), sizeof(float) * (size_t)n * D);
+    out_theta.resize(ntot * D);
+    out_logL = all_l;
+    out_logw.resize(ntot);
+    for (size_t i = 0; i < ntot; ++i) out_logw[i] = terms[i] - logZ;
+    for (size_t off = 0; off < ntot; off += (size_t)ctx->max_batch) {
+      const int nb = (int)std::min<size_t>((size_t)ctx->max_batch, ntot - off);
+      NSGPU_CUDA(cudaMemcpyAsync(S->xprop, all_u.data() + off * D, sizeof(float) * (size_t)nb * D, cudaMemcpyHostToDevice, st));
+      s = nsgpu_prior_transform(ctx, S->xprop, nb, S->theta_prop, st);
+      if (s != NSGPU_OK) return s;
+      NSGPU_CUDA(cudaMemcpyAsync(out_theta.data() + off * D, S->theta_prop, sizeof(float) * (size_t)nb * D, cudaMemcpyDeviceToHost, st));
+      NSGPU_CUDA(cudaStreamSynchronize(st));   // copies and kernel ordered on the run's stream (not the legacy default one)
+    }
+  }
+  return s;
 }
 
 static nsgpu_status run_impl(nsgpu_ctx* ctx, const nsgpu_run_opts* o, int rank, int world, nsgpu_allgather_fn exch,
@@ -938,74 +1045,11 @@ static nsgpu_status run_impl(nsgpu_ctx* ctx, const nsgpu_run_opts* o, int rank, 
       n_fail_total += (int)all[4 * r + 2];
     }
   }
-  const size_t nd = dead_logL.size(), ntot = nd + n;
-  std::vector<double> all_l(ntot), all_w(ntot);
-  for (size_t i = 0; i < nd; ++i) { all_l[i] = dead_logL[i]; all_w[i] = dead_logw[i]; }
-  for (int i = 0; i < n; ++i) { all_l[nd + i] = live_l[i]; all_w[nd + i] = logX - log((double)n); }   // reading N8
-  auto logsumexp = [](const std::vector<double>& v) -> double {
-    double mx = -INFINITY;
-    for (double x : v) mx = std::max(mx, x);
-    if (!(mx > -INFINITY)) return (double)-INFINITY;
-    double sacc = 0.0;
-    for (double x : v) sacc += exp(x - mx);
-    return mx + log(sacc);
-  };
-  std::vector<double> terms(ntot);
-  for (size_t i = 0; i < ntot; ++i) terms[i] = all_l[i] + all_w[i];
-  const double logZ = logsumexp(terms);
-  double H = 0.0;
-  for (size_t i = 0; i < ntot; ++i) {
-    const double p = exp(terms[i] - logZ);
-    if (p > 0.0) H += p * (all_l[i] - logZ);
-  }
-  // error bar: redraw the volume sequence M = 1000 times with t_j = U^{1/n_j} (Skilling 2006; P:L182-184) -- one CTA per
-  // sequence (evidence_error_kernel); the host only takes the standard deviation of the 1000 results.  (Round 1 did
-  // this in a single-threaded host loop of 1000 x n_dead log/expm1/exp calls: 3.4 s for a c4 run.)
-  double err_sim = 0.0;
-  {
-    const int M = 1000;
-    double *d_dead = nullptr, *d_zs = nullptr;
-    NSGPU_CUDA(cudaMalloc((void**)&d_dead, sizeof(double) * std::max<size_t>(nd, 1)));
-    NSGPU_CUDA(cudaMalloc((void**)&d_zs, sizeof(double) * M));
-    std::vector<double> zs(M);
-    cudaError_t e1 = cudaMemcpyAsync(d_dead, dead_logL.data(), sizeof(double) * nd, cudaMemcpyHostToDevice, st);
-    evidence_error_kernel<<<M, 256, 0, st>>>(d_dead, (long long)nd, n, k, S->logL_live, key, d_zs);
-    ctx->launches++;
-    cudaError_t e2 = cudaMemcpyAsync(zs.data(), d_zs, sizeof(double) * M, cudaMemcpyDeviceToHost, st);
-    cudaError_t e3 = cudaStreamSynchronize(st);
-    cudaFree(d_dead); cudaFree(d_zs);
-    NSGPU_CUDA(e1); NSGPU_CUDA(e2); NSGPU_CUDA(e3);
-    double mean = 0.0;
-    for (double z : zs) mean += z;
-    mean /= M;
-    for (double z : zs) err_sim += (z - mean) * (z - mean);
-    err_sim = sqrt(err_sim / (M - 1));
-  }
-  double s1 = 0.0, s2 = 0.0;
-  for (int j = 0; j < k; ++j) { s1 += 1.0 / (n - j); s2 += 1.0 / ((double)(n - j) * (n - j)); }
-  const double cfac = n * s2 / s1;
-  res->logZ = logZ; res->logZ_err = err_sim; res->logZ_err_analytic = sqrt(std::max(cfac * H, 0.0) / n); res->H = H;
-  res->n_iter = it; res->n_dead = (int64_t)nd; res->n_like_evals = (int64_t)evals_all + n; res->n_rounds = rounds;
-  res->n_failed_moves = n_fail_total;
-  if (n_samples) *n_samples = (int64_t)ntot;
-  {
-    // theta = T(u) through the a1 kernel, in chunks of max_batch rows; kept in the ctx for nsgpu_last_samples
-    std::vector<float> all_u(ntot * D);
-    memcpy(all_u.data(), dead_u.data(), sizeof(float) * nd * D);
-    memcpy(all_u.data() + nd * D, live_u.data(), sizeof(float) * (size_t)n * D);
-    S->last_theta.resize(ntot * D);
-    S->last_logL = all_l;
-    S->last_logw.resize(ntot);
-    for (size_t i = 0; i < ntot; ++i) S->last_logw[i] = terms[i] - logZ;
-    for (size_t off = 0; off < ntot; off += (size_t)ctx->max_batch) {
-      const int nb = (int)std::min<size_t>((size_t)ctx->max_batch, ntot - off);
-      NSGPU_CUDA(cudaMemcpyAsync(S->xprop, all_u.data() + off * D, sizeof(float) * (size_t)nb * D, cudaMemcpyHostToDevice, st));
-      s = nsgpu_prior_transform(ctx, S->xprop, nb, S->theta_prop, st);
-      if (s != NSGPU_OK) return s;
-      NSGPU_CUDA(cudaMemcpyAsync(S->last_theta.data() + off * D, S->theta_prop, sizeof(float) * (size_t)nb * D, cudaMemcpyDeviceToHost, st));
-      NSGPU_CUDA(cudaStreamSynchronize(st));   // copies and kernel ordered on the run's stream (not the legacy default one)
-    }
-  }
+  s = summarize_run(ctx, n, k, key, logX, dead_u, dead_logL, dead_logw, live_u, live_l, S->logL_live, st, res, S->last_theta,
+                    S->last_logL, S->last_logw);
+  if (s != NSGPU_OK) return s;
+  res->n_iter = it; res->n_like_evals = (int64_t)evals_all + n; res->n_rounds = rounds; res->n_failed_moves = n_fail_total;
+  if (n_samples) *n_samples = (int64_t)S->last_logL.size();
   if (cap > 0 && theta_samples && logL_samples && logw_samples) {
     int64_t got = 0;
     s = nsgpu_last_samples(ctx, theta_samples, logL_samples, logw_samples, cap, &got);
@@ -1028,4 +1072,171 @@ extern "C" nsgpu_status nsgpu_run_sharded(nsgpu_ctx* ctx, const nsgpu_run_opts* 
                                           float* theta_samples, double* logL_samples, double* logw_samples, int64_t cap,
                                           int64_t* n_samples) {
   return run_impl(ctx, o, rank, world, allgather, user, res, theta_samples, logL_samples, logw_samples, cap, n_samples);
+}
+
+// ---------------------------------------------------------------------------------------------------
+// nsgpu_run_multi: R independent runs (seeds) of ONE model that share every likelihood batch.
+// A single run keeps the GPU half idle: a round carries <= k (on average ~0.6 k) proposals through ten launches
+// ("perfect scaling is hard to achieve").  Here the chains of all runs advance in the same rounds: chain slot
+// c belongs to run c / k, and slice_round_kernel takes L*, the direction factor, the Philox key and the iteration
+// number of that run; compaction and the likelihood see one batch of up to R k proposals.  Everything per run
+// (live set, deletion, evidence scan, stopping test, summary) is done per run with the same kernels, so every run
+// returns exactly what nsgpu_run returns for its seed.  Runs stay in lock step per iteration; a converged run drops out.
+// ---------------------------------------------------------------------------------------------------
+namespace {
+struct MultiBuf {
+  float *u_live = nullptr, *dead_u = nullptr;
+  double *logL_live = nullptr, *scal = nullptr, *Lsig = nullptr, *logw = nullptr, *dead_l = nullptr;
+  int *dead_idx = nullptr, *surv_idx = nullptr, *run_fails = nullptr;
+  uint2* keys = nullptr;
+  unsigned* iters = nullptr;
+  unsigned long long* run_evals = nullptr;
+  ~MultiBuf() {
+    void* p[] = {u_live, dead_u, logL_live, scal, Lsig, logw, dead_l, dead_idx, surv_idx, run_fails, keys, iters, run_evals};
+    for (void* q : p) cudaFree(q);
+  }
+};
+}  // namespace
+
+extern "C" nsgpu_status nsgpu_run_multi(nsgpu_ctx* ctx, const nsgpu_run_opts* o, int32_t n_runs, const uint64_t* seeds,
+                                        nsgpu_result* res) {
+  if (!ctx) return NSGPU_EINVAL;
+  if (!o || !res || !seeds || n_runs < 1 || n_runs > 64) { ctx->err = "run_multi: NULL pointer or n_runs outside 1..64"; return NSGPU_EINVAL; }
+  nsgpu_status s = check_sampler_args(ctx, o->n_live, o->n_delete);
+  if (s != NSGPU_OK) return s;
+  if (o->n_delete >= o->n_live || o->n_steps < 1 || !(o->stop_frac > 0) || o->max_iter < 1) { ctx->err = "run_multi: bad options"; return NSGPU_EINVAL; }
+  if (o->n_live < ctx->D + 1) { ctx->err = "run_multi: the live covariance needs n_live >= D + 1"; return NSGPU_EINVAL; }
+  if ((int64_t)n_runs * o->n_delete > ctx->max_batch) { ctx->err = "run_multi: n_runs x n_delete exceeds max_batch"; return NSGPU_ESHAPE; }
+  const auto t_start = std::chrono::steady_clock::now();
+  SamplerDev* S = ctx->sampler;
+  cudaStream_t st = S->run_stream;
+  const int D = ctx->D, n = o->n_live, k = o->n_delete, R = n_runs;
+  MultiBuf B;
+#define MB(p, T, cnt) NSGPU_CUDA(cudaMalloc((void**)&B.p, sizeof(T) * (size_t)(cnt)))
+  MB(u_live, float, (size_t)R * n * D); MB(logL_live, double, (size_t)R * n); MB(scal, double, R * 8); MB(Lsig, double, (size_t)R * D * D);
+  MB(dead_idx, int, (size_t)R * k); MB(surv_idx, int, (size_t)R * n); MB(logw, double, (size_t)R * k); MB(dead_u, float, (size_t)R * k * D);
+  MB(dead_l, double, (size_t)R * k); MB(keys, uint2, R); MB(iters, unsigned, R); MB(run_evals, unsigned long long, R); MB(run_fails, int, R);
+#undef MB
+  std::vector<uint2> keys(R);
+  for (int r = 0; r < R; ++r) keys[r] = make_uint2((unsigned)(seeds[r] & 0xffffffffu), (unsigned)(seeds[r] >> 32));
+  NSGPU_CUDA(cudaMemcpyAsync(B.keys, keys.data(), sizeof(uint2) * R, cudaMemcpyHostToDevice, st));
+  NSGPU_CUDA(cudaMemsetAsync(B.run_evals, 0, sizeof(unsigned long long) * R, st));
+  NSGPU_CUDA(cudaMemsetAsync(B.run_fails, 0, sizeof(int) * R, st));
+  std::vector<double> h_scal((size_t)R * 8, 0.0);
+  for (int r = 0; r < R; ++r) h_scal[8 * r + 2] = -INFINITY;
+  NSGPU_CUDA(cudaMemcpyAsync(B.scal, h_scal.data(), sizeof(double) * R * 8, cudaMemcpyHostToDevice, st));
+  for (int r = 0; r < R; ++r) {          // initial live sets: the same draws and likelihood calls as nsgpu_run(seed r)
+    memset(&res[r], 0, sizeof(nsgpu_result));
+    float* ul = B.u_live + (size_t)r * n * D;
+    init_live_kernel<<<(n * D + 255) / 256, 256, 0, st>>>(n, D, keys[r], ul);
+    NSGPU_LAUNCH_CHECK();
+    s = nsgpu_prior_transform(ctx, ul, n, S->theta_prop, st);
+    if (s != NSGPU_OK) return s;
+    s = loglike_device(ctx, S->theta_prop, n, nullptr, B.logL_live + (size_t)r * n, st);
+    if (s != NSGPU_OK) return s;
+  }
+  struct Host { std::vector<float> dead_u; std::vector<double> dead_logL, dead_logw; bool active = true, converged = false; int64_t n_iter = 0; double logX = 0.0; };
+  std::vector<Host> H(R);
+  std::vector<float> hu((size_t)R * k * D);
+  std::vector<double> hl((size_t)R * k), hw((size_t)R * k);
+  std::vector<unsigned> h_iters(R, 0u);
+  int64_t it = 0, rounds = 0;
+  int n_active = R;
+  while (n_active > 0 && it < o->max_iter) {
+    ++it;
+    for (int r = 0; r < R; ++r) {
+      if (!H[r].active) continue;
+      float* ul = B.u_live + (size_t)r * n * D;
+      double* ll = B.logL_live + (size_t)r * n;
+      s = launch_live_cholesky(ctx, ul, n, B.Lsig + (size_t)r * D * D, B.scal + 8 * r + 5, st);
+      if (s != NSGPU_OK) return s;
+      s = launch_delete(ctx, ll, n, k, st, B.scal + 8 * r, B.dead_idx + (size_t)r * k, B.surv_idx + (size_t)r * n, B.logw + (size_t)r * k);
+      if (s != NSGPU_OK) return s;
+      gather_rows_kernel<<<(k * D + 255) / 256, 256, 0, st>>>(k, D, B.dead_idx + (size_t)r * k, ul, ll, B.dead_u + (size_t)r * k * D,
+                                                              B.dead_l + (size_t)r * k);
+      NSGPU_LAUNCH_CHECK();
+      h_iters[r] = (unsigned)it;
+    }
+    NSGPU_CUDA(cudaMemcpyAsync(hu.data(), B.dead_u, sizeof(float) * hu.size(), cudaMemcpyDeviceToHost, st));
+    NSGPU_CUDA(cudaMemcpyAsync(hl.data(), B.dead_l, sizeof(double) * hl.size(), cudaMemcpyDeviceToHost, st));
+    NSGPU_CUDA(cudaMemcpyAsync(hw.data(), B.logw, sizeof(double) * hw.size(), cudaMemcpyDeviceToHost, st));
+    NSGPU_CUDA(cudaMemcpyAsync(B.iters, h_iters.data(), sizeof(unsigned) * R, cudaMemcpyHostToDevice, st));
+    NSGPU_CUDA(cudaStreamSynchronize(st));
+    for (int r = 0; r < R; ++r) {
+      if (!H[r].active) continue;
+      H[r].dead_u.insert(H[r].dead_u.end(), hu.begin() + (size_t)r * k * D, hu.begin() + (size_t)(r + 1) * k * D);
+      H[r].dead_logL.insert(H[r].dead_logL.end(), hl.begin() + (size_t)r * k, hl.begin() + (size_t)(r + 1) * k);
+      H[r].dead_logw.insert(H[r].dead_logw.end(), hw.begin() + (size_t)r * k, hw.begin() + (size_t)(r + 1) * k);
+      const size_t c0 = (size_t)r * k;      // this run's chain slots
+      chain_init_kernel<<<(k + 127) / 128, 128, 0, st>>>(k, 0, D, keys[r], (unsigned)it, B.surv_idx + (size_t)r * n, n - k, nullptr,
+                                                         S->start_idx + c0, B.u_live + (size_t)r * n * D, B.logL_live + (size_t)r * n,
+                                                         S->x0 + c0 * D, S->logL0 + c0, S->phase + c0, S->cnt + c0, S->step + c0,
+                                                         S->pending + c0, S->finished + c0, S->need + c0, S->rng_j + c0, n, B.scal + 8 * r);
+      NSGPU_LAUNCH_CHECK();
+    }
+    MultiArgs ma;
+    ma.n_per_run = k; ma.n_target = n_active * k; ma.keys = B.keys; ma.iters = B.iters; ma.run_evals = B.run_evals;
+    ma.run_fails = B.run_fails; ma.scal = B.scal; ma.Lsig = B.Lsig;
+    s = evolve(ctx, R * k, 0, o->n_steps, 0, (int)it, st, &rounds, &ma);
+    if (s != NSGPU_OK) return s;
+    for (int r = 0; r < R; ++r) {
+      if (!H[r].active) continue;
+      const size_t c0 = (size_t)r * k;
+      replace_kernel<<<(k * D + 255) / 256, 256, 0, st>>>(k, D, B.dead_idx + c0, S->u_out + c0 * D, S->logL_out + c0,
+                                                          B.u_live + (size_t)r * n * D, B.logL_live + (size_t)r * n);
+      NSGPU_LAUNCH_CHECK();
+      live_evidence_kernel<<<1, 1024, 0, st>>>(B.logL_live + (size_t)r * n, n, log(o->stop_frac), B.scal + 8 * r);
+      NSGPU_LAUNCH_CHECK();
+    }
+    NSGPU_CUDA(cudaMemcpyAsync(h_scal.data(), B.scal, sizeof(double) * R * 8, cudaMemcpyDeviceToHost, st));
+    NSGPU_CUDA(cudaStreamSynchronize(st));
+    for (int r = 0; r < R; ++r) {
+      if (!H[r].active) continue;
+      if (h_scal[8 * r + 5] != 0.0) { ctx->err = "run_multi: live-set covariance is not positive definite"; return NSGPU_ENOTSPD; }
+      H[r].n_iter = it; H[r].logX = h_scal[8 * r + 1];
+      if (h_scal[8 * r + 4] != 0.0) { H[r].converged = true; H[r].active = false; --n_active; }
+    }
+  }
+  const auto t_sampled = std::chrono::steady_clock::now();
+  std::vector<unsigned long long> evals(R);
+  std::vector<int> fails(R);
+  NSGPU_CUDA(cudaMemcpy(evals.data(), B.run_evals, sizeof(unsigned long long) * R, cudaMemcpyDeviceToHost));
+  NSGPU_CUDA(cudaMemcpy(fails.data(), B.run_fails, sizeof(int) * R, cudaMemcpyDeviceToHost));
+  S->multi.assign(R, SamplerDev::SampleSet());
+  bool all_conv = true;
+  std::vector<float> live_u((size_t)n * D);
+  std::vector<double> live_l(n);
+  for (int r = 0; r < R; ++r) {
+    NSGPU_CUDA(cudaMemcpy(live_u.data(), B.u_live + (size_t)r * n * D, sizeof(float) * (size_t)n * D, cudaMemcpyDeviceToHost));
+    NSGPU_CUDA(cudaMemcpy(live_l.data(), B.logL_live + (size_t)r * n, sizeof(double) * (size_t)n, cudaMemcpyDeviceToHost));
+    s = summarize_run(ctx, n, k, keys[r], H[r].logX, H[r].dead_u, H[r].dead_logL, H[r].dead_logw, live_u, live_l,
+                      B.logL_live + (size_t)r * n, st, &res[r], S->multi[r].theta, S->multi[r].logL, S->multi[r].logw);
+    if (s != NSGPU_OK) return s;
+    res[r].n_iter = H[r].n_iter; res[r].n_like_evals = (int64_t)evals[r] + n; res[r].n_rounds = rounds; res[r].n_failed_moves = fails[r];
+    all_conv = all_conv && H[r].converged;
+  }
+  const auto t_end = std::chrono::steady_clock::now();
+  for (int r = 0; r < R; ++r) {          // wall times are those of the whole call: the runs share every round
+    res[r].seconds = std::chrono::duration<double>(t_end - t_start).count();
+    res[r].seconds_sampling = std::chrono::duration<double>(t_sampled - t_start).count();
+    res[r].seconds_summary = std::chrono::duration<double>(t_end - t_sampled).count();
+  }
+  return all_conv ? NSGPU_OK : NSGPU_ENOCONV;
+}
+
+extern "C" nsgpu_status nsgpu_multi_samples(nsgpu_ctx* ctx, int32_t run, float* theta_samples, double* logL_samples,
+                                            double* logw_samples, int64_t cap, int64_t* n_samples) {
+  if (!ctx) return NSGPU_EINVAL;
+  SamplerDev* S = ctx->sampler;
+  if (run < 0 || run >= (int)S->multi.size()) { ctx->err = "multi_samples: no such run"; return NSGPU_EINVAL; }
+  const SamplerDev::SampleSet& X = S->multi[run];
+  const int64_t ntot = (int64_t)X.logL.size();
+  if (n_samples) *n_samples = ntot;
+  if (cap <= 0) return NSGPU_OK;
+  if (!theta_samples || !logL_samples || !logw_samples) { ctx->err = "multi_samples: NULL buffer"; return NSGPU_EINVAL; }
+  const size_t nw = (size_t)std::min<int64_t>(cap, ntot);
+  memcpy(theta_samples, X.theta.data(), sizeof(float) * nw * ctx->D);
+  memcpy(logL_samples, X.logL.data(), sizeof(double) * nw);
+  memcpy(logw_samples, X.logw.data(), sizeof(double) * nw);
+  return NSGPU_OK;
 }

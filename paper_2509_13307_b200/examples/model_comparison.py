@@ -2,13 +2,16 @@
 (37-D), on the synthetic cosmic-shear likelihood (c3a weights; mock data from the LambdaCDM truth).
 
     python -m paper_2509_13307_b200.examples.model_comparison [--n-live 1000] [--n-delete 500] [--seeds 1]
-                                                              [--shape c4|paper-interp|paper]
+                                                              [--shape c4|paper-interp|paper] [--batched] [--ranks N]
+
+`--batched` (with --seeds R > 1): the R seeds of a model run as ONE nsgpu_run_multi call that shares every likelihood
+batch between them (each result is what the single run returns, bit for bit), the two models on two host threads.
 
 `--shape paper-interp` / `paper` run the same comparison on the paper-shape likelihood (10 bins, 55 spectra,
 1025 quadrature nodes; emulator on 103 z nodes + linear interpolation, or on all 1025: PAPER.md L353, L359).
 
-Multi-GPU: launch with `python -m torch.distributed.run --nnodes=1 --nproc-per-node N --master-addr
-127.0.0.1 -m paper_2509_13307_b200.examples.model_comparison ...`; every rank holds the live set, evolves its share of
+Multi-GPU: `--ranks N` (re-executes itself under `python -m torch.distributed.run --nnodes=1
+--nproc-per-node N --master-addr 127.0.0.1`), or launch it under torchrun yourself; every rank holds the live set, evolves its share of
 the 500 chains per iteration and all-gathers the new points over NCCL (`Context.run_sharded`); rank 0 prints.
 
 Prints one JSON line per run and a summary with log Z +- error per model, the log Bayes factor, total
@@ -40,6 +43,19 @@ def _ranks():
     return dist.get_rank(), world, dev
 
 
+def _spawn(n):
+    """re-execute this module with n ranks (one per GPU) on this node"""
+    import socket
+    import subprocess
+    import sys
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={n}", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), "-m", "paper_2509_13307_b200.examples.model_comparison"] + sys.argv[1:]
+    return subprocess.call(cmd)
+
+
 def _mock_data(wl_w0wa, device=0):
     """d = model_w0wa(theta_0 with w0 = -1, wa = 0) + L eps, shared by both models."""
     n = wl_w0wa.n_data
@@ -63,8 +79,16 @@ def main():
     ap.add_argument("--sequential", action="store_true", help="one run after the other")
     ap.add_argument("--concurrent", type=int, default=4, help="runs in flight on one GPU (models x seeds; default 4)")
     ap.add_argument("--ctx-flags", type=int, default=0, help="extra nsgpu_create flags, e.g. 128 = NSGPU_NO_PDL (plain stream ordering)")
+    ap.add_argument("--batched", action="store_true", help="all seeds of a model in one nsgpu_run_multi call (shared likelihood batches)")
+    ap.add_argument("--ranks", type=int, default=1, help="GPUs: start this many ranks under torch.distributed.run (sharded runs)")
     args = ap.parse_args()
+    if args.ranks > 1 and "WORLD_SIZE" not in os.environ:
+        raise SystemExit(_spawn(args.ranks))
     rank, world, dev = _ranks()
+    if world > 1 and rank == 0:
+        for r in range(world):
+            first, count = nsgpu.shard_range(args.n_delete, r, world)
+            print(json.dumps({"rank": r, "chains": [first, first + count], "of": args.n_delete}), flush=True)
     if args.shape == "c4":
         full, rest = _mock_data(W.c3a(), dev), W.c4_lcdm()
     else:
@@ -76,7 +100,18 @@ def main():
 
     def run_model(name, wl, seeds):
         torch.cuda.set_device(dev)
-        with nsgpu.Context(wl, max_batch=args.n_live, device=dev, mlp=nsgpu.MLP_AUTO | args.ctx_flags) as ctx:
+        batched = args.batched and world == 1 and len(seeds) > 1
+        mb = max(args.n_live, args.n_delete * len(seeds)) if batched else args.n_live
+        with nsgpu.Context(wl, max_batch=mb, device=dev, mlp=nsgpu.MLP_AUTO | args.ctx_flags) as ctx:
+            if batched:
+                rs = ctx.run_multi(args.n_live, args.n_delete, 5 * wl.D, seeds, stop_frac=args.stop_frac, max_iter=args.max_iter,
+                                   return_samples=False)
+                for r in rs:
+                    r["model"], r["D"], r["n_gpus"], r["batched_with"] = name, wl.D, world, len(seeds)
+                    with lock:
+                        print(json.dumps(r), flush=True)
+                        out[name].append(r)
+                return
             for seed in seeds:
                 kw = dict(stop_frac=args.stop_frac, max_iter=args.max_iter, seed=seed, return_samples=False)
                 if world == 1:
@@ -97,7 +132,7 @@ def main():
         # The runs are independent and each keeps the GPU only partly busy (batches of <= n_delete proposals, fewer
         # as the chains of an iteration finish): one host thread and one context per worker, each nsgpu_run on its
         # context's own stream, so their kernels share the SMs.  Workers = models x groups of seeds.
-        per_model = max(1, min(len(all_seeds), n_conc // 2))
+        per_model = 1 if args.batched else max(1, min(len(all_seeds), n_conc // 2))
         jobs = [(name, wl, all_seeds[g::per_model]) for name, wl in models for g in range(per_model)]
         threads = [threading.Thread(target=run_model, args=j) for j in jobs]
         for t in threads:

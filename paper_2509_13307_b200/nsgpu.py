@@ -29,7 +29,7 @@ EXPORTS = ["nsgpu_create", "nsgpu_destroy", "nsgpu_last_error", "nsgpu_prior_tra
            "nsgpu_slice_step", "nsgpu_run", "nsgpu_last_samples", "nsgpu_delete_lowest", "nsgpu_live_cholesky",
            "nsgpu_debug_philox", "nsgpu_set_profiling", "nsgpu_stage_times", "nsgpu_mlp_path", "nsgpu_launch_count",
            "nsgpu_run_sharded", "nsgpu_shard_range", "nsgpu_sampler_counters", "nsgpu_nonfinite_rows",
-           "nsgpu_clock_mark", "nsgpu_clock_marks_read"]
+           "nsgpu_clock_mark", "nsgpu_clock_marks_read", "nsgpu_run_multi", "nsgpu_multi_samples"]
 
 
 class NsgpuError(RuntimeError):
@@ -121,6 +121,10 @@ def lib():
                                     vp, vp, vp, C.c_int64, C.POINTER(C.c_int64)]
     L.nsgpu_sampler_counters.restype = C.c_int
     L.nsgpu_sampler_counters.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
+    L.nsgpu_run_multi.restype = C.c_int
+    L.nsgpu_run_multi.argtypes = [vp, C.POINTER(_RunOpts), C.c_int32, C.POINTER(C.c_uint64), C.POINTER(_Result)]
+    L.nsgpu_multi_samples.restype = C.c_int
+    L.nsgpu_multi_samples.argtypes = [vp, C.c_int32, vp, vp, vp, C.c_int64, C.POINTER(C.c_int64)]
     L.nsgpu_clock_mark.restype = C.c_int
     L.nsgpu_clock_mark.argtypes = [vp, vp]
     L.nsgpu_clock_marks_read.restype = C.c_int
@@ -413,6 +417,30 @@ class Context:
                                                  lw.ctypes.data_as(C.c_void_p), n, C.byref(ns)))
             out.update(theta=th, logL=ll, logw=lw, n_samples=n)
         return out
+
+    def run_multi(self, n_live, n_delete, n_steps, seeds, stop_frac=1e-3, max_iter=100000, return_samples=True):
+        """nsgpu_run_multi: one dict per seed, each equal to `run(..., seed=s)`; the runs share every likelihood batch."""
+        seeds = [int(x) for x in seeds]
+        R = len(seeds)
+        o = _RunOpts(int(n_live), int(n_delete), int(n_steps), float(stop_frac), int(max_iter), 0)
+        res = (_Result * R)()
+        sd = (C.c_uint64 * R)(*seeds)
+        st = self._check(lib().nsgpu_run_multi(self._h, C.byref(o), R, sd, res), allow=(ENOCONV,))
+        outs = []
+        for r in range(R):
+            out = {f: getattr(res[r], f) for f, _ in _Result._fields_}
+            out["seed"] = seeds[r]
+            out["converged"] = st == OK or out["n_iter"] < int(max_iter)
+            if return_samples:
+                ns = C.c_int64(0)
+                self._check(lib().nsgpu_multi_samples(self._h, r, None, None, None, 0, C.byref(ns)))
+                n = ns.value
+                th = np.empty((n, self.D), np.float32); ll = np.empty(n, np.float64); lw = np.empty(n, np.float64)
+                self._check(lib().nsgpu_multi_samples(self._h, r, th.ctypes.data_as(C.c_void_p), ll.ctypes.data_as(C.c_void_p),
+                                                      lw.ctypes.data_as(C.c_void_p), n, C.byref(ns)))
+                out.update(theta=th, logL=ll, logw=lw, n_samples=n)
+            outs.append(out)
+        return outs
 
     def run_sharded(self, n_live, n_delete, n_steps, stop_frac=1e-3, max_iter=100000, seed=1, rank=None, world=None,
                     allgather=None, return_samples=True):

@@ -334,3 +334,39 @@ def test_concurrent_runs_on_two_contexts_equal_sequential_runs():
         np.testing.assert_array_equal(got[s]["logw"], alone[s]["logw"])
     assert plain["logZ"] == alone[1]["logZ"] and plain["n_like_evals"] == alone[1]["n_like_evals"]
     np.testing.assert_array_equal(plain["theta"], alone[1]["theta"])
+
+
+@pytest.mark.parametrize("name,n,k,steps,seeds", [("toy", 200, 100, 30, (1, 2, 3)), ("identity", 300, 30, 12, (5, 6, 7, 8, 9)),
+                                                 ("tiny_shear", 120, 60, 20, (3, 4))])
+def test_run_multi_equals_separate_runs(name, n, k, steps, seeds):
+    """nsgpu_run_multi: R runs of one model share every likelihood batch (per-run L*, direction factor, Philox key,
+    iteration number and stopping test inside the kernels).  Each run must return what nsgpu_run returns alone for its
+    seed -- evidences, iteration and evaluation counts, failed moves and every weighted sample, bit for bit -- although
+    the runs converge after different numbers of iterations."""
+    wl = workload(name)
+    with nsgpu.Context(wl, max_batch=max(n, k * len(seeds))) as ctx:
+        alone = [ctx.run(n, k, steps, seed=s) for s in seeds]
+        multi = ctx.run_multi(n, k, steps, seeds)
+        again = ctx.run(n, k, steps, seed=seeds[0])                     # the context is reusable afterwards
+    if name == "identity":
+        assert len({r["n_iter"] for r in alone}) > 1                     # runs of different lengths: some drop out early
+    for a, m in zip(alone, multi):
+        for key in ("logZ", "logZ_err", "logZ_err_analytic", "H", "n_iter", "n_dead", "n_like_evals", "n_failed_moves"):
+            assert m[key] == a[key], (key, m[key], a[key])
+        assert m["converged"] and a["converged"]
+        np.testing.assert_array_equal(m["theta"], a["theta"])
+        np.testing.assert_array_equal(m["logL"], a["logL"])
+        np.testing.assert_array_equal(m["logw"], a["logw"])
+    assert again["logZ"] == alone[0]["logZ"]
+    assert multi[0]["n_rounds"] <= sum(r["n_rounds"] for r in alone)
+
+
+def test_run_multi_argument_errors():
+    wl = workload("identity")
+    with nsgpu.Context(wl, max_batch=200) as ctx:
+        with pytest.raises(nsgpu.NsgpuError) as e:
+            ctx.run_multi(200, 100, 5, (1, 2, 3))                        # 3 x 100 chains > max_batch
+        assert e.value.status == nsgpu.ESHAPE
+        with pytest.raises(nsgpu.NsgpuError) as e:
+            ctx.run_multi(200, 100, 5, ())
+        assert e.value.status == nsgpu.EINVAL
