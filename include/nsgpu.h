@@ -131,6 +131,9 @@ typedef struct {
                                 * L2-resident scratch) wherever the shape allows it (width 512, even n_hidden, n_in 6/7/9);
                                 * bit-identical to the layered path; opt-in (measured no faster: profiles/r2_fused_mlp.md) */
 #define NSGPU_MLP_LAYERED 512u /* one kernel per layer, activations through HBM (the default) */
+#define NSGPU_MLP_FP64 1024u   /* precision study: CUDA-core MLP with fp64 activations and accumulation (fp32 weights as
+                                * given, fp32 spectrum table); implies the SIMT path */
+#define NSGPU_MLP_SPLIT4 2048u /* precision study: tcgen05 path with the fourth product lo.lo added (16 MMAs per k-block, not 12) */
 #define NSGPU_NO_PDL 128u /* launch every kernel with plain stream ordering (default: the kernels of a likelihood call and of a
                             * slice-sampling round are chained by programmatic dependent launch) */
 

@@ -356,7 +356,7 @@ nsgpu_status create_impl(nsgpu_ctx* ctx, int32_t D, const nsgpu_prior1d* prior, 
   const size_t M_max = (size_t)max_batch * ctx->rows_per_theta;
   if (n_emu > 0) {
     // fp32 [M][width] (SIMT) or two fp16 planes in 128-row tiles (tcgen05): pad M to a multiple of 128
-    const size_t act_bytes = ((M_max + 127) / 128 * 128) * (size_t)width_max * sizeof(float);
+    const size_t act_bytes = ((M_max + 127) / 128 * 128) * (size_t)width_max * ((flags & NSGPU_MLP_FP64) ? sizeof(double) : sizeof(float));
     NSGPU_CUDA(cudaMalloc(&ctx->act[0], act_bytes));
     NSGPU_CUDA(cudaMalloc(&ctx->act[1], act_bytes));
     ctx->spec_ld = th->kind == 3 ? emu[0].n_out : (emu[0].n_out + 3) & ~3;
@@ -383,7 +383,7 @@ nsgpu_status create_impl(nsgpu_ctx* ctx, int32_t D, const nsgpu_prior1d* prior, 
       ctx->err = "NSGPU_MLP_TC: tcgen05 path needs width % 64 == 0, 64 <= width <= 512 and an sm_100 device";
       return NSGPU_ESHAPE;
     }
-    E.path = ((flags & 3u) != NSGPU_MLP_SIMT && tc_ok) ? 1 : 0;
+    E.path = ((flags & 3u) != NSGPU_MLP_SIMT && (flags & NSGPU_MLP_FP64) == 0 && tc_ok) ? 1 : 0;
     if (E.path == 1) {
       nsgpu_status s = mlp_tc_prepare(ctx, e, &emu[e]);
       if (s != NSGPU_OK) return s;

@@ -73,6 +73,7 @@ struct GemmArgs {
   int rows_per_theta;
   int K;                      // fan-in (multiple of 64)
   int kpp;                    // k-blocks accumulated in TMEM per partial (1, 2, 4 ...; see mlp_gemm_tc)
+  int split4;                 // precision study: also issue the lo.lo product (NSGPU_MLP_SPLIT4)
   int N_pad;                  // padded fan-out (multiple of BLOCK_N)
   int n_valid;                // true fan-out
   const __half *a_hi, *a_lo;  // input planes, canonical layout, K columns
@@ -442,10 +443,15 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) mlp_gemm_tc(const __grid_cons
                                            : tc::smem_desc_sw64(s0 + 2 * A_TILE_BYTES + B_TILE_BYTES);
             // Corrections first (in the first k-block of a partial the accumulator is still ~2^-11 of its final
             // size), hi.hi last.
+            if (g.split4) {
+#pragma unroll
+              for (int k = 0; k < BK / 16; ++k)
+                tc::mma_f16_ss(d_tmem, a_lo + (uint64_t)(256 * k), b_lo + (uint64_t)(2 * k), IDESC, (k != 0) | (kb != kb0));
+            }
 #pragma unroll
             for (int k = 0; k < BK / 16; ++k) {
               const uint64_t adv_a = (uint64_t)(256 * k), adv_b = (uint64_t)(2 * k);
-              tc::mma_f16_ss(d_tmem, a_lo + adv_a, b_hi + adv_b, IDESC, (k != 0) | (kb != kb0));
+              tc::mma_f16_ss(d_tmem, a_lo + adv_a, b_hi + adv_b, IDESC, (k != 0) | (kb != kb0) | (g.split4 != 0));
               tc::mma_f16_ss(d_tmem, a_hi + adv_a, b_lo + adv_b, IDESC, 1);
             }
 #pragma unroll
@@ -1177,7 +1183,7 @@ namespace {
 // 9% better at B = 256, and 2% slower inside a nested-sampling run (rounds of ~300 proposals).
 bool use_fused(const nsgpu_ctx* ctx, const TcState* T, int M) {
   (void)M;
-  return T->fused_ok && (ctx->flags & NSGPU_MLP_FUSED) != 0 && (ctx->flags & NSGPU_MLP_LAYERED) == 0;
+  return T->fused_ok && (ctx->flags & NSGPU_MLP_FUSED) != 0 && (ctx->flags & (NSGPU_MLP_LAYERED | NSGPU_MLP_SPLIT4)) == 0;
 }
 
 template <int BN_O, int NIN, int OUT_MODE>
@@ -1273,7 +1279,7 @@ nsgpu_status mlp_forward_tc(nsgpu_ctx* ctx, int e, const float* theta, int B, co
     GemmArgs g;
     memset(&g, 0, sizeof(g));
     g.M_host = M; g.n_rows_dev = n_rows_dev; g.rows_per_theta = rpt; g.K = L.K; g.N_pad = L.N_pad; g.n_valid = L.n_valid;
-    g.p_hidden = L.p_hidden; g.p_out = (mode & NSGPU_SPEC_NOMEAN) ? L.p_out_nm : L.p_out; g.p_out4 = (mode & NSGPU_SPEC_NOMEAN) ? L.p_out4_nm : L.p_out4; g.cscale = ldexpf(1.0f, -(L.wexp + 4)) * trunc_comp(L.K, T->bk, T->kpp); g.kpp = T->kpp;
+    g.p_hidden = L.p_hidden; g.p_out = (mode & NSGPU_SPEC_NOMEAN) ? L.p_out_nm : L.p_out; g.p_out4 = (mode & NSGPU_SPEC_NOMEAN) ? L.p_out4_nm : L.p_out4; g.cscale = ldexpf(1.0f, -(L.wexp + 4)) * trunc_comp(L.K, T->bk, T->kpp); g.kpp = T->kpp; g.split4 = (ctx->flags & NSGPU_MLP_SPLIT4) ? 1 : 0;
     g.a_hi = T->act[cur][0]; g.a_lo = T->act[cur][1];
     g.out_hi = T->act[cur ^ 1][0]; g.out_lo = T->act[cur ^ 1][1]; g.ld_out = E.width;
     g.out_f32 = spec_out; g.ld_f32 = ld_spec; g.apply_exp10 = (mode & NSGPU_SPEC_EXP10) ? 1 : 0;

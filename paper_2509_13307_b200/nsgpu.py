@@ -22,6 +22,7 @@ CHI2_STREAMED, CHI2_TILED = 8, 16   # OR into `mlp`: force one of the two chi^2 
 MLP_CLUSTER, MLP_NO_CLUSTER = 32, 64   # OR into `mlp`: weight-multicast CTA pairs always / never (default: large batches)
 SHEAR_STREAM = 4          # OR into `mlp`: streaming projection kernels even for grids that fit shared memory
 MLP_FUSED, MLP_LAYERED = 256, 512   # OR into `mlp`: fused multi-layer tcgen05 kernel where the shape allows (opt-in) / layered (default)
+MLP_FP64, MLP_SPLIT4 = 1024, 2048   # OR into `mlp`: precision-study modes (fp64 CUDA-core emulator; 4-product tcgen05 split)
 NO_PDL = 128              # OR into `mlp`: plain stream ordering between kernels (default: programmatic dependent launch)
 
 EXPORTS = ["nsgpu_create", "nsgpu_destroy", "nsgpu_last_error", "nsgpu_prior_transform",
