@@ -134,6 +134,8 @@ typedef struct {
 #define NSGPU_MLP_FP64 1024u   /* precision study: CUDA-core MLP with fp64 activations and accumulation (fp32 weights as
                                 * given, fp32 spectrum table); implies the SIMT path */
 #define NSGPU_MLP_SPLIT4 2048u /* precision study: tcgen05 path with the fourth product lo.lo added (16 MMAs per k-block, not 12) */
+#define NSGPU_NO_OVERLAP 4096u  /* kind 3: keep the theta-only half of the projection on the caller's stream (default: on a side
+                                 * stream, under the emulator kernels) */
 #define NSGPU_NO_PDL 128u /* launch every kernel with plain stream ordering (default: the kernels of a likelihood call and of a
                             * slice-sampling round are chained by programmatic dependent launch) */
 
@@ -247,7 +249,9 @@ NSGPU_API nsgpu_status nsgpu_debug_philox(nsgpu_ctx* ctx, const uint32_t* ctr, i
 
 /* Per-stage device timing with CUDA events recorded on the caller's stream around the library's own
  * launches (for roofline accounting; off by default).  Stages: 0 first emulator layer (a2+a3),
- * 1 hidden-layer GEMMs (a3), 2 output-layer GEMM (a4), 3 shear projection (a5-a8), 4 CMB binning (a9),
+ * 1 hidden-layer GEMMs (a3; the whole MLP when it is the fused kernel), 2 output-layer GEMM (a4), 3 shear projection
+ * (a5-a8; without NSGPU_NO_OVERLAP only the half that reads the table: the theta-only half runs on a side stream under
+ * the MLP stages), 4 CMB binning (a9),
  * 5 chi^2 (a10), 6 slice round + compaction (a11-a12), 7 identity/emulator copy.
  * nsgpu_stage_times synchronises the device, adds the elapsed times since the last call into
  * ms[8] / count[8] (HOST, overwritten) and resets the accumulators.                                 */

@@ -375,6 +375,11 @@ nsgpu_status create_impl(nsgpu_ctx* ctx, int32_t D, const nsgpu_prior1d* prior, 
 
   NSGPU_CUDA(cudaMalloc((void**)&ctx->nonfinite_rows, sizeof(unsigned long long)));
   NSGPU_CUDA(cudaMemset(ctx->nonfinite_rows, 0, sizeof(unsigned long long)));
+  if (th->kind == 3) {
+    NSGPU_CUDA(cudaStreamCreateWithFlags(&ctx->side_stream, cudaStreamNonBlocking));
+    NSGPU_CUDA(cudaEventCreateWithFlags(&ctx->ev_in, cudaEventDisableTiming));
+    NSGPU_CUDA(cudaEventCreateWithFlags(&ctx->ev_side, cudaEventDisableTiming));
+  }
   // MLP path selection
   for (int e = 0; e < n_emu; ++e) {
     EmuDev& E = ctx->emu[e];
@@ -427,6 +432,9 @@ extern "C" nsgpu_status nsgpu_destroy(nsgpu_ctx* ctx) {
   nsgpu_probe_release(ctx);
   cudaDeviceSynchronize();
   sampler_destroy(ctx);
+  if (ctx->side_stream) cudaStreamDestroy(ctx->side_stream);
+  if (ctx->ev_in) cudaEventDestroy(ctx->ev_in);
+  if (ctx->ev_side) cudaEventDestroy(ctx->ev_side);
   for (auto& ev : ctx->stage_events) { cudaEventDestroy(ev.a); cudaEventDestroy(ev.b); }
   for (cudaEvent_t ev : ctx->event_pool) cudaEventDestroy(ev);
   for (size_t e = 0; e < ctx->emu.size(); ++e) {
@@ -504,8 +512,24 @@ static nsgpu_status run_emulators(nsgpu_ctx* ctx, const float* theta, int B, con
 }
 
 static nsgpu_status theory_device(nsgpu_ctx* ctx, const float* theta, int B, const int* n_rows_dev, cudaStream_t st) {
+  // Shear: background and windows (a6-a7) depend on theta only, so they run on a side stream while the emulator
+  // kernels (tensor-bound; the fp64 pipe is idle) work on `st`: theta is ready at ev_in, the table half waits for
+  // ev_side.  The next call's ev_in is recorded after this call's table half, which orders the reuse of `aux`.
+  const bool overlap = ctx->kind == 3 && ctx->side_stream && B > 0 && (ctx->flags & NSGPU_NO_OVERLAP) == 0 &&
+                       shear_has_split(ctx);
+  if (overlap) {
+    NSGPU_CUDA(cudaEventRecord(ctx->ev_in, st));
+    NSGPU_CUDA(cudaStreamWaitEvent(ctx->side_stream, ctx->ev_in, 0));
+    nsgpu_status s1 = shear_project(ctx, theta, B, n_rows_dev, ctx->side_stream, 1);
+    if (s1 != NSGPU_OK) return s1;
+    NSGPU_CUDA(cudaEventRecord(ctx->ev_side, ctx->side_stream));
+  }
   nsgpu_status s = run_emulators(ctx, theta, B, n_rows_dev, st);
   if (s != NSGPU_OK) return s;
+  if (overlap) {
+    NSGPU_CUDA(cudaStreamWaitEvent(st, ctx->ev_side, 0));
+    return shear_project(ctx, theta, B, n_rows_dev, st, 2);
+  }
   switch (ctx->kind) {
     case 0:
     case 1:

@@ -95,6 +95,8 @@ struct nsgpu_ctx {
   double* logL_pinned = nullptr;
   SamplerDev* sampler = nullptr;
   void* probe = nullptr;               // clock probe state (probe.cu)
+  cudaStream_t side_stream = nullptr;  // shear: the theta-only half of the projection runs here, under the emulator kernels
+  cudaEvent_t ev_in = nullptr, ev_side = nullptr;
   std::string err;
   int64_t launches = 0;
   unsigned long long* nonfinite_rows = nullptr;   // device counter: emulator rows with non-finite output (tcgen05 path)
@@ -111,7 +113,7 @@ struct nsgpu_ctx {
 struct StageTimer {
   nsgpu_ctx* ctx; cudaStream_t st; int idx = -1;
   StageTimer(nsgpu_ctx* c, int stage, cudaStream_t s) : ctx(c), st(s) {
-    if (!c->profiling) return;
+    if (!c->profiling || stage < 0) return;
     nsgpu_ctx::StageEv ev; ev.stage = stage;
     for (cudaEvent_t* e : {&ev.a, &ev.b}) {
       if (!c->event_pool.empty()) { *e = c->event_pool.back(); c->event_pool.pop_back(); }
@@ -194,7 +196,8 @@ nsgpu_status mlp_forward_tc(nsgpu_ctx* ctx, int e, const float* theta, int B, co
                             float* spec_out, int ld_spec, int mode, cudaStream_t st);
 nsgpu_status mlp_tc_prepare(nsgpu_ctx* ctx, int e, const nsgpu_emulator* h);
 void mlp_tc_release(nsgpu_ctx* ctx, int e);
-nsgpu_status shear_project(nsgpu_ctx* ctx, const float* theta, int B, const int* n_rows_dev, cudaStream_t st);
+nsgpu_status shear_project(nsgpu_ctx* ctx, const float* theta, int B, const int* n_rows_dev, cudaStream_t st, int phases = 3);
+bool shear_has_split(const nsgpu_ctx* ctx);
 size_t shear_resident_smem(const ShearDev& S);
 nsgpu_status cmb_bin(nsgpu_ctx* ctx, const float* theta, int B, const int* n_rows_dev, cudaStream_t st);
 nsgpu_status cmb_tt_loglike(nsgpu_ctx* ctx, const float* theta, int B, const int* n_rows_dev, double* logL, cudaStream_t st);

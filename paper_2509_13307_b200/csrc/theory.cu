@@ -912,7 +912,9 @@ static size_t shear_smem_bytes(const ShearDev& S) {
   return d * sizeof(double) + (size_t)S.n_z_emu * S.n_k * sizeof(float) + 16;
 }
 
-nsgpu_status shear_project(nsgpu_ctx* ctx, const float* theta, int B, const int* n_rows_dev, cudaStream_t st) {
+// `phases`: 1 = the theta-only half (background, windows -> aux), 2 = the half that reads the emulated table, 3 = both.
+// api.cu runs phase 1 on a side stream under the emulator kernels (its inputs do not depend on them).
+nsgpu_status shear_project(nsgpu_ctx* ctx, const float* theta, int B, const int* n_rows_dev, cudaStream_t st, int phases) {
   if (B == 0) return NSGPU_OK;
   const ShearDev& S = ctx->sh;
   ShearArgs A;
@@ -924,7 +926,9 @@ nsgpu_status shear_project(nsgpu_ctx* ctx, const float* theta, int B, const int*
   A.idx_omega_b = S.idx_omega_b; A.idx_omega_cdm = S.idx_omega_cdm; A.idx_h = S.idx_h; A.idx_w0 = S.idx_w0;
   A.idx_wa = S.idx_wa; A.idx_eta0 = S.idx_eta0; A.idx_dz = S.idx_dz; A.idx_ia = S.idx_ia; A.idx_m = S.idx_m;
   A.n_ia_terms = S.n_ia_terms; A.n_m_terms = S.n_m_terms;
-  StageTimer tm(ctx, 3, st);
+  // stage 3 is the half that reads the table (the HBM-roofline kernel); the theta-only half is timed with it only when it
+  // runs on the same stream -- on the side stream it sits under the MLP stages
+  StageTimer tm(ctx, (phases & 2) ? 3 : -1, st);
   if (S.streaming) {
     const size_t nqp = (size_t)S.n_chi | 1;
     // bins per scan pass: as many as keep the windows kernel at three CTAs per SM
@@ -940,9 +944,12 @@ nsgpu_status shear_project(nsgpu_ctx* ctx, const float* theta, int B, const int*
     }
     const int KS = (LIMBER_THREADS / 32) / MP;
     const size_t smem_l = std::max((size_t)2 * (S.n_tomo + 1 + NT * 8) * LIMBER_LD + 2, (size_t)KS * MT * 8 * NT * 8) * sizeof(double);
-    NSGPU_CUDA(nsgpu_ensure_smem(ctx, shear_windows_kernel, smem_w));
-    NSGPU_CUDA(launch_pdl(ctx, shear_windows_kernel, dim3(B), dim3(win_threads), smem_w, st, theta, ctx->D, n_rows_dev, A, G, S.aux));
-    NSGPU_LAUNCH_CHECK();
+    if (phases & 1) {
+      NSGPU_CUDA(nsgpu_ensure_smem(ctx, shear_windows_kernel, smem_w));
+      NSGPU_CUDA(launch_pdl(ctx, shear_windows_kernel, dim3(B), dim3(win_threads), smem_w, st, theta, ctx->D, n_rows_dev, A, G, S.aux));
+      NSGPU_LAUNCH_CHECK();
+    }
+    if (!(phases & 2)) return NSGPU_OK;
     const int bpt = (((S.n_ell + 3) / 4) * S.n_chi + 255) / 256;
     NSGPU_CUDA(launch_pdl(ctx, shear_power_kernel, dim3((unsigned)((size_t)B * bpt)), dim3(256), 0, st, theta, ctx->D, n_rows_dev, ctx->spec, A, S.aux, bpt, S.pg));
     NSGPU_LAUNCH_CHECK();
@@ -965,10 +972,14 @@ nsgpu_status shear_project(nsgpu_ctx* ctx, const float* theta, int B, const int*
   const bool split = ((size_t)S.n_z_emu * S.n_k * 4) % 16 == 0 && ((size_t)(3 + S.n_tomo) * S.n_chi * 8) % 16 == 0 &&
                      ((size_t)3 * S.n_chi * 8) % 16 == 0 && S.aux != nullptr;
   if (split) {
-    NSGPU_CUDA(launch_pdl(ctx, shear_project_kernel<1>, dim3(B), dim3(128), smem1, st, theta, ctx->D, n_rows_dev, ctx->spec, A, S.aux, ctx->model, ctx->n_data));
-    NSGPU_LAUNCH_CHECK();
+    if (phases & 1) {
+      NSGPU_CUDA(launch_pdl(ctx, shear_project_kernel<1>, dim3(B), dim3(128), smem1, st, theta, ctx->D, n_rows_dev, ctx->spec, A, S.aux, ctx->model, ctx->n_data));
+      NSGPU_LAUNCH_CHECK();
+    }
+    if (!(phases & 2)) return NSGPU_OK;
     NSGPU_CUDA(launch_pdl(ctx, shear_project_kernel<2>, dim3(B), dim3(SHEAR_THREADS), smem, st, theta, ctx->D, n_rows_dev, ctx->spec, A, S.aux, ctx->model, ctx->n_data));
   } else {
+    if (!(phases & 2)) return NSGPU_OK;          // no split possible: everything in phase 2
     NSGPU_CUDA(launch_pdl(ctx, shear_project_kernel<0>, dim3(B), dim3(SHEAR_THREADS), smem, st, theta, ctx->D, n_rows_dev, ctx->spec, A, S.aux, ctx->model, ctx->n_data));
   }
   NSGPU_LAUNCH_CHECK();
@@ -977,6 +988,14 @@ nsgpu_status shear_project(nsgpu_ctx* ctx, const float* theta, int B, const int*
 
 // shared memory of the resident projection; the caller switches to the streaming kernels when it does not fit
 size_t shear_resident_smem(const ShearDev& S) { return shear_smem_bytes(S); }
+
+// can the theta-only half run as a launch of its own? (streaming kernels: always; resident: when the bulk-copy pieces align)
+bool shear_has_split(const nsgpu_ctx* ctx) {
+  const ShearDev& S = ctx->sh;
+  if (S.streaming) return true;
+  return ((size_t)S.n_z_emu * S.n_k * 4) % 16 == 0 && ((size_t)(3 + S.n_tomo) * S.n_chi * 8) % 16 == 0 &&
+         ((size_t)3 * S.n_chi * 8) % 16 == 0 && S.aux != nullptr;
+}
 
 nsgpu_status cmb_bin(nsgpu_ctx* ctx, const float* theta, int B, const int* n_rows_dev, cudaStream_t st) {
   if (B == 0) return NSGPU_OK;

@@ -23,6 +23,7 @@ MLP_CLUSTER, MLP_NO_CLUSTER = 32, 64   # OR into `mlp`: weight-multicast CTA pai
 SHEAR_STREAM = 4          # OR into `mlp`: streaming projection kernels even for grids that fit shared memory
 MLP_FUSED, MLP_LAYERED = 256, 512   # OR into `mlp`: fused multi-layer tcgen05 kernel where the shape allows (opt-in) / layered (default)
 MLP_FP64, MLP_SPLIT4 = 1024, 2048   # OR into `mlp`: precision-study modes (fp64 CUDA-core emulator; 4-product tcgen05 split)
+NO_OVERLAP = 4096         # OR into `mlp`: no side stream for the theta-only half of the shear projection
 NO_PDL = 128              # OR into `mlp`: plain stream ordering between kernels (default: programmatic dependent launch)
 
 EXPORTS = ["nsgpu_create", "nsgpu_destroy", "nsgpu_last_error", "nsgpu_prior_transform",

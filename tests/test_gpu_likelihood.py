@@ -326,6 +326,28 @@ def test_fused_mlp_is_bit_identical_to_the_layered_path(name, B):
     assert res[1][3] < res[0][3]                                          # one launch instead of one per layer
 
 
+@pytest.mark.parametrize("name,B", [("c3a", 300), ("c3b", 77), ("tiny_shear_paper", 21), ("c5i", 40)])
+def test_side_stream_projection_half_changes_nothing(name, B):
+    """the theta-only half of the shear projection runs on a side stream under the emulator kernels:
+    same bits as with everything on one stream, call after call (the hand-off buffer is reused), on the caller's
+    stream and through the host entry"""
+    wl = workload(name)
+    theta = theta_of_u(wl, np.concatenate([W.u_post_set(wl, B // 2), W.u_prior_set(wl, B - B // 2)]))
+    with nsgpu.Context(wl, max_batch=B, mlp=nsgpu.NO_OVERLAP) as ctx:
+        ref = ctx.loglike_batch(dev(theta)).cpu().numpy()
+    with nsgpu.Context(wl, max_batch=B) as ctx:
+        s2 = torch.cuda.Stream()
+        for i in range(4):
+            t = dev(np.roll(theta, i, axis=0))
+            np.testing.assert_array_equal(ctx.loglike_batch(t).cpu().numpy(), np.roll(ref, i))
+        with torch.cuda.stream(s2):
+            got = ctx.loglike_batch(dev(theta), stream=s2)
+        s2.synchronize()
+        np.testing.assert_array_equal(got.cpu().numpy(), ref)
+        np.testing.assert_array_equal(ctx.loglike_batch_host(theta), ref)
+        np.testing.assert_array_equal(ctx.theory_batch(dev(theta)).cpu().numpy()[:3], ctx.theory_batch(dev(theta[:3])).cpu().numpy())
+
+
 def test_tensor_core_and_simt_paths_agree_on_shear():
     """the two on-device MLP paths (different table layouts into the projection) give the same log L"""
     wl = W.shear(seed=21, w0wa=True, n_z_emu=9, n_z=9, width=64, n_hidden=2, n_k=40, n_chi=24, n_ell=6, n_tomo=3, name="s64")
