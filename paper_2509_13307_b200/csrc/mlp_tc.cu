@@ -233,6 +233,14 @@ __global__ void __launch_bounds__(256) mlp_first_layer_tc(const float* __restric
   }
 }
 
+// Store under a predicate, never a branch.  The [theta][k][z] table epilogue does 2 x 56 guarded stores per thread and tile;
+// whether the compiler predicates them or builds a convergence region around each one is a heuristic that flipped with
+// unrelated changes to the kernel this round (output layer 0.289 -> 0.338 ms on c3a with identical arithmetic, found by
+// bisecting against the round-1 build and diffing the SASS); with the predicate written out: 0.303 ms.
+__device__ __forceinline__ void st_global_if(float* p, float v, bool ok) {
+  asm volatile("{\n.reg .pred q;\nsetp.ne.b32 q, %2, 0;\n@q st.global.f32 [%0], %1;\n}" ::"l"(p), "f"(v), "r"((int)ok) : "memory");
+}
+
 // Epilogue of NP column pairs (pairs P0 .. P0+NP-1 of the thread's CPT/2; a[i] is pair P0 + i) of one accumulator
 // row: EPI 0 bias + gated activation + hi/lo split into the next layer's canonical planes; EPI 1 de-standardised
 // fp32 output (row-major, or [theta][n][z] for the shear table).
@@ -276,8 +284,8 @@ __device__ __forceinline__ void epi_pairs(const f32x2* a, const TileRef& t, cons
         upk2(fma2(a[j], pk2(pj.x, pj.y), pk2(pj.z, pj.w)), y0, y1);
         if (exp10_on) { y0 = exp10f(y0); y1 = exp10f(y1); }
         const int n = n0 + 2 * j;
-        if (t.row_ok && n < g.n_valid) dst[(size_t)n * g.rows_per_theta] = y0;
-        if (t.row_ok && n + 1 < g.n_valid) dst[(size_t)(n + 1) * g.rows_per_theta] = y1;
+        st_global_if(dst + (size_t)n * g.rows_per_theta, y0, t.row_ok && n < g.n_valid);
+        st_global_if(dst + (size_t)(n + 1) * g.rows_per_theta, y1, t.row_ok && n + 1 < g.n_valid);
       }
     } else {
       float* dst = g.out_f32 + (size_t)rr * g.ld_f32 + n0;
