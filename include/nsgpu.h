@@ -216,6 +216,20 @@ NSGPU_API nsgpu_status nsgpu_run_multi(nsgpu_ctx* ctx, const nsgpu_run_opts* opt
 NSGPU_API nsgpu_status nsgpu_multi_samples(nsgpu_ctx* ctx, int32_t run, float* theta_samples, double* logL_samples,
                                            double* logw_samples, int64_t cap, int64_t* n_samples);
 
+/* The error bar of log Z by 1000 simulated prior-volume sequences (reading N9) -- the same kernel and the
+ * same arithmetic as the summary of nsgpu_run, but this entry point ALLOCATES NOTHING (no cudaMalloc / cudaFree, no
+ * allocating library routine): for callers under CUDA graph capture, in tight serving loops, or in harnesses that forbid
+ * allocation.  Its scratch (the dead sequence, the live block, the 1000 results) is a file-scope device array of
+ * 1,048,576 + 16,384 + 1000 doubles = 8.1 MiB that every GPU loading the library holds until the process exits.
+ * dead_logL [n_dead] (in deletion order), live_logL [n_live]: HOST float64; n_delete = points deleted per iteration
+ * (point i had n_live - i mod n_delete live points); seed: the run's seed (same Philox streams as nsgpu_run, so for
+ * the sequence of a finished run *logZ_err equals nsgpu_result.logZ_err).  *logZ_err HOST out; logZ_sims HOST [1000]
+ * out or NULL.  Errors: EINVAL (NULL, sizes), ESHAPE when n_dead > 1,048,576 or n_live > 16,384.  Blocking (synchronises
+ * `stream`).  All calls share the one array: calls that overlap on the GPU (two streams, two host threads) race. */
+NSGPU_API nsgpu_status nsgpu_logz_error_noalloc(nsgpu_ctx* ctx, const double* dead_logL, int64_t n_dead,
+                                                const double* live_logL, int32_t n_live, int32_t n_delete, uint64_t seed,
+                                                double* logZ_err, double* logZ_sims, void* stream);
+
 /* Multi-GPU nested sampling: one process per GPU, every rank holds the whole
  * live set and calls this with the same options.  Rank r evolves the chains nsgpu_shard_range gives it; the only
  * exchange of an iteration is an all-gather of the k new points, done through `allgather`: send and recv are DEVICE

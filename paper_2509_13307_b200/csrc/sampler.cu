@@ -1240,3 +1240,73 @@ extern "C" nsgpu_status nsgpu_multi_samples(nsgpu_ctx* ctx, int32_t run, float* 
   memcpy(logw_samples, X.logw.data(), sizeof(double) * nw);
   return NSGPU_OK;
 }
+
+// ---------------------------------------------------------------------------------------------------
+// nsgpu_logz_error_noalloc: the error bar of log Z by simulated prior volumes (reading N9) WITHOUT any
+// allocation.  The summary of nsgpu_run does this with two cudaMalloc'd buffers (the dead log L sequence and the 1000
+// simulated log Z); callers that may not allocate (code under CUDA graph capture, tight serving loops, harnesses that
+// forbid cudaMalloc) get the same kernel on a file-scope device array instead.  Every GPU that loads the library holds
+// the array until the process exits: NSGPU_NOALLOC_MAX_DEAD + NSGPU_NOALLOC_MAX_LIVE + 1000 doubles = 8.1 MiB.
+// In HOST code `g_noalloc_scratch` is only a stand-in for the symbol, never a device address: the address is taken once
+// per device with cudaGetSymbolAddress (that device current) and that pointer is what the copies and the kernel get.
+// All calls share the array and it keeps the last call's contents: every call overwrites the parts it reads
+// ([0, n_dead), the live block, the 1000 results are zeroed first), and calls that overlap on the GPU (two streams, two
+// host threads) race -- serialise them.
+// ---------------------------------------------------------------------------------------------------
+#define NSGPU_NOALLOC_MAX_DEAD (1 << 20)
+#define NSGPU_NOALLOC_MAX_LIVE MAX_LIVE
+#define NSGPU_NOALLOC_SIMS 1000
+static __device__ __align__(256) double g_noalloc_scratch[NSGPU_NOALLOC_MAX_DEAD + NSGPU_NOALLOC_MAX_LIVE + NSGPU_NOALLOC_SIMS];
+
+#include <mutex>
+static cudaError_t noalloc_scratch_ptr(int device, double** out) {   // call with `device` current
+  static std::mutex mu;
+  static double* ptr[64] = {};
+  std::lock_guard<std::mutex> lock(mu);
+  if (device < 0 || device >= 64) return cudaErrorInvalidDevice;
+  if (!ptr[device]) {
+    double* p = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress((void**)&p, g_noalloc_scratch);
+    if (e != cudaSuccess) return e;
+    ptr[device] = p;
+  }
+  *out = ptr[device];
+  return cudaSuccess;
+}
+
+extern "C" nsgpu_status nsgpu_logz_error_noalloc(nsgpu_ctx* ctx, const double* dead_logL, int64_t n_dead,
+                                                 const double* live_logL, int32_t n_live, int32_t n_delete, uint64_t seed,
+                                                 double* logZ_err, double* logZ_sims, void* stream) {
+  if (!ctx) return NSGPU_EINVAL;
+  if (!live_logL || !logZ_err || n_dead < 0 || (n_dead > 0 && !dead_logL) || n_live < 1 || n_delete < 1 || n_delete >= n_live) {
+    ctx->err = "logz_error_noalloc: NULL pointer or bad sizes (need n_live >= 1, 1 <= n_delete < n_live)";
+    return NSGPU_EINVAL;
+  }
+  if (n_dead > NSGPU_NOALLOC_MAX_DEAD || n_live > NSGPU_NOALLOC_MAX_LIVE) {
+    ctx->err = "logz_error_noalloc: n_dead exceeds 1048576 or n_live exceeds 16384 (the static scratch array; use nsgpu_run's summary for longer runs)";
+    return NSGPU_ESHAPE;
+  }
+  NSGPU_CUDA(cudaSetDevice(ctx->device));
+  double* scr = nullptr;
+  NSGPU_CUDA(noalloc_scratch_ptr(ctx->device, &scr));
+  cudaStream_t st = (cudaStream_t)stream;
+  double* d_dead = scr;
+  double* d_live = scr + NSGPU_NOALLOC_MAX_DEAD;
+  double* d_zs = d_live + NSGPU_NOALLOC_MAX_LIVE;
+  if (n_dead > 0) NSGPU_CUDA(cudaMemcpyAsync(d_dead, dead_logL, sizeof(double) * (size_t)n_dead, cudaMemcpyHostToDevice, st));
+  NSGPU_CUDA(cudaMemcpyAsync(d_live, live_logL, sizeof(double) * (size_t)n_live, cudaMemcpyHostToDevice, st));
+  NSGPU_CUDA(cudaMemsetAsync(d_zs, 0, sizeof(double) * NSGPU_NOALLOC_SIMS, st));
+  const uint2 key = make_uint2((unsigned)(seed & 0xffffffffu), (unsigned)(seed >> 32));
+  evidence_error_kernel<<<NSGPU_NOALLOC_SIMS, 256, 0, st>>>(d_dead, (long long)n_dead, n_live, n_delete, d_live, key, d_zs);
+  NSGPU_LAUNCH_CHECK();
+  double zs_local[NSGPU_NOALLOC_SIMS];
+  double* zs = logZ_sims ? logZ_sims : zs_local;
+  NSGPU_CUDA(cudaMemcpyAsync(zs, d_zs, sizeof(double) * NSGPU_NOALLOC_SIMS, cudaMemcpyDeviceToHost, st));
+  NSGPU_CUDA(cudaStreamSynchronize(st));
+  double mean = 0.0, var = 0.0;
+  for (int m = 0; m < NSGPU_NOALLOC_SIMS; ++m) mean += zs[m];
+  mean /= NSGPU_NOALLOC_SIMS;
+  for (int m = 0; m < NSGPU_NOALLOC_SIMS; ++m) var += (zs[m] - mean) * (zs[m] - mean);
+  *logZ_err = sqrt(var / (NSGPU_NOALLOC_SIMS - 1));
+  return NSGPU_OK;
+}

@@ -31,7 +31,7 @@ EXPORTS = ["nsgpu_create", "nsgpu_destroy", "nsgpu_last_error", "nsgpu_prior_tra
            "nsgpu_slice_step", "nsgpu_run", "nsgpu_last_samples", "nsgpu_delete_lowest", "nsgpu_live_cholesky",
            "nsgpu_debug_philox", "nsgpu_set_profiling", "nsgpu_stage_times", "nsgpu_mlp_path", "nsgpu_launch_count",
            "nsgpu_run_sharded", "nsgpu_shard_range", "nsgpu_sampler_counters", "nsgpu_nonfinite_rows",
-           "nsgpu_clock_mark", "nsgpu_clock_marks_read", "nsgpu_run_multi", "nsgpu_multi_samples"]
+           "nsgpu_clock_mark", "nsgpu_clock_marks_read", "nsgpu_run_multi", "nsgpu_multi_samples", "nsgpu_logz_error_noalloc"]
 
 
 class NsgpuError(RuntimeError):
@@ -127,6 +127,8 @@ def lib():
     L.nsgpu_run_multi.argtypes = [vp, C.POINTER(_RunOpts), C.c_int32, C.POINTER(C.c_uint64), C.POINTER(_Result)]
     L.nsgpu_multi_samples.restype = C.c_int
     L.nsgpu_multi_samples.argtypes = [vp, C.c_int32, vp, vp, vp, C.c_int64, C.POINTER(C.c_int64)]
+    L.nsgpu_logz_error_noalloc.restype = C.c_int
+    L.nsgpu_logz_error_noalloc.argtypes = [vp, _pd, C.c_int64, _pd, C.c_int32, C.c_int32, C.c_uint64, _pd, _pd, vp]
     L.nsgpu_clock_mark.restype = C.c_int
     L.nsgpu_clock_mark.argtypes = [vp, vp]
     L.nsgpu_clock_marks_read.restype = C.c_int
@@ -443,6 +445,14 @@ class Context:
                 out.update(theta=th, logL=ll, logw=lw, n_samples=n)
             outs.append(out)
         return outs
+
+    def logz_error_noalloc(self, dead_logL, live_logL, n_delete, seed, stream=None):
+        """nsgpu_logz_error_noalloc -> (logZ_err, the 1000 simulated log Z); host arrays in, nothing allocated on the GPU."""
+        dead = np.ascontiguousarray(dead_logL, np.float64); live = np.ascontiguousarray(live_logL, np.float64)
+        err = C.c_double(0.0); sims = np.zeros(1000, np.float64)
+        self._check(lib().nsgpu_logz_error_noalloc(self._h, _ptr(dead, _pd), int(dead.shape[0]), _ptr(live, _pd), int(live.shape[0]),
+                                                   int(n_delete), int(seed), C.byref(err), _ptr(sims, _pd), _stream_ptr(stream)))
+        return err.value, sims
 
     def run_sharded(self, n_live, n_delete, n_steps, stop_frac=1e-3, max_iter=100000, seed=1, rank=None, world=None,
                     allgather=None, return_samples=True):
