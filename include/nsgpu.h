@@ -134,8 +134,8 @@ typedef struct {
 #define NSGPU_MLP_FP64 1024u   /* precision study: CUDA-core MLP with fp64 activations and accumulation (fp32 weights as
                                 * given, fp32 spectrum table); implies the SIMT path */
 #define NSGPU_MLP_SPLIT4 2048u /* precision study: tcgen05 path with the fourth product lo.lo added (16 MMAs per k-block, not 12) */
-#define NSGPU_NO_OVERLAP 4096u  /* kind 3: keep the theta-only half of the projection on the caller's stream (default: on a side
-                                 * stream, under the emulator kernels) */
+#define NSGPU_NO_OVERLAP 4096u  /* kind 3: keep the theta-only half of the projection on the caller's stream (default: batches of
+                                 * at most 1024 run it on a side stream, under the emulator kernels) */
 #define NSGPU_NO_PDL 128u /* launch every kernel with plain stream ordering (default: the kernels of a likelihood call and of a
                             * slice-sampling round are chained by programmatic dependent launch) */
 

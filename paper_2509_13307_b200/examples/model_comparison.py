@@ -81,9 +81,16 @@ def main():
     ap.add_argument("--ctx-flags", type=int, default=0, help="extra nsgpu_create flags, e.g. 128 = NSGPU_NO_PDL (plain stream ordering)")
     ap.add_argument("--batched", action="store_true", help="all seeds of a model in one nsgpu_run_multi call (shared likelihood batches)")
     ap.add_argument("--ranks", type=int, default=1, help="GPUs: start this many ranks under torch.distributed.run (sharded runs)")
+    ap.add_argument("--print-shards", action="store_true",
+                    help="print which chains each rank would evolve (nsgpu_shard_range) and exit: needs no GPU")
     args = ap.parse_args()
     if args.ranks > 1 and "WORLD_SIZE" not in os.environ:
         raise SystemExit(_spawn(args.ranks))
+    if args.print_shards:
+        world, rank = int(os.environ.get("WORLD_SIZE", "1")), int(os.environ.get("RANK", "0"))
+        first, count = nsgpu.shard_range(args.n_delete, rank, world)
+        print(json.dumps({"rank": rank, "world": world, "chains": [first, first + count], "of": args.n_delete}), flush=True)
+        return
     rank, world, dev = _ranks()
     if world > 1 and rank == 0:
         for r in range(world):
