@@ -285,6 +285,11 @@ nsgpu_status create_impl(nsgpu_ctx* ctx, int32_t D, const nsgpu_prior1d* prior, 
   if ((th->kind == 1 || th->kind == 4) && emu[0].n_out != n_data) { ctx->err = "emulator theory needs n_out == n_data"; return NSGPU_ESHAPE; }
   if (th->kind == 4 && (emu[0].out_kind != 1 || th->ell_min < 0)) { ctx->err = "cmb_tt_cv needs an exp10 emulator and ell_min >= 0"; return NSGPU_EINVAL; }
   if (th->kind == 3 && emu[0].n_out != th->n_k) { ctx->err = "shear: emulator n_out != n_k"; return NSGPU_ESHAPE; }
+  if (th->kind == 3) {
+    std::vector<double> mu((size_t)th->n_k);
+    for (int i = 0; i < th->n_k; ++i) mu[i] = (double)emu[0].out_mean[i];
+    NSGPU_CUDA(upload(&ctx->sh.mu_k, mu.data(), mu.size()));
+  }
   if (th->kind == 2) {
     if (!th->bin_ptr || !th->bin_col || !th->bin_val || th->cal_index < 0 || th->cal_index >= D) {
       ctx->err = "cmb_binned: NULL binning matrix or bad cal_index";
@@ -447,7 +452,7 @@ extern "C" nsgpu_status nsgpu_destroy(nsgpu_ctx* ctx) {
   cudaFree(ctx->emu_in_idx); cudaFree(ctx->emu_in_const); cudaFree(ctx->z_emu);
   cudaFree(ctx->bin_ptr); cudaFree(ctx->bin_col); cudaFree(ctx->bin_val);
   ShearDev& S = ctx->sh;
-  cudaFree(S.aux); cudaFree(S.pg); cudaFree(S.a_q); cudaFree(S.z_q); cudaFree(S.ln1pz); cudaFree(S.lellh); cudaFree(S.lf); cudaFree(S.tap_start); cudaFree(S.tap_w); cudaFree(S.ell); cudaFree(S.nz_mean);
+  cudaFree(S.aux); cudaFree(S.pg); cudaFree(S.mu_k); cudaFree(S.a_q); cudaFree(S.z_q); cudaFree(S.ln1pz); cudaFree(S.lellh); cudaFree(S.lf); cudaFree(S.tap_start); cudaFree(S.tap_w); cudaFree(S.ell); cudaFree(S.nz_mean);
   cudaFree(ctx->data); cudaFree(ctx->Linv); cudaFree(ctx->tt_a); cudaFree(ctx->tt_b); cudaFree(ctx->tt_mu);
   cudaFree(ctx->act[0]); cudaFree(ctx->act[1]); cudaFree(ctx->fused_scratch); cudaFree(ctx->spec); cudaFree(ctx->model); cudaFree(ctx->resid_t); cudaFree(ctx->chi2_part);
   cudaFree(ctx->theta_stage); cudaFree(ctx->logL_stage); cudaFree(ctx->nonfinite_rows);
@@ -511,7 +516,8 @@ static nsgpu_status run_emulators(nsgpu_ctx* ctx, const float* theta, int B, con
   const size_t stride = (size_t)ctx->max_batch * ctx->rows_per_theta * ctx->spec_ld;
   for (int e = 0; e < ctx->n_emu; ++e) {
     float* out = ctx->spec + e * stride;
-    const int mode = (ctx->spec_kz ? NSGPU_SPEC_KZ : 0) | (ctx->kind == 4 ? NSGPU_SPEC_NOMEAN : 0);
+    // kinds 3 and 4: the fp32 table carries only the O(sigma_out) deviation y - mu_out; the consumer adds mu_out in fp64
+    const int mode = (ctx->spec_kz ? NSGPU_SPEC_KZ : 0) | ((ctx->kind == 4 || ctx->kind == 3) ? NSGPU_SPEC_NOMEAN : 0);
     nsgpu_status s = ctx->emu[e].path == 1 ? mlp_forward_tc(ctx, e, theta, B, n_rows_dev, out, ctx->spec_ld, mode, st)
                                            : mlp_forward_simt(ctx, e, theta, B, n_rows_dev, out, ctx->spec_ld, mode & NSGPU_SPEC_NOMEAN, st);
     if (s != NSGPU_OK) return s;

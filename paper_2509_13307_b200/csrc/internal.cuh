@@ -46,6 +46,7 @@ struct ShearDev {
   int* tap_start = nullptr;                // [n_chi] first emulator z node used by node q
   double* tap_w = nullptr;                 // [n_chi][n_tap] z-interpolation weights (spline folded in)
   double *ell = nullptr, *nz_mean = nullptr;
+  double* mu_k = nullptr;                  // [n_k] emulator mu_out in fp64 (the spectrum table holds y - mu_out)
   double* aux = nullptr;                   // [max_batch][(3 + n_tomo) n_chi] hand-off between the two projection kernels
   double* pg = nullptr;                    // streaming path: [max_batch][n_ell][n_chi rounded up to even] P g_q
   int idx_omega_b = -1, idx_omega_cdm = -1, idx_h = -1, idx_w0 = -1, idx_wa = -1, idx_eta0 = -1;

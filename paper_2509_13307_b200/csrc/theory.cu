@@ -96,6 +96,7 @@ struct ShearArgs {
   int n_z_emu, n_chi, n_k, n_ell, n_tomo, n_tap;
   int sz, sk;   // table strides: element (z node m, k node j) at m sz + j sk
   double k_min, k_max, lk0, dlk, da, nz_sigma;
+  const double* mu_k;          // [n_k] mu_out of the emulator in fp64: the fp32 table holds y - mu_out
   const double *a_q, *z_q, *ln1pz, *tap_w, *ell, *lellh, *lf, *nz_mean;
   const int* tap_start;
   int idx_omega_b, idx_omega_cdm, idx_h, idx_w0, idx_wa, idx_eta0, idx_dz, idx_ia, idx_m, n_ia_terms, n_m_terms;
@@ -310,6 +311,8 @@ __global__ void __launch_bounds__(SHEAR_THREADS, 2) shear_project_kernel(const f
           }
         }
         double y = fma(s, hi - lo, lo);
+        const double mu0 = __ldg(A.mu_k + j);                  // the table holds the deviation from mu_out(k): add it in fp64
+        y += fma(s, __ldg(A.mu_k + j + 1) - mu0, mu0);
         const double k2 = k * k;
         y -= bar_amp * k2 * rcp_fast(k2 + 1.0);
         P = exp_fast(y * 2.302585092994046);
@@ -590,7 +593,7 @@ __global__ void __launch_bounds__(256) shear_power_kernel(const float* __restric
   const double* tw = A.tap_w + (size_t)q * A.n_tap;
   const float* col0 = table + (size_t)A.tap_start[q] * A.sz;
   const int l0 = 4 * lg, nl = min(4, A.n_ell - l0);
-  double kk[4], ss[4];
+  double kk[4], ss[4], mu[4];
   const float* r0[4];
   bool ok[4];
 #pragma unroll
@@ -603,6 +606,8 @@ __global__ void __launch_bounds__(256) shear_power_kernel(const float* __restric
     j = min(max(j, 0), A.n_k - 2);
     ss[u] = (x - (A.lk0 + j * A.dlk)) * inv_dlk;
     r0[u] = col0 + (size_t)j * A.sk;
+    const double mu0 = __ldg(A.mu_k + j);                      // the table holds the deviation from mu_out(k)
+    mu[u] = fma(ss[u], __ldg(A.mu_k + j + 1) - mu0, mu0);
   }
   double lo[4], hi[4];
   if (A.n_tap == 2) {
@@ -634,7 +639,7 @@ __global__ void __launch_bounds__(256) shear_power_kernel(const float* __restric
     if (u >= nl) break;
     double P = 0.0;
     if (ok[u]) {
-      double y = fma(ss[u], hi[u] - lo[u], lo[u]);
+      double y = fma(ss[u], hi[u] - lo[u], lo[u]) + mu[u];
       const double k2 = kk[u] * kk[u];
       const float k2f = (float)k2;                     // |bar_amp| <= 0.03: fp32 is 3e-9 of log10 P here
       y -= bar_amp * (double)__fdividef(k2f, k2f + 1.0f);
@@ -921,6 +926,7 @@ nsgpu_status shear_project(nsgpu_ctx* ctx, const float* theta, int B, const int*
   A.n_z_emu = S.n_z_emu; A.n_chi = S.n_chi; A.n_k = S.n_k; A.n_ell = S.n_ell; A.n_tomo = S.n_tomo; A.n_tap = S.n_tap;
   A.sz = ctx->spec_kz ? 1 : S.n_k; A.sk = ctx->spec_kz ? S.n_z_emu : 1;
   A.k_min = S.k_min; A.k_max = S.k_max; A.lk0 = S.lk0; A.dlk = S.dlk; A.da = S.da; A.nz_sigma = S.nz_sigma;
+  A.mu_k = S.mu_k;
   A.a_q = S.a_q; A.z_q = S.z_q; A.ln1pz = S.ln1pz; A.tap_w = S.tap_w; A.ell = S.ell; A.lellh = S.lellh; A.lf = S.lf;
   A.nz_mean = S.nz_mean; A.tap_start = S.tap_start;
   A.idx_omega_b = S.idx_omega_b; A.idx_omega_cdm = S.idx_omega_cdm; A.idx_h = S.idx_h; A.idx_w0 = S.idx_w0;
