@@ -453,7 +453,7 @@ def main():
     ap.add_argument("--impl", default="nsgpu", choices=["nsgpu", "reference"])
     ap.add_argument("--workload", default="c3a", choices=sorted(MAKERS))
     ap.add_argument("--batch", type=int, default=4096)
-    ap.add_argument("--cpu-sample", type=int, default=768)
+    ap.add_argument("--cpu-sample", type=int, default=1536)     # ~14 s of oracle work for c3a
     ap.add_argument("--ref-sample", type=int, default=16)
     ap.add_argument("--shear-stream", action="store_true",
                     help="shear workloads: use the streaming projection kernels even where the resident one fits")

@@ -478,3 +478,31 @@ def test_both_chi2_kernels(name, B):
             got_p = ctx.loglike_batch(dev(theta[perm])).cpu().numpy()
         assert np.all(np.abs(got - ref) <= loglike_tolerance(chi2)), flag
         np.testing.assert_array_equal(got_p, got[perm])
+
+
+def test_clock_marks_and_stage_timers():
+    """bench.py's measurement taps: clock marks give one plausible SM clock per interval between marks, stage timers count
+    every launch group of a likelihood call, and neither changes the result."""
+    wl = workload("toy_w64")
+    theta = theta_of_u(wl, W.u_prior_set(wl, 200))
+    with nsgpu.Context(wl, max_batch=200) as ctx:
+        t = dev(theta)
+        ref = ctx.loglike_batch(t).cpu().numpy()
+        assert ctx.clock_marks_read()[0].shape == (0,)                     # no marks yet
+        ctx.set_profiling(True)
+        ctx.stage_times()
+        l0 = ctx.launch_count()
+        ctx.clock_mark()
+        for _ in range(3):
+            got = ctx.loglike_batch(t)
+            ctx.clock_mark()
+        mhz, t_ms = ctx.clock_marks_read()
+        st = ctx.stage_times()
+        ctx.set_profiling(False)
+        n_launch = ctx.launch_count() - l0                                 # first layer, 2 hidden GEMMs, output, copy, chi^2 (marks not counted)
+        assert n_launch % 3 == 0 and 6 <= n_launch // 3 <= 8
+    np.testing.assert_array_equal(got.cpu().numpy(), ref)
+    assert mhz.shape == (3,) and np.all((mhz > 200.0) & (mhz < 2200.0)), mhz
+    assert np.all(np.diff(t_ms) > 0) and t_ms[0] > 0
+    assert st["mlp_first"][1] == 3 and st["mlp_hidden"][1] == 6 and st["mlp_out"][1] == 3 and st["chi2"][1] == 3
+    assert all(ms > 0 for ms, cnt in st.values() if cnt)
