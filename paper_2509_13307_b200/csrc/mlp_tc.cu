@@ -22,6 +22,7 @@
 #include <cuda.h>
 
 #include <cmath>
+#include <cstdio>
 #include <cstdlib>
 #include <cstring>
 
@@ -1027,6 +1028,16 @@ nsgpu_status launch_gemm_cluster(nsgpu_ctx* ctx, const CUtensorMap& whi, const C
   attr[1].val.programmaticStreamSerializationAllowed = (ctx->flags & NSGPU_NO_PDL) ? 0 : 1;
   cfg.attrs = attr;
   cfg.numAttrs = 2;
+  if (CS > 2) {   // clusters of more than two CTAs do not fit every SM (GPC sizes): a persistent grid must not exceed what is co-resident
+    static int max_clusters = -1;
+    if (max_clusters < 0) {
+      int n = 0;
+      if (cudaOccupancyMaxActiveClusters(&n, mlp_gemm_tc<BN, EPI, CS, BK>, &cfg) != cudaSuccess || n < 1) n = ctx->sm_count / CS;
+      max_clusters = n;
+      if (getenv("NSGPU_VERBOSE")) fprintf(stderr, "nsgpu: clusters of %d: %d co-resident\n", CS, n);
+    }
+    cfg.gridDim = dim3(std::min(clusters, max_clusters) * CS);
+  }
   NSGPU_CUDA(cudaLaunchKernelEx(&cfg, mlp_gemm_tc<BN, EPI, CS, BK>, whi, wlo, g));
   NSGPU_LAUNCH_CHECK();
   return NSGPU_OK;
@@ -1052,6 +1063,10 @@ nsgpu_status dispatch_gemm_bk(nsgpu_ctx* ctx, const TcLayer& L, const GemmArgs& 
     bool pair = m_blocks_all * (g.N_pad / L.block_n) >= 2 * ctx->sm_count;
     if (ctx->flags & NSGPU_MLP_NO_CLUSTER) pair = false;
     if (ctx->flags & NSGPU_MLP_CLUSTER) pair = true;
+    // kernel A/B runs (NSGPU_CS4): hidden layers in clusters of 4 (each CTA loads a quarter of the weight tile: the 64-row maps)
+    static const bool cs4 = getenv("NSGPU_CS4") != nullptr;
+    if (pair && cs4 && EPI == 0 && L.block_n == 256 && L.has_s[1])
+      return launch_gemm_cluster<256, EPI, 4, BK>(ctx, L.tm_whi_s[1], L.tm_wlo_s[1], g, st);
     if (pair) return L.block_n == 256 ? launch_gemm_cluster<256, EPI, 2, BK>(ctx, L.tm_whi_c, L.tm_wlo_c, g, st)
                                       : launch_gemm_cluster<224, EPI, 2, BK>(ctx, L.tm_whi_c, L.tm_wlo_c, g, st);
   }
