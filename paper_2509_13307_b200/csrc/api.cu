@@ -385,6 +385,10 @@ nsgpu_status create_impl(nsgpu_ctx* ctx, int32_t D, const nsgpu_prior1d* prior, 
     NSGPU_CUDA(cudaEventCreateWithFlags(&ctx->ev_in, cudaEventDisableTiming));
     NSGPU_CUDA(cudaEventCreateWithFlags(&ctx->ev_side, cudaEventDisableTiming));
   }
+  for (int e = 1; e < n_emu && e < 8; ++e) {
+    NSGPU_CUDA(cudaStreamCreateWithFlags(&ctx->emu_stream[e], cudaStreamNonBlocking));
+    NSGPU_CUDA(cudaEventCreateWithFlags(&ctx->emu_done[e], cudaEventDisableTiming));
+  }
   // MLP path selection
   for (int e = 0; e < n_emu; ++e) {
     EmuDev& E = ctx->emu[e];
@@ -438,6 +442,7 @@ extern "C" nsgpu_status nsgpu_destroy(nsgpu_ctx* ctx) {
   cudaDeviceSynchronize();
   sampler_destroy(ctx);
   if (ctx->side_stream) cudaStreamDestroy(ctx->side_stream);
+  for (int e = 0; e < 8; ++e) { if (ctx->emu_stream[e]) cudaStreamDestroy(ctx->emu_stream[e]); if (ctx->emu_done[e]) cudaEventDestroy(ctx->emu_done[e]); }
   if (ctx->ev_in) cudaEventDestroy(ctx->ev_in);
   if (ctx->ev_side) cudaEventDestroy(ctx->ev_side);
   for (auto& ev : ctx->stage_events) { cudaEventDestroy(ev.a); cudaEventDestroy(ev.b); }
@@ -514,6 +519,24 @@ extern "C" int64_t nsgpu_nonfinite_rows(nsgpu_ctx* ctx) {
 
 static nsgpu_status run_emulators(nsgpu_ctx* ctx, const float* theta, int B, const int* n_rows_dev, cudaStream_t st) {
   const size_t stride = (size_t)ctx->max_batch * ctx->rows_per_theta * ctx->spec_ld;
+  // Several emulators (c1: TT, TE, EE at one row per theta: hidden GEMMs of 64 tiles on 148 SMs) run concurrently: fork after
+  // theta is ready, emulator e on its own stream and activation buffers, join before the consumer.
+  bool conc = ctx->n_emu > 1 && ctx->emu_stream[1] != nullptr && (ctx->flags & (NSGPU_NO_OVERLAP | NSGPU_MLP_FUSED)) == 0;
+  for (int e = 0; e < ctx->n_emu && conc; ++e) conc = ctx->emu[e].path == 1;
+  if (conc) {
+    if (!ctx->ev_in) NSGPU_CUDA(cudaEventCreateWithFlags(&ctx->ev_in, cudaEventDisableTiming));
+    NSGPU_CUDA(cudaEventRecord(ctx->ev_in, st));
+    const int mode = ctx->kind == 4 ? NSGPU_SPEC_NOMEAN : 0;
+    for (int e = 0; e < ctx->n_emu; ++e) {
+      cudaStream_t se = e == 0 ? st : ctx->emu_stream[e];
+      if (e > 0) NSGPU_CUDA(cudaStreamWaitEvent(se, ctx->ev_in, 0));
+      nsgpu_status s = mlp_forward_tc(ctx, e, theta, B, n_rows_dev, ctx->spec + e * stride, ctx->spec_ld, mode, se);
+      if (s != NSGPU_OK) return s;
+      if (e > 0) NSGPU_CUDA(cudaEventRecord(ctx->emu_done[e], se));
+    }
+    for (int e = 1; e < ctx->n_emu; ++e) NSGPU_CUDA(cudaStreamWaitEvent(st, ctx->emu_done[e], 0));
+    return NSGPU_OK;
+  }
   for (int e = 0; e < ctx->n_emu; ++e) {
     float* out = ctx->spec + e * stride;
     // kinds 3 and 4: the fp32 table carries only the O(sigma_out) deviation y - mu_out; the consumer adds mu_out in fp64

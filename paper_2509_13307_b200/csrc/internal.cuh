@@ -98,6 +98,8 @@ struct nsgpu_ctx {
   void* probe = nullptr;               // clock probe state (probe.cu)
   cudaStream_t side_stream = nullptr;  // shear: the theta-only half of the projection runs here, under the emulator kernels
   cudaEvent_t ev_in = nullptr, ev_side = nullptr;
+  cudaStream_t emu_stream[8] = {};     // kind 2: emulators 1.. run on streams of their own, concurrently with emulator 0
+  cudaEvent_t emu_done[8] = {};
   std::string err;
   int64_t launches = 0;
   unsigned long long* nonfinite_rows = nullptr;   // device counter: emulator rows with non-finite output (tcgen05 path)

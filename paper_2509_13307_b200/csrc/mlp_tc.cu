@@ -944,6 +944,7 @@ struct TcLayer {
 struct TcState {
   std::vector<TcLayer> layers;               // index = layer 0 .. n_hidden (layer 0 uses p_hidden only)
   __half* act[2][2] = {};                    // [buffer][hi, lo] canonical-layout planes
+  void* own_act[2] = {nullptr, nullptr};     // emulators 1.. own their activation buffers (emulator 0 uses ctx->act)
   size_t M_pad = 0;
   bool fused_ok = false;                     // shapes the fused multi-layer kernel takes (mlp_fused_tc)
   FusedMaps fmaps;
@@ -1181,10 +1182,17 @@ nsgpu_status mlp_tc_prepare(nsgpu_ctx* ctx, int e, const nsgpu_emulator* h) {
     }
   }
   for (int i = 0; i < 2; ++i) {
-    T->act[i][0] = reinterpret_cast<__half*>(ctx->act[i]);
+    // emulator 0 ping-pongs through the context's buffers; further emulators (kind 2: TT, TE, EE) get buffers of their own so
+    // that the emulators of one likelihood call can run concurrently on separate streams (api.cu run_emulators)
+    void* base = ctx->act[i];
+    if (e > 0) {
+      NSGPU_CUDA(cudaMalloc(&T->own_act[i], M_pad * width * 2 * sizeof(__half)));
+      base = T->own_act[i];
+    }
+    T->act[i][0] = reinterpret_cast<__half*>(base);
     T->act[i][1] = T->act[i][0] + M_pad * width;
     // rows past the live ones are read by the last tile of a batch (results discarded): keep them finite
-    NSGPU_CUDA(cudaMemset(ctx->act[i], 0, M_pad * width * 2 * sizeof(__half)));
+    NSGPU_CUDA(cudaMemset(base, 0, M_pad * width * 2 * sizeof(__half)));
   }
   return NSGPU_OK;
 }
@@ -1192,6 +1200,7 @@ nsgpu_status mlp_tc_prepare(nsgpu_ctx* ctx, int e, const nsgpu_emulator* h) {
 void mlp_tc_release(nsgpu_ctx* ctx, int e) {
   TcState* T = reinterpret_cast<TcState*>(ctx->emu[e].tmaps);
   if (!T) return;
+  cudaFree(T->own_act[0]); cudaFree(T->own_act[1]);
   for (TcLayer& L : T->layers) { cudaFree(L.Whi); cudaFree(L.Wlo); cudaFree(L.p_hidden); cudaFree(L.p_out); cudaFree(L.p_out4); cudaFree(L.p_out_nm); cudaFree(L.p_out4_nm); }
   delete T;
   ctx->emu[e].tmaps = nullptr;

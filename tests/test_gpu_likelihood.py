@@ -326,11 +326,12 @@ def test_fused_mlp_is_bit_identical_to_the_layered_path(name, B):
     assert res[1][3] < res[0][3]                                          # one launch instead of one per layer
 
 
-@pytest.mark.parametrize("name,B", [("c3a", 300), ("c3b", 77), ("tiny_shear_paper", 21), ("c5i", 40)])
+@pytest.mark.parametrize("name,B", [("c3a", 300), ("c3b", 77), ("tiny_shear_paper", 21), ("c5i", 40), ("c1", 300), ("c1", 2100)])
 def test_side_stream_projection_half_changes_nothing(name, B):
-    """the theta-only half of the shear projection runs on a side stream under the emulator kernels:
-    same bits as with everything on one stream, call after call (the hand-off buffer is reused), on the caller's
-    stream and through the host entry"""
+    """the theta-only half of the shear projection runs on a side stream under the emulator kernels, and the three emulators of
+    the CMB likelihood (c1) run concurrently on streams and activation buffers of their own: same bits as with
+    everything on one stream, call after call (the hand-off buffers are reused), on the caller's stream and through the
+    host entry"""
     wl = workload(name)
     theta = theta_of_u(wl, np.concatenate([W.u_post_set(wl, B // 2), W.u_prior_set(wl, B - B // 2)]))
     with nsgpu.Context(wl, max_batch=B, mlp=nsgpu.NO_OVERLAP) as ctx:
