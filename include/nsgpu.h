@@ -193,6 +193,9 @@ typedef struct {
   int64_t n_iter, n_dead, n_like_evals, n_rounds, n_failed_moves;
   double seconds; /* wall time of the run, host clock */
   double seconds_sampling, seconds_summary; /* ... split: the nested-sampling loop | final log Z, H, error bar, samples */
+  int64_t n_nonfinite_rows; /* emulator rows whose output was not finite during this run (tcgen05 path: |h| >= 4094 overflows the
+                             * fp16 activation planes).  Such proposals count as log L = -inf, i.e. as
+                             * excluded prior volume: a non-zero value means log Z may be biased -- rerun with NSGPU_MLP_SIMT. */
 } nsgpu_result;
 
 /* a1-a14: the whole nested-sampling run.  Samples go to caller-allocated HOST buffers of

@@ -908,6 +908,15 @@ static nsgpu_status summarize_run(nsgpu_ctx* ctx, int n, int k, uint2 key, doubl
   return s;
 }
 
+// non-finite emulator rows so far on this context (device counter, see nsgpu_nonfinite_rows); -1 on error
+static long long read_nonfinite(nsgpu_ctx* ctx, cudaStream_t st) {
+  unsigned long long v = 0;
+  if (!ctx->nonfinite_rows || cudaStreamSynchronize(st) != cudaSuccess ||
+      cudaMemcpy(&v, ctx->nonfinite_rows, sizeof(v), cudaMemcpyDeviceToHost) != cudaSuccess)
+    return -1;
+  return (long long)v;
+}
+
 static nsgpu_status run_impl(nsgpu_ctx* ctx, const nsgpu_run_opts* o, int rank, int world, nsgpu_allgather_fn exch,
                              void* user, nsgpu_result* res, float* theta_samples, double* logL_samples,
                              double* logw_samples, int64_t cap, int64_t* n_samples) {
@@ -919,10 +928,12 @@ static nsgpu_status run_impl(nsgpu_ctx* ctx, const nsgpu_run_opts* o, int rank, 
   if (o->n_delete >= o->n_live || o->n_steps < 1 || !(o->stop_frac > 0) || o->max_iter < 1) { ctx->err = "run: bad options"; return NSGPU_EINVAL; }
   if (o->n_live < ctx->D + 1) { ctx->err = "run: the live covariance needs n_live >= D + 1"; return NSGPU_EINVAL; }
   const auto t_start = std::chrono::steady_clock::now();
+  long long nf0 = -2;   // read once the stream is known
   SamplerDev* S = ctx->sampler;
   // one rank: the context's own stream, so that runs of several contexts (the two models of a comparison, driven from
   // two host threads) share the GPU; sharded runs stay on the legacy default stream the exchange callback is ordered with
   cudaStream_t st = world == 1 ? S->run_stream : (cudaStream_t)0;
+  nf0 = read_nonfinite(ctx, st);
   const int D = ctx->D, n = o->n_live, k = o->n_delete;
   const uint2 key = make_uint2((unsigned)(o->seed & 0xffffffffu), (unsigned)(o->seed >> 32));
   std::vector<float> dead_u;
@@ -1059,6 +1070,7 @@ static nsgpu_status run_impl(nsgpu_ctx* ctx, const nsgpu_run_opts* o, int rank, 
   res->seconds = std::chrono::duration<double>(t_end - t_start).count();
   res->seconds_sampling = std::chrono::duration<double>(t_sampled - t_start).count();
   res->seconds_summary = std::chrono::duration<double>(t_end - t_sampled).count();
+  { const long long nf1 = read_nonfinite(ctx, st); res->n_nonfinite_rows = (nf0 >= 0 && nf1 >= 0) ? nf1 - nf0 : -1; }
   return converged ? NSGPU_OK : NSGPU_ENOCONV;
 }
 
@@ -1108,9 +1120,11 @@ extern "C" nsgpu_status nsgpu_run_multi(nsgpu_ctx* ctx, const nsgpu_run_opts* o,
   if (o->n_live < ctx->D + 1) { ctx->err = "run_multi: the live covariance needs n_live >= D + 1"; return NSGPU_EINVAL; }
   if ((int64_t)n_runs * o->n_delete > ctx->max_batch) { ctx->err = "run_multi: n_runs x n_delete exceeds max_batch"; return NSGPU_ESHAPE; }
   const auto t_start = std::chrono::steady_clock::now();
+  long long nf0 = -2;
   SamplerDev* S = ctx->sampler;
   cudaStream_t st = S->run_stream;
   const int D = ctx->D, n = o->n_live, k = o->n_delete, R = n_runs;
+  nf0 = read_nonfinite(ctx, st);
   MultiBuf B;
 #define MB(p, T, cnt) NSGPU_CUDA(cudaMalloc((void**)&B.p, sizeof(T) * (size_t)(cnt)))
   MB(u_live, float, (size_t)R * n * D); MB(logL_live, double, (size_t)R * n); MB(scal, double, R * 8); MB(Lsig, double, (size_t)R * D * D);
@@ -1220,6 +1234,10 @@ extern "C" nsgpu_status nsgpu_run_multi(nsgpu_ctx* ctx, const nsgpu_run_opts* o,
     res[r].seconds = std::chrono::duration<double>(t_end - t_start).count();
     res[r].seconds_sampling = std::chrono::duration<double>(t_sampled - t_start).count();
     res[r].seconds_summary = std::chrono::duration<double>(t_end - t_sampled).count();
+  }
+  {   // the runs share every batch: the count is that of the whole call, reported with each run
+    const long long nf1 = read_nonfinite(ctx, st);
+    for (int r = 0; r < R; ++r) res[r].n_nonfinite_rows = (nf0 >= 0 && nf1 >= 0) ? nf1 - nf0 : -1;
   }
   return all_conv ? NSGPU_OK : NSGPU_ENOCONV;
 }

@@ -77,7 +77,7 @@ class _Result(C.Structure):
     _fields_ = [("logZ", C.c_double), ("logZ_err", C.c_double), ("logZ_err_analytic", C.c_double), ("H", C.c_double),
                 ("n_iter", C.c_int64), ("n_dead", C.c_int64), ("n_like_evals", C.c_int64), ("n_rounds", C.c_int64),
                 ("n_failed_moves", C.c_int64), ("seconds", C.c_double), ("seconds_sampling", C.c_double),
-                ("seconds_summary", C.c_double)]
+                ("seconds_summary", C.c_double), ("n_nonfinite_rows", C.c_int64)]
 
 
 # int32 allgather(void* user, const void* send, void* recv, int64 bytes_per_rank, void* stream)  (include/nsgpu.h)

@@ -172,6 +172,9 @@ def test_activation_overflow_is_counted_not_silent():
         ll = ctx.loglike_batch(dev(theta)).cpu().numpy()
         n_bad = ctx.nonfinite_rows()
     assert n_bad > 0 and np.sum(ll == -np.inf) == n_bad and not np.any(np.isnan(ll))
+    with nsgpu.Context(wl, max_batch=64, mlp=nsgpu.MLP_TC) as ctx:               # ... and a nested-sampling run reports it
+        r = ctx.run(64, 32, 3, max_iter=2, return_samples=False)
+    assert r["n_nonfinite_rows"] > 0
     with nsgpu.Context(wl, max_batch=40, mlp=nsgpu.MLP_SIMT) as ctx:
         ll32 = ctx.loglike_batch(dev(theta)).cpu().numpy()
     chi2 = -2.0 * (ref - gaussian.log_norm(wl.chol))

@@ -296,6 +296,7 @@ def test_run_toy_emulator_agrees_with_oracle_ns():
     wl = workload("toy")
     with nsgpu.Context(wl, max_batch=200) as ctx:
         g = [ctx.run(200, 100, 30, seed=s, return_samples=False) for s in (1, 2, 3)]
+    assert all(r["n_nonfinite_rows"] == 0 for r in g)
     o = nested.run(lambda u: LK.loglike_u(wl, u), wl.D, 200, 100, 30, seed=11)
     zg = np.mean([r["logZ"] for r in g]); eg = np.mean([r["logZ_err"] for r in g]) / math.sqrt(3)
     assert all(r["converged"] for r in g) and o["converged"]
