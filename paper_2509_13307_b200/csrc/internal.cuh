@@ -4,6 +4,7 @@
 
 #include <cuda_runtime.h>
 #include <cuda_fp16.h>
+#include <nvtx3/nvToolsExt.h>
 #include <stdint.h>
 
 #include <algorithm>
@@ -112,11 +113,15 @@ struct nsgpu_ctx {
   int64_t stage_count[NSGPU_N_STAGES] = {};
 };
 
-// RAII stage timer: records an event pair on `st` around the enclosed launches when profiling is on
+// RAII stage timer: records an event pair on `st` around the enclosed launches when profiling is on, inside an NVTX range
+// named after the stage (header-only NVTX3: a no-op unless a tool that collects NVTX is attached, e.g. `ncu --nvtx`)
+static const char* const NSGPU_STAGE_NAMES[NSGPU_N_STAGES] = {"nsgpu:mlp_first", "nsgpu:mlp_hidden", "nsgpu:mlp_out", "nsgpu:shear_project",
+                                                              "nsgpu:cmb_bin", "nsgpu:chi2", "nsgpu:slice_round", "nsgpu:copy_model"};
 struct StageTimer {
   nsgpu_ctx* ctx; cudaStream_t st; int idx = -1;
   StageTimer(nsgpu_ctx* c, int stage, cudaStream_t s) : ctx(c), st(s) {
     if (!c->profiling || stage < 0) return;
+    nvtxRangePushA(NSGPU_STAGE_NAMES[stage]);
     nsgpu_ctx::StageEv ev; ev.stage = stage;
     for (cudaEvent_t* e : {&ev.a, &ev.b}) {
       if (!c->event_pool.empty()) { *e = c->event_pool.back(); c->event_pool.pop_back(); }
@@ -126,7 +131,7 @@ struct StageTimer {
     c->stage_events.push_back(ev);
     idx = (int)c->stage_events.size() - 1;
   }
-  ~StageTimer() { if (idx >= 0) cudaEventRecord(ctx->stage_events[idx].b, st); }
+  ~StageTimer() { if (idx >= 0) { cudaEventRecord(ctx->stage_events[idx].b, st); nvtxRangePop(); } }
 };
 
 #define NSGPU_CUDA(call)                                                                  \
