@@ -136,13 +136,24 @@ struct RoundArgs {
 // next proposal that needs a likelihood.  Phase transitions are taken from the state as it was when the
 // result was requested: a chain consumes exactly one likelihood result per round.
 __global__ void __launch_bounds__(128) slice_round_kernel(RoundArgs a) {
+  extern __shared__ double sL[];   // [D][D] direction factor of the run this block's first chain belongs to
   pdl_wait();      // logL_prop comes from the likelihood kernels of the previous round (launch_pdl contract)
   pdl_trigger();
+  const int D = a.D;
+  // A kernel of 500 warps on 148 SMs is pure latency: the D-step product L_Sigma z read its factor from global memory with
+  // a dependent load per step (~39 L2 round trips in series for every new slice; ncu: 24 us per round).  Stage the factor
+  // once per block (coalesced, one round trip); the accumulation order below is unchanged.
+  const int c_first = min((int)((blockIdx.x * blockDim.x) >> 5), a.n_chains - 1);
+  const int run_blk = a.n_per_run ? c_first / a.n_per_run : 0;
+  {
+    const double* src = a.Lsig + (size_t)run_blk * D * D;
+    for (int i = threadIdx.x; i < D * D; i += blockDim.x) sL[i] = src[i];
+  }
+  __syncthreads();
   const int c = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   const int lane = threadIdx.x & 31;
   if (c >= a.n_chains) return;
   if (a.finished[c]) { if (lane == 0) a.need[c] = 0; return; }
-  const int D = a.D;
   const int d0 = lane, d1 = lane + 32;
   const bool v0 = d0 < D, v1 = d1 < D;
   const size_t base = (size_t)c * D;
@@ -155,7 +166,7 @@ __global__ void __launch_bounds__(128) slice_round_kernel(RoundArgs a) {
   const int run = a.n_per_run ? c / a.n_per_run : 0;
   const int lc = c - run * a.n_per_run;                          // chain index within its run (= c for one run)
   const double Lstar = a.scal[8 * run];
-  const double* Lsig = a.Lsig + (size_t)run * D * D;
+  const double* Lsig = run == run_blk ? sL : a.Lsig + (size_t)run * D * D;   // a block that straddles two runs: the other run reads global
   Stream S{a.n_per_run ? a.keys[run] : a.key, (unsigned)(a.chain0 + lc), a.n_per_run ? a.iters[run] : a.iteration, 0u};
   bool inside = false;
   double val = 0.0;
@@ -256,12 +267,15 @@ __device__ int block_excl_scan_int(int v, int* wsum, int* total) {
   return out;
 }
 
-// compaction of the proposals that need a likelihood into a dense batch (deterministic: chain order)
+// compaction of the proposals that need a likelihood into a dense batch (deterministic: chain order).  Every CTA repeats
+// the (cheap) scan of the flags into shared memory; CTA 0 publishes the rows and the count; the rows are then copied by all
+// CTAs, one warp per chain (a single CTA walking all n_chains D floats through dependent loads took 12.7 us per round).
 __global__ void __launch_bounds__(1024) compact_kernel(int n_chains, int D, const int* __restrict__ need,
                                                         int* __restrict__ row_of_chain,
                                                         const float* __restrict__ theta_chain,
                                                         float* __restrict__ theta_prop, int* counters,
                                                         unsigned long long* n_evals) {
+  extern __shared__ int srow[];   // [n_chains]
   __shared__ int wsum[32];
   __shared__ int total;
   int carry = 0;
@@ -271,14 +285,20 @@ __global__ void __launch_bounds__(1024) compact_kernel(int n_chains, int D, cons
     const int c = base + threadIdx.x;
     const int f = (c < n_chains) ? need[c] : 0;
     const int ex = block_excl_scan_int(f, wsum, &total);
-    if (c < n_chains) row_of_chain[c] = f ? carry + ex : -1;
+    if (c < n_chains) srow[c] = f ? carry + ex : -1;
     carry += total;
     __syncthreads();
   }
-  if (threadIdx.x == 0) { counters[0] = carry; *n_evals += (unsigned long long)carry; }
-  for (int i = threadIdx.x; i < n_chains * D; i += blockDim.x) {
-    const int c = i / D, row = row_of_chain[c];
-    if (row >= 0) theta_prop[(size_t)row * D + (i - c * D)] = theta_chain[i];
+  if (blockIdx.x == 0) {
+    for (int c = threadIdx.x; c < n_chains; c += blockDim.x) row_of_chain[c] = srow[c];
+    if (threadIdx.x == 0) { counters[0] = carry; *n_evals += (unsigned long long)carry; }
+  }
+  const int lane = threadIdx.x & 31;
+  const int gw = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), nw = gridDim.x * (blockDim.x >> 5);
+  for (int c = gw; c < n_chains; c += nw) {
+    const int row = srow[c];
+    if (row < 0) continue;
+    for (int d = lane; d < D; d += 32) theta_prop[(size_t)row * D + d] = theta_chain[(size_t)c * D + d];
   }
 }
 
@@ -673,6 +693,9 @@ static nsgpu_status evolve(nsgpu_ctx* ctx, int n_chains, int chain0, int n_steps
   const int n_target = multi ? multi->n_target : n_chains;
   NSGPU_CUDA(cudaMemsetAsync(S->counters, 0, 4 * sizeof(int), st));
   const int blocks = (n_chains * 32 + 127) / 128;
+  const int compact_ctas = std::min(std::max((n_chains + 127) / 128, 1), 16);   // 32 warps each, one warp per chain row
+  if (n_chains > 51200) { ctx->err = "sampler: more than 51200 chains in one round (the compaction keeps its row table in shared memory)"; return NSGPU_ESHAPE; }
+  if (sizeof(int) * (size_t)n_chains > 48 * 1024) NSGPU_CUDA(nsgpu_ensure_smem(ctx, compact_kernel, sizeof(int) * (size_t)n_chains));
   int64_t rounds = 0;
   // Rounds are launched in bursts and the finished-counter is read after each burst (one small D2H).  A round
   // after the last chain has finished is a dozen empty launches, a check is a pipeline drain: the first burst
@@ -683,10 +706,10 @@ static nsgpu_status evolve(nsgpu_ctx* ctx, int n_chains, int chain0, int n_steps
     for (int i = 0; i < burst; ++i) {
       {
       StageTimer tm(ctx, 6, st);
-      NSGPU_CUDA(launch_pdl(ctx, slice_round_kernel, dim3(blocks), dim3(128), 0, st, a));
+      NSGPU_CUDA(launch_pdl(ctx, slice_round_kernel, dim3(blocks), dim3(128), sizeof(double) * ctx->D * ctx->D, st, a));
       NSGPU_LAUNCH_CHECK();
-      NSGPU_CUDA(launch_pdl(ctx, compact_kernel, dim3(1), dim3(1024), 0, st, n_chains, ctx->D, S->need, S->row_of_chain, S->theta_chain,
-                            S->theta_prop, S->counters, S->n_evals));
+      NSGPU_CUDA(launch_pdl(ctx, compact_kernel, dim3(compact_ctas), dim3(1024), sizeof(int) * n_chains, st, n_chains, ctx->D, S->need,
+                            S->row_of_chain, S->theta_chain, S->theta_prop, S->counters, S->n_evals));
       NSGPU_LAUNCH_CHECK();
       }
       nsgpu_status s = loglike_device(ctx, S->theta_prop, n_chains, S->counters, S->logL_prop, st);

@@ -12,7 +12,7 @@ from typing import Optional
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "lib", "libnsgpu.so")
+LIB_PATH = os.environ.get("NSGPU_LIB") or os.path.join(_HERE, "lib", "libnsgpu.so")   # NSGPU_LIB: another build of the library (kernel A/B runs)
 
 OK, EINVAL, ENOMEM, ECUDA, ESHAPE, ENOTSPD, ENOCONV = 0, -1, -2, -3, -4, -5, -6
 STATUS_NAMES = {0: "NSGPU_OK", -1: "NSGPU_EINVAL", -2: "NSGPU_ENOMEM", -3: "NSGPU_ECUDA",
