@@ -146,8 +146,17 @@ __global__ void __launch_bounds__(128) slice_round_kernel(RoundArgs a) {
   const int c_first = min((int)((blockIdx.x * blockDim.x) >> 5), a.n_chains - 1);
   const int run_blk = a.n_per_run ? c_first / a.n_per_run : 0;
   {
+    // sixteen loads in flight per thread before the first store: one L2 round trip for D <= 45, two for D = 64 (a plain
+    // load-store loop was twelve round trips in series: the ncu source page had 69% of this kernel's samples on it)
     const double* src = a.Lsig + (size_t)run_blk * D * D;
-    for (int i = threadIdx.x; i < D * D; i += blockDim.x) sL[i] = src[i];
+    const int n = D * D;
+    for (int i0 = threadIdx.x; i0 < n; i0 += 16 * blockDim.x) {
+      double v[16];
+#pragma unroll
+      for (int u = 0; u < 16; ++u) { const int i = i0 + u * blockDim.x; v[u] = i < n ? src[i] : 0.0; }
+#pragma unroll
+      for (int u = 0; u < 16; ++u) { const int i = i0 + u * blockDim.x; if (i < n) sL[i] = v[u]; }
+    }
   }
   __syncthreads();
   const int c = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
@@ -693,7 +702,7 @@ static nsgpu_status evolve(nsgpu_ctx* ctx, int n_chains, int chain0, int n_steps
   const int n_target = multi ? multi->n_target : n_chains;
   NSGPU_CUDA(cudaMemsetAsync(S->counters, 0, 4 * sizeof(int), st));
   const int blocks = (n_chains * 32 + 127) / 128;
-  const int compact_ctas = std::min(std::max((n_chains + 127) / 128, 1), 16);   // 32 warps each, one warp per chain row
+  const int compact_ctas = std::min(std::max((n_chains + 31) / 32, 1), 16);   // 32 warps each: one chain row per warp up to 512 chains
   if (n_chains > 51200) { ctx->err = "sampler: more than 51200 chains in one round (the compaction keeps its row table in shared memory)"; return NSGPU_ESHAPE; }
   if (sizeof(int) * (size_t)n_chains > 48 * 1024) NSGPU_CUDA(nsgpu_ensure_smem(ctx, compact_kernel, sizeof(int) * (size_t)n_chains));
   int64_t rounds = 0;
